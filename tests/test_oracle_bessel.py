@@ -1,0 +1,113 @@
+"""Pins of the oracle's modified Bessel function K_nu(x) (oracle/ipa_oracle.cpp, reading C4).
+
+None of these re-use the oracle's formulae: they compare against mpmath at 40 digits, scipy,
+closed forms for half-integer order (A&S 10.2.17), the three-term recurrence (A&S 9.6.26),
+the golden spot values and the confluent-hypergeometric identities the
+large-x branch rests on (DLMF 13.6.10, Temme 1975) evaluated with mpmath.hyperu.
+"""
+import math
+import os
+
+import mpmath as mp
+import numpy as np
+import pytest
+from hypothesis import given, settings, strategies as st
+
+mp.mp.dps = 40
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _rel(got, ref):
+    return float(abs((mp.mpf(got) - ref) / ref))
+
+
+def test_spot_values_golden(orc):
+    for line in open(os.path.join(GOLD, "bessel_spot_values.txt")):
+        if line.startswith("#") or not line.strip():
+            continue
+        nu, x, val = line.split()
+        got = orc.besselk_scaled(float(nu), float(x)) * math.exp(-float(x))
+        assert abs(got - float(val)) <= 4e-16 * abs(float(val)), (nu, x, got, val)
+
+
+def test_grid_vs_mpmath(orc):
+    worst = 0.0
+    for nu in np.concatenate([np.linspace(-5, 5, 41), [0.5, 1.5, -0.5, 1e-12, 0.49999999, 0.50000001]]):
+        for x in [1e-3, 3e-3, 0.02, 0.11, 0.7, 1.0, 1.7, 1.9999999, 2.0, 2.0000001, 2.7, 4.4, 9.0, 33.0, 120.0, 699.0]:
+            ref = mp.besselk(mp.mpf(float(nu)), mp.mpf(x)) * mp.exp(mp.mpf(x))
+            worst = max(worst, _rel(orc.besselk_scaled(float(nu), x), ref))
+    assert worst <= 5e-15, worst   # SURVEY.md C8.1 bar
+    assert worst <= 4e-16, worst   # what the long-double implementation actually reaches
+
+
+@settings(max_examples=150, deadline=None)
+@given(nu=st.floats(-5, 5), lx=st.floats(math.log(1e-3), math.log(700.0)))
+def test_hypothesis_vs_mpmath(orc, nu, lx):
+    x = math.exp(lx)
+    ref = mp.besselk(mp.mpf(nu), mp.mpf(x)) * mp.exp(mp.mpf(x))
+    assert _rel(orc.besselk_scaled(nu, x), ref) <= 5e-15
+
+
+def test_log_besselk_vs_mpmath(orc):
+    for nu, x in [(0.5, 1.0), (-1.8, 2.0), (-1.8, 7.3), (0.0, 0.3), (2.2, 150.0)]:
+        ref = mp.log(mp.besselk(nu, x))
+        assert abs(mp.mpf(orc.log_besselk(nu, x)) - ref) <= 4e-16 * max(1, abs(ref))
+
+
+def test_half_integer_closed_forms(orc):
+    for x in [0.05, 0.5, 1.0, 2.0, 2.5, 10.0, 300.0]:
+        k12 = math.sqrt(math.pi / (2 * x))  # scaled by e^x
+        assert abs(orc.besselk_scaled(0.5, x) - k12) <= 4e-16 * k12
+        assert abs(orc.besselk_scaled(1.5, x) - k12 * (1 + 1 / x)) <= 4e-16 * k12 * (1 + 1 / x)
+        k52 = k12 * (1 + 3 / x + 3 / x ** 2)
+        assert abs(orc.besselk_scaled(2.5, x) - k52) <= 4e-16 * k52
+
+
+def test_recurrence_and_symmetry(orc):
+    rng = np.random.default_rng(11)
+    for _ in range(200):
+        nu = rng.uniform(-4, 4)
+        x = math.exp(rng.uniform(math.log(0.01), math.log(300)))
+        km, k0, kp = (orc.besselk_scaled(nu + s, x) for s in (-1, 0, 1))
+        resid = kp - km - (2 * nu / x) * k0
+        assert abs(resid) <= 1e-14 * (abs(kp) + abs(km) + abs(2 * nu / x * k0))
+        assert orc.besselk_scaled(-nu, x) == orc.besselk_scaled(nu, x)
+
+
+def test_scipy_secondary(orc):
+    sp = pytest.importorskip("scipy.special")
+    rng = np.random.default_rng(5)
+    for _ in range(300):
+        nu = rng.uniform(-5, 5)
+        x = math.exp(rng.uniform(math.log(1e-3), math.log(500)))
+        ref = sp.kve(nu, x)
+        assert abs(orc.besselk_scaled(nu, x) - ref) <= 1e-13 * ref
+
+
+def test_miller_identities_hold_in_mpmath():
+    """The large-x branch rests on three identities; check them with mpmath so that a wrong
+    recurrence coefficient or normalisation weight in the oracle cannot hide behind them."""
+    for mu, x in [(0.3, 2.5), (-0.45, 7.0), (0.0, 3.0)]:
+        mu, x = mp.mpf(mu), mp.mpf(x)
+        z = lambda n: mp.hyperu(mu + mp.mpf(1) / 2 + n, 2 * mu + 1, 2 * x)
+        # K_mu(x) = sqrt(pi) (2x)^mu e^-x U(mu+1/2, 2mu+1, 2x)
+        assert abs(mp.sqrt(mp.pi) * (2 * x) ** mu * mp.exp(-x) * z(0) / mp.besselk(mu, x) - 1) < mp.mpf(10) ** -30
+        # z_{n-1} = 2(n+x) z_n - ((n+1/2)^2-mu^2) z_{n+1}
+        for n in (1, 2, 5):
+            lhs = z(n - 1)
+            rhs = 2 * (n + x) * z(n) - ((n + mp.mpf(1) / 2) ** 2 - mu ** 2) * z(n + 1)
+            assert abs(lhs / rhs - 1) < mp.mpf(10) ** -28
+        # sum C_n z_n = (2x)^(-mu-1/2), C_n = C_{n-1} ((n-1/2)^2-mu^2)/n
+        C, S = mp.mpf(1), z(0)
+        for n in range(1, 400):
+            C *= ((n - mp.mpf(1) / 2) ** 2 - mu ** 2) / n
+            S += C * z(n)
+        assert abs(S / (2 * x) ** (-mu - mp.mpf(1) / 2) - 1) < mp.mpf(10) ** -9  # slowly convergent tail
+        # K_{mu+1}/K_mu = [1/2 + mu + x - (1/4-mu^2) z_1/z_0]/x
+        ratio = (mp.mpf(1) / 2 + mu + x - (mp.mpf(1) / 4 - mu ** 2) * z(1) / z(0)) / x
+        assert abs(ratio / (mp.besselk(mu + 1, x) / mp.besselk(mu, x)) - 1) < mp.mpf(10) ** -30
+
+
+def test_zeta_values(orc):
+    for k in (2, 3, 4, 7, 20, 60):
+        assert abs(mp.mpf(orc.zeta_int(k)) - mp.zeta(k)) <= 3e-16

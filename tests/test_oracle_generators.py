@@ -1,0 +1,179 @@
+"""Pins of the oracle's generators and binned path (rows T0, T1, B1-B3; readings D13-D16).
+
+Philox is pinned against the CUDA toolkit's own header implementation compiled for the host
+(library routine, different code); the samplers are pinned by exact distributional facts.
+"""
+import math
+import os
+import shutil
+import subprocess
+
+import numpy as np
+import pytest
+
+import ipa_inputs as inp
+
+LO, HI = inp.LO, inp.HI
+P1, P2 = inp.GEN, inp.P2
+HERE = os.path.dirname(os.path.abspath(__file__))
+
+
+def test_philox_vs_cuda_toolkit_header(orc, tmp_path):
+    nvcc = shutil.which("nvcc") or "/usr/local/cuda/bin/nvcc"
+    if not os.path.exists(nvcc):
+        pytest.skip("no nvcc")
+    exe = str(tmp_path / "philox_host")
+    subprocess.check_call([nvcc, "-Wno-deprecated-gpu-targets", "-o", exe, os.path.join(HERE, "philox_curand_host.cu")])
+    rng = np.random.default_rng(77)
+    cases = rng.integers(0, 2 ** 32, size=(256, 6), dtype=np.uint64)
+    cases[0] = 0
+    cases[1] = 2 ** 32 - 1
+    cases[2] = [1, 0, 0, 0, 0, 0]
+    cases[3] = [0, 0, 1, 0, 0, 0]
+    out = subprocess.run([exe], input="\n".join(" ".join(str(int(v)) for v in c) for c in cases), text=True,
+                         capture_output=True, check=True).stdout.split("\n")
+    for c, line in zip(cases, out):
+        ref = np.array([int(v) for v in line.split()], dtype=np.uint32)
+        got = orc.philox4x32_10(c[:2], c[2:])
+        assert (got == ref).all(), (c, got, ref)
+
+
+def test_uniform_mapping(orc):
+    """u = ((w0>>5) 2^26 + (w1>>6) + 0.5) 2^-53 in (0,1) (reading D13), checked from the raw words."""
+    for seed, slot, att, stream in [(1, 0, 0, 0), (2 ** 40 + 5, 2 ** 33 + 1, 7, 2), (99, 12345, 3, 1)]:
+        w = orc.philox4x32_10([seed & 0xFFFFFFFF, seed >> 32], [slot & 0xFFFFFFFF, slot >> 32, att, stream]).astype(np.uint64)
+        u = orc.uniforms2(seed, slot, att, stream)
+        for j in (0, 1):
+            ref = ((int(w[2 * j]) >> 5) * 2 ** 26 + (int(w[2 * j + 1]) >> 6) + 0.5) / 2 ** 53
+            assert u[j] == ref and 0.0 < u[j] < 1.0
+    us = np.array([orc.uniforms2(5, i, 0, 0) for i in range(20000)]).ravel()
+    assert abs(us.mean() - 0.5) < 4 / math.sqrt(12 * us.size) and abs(us.var() - 1 / 12) < 2e-3
+
+
+def test_poisson_moments(orc):
+    """mean / variance / skewness at means {0.5, 5, 50, 3e4, 1e5} (C8.12)."""
+    for mean, n in ((0.5, 40000), (5.0, 40000), (50.0, 40000), (3e4, 40000), (1e5, 40000)):
+        k = np.array([orc.poisson(1234, i, 3, mean) for i in range(n)], dtype=np.float64)
+        se = math.sqrt(mean / n)
+        assert abs(k.mean() - mean) < 4.5 * se, (mean, k.mean())
+        assert abs(k.var() - mean) < 5 * mean * math.sqrt(2.0 / n + 1.0 / (mean * n)), (mean, k.var())
+        skew = ((k - k.mean()) ** 3).mean() / k.std() ** 3
+        assert abs(skew - 1 / math.sqrt(mean)) < 5 * math.sqrt(6.0 / n) + 0.02, (mean, skew)
+    assert orc.poisson(1, 0, 3, 0.0) == 0
+
+
+def test_poisson_small_mean_exact_pmf(orc):
+    n = 60000
+    k = np.array([orc.poisson(42, i, 4, 3.2) for i in range(n)])
+    for j in range(9):
+        p = math.exp(-3.2) * 3.2 ** j / math.factorial(j)
+        assert abs((k == j).mean() - p) < 5 * math.sqrt(p * (1 - p) / n)
+
+
+def _chi2_vs_pdf(orc, x, p, nb=200):
+    edges = np.linspace(LO, HI, nb + 1)
+    obs, _ = np.histogram(x, edges)
+    # expected from the oracle's own normalised mixture pdf, Simpson within each bin
+    def pdf(t):
+        return np.exp(orc.logpdf(t, p, LO, HI))
+    a, b = edges[:-1], edges[1:]
+    m = 0.5 * (a + b)
+    exp = x.size * (b - a) / 6 * (pdf(a) + 4 * pdf(m) + pdf(b))
+    return float(((obs - exp) ** 2 / exp).sum()), nb
+
+
+def test_mixture_generator_chi2(orc):
+    """chi^2 of generated events against f S + (1-f) B in 200 bins (C8.12)."""
+    for seed, p in ((1, P1), (7, P2)):
+        x = orc.generate_mixture(seed, 60000, p, LO, HI)
+        assert x.min() >= LO and x.max() <= HI
+        chi2, nb = _chi2_vs_pdf(orc, x, p)
+        assert chi2 < nb + 5 * math.sqrt(2 * nb), chi2
+        # deterministic and prefix-stable: slot i does not depend on n
+        assert (orc.generate_mixture(seed, 100, p, LO, HI) == x[:100]).all()
+    assert abs((np.abs(orc.generate_mixture(1, 60000, P1, LO, HI) - 5280) <= 30).mean() - 0.34443) < 0.01
+
+
+def test_toy_generator_structure(orc):
+    seeds = inp.toy_seeds(6)
+    x, off = orc.toy_generate(seeds, P1, 300.0, 700.0, LO, HI)
+    assert off[0] == 0 and (np.diff(off) > 0).all() and off[-1] == x.size
+    for t, s in enumerate(seeds):
+        ns, nb = orc.poisson(int(s), 0, 3, 300.0), orc.poisson(int(s), 1, 3, 700.0)
+        assert off[t + 1] - off[t] == ns + nb
+        seg = x[off[t]:off[t + 1]]
+        # signal block first: concentrated around mu; background block: spread over the range
+        assert (np.abs(seg[:ns] - 5280) < 30).mean() > 0.8
+        assert (np.abs(seg[ns:] - 5280) < 30).mean() < 0.2
+    _, off2 = orc.toy_generate(seeds, P1, 300.0, 700.0, LO, HI, offsets_only=True)
+    assert (off2 == off).all()
+    # a per-toy parameter array gives the same events as the single set when all rows are equal
+    x3, off3 = orc.toy_generate(seeds, [P1] * 6, 300.0, 700.0, LO, HI)
+    assert (off3 == off).all() and (x3 == x).all()
+
+
+def test_background_inverse_cdf_ks(orc):
+    sp = pytest.importorskip("scipy.stats")
+    x = orc.generate_mixture(11, 20000, dict(P1, f=0.0), LO, HI)
+    k = P1["k"]
+    cdf = lambda t: np.expm1(k * (t - LO)) / math.expm1(k * (HI - LO))
+    assert sp.kstest(x, cdf).pvalue > 1e-3
+
+
+def test_hist_fill_exact(orc):
+    rng = np.random.default_rng(2)
+    x = np.concatenate([rng.uniform(LO, HI, 50000), [LO, HI, LO - 1, HI + 1, 5000.6, 5599.4]])
+    c = orc.hist_fill(x, LO, HI, 1000)
+    ref, _ = np.histogram(x[(x >= LO) & (x <= HI)], bins=1000, range=(LO, HI))
+    assert c.sum() == 50004 and c.dtype == np.uint64
+    # numpy's binning differs only in how it treats edges that are not representable; compare exactly
+    # against the stated rule instead: bin = floor((x-lo)*nbins/(hi-lo)), x==hi -> last bin
+    b = np.floor((x - LO) * (1000 / (HI - LO))).astype(np.int64)
+    keep = (x >= LO) & (x <= HI)
+    b = np.minimum(b[keep], 999)
+    assert (np.bincount(b, minlength=1000) == c.astype(np.int64)).all()
+    assert np.abs(ref - c.astype(np.int64)).sum() <= 4
+
+
+def test_binned_nll_definition(orc):
+    """B2 (reading D15) against a direct numpy evaluation built from orc.log_I only."""
+    nb_ = 50
+    rng = np.random.default_rng(4)
+    counts = rng.poisson(200, nb_).astype(np.uint64)
+    counts[3] = 0
+    ns, nb, kk = np.array([0.0, 120.0, 500.0]), np.array([10000.0, 9880.0, 9500.0]), np.array([-0.002, -0.0021, 0.0])
+    got = orc.binned_nll_scan(counts, LO, HI, P1, ns, nb, kk)
+    c = LO + (np.arange(nb_) + 0.5) * (HI - LO) / nb_
+    s = np.exp([orc.log_I(P1, float(t) - P1["mu"]) for t in c]); s /= s.sum()
+    for q in range(3):
+        b = np.exp(kk[q] * c); b /= b.sum()
+        nu = ns[q] * s + nb[q] * b
+        n = counts.astype(np.float64)
+        ref = float(math.fsum(nu - np.where(n > 0, n * np.log(nu), 0.0)))
+        assert abs(got[q] - ref) <= 1e-12 * abs(ref)
+        e = orc.expected_hist(nb_, LO, HI, P1, ns[q], nb[q], kk[q])
+        assert np.allclose(e, nu, rtol=1e-13, atol=0) and abs(e.sum() - (ns[q] + nb[q])) <= 1e-9
+
+
+def test_binned_scan_minimum_near_truth(orc):
+    """Scan minimum near the generating (ns, k) (C8.12), small version of config 5."""
+    nbins, N, nsig = 200, 200000, 2500
+    x = np.concatenate([orc.generate_mixture(5, nsig, dict(P1, f=1.0), LO, HI),
+                        orc.generate_mixture(6, N - nsig, dict(P1, f=0.0), LO, HI)])
+    counts = orc.hist_fill(x, LO, HI, nbins)
+    NS, NB, KK = inp.scan_grid(21, 21, n_obs=float(N))
+    nll = orc.binned_nll_scan(counts, LO, HI, P1, NS, NB, KK)
+    q = int(np.argmin(nll))
+    assert abs(NS[q] - nsig) <= 750 and abs(KK[q] + 0.002) <= 1.01e-4
+
+
+def test_poisson_hist_toys(orc):
+    mean = np.array([0.0, 0.7, 8.0, 120.0, 1e5])
+    t = orc.poisson_hist_toys(mean, np.arange(1, 3001, dtype=np.uint64))
+    assert t.shape == (3000, 5) and t.dtype == np.uint32 and (t[:, 0] == 0).all()
+    for b in range(1, 5):
+        col = t[:, b].astype(np.float64)
+        assert abs(col.mean() - mean[b]) < 4.5 * math.sqrt(mean[b] / 3000)
+        assert abs(col.var() / mean[b] - 1) < 0.15
+    # element (t, b) depends only on (seed_t, b, mean_b)
+    assert orc.poisson(7, 3, 4, 120.0) == t[6, 3]
