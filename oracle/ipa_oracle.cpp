@@ -162,6 +162,8 @@ static void miller_once(ld mu, ld x, int N, ld* Ks, ld* K1s) {
     tn = tm;
     S += C[n - 1] * tn;
     if (n == 1) t1_keep = tn1;
+    /* only ratios matter: rescale so that a long recurrence cannot overflow */
+    if (n > 1 && fabsl(tn) > 1e2000L) { tn *= 1e-2000L; tn1 *= 1e-2000L; S *= 1e-2000L; }
   }
   const ld t0 = tn;
   *Ks = sqrtl(PI_L / (2 * x)) * t0 / S;
@@ -177,7 +179,9 @@ static void miller(ld mu, ld x, ld* Ks, ld* K1s) {
     N *= 2;
     ld a2, b2;
     miller_once(mu, x, N, &a2, &b2);
-    const bool ok = fabsl(a2 - a) <= 2e-19L * fabsl(a2) && fabsl(b2 - b) <= 2e-19L * fabsl(b2);
+    /* 1e-17 relative: ~100 ulp of long double, still 10x below fp64 resolution (a 2e-19 test is
+     * within rounding noise of the recurrence and fails at random) */
+    const bool ok = fabsl(a2 - a) <= 1e-17L * fabsl(a2) && fabsl(b2 - b) <= 1e-17L * fabsl(b2);
     a = a2; b = b2;
     if (ok) break;
   }

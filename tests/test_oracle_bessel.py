@@ -111,3 +111,14 @@ def test_miller_identities_hold_in_mpmath():
 def test_zeta_values(orc):
     for k in (2, 3, 4, 7, 20, 60):
         assert abs(mp.mpf(orc.zeta_int(k)) - mp.zeta(k)) <= 3e-16
+
+
+def test_dense_scan_is_finite_and_smooth(orc):
+    """Regression pin: the backward recurrence must not overflow when its stopping test needs many
+    doublings (a 2e-19 test once failed at random and produced NaN at ~1e-4 of all arguments).
+    e^x K_nu(x) is smooth and decreasing in x, so a dense scan must be finite and monotone."""
+    for nu in (1.8, 0.3, 2.5):
+        xs = np.linspace(2.0001, 12.0, 60001)
+        v = np.array([orc.besselk_scaled(nu, x) for x in xs])
+        assert np.isfinite(v).all()
+        assert (np.diff(v) < 0).all()
