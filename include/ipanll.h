@@ -1,0 +1,163 @@
+/*
+ * ipanll.h -- C ABI of libipanll.so: the B200 (sm_100a) hot path of the unbinned maximum-likelihood
+ * fit of arXiv:1706.01420 ("Ipanema-beta"), Example 1: the negative log-likelihood
+ *
+ *      NLL(theta) = - sum_i log( f S(x_i; theta) + (1-f) B(x_i; theta) )
+ *
+ * of an Ipatia signal S (generalised-hyperbolic Bessel-K core with two power-law tails; the paper only
+ * names it -- `__device__ double log_apIpatia`, PAPER.md:54 -- and cites its ref. [10], PAPER.md:450;
+ * the definition used here is DESIGN.md reading C1) plus an exponential background B,
+ * each normalised over the fit range, evaluated for a batch of K parameter sets per
+ * pass over the events; plus the toy-MC generators and the binned Poisson
+ * variant that feed the same likelihood.
+ *
+ * Conventions common to every entry point
+ *   - `*_dev` pointers are CUDA device pointers, `*_host` pointers are host pointers.  The caller owns
+ *     every buffer.  The library never allocates or frees device memory and never synchronises: all
+ *     work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default
+ *     stream) and results are valid once the caller has synchronised that stream.  `*_host` inputs are
+ *     read completely before the call returns (they are copied into the kernel-parameter space or
+ *     into the workspace with kernel arguments, never with an asynchronous host read), so they may be
+ *     reused immediately.  Every call is CUDA-graph capturable.
+ *   - `ws_dev` is a scratch workspace of at least ipa_workspace_bytes(...) bytes, 256-byte aligned,
+ *     private to one stream at a time.
+ *   - Return value: IPA_OK (0) or a negative ipa_status.  Argument errors are detected before any
+ *     work is enqueued.  CUDA launch errors are returned as IPA_ERR_CUDA (text: ipa_last_cuda_error).
+ *   - Per-parameter-set DOMAIN errors do not fail the call: the set gets status != 0 in `status_dev`
+ *     and NLL = +inf, so that a minimiser stepping outside the domain can recover.  Status values:
+ *     0 ok; 1 basic domain (non-finite field, sigma<=0, zeta<=0, a<=0, a2<=0, n<=0, n2<=0, f outside
+ *     [0,1]); 2 join slope sign (L(d0)<=0 or L(d1)>=0: the power-law tail does not exist);
+ *     3 internal numerical failure (normalisation not finite or not positive).
+ *   - Events outside [lo,hi] are evaluated by the same formulae (no clipping); NaN events give NaN.
+ *     Any n >= 0 is accepted (n == 0 gives NLL = +0.0).
+ *   - Determinism: for fixed device, build, n and launch geometry the results are bitwise
+ *     reproducible, and the result of set k does not depend on which other sets share the batch.
+ */
+#ifndef IPANLL_H
+#define IPANLL_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+/* One parameter set: 11 doubles.  Order follows the positional argument list of the paper's signal
+ * kernel (mu, sigma, <unnamed 1>, beta, a, n, a2, n2) with the unnamed shape argument
+ * expanded to (lambda, zeta) (reading D2), followed by the mixture parameters of
+ * PAPER.md:77-85. */
+typedef struct {
+  double mu;     /* peak position */
+  double sigma;  /* core width: the untruncated symmetric core has variance sigma^2 */
+  double lambda; /* generalised-hyperbolic index; Bessel order nu = lambda - 1/2 */
+  double zeta;   /* > 0; shape of the core (zeta -> inf: Gaussian) */
+  double beta;   /* asymmetry, exp(beta d) factor */
+  double a;      /* left join at d0 = -a sigma, a > 0 */
+  double n;      /* left tail power, > 0 */
+  double a2;     /* right join at d1 = +a2 sigma, a2 > 0 */
+  double n2;     /* right tail power, > 0 */
+  double f;      /* signal fraction in [0,1] */
+  double k;      /* background slope: B(x) ~ exp(k x); k == 0 allowed */
+} ipa_params;
+
+typedef struct { double lo, hi; } ipa_range; /* fit range, finite, hi > lo */
+
+typedef enum {
+  IPA_OK = 0,
+  IPA_ERR_INVALID_ARG = -1, /* null pointer, negative size, K < 1, hi <= lo, misaligned pointer */
+  IPA_ERR_WORKSPACE = -2,   /* ws_bytes < ipa_workspace_bytes(...) or ws_dev misaligned */
+  IPA_ERR_CUDA = -3,        /* a CUDA runtime call or launch failed */
+  IPA_ERR_NO_DEVICE = -4    /* no usable sm_100 device / kernel image */
+} ipa_status;
+
+const char* ipa_strerror(int code);
+/* Text of the last CUDA error seen by this thread inside the library ("" if none). */
+const char* ipa_last_cuda_error(void);
+/* Library build tag, e.g. "ipanll 0.1 sm_100a". */
+const char* ipa_version(void);
+
+/* Core-approximant degree policy (prologue): 0 = adaptive (the Chebyshev series of
+ * log(z^nu K_nu(z)) is cut where its coefficients fall under the fp64 noise floor, so a half-integer
+ * order collapses to a very short polynomial); 1 = geometric (at least the a-priori degree for a
+ * general order on the same z-interval: no half-integer shortcut; reading D2).  Default 0.
+ * Returns the previous policy.  Process-wide; not thread-safe against concurrent calls. */
+int ipa_set_degree_policy(int policy);
+
+/* Bytes of workspace needed by any call below for n events, K parameter sets (or T segments / toys:
+ * pass the larger of K and T) and nbins histogram bins (0 if unused). */
+size_t ipa_workspace_bytes(int64_t n, int64_t K, int64_t nbins);
+
+/* Normalisation integrals of K parameter sets (readings C2, C5):
+ *   norm_sig_dev[k] = N_S = int_lo^hi I(x - mu) dx   (closed-form tails + Gauss-Legendre core)
+ *   norm_bkg_dev[k] = N_B = int_lo^hi exp(k (x - lo)) dx = expm1(k (hi-lo)) / k   (hi-lo at k=0)
+ * status_dev[k] as described above (may be NULL).  Invalid sets give NaN. */
+int ipa_norm(const ipa_params* p_host, int K, ipa_range r, double* norm_sig_dev, double* norm_bkg_dev,
+             int32_t* status_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
+
+/* The hot path (fused into one pass): NLL of n events for K parameter sets.
+ *   x_dev      [n]    event masses, fp64, 8-byte aligned
+ *   p_host     [K]    parameter sets
+ *   nll_dev    [K]    out: -sum_i log(f S + (1-f) B); +inf for a set with status != 0
+ *   logpdf_dev [K*n]  out, optional (NULL to skip): per-event log(f S + (1-f) B), set-major
+ *   status_dev [K]    out, optional
+ * K <= IPA_MAX_K per call. */
+#define IPA_MAX_K 32
+int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r,
+                 double* nll_dev, double* logpdf_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
+                 void* cuda_stream);
+
+/* Same likelihood over T segments (toys, categories) of one event array, one parameter set per
+ * segment, all in one launch (BASELINE.json config 4; PAPER.md:139-149 loops categories on the host).
+ *   offsets_dev [T+1]  segment t = x_dev[offsets[t] .. offsets[t+1]), non-decreasing, on the device
+ *   p_host      [T]    parameter sets (copied through the workspace by a kernel argument path)
+ *   nll_dev     [T]    out */
+int ipa_nll_eval_segmented(const double* x_dev, const int64_t* offsets_dev, int64_t T, const ipa_params* p_host,
+                           ipa_range r, double* nll_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
+                           void* cuda_stream);
+
+/* Toy-MC generation on the device (readings D13, D14).
+ * Toy t draws Ns ~ Poisson(mean_sig), Nb ~ Poisson(mean_bkg) from seeds_host[t] (Philox-4x32-10
+ * counter-based streams), then Ns signal events by accept-reject under a flat envelope followed by
+ * Nb background events by the inverse CDF of the truncated exponential.
+ *   gen_host   [T] or [1] (gen_count = T or 1): generating parameter sets
+ *   mean_sig/mean_bkg < 0 selects MIXTURE mode for configs 1-3: T must be 1, exactly `capacity`
+ *     events are generated and the component of each event is chosen by u < f.
+ *   capacity   size of x_dev in events; if the drawn total exceeds it, offsets are still written,
+ *              no event beyond capacity is written and overflow_dev[0] is set to 1.
+ *   x_dev      [capacity] out;  offsets_dev [T+1] out;  overflow_dev [1] out (int32) */
+int ipa_toy_generate(const uint64_t* seeds_host, int64_t T, const ipa_params* gen_host, int64_t gen_count,
+                     double mean_sig, double mean_bkg, ipa_range r, int64_t capacity, double* x_dev,
+                     int64_t* offsets_dev, int32_t* overflow_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
+
+/* Histogram of n events in nbins uniform bins on [lo,hi]:
+ * bin = floor((x-lo) nbins/(hi-lo)), x == hi goes to the last bin, events outside are dropped.
+ * counts_dev [nbins] is overwritten. */
+int ipa_hist_fill(const double* x_dev, int64_t n, ipa_range r, int nbins, uint64_t* counts_dev, void* cuda_stream);
+
+/* Binned Poisson likelihood over a list of parameter points (reading D15):
+ *   s_b = I(c_b - mu) / sum_b' I(c_b' - mu),  b_b = e^{k c_b} / sum_b' e^{k c_b'}  at bin centres c_b,
+ *   nu_b = ns s_b + nb b_b,   NLL = sum_b [ nu_b - n_b log nu_b ]   (n_b = 0: nu_b).
+ *   counts_dev [nbins]; shape_host: one parameter set (its f and k are ignored);
+ *   ns_host, nb_host, k_host [npoints]; nll_dev [npoints] out. */
+int ipa_binned_nll_scan(const uint64_t* counts_dev, int nbins, ipa_range r, const ipa_params* shape_host,
+                        const double* ns_host, const double* nb_host, const double* k_host, int64_t npoints,
+                        double* nll_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
+
+/* Expected histogram nu_b = ns s_b + nb b_b for one point (input of ipa_poisson_hist_toys). */
+int ipa_expected_hist(int nbins, ipa_range r, const ipa_params* shape_host, double ns, double nb, double k,
+                      double* nu_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
+
+/* Per-bin Poisson toys, a separate mean per generated value:
+ * counts_dev[t*nbins + b] ~ Poisson(mean_dev[b]) from key seeds_host[t], counter slot b. */
+int ipa_poisson_hist_toys(const double* mean_dev, int nbins, const uint64_t* seeds_host, int64_t T,
+                          uint32_t* counts_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
+
+/* Measurement aid (not on the hot path): runs `iters` dependent DFMA per thread in 8 independent
+ * chains on a full grid, for the FP64 roofline denominator.  out_dev [1]. */
+int ipa_fp64_peak_probe(int64_t iters, double* out_dev, void* cuda_stream);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* IPANLL_H */

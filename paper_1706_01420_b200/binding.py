@@ -1,0 +1,269 @@
+"""ctypes binding of libipanll.so: same names as include/ipanll.h, torch tensors for device memory
+and streams (plumbing only).  Each wrapper marshals arguments, sizes the workspace and checks the
+return code; no arithmetic of the method happens here.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+import torch
+
+from . import build as _build
+
+__all__ = [
+    "PARAM_FIELDS", "NPAR", "IPA_MAX_K", "IpaError", "lib", "library_path", "pack_params", "workspace",
+    "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes", "ipa_norm", "ipa_nll_eval",
+    "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill", "ipa_binned_nll_scan", "ipa_expected_hist",
+    "ipa_poisson_hist_toys", "ipa_fp64_peak_probe", "nll_host", "EXPORTS",
+]
+
+PARAM_FIELDS = ("mu", "sigma", "lambda", "zeta", "beta", "a", "n", "a2", "n2", "f", "k")
+NPAR = len(PARAM_FIELDS)
+IPA_MAX_K = 32
+
+# every symbol include/ipanll.h declares
+EXPORTS = (
+    "ipa_strerror", "ipa_last_cuda_error", "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes",
+    "ipa_norm", "ipa_nll_eval", "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill",
+    "ipa_binned_nll_scan", "ipa_expected_hist", "ipa_poisson_hist_toys", "ipa_fp64_peak_probe",
+)
+
+
+class IpaError(RuntimeError):
+    pass
+
+
+class _Range(C.Structure):
+    _fields_ = [("lo", C.c_double), ("hi", C.c_double)]
+
+
+_lib = None
+
+
+def library_path():
+    return _build.LIB
+
+
+def lib():
+    """Load (building if needed) libipanll.so.  Fails loudly if it cannot be built or loaded."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.build()
+    L = C.CDLL(path)
+    vp, i64, i32, d, sz = C.c_void_p, C.c_int64, C.c_int, C.c_double, C.c_size_t
+    L.ipa_strerror.restype = C.c_char_p; L.ipa_strerror.argtypes = [i32]
+    L.ipa_last_cuda_error.restype = C.c_char_p; L.ipa_last_cuda_error.argtypes = []
+    L.ipa_version.restype = C.c_char_p; L.ipa_version.argtypes = []
+    L.ipa_set_degree_policy.restype = i32; L.ipa_set_degree_policy.argtypes = [i32]
+    L.ipa_workspace_bytes.restype = sz; L.ipa_workspace_bytes.argtypes = [i64, i64, i64]
+    L.ipa_norm.restype = i32; L.ipa_norm.argtypes = [vp, i32, _Range, vp, vp, vp, vp, sz, vp]
+    L.ipa_nll_eval.restype = i32; L.ipa_nll_eval.argtypes = [vp, i64, vp, i32, _Range, vp, vp, vp, vp, sz, vp]
+    L.ipa_nll_eval_segmented.restype = i32
+    L.ipa_nll_eval_segmented.argtypes = [vp, vp, i64, vp, _Range, vp, vp, vp, sz, vp]
+    L.ipa_toy_generate.restype = i32
+    L.ipa_toy_generate.argtypes = [vp, i64, vp, i64, d, d, _Range, i64, vp, vp, vp, vp, sz, vp]
+    L.ipa_hist_fill.restype = i32; L.ipa_hist_fill.argtypes = [vp, i64, _Range, i32, vp, vp]
+    L.ipa_binned_nll_scan.restype = i32
+    L.ipa_binned_nll_scan.argtypes = [vp, i32, _Range, vp, vp, vp, vp, i64, vp, vp, sz, vp]
+    L.ipa_expected_hist.restype = i32; L.ipa_expected_hist.argtypes = [i32, _Range, vp, d, d, d, vp, vp, sz, vp]
+    L.ipa_poisson_hist_toys.restype = i32; L.ipa_poisson_hist_toys.argtypes = [vp, i32, vp, i64, vp, vp, sz, vp]
+    L.ipa_fp64_peak_probe.restype = i32; L.ipa_fp64_peak_probe.argtypes = [i64, vp, vp]
+    _lib = L
+    return L
+
+
+def _check(rc):
+    if rc != 0:
+        L = lib()
+        msg = L.ipa_strerror(rc).decode()
+        extra = L.ipa_last_cuda_error().decode()
+        raise IpaError(f"libipanll: {msg} ({rc})" + (f": {extra}" if extra else ""))
+
+
+def _need_cuda():
+    if not torch.cuda.is_available():
+        raise IpaError("libipanll needs a CUDA device (sm_100a); there is no CPU fallback")
+
+
+def _stream(stream):
+    if stream is None:
+        stream = torch.cuda.current_stream()
+    return C.c_void_p(stream.cuda_stream)
+
+
+def _dptr(t, dtype=None):
+    if t is None:
+        return None
+    assert t.is_cuda and t.is_contiguous(), "device tensors must be contiguous CUDA tensors"
+    if dtype is not None:
+        assert t.dtype == dtype, (t.dtype, dtype)
+    return C.c_void_p(t.data_ptr())
+
+
+def _hptr(a):
+    return a.ctypes.data_as(C.c_void_p)
+
+
+def pack_params(p):
+    """dict / list of dicts / (K,11) array -> contiguous (K,11) float64 numpy array."""
+    if isinstance(p, dict):
+        p = [p]
+    if isinstance(p, (list, tuple)) and len(p) and isinstance(p[0], dict):
+        arr = np.array([[q[name] for name in PARAM_FIELDS] for q in p], dtype=np.float64)
+    else:
+        arr = np.array(p, dtype=np.float64)
+        if arr.ndim == 1:
+            arr = arr[None, :]
+    assert arr.ndim == 2 and arr.shape[1] == NPAR
+    return np.ascontiguousarray(arr)
+
+
+def ipa_version():
+    return lib().ipa_version().decode()
+
+
+def ipa_set_degree_policy(policy):
+    return lib().ipa_set_degree_policy(int(policy))
+
+
+def ipa_workspace_bytes(n, K, nbins=0):
+    return int(lib().ipa_workspace_bytes(int(n), int(K), int(nbins)))
+
+
+def workspace(n, K, nbins=0, device="cuda"):
+    """Allocate a workspace tensor (uint8) large enough for the given sizes."""
+    _need_cuda()
+    return torch.empty(ipa_workspace_bytes(n, K, nbins), dtype=torch.uint8, device=device)
+
+
+def _ws(ws, n, K, nbins=0):
+    if ws is None:
+        ws = workspace(n, K, nbins)
+    return ws
+
+
+def ipa_norm(params, lo, hi, ws=None, stream=None):
+    """-> (norm_sig[K], norm_bkg[K], status[K]) device tensors."""
+    _need_cuda()
+    P = pack_params(params)
+    K = P.shape[0]
+    ws = _ws(ws, 0, K)
+    ns = torch.empty(K, dtype=torch.float64, device="cuda")
+    nb = torch.empty(K, dtype=torch.float64, device="cuda")
+    st = torch.empty(K, dtype=torch.int32, device="cuda")
+    _check(lib().ipa_norm(_hptr(P), K, _Range(lo, hi), _dptr(ns), _dptr(nb), _dptr(st), _dptr(ws), ws.numel(),
+                          _stream(stream)))
+    return ns, nb, st
+
+
+def ipa_nll_eval(x, params, lo, hi, want_logpdf=False, ws=None, stream=None, out=None, status=None):
+    """NLL of the events in device tensor x (fp64) for K parameter sets.
+
+    -> (nll[K], logpdf[K,n] or None, status[K]) device tensors; nothing is synchronised.
+    """
+    _need_cuda()
+    P = pack_params(params)
+    K = P.shape[0]
+    n = x.numel()
+    ws = _ws(ws, n, K)
+    nll = out if out is not None else torch.empty(K, dtype=torch.float64, device="cuda")
+    st = status if status is not None else torch.empty(K, dtype=torch.int32, device="cuda")
+    lp = torch.empty((K, n), dtype=torch.float64, device="cuda") if want_logpdf else None
+    _check(lib().ipa_nll_eval(_dptr(x, torch.float64) if n else None, n, _hptr(P), K, _Range(lo, hi), _dptr(nll),
+                              _dptr(lp), _dptr(st), _dptr(ws), ws.numel(), _stream(stream)))
+    return nll, lp, st
+
+
+def ipa_nll_eval_segmented(x, offsets, params, lo, hi, ws=None, stream=None):
+    """-> (nll[T], status[T]); offsets is an int64 device tensor [T+1]."""
+    _need_cuda()
+    P = pack_params(params)
+    T = offsets.numel() - 1
+    assert P.shape[0] == T
+    ws = _ws(ws, x.numel(), T)
+    nll = torch.empty(T, dtype=torch.float64, device="cuda")
+    st = torch.empty(T, dtype=torch.int32, device="cuda")
+    _check(lib().ipa_nll_eval_segmented(_dptr(x, torch.float64), _dptr(offsets, torch.int64), T, _hptr(P),
+                                        _Range(lo, hi), _dptr(nll), _dptr(st), _dptr(ws), ws.numel(), _stream(stream)))
+    return nll, st
+
+
+def ipa_toy_generate(seeds, gen, mean_sig, mean_bkg, lo, hi, capacity, ws=None, stream=None, x=None):
+    """Toy generation.  mean_sig < 0 selects mixture mode (one toy of exactly `capacity` events).
+
+    -> (x[capacity], offsets[T+1] int64, overflow[1] int32) device tensors."""
+    _need_cuda()
+    seeds = np.ascontiguousarray(seeds, dtype=np.uint64).ravel()
+    T = seeds.size
+    P = pack_params(gen)
+    ws = _ws(ws, capacity, T)
+    if x is None:
+        x = torch.empty(int(capacity), dtype=torch.float64, device="cuda")
+    off = torch.empty(T + 1, dtype=torch.int64, device="cuda")
+    ovf = torch.zeros(1, dtype=torch.int32, device="cuda")
+    _check(lib().ipa_toy_generate(_hptr(seeds), T, _hptr(P), P.shape[0], float(mean_sig), float(mean_bkg),
+                                  _Range(lo, hi), int(capacity), _dptr(x) if capacity else None, _dptr(off), _dptr(ovf),
+                                  _dptr(ws), ws.numel(), _stream(stream)))
+    return x, off, ovf
+
+
+def ipa_hist_fill(x, lo, hi, nbins, stream=None):
+    _need_cuda()
+    counts = torch.empty(int(nbins), dtype=torch.int64, device="cuda")  # uint64 payload
+    n = x.numel()
+    _check(lib().ipa_hist_fill(_dptr(x, torch.float64) if n else None, n, _Range(lo, hi), int(nbins), _dptr(counts),
+                               _stream(stream)))
+    return counts
+
+
+def ipa_binned_nll_scan(counts, lo, hi, shape, ns, nb, k, ws=None, stream=None):
+    _need_cuda()
+    P = pack_params(shape)
+    ns = np.ascontiguousarray(ns, dtype=np.float64); nb = np.ascontiguousarray(nb, dtype=np.float64)
+    k = np.ascontiguousarray(k, dtype=np.float64)
+    npts, nbins = ns.size, counts.numel()
+    ws = _ws(ws, 0, npts, nbins)
+    out = torch.empty(npts, dtype=torch.float64, device="cuda")
+    _check(lib().ipa_binned_nll_scan(_dptr(counts, torch.int64), nbins, _Range(lo, hi), _hptr(P), _hptr(ns), _hptr(nb),
+                                     _hptr(k), npts, _dptr(out), _dptr(ws), ws.numel(), _stream(stream)))
+    return out
+
+
+def ipa_expected_hist(nbins, lo, hi, shape, ns, nb, k, ws=None, stream=None):
+    _need_cuda()
+    P = pack_params(shape)
+    ws = _ws(ws, 0, 1, nbins)
+    out = torch.empty(int(nbins), dtype=torch.float64, device="cuda")
+    _check(lib().ipa_expected_hist(int(nbins), _Range(lo, hi), _hptr(P), float(ns), float(nb), float(k), _dptr(out),
+                                   _dptr(ws), ws.numel(), _stream(stream)))
+    return out
+
+
+def ipa_poisson_hist_toys(mean, seeds, ws=None, stream=None):
+    _need_cuda()
+    seeds = np.ascontiguousarray(seeds, dtype=np.uint64).ravel()
+    T, nbins = seeds.size, mean.numel()
+    ws = _ws(ws, 0, T)
+    out = torch.empty((T, nbins), dtype=torch.int32, device="cuda")  # uint32 payload
+    _check(lib().ipa_poisson_hist_toys(_dptr(mean, torch.float64), nbins, _hptr(seeds), T, _dptr(out), _dptr(ws),
+                                       ws.numel(), _stream(stream)))
+    return out
+
+
+def ipa_fp64_peak_probe(iters, stream=None):
+    _need_cuda()
+    out = torch.zeros(1, dtype=torch.float64, device="cuda")
+    _check(lib().ipa_fp64_peak_probe(int(iters), _dptr(out), _stream(stream)))
+    return out
+
+
+def nll_host(x_host, params, lo, hi, x_dev=None, ws=None):
+    """End-to-end convenience used by bench.py's e2e leg: host (pinned) events in, host NLL out.
+    Copies x to the device, runs ipa_nll_eval, copies the K results back and synchronises."""
+    _need_cuda()
+    if x_dev is None:
+        x_dev = torch.empty(x_host.numel(), dtype=torch.float64, device="cuda")
+    x_dev.copy_(x_host, non_blocking=True)
+    nll, _, _ = ipa_nll_eval(x_dev, params, lo, hi, ws=ws)
+    return nll.cpu()

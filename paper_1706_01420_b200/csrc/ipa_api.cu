@@ -1,0 +1,332 @@
+// ipa_api.cu -- the C ABI of include/ipanll.h: argument validation, workspace layout and launch
+// sequencing on the caller's stream.  No allocation, no synchronisation, no CPU arithmetic of the
+// method: every step of the path runs in the kernels of ipa_kernels.cuh.
+#include <cstdio>
+#include <cstring>
+#include <string>
+#include "ipa_kernels.cuh"
+
+namespace {
+
+thread_local std::string g_last_cuda_error;
+int g_degree_policy = 0;
+
+#define IPA_CK(call)                                                                       \
+  do {                                                                                     \
+    cudaError_t e_ = (call);                                                               \
+    if (e_ != cudaSuccess) {                                                               \
+      g_last_cuda_error = std::string(#call) + ": " + cudaGetErrorString(e_);              \
+      return IPA_ERR_CUDA;                                                                 \
+    }                                                                                      \
+  } while (0)
+
+constexpr int64_t kGridMax = 2048;  // upper bound of the streaming grid (partials sizing)
+
+size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// Workspace layout (offsets in bytes, every block 256-byte aligned).
+struct Layout {
+  size_t consts, counter, partials, params, seeds, nsig, ntot, pts, sbin, flag, total;
+};
+Layout make_layout(int64_t K, int64_t nbins) {
+  if (K < 1) K = 1;
+  if (nbins < 0) nbins = 0;
+  Layout L;
+  size_t o = 0;
+  L.consts = o;   o += align_up((size_t)K * sizeof(IpaSetConsts), 256);
+  L.counter = o;  o += 256;
+  const int64_t kk = K < IPA_MAX_K ? K : IPA_MAX_K;
+  size_t pb = (size_t)kk * kGridMax * 8;
+  if ((size_t)K * IPA_SEGC * 8 > pb) pb = (size_t)K * IPA_SEGC * 8;
+  L.partials = o; o += align_up(pb, 256);
+  L.params = o;   o += align_up((size_t)K * sizeof(ipa_params), 256);
+  L.seeds = o;    o += align_up((size_t)K * 8, 256);
+  L.nsig = o;     o += align_up((size_t)K * 8, 256);
+  L.ntot = o;     o += align_up((size_t)K * 8, 256);
+  L.pts = o;      o += align_up((size_t)K * 3 * 8, 256);
+  L.sbin = o;     o += align_up((size_t)nbins * 8, 256);
+  L.flag = o;     o += 256;
+  L.total = o;
+  return L;
+}
+
+struct DevInfo { int dev = -1; int sms = 0; bool attr_set = false; };
+thread_local DevInfo g_dev;
+
+int device_info(int* sms) {
+  int dev = 0;
+  IPA_CK(cudaGetDevice(&dev));
+  if (g_dev.dev != dev || !g_dev.attr_set) {
+    int n = 0;
+    IPA_CK(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev));
+    const int smem = IPA_MAX_K * (int)(sizeof(IpaSetConsts) + IPA_BLOCK * 8);
+    IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    g_dev.dev = dev;
+    g_dev.sms = n;
+    g_dev.attr_set = true;
+  }
+  *sms = g_dev.sms;
+  return IPA_OK;
+}
+
+bool range_ok(ipa_range r) {
+  return ipa_finite(r.lo) && ipa_finite(r.hi) && r.hi > r.lo;
+}
+bool ws_ok(const void* ws, size_t bytes, size_t need) {
+  return ws != nullptr && ((uintptr_t)ws % 256) == 0 && bytes >= need;
+}
+
+// Runs the prologue for K sets.  K <= IPA_MAX_K: the sets travel in the kernel-parameter space;
+// larger batches go through the workspace with one host-to-device copy.
+int run_prologue(const ipa_params* p_host, int64_t K, ipa_range r, char* ws, const Layout& L, double* norm_sig,
+                 double* norm_bkg, int32_t* status_out, cudaStream_t st) {
+  IpaSetConsts* consts = reinterpret_cast<IpaSetConsts*>(ws + L.consts);
+  unsigned int* counter = reinterpret_cast<unsigned int*>(ws + L.counter);
+  static thread_local IpaParamBatch batch;
+  const ipa_params* p_dev = nullptr;
+  if (K <= IPA_MAX_K) {
+    std::memcpy(batch.p, p_host, (size_t)K * sizeof(ipa_params));
+  } else {
+    IPA_CK(cudaMemcpyAsync(ws + L.params, p_host, (size_t)K * sizeof(ipa_params), cudaMemcpyHostToDevice, st));
+    p_dev = reinterpret_cast<const ipa_params*>(ws + L.params);
+  }
+  ipa_prologue_kernel<<<(unsigned)K, IPA_PRO_THREADS, 0, st>>>(batch, p_dev, r.lo, r.hi, g_degree_policy, consts,
+                                                               counter, norm_sig, norm_bkg, status_out);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
+}  // namespace
+
+extern "C" {
+
+const char* ipa_strerror(int code) {
+  switch (code) {
+    case IPA_OK: return "ok";
+    case IPA_ERR_INVALID_ARG: return "invalid argument";
+    case IPA_ERR_WORKSPACE: return "workspace too small or misaligned";
+    case IPA_ERR_CUDA: return "CUDA error (see ipa_last_cuda_error)";
+    case IPA_ERR_NO_DEVICE: return "no usable CUDA device";
+    default: return "unknown error code";
+  }
+}
+
+const char* ipa_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
+const char* ipa_version(void) { return "ipanll 0.1 sm_100a"; }
+
+int ipa_set_degree_policy(int policy) {
+  const int old = g_degree_policy;
+  g_degree_policy = policy ? 1 : 0;
+  return old;
+}
+
+size_t ipa_workspace_bytes(int64_t n, int64_t K, int64_t nbins) {
+  (void)n;
+  return make_layout(K, nbins).total;
+}
+
+int ipa_norm(const ipa_params* p_host, int K, ipa_range r, double* norm_sig_dev, double* norm_bkg_dev,
+             int32_t* status_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (!p_host || K < 1 || !range_ok(r) || !norm_sig_dev || !norm_bkg_dev) return IPA_ERR_INVALID_ARG;
+  const Layout L = make_layout(K, 0);
+  if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
+  return run_prologue(p_host, K, r, static_cast<char*>(ws_dev), L, norm_sig_dev, norm_bkg_dev, status_dev,
+                      static_cast<cudaStream_t>(cuda_stream));
+}
+
+int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r, double* nll_dev,
+                 double* logpdf_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (n < 0 || (n > 0 && !x_dev) || !p_host || K < 1 || K > IPA_MAX_K || !range_ok(r) || !nll_dev)
+    return IPA_ERR_INVALID_ARG;
+  if (((uintptr_t)x_dev % 8) != 0) return IPA_ERR_INVALID_ARG;
+  const Layout L = make_layout(K, 0);
+  if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
+  int sms = 0;
+  int rc = device_info(&sms);
+  if (rc) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* ws = static_cast<char*>(ws_dev);
+  rc = run_prologue(p_host, K, r, ws, L, nullptr, nullptr, nullptr, st);
+  if (rc) return rc;
+  const int64_t ntiles = (n + IPA_TILE - 1) / IPA_TILE;
+  int64_t G = (int64_t)sms * IPA_BLOCKS_PER_SM;
+  if (G > kGridMax) G = kGridMax;
+  if (G > ntiles) G = ntiles;
+  if (G < 1) G = 1;
+  const size_t smem = (size_t)K * (sizeof(IpaSetConsts) + IPA_BLOCK * 8);
+  const int vec_ok = ((uintptr_t)x_dev % 16) == 0;
+  const IpaSetConsts* consts = reinterpret_cast<const IpaSetConsts*>(ws + L.consts);
+  double* partials = reinterpret_cast<double*>(ws + L.partials);
+  unsigned int* counter = reinterpret_cast<unsigned int*>(ws + L.counter);
+  if (logpdf_dev)
+    ipa_nll_kernel<true><<<(unsigned)G, IPA_BLOCK, smem, st>>>(x_dev, n, vec_ok, consts, K, partials, logpdf_dev, counter,
+                                                               nll_dev, status_dev);
+  else
+    ipa_nll_kernel<false><<<(unsigned)G, IPA_BLOCK, smem, st>>>(x_dev, n, vec_ok, consts, K, partials, nullptr, counter,
+                                                                nll_dev, status_dev);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
+int ipa_nll_eval_segmented(const double* x_dev, const int64_t* offsets_dev, int64_t T, const ipa_params* p_host,
+                           ipa_range r, double* nll_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
+                           void* cuda_stream) {
+  if (!x_dev || !offsets_dev || T < 1 || T > 0x7fffffffLL || !p_host || !range_ok(r) || !nll_dev)
+    return IPA_ERR_INVALID_ARG;
+  const Layout L = make_layout(T, 0);
+  if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* ws = static_cast<char*>(ws_dev);
+  int rc = run_prologue(p_host, T, r, ws, L, nullptr, nullptr, nullptr, st);
+  if (rc) return rc;
+  const IpaSetConsts* consts = reinterpret_cast<const IpaSetConsts*>(ws + L.consts);
+  double* partials = reinterpret_cast<double*>(ws + L.partials);
+  ipa_nll_seg_kernel<<<dim3((unsigned)T, IPA_SEGC), IPA_BLOCK, 0, st>>>(
+      x_dev, reinterpret_cast<const long long*>(offsets_dev), consts, partials);
+  IPA_CK(cudaGetLastError());
+  ipa_seg_finalize_kernel<<<(unsigned)((T + 127) / 128), 128, 0, st>>>(partials, consts, T, nll_dev, status_dev);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
+int ipa_toy_generate(const uint64_t* seeds_host, int64_t T, const ipa_params* gen_host, int64_t gen_count,
+                     double mean_sig, double mean_bkg, ipa_range r, int64_t capacity, double* x_dev,
+                     int64_t* offsets_dev, int32_t* overflow_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  const bool mixture = (mean_sig < 0.0) || (mean_bkg < 0.0);
+  if (!seeds_host || T < 1 || T > 0x7fffffffLL || !gen_host || (gen_count != 1 && gen_count != T) || !range_ok(r) ||
+      capacity < 0 || (capacity > 0 && !x_dev) || !offsets_dev)
+    return IPA_ERR_INVALID_ARG;
+  if (mixture && T != 1) return IPA_ERR_INVALID_ARG;
+  const Layout L = make_layout(T, 0);
+  if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
+  int sms = 0;
+  int rc = device_info(&sms);
+  if (rc) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* ws = static_cast<char*>(ws_dev);
+  rc = run_prologue(gen_host, gen_count, r, ws, L, nullptr, nullptr, nullptr, st);
+  if (rc) return rc;
+  IPA_CK(cudaMemcpyAsync(ws + L.seeds, seeds_host, (size_t)T * 8, cudaMemcpyHostToDevice, st));
+  const unsigned long long* seeds = reinterpret_cast<const unsigned long long*>(ws + L.seeds);
+  const IpaSetConsts* consts = reinterpret_cast<const IpaSetConsts*>(ws + L.consts);
+  long long* nsig = reinterpret_cast<long long*>(ws + L.nsig);
+  long long* ntot = reinterpret_cast<long long*>(ws + L.ntot);
+  long long* offsets = reinterpret_cast<long long*>(offsets_dev);
+  int64_t chunks;
+  if (mixture) {
+    // offsets = {0, capacity}
+    const long long two[2] = {0, (long long)capacity};
+    IPA_CK(cudaMemcpyAsync(offsets, two, sizeof(two), cudaMemcpyHostToDevice, st));
+    if (overflow_dev) IPA_CK(cudaMemsetAsync(overflow_dev, 0, sizeof(int32_t), st));
+    chunks = (capacity + IPA_BLOCK - 1) / IPA_BLOCK;
+    if (chunks > (int64_t)sms * 16) chunks = (int64_t)sms * 16;
+  } else {
+    ipa_toy_yields_kernel<<<(unsigned)((T + 127) / 128), 128, 0, st>>>(seeds, T, mean_sig, mean_bkg, nsig, ntot);
+    IPA_CK(cudaGetLastError());
+    ipa_scan_kernel<<<1, 1024, 0, st>>>(ntot, T, offsets, capacity, overflow_dev);
+    IPA_CK(cudaGetLastError());
+    chunks = ((int64_t)sms * 16 + T - 1) / T;
+    if (chunks > 1024) chunks = 1024;
+  }
+  if (chunks < 1) chunks = 1;
+  if (capacity > 0) {
+    ipa_toy_events_kernel<<<dim3((unsigned)T, (unsigned)chunks), IPA_BLOCK, 0, st>>>(
+        seeds, consts, gen_count == T && T > 1 ? 1 : 0, nsig, offsets, r.lo, r.hi, capacity, mixture ? 1 : 0, x_dev);
+    IPA_CK(cudaGetLastError());
+  }
+  return IPA_OK;
+}
+
+int ipa_hist_fill(const double* x_dev, int64_t n, ipa_range r, int nbins, uint64_t* counts_dev, void* cuda_stream) {
+  if (n < 0 || (n > 0 && !x_dev) || !range_ok(r) || nbins < 1 || !counts_dev) return IPA_ERR_INVALID_ARG;
+  int sms = 0;
+  int rc = device_info(&sms);
+  if (rc) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  IPA_CK(cudaMemsetAsync(counts_dev, 0, (size_t)nbins * 8, st));
+  if (n == 0) return IPA_OK;
+  int64_t G = (n + 255) / 256;
+  if (G > (int64_t)sms * 8) G = (int64_t)sms * 8;
+  ipa_hist_kernel<<<(unsigned)G, 256, 0, st>>>(x_dev, n, r.lo, r.hi, nbins,
+                                               reinterpret_cast<unsigned long long*>(counts_dev));
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
+static int binned_common(const uint64_t* counts_dev, int nbins, ipa_range r, const ipa_params* shape_host,
+                         const double* ns_host, const double* nb_host, const double* k_host, int64_t npoints,
+                         double* nll_dev, double* nu_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  const Layout L = make_layout(npoints, nbins);
+  if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* ws = static_cast<char*>(ws_dev);
+  ipa_params shape = *shape_host;
+  shape.f = 0.5;  // f and k of the shape set are not used by the binned path
+  shape.k = 0.0;
+  int rc = run_prologue(&shape, 1, r, ws, L, nullptr, nullptr, nullptr, st);
+  if (rc) return rc;
+  const IpaSetConsts* consts = reinterpret_cast<const IpaSetConsts*>(ws + L.consts);
+  double* sbin = reinterpret_cast<double*>(ws + L.sbin);
+  int32_t* flag = reinterpret_cast<int32_t*>(ws + L.flag);
+  double* pts = reinterpret_cast<double*>(ws + L.pts);
+  ipa_binned_shape_kernel<<<1, 256, 0, st>>>(consts, r.lo, r.hi, nbins, sbin, flag);
+  IPA_CK(cudaGetLastError());
+  IPA_CK(cudaMemcpyAsync(pts, ns_host, (size_t)npoints * 8, cudaMemcpyHostToDevice, st));
+  IPA_CK(cudaMemcpyAsync(pts + npoints, nb_host, (size_t)npoints * 8, cudaMemcpyHostToDevice, st));
+  IPA_CK(cudaMemcpyAsync(pts + 2 * npoints, k_host, (size_t)npoints * 8, cudaMemcpyHostToDevice, st));
+  ipa_binned_scan_kernel<<<(unsigned)npoints, 256, 0, st>>>(reinterpret_cast<const unsigned long long*>(counts_dev), sbin,
+                                                            nbins, r.lo, r.hi, pts, pts + npoints, pts + 2 * npoints, flag,
+                                                            nll_dev, nu_dev);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
+int ipa_binned_nll_scan(const uint64_t* counts_dev, int nbins, ipa_range r, const ipa_params* shape_host,
+                        const double* ns_host, const double* nb_host, const double* k_host, int64_t npoints,
+                        double* nll_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (!counts_dev || nbins < 1 || !range_ok(r) || !shape_host || !ns_host || !nb_host || !k_host || npoints < 1 ||
+      npoints > 0x7fffffffLL || !nll_dev)
+    return IPA_ERR_INVALID_ARG;
+  return binned_common(counts_dev, nbins, r, shape_host, ns_host, nb_host, k_host, npoints, nll_dev, nullptr, ws_dev,
+                       ws_bytes, cuda_stream);
+}
+
+int ipa_expected_hist(int nbins, ipa_range r, const ipa_params* shape_host, double ns, double nb, double k,
+                      double* nu_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (nbins < 1 || !range_ok(r) || !shape_host || !nu_dev) return IPA_ERR_INVALID_ARG;
+  return binned_common(nullptr, nbins, r, shape_host, &ns, &nb, &k, 1, nullptr, nu_dev, ws_dev, ws_bytes, cuda_stream);
+}
+
+int ipa_poisson_hist_toys(const double* mean_dev, int nbins, const uint64_t* seeds_host, int64_t T,
+                          uint32_t* counts_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (!mean_dev || nbins < 1 || !seeds_host || T < 1 || !counts_dev) return IPA_ERR_INVALID_ARG;
+  const Layout L = make_layout(T, 0);
+  if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
+  int sms = 0;
+  int rc = device_info(&sms);
+  if (rc) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* ws = static_cast<char*>(ws_dev);
+  IPA_CK(cudaMemcpyAsync(ws + L.seeds, seeds_host, (size_t)T * 8, cudaMemcpyHostToDevice, st));
+  const int64_t total = T * (int64_t)nbins;
+  int64_t G = (total + 255) / 256;
+  if (G > (int64_t)sms * 16) G = (int64_t)sms * 16;
+  ipa_poisson_hist_kernel<<<(unsigned)G, 256, 0, st>>>(mean_dev, nbins,
+                                                       reinterpret_cast<const unsigned long long*>(ws + L.seeds), T,
+                                                       counts_dev);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
+int ipa_fp64_peak_probe(int64_t iters, double* out_dev, void* cuda_stream) {
+  if (iters < 1 || !out_dev) return IPA_ERR_INVALID_ARG;
+  int sms = 0;
+  int rc = device_info(&sms);
+  if (rc) return rc;
+  ipa_fp64_probe_kernel<<<(unsigned)(sms * 8), 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(iters, out_dev);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
+}  // extern "C"

@@ -1,0 +1,543 @@
+// ipa_kernels.cuh -- sm_100a kernels of the hot path.  Included once, by
+// ipa_api.cu.  Steps of SURVEY.md 8(a): prologue A1a-A1e, streaming NLL A2-A5 (K sets per event
+// read), segmented NLL T2, generators T0/T1, histogram B1, binned scan B2, per-bin Poisson toys B3.
+#pragma once
+#include <cuda_runtime.h>
+#include "ipa_prologue.cuh"
+
+#define IPA_BLOCK 128                     // threads per streaming block
+#define IPA_E 8                           // events per thread and tile (register blocking)
+#define IPA_TILE (IPA_BLOCK * IPA_E)
+#define IPA_BLOCKS_PER_SM 4
+#define IPA_SEGC 8                        // blocks per segment in the segmented kernel
+#define IPA_FULL 0xffffffffu
+
+struct IpaParamBatch { ipa_params p[IPA_MAX_K]; };
+
+// ------------------------------------------------------------------------------------------------
+// Prologue: one block per parameter set.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(IPA_PRO_THREADS)
+ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_params* __restrict__ p_dev, double lo,
+                    double hi, int policy, IpaSetConsts* __restrict__ consts, unsigned int* counter,
+                    double* norm_sig, double* norm_bkg, int32_t* status_out) {
+  __shared__ IpaProWork w;
+  const int tid = threadIdx.x, set = blockIdx.x;
+  if (tid == 0) {
+    w.p = p_dev ? p_dev[set] : batch.p[set];
+    w.lo = lo; w.hi = hi; w.policy = policy;
+    if (set == 0 && counter) *counter = 0u;
+  }
+  __syncthreads();
+  ipa_pro_phase0(w, tid); __syncthreads();
+  ipa_pro_phase1(w, tid); __syncthreads();
+  ipa_pro_phase2(w, tid); __syncthreads();
+  ipa_pro_phase3(w, tid, IPA_PRO_THREADS); __syncthreads();
+  ipa_pro_phase4(w, tid); __syncthreads();
+  ipa_pro_phase5(w, tid); __syncthreads();
+  ipa_pro_phase6(w, tid); __syncthreads();
+  ipa_pro_phase7(w, tid); __syncthreads();
+  const int D = w.degree;  // uniform
+  if (!w.status && !w.mode) {
+    for (int j = 0; j <= D; ++j) { ipa_pro_phase8_step(w, j, tid); __syncthreads(); }
+  }
+  ipa_pro_phase8_finish(w, tid); __syncthreads();
+  ipa_pro_phase9(w, tid); __syncthreads();
+  ipa_pro_phase10(w, tid, IPA_PRO_THREADS); __syncthreads();
+  ipa_pro_phase11(w, tid); __syncthreads();
+  IpaSetConsts& o = consts[set];
+  ipa_pro_phase12(w, o, tid); __syncthreads();
+  ipa_pro_phase13(w, o, tid);
+  if (tid == 0) {
+    if (norm_sig) norm_sig[set] = o.normS;
+    if (norm_bkg) norm_bkg[set] = o.normB;
+    if (status_out) status_out[set] = o.status;
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Per-event arithmetic, E events per thread in registers, one parameter set (record in smem).
+//   core:  t = tA sqrt(d^2+delta^2) + tB,  Delta = Horner(a, t) + (beta-k) d          (A2 core)
+//   tail:  u = uA d + uB,                  Delta = cT - n log u - k d                 (A2 tails)
+//   l = E_B + log(1 + e^Delta),  E_B = k d + eB0                                      (A3, A4)
+// The polynomial coefficient is read once (uniform LDS) per E fused multiply-adds.
+// ------------------------------------------------------------------------------------------------
+IPA_HD double ipa_softplus(double D) { return fmax(D, 0.0) + log1p(exp(-fabs(D))); }
+
+// direct-mode core term H(z) = log(z^nu K_nu(z)) (kept out of line: it is the slow path)
+__host__ __device__ __noinline__ double ipa_direct_H(double nu, double z) {
+  return nu * log(z) + log(ipa_besselk_scaled(nu, z)) - z;
+}
+
+template <int E>
+IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l)[E]) {
+  double d[E], P[E];
+  const double mu = c.mu;
+#pragma unroll
+  for (int e = 0; e < E; ++e) d[e] = x[e] - mu;
+  if (c.mode == 0) {
+    double t[E];
+    const double d2 = c.delta2, tA = c.tA, tB = c.tB;
+#pragma unroll
+    for (int e = 0; e < E; ++e) t[e] = fma(tA, sqrt(fma(d[e], d[e], d2)), tB);
+    const int D = c.degree;
+    double aj = c.a[D];
+#pragma unroll
+    for (int e = 0; e < E; ++e) P[e] = aj;
+    for (int j = D - 1; j >= 0; --j) {
+      aj = c.a[j];
+#pragma unroll
+      for (int e = 0; e < E; ++e) P[e] = fma(P[e], t[e], aj);
+    }
+  } else {
+    // direct mode (shapes the polynomial cannot cover): per-event trapezoid Bessel, core events only
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      P[e] = 0.0;
+      if (d[e] >= c.d0 && d[e] <= c.d1) P[e] = ipa_direct_H(c.nu, c.alpha * sqrt(fma(d[e], d[e], c.delta2))) + c.cDir;
+    }
+  }
+  const double kd = c.kd, eB0 = c.eB0, bmk = c.bmk;
+  const bool pure = c.pure != 0;
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const bool left = d[e] < c.d0, right = d[e] > c.d1;
+    const double uA = left ? c.uA0 : c.uA1, uB = left ? c.uB0 : c.uB1;
+    const double nT = left ? c.n0 : c.n1, cT = left ? c.cT0 : c.cT1;
+    const double u = fma(uA, d[e], uB);
+    const double tail = fma(-nT, log(u), cT) - kd * d[e];
+    const double Dl = (left || right) ? tail : fma(bmk, d[e], P[e]);
+    const double eb = fma(kd, d[e], eB0);
+    l[e] = eb + (pure ? Dl : ipa_softplus(Dl));
+  }
+}
+
+__device__ __forceinline__ double ipa_warp_sum(double v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(IPA_FULL, v, o);
+  return v;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Streaming NLL: persistent grid, tile = 128 threads x 8 events, all K sets per event read.
+// partials[k*G + b]; the last block to finish adds them in a fixed order (A5).
+// ------------------------------------------------------------------------------------------------
+template <bool LOGPDF>
+__global__ void __launch_bounds__(IPA_BLOCK, IPA_BLOCKS_PER_SM)
+ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaSetConsts* __restrict__ consts, int K,
+               double* __restrict__ partials, double* __restrict__ logpdf, unsigned int* counter,
+               double* __restrict__ nll_out, int32_t* __restrict__ status_out) {
+  extern __shared__ __align__(16) unsigned char ipa_smem[];
+  IpaSetConsts* sc = reinterpret_cast<IpaSetConsts*>(ipa_smem);
+  double* acc = reinterpret_cast<double*>(sc + K);
+  __shared__ int s_last;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int G = gridDim.x;
+  {
+    const int nd = K * (int)(sizeof(IpaSetConsts) / 8);
+    const double* src = reinterpret_cast<const double*>(consts);
+    double* dst = reinterpret_cast<double*>(sc);
+    for (int i = tid; i < nd; i += IPA_BLOCK) dst[i] = src[i];
+    for (int k = 0; k < K; ++k) acc[k * IPA_BLOCK + tid] = 0.0;
+  }
+  __syncthreads();
+  const long long ntiles = (n + IPA_TILE - 1) / IPA_TILE;
+  for (long long tile = blockIdx.x; tile < ntiles; tile += G) {
+    const long long base = tile * IPA_TILE;
+    double xv[IPA_E];
+    long long idx[IPA_E];
+    const bool full = base + IPA_TILE <= n;
+#pragma unroll
+    for (int p = 0; p < IPA_E / 2; ++p) {
+      idx[2 * p] = base + 2LL * (p * IPA_BLOCK + tid);
+      idx[2 * p + 1] = idx[2 * p] + 1;
+    }
+    if (full && vec_ok) {
+#pragma unroll
+      for (int p = 0; p < IPA_E / 2; ++p) {
+        const double2 v = __ldcs(reinterpret_cast<const double2*>(x + idx[2 * p]));
+        xv[2 * p] = v.x;
+        xv[2 * p + 1] = v.y;
+      }
+    } else {
+#pragma unroll
+      for (int e = 0; e < IPA_E; ++e) xv[e] = (idx[e] < n) ? x[idx[e]] : 0.0;
+    }
+    for (int k = 0; k < K; ++k) {
+      const IpaSetConsts& c = sc[k];
+      if (c.status) continue;
+      double l[IPA_E];
+      ipa_eval_set<IPA_E>(c, xv, l);
+      double s = 0.0;
+      if (full) {
+#pragma unroll
+        for (int e = 0; e < IPA_E; ++e) s += l[e];
+      } else {
+#pragma unroll
+        for (int e = 0; e < IPA_E; ++e) s += (idx[e] < n) ? l[e] : 0.0;
+      }
+      acc[k * IPA_BLOCK + tid] += s;
+      if (LOGPDF) {
+#pragma unroll
+        for (int e = 0; e < IPA_E; ++e)
+          if (idx[e] < n) logpdf[(long long)k * n + idx[e]] = l[e];
+      }
+    }
+  }
+  __syncthreads();
+  for (int k = warp; k < K; k += IPA_BLOCK / 32) {
+    const double* a = acc + k * IPA_BLOCK;
+    double v = (a[lane] + a[lane + 32]) + (a[lane + 64] + a[lane + 96]);
+    v = ipa_warp_sum(v);
+    if (lane == 0) partials[(long long)k * G + blockIdx.x] = v;
+  }
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) s_last = (atomicAdd(counter, 1u) == (unsigned)(G - 1));
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  for (int k = warp; k < K; k += IPA_BLOCK / 32) {
+    double v = 0.0;
+    for (int i = lane; i < G; i += 32) v += __ldcg(partials + (long long)k * G + i);
+    v = ipa_warp_sum(v);
+    if (lane == 0) {
+      const int st = sc[k].status;
+      nll_out[k] = st ? INFINITY : 0.0 - v;
+      if (status_out) status_out[k] = st;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Segmented NLL (T2): grid (T, IPA_SEGC); block (t, c) takes the c-th eighth of segment t with the
+// parameter set of that segment.
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(IPA_BLOCK, IPA_BLOCKS_PER_SM)
+ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ offsets,
+                   const IpaSetConsts* __restrict__ consts, double* __restrict__ partials) {
+  __shared__ IpaSetConsts c;
+  __shared__ double red[IPA_BLOCK / 32];
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const long long t = blockIdx.x;
+  {
+    const double* src = reinterpret_cast<const double*>(consts + t);
+    double* dst = reinterpret_cast<double*>(&c);
+    for (int i = tid; i < (int)(sizeof(IpaSetConsts) / 8); i += IPA_BLOCK) dst[i] = src[i];
+  }
+  __syncthreads();
+  const long long beg = offsets[t], len = offsets[t + 1] - beg;
+  const long long cb = beg + len * blockIdx.y / IPA_SEGC, ce = beg + len * (blockIdx.y + 1) / IPA_SEGC;
+  double acc = 0.0;
+  if (!c.status) {
+    for (long long base = cb; base < ce; base += IPA_TILE) {
+      double xv[IPA_E], l[IPA_E];
+      long long idx[IPA_E];
+#pragma unroll
+      for (int e = 0; e < IPA_E; ++e) {
+        idx[e] = base + e * IPA_BLOCK + tid;
+        xv[e] = (idx[e] < ce) ? __ldcs(x + idx[e]) : 0.0;
+      }
+      ipa_eval_set<IPA_E>(c, xv, l);
+      double s = 0.0;
+#pragma unroll
+      for (int e = 0; e < IPA_E; ++e) s += (idx[e] < ce) ? l[e] : 0.0;
+      acc += s;
+    }
+  }
+  acc = ipa_warp_sum(acc);
+  if (lane == 0) red[warp] = acc;
+  __syncthreads();
+  if (tid == 0) partials[t * IPA_SEGC + blockIdx.y] = (red[0] + red[1]) + (red[2] + red[3]);
+}
+
+__global__ void ipa_seg_finalize_kernel(const double* __restrict__ partials, const IpaSetConsts* __restrict__ consts,
+                                        long long T, double* __restrict__ nll, int32_t* __restrict__ status_out) {
+  const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (t >= T) return;
+  double v = 0.0;
+  for (int c = 0; c < IPA_SEGC; ++c) v += partials[t * IPA_SEGC + c];
+  const int st = consts[t].status;
+  nll[t] = st ? INFINITY : 0.0 - v;
+  if (status_out) status_out[t] = st;
+}
+
+// ------------------------------------------------------------------------------------------------
+// log I(d) from a constants record (generators, binned path)
+// ------------------------------------------------------------------------------------------------
+IPA_HD double ipa_logI_rec(const IpaSetConsts& c, double d) {
+  if (d < c.d0) return c.logG0 - c.n0 * log(fma(c.uA0, d, c.uB0));
+  if (d > c.d1) return c.logG1 - c.n1 * log(fma(c.uA1, d, c.uB1));
+  const double r = sqrt(fma(d, d, c.delta2));
+  double H;
+  if (c.mode == 0) {
+    const double t = fma(c.tA, r, c.tB);
+    double acc = c.a[c.degree];
+    for (int j = c.degree - 1; j >= 1; --j) acc = fma(acc, t, c.a[j]);
+    H = c.degree >= 1 ? fma(acc, t, c.araw0) : c.araw0;
+  } else {
+    H = ipa_direct_H(c.nu, c.alpha * r);
+  }
+  return H - c.nu * log(c.alpha) + c.beta * d;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Toy generation (T0, T1)
+// ------------------------------------------------------------------------------------------------
+__global__ void ipa_toy_yields_kernel(const unsigned long long* __restrict__ seeds, long long T, double mean_sig,
+                                      double mean_bkg, long long* __restrict__ nsig, long long* __restrict__ ntot) {
+  const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  if (t >= T) return;
+  const long long ns = ipa_poisson(seeds[t], 0ull, IPA_STREAM_YIELD, mean_sig);
+  const long long nb = ipa_poisson(seeds[t], 1ull, IPA_STREAM_YIELD, mean_bkg);
+  nsig[t] = ns;
+  ntot[t] = ns + nb;
+}
+
+// exclusive scan of ntot[T] into offsets[T+1], one block of 1024 threads, chunk by chunk
+__global__ void __launch_bounds__(1024)
+ipa_scan_kernel(const long long* __restrict__ ntot, long long T, long long* __restrict__ offsets, long long capacity,
+                int32_t* overflow) {
+  __shared__ long long buf[1024];
+  __shared__ long long carry;
+  const int tid = threadIdx.x;
+  if (tid == 0) carry = 0;
+  __syncthreads();
+  for (long long base = 0; base < T; base += 1024) {
+    const long long i = base + tid;
+    const long long v = (i < T) ? ntot[i] : 0;
+    buf[tid] = v;
+    __syncthreads();
+    for (int o = 1; o < 1024; o <<= 1) {
+      const long long add = (tid >= o) ? buf[tid - o] : 0;
+      __syncthreads();
+      buf[tid] += add;
+      __syncthreads();
+    }
+    if (i < T) offsets[i] = carry + buf[tid] - v;
+    __syncthreads();
+    if (tid == 1023) carry += buf[1023];
+    __syncthreads();
+  }
+  if (tid == 0) {
+    offsets[T] = carry;
+    if (overflow) *overflow = (carry > capacity) ? 1 : 0;
+  }
+}
+
+__device__ __forceinline__ double ipa_draw_background(double k, unsigned long long seed, unsigned long long slot,
+                                                      double lo, double hi) {
+  double u, v;
+  ipa_uniforms2(seed, slot, 0u, IPA_STREAM_BKG, &u, &v);
+  const double w = hi - lo, t = k * w;
+  if (fabs(t) < 1e-8) return lo + u * w;
+  return lo + log1p(u * expm1(t)) / k;
+}
+
+__device__ __forceinline__ double ipa_draw_signal(const IpaSetConsts& c, double logImax, unsigned long long seed,
+                                                  unsigned long long slot, double lo, double hi) {
+  double x = lo;
+  for (unsigned attempt = 0; attempt <= 100001u; ++attempt) {
+    double u1, u2;
+    ipa_uniforms2(seed, slot, attempt, IPA_STREAM_SIG, &u1, &u2);
+    x = lo + (hi - lo) * u1;
+    const double ratio = exp(ipa_logI_rec(c, x - c.mu) - logImax);
+    if (u2 * 1.02 < ratio) break;
+  }
+  return x;
+}
+
+// grid (T, chunks).  mixture != 0: T == 1, `capacity` events, component by u < f (configs 1-3).
+__global__ void __launch_bounds__(IPA_BLOCK)
+ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSetConsts* __restrict__ consts,
+                      int gen_stride,
+                      const long long* __restrict__ nsig, const long long* __restrict__ offsets, double lo, double hi,
+                      long long capacity, int mixture, double* __restrict__ x) {
+  __shared__ IpaSetConsts c;
+  __shared__ double red[IPA_BLOCK / 32];
+  __shared__ double s_logImax;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const long long t = blockIdx.x;
+  const long long g = gen_stride ? t : 0;
+  {
+    const double* src = reinterpret_cast<const double*>(consts + g);
+    double* dst = reinterpret_cast<double*>(&c);
+    for (int i = tid; i < (int)(sizeof(IpaSetConsts) / 8); i += IPA_BLOCK) dst[i] = src[i];
+  }
+  __syncthreads();
+  if (c.status) return;
+  // envelope: log of the maximum of I over the range (reading D13)
+  if (c.beta == 0.0 && lo <= c.mu && c.mu <= hi) {
+    if (tid == 0) s_logImax = ipa_logI_rec(c, 0.0);
+  } else {
+    double best = -INFINITY;
+    for (int j = tid; j < 4096; j += IPA_BLOCK) {
+      const double xx = lo + ((double)j + 0.5) * (hi - lo) / 4096.0;
+      best = fmax(best, ipa_logI_rec(c, xx - c.mu));
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) best = fmax(best, __shfl_xor_sync(IPA_FULL, best, o));
+    if (lane == 0) red[warp] = best;
+    __syncthreads();
+    if (tid == 0) s_logImax = fmax(fmax(red[0], red[1]), fmax(red[2], red[3]));
+  }
+  __syncthreads();
+  const double logImax = s_logImax;
+  const unsigned long long seed = seeds[t];
+  const double f = c.fsig, k = c.kraw;
+  const long long beg = mixture ? 0 : offsets[t];
+  const long long len = mixture ? capacity : offsets[t + 1] - beg;
+  const long long ns = mixture ? 0 : nsig[t];
+  for (long long j = (long long)blockIdx.y * IPA_BLOCK + tid; j < len; j += (long long)gridDim.y * IPA_BLOCK) {
+    if (beg + j >= capacity) break;
+    bool is_sig;
+    if (mixture) {
+      double uc, v;
+      ipa_uniforms2(seed, (unsigned long long)j, 0u, IPA_STREAM_COMP, &uc, &v);
+      is_sig = uc < f;
+    } else {
+      is_sig = j < ns;
+    }
+    x[beg + j] = is_sig ? ipa_draw_signal(c, logImax, seed, (unsigned long long)j, lo, hi)
+                        : ipa_draw_background(k, seed, (unsigned long long)j, lo, hi);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Histogram (B1): shared-memory privatised 32-bit counters, merged with 64-bit global atomics.
+// Integer work: exact and order-independent.
+// ------------------------------------------------------------------------------------------------
+#define IPA_HIST_SMEM_BINS 8192
+__global__ void __launch_bounds__(256)
+ipa_hist_kernel(const double* __restrict__ x, long long n, double lo, double hi, int nbins,
+                unsigned long long* __restrict__ counts) {
+  __shared__ unsigned int sh[IPA_HIST_SMEM_BINS];
+  const bool priv = nbins <= IPA_HIST_SMEM_BINS;
+  if (priv) {
+    for (int b = threadIdx.x; b < nbins; b += blockDim.x) sh[b] = 0u;
+    __syncthreads();
+  }
+  const double scale = (double)nbins / (hi - lo);
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  // a block handles at most 2^31 events between flushes (32-bit private counters): n / gridDim is far below that
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += stride) {
+    const double xi = __ldcs(x + i);
+    const double t = (xi - lo) * scale;
+    if (!(t >= 0.0) || !(xi <= hi)) continue;
+    int b = (int)t;
+    if (b >= nbins) b = nbins - 1;
+    if (priv) atomicAdd(&sh[b], 1u);
+    else atomicAdd(&counts[b], 1ull);
+  }
+  if (priv) {
+    __syncthreads();
+    for (int b = threadIdx.x; b < nbins; b += blockDim.x) {
+      const unsigned int v = sh[b];
+      if (v) atomicAdd(&counts[b], (unsigned long long)v);
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Binned path (B2): signal shape at bin centres, normalised to unit sum; scan kernel.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double ipa_block_sum_256(double v, double* red) {
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  v = ipa_warp_sum(v);
+  __syncthreads();
+  if (lane == 0) red[warp] = v;
+  __syncthreads();
+  double s = 0.0;
+#pragma unroll
+  for (int i = 0; i < 8; ++i) s += red[i];
+  return s;
+}
+
+// one block of 256 threads: sraw[b] = exp(logI(c_b - mu) - ref), then s[b] = sraw[b] / sum
+__global__ void __launch_bounds__(256)
+ipa_binned_shape_kernel(const IpaSetConsts* __restrict__ consts, double lo, double hi, int nbins,
+                        double* __restrict__ s_out, int32_t* __restrict__ shape_status) {
+  __shared__ IpaSetConsts c;
+  __shared__ double red[8];
+  {
+    const double* src = reinterpret_cast<const double*>(consts);
+    double* dst = reinterpret_cast<double*>(&c);
+    for (int i = threadIdx.x; i < (int)(sizeof(IpaSetConsts) / 8); i += 256) dst[i] = src[i];
+  }
+  __syncthreads();
+  if (threadIdx.x == 0) *shape_status = c.status;
+  if (c.status) {
+    for (int b = threadIdx.x; b < nbins; b += 256) s_out[b] = NAN;
+    return;
+  }
+  const double w = (hi - lo) / (double)nbins;
+  const double ref = ipa_logI_rec(c, fmin(fmax(0.0, lo - c.mu), hi - c.mu));
+  double part = 0.0;
+  for (int b = threadIdx.x; b < nbins; b += 256) {
+    const double cb = lo + ((double)b + 0.5) * w;
+    const double v = exp(ipa_logI_rec(c, cb - c.mu) - ref);
+    s_out[b] = v;
+    part += v;
+  }
+  const double tot = ipa_block_sum_256(part, red);
+  for (int b = threadIdx.x; b < nbins; b += 256) s_out[b] = s_out[b] / tot;
+}
+
+// one block per scan point q: nu_b = ns s_b + nb e^{k (c_b-lo)} / sum_b' e^{k (c_b'-lo)};
+// NLL = sum_b [nu_b - n_b log nu_b].  With nu_out != NULL (npoints == 1) the expected histogram is
+// written instead.
+__global__ void __launch_bounds__(256)
+ipa_binned_scan_kernel(const unsigned long long* __restrict__ counts, const double* __restrict__ s, int nbins,
+                       double lo, double hi, const double* __restrict__ ns, const double* __restrict__ nb,
+                       const double* __restrict__ kk, const int32_t* __restrict__ shape_status,
+                       double* __restrict__ nll, double* __restrict__ nu_out) {
+  __shared__ double red[8];
+  const long long q = blockIdx.x;
+  const double w = (hi - lo) / (double)nbins;
+  const double k = kk[q], vs = ns[q], vb = nb[q];
+  double part = 0.0;
+  for (int b = threadIdx.x; b < nbins; b += 256) part += exp(k * (((double)b + 0.5) * w));
+  const double bsum = ipa_block_sum_256(part, red);
+  double acc = 0.0;
+  for (int b = threadIdx.x; b < nbins; b += 256) {
+    const double v = vs * s[b] + vb * exp(k * (((double)b + 0.5) * w)) / bsum;
+    if (nu_out) nu_out[b] = v;
+    else {
+      const unsigned long long nobs = counts[b];
+      acc += nobs ? v - (double)nobs * log(v) : v;
+    }
+  }
+  if (nu_out) return;
+  const double tot = ipa_block_sum_256(acc, red);
+  if (threadIdx.x == 0) nll[q] = (*shape_status) ? INFINITY : tot;
+}
+
+// ------------------------------------------------------------------------------------------------
+// Per-bin Poisson toys (B3)
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+ipa_poisson_hist_kernel(const double* __restrict__ mean, int nbins, const unsigned long long* __restrict__ seeds,
+                        long long T, unsigned int* __restrict__ counts) {
+  const long long total = T * (long long)nbins;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += stride) {
+    const long long t = i / nbins;
+    const int b = (int)(i - t * nbins);
+    counts[i] = (unsigned int)ipa_poisson(seeds[t], (unsigned long long)b, IPA_STREAM_BIN, mean[b]);
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
+// FP64 peak probe: 8 independent DFMA chains per thread
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+ipa_fp64_probe_kernel(long long iters, double* out) {
+  double a0 = threadIdx.x * 1e-9, a1 = a0 + 1, a2 = a0 + 2, a3 = a0 + 3, a4 = a0 + 4, a5 = a0 + 5, a6 = a0 + 6, a7 = a0 + 7;
+  const double m = 0.999999999, c = 1e-9;
+  for (long long i = 0; i < iters; ++i) {
+    a0 = fma(a0, m, c); a1 = fma(a1, m, c); a2 = fma(a2, m, c); a3 = fma(a3, m, c);
+    a4 = fma(a4, m, c); a5 = fma(a5, m, c); a6 = fma(a6, m, c); a7 = fma(a7, m, c);
+  }
+  const double s = ((a0 + a1) + (a2 + a3)) + ((a4 + a5) + (a6 + a7));
+  if (s == 123.456) out[0] = s;  // never true: keeps the chains alive
+}

@@ -1,0 +1,396 @@
+// ipa_prologue.cuh -- per-parameter-set constants ("precomputed once per launch", north star):
+// steps A1a-A1e of DESIGN.md.  One thread block per parameter set runs the phases below with a
+// __syncthreads() between them; tests/devmath_host.cu runs the same phases serially on the CPU.
+//
+//   A1a  delta, alpha from K_lambda(zeta), K_{lambda+1}(zeta)                      (reading C1)
+//   A1b  joins d0, d1: log G and log-derivative L = beta - alpha (d/r) K_{nu-1}/K_nu (reading C1)
+//   A1e  core approximant: Chebyshev interpolation of  H(z) = log( z^nu K_nu(z) )  on
+//        z in [zeta, zmax] (the core region maps onto exactly this interval, whatever mu and sigma
+//        are), truncated at the fp64 noise floor and converted exactly (integer Chebyshev
+//        coefficients, double-double accumulation) to a monomial in t = tA r + tB for Horner.
+//   A1c  N_S: closed-form tails + 16-point Gauss-Legendre on panels [b, max(delta, 3b)] of the core
+//        (each panel keeps the branch points d = +-i delta outside a Bernstein ellipse of
+//        parameter >= 3.7, so 16 nodes give < 1e-18)                               (reading C5)
+//   A1d  N_B = expm1(k (hi-lo)) / k
+//   A1e  folded constants so that the per-event work is  Delta = E_S - E_B  and
+//        l = E_B + log(1 + e^Delta).
+#pragma once
+#include "ipa_math.cuh"
+#include "../../include/ipanll.h"
+
+#define IPA_NCOEF 48            // max polynomial degree 47
+#define IPA_MCHEB 64            // Chebyshev nodes of the core approximant
+#define IPA_JMAX 256            // trapezoid table length
+#define IPA_GL 16               // Gauss-Legendre nodes per panel
+#define IPA_MAXPANEL 24         // 12 per side
+#define IPA_PRO_THREADS 512
+#define IPA_SUB 4               // threads sharing one table-based Bessel evaluation
+#define IPA_NBTASK (IPA_MCHEB + 4)  // Chebyshev nodes + K_nu(z0), K_nu(z1), K_{nu-1}(z0), K_{nu-1}(z1)
+
+// What the streaming kernels read, per parameter set (all fp64 except the flags).
+struct IpaSetConsts {
+  double mu, d0, d1, delta2;
+  double tA, tB;                // t = tA r + tB in [-1,1] on the core
+  double bmk;                   // beta - kd
+  double kd, eB0;               // E_B = kd d + eB0      (kd = k; both 0 for f == 1)
+  double uA0, uB0, n0, cT0;     // left tail:  u = uA0 d + uB0,  Delta = cT0 - n0 log u - kd d
+  double uA1, uB1, n1, cT1;     // right tail
+  double alpha, nu, cDir;       // direct mode: Delta = H(alpha r) + bmk d + cDir, H(z) = log(z^nu K_nu(z))
+  double fsig, kraw;            // f and k as given (generators)
+  double beta, logG0, logG1, logNS, logref;  // for the generators / binned path: log I(d)
+  double normS, normB;          // N_S, N_B (absolute)
+  int32_t status, degree, mode, pure;
+  double a[IPA_NCOEF];          // Delta_core = sum_j a[j] t^j + bmk d   (a[0] carries the constants)
+  double araw0;                 // a[0] before folding: H(z) itself = sum araw t^j
+};
+
+struct IpaProWork {
+  ipa_params p;
+  double lo, hi;
+  int policy;
+  int status;
+  double nu, delta, alpha, d0, d1, r0, r1, z0, z1, zc, zh;
+  double part[2][32];
+  double Kl, Kl1;
+  double glx[IPA_GL], glw[IPA_GL];
+  // trapezoid table, orders |nu| (index 0) and |nu-1| (index 1)
+  double h;
+  int J;
+  double tc[IPA_JMAX], te[2][IPA_JMAX], tw[2][IPA_JMAX];
+  double bpart[IPA_NBTASK][IPA_SUB];
+  double Ks[IPA_NBTASK];        // scaled Bessel values e^z K(z) of the tasks
+  double H[IPA_MCHEB], c[IPA_MCHEB];
+  int degree, mode;
+  long long T[3][IPA_NCOEF];    // integer coefficients of T_{j-1}, T_j, T_{j+1}
+  double ahi[IPA_NCOEF], alo[IPA_NCOEF], araw[IPA_NCOEF];
+  double logG0, logG1, L0, L1;
+  int npanel;
+  double pa[IPA_MAXPANEL], pb[IPA_MAXPANEL], pval[IPA_MAXPANEL * IPA_GL], psum[IPA_MAXPANEL];
+  double logref, dl, dh;
+};
+
+IPA_HD bool ipa_finite(double v) { return fabs(v) <= 1.7976931348623157e308; }
+
+// ---- evaluation helpers shared by the prologue, the generators and the binned path ---------------
+IPA_HD double ipa_horner(const double* a, int D, double t) {
+  double acc = a[D];
+  for (int j = D - 1; j >= 0; --j) acc = fma(acc, t, a[j]);
+  return acc;
+}
+
+// table-based partial sum of e^z K(z): terms j = 1+sub, 1+sub+IPA_SUB, ... < J
+IPA_HD double ipa_table_partial(const IpaProWork& w, int ord, double z, int sub) {
+  double s = 0.0;
+  for (int j = 1 + sub; j < w.J; j += IPA_SUB) s += w.tw[ord][j] * exp(w.te[ord][j] - z * w.tc[j]);
+  return s;
+}
+
+// H(z) = log(z^nu K_nu(z)) from the raw polynomial, r given
+IPA_HD double ipa_core_H(const IpaProWork& w, double r) {
+  const double z = w.alpha * r;
+  if (w.mode == 0) return ipa_horner(w.araw, w.degree, (z - w.zc) / w.zh);
+  return w.nu * log(z) + log(ipa_besselk_scaled(w.nu, z)) - z;
+}
+// log G(d) = nu log r + beta d + log K_nu(alpha r) = H - nu log alpha + beta d
+IPA_HD double ipa_core_logG(const IpaProWork& w, double d) {
+  const double r = sqrt(fma(d, d, w.delta * w.delta));
+  return ipa_core_H(w, r) - w.nu * log(w.alpha) + w.p.beta * d;
+}
+IPA_HD double ipa_logI(const IpaProWork& w, double d) {
+  if (d < w.d0) return w.logG0 - w.p.n * log(1.0 - (d - w.d0) * w.L0 / w.p.n);
+  if (d > w.d1) return w.logG1 - w.p.n2 * log(1.0 - (d - w.d1) * w.L1 / w.p.n2);
+  return ipa_core_logG(w, d);
+}
+
+// ================================ phases =========================================================
+// phase 0: validation (one thread)
+IPA_HD void ipa_pro_phase0(IpaProWork& w, int tid) {
+  if (tid != 0) return;
+  const ipa_params& p = w.p;
+  const double* v = &p.mu;
+  bool ok = true;
+  for (int i = 0; i < 11; ++i) ok = ok && ipa_finite(v[i]);
+  ok = ok && (p.sigma > 0.0) && (p.zeta > 0.0) && (p.a > 0.0) && (p.a2 > 0.0) && (p.n > 0.0) && (p.n2 > 0.0) &&
+       (p.f >= 0.0) && (p.f <= 1.0);
+  w.status = ok ? 0 : 1;
+  w.nu = p.lambda - 0.5;
+  w.mode = 0;
+  w.degree = 0;
+  w.npanel = 0;
+}
+
+// phase 1: partial trapezoid sums of K_lambda(zeta) (warp 0) and K_{lambda+1}(zeta) (warp 1);
+// threads 64..79 compute the Gauss-Legendre rule.
+IPA_HD void ipa_pro_phase1(IpaProWork& w, int tid) {
+  if (w.status) return;
+  if (tid < 64) {
+    const int which = tid >> 5, lane = tid & 31;
+    const double ord = fabs(w.p.lambda + (double)which);
+    const double x = w.p.zeta;
+    const double h = ipa_trap_step(ord, x);
+    double s = 0.0, prev = 1.7976931348623157e308;
+    for (int j = 1 + lane; j < 8192; j += 32) {
+      const double term = ipa_trap_term(ord, x, h, j);
+      s += term;
+      if (term <= prev && term < 1e-19 * (s + 0.5)) break;
+      prev = term;
+    }
+    w.part[which][lane] = s;
+  } else if (tid < 64 + IPA_GL) {
+    ipa_gauss_legendre(IPA_GL, tid - 64, &w.glx[tid - 64], &w.glw[tid - 64]);
+  }
+}
+
+// phase 2: delta, alpha, joins, z-interval, trapezoid step and length (one thread)
+IPA_HD void ipa_pro_phase2(IpaProWork& w, int tid) {
+  if (w.status || tid != 0) return;
+  const ipa_params& p = w.p;
+  double s0 = 0.5, s1 = 0.5;
+  for (int l = 0; l < 32; ++l) { s0 += w.part[0][l]; s1 += w.part[1][l]; }
+  w.Kl = s0 * ipa_trap_step(fabs(p.lambda), p.zeta);
+  w.Kl1 = s1 * ipa_trap_step(fabs(p.lambda + 1.0), p.zeta);
+  const double q = p.zeta * w.Kl / w.Kl1;       // (delta/sigma)^2
+  w.delta = p.sigma * sqrt(q);
+  w.alpha = p.zeta / w.delta;                   // = sqrt(zeta K_{l+1}/K_l)/sigma, alpha delta = zeta
+  w.d0 = -p.a * p.sigma;
+  w.d1 = p.a2 * p.sigma;
+  w.r0 = sqrt(fma(w.d0, w.d0, w.delta * w.delta));
+  w.r1 = sqrt(fma(w.d1, w.d1, w.delta * w.delta));
+  w.z0 = w.alpha * w.r0;
+  w.z1 = w.alpha * w.r1;
+  const double zmin = p.zeta;
+  double zmax = fmax(w.z0, w.z1);
+  zmax = fmax(zmax, zmin * 1.001);
+  w.zc = 0.5 * (zmax + zmin);
+  w.zh = 0.5 * (zmax - zmin);
+  const double o0 = fabs(w.nu), o1 = fabs(w.nu - 1.0), om = fmax(o0, o1);
+  w.h = ipa_trap_step(om, zmax);
+  // table length: smallest t with zmin (cosh t - 1) - om t > 46, by fixed-point iteration
+  double t = 1.0;
+  for (int it = 0; it < 6; ++it) t = acosh(1.0 + (46.0 + om * t) / zmin);
+  int J = (int)(t / w.h) + 2;
+  if (J > IPA_JMAX) J = IPA_JMAX;
+  w.J = J;
+  if (!ipa_finite(w.delta) || !(w.delta > 0.0) || !ipa_finite(w.alpha)) w.status = 3;
+}
+
+// phase 3: trapezoid table (all threads)
+IPA_HD void ipa_pro_phase3(IpaProWork& w, int tid, int nthr) {
+  if (w.status) return;
+  for (int j = tid; j < w.J; j += nthr) {
+    const double t = (double)j * w.h;
+    const double s = sinh(0.5 * t);
+    w.tc[j] = 2.0 * s * s;
+    const double e0 = fabs(w.nu) * t, e1 = fabs(w.nu - 1.0) * t;
+    w.te[0][j] = e0;
+    w.te[1][j] = e1;
+    w.tw[0][j] = 0.5 * (1.0 + exp(-2.0 * e0));
+    w.tw[1][j] = 0.5 * (1.0 + exp(-2.0 * e1));
+  }
+}
+
+IPA_HD double ipa_pro_task_z(const IpaProWork& w, int q) {
+  if (q < IPA_MCHEB) return w.zc + w.zh * cos(3.14159265358979323846 * ((double)q + 0.5) / (double)IPA_MCHEB);
+  return ((q - IPA_MCHEB) & 1) ? w.z1 : w.z0;
+}
+
+// phase 4: Bessel tasks, IPA_SUB threads each
+IPA_HD void ipa_pro_phase4(IpaProWork& w, int tid) {
+  if (w.status) return;
+  const int q = tid / IPA_SUB, sub = tid % IPA_SUB;
+  if (q >= IPA_NBTASK) return;
+  const int ord = (q >= IPA_MCHEB + 2) ? 1 : 0;
+  w.bpart[q][sub] = ipa_table_partial(w, ord, ipa_pro_task_z(w, q), sub);
+}
+
+// phase 5: combine partial sums; H at the Chebyshev nodes
+IPA_HD void ipa_pro_phase5(IpaProWork& w, int tid) {
+  if (w.status || tid >= IPA_NBTASK) return;
+  double s = 0.5;
+  for (int i = 0; i < IPA_SUB; ++i) s += w.bpart[tid][i];
+  const double Ks = s * w.h;
+  w.Ks[tid] = Ks;
+  if (tid < IPA_MCHEB) {
+    const double z = ipa_pro_task_z(w, tid);
+    w.H[tid] = w.nu * log(z) + log(Ks) - z;
+  }
+}
+
+// phase 6: Chebyshev coefficients c_j = (2/M) sum_i H_i cos(pi j (i+1/2)/M), c_0 halved
+IPA_HD void ipa_pro_phase6(IpaProWork& w, int tid) {
+  if (w.status || tid >= IPA_MCHEB) return;
+  const int M = IPA_MCHEB;
+  double s = 0.0;
+  for (int i = 0; i < M; ++i) {
+    const int m = (tid * (2 * i + 1)) % (4 * M);  // angle = pi m / (2M)
+    s += w.H[i] * cos(3.14159265358979323846 * (double)m / (double)(2 * M));
+  }
+  w.c[tid] = s * (tid == 0 ? 1.0 : 2.0) / (double)M;
+}
+
+// phase 7: degree selection, joins (one thread)
+IPA_HD void ipa_pro_phase7(IpaProWork& w, int tid) {
+  if (w.status || tid != 0) return;
+  const ipa_params& p = w.p;
+  double scale = 1.0;
+  for (int i = 0; i < IPA_MCHEB; ++i) scale = fmax(scale, fabs(w.H[i]));
+  const double thr = 2.5e-16 * scale;
+  int D = IPA_MCHEB - 1;
+  while (D > 1 && fabs(w.c[D]) <= thr) --D;
+  // a-priori degree for a general order on this interval: the nearest singularity of H is z = 0
+  const double t0 = w.zc / w.zh;
+  const double rho = t0 + sqrt(t0 * t0 - 1.0);
+  int Dg = (int)ceil(37.0 / log(rho));
+  if (w.policy == 1 && D < Dg) D = Dg;
+  // conditioning of the power basis: needs rho comfortably above 1+sqrt(2)
+  if (D > IPA_NCOEF - 1 || rho < 2.6) { w.mode = 1; D = 0; }
+  w.degree = D;
+  const double K0 = w.Ks[IPA_MCHEB], K1 = w.Ks[IPA_MCHEB + 1], Km0 = w.Ks[IPA_MCHEB + 2], Km1 = w.Ks[IPA_MCHEB + 3];
+  w.logG0 = w.nu * log(w.r0) + p.beta * w.d0 + log(K0) - w.z0;
+  w.logG1 = w.nu * log(w.r1) + p.beta * w.d1 + log(K1) - w.z1;
+  w.L0 = p.beta - w.alpha * (w.d0 / w.r0) * (Km0 / K0);
+  w.L1 = p.beta - w.alpha * (w.d1 / w.r1) * (Km1 / K1);
+  if (!(w.L0 > 0.0) || !(w.L1 < 0.0)) w.status = 2;
+}
+
+// phase 8: Chebyshev -> monomial.  Step j (0..D): thread k holds the integer coefficient of t^k in
+// T_j and adds c_j T_{j,k} to a_k in double-double.  T_{j+1,k} = 2 T_{j,k-1} - T_{j-1,k} (exact in
+// int64 up to degree 47: |T_{47,k}| < 2^59).
+IPA_HD void ipa_pro_phase8_step(IpaProWork& w, int j, int k) {
+  if (w.status || w.mode || k >= IPA_NCOEF) return;
+  long long* Tm = w.T[(j + 2) % 3];  // T_{j-1}
+  long long* Tc = w.T[j % 3];        // T_j   (written in this step)
+  const long long* Tp = w.T[(j + 1) % 3];  // T_{j-2} ... see below
+  long long v;
+  if (j == 0) {
+    v = (k == 0) ? 1 : 0;
+    w.ahi[k] = 0.0;
+    w.alo[k] = 0.0;
+  } else if (j == 1) {
+    v = (k == 1) ? 1 : 0;
+  } else {
+    // T_j,k = 2 T_{j-1,k-1} - T_{j-2,k}
+    v = (k > 0 ? 2 * Tm[k - 1] : 0) - Tp[k];
+  }
+  Tc[k] = v;
+  if (v != 0 && j <= w.degree) {
+    double ph, pl, sh, sl;
+    ipa_two_prod(w.c[j], (double)v, &ph, &pl);
+    ipa_two_sum(w.ahi[k], ph, &sh, &sl);
+    sl += w.alo[k] + pl;
+    const double hi = sh + sl;
+    w.alo[k] = sl - (hi - sh);
+    w.ahi[k] = hi;
+  }
+}
+IPA_HD void ipa_pro_phase8_finish(IpaProWork& w, int k) {
+  if (w.status || w.mode || k >= IPA_NCOEF) return;
+  w.araw[k] = (k <= w.degree) ? w.ahi[k] + w.alo[k] : 0.0;
+}
+
+// phase 9: range, panels, reference level (one thread)
+IPA_HD void ipa_pro_phase9(IpaProWork& w, int tid) {
+  if (w.status || tid != 0) return;
+  w.dl = w.lo - w.p.mu;
+  w.dh = w.hi - w.p.mu;
+  const double dref = fmin(fmax(0.0, w.dl), w.dh);
+  w.logref = ipa_logI(w, dref);
+  const double A = fmax(w.dl, w.d0), B = fmin(w.dh, w.d1);
+  int np = 0;
+  if (B > A) {
+    for (int side = 0; side < 2; ++side) {
+      // side 0: d >= 0 part, side 1: d <= 0 part, both in |d| = [p, q]
+      double pp, qq;
+      if (side == 0) { if (B <= 0.0) continue; pp = fmax(A, 0.0); qq = B; }
+      else { if (A >= 0.0) continue; pp = fmax(-B, 0.0); qq = -A; }
+      double b = pp;
+      int cnt = 0;
+      while (b < qq) {
+        double nb = fmin(qq, fmax(w.delta, 3.0 * b));
+        if (++cnt == IPA_MAXPANEL / 2) nb = qq;
+        w.pa[np] = side == 0 ? b : -nb;
+        w.pb[np] = side == 0 ? nb : -b;
+        ++np;
+        b = nb;
+      }
+    }
+  }
+  w.npanel = np;
+}
+
+// phase 10: quadrature nodes (all threads)
+IPA_HD void ipa_pro_phase10(IpaProWork& w, int tid, int nthr) {
+  if (w.status) return;
+  for (int q = tid; q < w.npanel * IPA_GL; q += nthr) {
+    const int pnl = q / IPA_GL, i = q % IPA_GL;
+    const double c = 0.5 * (w.pa[pnl] + w.pb[pnl]), hl = 0.5 * (w.pb[pnl] - w.pa[pnl]);
+    w.pval[q] = w.glw[i] * hl * exp(ipa_core_logG(w, c + hl * w.glx[i]) - w.logref);
+  }
+}
+IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
+  if (w.status || tid >= w.npanel) return;
+  double s = 0.0;
+  for (int i = 0; i < IPA_GL; ++i) s += w.pval[tid * IPA_GL + i];
+  w.psum[tid] = s;
+}
+
+// phase 12: normalisations and folded constants (one thread writes the header of the record)
+IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
+  if (tid != 0) return;
+  o.status = w.status;
+  o.degree = w.degree;
+  o.mode = w.mode;
+  o.pure = 0;
+  o.normS = o.normB = NAN;
+  if (w.status) return;
+  const ipa_params& p = w.p;
+  double core = 0.0;
+  for (int i = 0; i < w.npanel; ++i) core += w.psum[i];
+  double left = 0.0, right = 0.0;
+  if (w.dl < w.d0) {
+    const double dr = fmin(w.d0, w.dh);
+    const double ul = 1.0 - (w.dl - w.d0) * w.L0 / p.n, ur = 1.0 - (dr - w.d0) * w.L0 / p.n;
+    left = exp(w.logG0 - w.logref) * (p.n / w.L0) * (ipa_powint(ul, p.n) - ipa_powint(ur, p.n));
+  }
+  if (w.dh > w.d1) {
+    const double dL = fmax(w.d1, w.dl);
+    const double uh = 1.0 - (w.dh - w.d1) * w.L1 / p.n2, ul = 1.0 - (dL - w.d1) * w.L1 / p.n2;
+    right = exp(w.logG1 - w.logref) * (p.n2 / (-w.L1)) * (ipa_powint(uh, p.n2) - ipa_powint(ul, p.n2));
+  }
+  const double NSr = left + core + right;  // in units of exp(logref)
+  const double wd = w.hi - w.lo, tk = p.k * wd;
+  const double NB = (fabs(tk) < 1e-8) ? wd * (1.0 + 0.5 * tk + tk * tk / 6.0) : expm1(tk) / p.k;
+  if (!(NSr > 0.0) || !ipa_finite(NSr) || !(NB > 0.0) || !ipa_finite(NB)) {
+    w.status = 3;
+    o.status = 3;
+    return;
+  }
+  o.normS = NSr * exp(w.logref);
+  o.normB = NB;
+  const double logNS = log(NSr) + w.logref;
+  const bool pure = !(p.f < 1.0);
+  const double cS = log(p.f) - logNS;  // -inf at f = 0
+  const double kd = pure ? 0.0 : p.k;
+  const double eB0 = pure ? 0.0 : (p.k * (p.mu - w.lo) + log1p(-p.f) - log(NB));
+  o.pure = pure ? 1 : 0;
+  o.mu = p.mu; o.d0 = w.d0; o.d1 = w.d1; o.delta2 = w.delta * w.delta;
+  o.tA = w.alpha / w.zh; o.tB = -w.zc / w.zh;
+  o.bmk = p.beta - kd; o.kd = kd; o.eB0 = eB0;
+  o.uA0 = -w.L0 / p.n;  o.uB0 = 1.0 + w.d0 * w.L0 / p.n;  o.n0 = p.n;  o.cT0 = w.logG0 + cS - eB0;
+  o.uA1 = -w.L1 / p.n2; o.uB1 = 1.0 + w.d1 * w.L1 / p.n2; o.n1 = p.n2; o.cT1 = w.logG1 + cS - eB0;
+  o.alpha = w.alpha; o.nu = w.nu;
+  o.cDir = cS - eB0 - w.nu * log(w.alpha);
+  o.fsig = p.f; o.kraw = p.k;
+  o.beta = p.beta; o.logG0 = w.logG0; o.logG1 = w.logG1; o.logNS = logNS; o.logref = w.logref;
+  o.araw0 = w.mode ? 0.0 : w.araw[0];
+}
+// phase 13: coefficients (threads 0..47), after phase 12
+IPA_HD void ipa_pro_phase13(IpaProWork& w, IpaSetConsts& o, int k) {
+  if (k >= IPA_NCOEF) return;
+  double v = 0.0;
+  if (!w.status && !w.mode) {
+    v = w.araw[k];
+    if (k == 0) v += o.cDir;  // cS - eB0 - nu log alpha
+  }
+  o.a[k] = v;
+}

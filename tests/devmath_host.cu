@@ -1,0 +1,67 @@
+// Test helper (tests/test_devmath_host.py): compiles the CUDA path's __host__ __device__ arithmetic
+// (paper_1706_01420_b200/csrc/*.cuh) for the CPU and runs the prologue phases serially, so that the
+// kernel math can be checked against the oracle on the GPU-less build box.  TEST ONLY: the product
+// library never executes these functions on the host and nothing in the package links this file.
+#include <cstring>
+#include <vector>
+#include "../paper_1706_01420_b200/csrc/ipa_kernels.cuh"
+
+static void run_prologue_host(const ipa_params& p, double lo, double hi, int policy, IpaSetConsts* out) {
+  static IpaProWork w;
+  std::memset(&w, 0, sizeof(w));
+  std::memset(out, 0, sizeof(*out));
+  w.p = p; w.lo = lo; w.hi = hi; w.policy = policy;
+  const int NT = IPA_PRO_THREADS;
+#define ALL(stmt) for (int tid = 0; tid < NT; ++tid) { stmt; }
+  ALL(ipa_pro_phase0(w, tid))
+  ALL(ipa_pro_phase1(w, tid))
+  ALL(ipa_pro_phase2(w, tid))
+  ALL(ipa_pro_phase3(w, tid, NT))
+  ALL(ipa_pro_phase4(w, tid))
+  ALL(ipa_pro_phase5(w, tid))
+  ALL(ipa_pro_phase6(w, tid))
+  ALL(ipa_pro_phase7(w, tid))
+  if (!w.status && !w.mode)
+    for (int j = 0; j <= w.degree; ++j) { ALL(ipa_pro_phase8_step(w, j, tid)) }
+  ALL(ipa_pro_phase8_finish(w, tid))
+  ALL(ipa_pro_phase9(w, tid))
+  ALL(ipa_pro_phase10(w, tid, NT))
+  ALL(ipa_pro_phase11(w, tid))
+  ALL(ipa_pro_phase12(w, *out, tid))
+  ALL(ipa_pro_phase13(w, *out, tid))
+#undef ALL
+}
+
+extern "C" {
+int emu_sizeof_consts() { return (int)sizeof(IpaSetConsts); }
+double emu_besselk_scaled(double nu, double x) { return ipa_besselk_scaled(nu, x); }
+// out: status, degree, mode, normS, normB, delta2, alpha, logG0, logG1, L0 (= -uA0 n0), L1
+void emu_consts(const ipa_params* p, double lo, double hi, int policy, double* out) {
+  IpaSetConsts c;
+  run_prologue_host(*p, lo, hi, policy, &c);
+  out[0] = c.status; out[1] = c.degree; out[2] = c.mode; out[3] = c.normS; out[4] = c.normB;
+  out[5] = c.delta2; out[6] = c.alpha; out[7] = c.logG0; out[8] = c.logG1; out[9] = -c.uA0 * c.n0; out[10] = -c.uA1 * c.n1;
+}
+void emu_logpdf(const ipa_params* p, double lo, double hi, int policy, const double* x, long long n, double* out) {
+  IpaSetConsts c;
+  run_prologue_host(*p, lo, hi, policy, &c);
+  for (long long i = 0; i < n; i += 8) {
+    double xv[8], l[8];
+    for (int e = 0; e < 8; ++e) xv[e] = (i + e < n) ? x[i + e] : x[n - 1];
+    if (c.status) { for (int e = 0; e < 8; ++e) l[e] = -INFINITY; }
+    else ipa_eval_set<8>(c, xv, l);
+    for (int e = 0; e < 8 && i + e < n; ++e) out[i + e] = l[e];
+  }
+}
+void emu_logI(const ipa_params* p, double lo, double hi, const double* d, long long n, double* out) {
+  IpaSetConsts c;
+  run_prologue_host(*p, lo, hi, 0, &c);
+  for (long long i = 0; i < n; ++i) out[i] = ipa_logI_rec(c, d[i]);
+}
+void emu_uniforms2(unsigned long long seed, unsigned long long slot, unsigned attempt, unsigned stream, double* u) {
+  ipa_uniforms2(seed, slot, attempt, stream, u, u + 1);
+}
+long long emu_poisson(unsigned long long seed, unsigned long long slot, unsigned stream, double mean) {
+  return ipa_poisson(seed, slot, stream, mean);
+}
+}

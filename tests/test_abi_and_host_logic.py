@@ -1,0 +1,145 @@
+"""CPU-side checks of the CUDA library: it builds, loads and exports every symbol include/ipanll.h
+declares; argument validation works without a GPU; compute calls fail loudly without one; and the
+kernels' __host__ __device__ arithmetic, compiled for the CPU by tests/devmath_host.cu, agrees with
+the oracle (the same source runs on the GPU in the `-m gpu` tests)."""
+import ctypes as C
+import os
+import re
+import subprocess
+
+import numpy as np
+import pytest
+
+import ipa_inputs as inp
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+LO, HI = inp.LO, inp.HI
+
+
+@pytest.fixture(scope="module")
+def ipa():
+    import paper_1706_01420_b200 as m
+    m.lib()
+    return m
+
+
+def test_library_exports_every_declared_symbol(ipa):
+    hdr = open(os.path.join(ROOT, "include", "ipanll.h")).read()
+    declared = set(re.findall(r"\b(ipa_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(ipa.EXPORTS), declared ^ set(ipa.EXPORTS)
+    L = ipa.lib()
+    for name in declared:
+        assert hasattr(L, name), name
+    out = subprocess.check_output(["nm", "-D", "--defined-only", ipa.library_path()], text=True)
+    for name in declared:
+        assert re.search(r"\bT %s\b" % name, out), name
+    # the product library must not link the oracle nor contain its symbols
+    assert "orc_" not in out
+    assert ipa.ipa_version().startswith("ipanll")
+
+
+def test_sm100a_image_present(ipa):
+    out = subprocess.check_output(["cuobjdump", "-lelf", ipa.library_path()], text=True)
+    assert "sm_100a" in out
+
+
+def test_argument_validation_without_gpu(ipa):
+    L = ipa.lib()
+    P = ipa.pack_params(inp.GEN)
+    rng = ipa.binding._Range(LO, HI)
+    bad = ipa.binding._Range(HI, LO)
+    one = C.c_void_p(256)  # non-null dummy; never dereferenced because validation fails first
+    p = P.ctypes.data_as(C.c_void_p)
+    assert L.ipa_nll_eval(one, -1, p, 1, rng, one, None, None, one, 1 << 30, None) == -1
+    assert L.ipa_nll_eval(one, 10, p, 0, rng, one, None, None, one, 1 << 30, None) == -1
+    assert L.ipa_nll_eval(one, 10, p, 33, rng, one, None, None, one, 1 << 30, None) == -1
+    assert L.ipa_nll_eval(one, 10, p, 1, bad, one, None, None, one, 1 << 30, None) == -1
+    assert L.ipa_nll_eval(None, 10, p, 1, rng, one, None, None, one, 1 << 30, None) == -1
+    assert L.ipa_nll_eval(C.c_void_p(260), 10, p, 1, rng, one, None, None, one, 1 << 30, None) == -1
+    assert L.ipa_nll_eval(one, 10, p, 1, rng, one, None, None, one, 16, None) == -2
+    assert L.ipa_nll_eval(one, 10, p, 1, rng, one, None, None, C.c_void_p(264), 1 << 30, None) == -2
+    assert L.ipa_norm(None, 1, rng, one, one, None, one, 1 << 30, None) == -1
+    assert L.ipa_hist_fill(one, 5, rng, 0, one, None) == -1
+    assert L.ipa_strerror(-2).decode().startswith("workspace")
+    assert ipa.ipa_workspace_bytes(10 ** 8, 9) >= 9 * 600
+    assert ipa.ipa_workspace_bytes(10 ** 8, 1000) > ipa.ipa_workspace_bytes(10 ** 8, 9)
+    assert ipa.ipa_set_degree_policy(1) == 0 and ipa.ipa_set_degree_policy(0) == 1
+
+
+def test_compute_fails_loudly_without_gpu(ipa):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    with pytest.raises(ipa.IpaError):
+        ipa.ipa_norm(inp.GEN, LO, HI)
+    with pytest.raises(ipa.IpaError):
+        ipa.ipa_nll_eval(torch.zeros(4, dtype=torch.float64), inp.GEN, LO, HI)
+
+
+# ---- the kernels' arithmetic, compiled for the host ------------------------------------------------
+@pytest.fixture(scope="module")
+def emu(tmp_path_factory):
+    out = str(tmp_path_factory.mktemp("emu") / "libdevmath_host.so")
+    subprocess.check_call(["nvcc", "-arch=sm_100a", "-O2", "-std=c++17", "-Xcompiler", "-fPIC", "-shared",
+                           "-I", os.path.join(ROOT, "include"), "-o", out, os.path.join(ROOT, "tests", "devmath_host.cu")])
+    L = C.CDLL(out)
+    d, vp, ll = C.c_double, C.c_void_p, C.c_longlong
+    L.emu_besselk_scaled.restype = d; L.emu_besselk_scaled.argtypes = [d, d]
+    L.emu_consts.argtypes = [vp, d, d, C.c_int, vp]
+    L.emu_logpdf.argtypes = [vp, d, d, C.c_int, vp, ll, vp]
+    L.emu_logI.argtypes = [vp, d, d, vp, ll, vp]
+    L.emu_uniforms2.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, vp]
+    L.emu_poisson.restype = ll; L.emu_poisson.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, d]
+    return L
+
+
+def test_device_bessel_vs_mpmath(emu):
+    import mpmath as mp
+    mp.mp.dps = 30
+    worst = 0.0
+    for nu in (0.0, 0.3, 0.5, 1.0, 1.8, 2.5, -1.3, 5.0):
+        for x in (1e-3, 0.01, 0.1, 0.5, 1.0, 2.0, 3.43, 10.0, 50.0, 300.0, 700.0):
+            ref = mp.besselk(nu, x) * mp.exp(x)
+            worst = max(worst, float(abs((mp.mpf(emu.emu_besselk_scaled(nu, x)) - ref) / ref)))
+    assert worst <= 3e-15
+
+
+@pytest.mark.parametrize("policy", [0, 1])
+@pytest.mark.parametrize("shape", ["P1", "P2", "direct"])
+def test_device_math_vs_oracle(emu, orc, shape, policy):
+    P = {"P1": inp.GEN, "P2": inp.P2, "direct": dict(inp.GEN, zeta=0.2)}[shape]
+    p = inp.as_array(P)
+    out = np.zeros(11)
+    emu.emu_consts(p.ctypes.data, LO, HI, policy, out.ctypes.data)
+    st, sc = orc.shape_consts(P)
+    _, nm = orc.norm(P, LO, HI)
+    assert out[0] == 0 and st == 0
+    assert out[2] == (1 if shape == "direct" else 0)
+    if shape == "P1":
+        assert out[1] == (1 if policy == 0 else 31)   # K_{1/2}: H(z) is linear in z
+    assert abs(out[3] / nm["NS"] - 1) <= 5e-14 and abs(out[4] / nm["NB"] - 1) <= 1e-15
+    assert abs(np.sqrt(out[5]) / sc["delta"] - 1) <= 1e-14 and abs(out[6] / sc["alpha"] - 1) <= 1e-14
+    assert abs(out[7] - sc["logG0"]) <= 1e-13 and abs(out[9] / sc["L0"] - 1) <= 1e-13 and abs(out[10] / sc["L1"] - 1) <= 1e-13
+    n = 4000 if shape != "direct" else 400
+    x = inp.standin_masses(1, n)
+    x[:5] = [LO, HI, 5280.0, 5250.0, 5310.0]
+    got = np.empty_like(x)
+    emu.emu_logpdf(p.ctypes.data, LO, HI, policy, x.ctypes.data, x.size, got.ctypes.data)
+    assert np.abs(got - orc.logpdf(x, P, LO, HI)).max() <= 2e-14
+    d = np.linspace(-300.0, 330.0, 501)
+    gi = np.empty_like(d)
+    emu.emu_logI(p.ctypes.data, LO, HI, d.ctypes.data, d.size, gi.ctypes.data)
+    assert np.abs(gi - np.array([orc.log_I(P, v) for v in d])).max() <= 5e-14
+
+
+def test_device_generators_vs_oracle(emu, orc):
+    rng = np.random.Generator(np.random.Philox(3))
+    for _ in range(200):
+        seed, slot = int(rng.integers(0, 2 ** 63)), int(rng.integers(0, 2 ** 40))
+        att, stream = int(rng.integers(0, 1000)), int(rng.integers(0, 5))
+        u = np.empty(2)
+        emu.emu_uniforms2(seed, slot, att, stream, u.ctypes.data)
+        assert np.array_equal(u, orc.uniforms2(seed, slot, att, stream))
+    for mean in (0.5, 5.0, 9.99, 10.0, 50.0, 3.0e4, 7.0e4, 1.0e5):
+        for slot in range(300):
+            assert emu.emu_poisson(1234, slot, 3, mean) == orc.poisson(1234, slot, 3, mean)

@@ -1,0 +1,299 @@
+"""GPU parity: the CUDA path (through the C ABI of include/ipanll.h) against the CPU oracle on the
+same seeded inputs.  Tolerances are BASELINE.json's: per-event log-pdf 1e-10 absolute, total NLL
+1e-10 relative, finite-difference gradient 1e-7 relative (reading D18), integer work bit-exact.
+"""
+import numpy as np
+import pytest
+
+import ipa_inputs as inp
+
+pytestmark = pytest.mark.gpu
+
+LO, HI = inp.LO, inp.HI
+
+
+@pytest.fixture(scope="module")
+def ipa():
+    import torch
+    assert torch.cuda.is_available(), "GPU tests need a CUDA device"
+    import paper_1706_01420_b200 as m
+    m.lib()
+    return m
+
+
+@pytest.fixture(scope="module")
+def torch_():
+    import torch
+    return torch
+
+
+def dev(torch, a):
+    return torch.from_numpy(np.ascontiguousarray(a)).cuda()
+
+
+def grad_ok(g_gpu, g_orc):
+    s = np.array([inp.GRAD_SCALE[name] for name in inp.FLOATED])
+    return np.all(np.abs(g_gpu - g_orc) <= 1e-7 * np.maximum(np.abs(g_orc), 1.0 / s))
+
+
+@pytest.fixture(scope="module")
+def x1(orc):
+    """config 1: 10,000 events, seed 1, from the oracle's generator"""
+    return orc.generate_mixture(1, 10000, inp.GEN, LO, HI)
+
+
+@pytest.mark.parametrize("shape", ["P1", "P2"])
+@pytest.mark.parametrize("policy", [0, 1])
+def test_config1_logpdf_nll_gradient(ipa, torch_, orc, x1, shape, policy):
+    theta = inp.GEN if shape == "P1" else inp.P2
+    batch, h = inp.fd_batch(theta)
+    old = ipa.ipa_set_degree_policy(policy)
+    try:
+        nll, lp, st = ipa.ipa_nll_eval(dev(torch_, x1), batch, LO, HI, want_logpdf=True)
+        torch_.cuda.synchronize()
+    finally:
+        ipa.ipa_set_degree_policy(old)
+    nll, lp, st = nll.cpu().numpy(), lp.cpu().numpy(), st.cpu().numpy()
+    assert (st == 0).all()
+    ref = orc.nll(x1, batch, LO, HI)
+    for k in range(batch.shape[0]):
+        ref_lp = orc.logpdf(x1, batch[k], LO, HI)
+        assert np.abs(lp[k] - ref_lp).max() <= 1e-10
+    assert np.all(np.abs(nll - ref) <= 1e-10 * np.abs(ref))
+    assert grad_ok(inp.fd_gradient(nll, h), inp.fd_gradient(ref, h))
+
+
+def test_batch_independence_and_determinism(ipa, torch_, x1):
+    batch, _ = inp.fd_batch(inp.GEN)
+    xd = dev(torch_, x1)
+    a, _, _ = ipa.ipa_nll_eval(xd, batch, LO, HI)
+    b, _, _ = ipa.ipa_nll_eval(xd, batch, LO, HI)
+    singles = [ipa.ipa_nll_eval(xd, batch[k], LO, HI)[0] for k in range(batch.shape[0])]
+    perm = np.arange(batch.shape[0])[::-1].copy()
+    c, _, _ = ipa.ipa_nll_eval(xd, batch[perm], LO, HI)
+    torch_.cuda.synchronize()
+    a, b, c = a.cpu().numpy(), b.cpu().numpy(), c.cpu().numpy()
+    assert np.array_equal(a, b)  # run-to-run bitwise
+    assert np.array_equal(a, np.array([s.item() for s in singles]))  # set k does not depend on its batch
+    assert np.array_equal(a[perm], c)
+
+
+@pytest.mark.parametrize("n", [0, 1, 2, 31, 1023, 1024, 1025, 4099])
+def test_ragged_sizes_and_misalignment(ipa, torch_, orc, x1, n):
+    big = dev(torch_, x1)
+    for off in (0, 1):  # off=1: 8-byte but not 16-byte aligned -> scalar-load path
+        xd = big[off:off + n]
+        nll, lp, _ = ipa.ipa_nll_eval(xd, [inp.GEN, inp.P2], LO, HI, want_logpdf=True)
+        torch_.cuda.synchronize()
+        ref = orc.nll(x1[off:off + n], [inp.GEN, inp.P2], LO, HI)
+        got = nll.cpu().numpy()
+        if n == 0:
+            assert np.array_equal(got, [0.0, 0.0]) and not np.signbit(got).any()
+        else:
+            assert np.all(np.abs(got - ref) <= 1e-10 * np.abs(ref))
+            assert np.abs(lp[0].cpu().numpy() - orc.logpdf(x1[off:off + n], inp.GEN, LO, HI)).max() <= 1e-10
+
+
+def test_norm(ipa, torch_, orc):
+    sets = [dict(inp.GEN), dict(inp.P2)]
+    sets.append(dict(inp.GEN, k=0.0))
+    sets.append(dict(inp.GEN, n=1.0, n2=1.0))
+    sets.append(dict(inp.GEN, mu=4900.0))           # range entirely inside the right tail
+    sets.append(dict(inp.GEN, mu=5590.0, a2=0.5))   # right join inside, range cuts the core
+    sets.append(dict(inp.P2, zeta=8.0, **{"lambda": 2.2}))
+    sets.append(dict(inp.GEN, zeta=40.0))
+    ns, nb, st = ipa.ipa_norm(sets, LO, HI)
+    torch_.cuda.synchronize()
+    ns, nb, st = ns.cpu().numpy(), nb.cpu().numpy(), st.cpu().numpy()
+    for i, p in enumerate(sets):
+        ost, o = orc.norm(p, LO, HI)
+        assert st[i] == ost == 0
+        assert abs(ns[i] / o["NS"] - 1) <= 2e-13, (i, ns[i], o["NS"])
+        assert abs(nb[i] / o["NB"] - 1) <= 1e-14
+
+
+def test_domain_status_does_not_poison_batch(ipa, torch_, orc, x1):
+    bad = [dict(inp.GEN, sigma=-1.0), dict(inp.GEN, f=1.5), dict(inp.GEN, zeta=0.0), dict(inp.GEN, mu=float("nan")),
+           dict(inp.GEN, beta=5.0)]  # beta=5: slope at the right join is positive -> status 2
+    batch = [inp.GEN] + bad + [inp.P2]
+    nll, _, st = ipa.ipa_nll_eval(dev(torch_, x1), batch, LO, HI)
+    torch_.cuda.synchronize()
+    nll, st = nll.cpu().numpy(), st.cpu().numpy()
+    assert list(st) == [0, 1, 1, 1, 1, 2, 0]
+    assert np.isposinf(nll[1:6]).all()
+    ref = orc.nll(x1, [inp.GEN, inp.P2], LO, HI)
+    assert np.all(np.abs(nll[[0, 6]] - ref) <= 1e-10 * np.abs(ref))
+    assert orc.shape_consts(bad[4])[0] == 2
+
+
+def test_limits_f0_f1_k0_outside_and_nan(ipa, torch_, orc, x1):
+    x = x1[:3000].copy()
+    x[:4] = [4990.0, 5610.0, LO, HI]  # events outside the range: same formulae, no clipping
+    sets = [dict(inp.GEN, f=0.0), dict(inp.GEN, f=1.0), dict(inp.GEN, k=0.0), dict(inp.P2, f=1.0)]
+    nll, lp, st = ipa.ipa_nll_eval(dev(torch_, x), sets, LO, HI, want_logpdf=True)
+    torch_.cuda.synchronize()
+    assert (st.cpu().numpy() == 0).all()
+    for i, p in enumerate(sets):
+        assert np.abs(lp[i].cpu().numpy() - orc.logpdf(x, p, LO, HI)).max() <= 1e-10
+    ref = orc.nll(x, sets, LO, HI)
+    assert np.all(np.abs(nll.cpu().numpy() - ref) <= 1e-10 * np.abs(ref))
+    x[7] = float("nan")
+    nll, _, _ = ipa.ipa_nll_eval(dev(torch_, x), inp.GEN, LO, HI)
+    assert np.isnan(nll.cpu().numpy()[0])
+
+
+def test_direct_mode_shapes(ipa, torch_, orc, x1):
+    """Shapes whose core interval is too wide for one polynomial run the per-event Bessel path."""
+    x = x1[:2000]
+    sets = [dict(inp.GEN, zeta=0.2), dict(inp.GEN, zeta=0.05, **{"lambda": -2.0}), dict(inp.GEN, a=6.0, a2=7.0)]
+    nll, lp, st = ipa.ipa_nll_eval(dev(torch_, x), sets, LO, HI, want_logpdf=True)
+    torch_.cuda.synchronize()
+    assert (st.cpu().numpy() == 0).all()
+    for i, p in enumerate(sets):
+        assert np.abs(lp[i].cpu().numpy() - orc.logpdf(x, p, LO, HI)).max() <= 1e-10, i
+    ref = orc.nll(x, sets, LO, HI)
+    assert np.all(np.abs(nll.cpu().numpy() - ref) <= 1e-10 * np.abs(ref))
+
+
+def test_hypothesis_like_sweep(ipa, torch_, orc, x1):
+    """Random valid shapes over the domain (seeded): per-event parity and normalisation."""
+    rng = np.random.Generator(np.random.Philox(77))
+    x = x1[:1500]
+    sets = []
+    for _ in range(24):
+        sets.append(dict(mu=5280 + rng.uniform(-60, 60), sigma=rng.uniform(5, 40), **{"lambda": rng.uniform(-3, 3)},
+                         zeta=10 ** rng.uniform(-0.3, 1.5), beta=rng.uniform(-0.01, 0.01), a=rng.uniform(0.8, 3.5),
+                         n=rng.uniform(1.0, 6.0), a2=rng.uniform(0.8, 3.5), n2=rng.uniform(1.0, 6.0),
+                         f=rng.uniform(0.05, 0.95), k=rng.uniform(-0.004, 0.001)))
+    nll, lp, st = ipa.ipa_nll_eval(dev(torch_, x), sets, LO, HI, want_logpdf=True)
+    torch_.cuda.synchronize()
+    st = st.cpu().numpy()
+    for i, p in enumerate(sets):
+        ost, _ = orc.shape_consts(p)
+        assert st[i] == ost
+        if ost == 0:
+            assert np.abs(lp[i].cpu().numpy() - orc.logpdf(x, p, LO, HI)).max() <= 1e-10, (i, p)
+
+
+# ---------------------------------------------------------------------------------------------
+# generators (T0, T1), segmented NLL (T2)
+# ---------------------------------------------------------------------------------------------
+def test_mixture_generator_matches_oracle(ipa, torch_, orc):
+    n = 20000
+    for theta, seed in ((inp.GEN, 1), (inp.P2, 9)):
+        x, off, ovf = ipa.ipa_toy_generate([seed], theta, -1.0, -1.0, LO, HI, n)
+        torch_.cuda.synchronize()
+        ref = orc.generate_mixture(seed, n, theta, LO, HI)
+        got = x.cpu().numpy()
+        assert list(off.cpu().numpy()) == [0, n] and ovf.item() == 0
+        close = np.abs(got - ref) <= 1e-9
+        assert close.mean() >= 1 - 1e-4          # an accept/reject flip needs |u - ratio| < 1e-15
+        assert ((got >= LO) & (got <= HI)).all()
+
+
+def test_toy_generator_and_segmented_nll(ipa, torch_, orc):
+    T = 24
+    seeds = inp.toy_seeds(T)
+    ms, mb = 300.0, 700.0
+    _, off_ref = orc.toy_generate(seeds, inp.GEN, ms, mb, LO, HI, offsets_only=True)
+    cap = int(off_ref[-1])
+    x, off, ovf = ipa.ipa_toy_generate(seeds, inp.GEN, ms, mb, LO, HI, cap)
+    torch_.cuda.synchronize()
+    assert np.array_equal(off.cpu().numpy(), off_ref) and ovf.item() == 0   # Poisson yields: bit-exact
+    x_ref, _ = orc.toy_generate(seeds, inp.GEN, ms, mb, LO, HI)
+    got = x.cpu().numpy()
+    assert (np.abs(got - x_ref) <= 1e-9).mean() >= 1 - 1e-4
+    # per-toy parameter sets (reading D17), NLL of every toy in one launch, on the GPU-generated events
+    sets = inp.toy_param_sets(T)
+    nll, st = ipa.ipa_nll_eval_segmented(x, off, sets, LO, HI)
+    torch_.cuda.synchronize()
+    ref = orc.nll_segmented(got, off_ref, sets, LO, HI)
+    assert (st.cpu().numpy() == 0).all()
+    assert np.all(np.abs(nll.cpu().numpy() - ref) <= 1e-10 * np.abs(ref))
+    # capacity too small: offsets still written, overflow flagged, nothing written past capacity
+    x2, off2, ovf2 = ipa.ipa_toy_generate(seeds, inp.GEN, ms, mb, LO, HI, cap - 100)
+    torch_.cuda.synchronize()
+    assert ovf2.item() == 1 and np.array_equal(off2.cpu().numpy(), off_ref)
+
+
+def test_segmented_many_sets_and_empty_segments(ipa, torch_, orc, x1):
+    """T > IPA_MAX_K (parameter sets travel through the workspace) with empty and tiny segments."""
+    T = 70
+    rng = np.random.Generator(np.random.Philox(5))
+    cuts = np.sort(rng.integers(0, x1.size, size=T - 1))
+    off = np.concatenate([[0], cuts, [x1.size]]).astype(np.int64)
+    off[10] = off[9]  # force an empty segment
+    off = np.maximum.accumulate(off)
+    sets = inp.toy_param_sets(T, seed=11)
+    nll, st = ipa.ipa_nll_eval_segmented(dev(torch_, x1), dev(torch_, off), sets, LO, HI)
+    torch_.cuda.synchronize()
+    ref = orc.nll_segmented(x1, off, sets, LO, HI)
+    got = nll.cpu().numpy()
+    assert np.all(np.abs(got - ref) <= 1e-10 * np.abs(ref) + 0.0)
+    assert got[9] == 0.0 or off[10] != off[9]
+
+
+# ---------------------------------------------------------------------------------------------
+# binned path (B1-B3)
+# ---------------------------------------------------------------------------------------------
+def test_hist_fill_exact(ipa, torch_, orc, x1):
+    x = np.concatenate([x1, [LO, HI, LO - 1e-9, HI + 1e-9, np.nextafter(HI, 0)]])
+    for nbins in (1, 7, 1000, 10000):
+        c = ipa.ipa_hist_fill(dev(torch_, x), LO, HI, nbins)
+        torch_.cuda.synchronize()
+        assert np.array_equal(c.cpu().numpy().astype(np.uint64), orc.hist_fill(x, LO, HI, nbins))
+
+
+def test_binned_scan_expected_hist_and_poisson_toys(ipa, torch_, orc):
+    nbins = 1000
+    x = inp.standin_masses(5, 200000, f=0.02)
+    counts = orc.hist_fill(x, LO, HI, nbins)
+    ns, nb, kk = inp.scan_grid(12, 9, n_obs=float(x.size))
+    cd = dev(torch_, counts.astype(np.int64))
+    got = ipa.ipa_binned_nll_scan(cd, LO, HI, inp.GEN, ns, nb, kk)
+    torch_.cuda.synchronize()
+    ref = orc.binned_nll_scan(counts, LO, HI, inp.GEN, ns, nb, kk)
+    assert np.all(np.abs(got.cpu().numpy() - ref) <= 1e-10 * np.abs(ref))
+    nu = ipa.ipa_expected_hist(nbins, LO, HI, inp.GEN, 2500.0, 1e5, -0.002)
+    torch_.cuda.synchronize()
+    nu_ref = orc.expected_hist(nbins, LO, HI, inp.GEN, 2500.0, 1e5, -0.002)
+    assert np.all(np.abs(nu.cpu().numpy() - nu_ref) <= 1e-12 * nu_ref)
+    seeds = np.arange(1, 41, dtype=np.uint64)
+    mean = np.concatenate([nu_ref[:500], [0.0, 0.3, 3.0, 9.99, 10.0, 55.5]])
+    toys = ipa.ipa_poisson_hist_toys(dev(torch_, mean), seeds)
+    torch_.cuda.synchronize()
+    ref_t = orc.poisson_hist_toys(mean, seeds)
+    got_t = toys.cpu().numpy().astype(np.uint32)
+    assert (got_t == ref_t).mean() >= 1 - 1e-4    # a flip needs a uniform within ~1e-15 of a boundary
+    assert abs(got_t.astype(np.int64).sum() - ref_t.astype(np.int64).sum()) <= 50
+
+
+# ---------------------------------------------------------------------------------------------
+# full size, in the launch configuration bench.py times (config 3: 1e8 events, K = 1 and K = 9)
+# ---------------------------------------------------------------------------------------------
+def test_full_size_sampled(ipa, torch_, orc):
+    n = 100_000_000
+    x = inp.standin_masses(3, n)
+    xd = dev(torch_, x)
+    batch, h = inp.fd_batch(inp.GEN)
+    old = ipa.ipa_set_degree_policy(1)
+    try:
+        nll1, lp, _ = ipa.ipa_nll_eval(xd, inp.GEN, LO, HI, want_logpdf=True)
+        nll9, _, _ = ipa.ipa_nll_eval(xd, batch, LO, HI)
+        torch_.cuda.synchronize()
+    finally:
+        ipa.ipa_set_degree_policy(old)
+    # property: the reduction equals the fp64 sum of the per-event outputs
+    s = -lp[0].sum().item()
+    assert abs(nll1.item() - s) <= 1e-11 * abs(s)
+    assert nll9[0].item() == nll1.item()
+    # sampled outputs against the oracle, one by one (includes the ragged last tile)
+    rng = np.random.Generator(np.random.Philox(123))
+    idx = np.concatenate([rng.integers(0, n, size=40000), np.arange(n - 3000, n), np.arange(0, 3000)])
+    got = lp[0][torch_.from_numpy(idx).cuda()].cpu().numpy()
+    assert np.abs(got - orc.logpdf(x[idx], inp.GEN, LO, HI)).max() <= 1e-10
+    # total against the oracle (threads only split the event range; same per-event routine)
+    import os
+    ref = orc.nll(x[:20_000_000], batch[:3], LO, HI, nthreads=max(1, os.cpu_count() or 1))
+    part, _, _ = ipa.ipa_nll_eval(xd[:20_000_000], batch[:3], LO, HI)
+    assert np.all(np.abs(part.cpu().numpy() - ref) <= 1e-10 * np.abs(ref))
