@@ -14,7 +14,8 @@ CSRC = os.path.join(HERE, "csrc")
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "libipanll.so")
 SOURCES = [os.path.join(CSRC, "ipa_api.cu")]
-DEPS = SOURCES + [os.path.join(CSRC, n) for n in ("ipa_kernels.cuh", "ipa_prologue.cuh", "ipa_math.cuh")] + [
+DEPS = SOURCES + [os.path.join(CSRC, n) for n in ("ipa_kernels.cuh", "ipa_prologue.cuh", "ipa_math.cuh", "ipa_fastmath.cuh",
+                                                      "ipa_fastmath_tables.inc")] + [
     os.path.join(ROOT, "include", "ipanll.h")]
 
 NVCC_FLAGS = [

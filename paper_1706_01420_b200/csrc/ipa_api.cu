@@ -59,7 +59,7 @@ int device_info(int* sms) {
   if (g_dev.dev != dev || !g_dev.attr_set) {
     int n = 0;
     IPA_CK(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev));
-    const int smem = IPA_MAX_K * (int)(sizeof(IpaSetConsts) + IPA_BLOCK * 8);
+    const int smem = IPA_MAX_K * (int)(sizeof(IpaSetConsts) + IPA_NB * 8);
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     g_dev.dev = dev;
@@ -149,21 +149,21 @@ int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K
   char* ws = static_cast<char*>(ws_dev);
   rc = run_prologue(p_host, K, r, ws, L, nullptr, nullptr, nullptr, st);
   if (rc) return rc;
-  const int64_t ntiles = (n + IPA_TILE - 1) / IPA_TILE;
-  int64_t G = (int64_t)sms * IPA_BLOCKS_PER_SM;
+  const int64_t ntiles = (n + IPA_NTILE - 1) / IPA_NTILE;
+  int64_t G = (int64_t)sms * IPA_NB_PER_SM;
   if (G > kGridMax) G = kGridMax;
   if (G > ntiles) G = ntiles;
   if (G < 1) G = 1;
-  const size_t smem = (size_t)K * (sizeof(IpaSetConsts) + IPA_BLOCK * 8);
+  const size_t smem = (size_t)K * (sizeof(IpaSetConsts) + IPA_NB * 8);
   const int vec_ok = ((uintptr_t)x_dev % 16) == 0;
   const IpaSetConsts* consts = reinterpret_cast<const IpaSetConsts*>(ws + L.consts);
   double* partials = reinterpret_cast<double*>(ws + L.partials);
   unsigned int* counter = reinterpret_cast<unsigned int*>(ws + L.counter);
   if (logpdf_dev)
-    ipa_nll_kernel<true><<<(unsigned)G, IPA_BLOCK, smem, st>>>(x_dev, n, vec_ok, consts, K, partials, logpdf_dev, counter,
+    ipa_nll_kernel<true><<<(unsigned)G, IPA_NB, smem, st>>>(x_dev, n, vec_ok, consts, K, partials, logpdf_dev, counter,
                                                                nll_dev, status_dev);
   else
-    ipa_nll_kernel<false><<<(unsigned)G, IPA_BLOCK, smem, st>>>(x_dev, n, vec_ok, consts, K, partials, nullptr, counter,
+    ipa_nll_kernel<false><<<(unsigned)G, IPA_NB, smem, st>>>(x_dev, n, vec_ok, consts, K, partials, nullptr, counter,
                                                                 nll_dev, status_dev);
   IPA_CK(cudaGetLastError());
   return IPA_OK;

@@ -1,0 +1,145 @@
+// ipa_fastmath.cuh -- the streaming kernels' own fp64 sqrt / exp / log, written for the argument
+// ranges of the hot path.  Polynomial coefficients live
+// in __constant__ memory so that every DFMA takes its coefficient as a constant-bank operand (no
+// register, no literal materialisation); the 33-entry log table is copied to shared memory by the
+// kernels (per-lane index).  Marked __host__ __device__ so that tests/devmath_host.cu can run the
+// same source on the GPU-less box (the rsqrt seed is emulated there with 20 good bits).
+//
+// Accuracy targets (checked in tests/test_abi_and_host_logic.py against mpmath):
+//   ipa_fsqrt    relative error <= 1.2e-16 for normal positive arguments
+//   ipa_fexp_neg relative error <= 3e-16 for a in [-90, 0]
+//   ipa_flog     absolute error <= 2.5e-16 + 1.5e-16 |log u| for normal positive u
+#pragma once
+#include <math.h>
+#include <stdint.h>
+#include <string.h>
+#include "ipa_fastmath_tables.inc"
+
+#ifndef IPA_HD
+#define IPA_HD __host__ __device__ __forceinline__
+#endif
+
+__constant__ double ipa_c_exp[IPA_EXP_DEG + 1] = IPA_EXP_COEFS;
+__constant__ double ipa_c_log1p[IPA_LOG_DEG] = IPA_LOG1P_COEFS;
+__constant__ double2 ipa_c_logtab[33] = IPA_LOG_TABLE;
+// host copies (tests/devmath_host.cu only)
+struct ipa_host_double2 { double x, y; };
+static const double ipa_h_exp[IPA_EXP_DEG + 1] = IPA_EXP_COEFS;
+static const double ipa_h_log1p[IPA_LOG_DEG] = IPA_LOG1P_COEFS;
+static const ipa_host_double2 ipa_h_logtab[33] = IPA_LOG_TABLE;
+#ifdef __CUDA_ARCH__
+#define IPA_CEXP(j) ipa_c_exp[j]
+#define IPA_CLOG(j) ipa_c_log1p[j]
+#else
+#define IPA_CEXP(j) ipa_h_exp[j]
+#define IPA_CLOG(j) ipa_h_log1p[j]
+#endif
+
+// ---- bit access ---------------------------------------------------------------------------------
+IPA_HD int ipa_hi(double v) {
+#ifdef __CUDA_ARCH__
+  return __double2hiint(v);
+#else
+  uint64_t b; memcpy(&b, &v, 8); return (int)(uint32_t)(b >> 32);
+#endif
+}
+IPA_HD int ipa_lo(double v) {
+#ifdef __CUDA_ARCH__
+  return __double2loint(v);
+#else
+  uint64_t b; memcpy(&b, &v, 8); return (int)(uint32_t)b;
+#endif
+}
+IPA_HD double ipa_mk(int hi, int lo) {
+#ifdef __CUDA_ARCH__
+  return __hiloint2double(hi, lo);
+#else
+  uint64_t b = ((uint64_t)(uint32_t)hi << 32) | (uint32_t)lo; double v; memcpy(&v, &b, 8); return v;
+#endif
+}
+
+// 1/sqrt(q) seed, about 20 good bits (MUFU.RSQ64H on the device)
+IPA_HD double ipa_rsqrt_seed(double q) {
+#ifdef __CUDA_ARCH__
+  double y;
+  asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(q));
+  return y;
+#else
+  const double y = 1.0 / sqrt(q);
+  return ipa_mk(ipa_hi(y), 0);   // 20 mantissa bits, truncated: what the hardware seed guarantees
+#endif
+}
+
+// sqrt(q), q > 0 normal: one third-order (Householder) step from the seed.  5 FP64 instructions.
+//   e = 1 - q y^2,  sqrt(q) = q y (1 - e)^(-1/2) = q y (1 + e/2 + 3 e^2/8 + O(e^3))
+IPA_HD double ipa_fsqrt(double q) {
+  const double y = ipa_rsqrt_seed(q);
+  const double g = q * y;
+  const double e = fma(-g, y, 1.0);
+  const double p = fma(0.375, e, 0.5) * e;
+  return fma(g, p, g);
+}
+
+// e^a for a <= 0 (|a| is clamped to about 64 by the caller or here: results below 1e-27 are not
+// distinguished).  n = round(a log2 e) by the 1.5 2^52 shift, Cody-Waite reduction with a 32-bit
+// ln2_hi, degree-11 polynomial, scaling through the exponent field.  15 FP64 instructions.
+IPA_HD double ipa_fexp_neg(double a) {
+  const double SHIFT = 6755399441055744.0;
+  const double t = fma(a, IPA_LOG2E, SHIFT);
+  const int n = ipa_lo(t);
+  const double nf = t - SHIFT;
+  double r = fma(nf, -IPA_LN2_HI, a);
+  r = fma(nf, -IPA_LN2_LO, r);
+  double p = IPA_CEXP(IPA_EXP_DEG);
+#pragma unroll
+  for (int j = IPA_EXP_DEG - 1; j >= 0; --j) p = fma(p, r, IPA_CEXP(j));
+  return ipa_mk(ipa_hi(p) + (n << 20), ipa_lo(p));
+}
+
+// -min(|D|, ~64) with the sign forced negative: integer work only
+IPA_HD double ipa_neg_abs_clamped(double D) {
+  int h = ipa_hi(D) & 0x7fffffff;
+  h = h < 0x40500000 ? h : 0x40500000;
+  return ipa_mk(h | (int)0x80000000, ipa_lo(D));
+}
+// max(D, 0) by the sign bit: integer work only (NaN with the sign clear passes through)
+IPA_HD double ipa_relu_bits(double D) {
+  const int m = ~(ipa_hi(D) >> 31);
+  return ipa_mk(ipa_hi(D) & m, ipa_lo(D) & m);
+}
+
+// log(u), u > 0 normal.  tab[j] = {c_j, -log c_j}; u = 2^e m, j = top 5 mantissa bits,
+// r = m c_j - 1 (|r| < 2^-6), log u = e ln2 + l_j + log1p(r).  11 FP64 instructions.
+template <class Tab>
+IPA_HD double ipa_flog(double u, const Tab* tab) {
+  const int hu = ipa_hi(u);
+  const int e = (hu >> 20) - 1023;
+  const int j = (hu >> 15) & 31;
+  const double m = ipa_mk((hu & 0x000fffff) | 0x3ff00000, ipa_lo(u));
+  const double ef = ipa_mk(0x43300000, e ^ (int)0x80000000) - 4503601774854144.0;  // 2^52 + 2^31
+  const double cj = tab[j].x, lj = tab[j].y;
+  const double r = fma(m, cj, -1.0);
+  double p = IPA_CLOG(IPA_LOG_DEG - 1);
+#pragma unroll
+  for (int k = IPA_LOG_DEG - 2; k >= 0; --k) p = fma(p, r, IPA_CLOG(k));
+  return fma(ef, IPA_LN2, fma(p, r, lj));
+}
+
+// log(s) for s in [1, 2] (s = 1 + w, w in [0,1]): entry 32 of the table serves s == 2.  10 FP64.
+template <class Tab>
+IPA_HD double ipa_flog_1to2(double s, const Tab* tab) {
+  const int j = (ipa_hi(s) - 0x3ff00000) >> 15;
+  const double cj = tab[j].x, lj = tab[j].y;
+  const double r = fma(s, cj, -1.0);
+  double p = IPA_CLOG(IPA_LOG_DEG - 1);
+#pragma unroll
+  for (int k = IPA_LOG_DEG - 2; k >= 0; --k) p = fma(p, r, IPA_CLOG(k));
+  return fma(p, r, lj);
+}
+
+// log(1 + e^D) = max(D,0) + log(1 + e^{-|D|})
+template <class Tab>
+IPA_HD double ipa_fsoftplus(double D, const Tab* tab) {
+  const double w = ipa_fexp_neg(ipa_neg_abs_clamped(D));
+  return ipa_relu_bits(D) + ipa_flog_1to2(1.0 + w, tab);
+}

@@ -62,24 +62,24 @@ ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_param
 //   l = E_B + log(1 + e^Delta),  E_B = k d + eB0                                      (A3, A4)
 // The polynomial coefficient is read once (uniform LDS) per E fused multiply-adds.
 // ------------------------------------------------------------------------------------------------
-IPA_HD double ipa_softplus(double D) { return fmax(D, 0.0) + log1p(exp(-fabs(D))); }
-
 // direct-mode core term H(z) = log(z^nu K_nu(z)) (kept out of line: it is the slow path)
 __host__ __device__ __noinline__ double ipa_direct_H(double nu, double z) {
   return nu * log(z) + log(ipa_besselk_scaled(nu, z)) - z;
 }
 
-template <int E>
-IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l)[E]) {
+// FP64 instructions per event (SASS, branch-free form): d 1; core q 1 + sqrt 5 + t 1 + Horner D + 1;
+// tail u 1 + log 11 + 2; region 2 DSETP; softplus 15 + 1 + 10; E_B 1; l 2  ->  55 + D.
+template <int E, class Tab>
+IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l)[E], const Tab* tab) {
   double d[E], P[E];
   const double mu = c.mu;
 #pragma unroll
   for (int e = 0; e < E; ++e) d[e] = x[e] - mu;
   if (c.mode == 0) {
-    double t[E];
     const double d2 = c.delta2, tA = c.tA, tB = c.tB;
+    double t[E];
 #pragma unroll
-    for (int e = 0; e < E; ++e) t[e] = fma(tA, sqrt(fma(d[e], d[e], d2)), tB);
+    for (int e = 0; e < E; ++e) t[e] = fma(tA, ipa_fsqrt(fma(d[e], d[e], d2)), tB);
     const int D = c.degree;
     double aj = c.a[D];
 #pragma unroll
@@ -97,18 +97,24 @@ IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l
       if (d[e] >= c.d0 && d[e] <= c.d1) P[e] = ipa_direct_H(c.nu, c.alpha * sqrt(fma(d[e], d[e], c.delta2))) + c.cDir;
     }
   }
-  const double kd = c.kd, eB0 = c.eB0, bmk = c.bmk;
-  const bool pure = c.pure != 0;
+  const double kd = c.kd, eB0 = c.eB0, bmk = c.bmk, d0 = c.d0, d1 = c.d1;
+  double Dl[E];
 #pragma unroll
   for (int e = 0; e < E; ++e) {
-    const bool left = d[e] < c.d0, right = d[e] > c.d1;
+    const bool left = d[e] < d0, right = d[e] > d1;
     const double uA = left ? c.uA0 : c.uA1, uB = left ? c.uB0 : c.uB1;
     const double nT = left ? c.n0 : c.n1, cT = left ? c.cT0 : c.cT1;
-    const double u = fma(uA, d[e], uB);
-    const double tail = fma(-nT, log(u), cT) - kd * d[e];
-    const double Dl = (left || right) ? tail : fma(bmk, d[e], P[e]);
-    const double eb = fma(kd, d[e], eB0);
-    l[e] = eb + (pure ? Dl : ipa_softplus(Dl));
+    const double lu = ipa_flog(fma(uA, d[e], uB), tab);
+    const double tail = fma(-kd, d[e], fma(-nT, lu, cT));
+    Dl[e] = (left || right) ? tail : fma(bmk, d[e], P[e]);
+  }
+  if (c.pure) {
+#pragma unroll
+    for (int e = 0; e < E; ++e) l[e] = fma(kd, d[e], eB0) + Dl[e];
+  } else {
+#pragma unroll
+    for (int e = 0; e < E; ++e) l[e] = (fma(kd, d[e], eB0) + ipa_relu_bits(Dl[e])) +
+                                       ipa_flog_1to2(1.0 + ipa_fexp_neg(ipa_neg_abs_clamped(Dl[e])), tab);
   }
 }
 
@@ -119,17 +125,28 @@ __device__ __forceinline__ double ipa_warp_sum(double v) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// Streaming NLL: persistent grid, tile = 128 threads x 8 events, all K sets per event read.
-// partials[k*G + b]; the last block to finish adds them in a fixed order (A5).
+// Streaming NLL: persistent grid, tile = 256 threads x 4 events (two 128-bit loads per thread, the
+// next tile prefetched into registers while the current one is evaluated), all K sets per event
+// read.  partials[k*G + b]; the last block to finish adds them in a fixed order (A5).
 // ------------------------------------------------------------------------------------------------
+#define IPA_NB 256
+#define IPA_NE 4
+#define IPA_NTILE (IPA_NB * IPA_NE)
+#define IPA_NB_PER_SM 3
+
+__device__ __forceinline__ void ipa_load_logtab(double2* tab) {
+  if (threadIdx.x < 33) tab[threadIdx.x] = ipa_c_logtab[threadIdx.x];
+}
+
 template <bool LOGPDF>
-__global__ void __launch_bounds__(IPA_BLOCK, IPA_BLOCKS_PER_SM)
+__global__ void __launch_bounds__(IPA_NB, IPA_NB_PER_SM)
 ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaSetConsts* __restrict__ consts, int K,
                double* __restrict__ partials, double* __restrict__ logpdf, unsigned int* counter,
                double* __restrict__ nll_out, int32_t* __restrict__ status_out) {
   extern __shared__ __align__(16) unsigned char ipa_smem[];
   IpaSetConsts* sc = reinterpret_cast<IpaSetConsts*>(ipa_smem);
   double* acc = reinterpret_cast<double*>(sc + K);
+  __shared__ double2 s_tab[33];
   __shared__ int s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int G = gridDim.x;
@@ -137,57 +154,64 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
     const int nd = K * (int)(sizeof(IpaSetConsts) / 8);
     const double* src = reinterpret_cast<const double*>(consts);
     double* dst = reinterpret_cast<double*>(sc);
-    for (int i = tid; i < nd; i += IPA_BLOCK) dst[i] = src[i];
-    for (int k = 0; k < K; ++k) acc[k * IPA_BLOCK + tid] = 0.0;
+    for (int i = tid; i < nd; i += IPA_NB) dst[i] = src[i];
+    for (int k = 0; k < K; ++k) acc[k * IPA_NB + tid] = 0.0;
+    ipa_load_logtab(s_tab);
   }
   __syncthreads();
-  const long long ntiles = (n + IPA_TILE - 1) / IPA_TILE;
-  for (long long tile = blockIdx.x; tile < ntiles; tile += G) {
-    const long long base = tile * IPA_TILE;
-    double xv[IPA_E];
-    long long idx[IPA_E];
-    const bool full = base + IPA_TILE <= n;
+  const long long ntiles = (n + IPA_NTILE - 1) / IPA_NTILE;
+  double xn[IPA_NE];
+  auto load_tile = [&](long long tile, double (&xv)[IPA_NE]) {
+    const long long base = tile * IPA_NTILE;
+    if (base + IPA_NTILE <= n && vec_ok) {
 #pragma unroll
-    for (int p = 0; p < IPA_E / 2; ++p) {
-      idx[2 * p] = base + 2LL * (p * IPA_BLOCK + tid);
-      idx[2 * p + 1] = idx[2 * p] + 1;
-    }
-    if (full && vec_ok) {
-#pragma unroll
-      for (int p = 0; p < IPA_E / 2; ++p) {
-        const double2 v = __ldcs(reinterpret_cast<const double2*>(x + idx[2 * p]));
+      for (int p = 0; p < IPA_NE / 2; ++p) {
+        const double2 v = __ldcs(reinterpret_cast<const double2*>(x + base + 2LL * (p * IPA_NB + tid)));
         xv[2 * p] = v.x;
         xv[2 * p + 1] = v.y;
       }
     } else {
 #pragma unroll
-      for (int e = 0; e < IPA_E; ++e) xv[e] = (idx[e] < n) ? x[idx[e]] : 0.0;
+      for (int e = 0; e < IPA_NE; ++e) {
+        const long long i = base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1);
+        xv[e] = (i < n) ? x[i] : 0.0;
+      }
     }
+  };
+  long long tile = blockIdx.x;
+  if (tile < ntiles) load_tile(tile, xn);
+  for (; tile < ntiles; tile += G) {
+    double xv[IPA_NE];
+#pragma unroll
+    for (int e = 0; e < IPA_NE; ++e) xv[e] = xn[e];
+    if (tile + G < ntiles) load_tile(tile + G, xn);
+    const long long base = tile * IPA_NTILE;
+    const bool full = base + IPA_NTILE <= n;
     for (int k = 0; k < K; ++k) {
       const IpaSetConsts& c = sc[k];
       if (c.status) continue;
-      double l[IPA_E];
-      ipa_eval_set<IPA_E>(c, xv, l);
-      double s = 0.0;
-      if (full) {
+      double l[IPA_NE];
+      ipa_eval_set<IPA_NE>(c, xv, l, s_tab);
+      if (!full) {
 #pragma unroll
-        for (int e = 0; e < IPA_E; ++e) s += l[e];
-      } else {
+        for (int e = 0; e < IPA_NE; ++e) {
+          const long long i = base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1);
+          if (LOGPDF && i < n) logpdf[(long long)k * n + i] = l[e];
+          if (i >= n) l[e] = 0.0;
+        }
+      } else if (LOGPDF) {
 #pragma unroll
-        for (int e = 0; e < IPA_E; ++e) s += (idx[e] < n) ? l[e] : 0.0;
+        for (int e = 0; e < IPA_NE; ++e)
+          logpdf[(long long)k * n + base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1)] = l[e];
       }
-      acc[k * IPA_BLOCK + tid] += s;
-      if (LOGPDF) {
-#pragma unroll
-        for (int e = 0; e < IPA_E; ++e)
-          if (idx[e] < n) logpdf[(long long)k * n + idx[e]] = l[e];
-      }
+      acc[k * IPA_NB + tid] += (l[0] + l[1]) + (l[2] + l[3]);
     }
   }
   __syncthreads();
-  for (int k = warp; k < K; k += IPA_BLOCK / 32) {
-    const double* a = acc + k * IPA_BLOCK;
-    double v = (a[lane] + a[lane + 32]) + (a[lane + 64] + a[lane + 96]);
+  for (int k = warp; k < K; k += IPA_NB / 32) {
+    const double* a = acc + k * IPA_NB;
+    double v = ((a[lane] + a[lane + 32]) + (a[lane + 64] + a[lane + 96])) +
+               ((a[lane + 128] + a[lane + 160]) + (a[lane + 192] + a[lane + 224]));
     v = ipa_warp_sum(v);
     if (lane == 0) partials[(long long)k * G + blockIdx.x] = v;
   }
@@ -197,7 +221,7 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
   __syncthreads();
   if (!s_last) return;
   __threadfence();
-  for (int k = warp; k < K; k += IPA_BLOCK / 32) {
+  for (int k = warp; k < K; k += IPA_NB / 32) {
     double v = 0.0;
     for (int i = lane; i < G; i += 32) v += __ldcg(partials + (long long)k * G + i);
     v = ipa_warp_sum(v);
@@ -218,12 +242,14 @@ ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ o
                    const IpaSetConsts* __restrict__ consts, double* __restrict__ partials) {
   __shared__ IpaSetConsts c;
   __shared__ double red[IPA_BLOCK / 32];
+  __shared__ double2 s_tab[33];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const long long t = blockIdx.x;
   {
     const double* src = reinterpret_cast<const double*>(consts + t);
     double* dst = reinterpret_cast<double*>(&c);
     for (int i = tid; i < (int)(sizeof(IpaSetConsts) / 8); i += IPA_BLOCK) dst[i] = src[i];
+    ipa_load_logtab(s_tab);
   }
   __syncthreads();
   const long long beg = offsets[t], len = offsets[t + 1] - beg;
@@ -238,7 +264,7 @@ ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ o
         idx[e] = base + e * IPA_BLOCK + tid;
         xv[e] = (idx[e] < ce) ? __ldcs(x + idx[e]) : 0.0;
       }
-      ipa_eval_set<IPA_E>(c, xv, l);
+      ipa_eval_set<IPA_E>(c, xv, l, s_tab);
       double s = 0.0;
 #pragma unroll
       for (int e = 0; e < IPA_E; ++e) s += (idx[e] < ce) ? l[e] : 0.0;

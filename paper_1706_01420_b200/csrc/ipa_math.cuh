@@ -9,6 +9,7 @@
 #include <stdint.h>
 
 #define IPA_HD __host__ __device__ __forceinline__
+#include "ipa_fastmath.cuh"
 
 // ------------------------------------------------------------------------------------------------
 // Scaled modified Bessel function of the second kind, real order:

@@ -49,7 +49,7 @@ void emu_logpdf(const ipa_params* p, double lo, double hi, int policy, const dou
     double xv[8], l[8];
     for (int e = 0; e < 8; ++e) xv[e] = (i + e < n) ? x[i + e] : x[n - 1];
     if (c.status) { for (int e = 0; e < 8; ++e) l[e] = -INFINITY; }
-    else ipa_eval_set<8>(c, xv, l);
+    else ipa_eval_set<8>(c, xv, l, ipa_h_logtab);
     for (int e = 0; e < 8 && i + e < n; ++e) out[i + e] = l[e];
   }
 }
@@ -63,5 +63,17 @@ void emu_uniforms2(unsigned long long seed, unsigned long long slot, unsigned at
 }
 long long emu_poisson(unsigned long long seed, unsigned long long slot, unsigned stream, double mean) {
   return ipa_poisson(seed, slot, stream, mean);
+}
+}
+
+// ---- the streaming kernels' own sqrt / exp / log (csrc/ipa_fastmath.cuh) ---------------------------
+extern "C" {
+void emu_fsqrt(const double* q, long long n, double* out) { for (long long i = 0; i < n; ++i) out[i] = ipa_fsqrt(q[i]); }
+void emu_fexp_neg(const double* a, long long n, double* out) {
+  for (long long i = 0; i < n; ++i) out[i] = ipa_fexp_neg(ipa_neg_abs_clamped(a[i]));
+}
+void emu_flog(const double* u, long long n, double* out) { for (long long i = 0; i < n; ++i) out[i] = ipa_flog(u[i], ipa_h_logtab); }
+void emu_fsoftplus(const double* D, long long n, double* out) {
+  for (long long i = 0; i < n; ++i) out[i] = ipa_fsoftplus(D[i], ipa_h_logtab);
 }
 }
