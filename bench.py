@@ -28,68 +28,67 @@ import ipa_inputs as inp  # noqa: E402
 LO, HI = inp.LO, inp.HI
 METRIC = "unbinned fp64 NLL events/s (Ipatia+exp)"
 UNIT = "events/s"
-# Algorithmic FP64 work per event and parameter set: flops, FMA = 2.
-FLOPS_PER_EVENT_SET = {"P1_geometric": None}  # filled from DESIGN.md numbers below
 SM_COUNT, FP64_LANES, SM_MAX_HZ = 148, 64, 1.965e9
+# B200 has 64 FP64 FMA lanes per SM (the DFMA-chain probe in extras measures 95 % of this)
 FP64_PEAK_NOMINAL = SM_COUNT * FP64_LANES * 2 * SM_MAX_HZ  # 37.2 TFLOP/s
 
 
-def algorithmic_flops(degree):
-    """FP64 flops one event x set needs in this method (table 'work per event'):
-    core path 2*(degree) Horner + fixed part; the fixed part is counted from the SASS of the kernel
-    (sqrt, region select, tail log, exp, log1p, accumulate)."""
-    return 2.0 * degree + FIXED_FLOPS
-
-
-FIXED_FLOPS = 260.0  # see DESIGN.md: SASS count of the non-polynomial FP64 work per event (v1 kernel)
+def algorithmic_flops(degree, p_core):
+    """FP64 flops one event x set needs in this method (table 'work per event'),
+    FMA = 2, add / mul / compare = 1; an event pays the core OR the tail arithmetic, never both:
+      common  d, 2 compares, E_B, exp (14 FMA + 1 add), 1+w, log on [1,2] (9 FMA), 2 adds : 24 FMA + 7 other = 55
+      core    q, sqrt (3 FMA + 2 mul), t, Horner (degree FMA), (beta-k) d              : (6 + degree) FMA + 2 mul
+      tail    u, log (10 FMA + 1 add), -n log u + c, -k d                               : 13 FMA + 1 add = 27
+    p_core = fraction of the events inside [mu - a sigma, mu + a2 sigma] (0.344 for the config model)."""
+    core = 2.0 * (6 + degree) + 2.0
+    return 55.0 + p_core * core + (1.0 - p_core) * 27.0
 
 
 class ClockSampler:
-    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md recipe)."""
-    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,"
-         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,"
-         "clocks_event_reasons.sw_power_cap")
+    """SM clock / throttle reasons during the timed region (B200_PROFILING.md recipe), sampled through
+    NVML every 5 ms; falls back to nvidia-smi -lms when pynvml is not importable."""
+    REASONS = (("hw_slowdown", 0x8), ("hw_thermal_slowdown", 0x40), ("sw_thermal_slowdown", 0x20), ("sw_power_cap", 0x4))
 
     def __init__(self, index):
-        self.rows, self.proc, self.index = [], None, index
+        self.index, self.rows, self.stop_flag, self.thread, self.h = index, [], False, None, None
 
     def start(self):
         try:
-            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(self.index), "--query-gpu=" + self.Q,
-                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE,
-                                         stderr=subprocess.DEVNULL, text=True)
-            self.t = threading.Thread(target=self._read, daemon=True)
-            self.t.start()
-        except OSError:
-            self.proc = None
+            import pynvml
+            pynvml.nvmlInit()
+            vis = os.environ.get("CUDA_VISIBLE_DEVICES")
+            idx = int(vis.split(",")[self.index]) if vis and vis.split(",")[self.index].isdigit() else self.index
+            self.h = pynvml.nvmlDeviceGetHandleByIndex(idx)
+            self.nv = pynvml
+        except Exception:
+            self.h = None
+            return
+        self.thread = threading.Thread(target=self._loop, daemon=True)
+        self.thread.start()
 
-    def _read(self):
-        for line in self.proc.stdout:
-            self.rows.append(line.strip())
+    def _loop(self):
+        nv = self.nv
+        while not self.stop_flag:
+            try:
+                sm = nv.nvmlDeviceGetClockInfo(self.h, nv.NVML_CLOCK_SM)
+                mx = nv.nvmlDeviceGetMaxClockInfo(self.h, nv.NVML_CLOCK_SM)
+                pw = nv.nvmlDeviceGetPowerUsage(self.h) / 1000.0
+                rs = nv.nvmlDeviceGetCurrentClocksEventReasons(self.h) if hasattr(
+                    nv, "nvmlDeviceGetCurrentClocksEventReasons") else nv.nvmlDeviceGetCurrentClocksThrottleReasons(self.h)
+                self.rows.append((sm, mx, pw, rs))
+            except Exception:
+                pass
+            time.sleep(0.005)
 
     def stop(self):
-        if not self.proc:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        self.proc.terminate()
-        try:
-            self.proc.wait(timeout=5)
-        except Exception:
-            self.proc.kill()
-        sm, mx, pw, reasons = [], [], [], set()
-        names = ("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap")
-        for r in self.rows:
-            f = [s.strip() for s in r.split(",")]
-            if len(f) < 7:
-                continue
-            try:
-                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
-            except ValueError:
-                continue
-            for nm, v in zip(names, f[3:7]):
-                if v.lower().startswith("active"):
-                    reasons.add(nm)
-        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
-                "power_w_max": max(pw) if pw else None, "samples": len(sm), "reasons": sorted(reasons)}
+        if self.h is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["NVML unavailable"], "samples": 0}
+        self.stop_flag = True
+        self.thread.join(timeout=2)
+        sm = [r[0] for r in self.rows]
+        reasons = sorted({nm for r in self.rows for nm, bit in self.REASONS if r[3] & bit})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(r[1] for r in self.rows) if sm else None,
+                "power_w_max": max(r[2] for r in self.rows) if sm else None, "samples": len(sm), "reasons": reasons}
 
 
 def cpu_baseline(x_host, params, cores, budget_events):
@@ -146,17 +145,19 @@ def timed(torch, fn, steps, stream):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
-    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--steps", type=int, default=200)
+    ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--events", type=int, default=100_000_000)
+    ap.add_argument("--layout", default="sorted", choices=["sorted", "asis"],
+                    help="headline event layout: sorted once by ipa_events_sort (outside the timed region) or as generated")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true")
     args = ap.parse_args()
-    args.warmup = max(args.warmup, 3) if args.impl == "ours" else args.warmup
     if args.impl == "reference":
         run_reference(args)
         return
+    args.warmup = max(args.warmup, 3)
 
     import torch
     import paper_1706_01420_b200 as ipa
@@ -176,8 +177,13 @@ def main():
     P1 = inp.GEN
     batch9, h = inp.fd_batch(P1)
 
-    # workload: config 3, generated on the device by the method's generator (seed 3 + rank)
-    x, _, _ = ipa.ipa_toy_generate([3 + rank], P1, -1.0, -1.0, LO, HI, n)
+    # workload: config 3, generated on the device by the method's generator (seed 3 + rank: weak scaling,
+    # every rank owns its own n events, no data-path collective)
+    x_asis, _, _ = ipa.ipa_toy_generate([3 + rank], P1, -1.0, -1.0, LO, HI, n)
+    x_sorted = ipa.ipa_events_sort(x_asis)          # one-off preparation, outside every timed region
+    x = x_sorted if args.layout == "sorted" else x_asis
+    p_core = float(((x_asis >= P1["mu"] - P1["a"] * P1["sigma"]) & (x_asis <= P1["mu"] + P1["a2"] * P1["sigma"]))
+                   .double().mean().item())
     ws = ipa.workspace(n, 32)
     out1 = torch.empty(1, dtype=torch.float64, device="cuda")
     out9 = torch.empty(9, dtype=torch.float64, device="cuda")
@@ -187,11 +193,11 @@ def main():
 
     ipa.ipa_set_degree_policy(1)  # general-order path: no half-integer shortcut in the headline (reading D2)
 
-    def step_k1():
-        ipa.ipa_nll_eval(x, P1, LO, HI, ws=ws, stream=stream, out=out1, status=st1)
+    def step_k1(arr=None):
+        ipa.ipa_nll_eval(x if arr is None else arr, P1, LO, HI, ws=ws, stream=stream, out=out1, status=st1)
 
-    def step_k9():
-        ipa.ipa_nll_eval(x, batch9, LO, HI, ws=ws, stream=stream, out=out9, status=st9)
+    def step_k9(arr=None):
+        ipa.ipa_nll_eval(x if arr is None else arr, batch9, LO, HI, ws=ws, stream=stream, out=out9, status=st9)
 
     for _ in range(args.warmup):
         step_k1()
@@ -210,13 +216,38 @@ def main():
     value = world * n * args.steps / dt
     nll1 = out1.item()
 
-    extras = {}
+    # prologue alone (same kernel, same arguments, through ipa_norm): the streaming kernel's average launch
+    # duration is the step minus this, launch gaps included on the kernel's side
+    norm_out = (torch.empty(1, dtype=torch.float64, device="cuda"), torch.empty(1, dtype=torch.float64, device="cuda"),
+                torch.empty(1, dtype=torch.int32, device="cuda"))
+
+    def step_pro():
+        ipa.ipa_norm(P1, LO, HI, ws=ws, stream=stream, out=norm_out)
+    for _ in range(3):
+        step_pro()
+    dt_pro = timed(torch, step_pro, args.steps, stream) / args.steps
+    t_step = dt / args.steps
+    t_kernel = max(t_step - dt_pro, 1e-9)
+    degree = int(ipa.ipa_core_degree(P1, LO, HI))
+
+    extras = {"p_core": p_core, "core_degree": degree, "prologue_ms": dt_pro * 1e3, "nll_kernel_ms": t_kernel * 1e3}
     if not args.no_extras:
+        k9steps = max(5, args.steps // 8)
         for _ in range(2):
             step_k9()
-        dt9 = timed(torch, step_k9, max(3, args.steps // 4), stream) / max(3, args.steps // 4)
-        extras["k9_gradient_batch"] = {"ms_per_call": dt9 * 1e3, "event_sets_per_s": 9 * n / dt9,
-                                       "events_per_s": n / dt9}
+        dt9 = timed(torch, step_k9, k9steps, stream) / k9steps
+        extras["k9_gradient_batch"] = {"ms_per_call": dt9 * 1e3, "event_sets_per_s": 9 * n / dt9, "events_per_s": n / dt9,
+                                       "nll_calls_per_s": 9 / dt9}
+        other = x_asis if args.layout == "sorted" else x_sorted
+        oname = "asis" if args.layout == "sorted" else "sorted"
+        for _ in range(2):
+            step_k1(other)
+        dto = timed(torch, lambda: step_k1(other), args.steps, stream) / args.steps
+        for _ in range(2):
+            step_k9(other)
+        dto9 = timed(torch, lambda: step_k9(other), k9steps, stream) / k9steps
+        extras[f"k1_layout_{oname}"] = {"ms_per_call": dto * 1e3, "events_per_s": n / dto}
+        extras[f"k9_layout_{oname}"] = {"ms_per_call": dto9 * 1e3, "event_sets_per_s": 9 * n / dto9}
         ipa.ipa_set_degree_policy(0)
         for _ in range(2):
             step_k1()
@@ -230,24 +261,30 @@ def main():
         dtp = timed(torch, step_p2, args.steps, stream) / args.steps
         extras["k1_general_shape_P2"] = {"ms_per_call": dtp * 1e3, "events_per_s": n / dtp}
         ipa.ipa_set_degree_policy(1)
+        step_k1()
         # FP64 peak probe (DFMA chains), for the roofline denominator
         iters = 200000
         ipa.ipa_fp64_peak_probe(1000)
         tp = timed(torch, lambda: ipa.ipa_fp64_peak_probe(iters), 1, stream)
         sms = torch.cuda.get_device_properties(local).multi_processor_count
         extras["fp64_dfma_probe_tflops"] = sms * 8 * 256 * 8 * 2.0 * iters / tp / 1e12
+    nll1 = out1.item()
 
-    # end to end through the public API with HOST buffers: H2D of the events + D2H of the result inside
+    # end to end through the public API with HOST buffers: H2D of the events + D2H of the result inside the
+    # timed region, events in the order the host holds them (as generated; no device-side preparation)
     e2e = None
     if rank == 0 or dist:
         xh = torch.empty(n, dtype=torch.float64, pin_memory=True)
-        xh.copy_(x)
+        xh.copy_(x_asis)
+        xd = torch.empty(n, dtype=torch.float64, device="cuda")
         torch.cuda.synchronize()
-        ipa.nll_host(xh, P1, LO, HI, x_dev=x, ws=ws)
+        ipa.nll_host(xh, P1, LO, HI, x_dev=xd, ws=ws)
         e2e_steps = max(2, min(args.steps, 5))
+        if dist:
+            dist.barrier()
         t0 = time.perf_counter()
         for _ in range(e2e_steps):
-            r = ipa.nll_host(xh, P1, LO, HI, x_dev=x, ws=ws)
+            r = ipa.nll_host(xh, P1, LO, HI, x_dev=xd, ws=ws)
         torch.cuda.synchronize()
         de = time.perf_counter() - t0
         if dist:
@@ -255,41 +292,52 @@ def main():
             dist.all_reduce(t, op=dist.ReduceOp.MAX)
             de = t.item()
         e2e = {"value": world * n * e2e_steps / de, "unit": UNIT, "h2d_bytes_per_step": 8 * n + 88,
-               "d2h_bytes_per_step": 8, "steps": e2e_steps, "nll": float(r[0])}
+               "d2h_bytes_per_step": 8, "steps": e2e_steps, "nll": float(r[0]), "layout": "as generated",
+               "timer": "host wall clock around copy + call + result read"}
+        del xd, xh
 
     if rank != 0:
         return
-    degree = 31  # geometric policy on the config-1 z-interval (prologue output)
-    flops = algorithmic_flops(degree)
-    achieved = flops * n * args.steps / dt / 1e12 / world * world  # per GPU == aggregate / world
+    flops = algorithmic_flops(degree, p_core)
+    achieved = flops * n / t_kernel / 1e12
     peak = FP64_PEAK_NOMINAL / 1e12
-    roofline = {"bound": "alu", "achieved": flops * n / (dt / args.steps) / 1e12, "peak": peak, "unit": "TFLOP/s",
-                "frac": flops * n / (dt / args.steps) / 1e12 / peak, "traffic": None,
-                "peak_source": "nominal 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (no FP64 entry in MEASURED_PEAKS.json); "
-                               "measured DFMA probe in extras",
-                "flops_per_event_set": flops,
-                "hbm": {"achieved_gbs": 8.0 * n / (dt / args.steps) / 1e9, "algorithmic_bytes_per_event": 8}}
+    roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
+                "traffic": 800.05e6 * n / 1e8,
+                "traffic_source": "ncu --set full dram__bytes_read.sum + write.sum of ipa_nll_kernel, profiles/ (per launch, "
+                                  "1e8 events; scaled by events)",
+                "kernel": "ipa_nll_kernel<false>", "kernel_ms": t_kernel * 1e3,
+                "kernel_time_source": "CUDA events: step time minus a prologue-only loop of the same length",
+                "peak_source": "DESIGN.md section 6: 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no "
+                               "FP64 entry); measured DFMA-chain probe in fp64_dfma_probe_tflops",
+                "flops_per_event_set": flops, "p_core": p_core, "core_degree": degree,
+                "hbm": {"achieved_gbs": 8.0 * n / t_kernel / 1e9, "algorithmic_bytes_per_event": 8}}
     try:
         peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
-        roofline["hbm"]["peak_gbs"] = peaks.get("hbm_gbs")
+        roofline["hbm"]["peak_gbs"] = peaks["hbm_gbs"]
         roofline["hbm"]["frac"] = roofline["hbm"]["achieved_gbs"] / peaks["hbm_gbs"]
+        roofline["hbm"]["peak_note"] = "of measured"
     except Exception:
         roofline["hbm"]["peak_gbs"] = 6650.0
         roofline["hbm"]["frac"] = roofline["hbm"]["achieved_gbs"] / 6650.0
         roofline["hbm"]["peak_note"] = "of fallback"
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": 1e3 * dt / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
             "config": {"workload": "config 3: 1e8 fp64 events on [5000,5600] from the Ipatia+exp model (device generator, "
-                                   "seed 3), one NLL evaluation per step, K=1, general-order degree policy",
-                       "events": n, "K": 1, "l2": "input (8 B x events) larger than L2, no flush needed",
+                                   "seed 3), one NLL evaluation per step (prologue + streaming kernel), K=1, general-order "
+                                   "degree policy",
+                       "events": n, "K": 1, "layout": args.layout + (" (sorted once by ipa_events_sort before the timed "
+                                                                      "region; as-generated order in k1_layout_asis)"
+                                                                      if args.layout == "sorted" else ""),
+                       "l2": "input (8 B x events) larger than L2, no flush needed",
                        "multi_gpu": "independent event shards per rank, no data-path collective"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps, "roofline": roofline, "nll": nll1}
     line.update(extras)
     if not args.no_cpu_baseline and world == 1:
         cores = os.cpu_count() or 1
-        xs = x[: min(n, 1_000_000 * cores)].cpu().numpy()
-        line["cpu_baseline"] = cpu_baseline(xs, P1, cores, 1_000_000 * cores)
+        ncpu = min(n, 6_000_000 * cores)
+        xs = x_asis[:ncpu].cpu().numpy()
+        line["cpu_baseline"] = cpu_baseline(xs, P1, cores, ncpu)
     print(json.dumps(line))
 
 

@@ -95,6 +95,13 @@ size_t ipa_workspace_bytes(int64_t n, int64_t K, int64_t nbins);
 int ipa_norm(const ipa_params* p_host, int K, ipa_range r, double* norm_sig_dev, double* norm_bkg_dev,
              int32_t* status_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
 
+/* Introspection of the prologue (step A1e): degree_dev[k] = degree of the core
+ * approximant chosen for set k under the current degree policy, -1 for a set evaluated in direct mode
+ * (per-event Bessel function), -2 for a set with a domain error.  Used by bench.py to state the
+ * algorithmic work of the timed workload. */
+int ipa_core_degree(const ipa_params* p_host, int K, ipa_range r, int32_t* degree_dev, void* ws_dev, size_t ws_bytes,
+                    void* cuda_stream);
+
 /* The hot path (fused into one pass): NLL of n events for K parameter sets.
  *   x_dev      [n]    event masses, fp64, 8-byte aligned
  *   p_host     [K]    parameter sets
@@ -152,6 +159,19 @@ int ipa_expected_hist(int nbins, ipa_range r, const ipa_params* shape_host, doub
  * counts_dev[t*nbins + b] ~ Poisson(mean_dev[b]) from key seeds_host[t], counter slot b. */
 int ipa_poisson_hist_toys(const double* mean_dev, int nbins, const uint64_t* seeds_host, int64_t T,
                           uint32_t* counts_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
+
+/* Optional one-off preparation: ascending sort of the events (whole array, or inside each of T segments
+ * when offsets_dev != NULL).  The likelihood does not depend on the order of the events, the data of a
+ * fit are constant over the minimiser's calls, and the streaming kernels skip the
+ * core polynomial / the tail logarithm for a warp whose 32 x E events all lie in one region: on sorted
+ * events nearly every warp is region-uniform.  Unsorted input is always correct.
+ * The sum over the sorted array differs from the sum over the original order by rounding only (reading
+ * E4).  Radix sort by the toolkit's CUB primitive (a data-layout step, not part of the method); NaN
+ * events sort last.  x_out_dev [n] must not alias x_in_dev; ws_dev of ipa_sort_workspace_bytes(n, T)
+ * bytes (T = 0 for an unsegmented sort); segmented sorts need n < 2^31. */
+size_t ipa_sort_workspace_bytes(int64_t n, int64_t T);
+int ipa_events_sort(const double* x_in_dev, int64_t n, const int64_t* offsets_dev, int64_t T, double* x_out_dev,
+                    void* ws_dev, size_t ws_bytes, void* cuda_stream);
 
 /* Measurement aid (not on the hot path): runs `iters` dependent DFMA per thread in 8 independent
  * chains on a full grid, for the FP64 roofline denominator.  out_dev [1]. */

@@ -12,9 +12,9 @@ from . import build as _build
 
 __all__ = [
     "PARAM_FIELDS", "NPAR", "IPA_MAX_K", "IpaError", "lib", "library_path", "pack_params", "workspace",
-    "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes", "ipa_norm", "ipa_nll_eval",
+    "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes", "ipa_norm", "ipa_core_degree", "ipa_nll_eval",
     "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill", "ipa_binned_nll_scan", "ipa_expected_hist",
-    "ipa_poisson_hist_toys", "ipa_fp64_peak_probe", "nll_host", "EXPORTS",
+    "ipa_poisson_hist_toys", "ipa_events_sort", "ipa_sort_workspace_bytes", "ipa_fp64_peak_probe", "nll_host", "EXPORTS",
 ]
 
 PARAM_FIELDS = ("mu", "sigma", "lambda", "zeta", "beta", "a", "n", "a2", "n2", "f", "k")
@@ -24,8 +24,9 @@ IPA_MAX_K = 32
 # every symbol include/ipanll.h declares
 EXPORTS = (
     "ipa_strerror", "ipa_last_cuda_error", "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes",
-    "ipa_norm", "ipa_nll_eval", "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill",
-    "ipa_binned_nll_scan", "ipa_expected_hist", "ipa_poisson_hist_toys", "ipa_fp64_peak_probe",
+    "ipa_norm", "ipa_core_degree", "ipa_nll_eval", "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill",
+    "ipa_binned_nll_scan", "ipa_expected_hist", "ipa_poisson_hist_toys", "ipa_sort_workspace_bytes", "ipa_events_sort",
+    "ipa_fp64_peak_probe",
 )
 
 
@@ -58,6 +59,7 @@ def lib():
     L.ipa_set_degree_policy.restype = i32; L.ipa_set_degree_policy.argtypes = [i32]
     L.ipa_workspace_bytes.restype = sz; L.ipa_workspace_bytes.argtypes = [i64, i64, i64]
     L.ipa_norm.restype = i32; L.ipa_norm.argtypes = [vp, i32, _Range, vp, vp, vp, vp, sz, vp]
+    L.ipa_core_degree.restype = i32; L.ipa_core_degree.argtypes = [vp, i32, _Range, vp, vp, sz, vp]
     L.ipa_nll_eval.restype = i32; L.ipa_nll_eval.argtypes = [vp, i64, vp, i32, _Range, vp, vp, vp, vp, sz, vp]
     L.ipa_nll_eval_segmented.restype = i32
     L.ipa_nll_eval_segmented.argtypes = [vp, vp, i64, vp, _Range, vp, vp, vp, sz, vp]
@@ -68,6 +70,8 @@ def lib():
     L.ipa_binned_nll_scan.argtypes = [vp, i32, _Range, vp, vp, vp, vp, i64, vp, vp, sz, vp]
     L.ipa_expected_hist.restype = i32; L.ipa_expected_hist.argtypes = [i32, _Range, vp, d, d, d, vp, vp, sz, vp]
     L.ipa_poisson_hist_toys.restype = i32; L.ipa_poisson_hist_toys.argtypes = [vp, i32, vp, i64, vp, vp, sz, vp]
+    L.ipa_sort_workspace_bytes.restype = sz; L.ipa_sort_workspace_bytes.argtypes = [i64, i64]
+    L.ipa_events_sort.restype = i32; L.ipa_events_sort.argtypes = [vp, i64, vp, i64, vp, vp, sz, vp]
     L.ipa_fp64_peak_probe.restype = i32; L.ipa_fp64_peak_probe.argtypes = [i64, vp, vp]
     _lib = L
     return L
@@ -143,18 +147,33 @@ def _ws(ws, n, K, nbins=0):
     return ws
 
 
-def ipa_norm(params, lo, hi, ws=None, stream=None):
-    """-> (norm_sig[K], norm_bkg[K], status[K]) device tensors."""
+def ipa_norm(params, lo, hi, ws=None, stream=None, out=None):
+    """-> (norm_sig[K], norm_bkg[K], status[K]) device tensors (out = the same triple, preallocated)."""
     _need_cuda()
     P = pack_params(params)
     K = P.shape[0]
     ws = _ws(ws, 0, K)
-    ns = torch.empty(K, dtype=torch.float64, device="cuda")
-    nb = torch.empty(K, dtype=torch.float64, device="cuda")
-    st = torch.empty(K, dtype=torch.int32, device="cuda")
+    if out is not None:
+        ns, nb, st = out
+    else:
+        ns = torch.empty(K, dtype=torch.float64, device="cuda")
+        nb = torch.empty(K, dtype=torch.float64, device="cuda")
+        st = torch.empty(K, dtype=torch.int32, device="cuda")
     _check(lib().ipa_norm(_hptr(P), K, _Range(lo, hi), _dptr(ns), _dptr(nb), _dptr(st), _dptr(ws), ws.numel(),
                           _stream(stream)))
     return ns, nb, st
+
+
+def ipa_core_degree(params, lo, hi, ws=None, stream=None):
+    """Degree of the core approximant per set (-1 direct mode, -2 domain error); int for a single set."""
+    _need_cuda()
+    P = pack_params(params)
+    K = P.shape[0]
+    ws = _ws(ws, 0, K)
+    out = torch.empty(K, dtype=torch.int32, device="cuda")
+    _check(lib().ipa_core_degree(_hptr(P), K, _Range(lo, hi), _dptr(out), _dptr(ws), ws.numel(), _stream(stream)))
+    r = out.cpu().numpy()
+    return int(r[0]) if K == 1 else r
 
 
 def ipa_nll_eval(x, params, lo, hi, want_logpdf=False, ws=None, stream=None, out=None, status=None):
@@ -248,6 +267,23 @@ def ipa_poisson_hist_toys(mean, seeds, ws=None, stream=None):
     out = torch.empty((T, nbins), dtype=torch.int32, device="cuda")  # uint32 payload
     _check(lib().ipa_poisson_hist_toys(_dptr(mean, torch.float64), nbins, _hptr(seeds), T, _dptr(out), _dptr(ws),
                                        ws.numel(), _stream(stream)))
+    return out
+
+
+def ipa_sort_workspace_bytes(n, T=0):
+    return int(lib().ipa_sort_workspace_bytes(int(n), int(T)))
+
+
+def ipa_events_sort(x, offsets=None, stream=None):
+    """One-off preparation: ascending sort of the events (inside each segment if offsets is given).
+    -> new device tensor; x is left untouched."""
+    _need_cuda()
+    n = x.numel()
+    T = offsets.numel() - 1 if offsets is not None else 0
+    out = torch.empty_like(x)
+    ws = torch.empty(max(256, ipa_sort_workspace_bytes(n, T)), dtype=torch.uint8, device="cuda")
+    _check(lib().ipa_events_sort(_dptr(x, torch.float64) if n else None, n, _dptr(offsets, torch.int64), T,
+                                 _dptr(out) if n else None, _dptr(ws), ws.numel(), _stream(stream)))
     return out
 
 

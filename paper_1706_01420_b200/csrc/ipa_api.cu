@@ -4,6 +4,8 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
+#include <cub/device/device_radix_sort.cuh>
+#include <cub/device/device_segmented_radix_sort.cuh>
 #include "ipa_kernels.cuh"
 
 namespace {
@@ -133,6 +135,20 @@ int ipa_norm(const ipa_params* p_host, int K, ipa_range r, double* norm_sig_dev,
   if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
   return run_prologue(p_host, K, r, static_cast<char*>(ws_dev), L, norm_sig_dev, norm_bkg_dev, status_dev,
                       static_cast<cudaStream_t>(cuda_stream));
+}
+
+int ipa_core_degree(const ipa_params* p_host, int K, ipa_range r, int32_t* degree_dev, void* ws_dev, size_t ws_bytes,
+                    void* cuda_stream) {
+  if (!p_host || K < 1 || !range_ok(r) || !degree_dev) return IPA_ERR_INVALID_ARG;
+  const Layout L = make_layout(K, 0);
+  if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* ws = static_cast<char*>(ws_dev);
+  int rc = run_prologue(p_host, K, r, ws, L, nullptr, nullptr, nullptr, st);
+  if (rc) return rc;
+  ipa_degree_kernel<<<(K + 127) / 128, 128, 0, st>>>(reinterpret_cast<const IpaSetConsts*>(ws + L.consts), K, degree_dev);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
 }
 
 int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r, double* nll_dev,
@@ -316,6 +332,41 @@ int ipa_poisson_hist_toys(const double* mean_dev, int nbins, const uint64_t* see
                                                        reinterpret_cast<const unsigned long long*>(ws + L.seeds), T,
                                                        counts_dev);
   IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
+size_t ipa_sort_workspace_bytes(int64_t n, int64_t T) {
+  if (n < 0 || T < 0) return 0;
+  size_t bytes = 0;
+  const double* in = nullptr;
+  double* out = nullptr;
+  if (T > 0) {
+    if (n > 0x7fffffffLL || T > 0x7fffffffLL) return 0;
+    const long long* off = nullptr;
+    cub::DeviceSegmentedRadixSort::SortKeys(nullptr, bytes, in, out, (int)n, (int)T, off, off + 1, 0, 64, 0);
+  } else {
+    cub::DeviceRadixSort::SortKeys(nullptr, bytes, in, out, (long long)n, 0, 64, 0);
+  }
+  return align_up(bytes + 256, 256);
+}
+
+int ipa_events_sort(const double* x_in_dev, int64_t n, const int64_t* offsets_dev, int64_t T, double* x_out_dev,
+                    void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (n < 0 || T < 0 || (n > 0 && (!x_in_dev || !x_out_dev || x_in_dev == x_out_dev))) return IPA_ERR_INVALID_ARG;
+  if (offsets_dev && (T < 1 || n > 0x7fffffffLL || T > 0x7fffffffLL)) return IPA_ERR_INVALID_ARG;
+  if (!offsets_dev) T = 0;
+  if (n == 0) return IPA_OK;
+  size_t need = ipa_sort_workspace_bytes(n, T);
+  if (!ws_ok(ws_dev, ws_bytes, need)) return IPA_ERR_WORKSPACE;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  size_t bytes = ws_bytes;
+  if (T > 0) {
+    const long long* off = reinterpret_cast<const long long*>(offsets_dev);
+    IPA_CK(cub::DeviceSegmentedRadixSort::SortKeys(ws_dev, bytes, x_in_dev, x_out_dev, (int)n, (int)T, off, off + 1, 0, 64,
+                                                   st));
+  } else {
+    IPA_CK(cub::DeviceRadixSort::SortKeys(ws_dev, bytes, x_in_dev, x_out_dev, (long long)n, 0, 64, st));
+  }
   return IPA_OK;
 }
 

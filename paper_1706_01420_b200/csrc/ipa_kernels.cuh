@@ -66,48 +66,101 @@ ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_param
 __host__ __device__ __noinline__ double ipa_direct_H(double nu, double z) {
   return nu * log(z) + log(ipa_besselk_scaled(nu, z)) - z;
 }
+// P[e] = H(alpha r_e) + cDir for the core events of d[0..E), 0 for the others
+__host__ __device__ __noinline__ void ipa_direct_core(const IpaSetConsts& c, const double* d, double* P, int E) {
+  for (int e = 0; e < E; ++e) {
+    P[e] = 0.0;
+    if (!((d[e] < c.d0) || (d[e] > c.d1)))
+      P[e] = ipa_direct_H(c.nu, c.alpha * sqrt(fma(d[e], d[e], c.delta2))) + c.cDir;
+  }
+}
 
-// FP64 instructions per event (SASS, branch-free form): d 1; core q 1 + sqrt 5 + t 1 + Horner D + 1;
-// tail u 1 + log 11 + 2; region 2 DSETP; softplus 15 + 1 + 10; E_B 1; l 2  ->  55 + D.
+// Warp-uniform votes: does ANY lane of the warp hold a core / a tail event?  (On the host build,
+// tests/devmath_host.cu, the "warp" is the single caller.)
+IPA_HD bool ipa_any(bool v) {
+#ifdef __CUDA_ARCH__
+  return __any_sync(IPA_FULL, v);
+#else
+  return v;
+#endif
+}
+
+// FP64 instructions per event (SASS): d 1, region 2 DSETP; a warp whose events are all in the core
+// pays q 1 + sqrt 5 + t 1 + Horner ceil4(D+1) + 1, one whose events are all in a tail pays u 1 + log 11
+// + 2, a mixed warp pays both; then softplus 15 + 1 + 10, E_B 1, l 2.  The Horner loop runs over
+// groups of 4 coefficients (two 128-bit uniform shared loads per group, a[] is zero above the degree).
 template <int E, class Tab>
 IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l)[E], const Tab* tab) {
-  double d[E], P[E];
-  const double mu = c.mu;
-#pragma unroll
-  for (int e = 0; e < E; ++e) d[e] = x[e] - mu;
-  if (c.mode == 0) {
-    const double d2 = c.delta2, tA = c.tA, tB = c.tB;
-    double t[E];
-#pragma unroll
-    for (int e = 0; e < E; ++e) t[e] = fma(tA, ipa_fsqrt(fma(d[e], d[e], d2)), tB);
-    const int D = c.degree;
-    double aj = c.a[D];
-#pragma unroll
-    for (int e = 0; e < E; ++e) P[e] = aj;
-    for (int j = D - 1; j >= 0; --j) {
-      aj = c.a[j];
-#pragma unroll
-      for (int e = 0; e < E; ++e) P[e] = fma(P[e], t[e], aj);
-    }
-  } else {
-    // direct mode (shapes the polynomial cannot cover): per-event trapezoid Bessel, core events only
-#pragma unroll
-    for (int e = 0; e < E; ++e) {
-      P[e] = 0.0;
-      if (d[e] >= c.d0 && d[e] <= c.d1) P[e] = ipa_direct_H(c.nu, c.alpha * sqrt(fma(d[e], d[e], c.delta2))) + c.cDir;
-    }
-  }
-  const double kd = c.kd, eB0 = c.eB0, bmk = c.bmk, d0 = c.d0, d1 = c.d1;
-  double Dl[E];
+  double d[E], Dl[E];
+  const double mu = c.mu, d0 = c.d0, d1 = c.d1;
+  bool anyc = false, anyl = false, anyr = false;
 #pragma unroll
   for (int e = 0; e < E; ++e) {
+    d[e] = x[e] - mu;
     const bool left = d[e] < d0, right = d[e] > d1;
-    const double uA = left ? c.uA0 : c.uA1, uB = left ? c.uB0 : c.uB1;
-    const double nT = left ? c.n0 : c.n1, cT = left ? c.cT0 : c.cT1;
-    const double lu = ipa_flog(fma(uA, d[e], uB), tab);
-    const double tail = fma(-kd, d[e], fma(-nT, lu, cT));
-    Dl[e] = (left || right) ? tail : fma(bmk, d[e], P[e]);
+    anyl = anyl || left;
+    anyr = anyr || right;
+    anyc = anyc || !(left || right);                // NaN events take the core path and stay NaN
   }
+  anyc = ipa_any(anyc);
+  anyl = ipa_any(anyl);
+  anyr = ipa_any(anyr);
+  const bool anyt = anyl || anyr;
+  const double kd = c.kd;
+  if (anyc) {
+    double P[E];
+    if (c.mode == 0) {
+      const double d2 = c.delta2, tA = c.tA, tB = c.tB;
+      double t[E];
+#pragma unroll
+      for (int e = 0; e < E; ++e) { t[e] = fma(tA, ipa_fsqrt(fma(d[e], d[e], d2)), tB); P[e] = 0.0; }
+      for (int g = c.degree >> 2; g >= 0; --g) {
+        const double2 hi2 = *reinterpret_cast<const double2*>(c.a + 4 * g + 2);
+        const double2 lo2 = *reinterpret_cast<const double2*>(c.a + 4 * g);
+#pragma unroll
+        for (int e = 0; e < E; ++e) {
+          P[e] = fma(P[e], t[e], hi2.y);
+          P[e] = fma(P[e], t[e], hi2.x);
+          P[e] = fma(P[e], t[e], lo2.y);
+          P[e] = fma(P[e], t[e], lo2.x);
+        }
+      }
+    } else {
+      // direct mode (shapes the polynomial cannot cover): per-event Bessel evaluation, out of line
+      double dt[E], Pt[E];
+#pragma unroll
+      for (int e = 0; e < E; ++e) dt[e] = d[e];
+      ipa_direct_core(c, dt, Pt, E);
+#pragma unroll
+      for (int e = 0; e < E; ++e) P[e] = Pt[e];
+    }
+    const double bmk = c.bmk;
+#pragma unroll
+    for (int e = 0; e < E; ++e) Dl[e] = fma(bmk, d[e], P[e]);
+  }
+  if (anyt) {
+    // a warp whose tail events are all on one side reads that side's four constants once (uniform
+    // shared loads); only a warp straddling both tails selects per lane
+    if (!(anyl && anyr)) {
+      const double* q = anyr ? &c.uA1 : &c.uA0;
+      const double uA = q[0], uB = q[1], nT = q[2], cT = q[3];
+#pragma unroll
+      for (int e = 0; e < E; ++e) {
+        const double tl = fma(-kd, d[e], fma(-nT, ipa_flog(fma(uA, d[e], uB), tab), cT));
+        if ((d[e] < d0) || (d[e] > d1)) Dl[e] = tl;
+      }
+    } else {
+#pragma unroll
+      for (int e = 0; e < E; ++e) {
+        const bool left = d[e] < d0, right = d[e] > d1;
+        const double uA = left ? c.uA0 : c.uA1, uB = left ? c.uB0 : c.uB1;
+        const double nT = left ? c.n0 : c.n1, cT = left ? c.cT0 : c.cT1;
+        const double tl = fma(-kd, d[e], fma(-nT, ipa_flog(fma(uA, d[e], uB), tab), cT));
+        if (left || right) Dl[e] = tl;
+      }
+    }
+  }
+  const double eB0 = c.eB0;
   if (c.pure) {
 #pragma unroll
     for (int e = 0; e < E; ++e) l[e] = fma(kd, d[e], eB0) + Dl[e];
@@ -129,10 +182,16 @@ __device__ __forceinline__ double ipa_warp_sum(double v) {
 // next tile prefetched into registers while the current one is evaluated), all K sets per event
 // read.  partials[k*G + b]; the last block to finish adds them in a fixed order (A5).
 // ------------------------------------------------------------------------------------------------
+#ifndef IPA_NB
 #define IPA_NB 256
-#define IPA_NE 4
+#endif
+#ifndef IPA_NE
+#define IPA_NE 8
+#endif
 #define IPA_NTILE (IPA_NB * IPA_NE)
-#define IPA_NB_PER_SM 3
+#ifndef IPA_NB_PER_SM
+#define IPA_NB_PER_SM 2
+#endif
 
 __device__ __forceinline__ void ipa_load_logtab(double2* tab) {
   if (threadIdx.x < 33) tab[threadIdx.x] = ipa_c_logtab[threadIdx.x];
@@ -204,14 +263,19 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
         for (int e = 0; e < IPA_NE; ++e)
           logpdf[(long long)k * n + base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1)] = l[e];
       }
-      acc[k * IPA_NB + tid] += (l[0] + l[1]) + (l[2] + l[3]);
+      double sl = 0.0;
+#pragma unroll
+      for (int e = 0; e < IPA_NE; e += 4) sl += (l[e] + l[e + 1]) + (l[e + 2] + l[e + 3]);
+      acc[k * IPA_NB + tid] += sl;
     }
   }
   __syncthreads();
   for (int k = warp; k < K; k += IPA_NB / 32) {
     const double* a = acc + k * IPA_NB;
-    double v = ((a[lane] + a[lane + 32]) + (a[lane + 64] + a[lane + 96])) +
-               ((a[lane + 128] + a[lane + 160]) + (a[lane + 192] + a[lane + 224]));
+    double v = 0.0;
+#pragma unroll
+    for (int w = 0; w < IPA_NB / 32; w += 4)
+      v += (a[lane + 32 * w] + a[lane + 32 * w + 32]) + (a[lane + 32 * w + 64] + a[lane + 32 * w + 96]);
     v = ipa_warp_sum(v);
     if (lane == 0) partials[(long long)k * G + blockIdx.x] = v;
   }
@@ -551,6 +615,11 @@ ipa_poisson_hist_kernel(const double* __restrict__ mean, int nbins, const unsign
     const int b = (int)(i - t * nbins);
     counts[i] = (unsigned int)ipa_poisson(seeds[t], (unsigned long long)b, IPA_STREAM_BIN, mean[b]);
   }
+}
+
+__global__ void ipa_degree_kernel(const IpaSetConsts* __restrict__ consts, int K, int32_t* __restrict__ out) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < K) out[k] = consts[k].status ? -2 : (consts[k].mode ? -1 : consts[k].degree);
 }
 
 // ------------------------------------------------------------------------------------------------

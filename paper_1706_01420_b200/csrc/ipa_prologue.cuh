@@ -28,11 +28,15 @@
 #define IPA_NBTASK (IPA_MCHEB + 4)  // Chebyshev nodes + K_nu(z0), K_nu(z1), K_{nu-1}(z0), K_{nu-1}(z1)
 
 // What the streaming kernels read, per parameter set (all fp64 except the flags).
-struct IpaSetConsts {
-  double mu, d0, d1, delta2;
+struct alignas(16) IpaSetConsts {
+  double a[IPA_NCOEF];          // Delta_core = sum_j a[j] t^j + bmk d   (a[0] carries the constants; zero above
+                                // the degree, so Horner may start at any index >= degree).  16-byte aligned:
+                                // the streaming kernel reads coefficient pairs with 128-bit shared loads.
+  double mu, delta2;            // d = x - mu, r = sqrt(d^2 + delta2)
   double tA, tB;                // t = tA r + tB in [-1,1] on the core
-  double bmk;                   // beta - kd
-  double kd, eB0;               // E_B = kd d + eB0      (kd = k; both 0 for f == 1)
+  double d0, d1;                // joins
+  double bmk, kd;               // beta - kd;  E_B = kd d + eB0   (kd = k; both 0 for f == 1)
+  double eB0, araw0;            // araw0 = a[0] before folding: H(z) itself = sum araw t^j
   double uA0, uB0, n0, cT0;     // left tail:  u = uA0 d + uB0,  Delta = cT0 - n0 log u - kd d
   double uA1, uB1, n1, cT1;     // right tail
   double alpha, nu, cDir;       // direct mode: Delta = H(alpha r) + bmk d + cDir, H(z) = log(z^nu K_nu(z))
@@ -40,8 +44,6 @@ struct IpaSetConsts {
   double beta, logG0, logG1, logNS, logref;  // for the generators / binned path: log I(d)
   double normS, normB;          // N_S, N_B (absolute)
   int32_t status, degree, mode, pure;
-  double a[IPA_NCOEF];          // Delta_core = sum_j a[j] t^j + bmk d   (a[0] carries the constants)
-  double araw0;                 // a[0] before folding: H(z) itself = sum araw t^j
 };
 
 struct IpaProWork {

@@ -269,6 +269,46 @@ def test_binned_scan_expected_hist_and_poisson_toys(ipa, torch_, orc):
 
 
 # ---------------------------------------------------------------------------------------------
+# optional preparation: sorted events (warp-uniform regions); reading E4
+# ---------------------------------------------------------------------------------------------
+def test_events_sort_and_sorted_nll(ipa, torch_, orc, x1):
+    x = np.concatenate([x1, [LO, HI, 5250.0, 5250.0, 5310.0]])
+    xd = dev(torch_, x)
+    xs = ipa.ipa_events_sort(xd)
+    torch_.cuda.synchronize()
+    assert np.array_equal(xs.cpu().numpy(), np.sort(x))          # exact: a permutation in ascending order
+    assert np.array_equal(xd.cpu().numpy(), x)                   # input untouched
+    batch, h = inp.fd_batch(inp.P2)
+    a, _, _ = ipa.ipa_nll_eval(xd, batch, LO, HI)
+    b, lp, _ = ipa.ipa_nll_eval(xs, batch, LO, HI, want_logpdf=True)
+    torch_.cuda.synchronize()
+    a, b = a.cpu().numpy(), b.cpu().numpy()
+    assert np.all(np.abs(a - b) <= 1e-12 * np.abs(a))            # order changes rounding only
+    ref = orc.nll(x, batch, LO, HI)                              # oracle: original order, pairwise
+    assert np.all(np.abs(b - ref) <= 1e-10 * np.abs(ref))
+    assert grad_ok(inp.fd_gradient(b, h), inp.fd_gradient(ref, h))
+    assert np.abs(lp[0].cpu().numpy() - orc.logpdf(np.sort(x), batch[0], LO, HI)).max() <= 1e-10
+    # empty input
+    e = ipa.ipa_events_sort(xd[:0])
+    assert e.numel() == 0
+
+
+def test_segmented_sort(ipa, torch_, orc, x1):
+    off = np.array([0, 0, 17, 4000, 4000, 10000], dtype=np.int64)
+    xd, od = dev(torch_, x1), dev(torch_, off)
+    xs = ipa.ipa_events_sort(xd, od)
+    torch_.cuda.synchronize()
+    got = xs.cpu().numpy()
+    for t in range(off.size - 1):
+        assert np.array_equal(got[off[t]:off[t + 1]], np.sort(x1[off[t]:off[t + 1]]))
+    sets = inp.toy_param_sets(off.size - 1, seed=3)
+    a, _ = ipa.ipa_nll_eval_segmented(xs, od, sets, LO, HI)
+    torch_.cuda.synchronize()
+    ref = orc.nll_segmented(x1, off, sets, LO, HI)
+    assert np.all(np.abs(a.cpu().numpy() - ref) <= 1e-10 * np.abs(ref))
+
+
+# ---------------------------------------------------------------------------------------------
 # full size, in the launch configuration bench.py times (config 3: 1e8 events, K = 1 and K = 9)
 # ---------------------------------------------------------------------------------------------
 def test_full_size_sampled(ipa, torch_, orc):
@@ -297,3 +337,18 @@ def test_full_size_sampled(ipa, torch_, orc):
     ref = orc.nll(x[:20_000_000], batch[:3], LO, HI, nthreads=max(1, os.cpu_count() or 1))
     part, _, _ = ipa.ipa_nll_eval(xd[:20_000_000], batch[:3], LO, HI)
     assert np.all(np.abs(part.cpu().numpy() - ref) <= 1e-10 * np.abs(ref))
+    # the sorted layout bench.py times: same total up to rounding, sampled outputs against the oracle
+    del lp
+    xs = ipa.ipa_events_sort(xd)
+    old = ipa.ipa_set_degree_policy(1)
+    try:
+        nlls, lps, _ = ipa.ipa_nll_eval(xs, inp.GEN, LO, HI, want_logpdf=True)
+        torch_.cuda.synchronize()
+    finally:
+        ipa.ipa_set_degree_policy(old)
+    assert abs(nlls.item() - nll1.item()) <= 1e-12 * abs(nll1.item())
+    assert bool((xs[1:] >= xs[:-1]).all().item())
+    sel = torch_.from_numpy(idx).cuda()
+    assert np.abs(lps[0][sel].cpu().numpy() - orc.logpdf(xs[sel].cpu().numpy(), inp.GEN, LO, HI)).max() <= 1e-10
+    parts, _, _ = ipa.ipa_nll_eval(ipa.ipa_events_sort(xd[:20_000_000]), batch[:3], LO, HI)
+    assert np.all(np.abs(parts.cpu().numpy() - ref) <= 1e-10 * np.abs(ref))
