@@ -61,7 +61,7 @@ int device_info(int* sms) {
   if (g_dev.dev != dev || !g_dev.attr_set) {
     int n = 0;
     IPA_CK(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev));
-    const int smem = IPA_MAX_K * (int)(sizeof(IpaSetConsts) + IPA_NB * 8);
+    const int smem = IPA_MAX_K * (int)(sizeof(IpaSetConsts) + IPA_NB * 8) + 2 * IPA_NTILE * 8;
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     g_dev.dev = dev;
@@ -170,7 +170,7 @@ int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K
   if (G > kGridMax) G = kGridMax;
   if (G > ntiles) G = ntiles;
   if (G < 1) G = 1;
-  const size_t smem = (size_t)K * (sizeof(IpaSetConsts) + IPA_NB * 8);
+  const size_t smem = (size_t)K * (sizeof(IpaSetConsts) + IPA_NB * 8) + 2 * IPA_NTILE * 8;
   const int vec_ok = ((uintptr_t)x_dev % 16) == 0;
   const IpaSetConsts* consts = reinterpret_cast<const IpaSetConsts*>(ws + L.consts);
   double* partials = reinterpret_cast<double*>(ws + L.partials);

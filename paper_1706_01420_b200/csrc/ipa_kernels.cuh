@@ -183,32 +183,57 @@ __device__ __forceinline__ double ipa_warp_sum(double v) {
 // read.  partials[k*G + b]; the last block to finish adds them in a fixed order (A5).
 // ------------------------------------------------------------------------------------------------
 #ifndef IPA_NB
-#define IPA_NB 256
+#define IPA_NB 512
 #endif
 #ifndef IPA_NE
 #define IPA_NE 8
 #endif
 #define IPA_NTILE (IPA_NB * IPA_NE)
 #ifndef IPA_NB_PER_SM
-#define IPA_NB_PER_SM 2
+#define IPA_NB_PER_SM 1
 #endif
 
 __device__ __forceinline__ void ipa_load_logtab(double2* tab) {
   if (threadIdx.x < 33) tab[threadIdx.x] = ipa_c_logtab[threadIdx.x];
 }
 
+// 16-byte asynchronous global -> shared copy (LDGSTS, L2 only) and its group fences
+__device__ __forceinline__ void ipa_cp_async16(void* smem_dst, const void* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ void ipa_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
+__device__ __forceinline__ void ipa_cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
+
+// Events travel global -> shared with cp.async, two tiles deep: while tile i is evaluated from
+// registers the copy of tile i+G is in flight and occupies no register (a register prefetch was
+// spilled by ptxas, which exposed the full DRAM latency at every tile: profiles/r01_v3_*).  Every
+// thread copies and later reads its OWN 16-byte slots, so no block barrier is needed in the loop.
 template <bool LOGPDF>
 __global__ void __launch_bounds__(IPA_NB, IPA_NB_PER_SM)
 ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaSetConsts* __restrict__ consts, int K,
                double* __restrict__ partials, double* __restrict__ logpdf, unsigned int* counter,
                double* __restrict__ nll_out, int32_t* __restrict__ status_out) {
   extern __shared__ __align__(16) unsigned char ipa_smem[];
-  IpaSetConsts* sc = reinterpret_cast<IpaSetConsts*>(ipa_smem);
-  double* acc = reinterpret_cast<double*>(sc + K);
+  double* stage = reinterpret_cast<double*>(ipa_smem);                       // [2][IPA_NTILE]
+  IpaSetConsts* sc = reinterpret_cast<IpaSetConsts*>(stage + 2 * IPA_NTILE);  // [K]
+  double* acc = reinterpret_cast<double*>(sc + K);                            // [K][IPA_NB]
   __shared__ double2 s_tab[33];
   __shared__ int s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int G = gridDim.x;
+  const long long ntiles = (n + IPA_NTILE - 1) / IPA_NTILE;
+  auto issue = [&](long long tile, int buf) {
+    const long long base = tile * IPA_NTILE;
+    if (base + IPA_NTILE <= n && vec_ok) {
+#pragma unroll
+      for (int p = 0; p < IPA_NE / 2; ++p)
+        ipa_cp_async16(stage + buf * IPA_NTILE + 2 * (p * IPA_NB + tid), x + base + 2LL * (p * IPA_NB + tid));
+    }
+    ipa_cp_async_commit();
+  };
+  long long tile = blockIdx.x;
+  if (tile < ntiles) issue(tile, 0);
   {
     const int nd = K * (int)(sizeof(IpaSetConsts) / 8);
     const double* src = reinterpret_cast<const double*>(consts);
@@ -218,14 +243,16 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
     ipa_load_logtab(s_tab);
   }
   __syncthreads();
-  const long long ntiles = (n + IPA_NTILE - 1) / IPA_NTILE;
-  double xn[IPA_NE];
-  auto load_tile = [&](long long tile, double (&xv)[IPA_NE]) {
+  int buf = 0;
+  for (; tile < ntiles; tile += G, buf ^= 1) {
     const long long base = tile * IPA_NTILE;
-    if (base + IPA_NTILE <= n && vec_ok) {
+    const bool full = base + IPA_NTILE <= n;
+    double xv[IPA_NE];
+    ipa_cp_async_wait_all();
+    if (full && vec_ok) {
 #pragma unroll
       for (int p = 0; p < IPA_NE / 2; ++p) {
-        const double2 v = __ldcs(reinterpret_cast<const double2*>(x + base + 2LL * (p * IPA_NB + tid)));
+        const double2 v = *reinterpret_cast<const double2*>(stage + buf * IPA_NTILE + 2 * (p * IPA_NB + tid));
         xv[2 * p] = v.x;
         xv[2 * p + 1] = v.y;
       }
@@ -236,16 +263,7 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
         xv[e] = (i < n) ? x[i] : 0.0;
       }
     }
-  };
-  long long tile = blockIdx.x;
-  if (tile < ntiles) load_tile(tile, xn);
-  for (; tile < ntiles; tile += G) {
-    double xv[IPA_NE];
-#pragma unroll
-    for (int e = 0; e < IPA_NE; ++e) xv[e] = xn[e];
-    if (tile + G < ntiles) load_tile(tile + G, xn);
-    const long long base = tile * IPA_NTILE;
-    const bool full = base + IPA_NTILE <= n;
+    if (tile + G < ntiles) issue(tile + G, buf ^ 1);
     for (int k = 0; k < K; ++k) {
       const IpaSetConsts& c = sc[k];
       if (c.status) continue;
