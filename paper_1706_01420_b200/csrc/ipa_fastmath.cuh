@@ -128,13 +128,36 @@ IPA_HD double ipa_flog(double u, const Tab* tab) {
 // log(s) for s in [1, 2] (s = 1 + w, w in [0,1]): entry 32 of the table serves s == 2.  10 FP64.
 template <class Tab>
 IPA_HD double ipa_flog_1to2(double s, const Tab* tab) {
-  const int j = (ipa_hi(s) - 0x3ff00000) >> 15;
+  unsigned j = (unsigned)((ipa_hi(s) - 0x3ff00000) >> 15);
+  j = j < 32u ? j : 32u;   // s outside [1,2] (a NaN event) must not index past the table
   const double cj = tab[j].x, lj = tab[j].y;
   const double r = fma(s, cj, -1.0);
   double p = IPA_CLOG(IPA_LOG_DEG - 1);
 #pragma unroll
   for (int k = IPA_LOG_DEG - 2; k >= 0; --k) p = fma(p, r, IPA_CLOG(k));
   return fma(p, r, lj);
+}
+
+// eb + log(1 + e^D) = eb + log(1 + e^{-|D|}) [+ D if D >= 0].  -|D| enters the exponential through operand
+// modifiers, the exponent shift is clamped instead of the argument, and max(D,0) is a predicated add on
+// the sign word: 2 integer instructions where the clamp / relu pair above needs 7.  |D| < 2^50.
+template <class Tab>
+IPA_HD double ipa_fsoftplus_add(double eb, double D, const Tab* tab) {
+  const double SHIFT = 6755399441055744.0;
+  const double a = -fabs(D);
+  const double t = fma(a, IPA_LOG2E, SHIFT);
+  int n = ipa_lo(t);
+  const double nf = t - SHIFT;
+  double r = fma(nf, -IPA_LN2_HI, a);
+  r = fma(nf, -IPA_LN2_LO, r);
+  double p = IPA_CEXP(IPA_EXP_DEG);
+#pragma unroll
+  for (int j = IPA_EXP_DEG - 1; j >= 0; --j) p = fma(p, r, IPA_CEXP(j));
+  n = n > -1000 ? n : -1000;
+  const double w = ipa_mk(ipa_hi(p) + (n << 20), ipa_lo(p));
+  double l = eb + ipa_flog_1to2(1.0 + w, tab);
+  if (ipa_hi(D) >= 0) l += D;
+  return l;
 }
 
 // log(1 + e^D) = max(D,0) + log(1 + e^{-|D|})

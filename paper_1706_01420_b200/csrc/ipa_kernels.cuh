@@ -75,89 +75,100 @@ __host__ __device__ __noinline__ void ipa_direct_core(const IpaSetConsts& c, con
   }
 }
 
-// Warp-uniform votes: does ANY lane of the warp hold a core / a tail event?  (On the host build,
-// tests/devmath_host.cu, the "warp" is the single caller.)
-IPA_HD bool ipa_any(bool v) {
+// Warp-wide min / max of a signed 32-bit value (REDUX on the device; the host build of
+// tests/devmath_host.cu has a "warp" of one caller).
+IPA_HD int ipa_warp_min(int v) {
 #ifdef __CUDA_ARCH__
-  return __any_sync(IPA_FULL, v);
+  return __reduce_min_sync(IPA_FULL, v);
+#else
+  return v;
+#endif
+}
+IPA_HD int ipa_warp_max(int v) {
+#ifdef __CUDA_ARCH__
+  return __reduce_max_sync(IPA_FULL, v);
 #else
   return v;
 #endif
 }
 
-// FP64 instructions per event (SASS): d 1, region 2 DSETP; a warp whose events are all in the core
-// pays q 1 + sqrt 5 + t 1 + Horner ceil4(D+1) + 1, one whose events are all in a tail pays u 1 + log 11
-// + 2, a mixed warp pays both; then softplus 15 + 1 + 10, E_B 1, l 2.  The Horner loop runs over
-// groups of 4 coefficients (two 128-bit uniform shared loads per group, a[] is zero above the degree).
+// Core term of E events: Delta = sum_j a[j] t^j + (beta - k) d, t = tA sqrt(d^2 + delta^2) + tB.
+// Horner over groups of 4 coefficients (two 128-bit uniform shared loads per group; a[] is zero above
+// the degree).  FP64 per event: q 1 + sqrt 5 + t 1 + 4 ceil((D+1)/4) + 1.
+template <int E>
+IPA_HD void ipa_core_delta(const IpaSetConsts& c, const double (&d)[E], double (&Dl)[E]) {
+  double P[E];
+  if (c.mode == 0) {
+    const double d2 = c.delta2, tA = c.tA, tB = c.tB;
+    double t[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) { t[e] = fma(tA, ipa_fsqrt(fma(d[e], d[e], d2)), tB); P[e] = 0.0; }
+    for (int g = c.degree >> 2; g >= 0; --g) {
+      const double2 hi2 = *reinterpret_cast<const double2*>(c.a + 4 * g + 2);
+      const double2 lo2 = *reinterpret_cast<const double2*>(c.a + 4 * g);
+#pragma unroll
+      for (int e = 0; e < E; ++e) {
+        P[e] = fma(P[e], t[e], hi2.y);
+        P[e] = fma(P[e], t[e], hi2.x);
+        P[e] = fma(P[e], t[e], lo2.y);
+        P[e] = fma(P[e], t[e], lo2.x);
+      }
+    }
+  } else {
+    // direct mode (shapes the polynomial cannot cover): per-event Bessel evaluation, out of line
+    double dt[E], Pt[E];
+#pragma unroll
+    for (int e = 0; e < E; ++e) dt[e] = d[e];
+    ipa_direct_core(c, dt, Pt, E);
+#pragma unroll
+    for (int e = 0; e < E; ++e) P[e] = Pt[e];
+  }
+  const double bmk = c.bmk;
+#pragma unroll
+  for (int e = 0; e < E; ++e) Dl[e] = fma(bmk, d[e], P[e]);
+}
+
+// Per-event log-likelihood of E events per thread for one parameter set.  The region of a WHOLE WARP
+// is decided on the high 32 bits of its events (integer min / max in the thread, one REDUX each across
+// the warp, compared with the high words of the joins mu+d0, mu+d1): strictly inside the core, strictly
+// left or strictly right means every event of the warp is there, and that warp runs only the core
+// polynomial or only the tail logarithm, with uniform constants and no per-event select.  Any other
+// warp (mixed regions, an event within 2^-20 relative of a join, non-positive or NaN events) takes
+// the general path: both terms, selected per event on d = x - mu (joins belong to the core).
+// FP64 per event: d 1, E_B 1, softplus 27, plus core 8 + 4 ceil((D+1)/4) or tail 14 (general path: both + 4).
 template <int E, class Tab>
 IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l)[E], const Tab* tab) {
   double d[E], Dl[E];
-  const double mu = c.mu, d0 = c.d0, d1 = c.d1;
-  bool anyc = false, anyl = false, anyr = false;
+  const double mu = c.mu, kd = c.kd;
+  int hmin = ipa_hi(x[0]), hmax = hmin;
 #pragma unroll
-  for (int e = 0; e < E; ++e) {
-    d[e] = x[e] - mu;
-    const bool left = d[e] < d0, right = d[e] > d1;
-    anyl = anyl || left;
-    anyr = anyr || right;
-    anyc = anyc || !(left || right);                // NaN events take the core path and stay NaN
+  for (int e = 1; e < E; ++e) {
+    const int h = ipa_hi(x[e]);
+    hmin = h < hmin ? h : hmin;
+    hmax = h > hmax ? h : hmax;
   }
-  anyc = ipa_any(anyc);
-  anyl = ipa_any(anyl);
-  anyr = ipa_any(anyr);
-  const bool anyt = anyl || anyr;
-  const double kd = c.kd;
-  if (anyc) {
-    double P[E];
-    if (c.mode == 0) {
-      const double d2 = c.delta2, tA = c.tA, tB = c.tB;
-      double t[E];
+  hmin = ipa_warp_min(hmin);
+  hmax = ipa_warp_max(hmax);
 #pragma unroll
-      for (int e = 0; e < E; ++e) { t[e] = fma(tA, ipa_fsqrt(fma(d[e], d[e], d2)), tB); P[e] = 0.0; }
-      for (int g = c.degree >> 2; g >= 0; --g) {
-        const double2 hi2 = *reinterpret_cast<const double2*>(c.a + 4 * g + 2);
-        const double2 lo2 = *reinterpret_cast<const double2*>(c.a + 4 * g);
+  for (int e = 0; e < E; ++e) d[e] = x[e] - mu;
+  const bool sane = hmin > 0 && hmax < 0x7ff00000;      // positive, finite events only
+  if (sane && hmin > c.hxl && hmax < c.hxr) {
+    ipa_core_delta<E>(c, d, Dl);
+  } else if (sane && (hmax < c.hxl || hmin > c.hxr)) {
+    const double* q = (hmin > c.hxr) ? &c.uA1 : &c.uA0;
+    const double uA = q[0], uB = q[1], nT = q[2], cT = q[3];
 #pragma unroll
-        for (int e = 0; e < E; ++e) {
-          P[e] = fma(P[e], t[e], hi2.y);
-          P[e] = fma(P[e], t[e], hi2.x);
-          P[e] = fma(P[e], t[e], lo2.y);
-          P[e] = fma(P[e], t[e], lo2.x);
-        }
-      }
-    } else {
-      // direct mode (shapes the polynomial cannot cover): per-event Bessel evaluation, out of line
-      double dt[E], Pt[E];
+    for (int e = 0; e < E; ++e) Dl[e] = fma(-kd, d[e], fma(-nT, ipa_flog(fma(uA, d[e], uB), tab), cT));
+  } else {
+    const double d0 = c.d0, d1 = c.d1;
+    ipa_core_delta<E>(c, d, Dl);
 #pragma unroll
-      for (int e = 0; e < E; ++e) dt[e] = d[e];
-      ipa_direct_core(c, dt, Pt, E);
-#pragma unroll
-      for (int e = 0; e < E; ++e) P[e] = Pt[e];
-    }
-    const double bmk = c.bmk;
-#pragma unroll
-    for (int e = 0; e < E; ++e) Dl[e] = fma(bmk, d[e], P[e]);
-  }
-  if (anyt) {
-    // a warp whose tail events are all on one side reads that side's four constants once (uniform
-    // shared loads); only a warp straddling both tails selects per lane
-    if (!(anyl && anyr)) {
-      const double* q = anyr ? &c.uA1 : &c.uA0;
-      const double uA = q[0], uB = q[1], nT = q[2], cT = q[3];
-#pragma unroll
-      for (int e = 0; e < E; ++e) {
-        const double tl = fma(-kd, d[e], fma(-nT, ipa_flog(fma(uA, d[e], uB), tab), cT));
-        if ((d[e] < d0) || (d[e] > d1)) Dl[e] = tl;
-      }
-    } else {
-#pragma unroll
-      for (int e = 0; e < E; ++e) {
-        const bool left = d[e] < d0, right = d[e] > d1;
-        const double uA = left ? c.uA0 : c.uA1, uB = left ? c.uB0 : c.uB1;
-        const double nT = left ? c.n0 : c.n1, cT = left ? c.cT0 : c.cT1;
-        const double tl = fma(-kd, d[e], fma(-nT, ipa_flog(fma(uA, d[e], uB), tab), cT));
-        if (left || right) Dl[e] = tl;
-      }
+    for (int e = 0; e < E; ++e) {
+      const bool left = d[e] < d0, right = d[e] > d1;   // NaN events keep the core value (NaN)
+      const double uA = left ? c.uA0 : c.uA1, uB = left ? c.uB0 : c.uB1;
+      const double nT = left ? c.n0 : c.n1, cT = left ? c.cT0 : c.cT1;
+      const double tl = fma(-kd, d[e], fma(-nT, ipa_flog(fma(uA, d[e], uB), tab), cT));
+      if (left || right) Dl[e] = tl;
     }
   }
   const double eB0 = c.eB0;
@@ -166,8 +177,7 @@ IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l
     for (int e = 0; e < E; ++e) l[e] = fma(kd, d[e], eB0) + Dl[e];
   } else {
 #pragma unroll
-    for (int e = 0; e < E; ++e) l[e] = (fma(kd, d[e], eB0) + ipa_relu_bits(Dl[e])) +
-                                       ipa_flog_1to2(1.0 + ipa_fexp_neg(ipa_neg_abs_clamped(Dl[e])), tab);
+    for (int e = 0; e < E; ++e) l[e] = ipa_fsoftplus_add(fma(kd, d[e], eB0), Dl[e], tab);
   }
 }
 

@@ -44,6 +44,8 @@ struct alignas(16) IpaSetConsts {
   double beta, logG0, logG1, logNS, logref;  // for the generators / binned path: log I(d)
   double normS, normB;          // N_S, N_B (absolute)
   int32_t status, degree, mode, pure;
+  int32_t hxl, hxr, pad0, pad1; // high words of the joins in x, mu+d0 and mu+d1 (0 / -1 if not positive): region
+                                // classification of a whole warp by integer min/max of the events' high words
 };
 
 struct IpaProWork {
@@ -371,7 +373,8 @@ IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
   o.normB = NB;
   const double logNS = log(NSr) + w.logref;
   const bool pure = !(p.f < 1.0);
-  const double cS = log(p.f) - logNS;  // -inf at f = 0
+  // f = 0: a finite, hugely negative signal term (softplus(-1e9) == 0 exactly) instead of -inf
+  const double cS = (p.f > 0.0) ? log(p.f) - logNS : -1.0e9;
   const double kd = pure ? 0.0 : p.k;
   const double eB0 = pure ? 0.0 : (p.k * (p.mu - w.lo) + log1p(-p.f) - log(NB));
   o.pure = pure ? 1 : 0;
@@ -385,6 +388,10 @@ IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
   o.fsig = p.f; o.kraw = p.k;
   o.beta = p.beta; o.logG0 = w.logG0; o.logG1 = w.logG1; o.logNS = logNS; o.logref = w.logref;
   o.araw0 = w.mode ? 0.0 : w.araw[0];
+  const double xl = p.mu + w.d0, xr = p.mu + w.d1;
+  o.hxl = (xl > 0.0) ? ipa_hi(xl) : 0;
+  o.hxr = (xr > 0.0) ? ipa_hi(xr) : -1;
+  o.pad0 = o.pad1 = 0;
 }
 // phase 13: coefficients (threads 0..47), after phase 12
 IPA_HD void ipa_pro_phase13(IpaProWork& w, IpaSetConsts& o, int k) {
