@@ -22,7 +22,11 @@
 __constant__ double ipa_c_exp[IPA_EXP_DEG + 1] = IPA_EXP_COEFS;
 __constant__ double ipa_c_log1p[IPA_LOG_DEG] = IPA_LOG1P_COEFS;
 __constant__ double2 ipa_c_logtab[33] = IPA_LOG_TABLE;
+__constant__ double ipa_c_gl16x[16] = IPA_GL16_X;
+__constant__ double ipa_c_gl16w[16] = IPA_GL16_W;
 // host copies (tests/devmath_host.cu only)
+static const double ipa_h_gl16x[16] = IPA_GL16_X;
+static const double ipa_h_gl16w[16] = IPA_GL16_W;
 struct ipa_host_double2 { double x, y; };
 static const double ipa_h_exp[IPA_EXP_DEG + 1] = IPA_EXP_COEFS;
 static const double ipa_h_log1p[IPA_LOG_DEG] = IPA_LOG1P_COEFS;
@@ -30,7 +34,11 @@ static const ipa_host_double2 ipa_h_logtab[33] = IPA_LOG_TABLE;
 #ifdef __CUDA_ARCH__
 #define IPA_CEXP(j) ipa_c_exp[j]
 #define IPA_CLOG(j) ipa_c_log1p[j]
+#define IPA_GL16X(i) ipa_c_gl16x[i]
+#define IPA_GL16W(i) ipa_c_gl16w[i]
 #else
+#define IPA_GL16X(i) ipa_h_gl16x[i]
+#define IPA_GL16W(i) ipa_h_gl16w[i]
 #define IPA_CEXP(j) ipa_h_exp[j]
 #define IPA_CLOG(j) ipa_h_log1p[j]
 #endif

@@ -64,9 +64,11 @@ struct IpaProWork {
   double bpart[IPA_NBTASK][IPA_SUB];
   double Ks[IPA_NBTASK];        // scaled Bessel values e^z K(z) of the tasks
   double H[IPA_MCHEB], c[IPA_MCHEB];
+  double ctab[4 * IPA_MCHEB];   // cos(pi m / (2 M)), m = 0 .. 4M-1 (Chebyshev nodes and the cosine transform)
+  double tl_left, tl_right, NB, logNB, logf, log1mf, nulogalpha, expref;   // pieces of phase 12 computed by other warps in phase 11
   int degree, mode;
-  long long T[3][IPA_NCOEF];    // integer coefficients of T_{j-1}, T_j, T_{j+1}
-  double ahi[IPA_NCOEF], alo[IPA_NCOEF], araw[IPA_NCOEF];
+  long long T[IPA_NCOEF][IPA_NCOEF];  // T[j][k] = integer coefficient of t^k in the Chebyshev polynomial T_j
+  double araw[IPA_NCOEF];
   double logG0, logG1, L0, L1;
   int npanel;
   double pa[IPA_MAXPANEL], pb[IPA_MAXPANEL], pval[IPA_MAXPANEL * IPA_GL], psum[IPA_MAXPANEL];
@@ -124,7 +126,7 @@ IPA_HD void ipa_pro_phase0(IpaProWork& w, int tid) {
 }
 
 // phase 1: partial trapezoid sums of K_lambda(zeta) (warp 0) and K_{lambda+1}(zeta) (warp 1);
-// threads 64..79 compute the Gauss-Legendre rule.
+// threads 64..79 copy the 16-point Gauss-Legendre rule from the generated table.
 IPA_HD void ipa_pro_phase1(IpaProWork& w, int tid) {
   if (w.status) return;
   if (tid < 64) {
@@ -141,7 +143,8 @@ IPA_HD void ipa_pro_phase1(IpaProWork& w, int tid) {
     }
     w.part[which][lane] = s;
   } else if (tid < 64 + IPA_GL) {
-    ipa_gauss_legendre(IPA_GL, tid - 64, &w.glx[tid - 64], &w.glw[tid - 64]);
+    w.glx[tid - 64] = IPA_GL16X(tid - 64);   // generated table (gen_fastmath_tables.py); IPA_GL == 16
+    w.glw[tid - 64] = IPA_GL16W(tid - 64);
   }
 }
 
@@ -170,8 +173,9 @@ IPA_HD void ipa_pro_phase2(IpaProWork& w, int tid) {
   const double o0 = fabs(w.nu), o1 = fabs(w.nu - 1.0), om = fmax(o0, o1);
   w.h = ipa_trap_step(om, zmax);
   // table length: smallest t with zmin (cosh t - 1) - om t > 46, by fixed-point iteration
-  double t = 1.0;
-  for (int it = 0; it < 6; ++it) t = acosh(1.0 + (46.0 + om * t) / zmin);
+  // (cosh t - 1 >= e^t / 2 - 1, so the root of  zmin (e^t/2 - 1) - om t = 46  is an upper bound)
+  double t = 4.0;
+  for (int it = 0; it < 4; ++it) t = log(2.0 * (1.0 + (46.0 + om * t) / zmin));
   int J = (int)(t / w.h) + 2;
   if (J > IPA_JMAX) J = IPA_JMAX;
   w.J = J;
@@ -181,6 +185,7 @@ IPA_HD void ipa_pro_phase2(IpaProWork& w, int tid) {
 // phase 3: trapezoid table (all threads)
 IPA_HD void ipa_pro_phase3(IpaProWork& w, int tid, int nthr) {
   if (w.status) return;
+  for (int m = tid; m < 4 * IPA_MCHEB; m += nthr) w.ctab[m] = cos(3.14159265358979323846 * (double)m / (double)(2 * IPA_MCHEB));
   for (int j = tid; j < w.J; j += nthr) {
     const double t = (double)j * w.h;
     const double s = sinh(0.5 * t);
@@ -194,7 +199,7 @@ IPA_HD void ipa_pro_phase3(IpaProWork& w, int tid, int nthr) {
 }
 
 IPA_HD double ipa_pro_task_z(const IpaProWork& w, int q) {
-  if (q < IPA_MCHEB) return w.zc + w.zh * cos(3.14159265358979323846 * ((double)q + 0.5) / (double)IPA_MCHEB);
+  if (q < IPA_MCHEB) return w.zc + w.zh * w.ctab[2 * q + 1];
   return ((q - IPA_MCHEB) & 1) ? w.z1 : w.z0;
 }
 
@@ -227,69 +232,71 @@ IPA_HD void ipa_pro_phase6(IpaProWork& w, int tid) {
   double s = 0.0;
   for (int i = 0; i < M; ++i) {
     const int m = (tid * (2 * i + 1)) % (4 * M);  // angle = pi m / (2M)
-    s += w.H[i] * cos(3.14159265358979323846 * (double)m / (double)(2 * M));
+    s += w.H[i] * w.ctab[m];
   }
   w.c[tid] = s * (tid == 0 ? 1.0 : 2.0) / (double)M;
 }
 
-// phase 7: degree selection, joins (one thread)
+// phase 7: degree selection (thread 0) and the two joins (threads 32 and 64, other warps)
 IPA_HD void ipa_pro_phase7(IpaProWork& w, int tid) {
-  if (w.status || tid != 0) return;
+  if (w.status) return;
   const ipa_params& p = w.p;
-  double scale = 1.0;
-  for (int i = 0; i < IPA_MCHEB; ++i) scale = fmax(scale, fabs(w.H[i]));
-  const double thr = 2.5e-16 * scale;
-  int D = IPA_MCHEB - 1;
-  while (D > 1 && fabs(w.c[D]) <= thr) --D;
-  // a-priori degree for a general order on this interval: the nearest singularity of H is z = 0
-  const double t0 = w.zc / w.zh;
-  const double rho = t0 + sqrt(t0 * t0 - 1.0);
-  int Dg = (int)ceil(37.0 / log(rho));
-  if (w.policy == 1 && D < Dg) D = Dg;
-  // conditioning of the power basis: needs rho comfortably above 1+sqrt(2)
-  if (D > IPA_NCOEF - 1 || rho < 2.6) { w.mode = 1; D = 0; }
-  w.degree = D;
-  const double K0 = w.Ks[IPA_MCHEB], K1 = w.Ks[IPA_MCHEB + 1], Km0 = w.Ks[IPA_MCHEB + 2], Km1 = w.Ks[IPA_MCHEB + 3];
-  w.logG0 = w.nu * log(w.r0) + p.beta * w.d0 + log(K0) - w.z0;
-  w.logG1 = w.nu * log(w.r1) + p.beta * w.d1 + log(K1) - w.z1;
-  w.L0 = p.beta - w.alpha * (w.d0 / w.r0) * (Km0 / K0);
-  w.L1 = p.beta - w.alpha * (w.d1 / w.r1) * (Km1 / K1);
+  if (tid == 0) {
+    double scale = 1.0;
+    for (int i = 0; i < IPA_MCHEB; ++i) scale = fmax(scale, fabs(w.H[i]));
+    const double thr = 2.5e-16 * scale;
+    int D = IPA_MCHEB - 1;
+    while (D > 1 && fabs(w.c[D]) <= thr) --D;
+    // a-priori degree for a general order on this interval: the nearest singularity of H is z = 0
+    const double t0 = w.zc / w.zh;
+    const double rho = t0 + sqrt(t0 * t0 - 1.0);
+    int Dg = (int)ceil(37.0 / log(rho));
+    if (w.policy == 1 && D < Dg) D = Dg;
+    // conditioning of the power basis: needs rho comfortably above 1+sqrt(2)
+    if (D > IPA_NCOEF - 1 || rho < 2.6) { w.mode = 1; D = 0; }
+    w.degree = D;
+  } else if (tid == 32) {
+    const double K0 = w.Ks[IPA_MCHEB], Km0 = w.Ks[IPA_MCHEB + 2];
+    w.logG0 = w.nu * log(w.r0) + p.beta * w.d0 + log(K0) - w.z0;
+    w.L0 = p.beta - w.alpha * (w.d0 / w.r0) * (Km0 / K0);
+  } else if (tid == 64) {
+    const double K1 = w.Ks[IPA_MCHEB + 1], Km1 = w.Ks[IPA_MCHEB + 3];
+    w.logG1 = w.nu * log(w.r1) + p.beta * w.d1 + log(K1) - w.z1;
+    w.L1 = p.beta - w.alpha * (w.d1 / w.r1) * (Km1 / K1);
+  }
+}
+// phase 7b: tail validity (after a barrier)
+IPA_HD void ipa_pro_phase7b(IpaProWork& w, int tid) {
+  if (w.status || tid != 0) return;
   if (!(w.L0 > 0.0) || !(w.L1 < 0.0)) w.status = 2;
 }
 
-// phase 8: Chebyshev -> monomial.  Step j (0..D): thread k holds the integer coefficient of t^k in
-// T_j and adds c_j T_{j,k} to a_k in double-double.  T_{j+1,k} = 2 T_{j,k-1} - T_{j-1,k} (exact in
-// int64 up to degree 47: |T_{47,k}| < 2^59).
-IPA_HD void ipa_pro_phase8_step(IpaProWork& w, int j, int k) {
+// phase 8: Chebyshev -> monomial, a_k = sum_j c_j T[j][k].
+// (a) integer table: row j from rows j-1 and j-2, T[j][k] = 2 T[j-1][k-1] - T[j-2][k]  (exact in int64 up
+//     to degree 47: |T[47][k]| < 2^59); one warp, one row per step.
+// (b) thread k accumulates its coefficient over the rows of matching parity in double-double.
+IPA_HD void ipa_pro_phase8_row(IpaProWork& w, int j, int k) {
   if (w.status || w.mode || k >= IPA_NCOEF) return;
-  long long* Tm = w.T[(j + 2) % 3];  // T_{j-1}
-  long long* Tc = w.T[j % 3];        // T_j   (written in this step)
-  const long long* Tp = w.T[(j + 1) % 3];  // T_{j-2} ... see below
   long long v;
-  if (j == 0) {
-    v = (k == 0) ? 1 : 0;
-    w.ahi[k] = 0.0;
-    w.alo[k] = 0.0;
-  } else if (j == 1) {
-    v = (k == 1) ? 1 : 0;
-  } else {
-    // T_j,k = 2 T_{j-1,k-1} - T_{j-2,k}
-    v = (k > 0 ? 2 * Tm[k - 1] : 0) - Tp[k];
-  }
-  Tc[k] = v;
-  if (v != 0 && j <= w.degree) {
-    double ph, pl, sh, sl;
-    ipa_two_prod(w.c[j], (double)v, &ph, &pl);
-    ipa_two_sum(w.ahi[k], ph, &sh, &sl);
-    sl += w.alo[k] + pl;
-    const double hi = sh + sl;
-    w.alo[k] = sl - (hi - sh);
-    w.ahi[k] = hi;
-  }
+  if (j == 0) v = (k == 0) ? 1 : 0;
+  else if (j == 1) v = (k == 1) ? 1 : 0;
+  else v = (k > 0 ? 2 * w.T[j - 1][k - 1] : 0) - w.T[j - 2][k];
+  w.T[j][k] = v;
 }
 IPA_HD void ipa_pro_phase8_finish(IpaProWork& w, int k) {
   if (w.status || w.mode || k >= IPA_NCOEF) return;
-  w.araw[k] = (k <= w.degree) ? w.ahi[k] + w.alo[k] : 0.0;
+  double ahi = 0.0, alo = 0.0;
+  for (int j = k; j <= w.degree; j += 2) {
+    const long long v = w.T[j][k];
+    double ph, pl, sh, sl;
+    ipa_two_prod(w.c[j], (double)v, &ph, &pl);
+    ipa_two_sum(ahi, ph, &sh, &sl);
+    sl += alo + pl;
+    const double hi = sh + sl;
+    alo = sl - (hi - sh);
+    ahi = hi;
+  }
+  w.araw[k] = (k <= w.degree) ? ahi + alo : 0.0;
 }
 
 // phase 9: range, panels, reference level (one thread)
@@ -332,10 +339,41 @@ IPA_HD void ipa_pro_phase10(IpaProWork& w, int tid, int nthr) {
   }
 }
 IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
-  if (w.status || tid >= w.npanel) return;
-  double s = 0.0;
-  for (int i = 0; i < IPA_GL; ++i) s += w.pval[tid * IPA_GL + i];
-  w.psum[tid] = s;
+  if (w.status) return;
+  const ipa_params& p = w.p;
+  if (tid < w.npanel) {
+    double s = 0.0;
+    for (int i = 0; i < IPA_GL; ++i) s += w.pval[tid * IPA_GL + i];
+    w.psum[tid] = s;
+  } else if (tid == 32) {          // left tail integral in units of exp(logref)  (reading C5)
+    double left = 0.0;
+    if (w.dl < w.d0) {
+      const double dr = fmin(w.d0, w.dh);
+      const double ul = 1.0 - (w.dl - w.d0) * w.L0 / p.n, ur = 1.0 - (dr - w.d0) * w.L0 / p.n;
+      left = exp(w.logG0 - w.logref) * (p.n / w.L0) * (ipa_powint(ul, p.n) - ipa_powint(ur, p.n));
+    }
+    w.tl_left = left;
+  } else if (tid == 64) {          // right tail integral
+    double right = 0.0;
+    if (w.dh > w.d1) {
+      const double dL = fmax(w.d1, w.dl);
+      const double uh = 1.0 - (w.dh - w.d1) * w.L1 / p.n2, ul = 1.0 - (dL - w.d1) * w.L1 / p.n2;
+      right = exp(w.logG1 - w.logref) * (p.n2 / (-w.L1)) * (ipa_powint(uh, p.n2) - ipa_powint(ul, p.n2));
+    }
+    w.tl_right = right;
+  } else if (tid == 96) {          // background normalisation (shifted by lo)
+    const double wd = w.hi - w.lo, tk = p.k * wd;
+    const double NB = (fabs(tk) < 1e-8) ? wd * (1.0 + 0.5 * tk + tk * tk / 6.0) : expm1(tk) / p.k;
+    w.NB = NB;
+    w.logNB = log(NB);
+  } else if (tid == 128) {
+    w.logf = (p.f > 0.0) ? log(p.f) : 0.0;
+    w.log1mf = (p.f < 1.0) ? log1p(-p.f) : 0.0;
+  } else if (tid == 160) {
+    w.nulogalpha = w.nu * log(w.alpha);
+  } else if (tid == 192) {
+    w.expref = exp(w.logref);
+  }
 }
 
 // phase 12: normalisations and folded constants (one thread writes the header of the record)
@@ -350,33 +388,22 @@ IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
   const ipa_params& p = w.p;
   double core = 0.0;
   for (int i = 0; i < w.npanel; ++i) core += w.psum[i];
-  double left = 0.0, right = 0.0;
-  if (w.dl < w.d0) {
-    const double dr = fmin(w.d0, w.dh);
-    const double ul = 1.0 - (w.dl - w.d0) * w.L0 / p.n, ur = 1.0 - (dr - w.d0) * w.L0 / p.n;
-    left = exp(w.logG0 - w.logref) * (p.n / w.L0) * (ipa_powint(ul, p.n) - ipa_powint(ur, p.n));
-  }
-  if (w.dh > w.d1) {
-    const double dL = fmax(w.d1, w.dl);
-    const double uh = 1.0 - (w.dh - w.d1) * w.L1 / p.n2, ul = 1.0 - (dL - w.d1) * w.L1 / p.n2;
-    right = exp(w.logG1 - w.logref) * (p.n2 / (-w.L1)) * (ipa_powint(uh, p.n2) - ipa_powint(ul, p.n2));
-  }
+  const double left = w.tl_left, right = w.tl_right;
   const double NSr = left + core + right;  // in units of exp(logref)
-  const double wd = w.hi - w.lo, tk = p.k * wd;
-  const double NB = (fabs(tk) < 1e-8) ? wd * (1.0 + 0.5 * tk + tk * tk / 6.0) : expm1(tk) / p.k;
+  const double NB = w.NB;
   if (!(NSr > 0.0) || !ipa_finite(NSr) || !(NB > 0.0) || !ipa_finite(NB)) {
     w.status = 3;
     o.status = 3;
     return;
   }
-  o.normS = NSr * exp(w.logref);
+  o.normS = NSr * w.expref;
   o.normB = NB;
   const double logNS = log(NSr) + w.logref;
   const bool pure = !(p.f < 1.0);
   // f = 0: a finite, hugely negative signal term (softplus(-1e9) == 0 exactly) instead of -inf
-  const double cS = (p.f > 0.0) ? log(p.f) - logNS : -1.0e9;
+  const double cS = (p.f > 0.0) ? w.logf - logNS : -1.0e9;
   const double kd = pure ? 0.0 : p.k;
-  const double eB0 = pure ? 0.0 : (p.k * (p.mu - w.lo) + log1p(-p.f) - log(NB));
+  const double eB0 = pure ? 0.0 : (p.k * (p.mu - w.lo) + w.log1mf - w.logNB);
   o.pure = pure ? 1 : 0;
   o.mu = p.mu; o.d0 = w.d0; o.d1 = w.d1; o.delta2 = w.delta * w.delta;
   o.tA = w.alpha / w.zh; o.tB = -w.zc / w.zh;
@@ -384,7 +411,7 @@ IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
   o.uA0 = -w.L0 / p.n;  o.uB0 = 1.0 + w.d0 * w.L0 / p.n;  o.n0 = p.n;  o.cT0 = w.logG0 + cS - eB0;
   o.uA1 = -w.L1 / p.n2; o.uB1 = 1.0 + w.d1 * w.L1 / p.n2; o.n1 = p.n2; o.cT1 = w.logG1 + cS - eB0;
   o.alpha = w.alpha; o.nu = w.nu;
-  o.cDir = cS - eB0 - w.nu * log(w.alpha);
+  o.cDir = cS - eB0 - w.nulogalpha;
   o.fsig = p.f; o.kraw = p.k;
   o.beta = p.beta; o.logG0 = w.logG0; o.logG1 = w.logG1; o.logNS = logNS; o.logref = w.logref;
   o.araw0 = w.mode ? 0.0 : w.araw[0];

@@ -21,8 +21,9 @@ static void run_prologue_host(const ipa_params& p, double lo, double hi, int pol
   ALL(ipa_pro_phase5(w, tid))
   ALL(ipa_pro_phase6(w, tid))
   ALL(ipa_pro_phase7(w, tid))
+  ALL(ipa_pro_phase7b(w, tid))
   if (!w.status && !w.mode)
-    for (int j = 0; j <= w.degree; ++j) { ALL(ipa_pro_phase8_step(w, j, tid)) }
+    for (int j = 0; j <= w.degree; ++j) { ALL(ipa_pro_phase8_row(w, j, tid)) }
   ALL(ipa_pro_phase8_finish(w, tid))
   ALL(ipa_pro_phase9(w, tid))
   ALL(ipa_pro_phase10(w, tid, NT))
@@ -60,6 +61,13 @@ void emu_logI(const ipa_params* p, double lo, double hi, const double* d, long l
 }
 void emu_uniforms2(unsigned long long seed, unsigned long long slot, unsigned attempt, unsigned stream, double* u) {
   ipa_uniforms2(seed, slot, attempt, stream, u, u + 1);
+}
+// generated 16-point Gauss-Legendre table against the in-source Newton iteration on P_16
+void emu_gl16(double* tab_x, double* tab_w, double* newton_x, double* newton_w) {
+  for (int i = 0; i < 16; ++i) {
+    tab_x[i] = IPA_GL16X(i); tab_w[i] = IPA_GL16W(i);
+    ipa_gauss_legendre(16, i, &newton_x[i], &newton_w[i]);
+  }
 }
 long long emu_poisson(unsigned long long seed, unsigned long long slot, unsigned stream, double mean) {
   return ipa_poisson(seed, slot, stream, mean);

@@ -143,3 +143,19 @@ def test_device_generators_vs_oracle(emu, orc):
     for mean in (0.5, 5.0, 9.99, 10.0, 50.0, 3.0e4, 7.0e4, 1.0e5):
         for slot in range(300):
             assert emu.emu_poisson(1234, slot, 3, mean) == orc.poisson(1234, slot, 3, mean)
+
+
+def test_gauss_legendre_table(emu):
+    """The prologue's generated 16-point rule: equals Newton on P_16 and numpy's leggauss, integrates
+    polynomials of degree <= 31 exactly."""
+    import ctypes as C
+    arr = [np.zeros(16) for _ in range(4)]
+    emu.emu_gl16.restype = None
+    emu.emu_gl16.argtypes = [C.c_void_p] * 4
+    emu.emu_gl16(*[a.ctypes.data_as(C.c_void_p) for a in arr])
+    tx, tw, nx, nw = arr
+    assert np.abs(tx - nx).max() < 5e-16 and np.abs(tw - nw).max() < 5e-16
+    gx, gw = np.polynomial.legendre.leggauss(16)
+    assert np.abs(np.sort(tx) - gx).max() < 5e-16 and np.abs(tw[np.argsort(tx)] - gw).max() < 5e-16
+    for deg in (0, 2, 30):
+        assert abs((tw * tx ** deg).sum() - 2.0 / (deg + 1)) < 1e-15
