@@ -264,7 +264,8 @@ int ipa_hist_fill(const double* x_dev, int64_t n, ipa_range r, int nbins, uint64
   if (n == 0) return IPA_OK;
   int64_t G = (n + 255) / 256;
   if (G > (int64_t)sms * 8) G = (int64_t)sms * 8;
-  ipa_hist_kernel<<<(unsigned)G, 256, 0, st>>>(x_dev, n, r.lo, r.hi, nbins,
+  const size_t hsmem = nbins <= IPA_HIST_SMEM_BINS ? (size_t)nbins * 4 : 0;
+  ipa_hist_kernel<<<(unsigned)G, 256, hsmem, st>>>(x_dev, n, r.lo, r.hi, nbins,
                                                reinterpret_cast<unsigned long long*>(counts_dev));
   IPA_CK(cudaGetLastError());
   return IPA_OK;

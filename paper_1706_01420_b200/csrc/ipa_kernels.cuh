@@ -349,14 +349,33 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
 // Segmented NLL (T2): grid (T, IPA_SEGC); block (t, c) takes the c-th eighth of segment t with the
 // parameter set of that segment.
 // ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void ipa_cp_async8(void* smem_dst, const void* gmem_src) {
+  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
+  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
+}
+
+// Same staging as the streaming kernel, with 8-byte copies (a segment starts at any event index): the copy
+// of the next tile flies while the current one is evaluated; each thread reads only its own slots.
 __global__ void __launch_bounds__(IPA_BLOCK, IPA_BLOCKS_PER_SM)
 ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ offsets,
                    const IpaSetConsts* __restrict__ consts, double* __restrict__ partials) {
   __shared__ IpaSetConsts c;
   __shared__ double red[IPA_BLOCK / 32];
   __shared__ double2 s_tab[33];
+  __shared__ __align__(16) double stage[2][IPA_TILE];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const long long t = blockIdx.x;
+  const long long beg = offsets[t], len = offsets[t + 1] - beg;
+  const long long cb = beg + len * blockIdx.y / IPA_SEGC, ce = beg + len * (blockIdx.y + 1) / IPA_SEGC;
+  auto issue = [&](long long base, int buf) {
+#pragma unroll
+    for (int e = 0; e < IPA_E; ++e) {
+      const long long i = base + e * IPA_BLOCK + tid;
+      if (i < ce) ipa_cp_async8(&stage[buf][e * IPA_BLOCK + tid], x + i);
+    }
+    ipa_cp_async_commit();
+  };
+  if (cb < ce) issue(cb, 0);
   {
     const double* src = reinterpret_cast<const double*>(consts + t);
     double* dst = reinterpret_cast<double*>(&c);
@@ -364,25 +383,25 @@ ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ o
     ipa_load_logtab(s_tab);
   }
   __syncthreads();
-  const long long beg = offsets[t], len = offsets[t + 1] - beg;
-  const long long cb = beg + len * blockIdx.y / IPA_SEGC, ce = beg + len * (blockIdx.y + 1) / IPA_SEGC;
   double acc = 0.0;
   if (!c.status) {
-    for (long long base = cb; base < ce; base += IPA_TILE) {
+    const double filler = c.mu;   // masked slots of a ragged tile: any finite value, the result is dropped
+    int buf = 0;
+    for (long long base = cb; base < ce; base += IPA_TILE, buf ^= 1) {
       double xv[IPA_E], l[IPA_E];
-      long long idx[IPA_E];
+      ipa_cp_async_wait_all();
 #pragma unroll
-      for (int e = 0; e < IPA_E; ++e) {
-        idx[e] = base + e * IPA_BLOCK + tid;
-        xv[e] = (idx[e] < ce) ? __ldcs(x + idx[e]) : 0.0;
-      }
+      for (int e = 0; e < IPA_E; ++e)
+        xv[e] = (base + e * IPA_BLOCK + tid < ce) ? stage[buf][e * IPA_BLOCK + tid] : filler;
+      if (base + IPA_TILE < ce) issue(base + IPA_TILE, buf ^ 1);
       ipa_eval_set<IPA_E>(c, xv, l, s_tab);
       double s = 0.0;
 #pragma unroll
-      for (int e = 0; e < IPA_E; ++e) s += (idx[e] < ce) ? l[e] : 0.0;
+      for (int e = 0; e < IPA_E; ++e) s += (base + e * IPA_BLOCK + tid < ce) ? l[e] : 0.0;
       acc += s;
     }
   }
+  ipa_cp_async_wait_all();
   acc = ipa_warp_sum(acc);
   if (lane == 0) red[warp] = acc;
   __syncthreads();
@@ -546,26 +565,48 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
 // Integer work: exact and order-independent.
 // ------------------------------------------------------------------------------------------------
 #define IPA_HIST_SMEM_BINS 8192
+#define IPA_HIST_UNROLL 4
+// HBM-bound (8 B per event, nothing else): every thread keeps IPA_HIST_UNROLL 128-bit streaming loads in
+// flight (64 B per thread, 128 KB per SM at full occupancy) before it touches the counters.
 __global__ void __launch_bounds__(256)
 ipa_hist_kernel(const double* __restrict__ x, long long n, double lo, double hi, int nbins,
                 unsigned long long* __restrict__ counts) {
-  __shared__ unsigned int sh[IPA_HIST_SMEM_BINS];
+  extern __shared__ unsigned int sh[];   // nbins counters when nbins <= IPA_HIST_SMEM_BINS, else unused
   const bool priv = nbins <= IPA_HIST_SMEM_BINS;
   if (priv) {
     for (int b = threadIdx.x; b < nbins; b += blockDim.x) sh[b] = 0u;
     __syncthreads();
   }
   const double scale = (double)nbins / (hi - lo);
-  const long long stride = (long long)gridDim.x * blockDim.x;
-  // a block handles at most 2^31 events between flushes (32-bit private counters): n / gridDim is far below that
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < n; i += stride) {
-    const double xi = __ldcs(x + i);
+  auto count = [&](double xi) {
     const double t = (xi - lo) * scale;
-    if (!(t >= 0.0) || !(xi <= hi)) continue;
+    if (!(t >= 0.0) || !(xi <= hi)) return;
     int b = (int)t;
     if (b >= nbins) b = nbins - 1;
     if (priv) atomicAdd(&sh[b], 1u);
     else atomicAdd(&counts[b], 1ull);
+  };
+  // a block handles at most 2^31 events between flushes (32-bit private counters): n / gridDim is far below that
+  const long long head = (n > 0 && ((unsigned long long)x & 8ull)) ? 1 : 0;   // 16-byte alignment of the body
+  const double2* x2 = reinterpret_cast<const double2*>(x + head);
+  const long long n2 = (n - head) / 2;
+  const long long stride = (long long)gridDim.x * blockDim.x;
+  long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x;
+  for (; i + (IPA_HIST_UNROLL - 1) * stride < n2; i += IPA_HIST_UNROLL * stride) {
+    double2 v[IPA_HIST_UNROLL];
+#pragma unroll
+    for (int u = 0; u < IPA_HIST_UNROLL; ++u) v[u] = __ldcs(x2 + i + u * stride);
+#pragma unroll
+    for (int u = 0; u < IPA_HIST_UNROLL; ++u) { count(v[u].x); count(v[u].y); }
+  }
+  for (; i < n2; i += stride) {
+    const double2 v = __ldcs(x2 + i);
+    count(v.x);
+    count(v.y);
+  }
+  if (blockIdx.x == 0 && threadIdx.x == 0) {
+    if (head) count(x[0]);
+    if (head + 2 * n2 < n) count(x[n - 1]);
   }
   if (priv) {
     __syncthreads();

@@ -352,3 +352,78 @@ def test_full_size_sampled(ipa, torch_, orc):
     assert np.abs(lps[0][sel].cpu().numpy() - orc.logpdf(xs[sel].cpu().numpy(), inp.GEN, LO, HI)).max() <= 1e-10
     parts, _, _ = ipa.ipa_nll_eval(ipa.ipa_events_sort(xd[:20_000_000]), batch[:3], LO, HI)
     assert np.all(np.abs(parts.cpu().numpy() - ref) <= 1e-10 * np.abs(ref))
+
+
+# ---------------------------------------------------------------------------------------------
+# full size, config 4 (1000 toys x ~1e5 events generated on the device, one segmented launch) and
+# config 5 (1e8 events -> 1000 bins, 100 x 100 scan, 10 000 Poisson toy histograms)
+# ---------------------------------------------------------------------------------------------
+def test_config4_full_size_sampled(ipa, torch_, orc):
+    T = 1000
+    seeds = inp.toy_seeds(T)
+    ms, mb = 30000.0, 70000.0
+    _, off_ref = orc.toy_generate(seeds, inp.GEN, ms, mb, LO, HI, offsets_only=True)
+    cap = int(off_ref[-1])
+    x, off, ovf = ipa.ipa_toy_generate(seeds, inp.GEN, ms, mb, LO, HI, cap)
+    sets = inp.toy_param_sets(T)
+    nll, st = ipa.ipa_nll_eval_segmented(x, off, sets, LO, HI)
+    xs = ipa.ipa_events_sort(x, off)
+    nll_s, _ = ipa.ipa_nll_eval_segmented(xs, off, sets, LO, HI)
+    torch_.cuda.synchronize()
+    assert ovf.item() == 0 and np.array_equal(off.cpu().numpy(), off_ref)      # all 1000 Poisson yields: bit-exact
+    assert abs(cap - 1e8) < 5e5
+    nll, nll_s = nll.cpu().numpy(), nll_s.cpu().numpy()
+    assert (st.cpu().numpy() == 0).all()
+    assert np.all(np.abs(nll - nll_s) <= 1e-12 * np.abs(nll))                  # per-toy sort: rounding only
+    pick = [0, 1, 137, 499, 998, 999]
+    # events of the sampled toys against the oracle's generator (same seeds -> same counters)
+    x_ref, o_ref = orc.toy_generate(seeds[pick], inp.GEN, ms, mb, LO, HI)
+    for j, t in enumerate(pick):
+        got = x[off_ref[t]:off_ref[t + 1]].cpu().numpy()
+        ref = x_ref[o_ref[j]:o_ref[j + 1]]
+        assert got.size == ref.size
+        assert (np.abs(got - ref) <= 1e-9).mean() >= 1 - 1e-4
+        # NLL of the toy with its own parameter set, oracle on the GPU-generated events
+        r = orc.nll(got, sets[t], LO, HI)[0]
+        assert abs(nll[t] - r) <= 1e-10 * abs(r), t
+        single, _, _ = ipa.ipa_nll_eval(x[off_ref[t]:off_ref[t + 1]], sets[t], LO, HI)
+        assert abs(single.item() - nll[t]) <= 1e-12 * abs(nll[t])
+    # property at full size: every toy's NLL per event sits at the population value 6.09 +- 5 sigma
+    per_event = nll / np.diff(off_ref)
+    assert np.all(np.abs(per_event - 6.0901) < 0.02)
+
+
+def test_config5_full_size(ipa, torch_, orc):
+    n, nbins = 100_000_000, 1000
+    x = inp.standin_masses(5, n, f=2.5e-5)
+    xd = dev(torch_, x)
+    counts = ipa.ipa_hist_fill(xd, LO, HI, nbins)
+    torch_.cuda.synchronize()
+    c_ref = orc.hist_fill(x, LO, HI, nbins)
+    got = counts.cpu().numpy().astype(np.uint64)
+    assert np.array_equal(got, c_ref) and int(got.sum()) == n                  # integer work: exact
+    cm = ipa.ipa_hist_fill(xd[1:], LO, HI, nbins)                              # 8-byte-aligned start: scalar head
+    assert np.array_equal(cm.cpu().numpy().astype(np.uint64), orc.hist_fill(x[1:], LO, HI, nbins))
+    del xd
+    ns, nb, kk = inp.scan_grid(100, 100, n_obs=float(n))
+    scan = ipa.ipa_binned_nll_scan(counts, LO, HI, inp.GEN, ns, nb, kk)
+    torch_.cuda.synchronize()
+    scan = scan.cpu().numpy()
+    ref = orc.binned_nll_scan(c_ref, LO, HI, inp.GEN, ns, nb, kk)
+    assert np.all(np.abs(scan - ref) <= 1e-10 * np.abs(ref))
+    # 10 000 toy histograms: 5 000 background-only at the best k, 5 000 with ns = 2500 (reading D16)
+    kbest = kk[int(np.argmin(ref))]
+    seeds = np.arange(1, 10001, dtype=np.uint64)
+    for ns_gen, sd in ((0.0, seeds[:5000]), (2500.0, seeds[5000:])):
+        nu = ipa.ipa_expected_hist(nbins, LO, HI, inp.GEN, ns_gen, n - ns_gen, kbest)
+        toys = ipa.ipa_poisson_hist_toys(nu, sd)
+        torch_.cuda.synchronize()
+        nu_ref = orc.expected_hist(nbins, LO, HI, inp.GEN, ns_gen, n - ns_gen, kbest)
+        assert np.all(np.abs(nu.cpu().numpy() - nu_ref) <= 1e-12 * nu_ref)
+        t = toys.cpu().numpy().astype(np.uint32)
+        sample = np.array([0, 1, 2499, 4999])
+        ref_t = orc.poisson_hist_toys(nu_ref, sd[sample])
+        assert (t[sample] == ref_t).mean() >= 1 - 1e-4
+        # property over all toys: pulls of the counts are standard normal
+        pull = (t.astype(np.float64) - nu_ref[None, :]) / np.sqrt(nu_ref[None, :])
+        assert abs(pull.mean()) < 3e-3 and abs(pull.std() - 1.0) < 3e-3
