@@ -131,6 +131,89 @@ def run_reference(args):
     print(json.dumps(line))
 
 
+def other_rows(torch, ipa, x, ws, stream, n):
+    """The other rows of SURVEY.md 8(a), timed at BASELINE.json's sizes in the same run (device time, CUDA events):
+    config 2 (fit loop on 1e6 events), config 4 (toys), config 5 (binned path).  Reported beside the headline;
+    parity of each is in tests/ (-m gpu)."""
+    from paper_1706_01420_b200 import minimiser
+    out = {}
+    peaks_hbm = 6650.0
+    try:
+        peaks_hbm = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+    except Exception:
+        pass
+
+    def t(fn, steps, warm=2):
+        for _ in range(warm):
+            fn()
+        return timed(torch, fn, steps, stream) / steps
+
+    # config 2: host minimiser loop, 1e6 events (seed 2), floating (mu, sigma, f, k)
+    n2 = min(1_000_000, n)
+    x2, _, _ = ipa.ipa_toy_generate([2], inp.GEN, -1.0, -1.0, LO, HI, n2)
+    x2 = ipa.ipa_events_sort(x2)
+    ws2 = ipa.workspace(n2, 32)
+    th0 = inp.as_array(inp.GEN)
+    for name, d in inp.FIT_START_SHIFT.items():
+        th0[inp.IDX[name]] += d
+
+    def nll_batch(th):
+        return ipa.ipa_nll_eval(x2, th, LO, HI, ws=ws2, stream=stream)[0].cpu().numpy()
+    minimiser.minimise(nll_batch, th0, inp.FLOATED, inp.FD_STEPS, inp.GRAD_SCALE)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    res = minimiser.minimise(nll_batch, th0, inp.FLOATED, inp.FD_STEPS, inp.GRAD_SCALE)
+    wall = time.perf_counter() - t0
+    b9, _ = inp.fd_batch(inp.GEN)
+    o9 = torch.empty(9, dtype=torch.float64, device="cuda")
+    d9 = t(lambda: ipa.ipa_nll_eval(x2, b9, LO, HI, ws=ws2, stream=stream, out=o9), 200, 10)
+    out["config2_fit_1e6_events"] = {
+        "wall_s": wall, "nll_evaluations": res.n_evals, "batched_calls": res.n_calls, "edm": res.edm,
+        "nll_evaluations_per_s_wall": res.n_evals / wall, "k9_call_ms_device": d9 * 1e3,
+        "nll_evaluations_per_s_device_k9": 9 / d9,
+        "fitted": {k: res.par[k] for k in inp.FLOATED}, "errors": {k: res.errors[k] for k in inp.FLOATED}}
+
+    # config 4: 1000 toys x ~1e5 events generated on the device, one segmented launch
+    T = 1000
+    seeds = inp.toy_seeds(T)
+    cap = 101_000_000
+    if n >= 100_000_000:
+        xt = torch.empty(cap, dtype=torch.float64, device="cuda")
+        wst = ipa.workspace(cap, T)
+        holder = {}
+
+        def gen():
+            holder["off"] = ipa.ipa_toy_generate(seeds, inp.GEN, 30000.0, 70000.0, LO, HI, cap, ws=wst, x=xt, stream=stream)[1]
+        dg = t(gen, 3, 1)
+        off = holder["off"]
+        ntot = int(off[-1].item())
+        sets = inp.toy_param_sets(T)
+        ds = t(lambda: ipa.ipa_nll_eval_segmented(xt, off, sets, LO, HI, ws=wst, stream=stream), 10)
+        xs = ipa.ipa_events_sort(xt[:ntot], off)
+        dss = t(lambda: ipa.ipa_nll_eval_segmented(xs, off, sets, LO, HI, ws=wst, stream=stream), 10)
+        out["config4_toys"] = {"toys": T, "events": ntot, "generate_ms": dg * 1e3, "generate_events_per_s": ntot / dg,
+                               "segmented_nll_ms": ds * 1e3, "segmented_nll_sorted_per_toy_ms": dss * 1e3,
+                               "toys_per_s_nll": T / dss, "events_per_s_nll": ntot / dss}
+        del xt, xs
+    # config 5: histogram (HBM-bound), 100 x 100 scan, 10 000 Poisson toy histograms
+    nbins = 1000
+    dh = t(lambda: ipa.ipa_hist_fill(x, LO, HI, nbins, stream=stream), 20)
+    counts = ipa.ipa_hist_fill(x, LO, HI, nbins, stream=stream)
+    ns, nb, kk = inp.scan_grid(100, 100, n_obs=float(n))
+    ws5 = ipa.workspace(0, 10000, nbins)
+    dsc = t(lambda: ipa.ipa_binned_nll_scan(counts, LO, HI, inp.GEN, ns, nb, kk, ws=ws5, stream=stream), 20)
+    nu = ipa.ipa_expected_hist(nbins, LO, HI, inp.GEN, 2500.0, n - 2500.0, -0.002)
+    sd = np.arange(1, 10001, dtype=np.uint64)
+    dp = t(lambda: ipa.ipa_poisson_hist_toys(nu, sd, ws=ws5, stream=stream), 20)
+    out["config5_binned"] = {
+        "hist_fill_ms": dh * 1e3, "hist_events_per_s": n / dh,
+        "hist_roofline": {"bound": "hbm", "achieved": 8.0 * n / dh / 1e9, "peak": peaks_hbm, "unit": "GB/s",
+                          "frac": 8.0 * n / dh / 1e9 / peaks_hbm},
+        "scan_points": int(ns.size), "scan_ms": dsc * 1e3, "scan_points_per_s": ns.size / dsc,
+        "poisson_toy_histograms": int(sd.size), "poisson_toys_ms": dp * 1e3, "poisson_draws_per_s": sd.size * nbins / dp}
+    return out
+
+
 def timed(torch, fn, steps, stream):
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     torch.cuda.synchronize()
@@ -262,6 +345,7 @@ def main():
         extras["k1_general_shape_P2"] = {"ms_per_call": dtp * 1e3, "events_per_s": n / dtp}
         ipa.ipa_set_degree_policy(1)
         step_k1()
+        extras.update(other_rows(torch, ipa, x_asis, ws, stream, n))
         # FP64 peak probe (DFMA chains), for the roofline denominator
         iters = 200000
         ipa.ipa_fp64_peak_probe(1000)
