@@ -164,7 +164,12 @@ IPA_HD double ipa_fsoftplus_add(double eb, double D, const Tab* tab) {
   n = n > -1000 ? n : -1000;
   const double w = ipa_mk(ipa_hi(p) + (n << 20), ipa_lo(p));
   double l = eb + ipa_flog_1to2(1.0 + w, tab);
+#ifdef __CUDA_ARCH__
+  // predicated add on the sign word (the compiler would otherwise add and select: two more instructions)
+  asm("{\n\t.reg .pred p;\n\tsetp.ge.s32 p, %2, 0;\n\t@p add.f64 %0, %0, %1;\n\t}" : "+d"(l) : "d"(D), "r"(ipa_hi(D)));
+#else
   if (ipa_hi(D) >= 0) l += D;
+#endif
   return l;
 }
 

@@ -235,10 +235,52 @@ __device__ __forceinline__ void ipa_cp_async16(void* smem_dst, const void* gmem_
 __device__ __forceinline__ void ipa_cp_async_commit() { asm volatile("cp.async.commit_group;" ::: "memory"); }
 __device__ __forceinline__ void ipa_cp_async_wait_all() { asm volatile("cp.async.wait_group 0;" ::: "memory"); }
 
+__device__ __forceinline__ void ipa_cp_async16_s(unsigned smem_addr, const void* gmem_src) {
+  asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(smem_addr), "l"(gmem_src) : "memory");
+}
+__device__ __forceinline__ double2 ipa_lds128(unsigned smem_addr) {
+  double2 v;
+  asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(v.x), "=d"(v.y) : "r"(smem_addr) : "memory");
+  return v;
+}
+
+// All K parameter sets on the IPA_NE events a thread holds in registers (A2-A4), optional per-event
+// output, accumulation into the thread's shared-memory accumulators (first level of A5).
+// Event e of thread tid in the tile at `base` is x[base + 2 ((e >> 1) IPA_NB + tid) + (e & 1)].
+template <bool LOGPDF, bool FULL>
+__device__ __forceinline__ void ipa_tile_sets(const IpaSetConsts* sc, int K, double* acc, const double (&xv)[IPA_NE],
+                                              long long base, long long n, int tid, double* __restrict__ logpdf,
+                                              const double2* s_tab) {
+  for (int k = 0; k < K; ++k) {
+    const IpaSetConsts& c = sc[k];
+    if (c.status) continue;
+    double l[IPA_NE];
+    ipa_eval_set<IPA_NE>(c, xv, l, s_tab);
+    if (!FULL) {
+#pragma unroll
+      for (int e = 0; e < IPA_NE; ++e) {
+        const long long i = base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1);
+        if (LOGPDF && i < n) logpdf[(long long)k * n + i] = l[e];
+        if (i >= n) l[e] = 0.0;
+      }
+    } else if (LOGPDF) {
+#pragma unroll
+      for (int e = 0; e < IPA_NE; ++e)
+        logpdf[(long long)k * n + base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1)] = l[e];
+    }
+    double sl = 0.0;
+#pragma unroll
+    for (int e = 0; e < IPA_NE; e += 4) sl += (l[e] + l[e + 1]) + (l[e + 2] + l[e + 3]);
+    acc[k * IPA_NB + tid] += sl;
+  }
+}
+
 // Events travel global -> shared with cp.async, two tiles deep: while tile i is evaluated from
 // registers the copy of tile i+G is in flight and occupies no register (a register prefetch was
 // spilled by ptxas, which exposed the full DRAM latency at every tile: profiles/r01_v3_*).  Every
 // thread copies and later reads its OWN 16-byte slots, so no block barrier is needed in the loop.
+// The staged loop covers the full tiles of a 16-byte aligned array with 32-bit tile counters and
+// shared addresses; the ragged last tile (or a misaligned array) takes plain loads afterwards.
 template <bool LOGPDF>
 __global__ void __launch_bounds__(IPA_NB, IPA_NB_PER_SM)
 ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaSetConsts* __restrict__ consts, int K,
@@ -252,69 +294,59 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
   __shared__ int s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int G = gridDim.x;
-  const long long ntiles = (n + IPA_NTILE - 1) / IPA_NTILE;
-  auto issue = [&](long long tile, int buf) {
-    const long long base = tile * IPA_NTILE;
-    if (base + IPA_NTILE <= n && vec_ok) {
+  const int nfull = vec_ok ? (int)(n / IPA_NTILE) : 0;            // tiles of the staged loop (n < 2^43)
+  const unsigned slot = (unsigned)__cvta_generic_to_shared(stage) + 16u * tid;
+  const double* src = x + (long long)blockIdx.x * IPA_NTILE + 2 * tid;
+  const long long src_step = (long long)G * IPA_NTILE;
+  int tile = blockIdx.x;
+  if (tile < nfull) {
 #pragma unroll
-      for (int p = 0; p < IPA_NE / 2; ++p)
-        ipa_cp_async16(stage + buf * IPA_NTILE + 2 * (p * IPA_NB + tid), x + base + 2LL * (p * IPA_NB + tid));
-    }
-    ipa_cp_async_commit();
-  };
-  long long tile = blockIdx.x;
-  if (tile < ntiles) issue(tile, 0);
+    for (int p = 0; p < IPA_NE / 2; ++p) ipa_cp_async16_s(slot + p * (IPA_NB * 16), src + p * (IPA_NB * 2));
+  }
+  ipa_cp_async_commit();
   {
     const int nd = K * (int)(sizeof(IpaSetConsts) / 8);
-    const double* src = reinterpret_cast<const double*>(consts);
+    const double* csrc = reinterpret_cast<const double*>(consts);
     double* dst = reinterpret_cast<double*>(sc);
-    for (int i = tid; i < nd; i += IPA_NB) dst[i] = src[i];
+    for (int i = tid; i < nd; i += IPA_NB) dst[i] = csrc[i];
     for (int k = 0; k < K; ++k) acc[k * IPA_NB + tid] = 0.0;
     ipa_load_logtab(s_tab);
   }
   __syncthreads();
-  int buf = 0;
-  for (; tile < ntiles; tile += G, buf ^= 1) {
-    const long long base = tile * IPA_NTILE;
-    const bool full = base + IPA_NTILE <= n;
+  unsigned bufoff = 0;
+  for (; tile < nfull; tile += G) {
     double xv[IPA_NE];
     ipa_cp_async_wait_all();
-    if (full && vec_ok) {
 #pragma unroll
-      for (int p = 0; p < IPA_NE / 2; ++p) {
-        const double2 v = *reinterpret_cast<const double2*>(stage + buf * IPA_NTILE + 2 * (p * IPA_NB + tid));
-        xv[2 * p] = v.x;
-        xv[2 * p + 1] = v.y;
-      }
-    } else {
+    for (int p = 0; p < IPA_NE / 2; ++p) {
+      const double2 v = ipa_lds128(slot + bufoff + p * (IPA_NB * 16));
+      xv[2 * p] = v.x;
+      xv[2 * p + 1] = v.y;
+    }
+    bufoff ^= IPA_NTILE * 8;
+    src += src_step;
+    if (tile + G < nfull) {
+#pragma unroll
+      for (int p = 0; p < IPA_NE / 2; ++p)
+        ipa_cp_async16_s(slot + bufoff + p * (IPA_NB * 16), src + p * (IPA_NB * 2));
+    }
+    ipa_cp_async_commit();
+    ipa_tile_sets<LOGPDF, true>(sc, K, acc, xv, (long long)tile * IPA_NTILE, n, tid, logpdf, s_tab);
+  }
+  ipa_cp_async_wait_all();
+  {
+    // remainder: events [nfull * IPA_NTILE, n) in ragged tiles with plain loads
+    const long long rem0 = (long long)nfull * IPA_NTILE;
+    const long long nrem = (n - rem0 + IPA_NTILE - 1) / IPA_NTILE;
+    for (long long r = blockIdx.x; r < nrem; r += G) {
+      const long long base = rem0 + r * IPA_NTILE;
+      double xv[IPA_NE];
 #pragma unroll
       for (int e = 0; e < IPA_NE; ++e) {
         const long long i = base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1);
         xv[e] = (i < n) ? x[i] : 0.0;
       }
-    }
-    if (tile + G < ntiles) issue(tile + G, buf ^ 1);
-    for (int k = 0; k < K; ++k) {
-      const IpaSetConsts& c = sc[k];
-      if (c.status) continue;
-      double l[IPA_NE];
-      ipa_eval_set<IPA_NE>(c, xv, l, s_tab);
-      if (!full) {
-#pragma unroll
-        for (int e = 0; e < IPA_NE; ++e) {
-          const long long i = base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1);
-          if (LOGPDF && i < n) logpdf[(long long)k * n + i] = l[e];
-          if (i >= n) l[e] = 0.0;
-        }
-      } else if (LOGPDF) {
-#pragma unroll
-        for (int e = 0; e < IPA_NE; ++e)
-          logpdf[(long long)k * n + base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1)] = l[e];
-      }
-      double sl = 0.0;
-#pragma unroll
-      for (int e = 0; e < IPA_NE; e += 4) sl += (l[e] + l[e + 1]) + (l[e + 2] + l[e + 3]);
-      acc[k * IPA_NB + tid] += sl;
+      ipa_tile_sets<LOGPDF, false>(sc, K, acc, xv, base, n, tid, logpdf, s_tab);
     }
   }
   __syncthreads();
