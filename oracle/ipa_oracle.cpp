@@ -301,8 +301,12 @@ static void gauss_legendre(int n, std::vector<ld>& x, std::vector<ld>& w) {
 static ld core_integral_scaled(const Shape& s, ld A, ld B, ld logref) {
   /* int_A^B exp(logG(d)-logref) dd, composite 20-point Gauss-Legendre, panels doubled until stable */
   if (!(B > A)) return 0;
-  static std::vector<ld> gx, gw;
-  if (gx.empty()) gauss_legendre(20, gx, gw);
+  /* the 20-point rule, computed once; C++11 initialises a function-local static exactly once even when
+   * the timed multi-threaded wrapper (orc_nll, nthreads > 1) enters here from several threads */
+  struct Rule { std::vector<ld> x, w; Rule() { gauss_legendre(20, x, w); } };
+  static const Rule rule;
+  const std::vector<ld>& gx = rule.x;
+  const std::vector<ld>& gw = rule.w;
   ld prev = 0;
   for (int P = 4; P <= 8192; P *= 2) {
     ld tot = 0;
