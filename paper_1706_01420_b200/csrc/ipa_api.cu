@@ -62,8 +62,10 @@ int device_info(int* sms) {
     int n = 0;
     IPA_CK(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev));
     const int smem = IPA_MAX_K * (int)(sizeof(IpaSetConsts) + IPA_NB * 8) + 2 * IPA_NTILE * 8;
-    IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
-    IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     g_dev.dev = dev;
     g_dev.sms = n;
     g_dev.attr_set = true;
@@ -175,12 +177,21 @@ int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K
   const IpaSetConsts* consts = reinterpret_cast<const IpaSetConsts*>(ws + L.consts);
   double* partials = reinterpret_cast<double*>(ws + L.partials);
   unsigned int* counter = reinterpret_cast<unsigned int*>(ws + L.counter);
-  if (logpdf_dev)
-    ipa_nll_kernel<true><<<(unsigned)G, IPA_NB, smem, st>>>(x_dev, n, vec_ok, consts, K, partials, logpdf_dev, counter,
-                                                               nll_dev, status_dev);
-  else
-    ipa_nll_kernel<false><<<(unsigned)G, IPA_NB, smem, st>>>(x_dev, n, vec_ok, consts, K, partials, nullptr, counter,
-                                                                nll_dev, status_dev);
+  // sets with bitwise equal signal-shape parameters (the first 9 doubles) share the shape stage
+  IpaGroups grp;
+  for (int k = 0; k < IPA_MAX_K; ++k) grp.leader[k] = (signed char)k;
+  for (int k = 1; k < K; ++k)
+    for (int j = 0; j < k; ++j)
+      if (grp.leader[j] == j && std::memcmp(&p_host[k], &p_host[j], 9 * sizeof(double)) == 0) {
+        grp.leader[k] = (signed char)j;
+        break;
+      }
+  bool grouped = false;
+  for (int k = 0; k < K; ++k) grouped = grouped || grp.leader[k] != k;
+  auto kern = logpdf_dev ? (grouped ? ipa_nll_kernel<true, true> : ipa_nll_kernel<true, false>)
+                         : (grouped ? ipa_nll_kernel<false, true> : ipa_nll_kernel<false, false>);
+  kern<<<(unsigned)G, IPA_NB, smem, st>>>(x_dev, n, vec_ok, consts, K, grp, partials, logpdf_dev, counter, nll_dev,
+                                          status_dev);
   IPA_CK(cudaGetLastError());
   return IPA_OK;
 }

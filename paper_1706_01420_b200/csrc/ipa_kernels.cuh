@@ -86,12 +86,12 @@ ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_param
 __host__ __device__ __noinline__ double ipa_direct_H(double nu, double z) {
   return nu * log(z) + log(ipa_besselk_scaled(nu, z)) - z;
 }
-// P[e] = H(alpha r_e) + cDir for the core events of d[0..E), 0 for the others
+// P[e] = H(alpha r_e) for the core events of d[0..E), 0 for the others
 __host__ __device__ __noinline__ void ipa_direct_core(const IpaSetConsts& c, const double* d, double* P, int E) {
   for (int e = 0; e < E; ++e) {
     P[e] = 0.0;
     if (!((d[e] < c.d0) || (d[e] > c.d1)))
-      P[e] = ipa_direct_H(c.nu, c.alpha * sqrt(fma(d[e], d[e], c.delta2))) + c.cDir;
+      P[e] = ipa_direct_H(c.nu, c.alpha * sqrt(fma(d[e], d[e], c.delta2)));
   }
 }
 
@@ -112,18 +112,30 @@ IPA_HD int ipa_warp_max(int v) {
 #endif
 }
 
-// Core term of E events: Delta = sum_j a[j] t^j + (beta - k) d, t = tA sqrt(d^2 + delta^2) + tB.
-// Horner over groups of 4 coefficients (two 128-bit uniform shared loads per group; a[] is zero above
-// the degree).  FP64 per event: q 1 + sqrt 5 + t 1 + 4 ceil((D+1)/4) + 1.
+// The per-event arithmetic is split in two stages so that parameter sets with the SAME signal shape
+// (mu, sigma, lambda, zeta, beta, a, n, a2, n2 bitwise equal: in a central-difference batch the base set
+// and the f+-, k+- sets) share the expensive one:
+//   shape stage   V = sum_{j>=1} a[j] t^j            (core: sqrt + Horner)     depends on the shape only
+//                 V = -n_T log(uA d + uB)             (tails: one logarithm)
+//   member stage  Delta = s d + (V + c),  (s, c) = (beta - k, a[0]) in the core, (-k, cT) in a tail,
+//                 l = E_B + log(1 + e^Delta)                                    one softplus per set
+// A set evaluated alone runs the same two stages, so its result does not depend on its batch.
+#define IPA_REG_CORE 0
+#define IPA_REG_LEFT 1
+#define IPA_REG_RIGHT 2
+#define IPA_REG_MIXED 3
+
+// Core shape value of E events: t = tA sqrt(d^2 + delta^2) + tB, Horner over groups of 4 coefficients
+// (two 128-bit uniform shared loads per group; a[] is zero above the degree) down to a[1], times t.
+// FP64 per event: q 1 + sqrt 5 + t 1 + 4 ceil((D+1)/4).
 template <int E>
-IPA_HD void ipa_core_delta(const IpaSetConsts& c, const double (&d)[E], double (&Dl)[E]) {
-  double P[E];
+IPA_HD void ipa_core_shape(const IpaSetConsts& c, const double (&d)[E], double (&V)[E]) {
   if (c.mode == 0) {
     const double d2 = c.delta2, tA = c.tA, tB = c.tB;
-    double t[E];
+    double t[E], P[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) { t[e] = fma(tA, ipa_fsqrt(fma(d[e], d[e], d2)), tB); P[e] = 0.0; }
-    for (int g = c.degree >> 2; g >= 0; --g) {
+    for (int g = c.degree >> 2; g >= 1; --g) {
       const double2 hi2 = *reinterpret_cast<const double2*>(c.a + 4 * g + 2);
       const double2 lo2 = *reinterpret_cast<const double2*>(c.a + 4 * g);
 #pragma unroll
@@ -134,6 +146,15 @@ IPA_HD void ipa_core_delta(const IpaSetConsts& c, const double (&d)[E], double (
         P[e] = fma(P[e], t[e], lo2.x);
       }
     }
+    const double2 hi2 = *reinterpret_cast<const double2*>(c.a + 2);
+    const double a1 = c.a[1];
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      P[e] = fma(P[e], t[e], hi2.y);
+      P[e] = fma(P[e], t[e], hi2.x);
+      P[e] = fma(P[e], t[e], a1);
+      V[e] = P[e] * t[e];
+    }
   } else {
     // direct mode (shapes the polynomial cannot cover): per-event Bessel evaluation, out of line
     double dt[E], Pt[E];
@@ -141,25 +162,20 @@ IPA_HD void ipa_core_delta(const IpaSetConsts& c, const double (&d)[E], double (
     for (int e = 0; e < E; ++e) dt[e] = d[e];
     ipa_direct_core(c, dt, Pt, E);
 #pragma unroll
-    for (int e = 0; e < E; ++e) P[e] = Pt[e];
+    for (int e = 0; e < E; ++e) V[e] = Pt[e];
   }
-  const double bmk = c.bmk;
-#pragma unroll
-  for (int e = 0; e < E; ++e) Dl[e] = fma(bmk, d[e], P[e]);
 }
 
-// Per-event log-likelihood of E events per thread for one parameter set.  The region of a WHOLE WARP
-// is decided on the high 32 bits of its events (integer min / max in the thread, one REDUX each across
-// the warp, compared with the high words of the joins mu+d0, mu+d1): strictly inside the core, strictly
-// left or strictly right means every event of the warp is there, and that warp runs only the core
-// polynomial or only the tail logarithm, with uniform constants and no per-event select.  Any other
-// warp (mixed regions, an event within 2^-20 relative of a join, non-positive or NaN events) takes
-// the general path: both terms, selected per event on d = x - mu (joins belong to the core).
-// FP64 per event: d 1, E_B 1, softplus 27, plus core 8 + 4 ceil((D+1)/4) or tail 14 (general path: both + 4).
+// Shape stage.  The region of a WHOLE WARP is decided on the high 32 bits of its events (integer
+// min / max in the thread, one REDUX each across the warp, compared with the high words of the joins
+// mu+d0, mu+d1): strictly inside the core, strictly left or strictly right means every event of the warp
+// is there, and that warp runs only the core polynomial or only the tail logarithm, with uniform
+// constants and no per-event select.  Any other warp (mixed regions, an event within 2^-20 relative
+// of a join, non-positive or NaN events) takes the general path: both terms, selected per event on
+// d = x - mu (joins belong to the core; NaN events keep the core value, NaN).
 template <int E, class Tab>
-IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l)[E], const Tab* tab) {
-  double d[E], Dl[E];
-  const double mu = c.mu, kd = c.kd;
+IPA_HD int ipa_shape_stage(const IpaSetConsts& c, const double (&x)[E], double (&d)[E], double (&V)[E], const Tab* tab) {
+  const double mu = c.mu;
   int hmin = ipa_hi(x[0]), hmax = hmin;
 #pragma unroll
   for (int e = 1; e < E; ++e) {
@@ -173,32 +189,66 @@ IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l
   for (int e = 0; e < E; ++e) d[e] = x[e] - mu;
   const bool sane = hmin > 0 && hmax < 0x7ff00000;      // positive, finite events only
   if (sane && hmin > c.hxl && hmax < c.hxr) {
-    ipa_core_delta<E>(c, d, Dl);
-  } else if (sane && (hmax < c.hxl || hmin > c.hxr)) {
-    const double* q = (hmin > c.hxr) ? &c.uA1 : &c.uA0;
-    const double uA = q[0], uB = q[1], nT = q[2], cT = q[3];
+    ipa_core_shape<E>(c, d, V);
+    return IPA_REG_CORE;
+  }
+  if (sane && (hmax < c.hxl || hmin > c.hxr)) {
+    const bool right = hmin > c.hxr;
+    const double* q = right ? &c.uA1 : &c.uA0;
+    const double uA = q[0], uB = q[1], nT = q[2];
 #pragma unroll
-    for (int e = 0; e < E; ++e) Dl[e] = fma(-kd, d[e], fma(-nT, ipa_flog(fma(uA, d[e], uB), tab), cT));
+    for (int e = 0; e < E; ++e) V[e] = -nT * ipa_flog(fma(uA, d[e], uB), tab);
+    return right ? IPA_REG_RIGHT : IPA_REG_LEFT;
+  }
+  const double d0 = c.d0, d1 = c.d1;
+  ipa_core_shape<E>(c, d, V);
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const bool left = d[e] < d0, right = d[e] > d1;
+    const double uA = left ? c.uA0 : c.uA1, uB = left ? c.uB0 : c.uB1, nT = left ? c.n0 : c.n1;
+    const double tl = -nT * ipa_flog(fma(uA, d[e], uB), tab);
+    if (left || right) V[e] = tl;
+  }
+  return IPA_REG_MIXED;
+}
+
+// Member stage: FP64 per event 2 + E_B 1 + softplus 27 (mixed warps: + 2 compares and selects).
+// `c` is the member's own record; d0, d1 (shape constants) are identical for every member of a group.
+template <int E, class Tab>
+IPA_HD void ipa_member_stage(const IpaSetConsts& c, int region, const double (&d)[E], const double (&V)[E],
+                             double (&l)[E], const Tab* tab) {
+  const double kd = c.kd, eB0 = c.eB0;
+  double D[E];
+  if (region != IPA_REG_MIXED) {
+    const double s = (region == IPA_REG_CORE) ? c.bmk : -kd;
+    const double k0 = (region == IPA_REG_CORE) ? c.a[0] : (region == IPA_REG_LEFT ? c.cT0 : c.cT1);
+#pragma unroll
+    for (int e = 0; e < E; ++e) D[e] = fma(s, d[e], V[e] + k0);
   } else {
-    const double d0 = c.d0, d1 = c.d1;
-    ipa_core_delta<E>(c, d, Dl);
+    const double d0 = c.d0, d1 = c.d1, a0 = c.a[0], cT0 = c.cT0, cT1 = c.cT1, bmk = c.bmk;
 #pragma unroll
     for (int e = 0; e < E; ++e) {
-      const bool left = d[e] < d0, right = d[e] > d1;   // NaN events keep the core value (NaN)
-      const double uA = left ? c.uA0 : c.uA1, uB = left ? c.uB0 : c.uB1;
-      const double nT = left ? c.n0 : c.n1, cT = left ? c.cT0 : c.cT1;
-      const double tl = fma(-kd, d[e], fma(-nT, ipa_flog(fma(uA, d[e], uB), tab), cT));
-      if (left || right) Dl[e] = tl;
+      const bool left = d[e] < d0, right = d[e] > d1;
+      const double k0 = left ? cT0 : (right ? cT1 : a0);
+      const double s = (left || right) ? -kd : bmk;
+      D[e] = fma(s, d[e], V[e] + k0);
     }
   }
-  const double eB0 = c.eB0;
   if (c.pure) {
 #pragma unroll
-    for (int e = 0; e < E; ++e) l[e] = fma(kd, d[e], eB0) + Dl[e];
+    for (int e = 0; e < E; ++e) l[e] = fma(kd, d[e], eB0) + D[e];
   } else {
 #pragma unroll
-    for (int e = 0; e < E; ++e) l[e] = ipa_fsoftplus_add(fma(kd, d[e], eB0), Dl[e], tab);
+    for (int e = 0; e < E; ++e) l[e] = ipa_fsoftplus_add(fma(kd, d[e], eB0), D[e], tab);
   }
+}
+
+// One set on its own: both stages with the same record.
+template <int E, class Tab>
+IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l)[E], const Tab* tab) {
+  double d[E], V[E];
+  const int region = ipa_shape_stage<E>(c, x, d, V, tab);
+  ipa_member_stage<E>(c, region, d, V, l, tab);
 }
 
 __device__ __forceinline__ double ipa_warp_sum(double v) {
@@ -244,34 +294,68 @@ __device__ __forceinline__ double2 ipa_lds128(unsigned smem_addr) {
   return v;
 }
 
-// All K parameter sets on the IPA_NE events a thread holds in registers (A2-A4), optional per-event
-// output, accumulation into the thread's shared-memory accumulators (first level of A5).
+// Sets of a batch grouped by signal shape: leader[k] = smallest index with the same shape parameters
+// (built on the host by ipa_nll_eval; leader[k] == k for a set on its own).
+struct IpaGroups { signed char leader[IPA_MAX_K]; };
+
+// All K parameter sets on the IPA_NE events a thread holds in registers (A2-A4): one shape stage per
+// group, one member stage per set; optional per-event output; accumulation into the thread's
+// shared-memory accumulators (first level of A5).
 // Event e of thread tid in the tile at `base` is x[base + 2 ((e >> 1) IPA_NB + tid) + (e & 1)].
 template <bool LOGPDF, bool FULL>
-__device__ __forceinline__ void ipa_tile_sets(const IpaSetConsts* sc, int K, double* acc, const double (&xv)[IPA_NE],
-                                              long long base, long long n, int tid, double* __restrict__ logpdf,
-                                              const double2* s_tab) {
-  for (int k = 0; k < K; ++k) {
-    const IpaSetConsts& c = sc[k];
-    if (c.status) continue;
-    double l[IPA_NE];
-    ipa_eval_set<IPA_NE>(c, xv, l, s_tab);
-    if (!FULL) {
+__device__ __forceinline__ void ipa_tile_store_acc(int k, double (&l)[IPA_NE], double* acc, long long base, long long n,
+                                                   int tid, double* __restrict__ logpdf) {
+  if (!FULL) {
 #pragma unroll
-      for (int e = 0; e < IPA_NE; ++e) {
-        const long long i = base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1);
-        if (LOGPDF && i < n) logpdf[(long long)k * n + i] = l[e];
-        if (i >= n) l[e] = 0.0;
-      }
-    } else if (LOGPDF) {
-#pragma unroll
-      for (int e = 0; e < IPA_NE; ++e)
-        logpdf[(long long)k * n + base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1)] = l[e];
+    for (int e = 0; e < IPA_NE; ++e) {
+      const long long i = base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1);
+      if (LOGPDF && i < n) logpdf[(long long)k * n + i] = l[e];
+      if (i >= n) l[e] = 0.0;
     }
-    double sl = 0.0;
+  } else if (LOGPDF) {
 #pragma unroll
-    for (int e = 0; e < IPA_NE; e += 4) sl += (l[e] + l[e + 1]) + (l[e + 2] + l[e + 3]);
-    acc[k * IPA_NB + tid] += sl;
+    for (int e = 0; e < IPA_NE; ++e)
+      logpdf[(long long)k * n + base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1)] = l[e];
+  }
+  double sl = 0.0;
+#pragma unroll
+  for (int e = 0; e < IPA_NE; e += 4) sl += (l[e] + l[e + 1]) + (l[e + 2] + l[e + 3]);
+  acc[k * IPA_NB + tid] += sl;
+}
+
+// GROUPED = false: no two sets of the batch share a shape (K = 1, a scan over shapes): plain loop over the
+// sets.  GROUPED = true: one shape stage per group, one member stage per set.  Same arithmetic either way.
+// (Inlined at both call sites: an out-of-line copy shared by the staged loop and the remainder cost 12 %
+// at 1e8 events -- call ABI spills -- and gained nothing at 1e6.)
+template <bool LOGPDF, bool FULL, bool GROUPED>
+__device__ __forceinline__ void ipa_tile_sets(const IpaSetConsts* sc, int K, const IpaGroups& grp, double* acc,
+                                              const double (&xv)[IPA_NE], long long base, long long n, int tid,
+                                              double* __restrict__ logpdf, const double2* s_tab) {
+  if (!GROUPED) {
+    for (int k = 0; k < K; ++k) {
+      const IpaSetConsts& c = sc[k];
+      if (c.status) continue;
+      double l[IPA_NE];
+      ipa_eval_set<IPA_NE>(c, xv, l, s_tab);
+      ipa_tile_store_acc<LOGPDF, FULL>(k, l, acc, base, n, tid, logpdf);
+    }
+    return;
+  }
+  for (int g = 0; g < K; ++g) {
+    if (grp.leader[g] != g) continue;
+    int v = g;                                   // first member with a usable record
+    while (v < K && (grp.leader[v] != g || sc[v].status)) ++v;
+    if (v >= K) continue;
+    double d[IPA_NE], V[IPA_NE];
+    const int region = ipa_shape_stage<IPA_NE>(sc[v], xv, d, V, s_tab);
+    for (int k = v; k < K; ++k) {
+      if (grp.leader[k] != g) continue;
+      const IpaSetConsts& c = sc[k];
+      if (c.status) continue;
+      double l[IPA_NE];
+      ipa_member_stage<IPA_NE>(c, region, d, V, l, s_tab);
+      ipa_tile_store_acc<LOGPDF, FULL>(k, l, acc, base, n, tid, logpdf);
+    }
   }
 }
 
@@ -281,10 +365,10 @@ __device__ __forceinline__ void ipa_tile_sets(const IpaSetConsts* sc, int K, dou
 // thread copies and later reads its OWN 16-byte slots, so no block barrier is needed in the loop.
 // The staged loop covers the full tiles of a 16-byte aligned array with 32-bit tile counters and
 // shared addresses; the ragged last tile (or a misaligned array) takes plain loads afterwards.
-template <bool LOGPDF>
+template <bool LOGPDF, bool GROUPED>
 __global__ void __launch_bounds__(IPA_NB, IPA_NB_PER_SM)
 ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaSetConsts* __restrict__ consts, int K,
-               double* __restrict__ partials, double* __restrict__ logpdf, unsigned int* counter,
+               const __grid_constant__ IpaGroups grp, double* __restrict__ partials, double* __restrict__ logpdf, unsigned int* counter,
                double* __restrict__ nll_out, int32_t* __restrict__ status_out) {
   extern __shared__ __align__(16) unsigned char ipa_smem[];
   double* stage = reinterpret_cast<double*>(ipa_smem);                       // [2][IPA_NTILE]
@@ -331,22 +415,27 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
         ipa_cp_async16_s(slot + bufoff + p * (IPA_NB * 16), src + p * (IPA_NB * 2));
     }
     ipa_cp_async_commit();
-    ipa_tile_sets<LOGPDF, true>(sc, K, acc, xv, (long long)tile * IPA_NTILE, n, tid, logpdf, s_tab);
+    ipa_tile_sets<LOGPDF, true, GROUPED>(sc, K, grp, acc, xv, (long long)tile * IPA_NTILE, n, tid, logpdf, s_tab);
   }
   ipa_cp_async_wait_all();
   {
     // remainder: events [nfull * IPA_NTILE, n) in ragged tiles with plain loads
+    // They continue the round-robin over the blocks where the staged tiles stopped (the ragged tile must
+    // not land on a block that already holds the largest share), and the empty slots of the last tile
+    // repeat the last event, so that a warp of a sorted array stays region-uniform; their results are dropped.
     const long long rem0 = (long long)nfull * IPA_NTILE;
     const long long nrem = (n - rem0 + IPA_NTILE - 1) / IPA_NTILE;
-    for (long long r = blockIdx.x; r < nrem; r += G) {
+    const int first = (int)((blockIdx.x + G - nfull % G) % G);   // block nfull % G takes remainder tile 0
+    const double xpad = (n > 0) ? x[n - 1] : 0.0;
+    for (long long r = first; r < nrem; r += G) {
       const long long base = rem0 + r * IPA_NTILE;
       double xv[IPA_NE];
 #pragma unroll
       for (int e = 0; e < IPA_NE; ++e) {
         const long long i = base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1);
-        xv[e] = (i < n) ? x[i] : 0.0;
+        xv[e] = (i < n) ? x[i] : xpad;
       }
-      ipa_tile_sets<LOGPDF, false>(sc, K, acc, xv, base, n, tid, logpdf, s_tab);
+      ipa_tile_sets<LOGPDF, false, GROUPED>(sc, K, grp, acc, xv, base, n, tid, logpdf, s_tab);
     }
   }
   __syncthreads();

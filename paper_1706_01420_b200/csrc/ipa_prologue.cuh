@@ -424,9 +424,9 @@ IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
 IPA_HD void ipa_pro_phase13(IpaProWork& w, IpaSetConsts& o, int k) {
   if (k >= IPA_NCOEF) return;
   double v = 0.0;
-  if (!w.status && !w.mode) {
-    v = w.araw[k];
-    if (k == 0) v += o.cDir;  // cS - eB0 - nu log alpha
+  if (!w.status) {
+    if (!w.mode) v = w.araw[k];
+    if (k == 0) v += o.cDir;  // cS - eB0 - nu log alpha: the per-set constant of the core term (both modes)
   }
   o.a[k] = v;
 }
