@@ -174,6 +174,25 @@ IPA_HD void ipa_core_shape(const IpaSetConsts& c, const double (&d)[E], double (
 // of a join, non-positive or NaN events) takes the general path: both terms, selected per event on
 // d = x - mu (joins belong to the core; NaN events keep the core value, NaN).
 template <int E, class Tab>
+IPA_HD void ipa_tail_shape(const IpaSetConsts& c, bool right, const double (&d)[E], double (&V)[E], const Tab* tab) {
+  const double* q = right ? &c.uA1 : &c.uA0;
+  const double uA = q[0], uB = q[1], nT = q[2];
+#pragma unroll
+  for (int e = 0; e < E; ++e) V[e] = -nT * ipa_flog(fma(uA, d[e], uB), tab);
+}
+template <int E, class Tab>
+IPA_HD void ipa_mixed_shape(const IpaSetConsts& c, const double (&d)[E], double (&V)[E], const Tab* tab) {
+  const double d0 = c.d0, d1 = c.d1;
+  ipa_core_shape<E>(c, d, V);
+#pragma unroll
+  for (int e = 0; e < E; ++e) {
+    const bool left = d[e] < d0, right = d[e] > d1;
+    const double uA = left ? c.uA0 : c.uA1, uB = left ? c.uB0 : c.uB1, nT = left ? c.n0 : c.n1;
+    const double tl = -nT * ipa_flog(fma(uA, d[e], uB), tab);
+    if (left || right) V[e] = tl;
+  }
+}
+template <int E, class Tab>
 IPA_HD int ipa_shape_stage(const IpaSetConsts& c, const double (&x)[E], double (&d)[E], double (&V)[E], const Tab* tab) {
   const double mu = c.mu;
   int hmin = ipa_hi(x[0]), hmax = hmin;
@@ -192,36 +211,22 @@ IPA_HD int ipa_shape_stage(const IpaSetConsts& c, const double (&x)[E], double (
     ipa_core_shape<E>(c, d, V);
     return IPA_REG_CORE;
   }
-  if (sane && (hmax < c.hxl || hmin > c.hxr)) {
-    const bool right = hmin > c.hxr;
-    const double* q = right ? &c.uA1 : &c.uA0;
-    const double uA = q[0], uB = q[1], nT = q[2];
-#pragma unroll
-    for (int e = 0; e < E; ++e) V[e] = -nT * ipa_flog(fma(uA, d[e], uB), tab);
-    return right ? IPA_REG_RIGHT : IPA_REG_LEFT;
-  }
-  const double d0 = c.d0, d1 = c.d1;
-  ipa_core_shape<E>(c, d, V);
-#pragma unroll
-  for (int e = 0; e < E; ++e) {
-    const bool left = d[e] < d0, right = d[e] > d1;
-    const double uA = left ? c.uA0 : c.uA1, uB = left ? c.uB0 : c.uB1, nT = left ? c.n0 : c.n1;
-    const double tl = -nT * ipa_flog(fma(uA, d[e], uB), tab);
-    if (left || right) V[e] = tl;
-  }
+  if (sane && hmax < c.hxl) { ipa_tail_shape<E>(c, false, d, V, tab); return IPA_REG_LEFT; }
+  if (sane && hmin > c.hxr) { ipa_tail_shape<E>(c, true, d, V, tab); return IPA_REG_RIGHT; }
+  ipa_mixed_shape<E>(c, d, V, tab);
   return IPA_REG_MIXED;
 }
 
 // Member stage: FP64 per event 2 + E_B 1 + softplus 27 (mixed warps: + 2 compares and selects).
 // `c` is the member's own record; d0, d1 (shape constants) are identical for every member of a group.
-template <int E, class Tab>
-IPA_HD void ipa_member_stage(const IpaSetConsts& c, int region, const double (&d)[E], const double (&V)[E],
-                             double (&l)[E], const Tab* tab) {
+template <int E, int REGION, class Tab>
+IPA_HD void ipa_member_stage_r(const IpaSetConsts& c, const double (&d)[E], const double (&V)[E], double (&l)[E],
+                               const Tab* tab) {
   const double kd = c.kd, eB0 = c.eB0;
   double D[E];
-  if (region != IPA_REG_MIXED) {
-    const double s = (region == IPA_REG_CORE) ? c.bmk : -kd;
-    const double k0 = (region == IPA_REG_CORE) ? c.a[0] : (region == IPA_REG_LEFT ? c.cT0 : c.cT1);
+  if (REGION != IPA_REG_MIXED) {
+    const double s = (REGION == IPA_REG_CORE) ? c.bmk : -kd;
+    const double k0 = (REGION == IPA_REG_CORE) ? c.a[0] : (REGION == IPA_REG_LEFT ? c.cT0 : c.cT1);
 #pragma unroll
     for (int e = 0; e < E; ++e) D[e] = fma(s, d[e], V[e] + k0);
   } else {
@@ -242,13 +247,45 @@ IPA_HD void ipa_member_stage(const IpaSetConsts& c, int region, const double (&d
     for (int e = 0; e < E; ++e) l[e] = ipa_fsoftplus_add(fma(kd, d[e], eB0), D[e], tab);
   }
 }
+template <int E, class Tab>
+IPA_HD void ipa_member_stage(const IpaSetConsts& c, int region, const double (&d)[E], const double (&V)[E],
+                             double (&l)[E], const Tab* tab) {
+  if (region == IPA_REG_CORE) ipa_member_stage_r<E, IPA_REG_CORE>(c, d, V, l, tab);
+  else if (region == IPA_REG_LEFT) ipa_member_stage_r<E, IPA_REG_LEFT>(c, d, V, l, tab);
+  else if (region == IPA_REG_RIGHT) ipa_member_stage_r<E, IPA_REG_RIGHT>(c, d, V, l, tab);
+  else ipa_member_stage_r<E, IPA_REG_MIXED>(c, d, V, l, tab);
+}
 
-// One set on its own: both stages with the same record.
+// One set on its own: the same two stages with the same record, the member stage inlined per region.
 template <int E, class Tab>
 IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l)[E], const Tab* tab) {
   double d[E], V[E];
-  const int region = ipa_shape_stage<E>(c, x, d, V, tab);
-  ipa_member_stage<E>(c, region, d, V, l, tab);
+  const double mu = c.mu;
+  int hmin = ipa_hi(x[0]), hmax = hmin;
+#pragma unroll
+  for (int e = 1; e < E; ++e) {
+    const int h = ipa_hi(x[e]);
+    hmin = h < hmin ? h : hmin;
+    hmax = h > hmax ? h : hmax;
+  }
+  hmin = ipa_warp_min(hmin);
+  hmax = ipa_warp_max(hmax);
+#pragma unroll
+  for (int e = 0; e < E; ++e) d[e] = x[e] - mu;
+  const bool sane = hmin > 0 && hmax < 0x7ff00000;
+  if (sane && hmin > c.hxl && hmax < c.hxr) {
+    ipa_core_shape<E>(c, d, V);
+    ipa_member_stage_r<E, IPA_REG_CORE>(c, d, V, l, tab);
+  } else if (sane && hmax < c.hxl) {
+    ipa_tail_shape<E>(c, false, d, V, tab);
+    ipa_member_stage_r<E, IPA_REG_LEFT>(c, d, V, l, tab);
+  } else if (sane && hmin > c.hxr) {
+    ipa_tail_shape<E>(c, true, d, V, tab);
+    ipa_member_stage_r<E, IPA_REG_RIGHT>(c, d, V, l, tab);
+  } else {
+    ipa_mixed_shape<E>(c, d, V, tab);
+    ipa_member_stage_r<E, IPA_REG_MIXED>(c, d, V, l, tab);
+  }
 }
 
 __device__ __forceinline__ double ipa_warp_sum(double v) {

@@ -76,6 +76,16 @@ def test_batch_independence_and_determinism(ipa, torch_, x1):
     assert np.array_equal(a, b)  # run-to-run bitwise
     assert np.array_equal(a, np.array([s.item() for s in singles]))  # set k does not depend on its batch
     assert np.array_equal(a[perm], c)
+    # sets sharing a signal shape are evaluated as a group: the first set of a group may be invalid (f out of
+    # range), members may be pure signal / pure background; every valid member equals its stand-alone value
+    grp = [dict(inp.GEN, f=1.5), dict(inp.GEN), dict(inp.GEN, f=0.2, k=-0.001), dict(inp.P2), dict(inp.GEN, f=1.0),
+           dict(inp.GEN, f=0.0), dict(inp.P2, k=0.0)]
+    g, _, st = ipa.ipa_nll_eval(xd, grp, LO, HI)
+    alone = [ipa.ipa_nll_eval(xd, q, LO, HI)[0] for q in grp]
+    torch_.cuda.synchronize()
+    g = g.cpu().numpy()
+    assert list(st.cpu().numpy()) == [1, 0, 0, 0, 0, 0, 0] and np.isposinf(g[0])
+    assert np.array_equal(g[1:], np.array([s.item() for s in alone[1:]]))
 
 
 @pytest.mark.parametrize("n", [0, 1, 2, 31, 1023, 1024, 1025, 4099])
