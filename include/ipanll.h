@@ -18,7 +18,10 @@
  *     stream) and results are valid once the caller has synchronised that stream.  `*_host` inputs are
  *     read completely before the call returns (they are copied into the kernel-parameter space or
  *     into the workspace with kernel arguments, never with an asynchronous host read), so they may be
- *     reused immediately.  Every call is CUDA-graph capturable.
+ *     reused immediately.  ipa_norm, ipa_core_degree and ipa_nll_eval (K <= IPA_MAX_K: the parameter sets
+ *     travel in the kernel-parameter space) can be captured in a CUDA graph; a replay re-evaluates the
+ *     parameter values given at capture time.  Calls that upload a host array with a copy (more than
+ *     IPA_MAX_K sets, toy seeds, scan points) capture only if that array is in pinned host memory.
  *   - `ws_dev` is a scratch workspace of at least ipa_workspace_bytes(...) bytes, 256-byte aligned,
  *     private to one stream at a time.
  *   - Return value: IPA_OK (0) or a negative ipa_status.  Argument errors are detected before any

@@ -185,6 +185,35 @@ def test_hypothesis_like_sweep(ipa, torch_, orc, x1):
             assert np.abs(lp[i].cpu().numpy() - orc.logpdf(x, p, LO, HI)).max() <= 1e-10, (i, p)
 
 
+def test_cuda_graph_capture_and_side_stream(ipa, torch_, orc, x1):
+    """The call enqueues on the caller's stream, never synchronises, and can be captured in a CUDA graph."""
+    xd = dev(torch_, x1)
+    batch, _ = inp.fd_batch(inp.GEN)
+    ws = ipa.workspace(x1.size, 32)
+    out = torch_.empty(9, dtype=torch_.float64, device="cuda")
+    st = torch_.empty(9, dtype=torch_.int32, device="cuda")
+    ref, _, _ = ipa.ipa_nll_eval(xd, batch, LO, HI)
+    side = torch_.cuda.Stream()
+    side.wait_stream(torch_.cuda.current_stream())
+    with torch_.cuda.stream(side):
+        ipa.ipa_nll_eval(xd, batch, LO, HI, ws=ws, stream=side, out=out, status=st)      # warm-up on the side stream
+        side.synchronize()
+        assert torch_.equal(out, ref)
+        g = torch_.cuda.CUDAGraph()
+        out.zero_()
+        with torch_.cuda.graph(g, stream=side):
+            ipa.ipa_nll_eval(xd, batch, LO, HI, ws=ws, stream=torch_.cuda.current_stream(), out=out, status=st)
+        assert float(out.abs().sum()) == 0.0          # capture enqueues nothing
+        g.replay()
+        side.synchronize()
+        assert torch_.equal(out, ref)
+        out.zero_()
+        g.replay()
+        g.replay()
+        torch_.cuda.synchronize()
+        assert torch_.equal(out, ref)
+
+
 # ---------------------------------------------------------------------------------------------
 # generators (T0, T1), segmented NLL (T2)
 # ---------------------------------------------------------------------------------------------
