@@ -44,6 +44,9 @@ def lib():
         L.orc_binned_nll_scan.argtypes = [vp, i32, d, d, vp, vp, vp, vp, i64, vp]
         L.orc_expected_hist.restype = i32; L.orc_expected_hist.argtypes = [i32, d, d, vp, d, d, d, vp]
         L.orc_poisson_hist_toys.restype = None; L.orc_poisson_hist_toys.argtypes = [vp, i32, vp, i64, vp]
+        L.orc_cls_teststat.restype = None; L.orc_cls_teststat.argtypes = [vp, i32, i64, i32, vp, vp, vp]
+        L.orc_cls_count_ge.restype = i64; L.orc_cls_count_ge.argtypes = [vp, i64, d]
+        L.orc_cls_from_counts.restype = None; L.orc_cls_from_counts.argtypes = [i64, i64, i64, i64, vp]
         _lib = L
     return _lib
 
@@ -218,4 +221,27 @@ def poisson_hist_toys(mean, seeds):
     seeds = np.ascontiguousarray(seeds, dtype=np.uint64)
     out = np.empty((seeds.size, mean.size), dtype=np.uint32)
     lib().orc_poisson_hist_toys(_p(mean), mean.size, _p(seeds), seeds.size, _p(out))
+    return out
+
+
+def cls_teststat(counts, nu_sb, nu_b):
+    """q_t for T toy histograms counts[T, nbins] (uint32 or uint64); reading F2."""
+    counts = np.ascontiguousarray(counts)
+    assert counts.dtype in (np.uint32, np.uint64)
+    counts2 = counts.reshape(-1, np.asarray(nu_b).size)
+    nu_sb = np.ascontiguousarray(nu_sb, dtype=np.float64)
+    nu_b = np.ascontiguousarray(nu_b, dtype=np.float64)
+    out = np.empty(counts2.shape[0])
+    lib().orc_cls_teststat(_p(counts2), counts.dtype.itemsize, counts2.shape[0], nu_b.size, _p(nu_sb), _p(nu_b), _p(out))
+    return out
+
+
+def cls_count_ge(q, q_obs):
+    q = np.ascontiguousarray(q, dtype=np.float64)
+    return int(lib().orc_cls_count_ge(_p(q), q.size, float(q_obs)))
+
+
+def cls_from_counts(count_sb, T_sb, count_b, T_b):
+    out = np.empty(3)
+    lib().orc_cls_from_counts(int(count_sb), int(T_sb), int(count_b), int(T_b), _p(out))
     return out

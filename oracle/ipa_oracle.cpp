@@ -661,4 +661,37 @@ void orc_poisson_hist_toys(const double* mean, int nbins, const uint64_t* seeds,
     for (int b = 0; b < nbins; ++b) counts[t * nbins + b] = (uint32_t)poisson_draw(seeds[t], (uint64_t)b, STREAM_BIN, mean[b]);
 }
 
+
+/* ------------------------------------------------------------------------------------------
+ * CLs on binned toys (CL.setData(fake_data),
+ * CL.setExpected(HistoPdf), CL.CLs(ns, toys = 10000)).  The paper does not print its test statistic
+ * (it cites its refs [11,12] for the CLs method) -> DESIGN.md reading F2: the likelihood ratio of the
+ * two fixed expected histograms,
+ *      q(n) = -2 ln [ L(n | nu_sb) / L(n | nu_b) ] = 2 sum_b [ (nu_sb_b - nu_b_b) - n_b ln(nu_sb_b / nu_b_b) ],
+ * larger q = more background-like;  CL_sb = P(q >= q_obs | s+b toys),  CL_b = P(q >= q_obs | b toys),
+ * CL_s = CL_sb / CL_b.  Plain left-to-right sums in long double.
+ * ---------------------------------------------------------------------------------------- */
+void orc_cls_teststat(const void* counts, int count_bytes, int64_t T, int nbins, const double* nu_sb,
+                      const double* nu_b, double* q) {
+  for (int64_t t = 0; t < T; ++t) {
+    ld acc = 0;
+    for (int b = 0; b < nbins; ++b) {
+      const ld n = count_bytes == 8 ? (ld)((const uint64_t*)counts)[t * nbins + b]
+                                    : (ld)((const uint32_t*)counts)[t * nbins + b];
+      acc += ((ld)nu_sb[b] - (ld)nu_b[b]) - n * logl((ld)nu_sb[b] / (ld)nu_b[b]);
+    }
+    q[t] = (double)(2 * acc);
+  }
+}
+int64_t orc_cls_count_ge(const double* q, int64_t T, double q_obs) {
+  int64_t c = 0;
+  for (int64_t t = 0; t < T; ++t) c += (q[t] >= q_obs) ? 1 : 0;
+  return c;
+}
+/* out = {CL_sb, CL_b, CL_s}; CL_s is NaN when no background toy reaches q_obs */
+void orc_cls_from_counts(int64_t count_sb, int64_t T_sb, int64_t count_b, int64_t T_b, double* out) {
+  out[0] = (double)count_sb / (double)T_sb;
+  out[1] = (double)count_b / (double)T_b;
+  out[2] = count_b > 0 ? out[0] / out[1] : NAN;
+}
 } /* extern "C" */
