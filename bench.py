@@ -205,6 +205,17 @@ def other_rows(torch, ipa, x, ws, stream, n):
     nu = ipa.ipa_expected_hist(nbins, LO, HI, inp.GEN, 2500.0, n - 2500.0, -0.002)
     sd = np.arange(1, 10001, dtype=np.uint64)
     dp = t(lambda: ipa.ipa_poisson_hist_toys(nu, sd, ws=ws5, stream=stream), 20)
+    # row f2: CLs for one signal hypothesis on the toy histograms above (statistic of 10 000 x 1000 counts is one
+    # HBM pass over 40 MB)
+    nu_b0 = ipa.ipa_expected_hist(nbins, LO, HI, inp.GEN, 0.0, float(n), -0.002)
+    toys = ipa.ipa_poisson_hist_toys(nu, sd, ws=ws5, stream=stream)
+    qobs = ipa.ipa_cls_teststat(counts, nu, nu_b0, ws=ws5, stream=stream)
+    dq = t(lambda: ipa.ipa_cls_teststat(toys, nu, nu_b0, ws=ws5, stream=stream), 20)
+    qt = ipa.ipa_cls_teststat(toys, nu, nu_b0, ws=ws5, stream=stream)
+    dc = t(lambda: ipa.ipa_cls_count_ge(qt, qobs, stream=stream), 20)
+    out["cls_f2"] = {"toy_histograms": int(sd.size), "bins": nbins, "teststat_ms": dq * 1e3, "count_ms": dc * 1e3,
+                     "teststat_roofline": {"bound": "hbm", "achieved": 4.0 * sd.size * nbins / dq / 1e9, "peak": peaks_hbm,
+                                           "unit": "GB/s", "frac": 4.0 * sd.size * nbins / dq / 1e9 / peaks_hbm}}
     out["config5_binned"] = {
         "hist_fill_ms": dh * 1e3, "hist_events_per_s": n / dh,
         "hist_roofline": {"bound": "hbm", "achieved": 8.0 * n / dh / 1e9, "peak": peaks_hbm, "unit": "GB/s",

@@ -163,6 +163,19 @@ int ipa_expected_hist(int nbins, ipa_range r, const ipa_params* shape_host, doub
 int ipa_poisson_hist_toys(const double* mean_dev, int nbins, const uint64_t* seeds_host, int64_t T,
                           uint32_t* counts_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
 
+/* CLs on binned toys (CL.setData, CL.setExpected(HistoPdf), CL.CLs(ns, toys); the paper
+ * does not print its statistic -- DESIGN.md reading F2): likelihood ratio of two fixed expected histograms,
+ *   q_t = -2 ln[ L(n_t | nu_sb) / L(n_t | nu_b) ] = 2 sum_b [ (nu_sb_b - nu_b_b) - n_tb ln(nu_sb_b / nu_b_b) ].
+ *   counts_dev [T*nbins] toy (or data, T = 1) histograms, count_bytes = 4 (ipa_poisson_hist_toys) or 8
+ *   (ipa_hist_fill);  nu_sb_dev, nu_b_dev [nbins] > 0 (ipa_expected_hist);  q_dev [T] out. */
+int ipa_cls_teststat(const void* counts_dev, int count_bytes, int64_t T, int nbins, const double* nu_sb_dev,
+                     const double* nu_b_dev, double* q_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
+/* count_dev[0] = #{ t : q_dev[t] >= q_obs_dev[0] }  (q_obs stays on the device: it is the statistic of the data). */
+int ipa_cls_count_ge(const double* q_dev, int64_t T, const double* q_obs_dev, int64_t* count_dev, void* cuda_stream);
+/* cl_dev = { CL_sb = count_sb/T_sb, CL_b = count_b/T_b, CL_s = CL_sb/CL_b (NaN if count_b == 0) }. */
+int ipa_cls_from_counts(const int64_t* count_sb_dev, int64_t T_sb, const int64_t* count_b_dev, int64_t T_b,
+                        double* cl_dev, void* cuda_stream);
+
 /* Optional one-off preparation: ascending sort of the events (whole array, or inside each of T segments
  * when offsets_dev != NULL).  The likelihood does not depend on the order of the events, the data of a
  * fit are constant over the minimiser's calls, and the streaming kernels skip the

@@ -14,7 +14,8 @@ __all__ = [
     "PARAM_FIELDS", "NPAR", "IPA_MAX_K", "IpaError", "lib", "library_path", "pack_params", "workspace",
     "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes", "ipa_norm", "ipa_core_degree", "ipa_nll_eval",
     "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill", "ipa_binned_nll_scan", "ipa_expected_hist",
-    "ipa_poisson_hist_toys", "ipa_events_sort", "ipa_sort_workspace_bytes", "ipa_fp64_peak_probe", "nll_host", "EXPORTS",
+    "ipa_poisson_hist_toys", "ipa_cls_teststat", "ipa_cls_count_ge", "ipa_cls_from_counts", "ipa_events_sort",
+    "ipa_sort_workspace_bytes", "ipa_fp64_peak_probe", "nll_host", "EXPORTS",
 ]
 
 PARAM_FIELDS = ("mu", "sigma", "lambda", "zeta", "beta", "a", "n", "a2", "n2", "f", "k")
@@ -25,7 +26,8 @@ IPA_MAX_K = 32
 EXPORTS = (
     "ipa_strerror", "ipa_last_cuda_error", "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes",
     "ipa_norm", "ipa_core_degree", "ipa_nll_eval", "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill",
-    "ipa_binned_nll_scan", "ipa_expected_hist", "ipa_poisson_hist_toys", "ipa_sort_workspace_bytes", "ipa_events_sort",
+    "ipa_binned_nll_scan", "ipa_expected_hist", "ipa_poisson_hist_toys", "ipa_cls_teststat", "ipa_cls_count_ge",
+    "ipa_cls_from_counts", "ipa_sort_workspace_bytes", "ipa_events_sort",
     "ipa_fp64_peak_probe",
 )
 
@@ -70,6 +72,9 @@ def lib():
     L.ipa_binned_nll_scan.argtypes = [vp, i32, _Range, vp, vp, vp, vp, i64, vp, vp, sz, vp]
     L.ipa_expected_hist.restype = i32; L.ipa_expected_hist.argtypes = [i32, _Range, vp, d, d, d, vp, vp, sz, vp]
     L.ipa_poisson_hist_toys.restype = i32; L.ipa_poisson_hist_toys.argtypes = [vp, i32, vp, i64, vp, vp, sz, vp]
+    L.ipa_cls_teststat.restype = i32; L.ipa_cls_teststat.argtypes = [vp, i32, i64, i32, vp, vp, vp, vp, sz, vp]
+    L.ipa_cls_count_ge.restype = i32; L.ipa_cls_count_ge.argtypes = [vp, i64, vp, vp, vp]
+    L.ipa_cls_from_counts.restype = i32; L.ipa_cls_from_counts.argtypes = [vp, i64, vp, i64, vp, vp]
     L.ipa_sort_workspace_bytes.restype = sz; L.ipa_sort_workspace_bytes.argtypes = [i64, i64]
     L.ipa_events_sort.restype = i32; L.ipa_events_sort.argtypes = [vp, i64, vp, i64, vp, vp, sz, vp]
     L.ipa_fp64_peak_probe.restype = i32; L.ipa_fp64_peak_probe.argtypes = [i64, vp, vp]
@@ -267,6 +272,36 @@ def ipa_poisson_hist_toys(mean, seeds, ws=None, stream=None):
     out = torch.empty((T, nbins), dtype=torch.int32, device="cuda")  # uint32 payload
     _check(lib().ipa_poisson_hist_toys(_dptr(mean, torch.float64), nbins, _hptr(seeds), T, _dptr(out), _dptr(ws),
                                        ws.numel(), _stream(stream)))
+    return out
+
+
+def ipa_cls_teststat(counts, nu_sb, nu_b, ws=None, stream=None):
+    """q[T] of T histograms counts[T, nbins] (int32 payload = uint32 toys, int64 payload = uint64 data)."""
+    _need_cuda()
+    nbins = nu_b.numel()
+    assert counts.dtype in (torch.int32, torch.int64) and counts.numel() % nbins == 0
+    T = counts.numel() // nbins
+    ws = _ws(ws, 0, 1, nbins)
+    q = torch.empty(T, dtype=torch.float64, device="cuda")
+    _check(lib().ipa_cls_teststat(_dptr(counts), counts.element_size(), T, nbins, _dptr(nu_sb, torch.float64),
+                                  _dptr(nu_b, torch.float64), _dptr(q), _dptr(ws), ws.numel(), _stream(stream)))
+    return q
+
+
+def ipa_cls_count_ge(q, q_obs, stream=None):
+    """-> int64 device tensor [1]: number of q >= q_obs[0] (q_obs a device tensor)."""
+    _need_cuda()
+    out = torch.empty(1, dtype=torch.int64, device="cuda")
+    _check(lib().ipa_cls_count_ge(_dptr(q, torch.float64), q.numel(), _dptr(q_obs, torch.float64), _dptr(out), _stream(stream)))
+    return out
+
+
+def ipa_cls_from_counts(count_sb, T_sb, count_b, T_b, stream=None):
+    """-> device tensor [CL_sb, CL_b, CL_s]."""
+    _need_cuda()
+    out = torch.empty(3, dtype=torch.float64, device="cuda")
+    _check(lib().ipa_cls_from_counts(_dptr(count_sb, torch.int64), int(T_sb), _dptr(count_b, torch.int64), int(T_b),
+                                     _dptr(out), _stream(stream)))
     return out
 
 

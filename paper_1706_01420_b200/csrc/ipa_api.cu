@@ -347,6 +347,52 @@ int ipa_poisson_hist_toys(const double* mean_dev, int nbins, const uint64_t* see
   return IPA_OK;
 }
 
+int ipa_cls_teststat(const void* counts_dev, int count_bytes, int64_t T, int nbins, const double* nu_sb_dev,
+                     const double* nu_b_dev, double* q_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (!counts_dev || (count_bytes != 4 && count_bytes != 8) || T < 1 || T > 0x7fffffffLL || nbins < 1 || !nu_sb_dev ||
+      !nu_b_dev || !q_dev)
+    return IPA_ERR_INVALID_ARG;
+  const Layout L = make_layout(1, nbins);
+  if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* ws = static_cast<char*>(ws_dev);
+  double* lr = reinterpret_cast<double*>(ws + L.sbin);
+  double* csum = reinterpret_cast<double*>(ws + L.pts);
+  ipa_cls_weights_kernel<<<1, 256, 0, st>>>(nu_sb_dev, nu_b_dev, nbins, lr, csum);
+  IPA_CK(cudaGetLastError());
+  // 128-bit loads need 16-byte aligned rows (and the weights are read in pairs)
+  const int vec_ok = (((uintptr_t)counts_dev % 16) == 0 && ((size_t)nbins * (size_t)count_bytes) % 16 == 0) ? 1 : 0;
+  const unsigned G = (unsigned)((T + 7) / 8);
+  if (count_bytes == 4)
+    ipa_cls_q_kernel<unsigned int><<<G, 256, 0, st>>>(static_cast<const unsigned int*>(counts_dev), T, nbins, vec_ok, lr,
+                                                      csum, q_dev);
+  else
+    ipa_cls_q_kernel<unsigned long long><<<G, 256, 0, st>>>(static_cast<const unsigned long long*>(counts_dev), T, nbins,
+                                                            vec_ok, lr, csum, q_dev);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
+int ipa_cls_count_ge(const double* q_dev, int64_t T, const double* q_obs_dev, int64_t* count_dev, void* cuda_stream) {
+  if (!q_dev || T < 1 || !q_obs_dev || !count_dev) return IPA_ERR_INVALID_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  IPA_CK(cudaMemsetAsync(count_dev, 0, 8, st));
+  int64_t G = (T + 255) / 256;
+  if (G > 1184) G = 1184;
+  ipa_cls_count_kernel<<<(unsigned)G, 256, 0, st>>>(q_dev, T, q_obs_dev, reinterpret_cast<unsigned long long*>(count_dev));
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
+int ipa_cls_from_counts(const int64_t* count_sb_dev, int64_t T_sb, const int64_t* count_b_dev, int64_t T_b,
+                        double* cl_dev, void* cuda_stream) {
+  if (!count_sb_dev || !count_b_dev || T_sb < 1 || T_b < 1 || !cl_dev) return IPA_ERR_INVALID_ARG;
+  ipa_cls_from_counts_kernel<<<1, 1, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+      reinterpret_cast<const long long*>(count_sb_dev), T_sb, reinterpret_cast<const long long*>(count_b_dev), T_b, cl_dev);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
 size_t ipa_sort_workspace_bytes(int64_t n, int64_t T) {
   if (n < 0 || T < 0) return 0;
   size_t bytes = 0;

@@ -850,6 +850,76 @@ ipa_binned_scan_kernel(const unsigned long long* __restrict__ counts, const doub
 }
 
 // ------------------------------------------------------------------------------------------------
+// CLs on binned toys (reading F2):
+//   q_t = 2 [ C - sum_b n_tb lr_b ],  lr_b = log(nu_sb_b / nu_b_b),  C = sum_b (nu_sb_b - nu_b_b).
+// ------------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256)
+ipa_cls_weights_kernel(const double* __restrict__ nu_sb, const double* __restrict__ nu_b, int nbins,
+                       double* __restrict__ lr, double* __restrict__ csum) {
+  __shared__ double red[8];
+  double part = 0.0;
+  for (int b = threadIdx.x; b < nbins; b += 256) {
+    lr[b] = log(nu_sb[b] / nu_b[b]);
+    part += nu_sb[b] - nu_b[b];
+  }
+  const double tot = ipa_block_sum_256(part, red);
+  if (threadIdx.x == 0) *csum = tot;
+}
+
+// one WARP per toy histogram (8 per block); the counts (4 or 8 bytes each) are the only HBM stream and are
+// read with 128-bit loads when the rows are 16-byte aligned; lanes add in a fixed order, then a shuffle tree.
+template <class CT>
+__global__ void __launch_bounds__(256)
+ipa_cls_q_kernel(const CT* __restrict__ counts, long long T, int nbins, int vec_ok, const double* __restrict__ lr,
+                 const double* __restrict__ csum, double* __restrict__ q) {
+  const int lane = threadIdx.x & 31;
+  const long long t = blockIdx.x * 8LL + (threadIdx.x >> 5);
+  if (t >= T) return;
+  const CT* row = counts + t * nbins;
+  double acc = 0.0;
+  constexpr int V = 16 / (int)sizeof(CT);          // counts per 128-bit load: 4 or 2
+  int done = 0;
+  if (vec_ok) {
+    const int nv = nbins / V;
+    for (int i = lane; i < nv; i += 32) {
+      if (V == 4) {
+        const uint4 c = __ldcs(reinterpret_cast<const uint4*>(row) + i);
+        const double2 l0 = reinterpret_cast<const double2*>(lr)[2 * i], l1 = reinterpret_cast<const double2*>(lr)[2 * i + 1];
+        acc = fma((double)c.x, l0.x, acc); acc = fma((double)c.y, l0.y, acc);
+        acc = fma((double)c.z, l1.x, acc); acc = fma((double)c.w, l1.y, acc);
+      } else {
+        const ulonglong2 c = __ldcs(reinterpret_cast<const ulonglong2*>(row) + i);
+        const double2 l0 = reinterpret_cast<const double2*>(lr)[i];
+        acc = fma((double)c.x, l0.x, acc); acc = fma((double)c.y, l0.y, acc);
+      }
+    }
+    done = nv * V;
+  }
+  for (int b = done + lane; b < nbins; b += 32) acc = fma((double)row[b], lr[b], acc);
+  acc = ipa_warp_sum(acc);
+  if (lane == 0) q[t] = 2.0 * (*csum - acc);
+}
+
+__global__ void __launch_bounds__(256)
+ipa_cls_count_kernel(const double* __restrict__ q, long long T, const double* __restrict__ q_obs,
+                     unsigned long long* __restrict__ count) {
+  const double thr = *q_obs;
+  unsigned int mine = 0;
+  for (long long i = blockIdx.x * 256LL + threadIdx.x; i < T; i += 256LL * gridDim.x) mine += (q[i] >= thr) ? 1u : 0u;
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) mine += __shfl_xor_sync(IPA_FULL, mine, o);
+  if ((threadIdx.x & 31) == 0 && mine) atomicAdd(count, (unsigned long long)mine);   // integer: exact, order-free
+}
+
+__global__ void ipa_cls_from_counts_kernel(const long long* count_sb, long long T_sb, const long long* count_b,
+                                           long long T_b, double* cl) {
+  const double sb = (double)*count_sb / (double)T_sb, b = (double)*count_b / (double)T_b;
+  cl[0] = sb;
+  cl[1] = b;
+  cl[2] = (*count_b > 0) ? sb / b : NAN;
+}
+
+// ------------------------------------------------------------------------------------------------
 // Per-bin Poisson toys (B3)
 // ------------------------------------------------------------------------------------------------
 __global__ void __launch_bounds__(256)

@@ -466,3 +466,53 @@ def test_config5_full_size(ipa, torch_, orc):
         # property over all toys: pulls of the counts are standard normal
         pull = (t.astype(np.float64) - nu_ref[None, :]) / np.sqrt(nu_ref[None, :])
         assert abs(pull.mean()) < 3e-3 and abs(pull.std() - 1.0) < 3e-3
+
+
+# ---------------------------------------------------------------------------------------------
+# CLs on binned toys (reading F2)
+# ---------------------------------------------------------------------------------------------
+def test_cls_teststat_counts_and_levels(ipa, torch_, orc):
+    n, nbins, T = 10_000_000, 1000, 5000
+    x = inp.standin_masses(5, n, f=2.5e-4)                       # "data": 2 500 signal-like events in 1e7
+    data = ipa.ipa_hist_fill(dev(torch_, x), LO, HI, nbins)       # uint64 payload
+    c_ref = orc.hist_fill(x, LO, HI, nbins)
+    ns, k = 2500.0, -0.002
+    nu_b = ipa.ipa_expected_hist(nbins, LO, HI, inp.GEN, 0.0, float(n), k)
+    nu_sb = ipa.ipa_expected_hist(nbins, LO, HI, inp.GEN, ns, float(n) - ns, k)
+    nu_b_ref = orc.expected_hist(nbins, LO, HI, inp.GEN, 0.0, float(n), k)
+    nu_sb_ref = orc.expected_hist(nbins, LO, HI, inp.GEN, ns, float(n) - ns, k)
+    toys_b = ipa.ipa_poisson_hist_toys(nu_b, np.arange(1, T + 1, dtype=np.uint64))
+    toys_sb = ipa.ipa_poisson_hist_toys(nu_sb, np.arange(T + 1, 2 * T + 1, dtype=np.uint64))
+    q_obs = ipa.ipa_cls_teststat(data, nu_sb, nu_b)
+    q_b = ipa.ipa_cls_teststat(toys_b, nu_sb, nu_b)
+    q_sb = ipa.ipa_cls_teststat(toys_sb, nu_sb, nu_b)
+    c_b = ipa.ipa_cls_count_ge(q_b, q_obs)
+    c_sb = ipa.ipa_cls_count_ge(q_sb, q_obs)
+    cl = ipa.ipa_cls_from_counts(c_sb, T, c_b, T)
+    torch_.cuda.synchronize()
+    # statistic: the oracle on the GPU's own toy histograms and expected histograms' oracle twins
+    scale = 2.0 * ns                                              # size of the two terms that cancel in q
+    for q_gpu, toys in ((q_b, toys_b), (q_sb, toys_sb)):
+        ref = orc.cls_teststat(toys.cpu().numpy().astype(np.uint32), nu_sb_ref, nu_b_ref)
+        assert np.all(np.abs(q_gpu.cpu().numpy() - ref) <= 1e-10 * (np.abs(ref) + scale))
+    ref_obs = orc.cls_teststat(c_ref.reshape(1, -1), nu_sb_ref, nu_b_ref)[0]
+    assert abs(q_obs.item() - ref_obs) <= 1e-10 * (abs(ref_obs) + scale)
+    # counting is integer work: exact against the oracle on the GPU's q values
+    qb, qsb = q_b.cpu().numpy(), q_sb.cpu().numpy()
+    assert c_b.item() == orc.cls_count_ge(qb, q_obs.item()) and c_sb.item() == orc.cls_count_ge(qsb, q_obs.item())
+    assert np.array_equal(cl.cpu().numpy(), orc.cls_from_counts(c_sb.item(), T, c_b.item(), T), equal_nan=True)
+    # ragged shapes: rows that are not 16-byte aligned take the scalar loads (both count widths)
+    rng = np.random.Generator(np.random.Philox(8))
+    for nb_, T_ in ((7, 9), (1, 3), (1001, 17)):
+        vb = rng.uniform(0.5, 300.0, nb_)
+        vsb = vb * rng.uniform(1.0, 1.5, nb_)
+        cnt = rng.poisson(vb, size=(T_, nb_))
+        for dt_np, dt_t in ((np.uint32, torch_.int32), (np.uint64, torch_.int64)):
+            qg = ipa.ipa_cls_teststat(dev(torch_, cnt.astype(np.int64)).to(dt_t), dev(torch_, vsb), dev(torch_, vb))
+            ref = orc.cls_teststat(cnt.astype(dt_np), vsb, vb)
+            assert np.all(np.abs(qg.cpu().numpy() - ref) <= 1e-10 * (np.abs(ref) + 2 * (vsb - vb).sum()))
+    # properties at this size: q is larger (more background-like) on background-only toys, so CL_b >= CL_sb for any
+    # observed value, and the two ensembles are separated by about the expected significance (2.5 sigma here)
+    v = cl.cpu().numpy()
+    assert 0.0 <= v[0] <= v[1] <= 1.0
+    assert (qb.mean() - qsb.mean()) > 1.5 * max(qb.std(), qsb.std())
