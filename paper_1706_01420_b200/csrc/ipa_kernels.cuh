@@ -1,12 +1,13 @@
 // ipa_kernels.cuh -- sm_100a kernels of the hot path.  Included once, by
 // ipa_api.cu.  Steps of SURVEY.md 8(a): prologue A1a-A1e, streaming NLL A2-A5 (K sets per event
-// read), segmented NLL T2, generators T0/T1, histogram B1, binned scan B2, per-bin Poisson toys B3.
+// read), segmented NLL T2, generators T0/T1, histogram B1, binned scan B2, per-bin Poisson toys B3,
+// CLs statistic on binned toys (row f2 of 8(f)).
 #pragma once
 #include <cuda_runtime.h>
 #include "ipa_prologue.cuh"
 
-#define IPA_BLOCK 128                     // threads per streaming block
-#define IPA_E 8                           // events per thread and tile (register blocking)
+#define IPA_BLOCK 128                     // threads per block of the segmented-NLL and generator kernels
+#define IPA_E 8                           // events per thread and tile in the segmented kernel
 #define IPA_TILE (IPA_BLOCK * IPA_E)
 #define IPA_BLOCKS_PER_SM 4
 #define IPA_SEGC 8                        // blocks per segment in the segmented kernel
@@ -295,9 +296,9 @@ __device__ __forceinline__ double ipa_warp_sum(double v) {
 }
 
 // ------------------------------------------------------------------------------------------------
-// Streaming NLL: persistent grid, tile = 256 threads x 4 events (two 128-bit loads per thread, the
-// next tile prefetched into registers while the current one is evaluated), all K sets per event
-// read.  partials[k*G + b]; the last block to finish adds them in a fixed order (A5).
+// Streaming NLL: persistent grid of one IPA_NB-thread block per SM, tile = IPA_NB threads x IPA_NE events
+// staged global -> shared with cp.async two tiles deep, all K sets per event read.
+// partials[k*G + b]; the last block to finish adds them in a fixed order (A5).
 // ------------------------------------------------------------------------------------------------
 #ifndef IPA_NB
 #define IPA_NB 512
