@@ -22,6 +22,8 @@
 __constant__ double ipa_c_exp[IPA_EXP_DEG + 1] = IPA_EXP_COEFS;
 __constant__ double ipa_c_log1p[IPA_LOG_DEG] = IPA_LOG1P_COEFS;
 __constant__ double2 ipa_c_logtab[33] = IPA_LOG_TABLE;
+__device__ const long long ipa_d_chebT[IPA_CHEB_NC * IPA_CHEB_NC] = IPA_CHEB_TABLE;   // global memory: per-lane index
+static const long long ipa_h_chebT[IPA_CHEB_NC * IPA_CHEB_NC] = IPA_CHEB_TABLE;
 __constant__ double ipa_c_gl16x[16] = IPA_GL16_X;
 __constant__ double ipa_c_gl16w[16] = IPA_GL16_W;
 // host copies (tests/devmath_host.cu only)
@@ -36,7 +38,9 @@ static const ipa_host_double2 ipa_h_logtab[33] = IPA_LOG_TABLE;
 #define IPA_CLOG(j) ipa_c_log1p[j]
 #define IPA_GL16X(i) ipa_c_gl16x[i]
 #define IPA_GL16W(i) ipa_c_gl16w[i]
+#define IPA_CHEBT(j, k) ipa_d_chebT[(j) * IPA_CHEB_NC + (k)]
 #else
+#define IPA_CHEBT(j, k) ipa_h_chebT[(j) * IPA_CHEB_NC + (k)]
 #define IPA_GL16X(i) ipa_h_gl16x[i]
 #define IPA_GL16W(i) ipa_h_gl16w[i]
 #define IPA_CEXP(j) ipa_h_exp[j]

@@ -30,6 +30,7 @@ ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_param
     if (set == 0 && counter) *counter = 0u;
   }
   __syncthreads();
+  ipa_pro_load_table(w, tid, IPA_PRO_THREADS);
   ipa_pro_phase0(w, tid); __syncthreads();
   ipa_pro_phase1(w, tid); __syncthreads();
   ipa_pro_phase2(w, tid); __syncthreads();
@@ -39,29 +40,6 @@ ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_param
   ipa_pro_phase6(w, tid); __syncthreads();
   ipa_pro_phase7(w, tid); __syncthreads();
   ipa_pro_phase7b(w, tid); __syncthreads();
-  if (tid < 32 && !w.status && !w.mode) {
-    // one warp builds the integer table T[j][k] row by row in registers (lane holds columns k = lane and
-    // k = lane + 32; T[j][k] = 2 T[j-1][k-1] - T[j-2][k], the left neighbour comes by shuffle); same
-    // integers as ipa_pro_phase8_row, which the host build of the tests runs
-    const int D = w.degree;
-    long long p2a = 0, p2b = 0;                       // row j-2
-    long long p1a = (tid == 0) ? 1 : 0, p1b = 0;      // row j-1 (row 0 to start with)
-    w.T[0][tid] = p1a;
-    if (tid + 32 < IPA_NCOEF) w.T[0][tid + 32] = p1b;
-    for (int j = 1; j <= D; ++j) {
-      long long ua = __shfl_up_sync(IPA_FULL, p1a, 1);
-      long long ub = __shfl_up_sync(IPA_FULL, p1b, 1);
-      const long long wrap = __shfl_sync(IPA_FULL, p1a, 31);
-      if (tid == 0) { ua = 0; ub = wrap; }
-      long long va, vb;
-      if (j == 1) { va = (tid == 1) ? 1 : 0; vb = 0; }
-      else { va = 2 * ua - p2a; vb = 2 * ub - p2b; }
-      w.T[j][tid] = va;
-      if (tid + 32 < IPA_NCOEF) w.T[j][tid + 32] = vb;
-      p2a = p1a; p2b = p1b; p1a = va; p1b = vb;
-    }
-  }
-  __syncthreads();
   ipa_pro_phase8_finish(w, tid); __syncthreads();
   ipa_pro_phase9(w, tid); __syncthreads();
   ipa_pro_phase10(w, tid, IPA_PRO_THREADS); __syncthreads();

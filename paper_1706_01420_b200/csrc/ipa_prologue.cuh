@@ -67,7 +67,7 @@ struct IpaProWork {
   double ctab[4 * IPA_MCHEB];   // cos(pi m / (2 M)), m = 0 .. 4M-1 (Chebyshev nodes and the cosine transform)
   double tl_left, tl_right, NB, logNB, logf, log1mf, nulogalpha, expref;   // pieces of phase 12 computed by other warps in phase 11
   int degree, mode;
-  long long T[IPA_NCOEF][IPA_NCOEF];  // T[j][k] = integer coefficient of t^k in the Chebyshev polynomial T_j
+  long long T[IPA_NCOEF * IPA_NCOEF];  // copy of the integer Chebyshev table (loaded at kernel start, used in phase 8)
   double araw[IPA_NCOEF];
   double logG0, logG1, L0, L1;
   int npanel;
@@ -109,6 +109,13 @@ IPA_HD double ipa_logI(const IpaProWork& w, double d) {
 }
 
 // ================================ phases =========================================================
+// before phase 0: every thread copies its share of the integer Chebyshev table into the work area (the
+// loads are in flight during the first phases; per-lane reads from global memory in phase 8 cost as
+// much as building the table)
+IPA_HD void ipa_pro_load_table(IpaProWork& w, int tid, int nthr) {
+  for (int i = tid; i < IPA_NCOEF * IPA_NCOEF; i += nthr) w.T[i] = IPA_CHEBT(0, i);
+}
+
 // phase 0: validation (one thread)
 IPA_HD void ipa_pro_phase0(IpaProWork& w, int tid) {
   if (tid != 0) return;
@@ -271,23 +278,15 @@ IPA_HD void ipa_pro_phase7b(IpaProWork& w, int tid) {
   if (!(w.L0 > 0.0) || !(w.L1 < 0.0)) w.status = 2;
 }
 
-// phase 8: Chebyshev -> monomial, a_k = sum_j c_j T[j][k].
-// (a) integer table: row j from rows j-1 and j-2, T[j][k] = 2 T[j-1][k-1] - T[j-2][k]  (exact in int64 up
-//     to degree 47: |T[47][k]| < 2^59); one warp, one row per step.
-// (b) thread k accumulates its coefficient over the rows of matching parity in double-double.
-IPA_HD void ipa_pro_phase8_row(IpaProWork& w, int j, int k) {
-  if (w.status || w.mode || k >= IPA_NCOEF) return;
-  long long v;
-  if (j == 0) v = (k == 0) ? 1 : 0;
-  else if (j == 1) v = (k == 1) ? 1 : 0;
-  else v = (k > 0 ? 2 * w.T[j - 1][k - 1] : 0) - w.T[j - 2][k];
-  w.T[j][k] = v;
-}
+// phase 8: Chebyshev -> monomial, a_k = sum_j c_j T[j][k] with the integer coefficients T[j][k] of the
+// Chebyshev polynomials (generated table, exact in int64 up to degree 47: |T[47][k]| < 2^59; the host test
+// rebuilds it from T_{j+1} = 2 t T_j - T_{j-1}).  Thread k accumulates its coefficient over the rows of
+// matching parity in double-double.
 IPA_HD void ipa_pro_phase8_finish(IpaProWork& w, int k) {
   if (w.status || w.mode || k >= IPA_NCOEF) return;
   double ahi = 0.0, alo = 0.0;
   for (int j = k; j <= w.degree; j += 2) {
-    const long long v = w.T[j][k];
+    const long long v = w.T[j * IPA_NCOEF + k];
     double ph, pl, sh, sl;
     ipa_two_prod(w.c[j], (double)v, &ph, &pl);
     ipa_two_sum(ahi, ph, &sh, &sl);

@@ -13,6 +13,7 @@ static void run_prologue_host(const ipa_params& p, double lo, double hi, int pol
   w.p = p; w.lo = lo; w.hi = hi; w.policy = policy;
   const int NT = IPA_PRO_THREADS;
 #define ALL(stmt) for (int tid = 0; tid < NT; ++tid) { stmt; }
+  ALL(ipa_pro_load_table(w, tid, NT))
   ALL(ipa_pro_phase0(w, tid))
   ALL(ipa_pro_phase1(w, tid))
   ALL(ipa_pro_phase2(w, tid))
@@ -22,8 +23,6 @@ static void run_prologue_host(const ipa_params& p, double lo, double hi, int pol
   ALL(ipa_pro_phase6(w, tid))
   ALL(ipa_pro_phase7(w, tid))
   ALL(ipa_pro_phase7b(w, tid))
-  if (!w.status && !w.mode)
-    for (int j = 0; j <= w.degree; ++j) { ALL(ipa_pro_phase8_row(w, j, tid)) }
   ALL(ipa_pro_phase8_finish(w, tid))
   ALL(ipa_pro_phase9(w, tid))
   ALL(ipa_pro_phase10(w, tid, NT))
@@ -68,6 +67,21 @@ void emu_gl16(double* tab_x, double* tab_w, double* newton_x, double* newton_w) 
     tab_x[i] = IPA_GL16X(i); tab_w[i] = IPA_GL16W(i);
     ipa_gauss_legendre(16, i, &newton_x[i], &newton_w[i]);
   }
+}
+// generated integer Chebyshev table against the three-term recurrence; returns the number of mismatches
+int emu_cheb_table_mismatches() {
+  static long long T[IPA_CHEB_NC][IPA_CHEB_NC];
+  int bad = 0;
+  for (int j = 0; j < IPA_CHEB_NC; ++j)
+    for (int k = 0; k < IPA_CHEB_NC; ++k) {
+      long long v;
+      if (j == 0) v = (k == 0);
+      else if (j == 1) v = (k == 1);
+      else v = (k > 0 ? 2 * T[j - 1][k - 1] : 0) - T[j - 2][k];
+      T[j][k] = v;
+      bad += (IPA_CHEBT(j, k) != v);
+    }
+  return bad;
 }
 long long emu_poisson(unsigned long long seed, unsigned long long slot, unsigned stream, double mean) {
   return ipa_poisson(seed, slot, stream, mean);

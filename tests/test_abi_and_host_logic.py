@@ -159,3 +159,10 @@ def test_gauss_legendre_table(emu):
     assert np.abs(np.sort(tx) - gx).max() < 5e-16 and np.abs(tw[np.argsort(tx)] - gw).max() < 5e-16
     for deg in (0, 2, 30):
         assert abs((tw * tx ** deg).sum() - 2.0 / (deg + 1)) < 1e-15
+
+
+def test_chebyshev_integer_table(emu):
+    """The prologue's generated table of integer Chebyshev coefficients equals the three-term recurrence
+    T_{j+1} = 2 t T_j - T_{j-1} evaluated in int64 (48 x 48 entries)."""
+    emu.emu_cheb_table_mismatches.restype = C.c_int
+    assert emu.emu_cheb_table_mismatches() == 0
