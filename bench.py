@@ -397,9 +397,9 @@ def main():
     achieved = flops * n / t_kernel / 1e12
     peak = FP64_PEAK_NOMINAL / 1e12
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": 800.05e6 * n / 1e8,
-                "traffic_source": "ncu --set full dram__bytes_read.sum + write.sum of ipa_nll_kernel, profiles/ (per launch, "
-                                  "1e8 events; scaled by events)",
+                "traffic": (800.13e6 + 3.98e6) * n / 1e8,
+                "traffic_source": "ncu --set full dram__bytes_read.sum + dram__bytes_write.sum of ipa_nll_kernel, "
+                                  "profiles/r01_v13_nll_kernel.md (800.13 MB + 3.98 MB per launch of 1e8 events; scaled by events)",
                 "kernel": "ipa_nll_kernel<false>", "kernel_ms": t_kernel * 1e3,
                 "kernel_time_source": "CUDA events: step time minus a prologue-only loop of the same length",
                 "peak_source": "DESIGN.md section 6: 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no "
