@@ -516,3 +516,26 @@ def test_cls_teststat_counts_and_levels(ipa, torch_, orc):
     v = cl.cpu().numpy()
     assert 0.0 <= v[0] <= v[1] <= 1.0
     assert (qb.mean() - qsb.mean()) > 1.5 * max(qb.std(), qsb.std())
+
+
+# ---------------------------------------------------------------------------------------------
+# maximum sizes: more than 2^31 events (64-bit indexing end to end)
+# ---------------------------------------------------------------------------------------------
+def test_more_than_2_pow_31_events(ipa, torch_, orc):
+    n = 2 ** 31 + 4099                                         # 17.2 GB of events; ragged last tile
+    x = torch_.empty(n, dtype=torch_.float64, device="cuda")
+    half = n // 2
+    x[:half] = 5250.0                                          # core region
+    x[half:] = 5400.0                                          # right tail
+    sets = [inp.GEN, inp.P2]
+    nll, _, st = ipa.ipa_nll_eval(x, sets, LO, HI)
+    counts = ipa.ipa_hist_fill(x, LO, HI, 1000)
+    torch_.cuda.synchronize()
+    assert (st.cpu().numpy() == 0).all()
+    got = nll.cpu().numpy()
+    for i, p in enumerate(sets):
+        l = orc.logpdf(np.array([5250.0, 5400.0]), p, LO, HI)
+        ref = -(half * l[0] + (n - half) * l[1])
+        assert abs(got[i] - ref) <= 1e-10 * abs(ref)
+    c = counts.cpu().numpy()
+    assert int(c.sum()) == n and int(c[416]) == half and int(c[666]) == n - half   # bins of 5250 and 5400
