@@ -12,6 +12,7 @@
 #define IPA_BLOCKS_PER_SM 4
 #define IPA_SEGC 8                        // blocks per segment in the segmented kernel
 #define IPA_FULL 0xffffffffu
+#define IPA_GEN_ROUND 1024                // slots per warp and round in the toy generator
 
 struct IpaParamBatch { ipa_params p[IPA_MAX_K]; };
 
@@ -628,19 +629,6 @@ __device__ __forceinline__ double ipa_draw_background(double k, unsigned long lo
   return lo + log1p(u * expm1(t)) / k;
 }
 
-__device__ __forceinline__ double ipa_draw_signal(const IpaSetConsts& c, double logImax, unsigned long long seed,
-                                                  unsigned long long slot, double lo, double hi) {
-  double x = lo;
-  for (unsigned attempt = 0; attempt <= 100001u; ++attempt) {
-    double u1, u2;
-    ipa_uniforms2(seed, slot, attempt, IPA_STREAM_SIG, &u1, &u2);
-    x = lo + (hi - lo) * u1;
-    const double ratio = exp(ipa_logI_rec(c, x - c.mu) - logImax);
-    if (u2 * 1.02 < ratio) break;
-  }
-  return x;
-}
-
 // grid (T, chunks).  mixture != 0: T == 1, `capacity` events, component by u < f (configs 1-3).
 __global__ void __launch_bounds__(IPA_BLOCK)
 ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSetConsts* __restrict__ consts,
@@ -682,18 +670,68 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
   const long long beg = mixture ? 0 : offsets[t];
   const long long len = mixture ? capacity : offsets[t + 1] - beg;
   const long long ns = mixture ? 0 : nsig[t];
-  for (long long j = (long long)blockIdx.y * IPA_BLOCK + tid; j < len; j += (long long)gridDim.y * IPA_BLOCK) {
-    if (beg + j >= capacity) break;
-    bool is_sig;
-    if (mixture) {
-      double uc, v;
-      ipa_uniforms2(seed, (unsigned long long)j, 0u, IPA_STREAM_COMP, &uc, &v);
-      is_sig = uc < f;
-    } else {
-      is_sig = j < ns;
+  // Every event depends only on (seed, slot) -- the Philox counter is (slot, attempt) -- so the slots may be
+  // handed to the lanes in any order.  A warp owns a contiguous range of slots and works in rounds of
+  // IPA_GEN_ROUND slots: (A) classify, draw the background events, list the signal slots in shared memory;
+  // (B) accept-reject on the listed slots with REFILL: a lane whose attempt is accepted takes the next slot
+  // of the list, so the warp does not wait for its unluckiest lane (the attempt count is geometric with
+  // mean ~20 under the flat envelope).
+  __shared__ int s_list[IPA_BLOCK / 32][IPA_GEN_ROUND];
+  const long long nwarp = (long long)gridDim.y * (IPA_BLOCK / 32), wid = (long long)blockIdx.y * (IPA_BLOCK / 32) + warp;
+  long long lim = len;
+  if (beg + lim > capacity) lim = capacity - beg;          // nothing is written past the capacity
+  if (lim < 0) lim = 0;
+  const long long w0 = lim * wid / nwarp, w1 = lim * (wid + 1) / nwarp;
+  const unsigned lt = (1u << lane) - 1u;
+  int* list = s_list[warp];
+  for (long long r0 = w0; r0 < w1; r0 += IPA_GEN_ROUND) {
+    const int cnt = (int)((w1 - r0 < IPA_GEN_ROUND) ? (w1 - r0) : IPA_GEN_ROUND);
+    int nlist = 0;
+    for (int o = lane; o < ((cnt + 31) & ~31); o += 32) {
+      const long long j = r0 + o;
+      bool is_sig = false;
+      if (o < cnt) {
+        if (mixture) {
+          double uc, v;
+          ipa_uniforms2(seed, (unsigned long long)j, 0u, IPA_STREAM_COMP, &uc, &v);
+          is_sig = uc < f;
+        } else {
+          is_sig = j < ns;
+        }
+        if (!is_sig) x[beg + j] = ipa_draw_background(k, seed, (unsigned long long)j, lo, hi);
+      }
+      const unsigned m = __ballot_sync(IPA_FULL, is_sig);
+      if (is_sig) list[nlist + __popc(m & lt)] = o;
+      nlist += __popc(m);
     }
-    x[beg + j] = is_sig ? ipa_draw_signal(c, logImax, seed, (unsigned long long)j, lo, hi)
-                        : ipa_draw_background(k, seed, (unsigned long long)j, lo, hi);
+    __syncwarp();
+    int next = 0, item = -1;          // item: -1 = needs a slot, -2 = no slot left, >= 0 = offset in the round
+    unsigned attempt = 0;
+    while (true) {
+      const bool need = item == -1;
+      const unsigned m = __ballot_sync(IPA_FULL, need);
+      if (need) {
+        const int q = next + __popc(m & lt);
+        item = (q < nlist) ? list[q] : -2;
+        attempt = 0;
+      }
+      next += __popc(m);
+      if (!__any_sync(IPA_FULL, item >= 0)) break;
+      if (item >= 0) {
+        const unsigned long long j = (unsigned long long)(r0 + item);
+        double u1, u2;
+        ipa_uniforms2(seed, j, attempt, IPA_STREAM_SIG, &u1, &u2);
+        const double xx = lo + (hi - lo) * u1;
+        const double ratio = exp(ipa_logI_rec(c, xx - c.mu) - logImax);
+        if (u2 * 1.02 < ratio || attempt == 100001u) {
+          x[beg + (long long)j] = xx;
+          item = -1;
+        } else {
+          ++attempt;
+        }
+      }
+    }
+    __syncwarp();
   }
 }
 
