@@ -629,6 +629,24 @@ __device__ __forceinline__ double ipa_draw_background(double k, unsigned long lo
   return lo + log1p(u * expm1(t)) / k;
 }
 
+// log I(d) with the streaming kernels' own sqrt / log and the Horner groups (accept-reject attempt loop).
+// Direct-mode shapes fall back to ipa_logI_rec.
+template <class Tab>
+__device__ __forceinline__ double ipa_logI_fast(const IpaSetConsts& c, double cshift, double d, const Tab* tab) {
+  if (c.mode != 0) return ipa_logI_rec(c, d);
+  if (d < c.d0) return c.logG0 - c.n0 * ipa_flog(fma(c.uA0, d, c.uB0), tab);
+  if (d > c.d1) return c.logG1 - c.n1 * ipa_flog(fma(c.uA1, d, c.uB1), tab);
+  const double t = fma(c.tA, ipa_fsqrt(fma(d, d, c.delta2)), c.tB);
+  double P = 0.0;
+  for (int g = c.degree >> 2; g >= 1; --g) {
+    const double2 hi2 = *reinterpret_cast<const double2*>(c.a + 4 * g + 2);
+    const double2 lo2 = *reinterpret_cast<const double2*>(c.a + 4 * g);
+    P = fma(P, t, hi2.y); P = fma(P, t, hi2.x); P = fma(P, t, lo2.y); P = fma(P, t, lo2.x);
+  }
+  P = fma(P, t, c.a[3]); P = fma(P, t, c.a[2]); P = fma(P, t, c.a[1]);
+  return fma(c.beta, d, fma(P, t, cshift));      // cshift = araw0 - nu log alpha
+}
+
 // grid (T, chunks).  mixture != 0: T == 1, `capacity` events, component by u < f (configs 1-3).
 __global__ void __launch_bounds__(IPA_BLOCK)
 ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSetConsts* __restrict__ consts,
@@ -638,9 +656,11 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
   __shared__ IpaSetConsts c;
   __shared__ double red[IPA_BLOCK / 32];
   __shared__ double s_logImax;
+  __shared__ double2 s_tab[33];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const long long t = blockIdx.x;
   const long long g = gen_stride ? t : 0;
+  ipa_load_logtab(s_tab);
   {
     const double* src = reinterpret_cast<const double*>(consts + g);
     double* dst = reinterpret_cast<double*>(&c);
@@ -665,6 +685,7 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
   }
   __syncthreads();
   const double logImax = s_logImax;
+  const double cshift = c.araw0 - c.nu * log(c.alpha);
   const unsigned long long seed = seeds[t];
   const double f = c.fsig, k = c.kraw;
   const long long beg = mixture ? 0 : offsets[t];
@@ -722,7 +743,7 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
         double u1, u2;
         ipa_uniforms2(seed, j, attempt, IPA_STREAM_SIG, &u1, &u2);
         const double xx = lo + (hi - lo) * u1;
-        const double ratio = exp(ipa_logI_rec(c, xx - c.mu) - logImax);
+        const double ratio = ipa_fexp_neg(fmax(ipa_logI_fast(c, cshift, xx - c.mu, s_tab) - logImax, -700.0));
         if (u2 * 1.02 < ratio || attempt == 100001u) {
           x[beg + (long long)j] = xx;
           item = -1;
