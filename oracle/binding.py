@@ -44,6 +44,7 @@ def lib():
         L.orc_binned_nll_scan.argtypes = [vp, i32, d, d, vp, vp, vp, vp, i64, vp]
         L.orc_expected_hist.restype = i32; L.orc_expected_hist.argtypes = [i32, d, d, vp, d, d, d, vp]
         L.orc_poisson_hist_toys.restype = None; L.orc_poisson_hist_toys.argtypes = [vp, i32, vp, i64, vp]
+        L.orc_nll_gradient.restype = i32; L.orc_nll_gradient.argtypes = [vp, i64, vp, d, d, vp, vp]
         L.orc_cls_teststat.restype = None; L.orc_cls_teststat.argtypes = [vp, i32, i64, i32, vp, vp, vp]
         L.orc_cls_count_ge.restype = i64; L.orc_cls_count_ge.argtypes = [vp, i64, d]
         L.orc_cls_from_counts.restype = None; L.orc_cls_from_counts.argtypes = [i64, i64, i64, i64, vp]
@@ -245,3 +246,15 @@ def cls_from_counts(count_sb, T_sb, count_b, T_b):
     out = np.empty(3)
     lib().orc_cls_from_counts(int(count_sb), int(T_sb), int(count_b), int(T_b), _p(out))
     return out
+
+
+def nll_gradient(x, p, lo, hi):
+    """Analytic (nll, d nll / d (mu, sigma, f, k)) of one parameter set; SURVEY.md 8(f) row f1."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    P = pack_params(p)
+    assert P.shape[0] == 1
+    nll = np.empty(1)
+    g = np.empty(4)
+    st = lib().orc_nll_gradient(_p(x), x.size, _p(P), float(lo), float(hi), _p(nll), _p(g))
+    assert st == 0, st
+    return float(nll[0]), g

@@ -1,0 +1,71 @@
+"""Pins of the oracle's analytic NLL gradient (oracle/ipa_oracle.cpp orc_nll_gradient).
+The paper gives no derivative formulae (PAPER.md:36, 383 only mention analytic gradients), so the pins are:
+the derivative of the DEFINITION taken by mpmath (numerical differentiation at 40 digits of an mpmath-only
+restatement of C1-C3, including its quad-based normalisation), the second-order convergence of the oracle's
+own central differences towards the analytic value, and the exact limits f = 0, f = 1, k = 0."""
+import mpmath as mp
+import numpy as np
+import pytest
+
+import ipa_inputs as inp
+from test_oracle_ipatia import MPModel
+
+LO, HI = inp.LO, inp.HI
+NAMES = ("mu", "sigma", "f", "k")
+
+
+def mp_nll(p, xs):
+    m = MPModel(p)
+    return -sum(m.l(x) for x in xs)
+
+
+@pytest.mark.parametrize("shape", ["P1", "P2"])
+def test_gradient_vs_mpmath_derivative_of_the_definition(orc, shape):
+    mp.mp.dps = 40
+    theta = dict(inp.GEN if shape == "P1" else inp.P2)
+    xs = [5003.5, 5249.0, 5262.25, 5281.0, 5299.75, 5330.5, 5588.0]      # both tails, both sides of the core
+    nll, g = orc.nll_gradient(np.array(xs), theta, LO, HI)
+    assert abs(nll - float(mp_nll(theta, xs))) <= 1e-12 * abs(nll)
+    for j, name in enumerate(NAMES):
+        def f(v, name=name):
+            q = dict(theta)
+            q[name] = v
+            return mp_nll(q, xs)
+        h = mp.mpf(10) ** -12 * max(1, abs(theta[name]))
+        ref = (f(mp.mpf(theta[name]) + h) - f(mp.mpf(theta[name]) - h)) / (2 * h)   # 40 digits: error ~ h^2
+        assert abs(g[j] - float(ref)) <= 2e-9 * max(abs(float(ref)), 1.0 / inp.GRAD_SCALE[name] * 1e-3), (name, g[j], ref)
+
+
+def test_central_differences_converge_quadratically_to_the_analytic_gradient(orc):
+    # few events, none within the largest step of a join (the density is only C^1 there)
+    x = np.array([5010.0, 5120.0, 5236.0, 5266.0, 5279.0, 5291.5, 5322.0, 5470.0])
+    theta = inp.as_array(inp.P2)
+    _, g = orc.nll_gradient(x, theta, LO, HI)
+    for j, name in enumerate(NAMES):
+        errs = []
+        for scale in (1.0, 0.5):
+            h = scale * 20 * inp.FD_STEPS[name]
+            tp, tm = theta.copy(), theta.copy()
+            tp[inp.IDX[name]] += h
+            tm[inp.IDX[name]] -= h
+            fd = (orc.nll(x, tp, LO, HI)[0] - orc.nll(x, tm, LO, HI)[0]) / (2 * h)
+            errs.append(fd - g[j])
+        assert abs(errs[0]) < 1e-3 * max(1.0, abs(g[j]))
+        assert 3.0 < errs[0] / errs[1] < 5.0, (name, errs)        # O(h^2): halving h divides the error by 4
+
+
+def test_gradient_limits(orc):
+    x = orc.generate_mixture(7, 500, inp.GEN, LO, HI)
+    # f = 0: no dependence on the signal shape; f = 1: none on k; k = 0 uses the series of d ln N_B / d k
+    _, g0 = orc.nll_gradient(x, dict(inp.GEN, f=0.0), LO, HI)
+    assert g0[0] == 0.0 and g0[1] == 0.0
+    _, g1 = orc.nll_gradient(x, dict(inp.GEN, f=1.0), LO, HI)
+    assert g1[3] == 0.0
+    _, gk = orc.nll_gradient(x, dict(inp.GEN, k=0.0), LO, HI)
+    _, gk2 = orc.nll_gradient(x, dict(inp.GEN, k=1e-9), LO, HI)
+    assert np.all(np.abs(gk - gk2) <= 1e-6 * np.maximum(1.0, np.abs(gk)))
+    # at the generating parameters of a large sample every component is small in units of its error
+    xl = orc.generate_mixture(2, 100000, inp.GEN, LO, HI)
+    _, g = orc.nll_gradient(xl, inp.GEN, LO, HI)
+    s = np.array([inp.GRAD_SCALE[k] for k in NAMES]) / np.sqrt(10.0)
+    assert np.all(np.abs(g * s) < 5.0)
