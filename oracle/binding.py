@@ -44,6 +44,7 @@ def lib():
         L.orc_binned_nll_scan.argtypes = [vp, i32, d, d, vp, vp, vp, vp, i64, vp]
         L.orc_expected_hist.restype = i32; L.orc_expected_hist.argtypes = [i32, d, d, vp, d, d, d, vp]
         L.orc_poisson_hist_toys.restype = None; L.orc_poisson_hist_toys.argtypes = [vp, i32, vp, i64, vp]
+        L.orc_norm_derivs.restype = i32; L.orc_norm_derivs.argtypes = [vp, d, d, vp]
         L.orc_nll_gradient.restype = i32; L.orc_nll_gradient.argtypes = [vp, i64, vp, d, d, vp, vp]
         L.orc_cls_teststat.restype = None; L.orc_cls_teststat.argtypes = [vp, i32, i64, i32, vp, vp, vp]
         L.orc_cls_count_ge.restype = i64; L.orc_cls_count_ge.argtypes = [vp, i64, d]
@@ -258,3 +259,12 @@ def nll_gradient(x, p, lo, hi):
     st = lib().orc_nll_gradient(_p(x), x.size, _p(P), float(lo), float(hi), _p(nll), _p(g))
     assert st == 0, st
     return float(nll[0]), g
+
+
+def norm_derivs(p, lo, hi):
+    """(d ln N_S / d mu, d ln N_S / d sigma, d ln N_B / d k) of one parameter set."""
+    P = pack_params(p)
+    out = np.empty(3)
+    st = lib().orc_norm_derivs(_p(P), float(lo), float(hi), _p(out))
+    assert st == 0, st
+    return out

@@ -444,6 +444,31 @@ static ld dsigma_integral_scaled(const Shape& s, ld A, ld B, ld logref) {
   }
   return prev;
 }
+/* d ln N_S / d mu, d ln N_S / d sigma, d ln N_B / d k  (N.NS is in units of exp(logref)) */
+static void norm_derivs(const Shape& s, const Norm& N, ld k, ld lo, ld hi, ld* dlnNS_dmu, ld* dlnNS_dsig, ld* dlnNB_dk) {
+  const ld dl = lo - s.mu, dh = hi - s.mu;
+  const ld dNS_dmu = expl(log_I(s, dl) - N.logref) - expl(log_I(s, dh) - N.logref);
+  ld dNS_dsig = 0;
+  ld cuts[6]; int nc = 0;
+  cuts[nc++] = dl;
+  const ld inner[3] = {s.d0, 0, s.d1};
+  for (int i = 0; i < 3; ++i) if (inner[i] > dl && inner[i] < dh) cuts[nc++] = inner[i];
+  cuts[nc++] = dh;
+  for (int i = 0; i + 1 < nc; ++i) dNS_dsig += dsigma_integral_scaled(s, cuts[i], cuts[i + 1], N.logref);
+  *dlnNS_dmu = dNS_dmu / N.NS;
+  *dlnNS_dsig = dNS_dsig / N.NS;
+  const ld w = hi - lo, t = k * w;
+  *dlnNB_dk = (fabsl(t) < 1e-6L) ? w * (0.5L + t / 12) : w * expl(t) / expm1l(t) - 1 / k;
+}
+extern "C" int orc_norm_derivs(const orc_params* pp, double lo, double hi, double* out /* [3] */) {
+  const Shape s = make_shape(*pp);
+  if (s.status) return s.status;
+  const Norm N = make_norm(s, pp->k, lo, hi);
+  ld a, b, c;
+  norm_derivs(s, N, pp->k, lo, hi, &a, &b, &c);
+  out[0] = (double)a; out[1] = (double)b; out[2] = (double)c;
+  return 0;
+}
 extern "C" int orc_nll_gradient(const double* x, int64_t n, const orc_params* pp, double lo_, double hi_, double* nll,
                                 double* grad /* d NLL / d (mu, sigma, f, k) */) {
   const orc_params& p = *pp;
@@ -452,20 +477,9 @@ extern "C" int orc_nll_gradient(const double* x, int64_t n, const orc_params* pp
   const ld lo = lo_, hi = hi_, f = p.f, k = p.k;
   const Norm N = make_norm(s, k, lo, hi);
   const ld dl = lo - s.mu, dh = hi - s.mu;
-  /* d ln N_S / d mu, d ln N_S / d sigma (N.NS is in units of exp(logref)) */
-  const ld dNS_dmu = expl(log_I(s, dl) - N.logref) - expl(log_I(s, dh) - N.logref);
-  ld dNS_dsig = 0;
-  {
-    ld cuts[6]; int nc = 0;
-    cuts[nc++] = dl;
-    const ld inner[3] = {s.d0, 0, s.d1};
-    for (int i = 0; i < 3; ++i) if (inner[i] > dl && inner[i] < dh) cuts[nc++] = inner[i];
-    cuts[nc++] = dh;
-    for (int i = 0; i + 1 < nc; ++i) dNS_dsig += dsigma_integral_scaled(s, cuts[i], cuts[i + 1], N.logref);
-  }
-  const ld dlnNS_dmu = dNS_dmu / N.NS, dlnNS_dsig = dNS_dsig / N.NS;
-  const ld w = hi - lo, t = k * w;
-  const ld dlnNB_dk = (fabsl(t) < 1e-6L) ? w * (0.5L + t / 12) : w * expl(t) / expm1l(t) - 1 / k;
+  ld dlnNS_dmu, dlnNS_dsig, dlnNB_dk;
+  norm_derivs(s, N, k, lo, hi, &dlnNS_dmu, &dlnNS_dsig, &dlnNB_dk);
+  (void)dl; (void)dh;
   std::vector<double> g0((size_t)n), g1((size_t)n), g2((size_t)n), g3((size_t)n), l((size_t)n);
   for (int64_t i = 0; i < n; ++i) {
     const ld d = (ld)x[i] - s.mu;

@@ -43,6 +43,11 @@ struct alignas(16) IpaSetConsts {
   double fsig, kraw;            // f and k as given (generators)
   double beta, logG0, logG1, logNS, logref;  // for the generators / binned path: log I(d)
   double normS, normB;          // N_S, N_B (absolute)
+  // gradient kernel (row f1): derivatives of the normalisations and the constants of d log I / d (d, sigma)
+  double dlnNS_dmu, dlnNS_dsig, dlnNB_dk, nuosig;   // nuosig = nu / sigma
+  double invsig, mulo, L0, L1;                      // 1 / sigma, mu - lo, join slopes
+  double A0, A1, aL0, a2L1;                         // nu/sigma - a beta, nu/sigma + a2 beta, a L0, a2 L1
+  double c0s, c1s, invf, inv1mf;                    // (L0 - beta)/sigma, (L1 - beta)/sigma, 1/f, 1/(1-f)
   int32_t status, degree, mode, pure;
   int32_t hxl, hxr, pad0, pad1; // high words of the joins in x, mu+d0 and mu+d1 (0 / -1 if not positive): region
                                 // classification of a whole warp by integer min/max of the events' high words
@@ -65,7 +70,9 @@ struct IpaProWork {
   double Ks[IPA_NBTASK];        // scaled Bessel values e^z K(z) of the tasks
   double H[IPA_MCHEB], c[IPA_MCHEB];
   double ctab[4 * IPA_MCHEB];   // cos(pi m / (2 M)), m = 0 .. 4M-1 (Chebyshev nodes and the cosine transform)
-  double tl_left, tl_right, NB, logNB, logf, log1mf, nulogalpha, expref;   // pieces of phase 12 computed by other warps in phase 11
+  double tl_left, tl_right, NB, logNB, logf, log1mf, nulogalpha, expref;
+  double tl_left2, tl_right2, dlnNB_dk, Iedge_l, Iedge_h;   // sigma-derivative tail integrals, d ln N_B / d k, I at the range ends
+  double pval2[IPA_MAXPANEL * IPA_GL], psum2[IPA_MAXPANEL];   // pieces of phase 12 computed by other warps in phase 11
   int degree, mode;
   long long T[IPA_NCOEF * IPA_NCOEF];  // copy of the integer Chebyshev table (loaded at kernel start, used in phase 8)
   double araw[IPA_NCOEF];
@@ -101,6 +108,22 @@ IPA_HD double ipa_core_H(const IpaProWork& w, double r) {
 IPA_HD double ipa_core_logG(const IpaProWork& w, double d) {
   const double r = sqrt(fma(d, d, w.delta * w.delta));
   return ipa_core_H(w, r) - w.nu * log(w.alpha) + w.p.beta * d;
+}
+// L(d) - beta = -alpha (d/r) K_{nu-1}/K_nu = alpha (d/r) H'(z)  (H' = -K_{nu-1}/K_nu): derivative of the fitted
+// polynomial, dH/dz = (1/zh) sum_j j a_j t^{j-1}; direct mode evaluates the Bessel ratio
+IPA_HD double ipa_core_Lmb(const IpaProWork& w, double d) {
+  const double r = sqrt(fma(d, d, w.delta * w.delta));
+  const double z = w.alpha * r;
+  double Hp;
+  if (w.mode == 0) {
+    const double t = (z - w.zc) / w.zh;
+    double acc = 0.0;
+    for (int j = w.degree; j >= 1; --j) acc = fma(acc, t, (double)j * w.araw[j]);
+    Hp = acc / w.zh;
+  } else {
+    Hp = -ipa_besselk_scaled(w.nu - 1.0, z) / ipa_besselk_scaled(w.nu, z);
+  }
+  return w.alpha * (d / r) * Hp;
 }
 IPA_HD double ipa_logI(const IpaProWork& w, double d) {
   if (d < w.d0) return w.logG0 - w.p.n * log(1.0 - (d - w.d0) * w.L0 / w.p.n);
@@ -334,37 +357,59 @@ IPA_HD void ipa_pro_phase10(IpaProWork& w, int tid, int nthr) {
   for (int q = tid; q < w.npanel * IPA_GL; q += nthr) {
     const int pnl = q / IPA_GL, i = q % IPA_GL;
     const double c = 0.5 * (w.pa[pnl] + w.pb[pnl]), hl = 0.5 * (w.pb[pnl] - w.pa[pnl]);
-    w.pval[q] = w.glw[i] * hl * exp(ipa_core_logG(w, c + hl * w.glx[i]) - w.logref);
+    const double d = c + hl * w.glx[i];
+    const double g = w.glw[i] * hl * exp(ipa_core_logG(w, d) - w.logref);
+    w.pval[q] = g;
+    w.pval2[q] = g * (w.nu / w.p.sigma - (d / w.p.sigma) * ipa_core_Lmb(w, d));   // G dlogG/dsigma
   }
 }
 IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
   if (w.status) return;
   const ipa_params& p = w.p;
   if (tid < w.npanel) {
-    double s = 0.0;
-    for (int i = 0; i < IPA_GL; ++i) s += w.pval[tid * IPA_GL + i];
+    double s = 0.0, s2 = 0.0;
+    for (int i = 0; i < IPA_GL; ++i) { s += w.pval[tid * IPA_GL + i]; s2 += w.pval2[tid * IPA_GL + i]; }
     w.psum[tid] = s;
-  } else if (tid == 32) {          // left tail integral in units of exp(logref)  (reading C5)
-    double left = 0.0;
+    w.psum2[tid] = s2;
+  } else if (tid == 32) {          // left tail: int I and int I dlogI/dsigma, in units of exp(logref)  (reading C5)
+    // with u = 1 - (d-d0) L0/n:  dlogI/dsigma = A + [a L0 - c] / u + c,  A = nu/sigma - a beta,
+    // c = n (L0 - beta) / (L0 sigma);  int u^-n du and int u^-(n+1) du are ipa_powint(u, n), ipa_powint(u, n+1)
+    double left = 0.0, left2 = 0.0;
     if (w.dl < w.d0) {
       const double dr = fmin(w.d0, w.dh);
       const double ul = 1.0 - (w.dl - w.d0) * w.L0 / p.n, ur = 1.0 - (dr - w.d0) * w.L0 / p.n;
-      left = exp(w.logG0 - w.logref) * (p.n / w.L0) * (ipa_powint(ul, p.n) - ipa_powint(ur, p.n));
+      const double pre = exp(w.logG0 - w.logref) * (p.n / w.L0);
+      const double F = ipa_powint(ul, p.n) - ipa_powint(ur, p.n);
+      const double F1 = ipa_powint(ul, p.n + 1.0) - ipa_powint(ur, p.n + 1.0);
+      const double A = w.nu / p.sigma - p.a * p.beta, c = p.n * (w.L0 - p.beta) / (w.L0 * p.sigma);
+      left = pre * F;
+      left2 = pre * ((A + c) * F + (p.a * w.L0 - c) * F1);
     }
     w.tl_left = left;
-  } else if (tid == 64) {          // right tail integral
-    double right = 0.0;
+    w.tl_left2 = left2;
+  } else if (tid == 64) {          // right tail: dlogI/dsigma = A' + c' - (a2 L1 + c') / u,  c' = n2 (L1 - beta) / (L1 sigma)
+    double right = 0.0, right2 = 0.0;
     if (w.dh > w.d1) {
       const double dL = fmax(w.d1, w.dl);
       const double uh = 1.0 - (w.dh - w.d1) * w.L1 / p.n2, ul = 1.0 - (dL - w.d1) * w.L1 / p.n2;
-      right = exp(w.logG1 - w.logref) * (p.n2 / (-w.L1)) * (ipa_powint(uh, p.n2) - ipa_powint(ul, p.n2));
+      const double pre = exp(w.logG1 - w.logref) * (p.n2 / (-w.L1));
+      const double F = ipa_powint(uh, p.n2) - ipa_powint(ul, p.n2);
+      const double F1 = ipa_powint(uh, p.n2 + 1.0) - ipa_powint(ul, p.n2 + 1.0);
+      const double A = w.nu / p.sigma + p.a2 * p.beta, c = p.n2 * (w.L1 - p.beta) / (w.L1 * p.sigma);
+      right = pre * F;
+      right2 = pre * ((A + c) * F - (p.a2 * w.L1 + c) * F1);
     }
     w.tl_right = right;
-  } else if (tid == 96) {          // background normalisation (shifted by lo)
+    w.tl_right2 = right2;
+  } else if (tid == 96) {          // background normalisation (shifted by lo) and d ln N_B / d k
     const double wd = w.hi - w.lo, tk = p.k * wd;
     const double NB = (fabs(tk) < 1e-8) ? wd * (1.0 + 0.5 * tk + tk * tk / 6.0) : expm1(tk) / p.k;
     w.NB = NB;
     w.logNB = log(NB);
+    w.dlnNB_dk = (fabs(tk) < 1e-6) ? wd * (0.5 + tk / 12.0) : wd * exp(tk) / expm1(tk) - 1.0 / p.k;
+  } else if (tid == 224) {         // I at the ends of the range (d N_S / d mu = I(lo - mu) - I(hi - mu))
+    w.Iedge_l = exp(ipa_logI(w, w.dl) - w.logref);
+    w.Iedge_h = exp(ipa_logI(w, w.dh) - w.logref);
   } else if (tid == 128) {
     w.logf = (p.f > 0.0) ? log(p.f) : 0.0;
     w.log1mf = (p.f < 1.0) ? log1p(-p.f) : 0.0;
@@ -414,6 +459,16 @@ IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
   o.fsig = p.f; o.kraw = p.k;
   o.beta = p.beta; o.logG0 = w.logG0; o.logG1 = w.logG1; o.logNS = logNS; o.logref = w.logref;
   o.araw0 = w.mode ? 0.0 : w.araw[0];
+  double core2 = 0.0;
+  for (int i = 0; i < w.npanel; ++i) core2 += w.psum2[i];
+  o.dlnNS_dmu = (w.Iedge_l - w.Iedge_h) / NSr;
+  o.dlnNS_dsig = (w.tl_left2 + core2 + w.tl_right2) / NSr;
+  o.dlnNB_dk = pure ? 0.0 : w.dlnNB_dk;
+  o.nuosig = w.nu / p.sigma; o.invsig = 1.0 / p.sigma; o.mulo = p.mu - w.lo; o.L0 = w.L0; o.L1 = w.L1;
+  o.A0 = w.nu / p.sigma - p.a * p.beta; o.A1 = w.nu / p.sigma + p.a2 * p.beta;
+  o.aL0 = p.a * w.L0; o.a2L1 = p.a2 * w.L1;
+  o.c0s = (w.L0 - p.beta) / p.sigma; o.c1s = (w.L1 - p.beta) / p.sigma;
+  o.invf = 1.0 / p.f; o.inv1mf = 1.0 / (1.0 - p.f);
   const double xl = p.mu + w.d0, xr = p.mu + w.d1;
   o.hxl = (xl > 0.0) ? ipa_hi(xl) : 0;
   o.hxr = (xr > 0.0) ? ipa_hi(xr) : -1;

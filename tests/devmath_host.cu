@@ -35,12 +35,14 @@ static void run_prologue_host(const ipa_params& p, double lo, double hi, int pol
 extern "C" {
 int emu_sizeof_consts() { return (int)sizeof(IpaSetConsts); }
 double emu_besselk_scaled(double nu, double x) { return ipa_besselk_scaled(nu, x); }
-// out: status, degree, mode, normS, normB, delta2, alpha, logG0, logG1, L0 (= -uA0 n0), L1
+// out: status, degree, mode, normS, normB, delta2, alpha, logG0, logG1, L0 (= -uA0 n0), L1, d ln N_S/d mu,
+// d ln N_S/d sigma, d ln N_B/d k
 void emu_consts(const ipa_params* p, double lo, double hi, int policy, double* out) {
   IpaSetConsts c;
   run_prologue_host(*p, lo, hi, policy, &c);
   out[0] = c.status; out[1] = c.degree; out[2] = c.mode; out[3] = c.normS; out[4] = c.normB;
   out[5] = c.delta2; out[6] = c.alpha; out[7] = c.logG0; out[8] = c.logG1; out[9] = -c.uA0 * c.n0; out[10] = -c.uA1 * c.n1;
+  out[11] = c.dlnNS_dmu; out[12] = c.dlnNS_dsig; out[13] = c.dlnNB_dk;
 }
 void emu_logpdf(const ipa_params* p, double lo, double hi, int policy, const double* x, long long n, double* out) {
   IpaSetConsts c;

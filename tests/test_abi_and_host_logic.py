@@ -109,7 +109,7 @@ def test_device_bessel_vs_mpmath(emu):
 def test_device_math_vs_oracle(emu, orc, shape, policy):
     P = {"P1": inp.GEN, "P2": inp.P2, "direct": dict(inp.GEN, zeta=0.2)}[shape]
     p = inp.as_array(P)
-    out = np.zeros(11)
+    out = np.zeros(14)
     emu.emu_consts(p.ctypes.data, LO, HI, policy, out.ctypes.data)
     st, sc = orc.shape_consts(P)
     _, nm = orc.norm(P, LO, HI)
@@ -120,6 +120,10 @@ def test_device_math_vs_oracle(emu, orc, shape, policy):
     assert abs(out[3] / nm["NS"] - 1) <= 5e-14 and abs(out[4] / nm["NB"] - 1) <= 1e-15
     assert abs(np.sqrt(out[5]) / sc["delta"] - 1) <= 1e-14 and abs(out[6] / sc["alpha"] - 1) <= 1e-14
     assert abs(out[7] - sc["logG0"]) <= 1e-13 and abs(out[9] / sc["L0"] - 1) <= 1e-13 and abs(out[10] / sc["L1"] - 1) <= 1e-13
+    # row f1: derivatives of the normalisations (d ln N_S / d mu, d ln N_S / d sigma, d ln N_B / d k)
+    nd = orc.norm_derivs(P, LO, HI)
+    assert abs(out[11] - nd[0]) <= 1e-12 * max(abs(nd[0]), 1e-3)
+    assert abs(out[12] - nd[1]) <= 1e-11 * abs(nd[1]) and abs(out[13] - nd[2]) <= 1e-13 * abs(nd[2])
     n = 4000 if shape != "direct" else 400
     x = inp.standin_masses(1, n)
     x[:5] = [LO, HI, 5280.0, 5250.0, 5310.0]
