@@ -30,7 +30,8 @@
  *     and NLL = +inf, so that a minimiser stepping outside the domain can recover.  Status values:
  *     0 ok; 1 basic domain (non-finite field, sigma<=0, zeta<=0, a<=0, a2<=0, n<=0, n2<=0, f outside
  *     [0,1]); 2 join slope sign (L(d0)<=0 or L(d1)>=0: the power-law tail does not exist);
- *     3 internal numerical failure (normalisation not finite or not positive).
+ *     3 internal numerical failure (normalisation not finite or not positive); 4 (ipa_nll_grad_eval only)
+ *     f == 0 or f == 1.
  *   - Events outside [lo,hi] are evaluated by the same formulae (no clipping); NaN events give NaN.
  *     Any n >= 0 is accepted (n == 0 gives NLL = +0.0).
  *   - Determinism: for fixed device, build, n and launch geometry the results are bitwise
@@ -116,6 +117,18 @@ int ipa_core_degree(const ipa_params* p_host, int K, ipa_range r, int32_t* degre
 int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r,
                  double* nll_dev, double* logpdf_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
                  void* cuda_stream);
+
+/* NLL and its ANALYTIC gradient with respect to (mu, sigma, f, k) in one pass (the
+ * paper mentions analytic gradients through iminuit and generated derivative code, PAPER.md:36, 383,
+ * without formulae; the derivatives are those of the definition above):
+ *   nll_dev  [K]    as ipa_nll_eval (same value up to rounding: the core term is evaluated with one Horner
+ *                   pass for the polynomial and its derivative)
+ *   grad_dev [4*K]  d NLL / d (mu, sigma, f, k) of set k at grad_dev[4 k .. 4 k + 3]
+ * Needs 0 < f < 1: a set with f == 0 or f == 1 gets status 4, NLL = +inf and NaN derivatives.  Every
+ * set streams the events on its own (the call is meant for one or a few sets).  K <= IPA_MAX_K. */
+int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r,
+                      double* nll_dev, double* grad_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
+                      void* cuda_stream);
 
 /* Same likelihood over T segments (toys, categories) of one event array, one parameter set per
  * segment, all in one launch (BASELINE.json config 4; PAPER.md:139-149 loops categories on the host).

@@ -196,6 +196,35 @@ int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K
   return IPA_OK;
 }
 
+int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r,
+                      double* nll_dev, double* grad_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
+                      void* cuda_stream) {
+  if (n < 0 || (n > 0 && !x_dev) || !p_host || K < 1 || K > IPA_MAX_K || !range_ok(r) || !nll_dev || !grad_dev)
+    return IPA_ERR_INVALID_ARG;
+  if (((uintptr_t)x_dev % 8) != 0) return IPA_ERR_INVALID_ARG;
+  const Layout L = make_layout(K, 0);
+  if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
+  int sms = 0;
+  int rc = device_info(&sms);
+  if (rc) return rc;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* ws = static_cast<char*>(ws_dev);
+  rc = run_prologue(p_host, K, r, ws, L, nullptr, nullptr, nullptr, st);
+  if (rc) return rc;
+  IPA_CK(cudaMemsetAsync(ws + L.counter, 0, 256, st));          // one ticket counter per set
+  const int64_t tile_n = (int64_t)IPA_GB * IPA_GE, ntiles = (n + tile_n - 1) / tile_n;
+  int64_t G = (int64_t)sms * 2;
+  if (G > ntiles) G = ntiles;
+  if (G < 1) G = 1;
+  if (G * 5 > kGridMax) G = kGridMax / 5;                        // partials: K x 5 x G doubles fit the K x kGridMax area
+  const int vec_ok = ((uintptr_t)x_dev % 16) == 0;
+  ipa_nll_grad_kernel<<<dim3((unsigned)G, (unsigned)K), IPA_GB, 0, st>>>(
+      x_dev, n, vec_ok, reinterpret_cast<const IpaSetConsts*>(ws + L.consts), reinterpret_cast<double*>(ws + L.partials),
+      reinterpret_cast<unsigned int*>(ws + L.counter), nll_dev, grad_dev, status_dev);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
 int ipa_nll_eval_segmented(const double* x_dev, const int64_t* offsets_dev, int64_t T, const ipa_params* p_host,
                            ipa_range r, double* nll_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
                            void* cuda_stream) {

@@ -92,6 +92,21 @@ IPA_HD double ipa_fsqrt(double q) {
   return fma(g, p, g);
 }
 
+// 1/u, u > 0 normal: reciprocal seed (about 20 good bits, MUFU.RCP64H on the device) + two Newton steps.
+IPA_HD double ipa_frcp(double u) {
+#ifdef __CUDA_ARCH__
+  double y;
+  asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(u));
+#else
+  double y = 1.0 / u;
+  y = ipa_mk(ipa_hi(y), 0);
+#endif
+  double e = fma(-u, y, 1.0);
+  y = fma(y, e, y);
+  e = fma(-u, y, 1.0);
+  return fma(y, e, y);
+}
+
 // e^a for a <= 0 (|a| is clamped to about 64 by the caller or here: results below 1e-27 are not
 // distinguished).  n = round(a log2 e) by the 1.5 2^52 shift, Cody-Waite reduction with a 32-bit
 // ln2_hi, degree-11 polynomial, scaling through the exponent field.  15 FP64 instructions.

@@ -484,6 +484,183 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
 }
 
 // ------------------------------------------------------------------------------------------------
+// Analytic gradient: per event l and d l / d (mu, sigma, f, k) from the chain rule
+// (formulae: oracle/ipa_oracle.cpp orc_nll_gradient):
+//   core  Delta = H(t) + (beta-k) d, with H and dH/dt from one Horner pass (a[0] carries the constants);
+//         L - beta = tA d (1/r) dH/dt;  dlogI/dd = beta + (L-beta);  dlogI/dsigma = nu/sigma - (d/sigma)(L-beta)
+//   tails u = uA d + uB;  dlogI/dd = L_j / u;  dlogI/dsigma = A_j -+ (a_j L_j -+ (d - d_j) c_j) / u
+//   w_S = sigmoid(Delta), w_B = 1 - w_S from the same e^{-|Delta|} as the softplus
+// The region of the whole warp is decided as in the NLL kernel; a mixed warp branches per event.
+// ------------------------------------------------------------------------------------------------
+template <class Tab>
+IPA_HD void ipa_grad_core(const IpaSetConsts& c, double d, double& D, double& dd, double& ds) {
+  const double q = fma(d, d, c.delta2);
+  const double r = ipa_fsqrt(q);
+  const double rinv = ipa_frcp(r);
+  const double t = fma(c.tA, r, c.tB);
+  double P = 0.0, Pd = 0.0;
+  for (int j = 4 * (c.degree >> 2) + 3; j >= 0; --j) {
+    Pd = fma(Pd, t, P);
+    P = fma(P, t, c.a[j]);
+  }
+  const double Lmb = c.tA * d * rinv * Pd;
+  D = fma(c.bmk, d, P);
+  dd = c.beta + Lmb;
+  ds = fma(-d * c.invsig, Lmb, c.nuosig);
+}
+template <class Tab>
+IPA_HD void ipa_grad_tail(const IpaSetConsts& c, bool right, double d, double& D, double& dd, double& ds, const Tab* tab) {
+  if (!right) {
+    const double u = fma(c.uA0, d, c.uB0), ru = ipa_frcp(u);
+    D = fma(-c.kd, d, fma(-c.n0, ipa_flog(u, tab), c.cT0));
+    dd = c.L0 * ru;
+    ds = fma(fma(-(d - c.d0), c.c0s, c.aL0), ru, c.A0);
+  } else {
+    const double u = fma(c.uA1, d, c.uB1), ru = ipa_frcp(u);
+    D = fma(-c.kd, d, fma(-c.n1, ipa_flog(u, tab), c.cT1));
+    dd = c.L1 * ru;
+    ds = fma(-fma(d - c.d1, c.c1s, c.a2L1), ru, c.A1);
+  }
+}
+// mixture: l = E_B + log(1 + e^Delta) and the four derivative contributions
+template <class Tab>
+IPA_HD void ipa_grad_mix(const IpaSetConsts& c, double d, double D, double dd, double ds, double& l, double& gm, double& gs,
+                         double& gf, double& gk, const Tab* tab) {
+  const double w = ipa_fexp_neg(ipa_neg_abs_clamped(D));
+  const double s1 = 1.0 + w;
+  const double rs = ipa_frcp(s1);
+  const bool pos = ipa_hi(D) >= 0;
+  const double wS = pos ? rs : w * rs, wB = pos ? w * rs : rs;
+  l = fma(c.kd, d, c.eB0) + ipa_relu_bits(D) + ipa_flog_1to2(s1, tab);
+  gm = wS * (-dd - c.dlnNS_dmu);
+  gs = wS * (ds - c.dlnNS_dsig);
+  gf = fma(wS, c.invf, -wB * c.inv1mf);
+  gk = wB * ((d + c.mulo) - c.dlnNB_dk);
+}
+template <int E, class Tab>
+IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&l)[E], double (&gm)[E], double (&gs)[E],
+                          double (&gf)[E], double (&gk)[E], const Tab* tab) {
+  int hmin = ipa_hi(x[0]), hmax = hmin;
+#pragma unroll
+  for (int e = 1; e < E; ++e) {
+    const int h = ipa_hi(x[e]);
+    hmin = h < hmin ? h : hmin;
+    hmax = h > hmax ? h : hmax;
+  }
+  hmin = ipa_warp_min(hmin);
+  hmax = ipa_warp_max(hmax);
+  const bool sane = hmin > 0 && hmax < 0x7ff00000;
+  double d[E], D[E], dd[E], ds[E];
+#pragma unroll
+  for (int e = 0; e < E; ++e) d[e] = x[e] - c.mu;
+  if (sane && c.mode == 0 && hmin > c.hxl && hmax < c.hxr) {
+#pragma unroll
+    for (int e = 0; e < E; ++e) ipa_grad_core<Tab>(c, d[e], D[e], dd[e], ds[e]);
+  } else if (sane && (hmax < c.hxl || hmin > c.hxr)) {
+    const bool right = hmin > c.hxr;
+#pragma unroll
+    for (int e = 0; e < E; ++e) ipa_grad_tail<Tab>(c, right, d[e], D[e], dd[e], ds[e], tab);
+  } else {
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      if (d[e] < c.d0) ipa_grad_tail<Tab>(c, false, d[e], D[e], dd[e], ds[e], tab);
+      else if (d[e] > c.d1) ipa_grad_tail<Tab>(c, true, d[e], D[e], dd[e], ds[e], tab);
+      else if (c.mode == 0) ipa_grad_core<Tab>(c, d[e], D[e], dd[e], ds[e]);
+      else {   // direct mode: Bessel functions per event (slow path)
+        const double r = sqrt(fma(d[e], d[e], c.delta2)), z = c.alpha * r;
+        const double Lmb = -c.alpha * (d[e] / r) * ipa_besselk_scaled(c.nu - 1.0, z) / ipa_besselk_scaled(c.nu, z);
+        D[e] = fma(c.bmk, d[e], ipa_direct_H(c.nu, z) + c.a[0]);
+        dd[e] = c.beta + Lmb;
+        ds[e] = fma(-d[e] * c.invsig, Lmb, c.nuosig);
+      }
+    }
+  }
+#pragma unroll
+  for (int e = 0; e < E; ++e) ipa_grad_mix<Tab>(c, d[e], D[e], dd[e], ds[e], l[e], gm[e], gs[e], gf[e], gk[e], tab);
+}
+
+#define IPA_GB 256                        // threads per block of the gradient kernel
+#define IPA_GE 4                          // events per thread and tile
+// grid (G, K): every set streams the events on its own (the gradient call is made for one or a few sets);
+// per-thread register accumulators, fixed block tree, partials[(k 5 + c) G + b], the last block of each
+// set (ticket counter[k]) adds them in a fixed order.  out: nll[k], grad[4 k + (mu, sigma, f, k)].
+__global__ void __launch_bounds__(IPA_GB, 2)
+ipa_nll_grad_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaSetConsts* __restrict__ consts,
+                    double* __restrict__ partials, unsigned int* counters, double* __restrict__ nll_out,
+                    double* __restrict__ grad_out, int32_t* __restrict__ status_out) {
+  __shared__ IpaSetConsts c;
+  __shared__ double2 s_tab[33];
+  __shared__ double red[5][IPA_GB / 32];
+  __shared__ int s_last;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, k = blockIdx.y, G = gridDim.x;
+  {
+    const double* src = reinterpret_cast<const double*>(consts + k);
+    double* dst = reinterpret_cast<double*>(&c);
+    for (int i = tid; i < (int)(sizeof(IpaSetConsts) / 8); i += IPA_GB) dst[i] = src[i];
+    ipa_load_logtab(s_tab);
+  }
+  __syncthreads();
+  const int st = c.status ? c.status : ((c.pure || !(c.fsig > 0.0)) ? 4 : 0);   // 4: the gradient needs 0 < f < 1
+  double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+  if (!st) {
+    const long long tile_n = (long long)IPA_GB * IPA_GE, ntiles = (n + tile_n - 1) / tile_n;
+    const double xpad = (n > 0) ? x[n - 1] : 0.0;
+    for (long long tile = blockIdx.x; tile < ntiles; tile += G) {
+      const long long base = tile * tile_n;
+      double xv[IPA_GE];
+      if (vec_ok && base + tile_n <= n) {
+#pragma unroll
+        for (int p = 0; p < IPA_GE / 2; ++p) {
+          const double2 v = __ldcs(reinterpret_cast<const double2*>(x + base) + p * IPA_GB + tid);
+          xv[2 * p] = v.x;
+          xv[2 * p + 1] = v.y;
+        }
+      } else {
+#pragma unroll
+        for (int e = 0; e < IPA_GE; ++e) {
+          const long long i = base + 2LL * ((e >> 1) * IPA_GB + tid) + (e & 1);
+          xv[e] = (i < n) ? x[i] : xpad;
+        }
+      }
+      double l[IPA_GE], gm[IPA_GE], gs[IPA_GE], gf[IPA_GE], gk[IPA_GE];
+      ipa_eval_grad<IPA_GE>(c, xv, l, gm, gs, gf, gk, s_tab);
+#pragma unroll
+      for (int e = 0; e < IPA_GE; ++e) {
+        const long long i = base + 2LL * ((e >> 1) * IPA_GB + tid) + (e & 1);
+        if (i < n) { acc[0] += l[e]; acc[1] += gm[e]; acc[2] += gs[e]; acc[3] += gf[e]; acc[4] += gk[e]; }
+      }
+    }
+  }
+#pragma unroll
+  for (int q = 0; q < 5; ++q) {
+    const double v = ipa_warp_sum(acc[q]);
+    if (lane == 0) red[q][warp] = v;
+  }
+  __syncthreads();
+  if (tid < 5) {
+    double v = 0.0;
+    for (int w = 0; w < IPA_GB / 32; ++w) v += red[tid][w];
+    partials[((long long)k * 5 + tid) * G + blockIdx.x] = v;
+  }
+  __threadfence();
+  __syncthreads();
+  if (tid == 0) s_last = (atomicAdd(counters + k, 1u) == (unsigned)(G - 1));
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (warp < 5) {
+    double v = 0.0;
+    for (int i = lane; i < G; i += 32) v += __ldcg(partials + ((long long)k * 5 + warp) * G + i);
+    v = ipa_warp_sum(v);
+    if (lane == 0) {
+      const double r = st ? (warp == 0 ? INFINITY : NAN) : 0.0 - v;
+      if (warp == 0) { nll_out[k] = r; if (status_out) status_out[k] = st; }
+      else grad_out[4 * k + warp - 1] = r;
+    }
+  }
+}
+
+// ------------------------------------------------------------------------------------------------
 // Segmented NLL (T2): grid (T, IPA_SEGC); block (t, c) takes the c-th eighth of segment t with the
 // parameter set of that segment.
 // ------------------------------------------------------------------------------------------------

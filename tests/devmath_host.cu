@@ -55,6 +55,18 @@ void emu_logpdf(const ipa_params* p, double lo, double hi, int policy, const dou
     for (int e = 0; e < 8 && i + e < n; ++e) out[i + e] = l[e];
   }
 }
+// row f1: sums of l and of the four derivative contributions over n events (plain left-to-right sums)
+void emu_grad(const ipa_params* p, double lo, double hi, int policy, const double* x, long long n, double* out) {
+  IpaSetConsts c;
+  run_prologue_host(*p, lo, hi, policy, &c);
+  for (int q = 0; q < 5; ++q) out[q] = 0.0;
+  for (long long i = 0; i < n; i += 4) {
+    double xv[4], l[4], gm[4], gs[4], gf[4], gk[4];
+    for (int e = 0; e < 4; ++e) xv[e] = (i + e < n) ? x[i + e] : x[n - 1];
+    ipa_eval_grad<4>(c, xv, l, gm, gs, gf, gk, ipa_h_logtab);
+    for (int e = 0; e < 4 && i + e < n; ++e) { out[0] -= l[e]; out[1] -= gm[e]; out[2] -= gs[e]; out[3] -= gf[e]; out[4] -= gk[e]; }
+  }
+}
 void emu_logI(const ipa_params* p, double lo, double hi, const double* d, long long n, double* out) {
   IpaSetConsts c;
   run_prologue_host(*p, lo, hi, 0, &c);

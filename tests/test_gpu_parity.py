@@ -539,3 +539,42 @@ def test_more_than_2_pow_31_events(ipa, torch_, orc):
         assert abs(got[i] - ref) <= 1e-10 * abs(ref)
     c = counts.cpu().numpy()
     assert int(c.sum()) == n and int(c[416]) == half and int(c[666]) == n - half   # bins of 5250 and 5400
+
+
+# ---------------------------------------------------------------------------------------------
+# analytic gradient in one pass
+# ---------------------------------------------------------------------------------------------
+def test_analytic_gradient_vs_oracle(ipa, torch_, orc, x1):
+    for x in (x1, np.sort(x1), x1[:4099], x1[1:2050]):                 # unsorted / sorted / ragged / misaligned
+        xd = dev(torch_, x1)[1:2050] if x.size == 2049 else dev(torch_, x)
+        sets = [inp.GEN, inp.P2, dict(inp.GEN, zeta=0.2), dict(inp.GEN, f=0.0), dict(inp.GEN, f=1.0),
+                dict(inp.GEN, sigma=-1.0), dict(inp.P2, k=0.0)]
+        nll, grad, st = ipa.ipa_nll_grad_eval(xd, sets, LO, HI)
+        plain, _, _ = ipa.ipa_nll_eval(xd, sets, LO, HI)
+        torch_.cuda.synchronize()
+        nll, grad, st, plain = nll.cpu().numpy(), grad.cpu().numpy(), st.cpu().numpy(), plain.cpu().numpy()
+        assert list(st) == [0, 0, 0, 4, 4, 1, 0]
+        assert np.isposinf(nll[3:6]).all() and np.isnan(grad[3:6]).all()
+        for i in (0, 1, 2, 6):
+            ref_nll, ref_g = orc.nll_gradient(x, sets[i], LO, HI)
+            assert abs(nll[i] - ref_nll) <= 1e-10 * abs(ref_nll)
+            assert abs(nll[i] - plain[i]) <= 1e-12 * abs(plain[i])     # same value as ipa_nll_eval up to rounding
+            assert grad_ok(grad[i], ref_g), (i, grad[i], ref_g)
+
+
+def test_analytic_gradient_1e6_and_fit_minimum(ipa, torch_, orc):
+    n = 1_000_000
+    x = orc.generate_mixture(2, n, inp.GEN, LO, HI)
+    xd = ipa.ipa_events_sort(dev(torch_, x))
+    for theta in (inp.GEN, dict(inp.GEN, mu=5281.0, sigma=16.0, f=0.32, k=-0.0019)):
+        nll, grad, st = ipa.ipa_nll_grad_eval(xd, theta, LO, HI)
+        torch_.cuda.synchronize()
+        ref_nll, ref_g = orc.nll_gradient(x, theta, LO, HI)
+        assert st.item() == 0 and abs(nll.item() - ref_nll) <= 1e-10 * abs(ref_nll)
+        assert grad_ok(grad[0].cpu().numpy(), ref_g)
+    # consistency with the finite-difference batch of the same library (truncation error of the differences)
+    batch, h = inp.fd_batch(inp.GEN)
+    fd = inp.fd_gradient(ipa.ipa_nll_eval(xd, batch, LO, HI)[0].cpu().numpy(), h)
+    an = ipa.ipa_nll_grad_eval(xd, inp.GEN, LO, HI)[1][0].cpu().numpy()
+    s = np.array([inp.GRAD_SCALE[k] for k in inp.FLOATED])
+    assert np.all(np.abs(fd - an) <= 1e-3 * np.maximum(np.abs(an), 1.0 / s))
