@@ -356,6 +356,12 @@ def main():
         extras["k1_general_shape_P2"] = {"ms_per_call": dtp * 1e3, "events_per_s": n / dtp}
         ipa.ipa_set_degree_policy(1)
         step_k1()
+        # row f1: analytic gradient in one pass, beside the K = 9 finite-difference batch it replaces
+        for _ in range(2):
+            ipa.ipa_nll_grad_eval(x, P1, LO, HI, ws=ws, stream=stream)
+        dtg = timed(torch, lambda: ipa.ipa_nll_grad_eval(x, P1, LO, HI, ws=ws, stream=stream), k9steps, stream) / k9steps
+        extras["f1_analytic_gradient"] = {"ms_per_call": dtg * 1e3, "events_per_s": n / dtg,
+                                          "speedup_vs_k9_finite_differences": dt9 / dtg}
         extras.update(other_rows(torch, ipa, x_asis, ws, stream, n))
         # FP64 peak probe (DFMA chains), for the roofline denominator
         iters = 200000
