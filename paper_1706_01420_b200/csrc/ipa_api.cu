@@ -213,7 +213,7 @@ int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, 
   if (rc) return rc;
   IPA_CK(cudaMemsetAsync(ws + L.counter, 0, 256, st));          // one ticket counter per set
   const int64_t tile_n = (int64_t)IPA_GB * IPA_GE, ntiles = (n + tile_n - 1) / tile_n;
-  int64_t G = (int64_t)sms * 2;
+  int64_t G = (int64_t)sms * IPA_GPSM;
   if (G > ntiles) G = ntiles;
   if (G < 1) G = 1;
   if (G * 5 > kGridMax) G = kGridMax / 5;                        // partials: K x 5 x G doubles fit the K x kGridMax area

@@ -554,8 +554,34 @@ IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&
 #pragma unroll
   for (int e = 0; e < E; ++e) d[e] = x[e] - c.mu;
   if (sane && c.mode == 0 && hmin > c.hxl && hmax < c.hxr) {
+    // all E events in the core: one pass over the coefficients (128-bit uniform loads) for H and dH/dt of all of them
+    double t[E], rinv[E], P[E], Pd[E];
 #pragma unroll
-    for (int e = 0; e < E; ++e) ipa_grad_core<Tab>(c, d[e], D[e], dd[e], ds[e]);
+    for (int e = 0; e < E; ++e) {
+      const double r = ipa_fsqrt(fma(d[e], d[e], c.delta2));
+      rinv[e] = ipa_frcp(r);
+      t[e] = fma(c.tA, r, c.tB);
+      P[e] = 0.0;
+      Pd[e] = 0.0;
+    }
+    for (int g = c.degree >> 2; g >= 0; --g) {
+      const double2 hi2 = *reinterpret_cast<const double2*>(c.a + 4 * g + 2);
+      const double2 lo2 = *reinterpret_cast<const double2*>(c.a + 4 * g);
+#pragma unroll
+      for (int e = 0; e < E; ++e) {
+        Pd[e] = fma(Pd[e], t[e], P[e]); P[e] = fma(P[e], t[e], hi2.y);
+        Pd[e] = fma(Pd[e], t[e], P[e]); P[e] = fma(P[e], t[e], hi2.x);
+        Pd[e] = fma(Pd[e], t[e], P[e]); P[e] = fma(P[e], t[e], lo2.y);
+        Pd[e] = fma(Pd[e], t[e], P[e]); P[e] = fma(P[e], t[e], lo2.x);
+      }
+    }
+#pragma unroll
+    for (int e = 0; e < E; ++e) {
+      const double Lmb = c.tA * d[e] * rinv[e] * Pd[e];
+      D[e] = fma(c.bmk, d[e], P[e]);
+      dd[e] = c.beta + Lmb;
+      ds[e] = fma(-d[e] * c.invsig, Lmb, c.nuosig);
+    }
   } else if (sane && (hmax < c.hxl || hmin > c.hxr)) {
     const bool right = hmin > c.hxr;
 #pragma unroll
@@ -579,12 +605,20 @@ IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&
   for (int e = 0; e < E; ++e) ipa_grad_mix<Tab>(c, d[e], D[e], dd[e], ds[e], l[e], gm[e], gs[e], gf[e], gk[e], tab);
 }
 
-#define IPA_GB 256                        // threads per block of the gradient kernel
+#ifndef IPA_GB
+#define IPA_GB 512                        // threads per block of the gradient kernel
+#endif
+#ifndef IPA_GE
 #define IPA_GE 4                          // events per thread and tile
+#endif
+#ifndef IPA_GPSM
+#define IPA_GPSM 1                        // blocks per SM
+#endif
+static_assert(IPA_GB >= 160 && IPA_GB % 32 == 0, "the final reduction of the gradient kernel uses one warp per sum");
 // grid (G, K): every set streams the events on its own (the gradient call is made for one or a few sets);
 // per-thread register accumulators, fixed block tree, partials[(k 5 + c) G + b], the last block of each
 // set (ticket counter[k]) adds them in a fixed order.  out: nll[k], grad[4 k + (mu, sigma, f, k)].
-__global__ void __launch_bounds__(IPA_GB, 2)
+__global__ void __launch_bounds__(IPA_GB, IPA_GPSM)
 ipa_nll_grad_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaSetConsts* __restrict__ consts,
                     double* __restrict__ partials, unsigned int* counters, double* __restrict__ nll_out,
                     double* __restrict__ grad_out, int32_t* __restrict__ status_out) {
