@@ -164,6 +164,14 @@ def other_rows(torch, ipa, x, ws, stream, n):
     t0 = time.perf_counter()
     res = minimiser.minimise(nll_batch, th0, inp.FLOATED, inp.FD_STEPS, inp.GRAD_SCALE)
     wall = time.perf_counter() - t0
+    def grad_batch(th):
+        nll, g, _ = ipa.ipa_nll_grad_eval(x2, th, LO, HI, ws=ws2, stream=stream)
+        return nll.cpu().numpy(), g.cpu().numpy()
+    minimiser.minimise(nll_batch, th0, inp.FLOATED, inp.FD_STEPS, inp.GRAD_SCALE, grad_batch=grad_batch)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    res_a = minimiser.minimise(nll_batch, th0, inp.FLOATED, inp.FD_STEPS, inp.GRAD_SCALE, grad_batch=grad_batch)
+    wall_a = time.perf_counter() - t0
     b9, _ = inp.fd_batch(inp.GEN)
     o9 = torch.empty(9, dtype=torch.float64, device="cuda")
     d9 = t(lambda: ipa.ipa_nll_eval(x2, b9, LO, HI, ws=ws2, stream=stream, out=o9), 200, 10)
@@ -171,7 +179,9 @@ def other_rows(torch, ipa, x, ws, stream, n):
         "wall_s": wall, "nll_evaluations": res.n_evals, "batched_calls": res.n_calls, "edm": res.edm,
         "nll_evaluations_per_s_wall": res.n_evals / wall, "k9_call_ms_device": d9 * 1e3,
         "nll_evaluations_per_s_device_k9": 9 / d9,
-        "fitted": {k: res.par[k] for k in inp.FLOATED}, "errors": {k: res.errors[k] for k in inp.FLOATED}}
+        "fitted": {k: res.par[k] for k in inp.FLOATED}, "errors": {k: res.errors[k] for k in inp.FLOATED},
+        "with_analytic_gradient": {"wall_s": wall_a, "evaluations": res_a.n_evals, "calls": res_a.n_calls, "edm": res_a.edm,
+                                   "fitted": {k: res_a.par[k] for k in inp.FLOATED}}}
 
     # config 4: 1000 toys x ~1e5 events generated on the device, one segmented launch
     T = 1000

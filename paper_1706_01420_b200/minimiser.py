@@ -30,8 +30,13 @@ def _batched(nll_batch, thetas, max_k):
     return out
 
 
-def minimise(nll_batch, theta0, floated, steps, scale, max_k=32, edm_tol=1e-9, max_iter=60, newton_iter=4):
+def minimise(nll_batch, theta0, floated, steps, scale, max_k=32, edm_tol=1e-9, max_iter=60, newton_iter=4,
+             grad_batch=None):
     """Minimise NLL over the `floated` parameters.
+
+    grad_batch(thetas[K, 11]) -> (nll[K], grad[K, P]) (optional): analytic gradient with respect to the floated
+    parameters in their order (`ipa_nll_grad_eval` for (mu, sigma, f, k)).  When given, gradients come from it
+    (one call per point instead of a 2P+1 batch) and the Newton finish differences the analytic gradient.
 
     theta0   (11,) start values (fixed parameters stay at these values)
     steps    {name: h}: central-difference step per floated parameter (reading C6)
@@ -60,7 +65,18 @@ def minimise(nll_batch, theta0, floated, steps, scale, max_k=32, edm_tol=1e-9, m
             pts[2 * j + 2, j] = p[j] - h[j]
         return pts
 
+    def gradients(points):  # analytic: (m, P) points -> nll[m], grad[m, P]
+        th = np.tile(theta0, (points.shape[0], 1))
+        th[:, idx] = points
+        counters["calls"] += 1
+        counters["evals"] += points.shape[0]
+        v, g = grad_batch(th)
+        return np.asarray(v, dtype=np.float64), np.asarray(g, dtype=np.float64)
+
     def value_gradient(p):
+        if grad_batch is not None:
+            v, g = gradients(p[None, :])
+            return v[0], g[0], np.zeros(P)          # no second derivatives: the metric starts from `scale`
         v = evaluate(fd_batch(p))
         g = (v[1::2] - v[2::2]) / (2.0 * h)
         d2 = (v[1::2] + v[2::2] - 2.0 * v[0]) / (h * h)
@@ -107,7 +123,7 @@ def minimise(nll_batch, theta0, floated, steps, scale, max_k=32, edm_tol=1e-9, m
 
     # Newton finish on a finite-difference Hessian (central second differences, one batch per iteration)
     H = None
-    for _ in range(newton_iter):
+    for _ in range(newton_iter if grad_batch is None else 0):
         pts = [fd_batch(p)]
         pairs = [(i, j) for i in range(P) for j in range(i + 1, P)]
         for (i, j) in pairs:
@@ -131,6 +147,26 @@ def minimise(nll_batch, theta0, floated, steps, scale, max_k=32, edm_tol=1e-9, m
         gu = g * s
         Hu_inv = np.linalg.inv(H * np.outer(s, s))
         edm = 0.5 * gu @ Hu_inv @ gu
+        if not np.all(np.isfinite(step)):
+            break
+        p = p + step
+        if edm < edm_tol and np.all(np.abs(step) < 1e-6 * s):
+            break
+    for _ in range(newton_iter if grad_batch is not None else 0):
+        # Hessian column j = central difference of the analytic gradient along parameter j: 2P + 1 points, one call
+        pts = fd_batch(p)
+        v, gg = gradients(pts)
+        f0, g = v[0], gg[0]
+        H = np.empty((P, P))
+        for j in range(P):
+            H[:, j] = (gg[2 * j + 1] - gg[2 * j + 2]) / (2.0 * h[j])
+        H = 0.5 * (H + H.T)
+        try:
+            step = -np.linalg.solve(H, g)
+        except np.linalg.LinAlgError:
+            break
+        gu = g * s
+        edm = 0.5 * gu @ np.linalg.inv(H * np.outer(s, s)) @ gu
         if not np.all(np.isfinite(step)):
             break
         p = p + step

@@ -21,8 +21,8 @@ def start_point():
     return th
 
 
-def fit(nll_batch):
-    return minimiser.minimise(nll_batch, start_point(), inp.FLOATED, inp.FD_STEPS, inp.GRAD_SCALE)
+def fit(nll_batch, grad_batch=None):
+    return minimiser.minimise(nll_batch, start_point(), inp.FLOATED, inp.FD_STEPS, inp.GRAD_SCALE, grad_batch=grad_batch)
 
 
 def test_oracle_fit_recovers_generating_parameters(orc):
@@ -61,6 +61,27 @@ def test_minimiser_on_a_quadratic():
     assert abs(res.nll - 7.0) < 1e-9
 
 
+def test_oracle_fit_with_analytic_gradient_lands_on_the_same_minimum(orc):
+    """Row f1 in the fit loop: the analytic gradient drives the same minimiser to the minimum the
+    finite-difference fit finds (the two differ by the truncation error of the differences)."""
+    n = 20_000
+    x = orc.generate_mixture(2, n, inp.GEN, LO, HI)
+
+    def nll_batch(th):
+        return orc.nll(x, th, LO, HI)
+
+    def grad_batch(th):
+        out = [orc.nll_gradient(x, t, LO, HI) for t in th]
+        return np.array([o[0] for o in out]), np.array([o[1] for o in out])
+    a = fit(nll_batch)
+    b = fit(nll_batch, grad_batch)
+    assert b.edm < 1e-9
+    for name in inp.FLOATED:
+        assert abs(a.par[name] - b.par[name]) <= 1e-4 * a.errors[name], (name, a.par[name], b.par[name])
+        assert abs(a.errors[name] / b.errors[name] - 1) < 1e-3
+    assert b.n_calls < a.n_calls + 20
+
+
 @pytest.mark.gpu
 def test_config2_fit_parity_gpu_vs_oracle(orc):
     import torch
@@ -91,3 +112,12 @@ def test_config2_fit_parity_gpu_vs_oracle(orc):
     res_s = fit(gpu_nll_sorted)
     for name in inp.FLOATED:
         assert abs(res_s.par[name] - res_o.par[name]) <= 1e-6 * abs(res_o.par[name])
+
+    # the same fit driven by the analytic gradient (row f1): same minimum
+    def gpu_grad(th):
+        nll, g, _ = ipa.ipa_nll_grad_eval(xs, th, LO, HI, ws=ws)
+        return nll.cpu().numpy(), g.cpu().numpy()
+    res_a = fit(gpu_nll_sorted, gpu_grad)
+    assert res_a.edm < 1e-9
+    for name in inp.FLOATED:
+        assert abs(res_a.par[name] - res_o.par[name]) <= 1e-6 * abs(res_o.par[name]), (name, res_a.par[name])
