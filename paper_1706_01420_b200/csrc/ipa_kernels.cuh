@@ -639,9 +639,8 @@ ipa_nll_grad_kernel(const double* __restrict__ x, long long n, int vec_ok, const
   if (!st) {
     const long long tile_n = (long long)IPA_GB * IPA_GE, ntiles = (n + tile_n - 1) / tile_n;
     const double xpad = (n > 0) ? x[n - 1] : 0.0;
-    for (long long tile = blockIdx.x; tile < ntiles; tile += G) {
+    auto load_tile = [&](long long tile, double (&xv)[IPA_GE]) {
       const long long base = tile * tile_n;
-      double xv[IPA_GE];
       if (vec_ok && base + tile_n <= n) {
 #pragma unroll
         for (int p = 0; p < IPA_GE / 2; ++p) {
@@ -656,6 +655,15 @@ ipa_nll_grad_kernel(const double* __restrict__ x, long long n, int vec_ok, const
           xv[e] = (i < n) ? x[i] : xpad;
         }
       }
+    };
+    double xn[IPA_GE];
+    if ((long long)blockIdx.x < ntiles) load_tile(blockIdx.x, xn);
+    for (long long tile = blockIdx.x; tile < ntiles; tile += G) {
+      const long long base = tile * tile_n;
+      double xv[IPA_GE];
+#pragma unroll
+      for (int e = 0; e < IPA_GE; ++e) xv[e] = xn[e];
+      if (tile + G < ntiles) load_tile(tile + G, xn);        // next tile in flight while this one is evaluated
       double l[IPA_GE], gm[IPA_GE], gs[IPA_GE], gf[IPA_GE], gk[IPA_GE];
       ipa_eval_grad<IPA_GE>(c, xv, l, gm, gs, gf, gk, s_tab);
 #pragma unroll
