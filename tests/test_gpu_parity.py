@@ -578,3 +578,23 @@ def test_analytic_gradient_1e6_and_fit_minimum(ipa, torch_, orc):
     an = ipa.ipa_nll_grad_eval(xd, inp.GEN, LO, HI)[1][0].cpu().numpy()
     s = np.array([inp.GRAD_SCALE[k] for k in inp.FLOATED])
     assert np.all(np.abs(fd - an) <= 1e-3 * np.maximum(np.abs(an), 1.0 / s))
+
+
+def test_maximum_batch_of_32_sets(ipa, torch_, orc, x1):
+    """K = IPA_MAX_K: the largest shared-memory footprint of the streaming kernel (grouped and ungrouped)."""
+    xd = dev(torch_, np.sort(x1))
+    rng = np.random.Generator(np.random.Philox(32))
+    distinct = [dict(inp.GEN, mu=5280 + rng.uniform(-5, 5), sigma=rng.uniform(12, 18), f=rng.uniform(0.1, 0.6),
+                     k=rng.uniform(-0.003, -0.001)) for _ in range(32)]
+    shared = [dict(inp.P2, f=rng.uniform(0.1, 0.6), k=rng.uniform(-0.003, -0.001)) for _ in range(32)]   # one shape
+    for sets in (distinct, shared):
+        nll, _, st = ipa.ipa_nll_eval(xd, sets, LO, HI)
+        torch_.cuda.synchronize()
+        assert (st.cpu().numpy() == 0).all()
+        got = nll.cpu().numpy()
+        ref = orc.nll(np.sort(x1), sets, LO, HI)
+        assert np.all(np.abs(got - ref) <= 1e-10 * np.abs(ref))
+        for i in (0, 13, 31):
+            assert got[i] == ipa.ipa_nll_eval(xd, sets[i], LO, HI)[0].item()
+    with pytest.raises(ipa.IpaError):
+        ipa.ipa_nll_eval(xd, distinct + [inp.GEN], LO, HI)          # 33 sets: invalid argument
