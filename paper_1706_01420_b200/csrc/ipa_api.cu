@@ -84,7 +84,7 @@ bool ws_ok(const void* ws, size_t bytes, size_t need) {
 // Runs the prologue for K sets.  K <= IPA_MAX_K: the sets travel in the kernel-parameter space;
 // larger batches go through the workspace with one host-to-device copy.
 int run_prologue(const ipa_params* p_host, int64_t K, ipa_range r, char* ws, const Layout& L, double* norm_sig,
-                 double* norm_bkg, int32_t* status_out, cudaStream_t st) {
+                 double* norm_bkg, int32_t* status_out, cudaStream_t st, bool want_grad = false) {
   IpaSetConsts* consts = reinterpret_cast<IpaSetConsts*>(ws + L.consts);
   unsigned int* counter = reinterpret_cast<unsigned int*>(ws + L.counter);
   static thread_local IpaParamBatch batch;
@@ -95,7 +95,8 @@ int run_prologue(const ipa_params* p_host, int64_t K, ipa_range r, char* ws, con
     IPA_CK(cudaMemcpyAsync(ws + L.params, p_host, (size_t)K * sizeof(ipa_params), cudaMemcpyHostToDevice, st));
     p_dev = reinterpret_cast<const ipa_params*>(ws + L.params);
   }
-  ipa_prologue_kernel<<<(unsigned)K, IPA_PRO_THREADS, 0, st>>>(batch, p_dev, r.lo, r.hi, g_degree_policy, consts,
+  ipa_prologue_kernel<<<(unsigned)K, IPA_PRO_THREADS, 0, st>>>(batch, p_dev, r.lo, r.hi,
+                                                               g_degree_policy | (want_grad ? 2 : 0), consts,
                                                                counter, norm_sig, norm_bkg, status_out);
   IPA_CK(cudaGetLastError());
   return IPA_OK;
@@ -209,7 +210,7 @@ int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, 
   if (rc) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   char* ws = static_cast<char*>(ws_dev);
-  rc = run_prologue(p_host, K, r, ws, L, nullptr, nullptr, nullptr, st);
+  rc = run_prologue(p_host, K, r, ws, L, nullptr, nullptr, nullptr, st, true);
   if (rc) return rc;
   IPA_CK(cudaMemsetAsync(ws + L.counter, 0, 256, st));          // one ticket counter per set
   const int64_t tile_n = (int64_t)IPA_GB * IPA_GE, ntiles = (n + tile_n - 1) / tile_n;

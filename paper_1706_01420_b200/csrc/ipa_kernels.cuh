@@ -27,7 +27,7 @@ ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_param
   const int tid = threadIdx.x, set = blockIdx.x;
   if (tid == 0) {
     w.p = p_dev ? p_dev[set] : batch.p[set];
-    w.lo = lo; w.hi = hi; w.policy = policy;
+    w.lo = lo; w.hi = hi; w.policy = policy & 1; w.want_grad = (policy >> 1) & 1;
     if (set == 0 && counter) *counter = 0u;
   }
   __syncthreads();

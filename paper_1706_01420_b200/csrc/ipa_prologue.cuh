@@ -57,6 +57,7 @@ struct IpaProWork {
   ipa_params p;
   double lo, hi;
   int policy;
+  int want_grad;                // compute the normalisation derivatives of the gradient call (row f1)
   int status;
   double nu, delta, alpha, d0, d1, r0, r1, z0, z1, zc, zh;
   double part[2][32];
@@ -360,7 +361,7 @@ IPA_HD void ipa_pro_phase10(IpaProWork& w, int tid, int nthr) {
     const double d = c + hl * w.glx[i];
     const double g = w.glw[i] * hl * exp(ipa_core_logG(w, d) - w.logref);
     w.pval[q] = g;
-    w.pval2[q] = g * (w.nu / w.p.sigma - (d / w.p.sigma) * ipa_core_Lmb(w, d));   // G dlogG/dsigma
+    w.pval2[q] = w.want_grad ? g * (w.nu / w.p.sigma - (d / w.p.sigma) * ipa_core_Lmb(w, d)) : 0.0;   // G dlogG/dsigma
   }
 }
 IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
@@ -380,7 +381,7 @@ IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
       const double ul = 1.0 - (w.dl - w.d0) * w.L0 / p.n, ur = 1.0 - (dr - w.d0) * w.L0 / p.n;
       const double pre = exp(w.logG0 - w.logref) * (p.n / w.L0);
       const double F = ipa_powint(ul, p.n) - ipa_powint(ur, p.n);
-      const double F1 = ipa_powint(ul, p.n + 1.0) - ipa_powint(ur, p.n + 1.0);
+      const double F1 = w.want_grad ? ipa_powint(ul, p.n + 1.0) - ipa_powint(ur, p.n + 1.0) : 0.0;
       const double A = w.nu / p.sigma - p.a * p.beta, c = p.n * (w.L0 - p.beta) / (w.L0 * p.sigma);
       left = pre * F;
       left2 = pre * ((A + c) * F + (p.a * w.L0 - c) * F1);
@@ -394,7 +395,7 @@ IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
       const double uh = 1.0 - (w.dh - w.d1) * w.L1 / p.n2, ul = 1.0 - (dL - w.d1) * w.L1 / p.n2;
       const double pre = exp(w.logG1 - w.logref) * (p.n2 / (-w.L1));
       const double F = ipa_powint(uh, p.n2) - ipa_powint(ul, p.n2);
-      const double F1 = ipa_powint(uh, p.n2 + 1.0) - ipa_powint(ul, p.n2 + 1.0);
+      const double F1 = w.want_grad ? ipa_powint(uh, p.n2 + 1.0) - ipa_powint(ul, p.n2 + 1.0) : 0.0;
       const double A = w.nu / p.sigma + p.a2 * p.beta, c = p.n2 * (w.L1 - p.beta) / (w.L1 * p.sigma);
       right = pre * F;
       right2 = pre * ((A + c) * F - (p.a2 * w.L1 + c) * F1);
@@ -408,8 +409,8 @@ IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
     w.logNB = log(NB);
     w.dlnNB_dk = (fabs(tk) < 1e-6) ? wd * (0.5 + tk / 12.0) : wd * exp(tk) / expm1(tk) - 1.0 / p.k;
   } else if (tid == 224) {         // I at the ends of the range (d N_S / d mu = I(lo - mu) - I(hi - mu))
-    w.Iedge_l = exp(ipa_logI(w, w.dl) - w.logref);
-    w.Iedge_h = exp(ipa_logI(w, w.dh) - w.logref);
+    w.Iedge_l = w.want_grad ? exp(ipa_logI(w, w.dl) - w.logref) : 0.0;
+    w.Iedge_h = w.want_grad ? exp(ipa_logI(w, w.dh) - w.logref) : 0.0;
   } else if (tid == 128) {
     w.logf = (p.f > 0.0) ? log(p.f) : 0.0;
     w.log1mf = (p.f < 1.0) ? log1p(-p.f) : 0.0;

@@ -10,7 +10,7 @@ static void run_prologue_host(const ipa_params& p, double lo, double hi, int pol
   static IpaProWork w;
   std::memset(&w, 0, sizeof(w));
   std::memset(out, 0, sizeof(*out));
-  w.p = p; w.lo = lo; w.hi = hi; w.policy = policy;
+  w.p = p; w.lo = lo; w.hi = hi; w.policy = policy; w.want_grad = 1;
   const int NT = IPA_PRO_THREADS;
 #define ALL(stmt) for (int tid = 0; tid < NT; ++tid) { stmt; }
   ALL(ipa_pro_load_table(w, tid, NT))
