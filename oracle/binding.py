@@ -46,6 +46,11 @@ def lib():
         L.orc_poisson_hist_toys.restype = None; L.orc_poisson_hist_toys.argtypes = [vp, i32, vp, i64, vp]
         L.orc_norm_derivs.restype = i32; L.orc_norm_derivs.argtypes = [vp, d, d, vp]
         L.orc_nll_gradient.restype = i32; L.orc_nll_gradient.argtypes = [vp, i64, vp, d, d, vp, vp]
+        L.orc_gauss_smear.restype = None; L.orc_gauss_smear.argtypes = [vp, i32, d, d, d, vp]
+        L.orc_expected_hist_shape.restype = i32; L.orc_expected_hist_shape.argtypes = [i32, d, d, vp, d, d, d, vp]
+        L.orc_binned_nll_scan_shape.restype = i32
+        L.orc_binned_nll_scan_shape.argtypes = [vp, i32, d, d, vp, vp, vp, vp, i64, vp]
+        L.orc_signal_shape.restype = i32; L.orc_signal_shape.argtypes = [i32, d, d, vp, vp]
         L.orc_cls_teststat.restype = None; L.orc_cls_teststat.argtypes = [vp, i32, i64, i32, vp, vp, vp]
         L.orc_cls_count_ge.restype = i64; L.orc_cls_count_ge.argtypes = [vp, i64, d]
         L.orc_cls_from_counts.restype = None; L.orc_cls_from_counts.argtypes = [i64, i64, i64, i64, vp]
@@ -266,5 +271,41 @@ def norm_derivs(p, lo, hi):
     P = pack_params(p)
     out = np.empty(3)
     st = lib().orc_norm_derivs(_p(P), float(lo), float(hi), _p(out))
+    assert st == 0, st
+    return out
+
+
+def gauss_smear(sig, lo, hi, sigma0):
+    """Gaussian smearing of a histogram-like array on the bin grid (reading F3)."""
+    sig = np.ascontiguousarray(sig, dtype=np.float64)
+    out = np.empty_like(sig)
+    lib().orc_gauss_smear(_p(sig), sig.size, float(lo), float(hi), float(sigma0), _p(out))
+    return out
+
+
+def signal_shape(nbins, lo, hi, shape):
+    out = np.empty(int(nbins))
+    st = lib().orc_signal_shape(int(nbins), float(lo), float(hi), _p(pack_params(shape)), _p(out))
+    assert st == 0, st
+    return out
+
+
+def expected_hist_shape(lo, hi, sig, ns, nb, k):
+    sig = np.ascontiguousarray(sig, dtype=np.float64)
+    out = np.empty_like(sig)
+    st = lib().orc_expected_hist_shape(sig.size, float(lo), float(hi), _p(sig), float(ns), float(nb), float(k), _p(out))
+    assert st == 0, st
+    return out
+
+
+def binned_nll_scan_shape(counts, lo, hi, sig, ns, nb, k):
+    counts = np.ascontiguousarray(counts, dtype=np.uint64)
+    sig = np.ascontiguousarray(sig, dtype=np.float64)
+    ns = np.ascontiguousarray(ns, dtype=np.float64)
+    nb = np.ascontiguousarray(nb, dtype=np.float64)
+    k = np.ascontiguousarray(k, dtype=np.float64)
+    out = np.empty(ns.size)
+    st = lib().orc_binned_nll_scan_shape(_p(counts), counts.size, float(lo), float(hi), _p(sig), _p(ns), _p(nb), _p(k),
+                                         ns.size, _p(out))
     assert st == 0, st
     return out

@@ -811,4 +811,67 @@ void orc_cls_from_counts(int64_t count_sb, int64_t T_sb, int64_t count_b, int64_
   out[1] = (double)count_b / (double)T_b;
   out[2] = count_b > 0 ? out[0] / out[1] : NAN;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Gaussian-smeared signal shape on the bin grid (PAPER.md:291-312:
+ * "SM = GaussSmear1(bins_cx, sigma0); sigf_gpu = SM.Smear(sigf_i_gpu)", an FFT convolution whose kernel,
+ * normalisation and edge treatment the paper does not state) -> DESIGN.md reading F3:
+ *   out_b = sum_j in_j g_{b-j},  g_m = exp(-(m w)^2 / (2 sigma0^2)) / sum_{|m'| <= M} g_{m'},  |m| <= M,
+ *   w = (hi - lo)/nbins,  M = ceil(8 sigma0 / w)  (relative tail 1e-14),  in_j = 0 outside the grid
+ * (linear convolution; the paper's FFT is circular, which is the same thing for a peak far from the edges).
+ * sigma0 <= 0 copies the input.  Plain double loop in long double.
+ * ---------------------------------------------------------------------------------------- */
+void orc_gauss_smear(const double* in, int nbins, double lo, double hi, double sigma0, double* out) {
+  if (!(sigma0 > 0)) { for (int b = 0; b < nbins; ++b) out[b] = in[b]; return; }
+  const ld w = ((ld)hi - lo) / nbins;
+  const int M = (int)ceill(8 * (ld)sigma0 / w);
+  std::vector<ld> g((size_t)(2 * M + 1));
+  ld norm = 0;
+  for (int m = -M; m <= M; ++m) { g[(size_t)(m + M)] = expl(-(m * w) * (m * w) / (2 * (ld)sigma0 * sigma0)); norm += g[(size_t)(m + M)]; }
+  for (int b = 0; b < nbins; ++b) {
+    ld acc = 0;
+    for (int j = std::max(0, b - M); j <= std::min(nbins - 1, b + M); ++j) acc += (ld)in[j] * g[(size_t)(b - j + M)];
+    out[b] = (double)(acc / norm);
+  }
+}
+/* binned path with a GIVEN signal shape sig[nbins] >= 0 (e.g. the smeared one), normalised to unit sum as
+ * PAPER.md:311-312 does; otherwise exactly orc_expected_hist / orc_binned_nll_scan (reading D15) */
+int orc_expected_hist_shape(int nbins, double lo, double hi, const double* sig, double ns, double nb, double k, double* nu) {
+  const ld w = ((ld)hi - lo) / nbins;
+  ld ssum = 0, bsum = 0;
+  std::vector<ld> bb((size_t)nbins);
+  for (int b = 0; b < nbins; ++b) { ssum += sig[b]; bb[(size_t)b] = expl((ld)k * ((b + 0.5L) * w)); bsum += bb[(size_t)b]; }
+  if (!(ssum > 0)) return 3;
+  for (int b = 0; b < nbins; ++b) nu[b] = (double)((ld)ns * sig[b] / ssum + (ld)nb * bb[(size_t)b] / bsum);
+  return 0;
+}
+int orc_binned_nll_scan_shape(const uint64_t* counts, int nbins, double lo, double hi, const double* sig,
+                              const double* ns, const double* nb, const double* kk, int64_t npoints, double* nll) {
+  const ld w = ((ld)hi - lo) / nbins;
+  ld ssum = 0;
+  for (int b = 0; b < nbins; ++b) ssum += sig[b];
+  if (!(ssum > 0)) return 3;
+  std::vector<ld> bb((size_t)nbins);
+  std::vector<double> terms((size_t)nbins);
+  for (int64_t q = 0; q < npoints; ++q) {
+    ld bsum = 0;
+    for (int b = 0; b < nbins; ++b) { bb[(size_t)b] = expl((ld)kk[q] * ((b + 0.5L) * w)); bsum += bb[(size_t)b]; }
+    for (int b = 0; b < nbins; ++b) {
+      const ld v = (ld)ns[q] * sig[b] / ssum + (ld)nb[q] * bb[(size_t)b] / bsum;
+      terms[(size_t)b] = (double)(counts[b] ? v - (ld)counts[b] * logl(v) : v);
+    }
+    nll[q] = (double)pairwise(terms.data(), 0, nbins);
+  }
+  return 0;
+}
+/* signal shape at the bin centres, I(c_b - mu) relative to its value at the reference point (what the
+ * paper's Ipatia kernel writes before the smearing); not normalised */
+int orc_signal_shape(int nbins, double lo, double hi, const orc_params* shape, double* out) {
+  const Shape s = make_shape(*shape);
+  if (s.status) return s.status;
+  const ld w = ((ld)hi - lo) / nbins;
+  const ld ref = log_I(s, std::min(std::max((ld)0, (ld)lo - s.mu), (ld)hi - s.mu));
+  for (int b = 0; b < nbins; ++b) out[b] = (double)expl(log_I(s, lo + (b + 0.5L) * w - s.mu) - ref);
+  return 0;
+}
 } /* extern "C" */
