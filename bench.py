@@ -226,6 +226,13 @@ def other_rows(torch, ipa, x, ws, stream, n):
     out["cls_f2"] = {"toy_histograms": int(sd.size), "bins": nbins, "teststat_ms": dq * 1e3, "count_ms": dc * 1e3,
                      "teststat_roofline": {"bound": "hbm", "achieved": 4.0 * sd.size * nbins / dq / 1e9, "peak": peaks_hbm,
                                            "unit": "GB/s", "frac": 4.0 * sd.size * nbins / dq / 1e9 / peaks_hbm}}
+    # row f3: Gaussian-smeared signal shape on the bin grid feeding the same binned scan
+    sig = ipa.ipa_signal_shape(nbins, LO, HI, inp.GEN, ws=ws5, stream=stream)
+    dsm = t(lambda: ipa.ipa_gauss_smear(sig, LO, HI, 10.0, stream=stream), 20)
+    sm = ipa.ipa_gauss_smear(sig, LO, HI, 10.0, stream=stream)
+    dss = t(lambda: ipa.ipa_binned_nll_scan_shape(counts, LO, HI, sm, ns, nb, kk, ws=ws5, stream=stream), 20)
+    out["smear_f3"] = {"bins": nbins, "sigma0": 10.0, "smear_ms": dsm * 1e3, "scan_with_smeared_shape_ms": dss * 1e3,
+                       "scan_points_per_s": ns.size / dss}
     out["config5_binned"] = {
         "hist_fill_ms": dh * 1e3, "hist_events_per_s": n / dh,
         "hist_roofline": {"bound": "hbm", "achieved": 8.0 * n / dh / 1e9, "peak": peaks_hbm, "unit": "GB/s",

@@ -171,6 +171,26 @@ int ipa_binned_nll_scan(const uint64_t* counts_dev, int nbins, ipa_range r, cons
 int ipa_expected_hist(int nbins, ipa_range r, const ipa_params* shape_host, double ns, double nb, double k,
                       double* nu_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
 
+/* Gaussian-smeared signal shape on the bin grid ("SM = GaussSmear1(bins_cx, sigma0);
+ * sigf_gpu = SM.Smear(sigf_i_gpu)"; kernel, normalisation and edges are not stated -- DESIGN.md reading F3):
+ *   ipa_signal_shape   sig_dev[b] = I(c_b - mu) / I(reference point) at the bin centres c_b (not normalised):
+ *                      what the paper's Ipatia kernel writes before the smearing
+ *   ipa_gauss_smear    out_b = sum_j in_j g_{b-j},  g_m = exp(-(m w)^2 / (2 sigma0^2)) / sum_{|m'|<=M} g_m',
+ *                      |m| <= M = ceil(8 sigma0 / w), w = bin width, in_j = 0 outside the grid; sigma0 <= 0
+ *                      copies; out_dev must not alias in_dev; M <= 2800
+ *   ipa_expected_hist_shape / ipa_binned_nll_scan_shape
+ *                      ipa_expected_hist / ipa_binned_nll_scan with a GIVEN signal shape sig_dev [nbins] >= 0
+ *                      (normalised to unit sum inside, as PAPER.md:311-312 does) instead of a parameter set;
+ *                      a shape whose sum is not positive gives NaN / +inf results */
+int ipa_signal_shape(int nbins, ipa_range r, const ipa_params* shape_host, double* sig_dev, void* ws_dev, size_t ws_bytes,
+                     void* cuda_stream);
+int ipa_gauss_smear(const double* in_dev, int nbins, ipa_range r, double sigma0, double* out_dev, void* cuda_stream);
+int ipa_expected_hist_shape(int nbins, ipa_range r, const double* sig_dev, double ns, double nb, double k, double* nu_dev,
+                            void* ws_dev, size_t ws_bytes, void* cuda_stream);
+int ipa_binned_nll_scan_shape(const uint64_t* counts_dev, int nbins, ipa_range r, const double* sig_dev,
+                              const double* ns_host, const double* nb_host, const double* k_host, int64_t npoints,
+                              double* nll_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
+
 /* Per-bin Poisson toys, a separate mean per generated value:
  * counts_dev[t*nbins + b] ~ Poisson(mean_dev[b]) from key seeds_host[t], counter slot b. */
 int ipa_poisson_hist_toys(const double* mean_dev, int nbins, const uint64_t* seeds_host, int64_t T,

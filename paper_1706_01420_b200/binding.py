@@ -14,7 +14,8 @@ __all__ = [
     "PARAM_FIELDS", "NPAR", "IPA_MAX_K", "IpaError", "lib", "library_path", "pack_params", "workspace",
     "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes", "ipa_norm", "ipa_core_degree", "ipa_nll_grad_eval", "ipa_nll_eval",
     "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill", "ipa_binned_nll_scan", "ipa_expected_hist",
-    "ipa_poisson_hist_toys", "ipa_cls_teststat", "ipa_cls_count_ge", "ipa_cls_from_counts", "ipa_events_sort",
+    "ipa_poisson_hist_toys", "ipa_signal_shape", "ipa_gauss_smear", "ipa_expected_hist_shape", "ipa_binned_nll_scan_shape",
+    "ipa_cls_teststat", "ipa_cls_count_ge", "ipa_cls_from_counts", "ipa_events_sort",
     "ipa_sort_workspace_bytes", "ipa_fp64_peak_probe", "nll_host", "EXPORTS",
 ]
 
@@ -26,7 +27,8 @@ IPA_MAX_K = 32
 EXPORTS = (
     "ipa_strerror", "ipa_last_cuda_error", "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes",
     "ipa_norm", "ipa_core_degree", "ipa_nll_eval", "ipa_nll_grad_eval", "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill",
-    "ipa_binned_nll_scan", "ipa_expected_hist", "ipa_poisson_hist_toys", "ipa_cls_teststat", "ipa_cls_count_ge",
+    "ipa_binned_nll_scan", "ipa_expected_hist", "ipa_poisson_hist_toys", "ipa_signal_shape", "ipa_gauss_smear",
+    "ipa_expected_hist_shape", "ipa_binned_nll_scan_shape", "ipa_cls_teststat", "ipa_cls_count_ge",
     "ipa_cls_from_counts", "ipa_sort_workspace_bytes", "ipa_events_sort",
     "ipa_fp64_peak_probe",
 )
@@ -73,6 +75,11 @@ def lib():
     L.ipa_binned_nll_scan.argtypes = [vp, i32, _Range, vp, vp, vp, vp, i64, vp, vp, sz, vp]
     L.ipa_expected_hist.restype = i32; L.ipa_expected_hist.argtypes = [i32, _Range, vp, d, d, d, vp, vp, sz, vp]
     L.ipa_poisson_hist_toys.restype = i32; L.ipa_poisson_hist_toys.argtypes = [vp, i32, vp, i64, vp, vp, sz, vp]
+    L.ipa_signal_shape.restype = i32; L.ipa_signal_shape.argtypes = [i32, _Range, vp, vp, vp, sz, vp]
+    L.ipa_gauss_smear.restype = i32; L.ipa_gauss_smear.argtypes = [vp, i32, _Range, d, vp, vp]
+    L.ipa_expected_hist_shape.restype = i32; L.ipa_expected_hist_shape.argtypes = [i32, _Range, vp, d, d, d, vp, vp, sz, vp]
+    L.ipa_binned_nll_scan_shape.restype = i32
+    L.ipa_binned_nll_scan_shape.argtypes = [vp, i32, _Range, vp, vp, vp, vp, i64, vp, vp, sz, vp]
     L.ipa_cls_teststat.restype = i32; L.ipa_cls_teststat.argtypes = [vp, i32, i64, i32, vp, vp, vp, vp, sz, vp]
     L.ipa_cls_count_ge.restype = i32; L.ipa_cls_count_ge.argtypes = [vp, i64, vp, vp, vp]
     L.ipa_cls_from_counts.restype = i32; L.ipa_cls_from_counts.argtypes = [vp, i64, vp, i64, vp, vp]
@@ -288,6 +295,48 @@ def ipa_poisson_hist_toys(mean, seeds, ws=None, stream=None):
     out = torch.empty((T, nbins), dtype=torch.int32, device="cuda")  # uint32 payload
     _check(lib().ipa_poisson_hist_toys(_dptr(mean, torch.float64), nbins, _hptr(seeds), T, _dptr(out), _dptr(ws),
                                        ws.numel(), _stream(stream)))
+    return out
+
+
+def ipa_signal_shape(nbins, lo, hi, shape, ws=None, stream=None):
+    """Un-normalised signal shape at the bin centres (device tensor [nbins])."""
+    _need_cuda()
+    P = pack_params(shape)
+    ws = _ws(ws, 0, 1, nbins)
+    out = torch.empty(int(nbins), dtype=torch.float64, device="cuda")
+    _check(lib().ipa_signal_shape(int(nbins), _Range(lo, hi), _hptr(P), _dptr(out), _dptr(ws), ws.numel(), _stream(stream)))
+    return out
+
+
+def ipa_gauss_smear(sig, lo, hi, sigma0, stream=None):
+    """Gaussian smearing of a shape on the bin grid (reading F3) -> new device tensor."""
+    _need_cuda()
+    out = torch.empty_like(sig)
+    _check(lib().ipa_gauss_smear(_dptr(sig, torch.float64), sig.numel(), _Range(lo, hi), float(sigma0), _dptr(out),
+                                 _stream(stream)))
+    return out
+
+
+def ipa_expected_hist_shape(sig, lo, hi, ns, nb, k, ws=None, stream=None):
+    _need_cuda()
+    nbins = sig.numel()
+    ws = _ws(ws, 0, 1, nbins)
+    out = torch.empty(nbins, dtype=torch.float64, device="cuda")
+    _check(lib().ipa_expected_hist_shape(nbins, _Range(lo, hi), _dptr(sig, torch.float64), float(ns), float(nb), float(k),
+                                         _dptr(out), _dptr(ws), ws.numel(), _stream(stream)))
+    return out
+
+
+def ipa_binned_nll_scan_shape(counts, lo, hi, sig, ns, nb, k, ws=None, stream=None):
+    _need_cuda()
+    ns = np.ascontiguousarray(ns, dtype=np.float64); nb = np.ascontiguousarray(nb, dtype=np.float64)
+    k = np.ascontiguousarray(k, dtype=np.float64)
+    npts, nbins = ns.size, counts.numel()
+    ws = _ws(ws, 0, npts, nbins)
+    out = torch.empty(npts, dtype=torch.float64, device="cuda")
+    _check(lib().ipa_binned_nll_scan_shape(_dptr(counts, torch.int64), nbins, _Range(lo, hi), _dptr(sig, torch.float64),
+                                           _hptr(ns), _hptr(nb), _hptr(k), npts, _dptr(out), _dptr(ws), ws.numel(),
+                                           _stream(stream)))
     return out
 
 

@@ -313,22 +313,26 @@ int ipa_hist_fill(const double* x_dev, int64_t n, ipa_range r, int nbins, uint64
 }
 
 static int binned_common(const uint64_t* counts_dev, int nbins, ipa_range r, const ipa_params* shape_host,
-                         const double* ns_host, const double* nb_host, const double* k_host, int64_t npoints,
+                         const double* sig_dev, const double* ns_host, const double* nb_host, const double* k_host, int64_t npoints,
                          double* nll_dev, double* nu_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
   const Layout L = make_layout(npoints, nbins);
   if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   char* ws = static_cast<char*>(ws_dev);
-  ipa_params shape = *shape_host;
-  shape.f = 0.5;  // f and k of the shape set are not used by the binned path
-  shape.k = 0.0;
-  int rc = run_prologue(&shape, 1, r, ws, L, nullptr, nullptr, nullptr, st);
-  if (rc) return rc;
-  const IpaSetConsts* consts = reinterpret_cast<const IpaSetConsts*>(ws + L.consts);
   double* sbin = reinterpret_cast<double*>(ws + L.sbin);
   int32_t* flag = reinterpret_cast<int32_t*>(ws + L.flag);
   double* pts = reinterpret_cast<double*>(ws + L.pts);
-  ipa_binned_shape_kernel<<<1, 256, 0, st>>>(consts, r.lo, r.hi, nbins, sbin, flag);
+  if (sig_dev) {   // a given signal shape (row f3)
+    ipa_shape_normalise_kernel<<<1, 256, 0, st>>>(sig_dev, nbins, sbin, flag);
+  } else {
+    ipa_params shape = *shape_host;
+    shape.f = 0.5;  // f and k of the shape set are not used by the binned path
+    shape.k = 0.0;
+    int rc = run_prologue(&shape, 1, r, ws, L, nullptr, nullptr, nullptr, st);
+    if (rc) return rc;
+    ipa_binned_shape_kernel<<<1, 256, 0, st>>>(reinterpret_cast<const IpaSetConsts*>(ws + L.consts), r.lo, r.hi, nbins, sbin,
+                                               flag, 1);
+  }
   IPA_CK(cudaGetLastError());
   IPA_CK(cudaMemcpyAsync(pts, ns_host, (size_t)npoints * 8, cudaMemcpyHostToDevice, st));
   IPA_CK(cudaMemcpyAsync(pts + npoints, nb_host, (size_t)npoints * 8, cudaMemcpyHostToDevice, st));
@@ -346,14 +350,64 @@ int ipa_binned_nll_scan(const uint64_t* counts_dev, int nbins, ipa_range r, cons
   if (!counts_dev || nbins < 1 || !range_ok(r) || !shape_host || !ns_host || !nb_host || !k_host || npoints < 1 ||
       npoints > 0x7fffffffLL || !nll_dev)
     return IPA_ERR_INVALID_ARG;
-  return binned_common(counts_dev, nbins, r, shape_host, ns_host, nb_host, k_host, npoints, nll_dev, nullptr, ws_dev,
+  return binned_common(counts_dev, nbins, r, shape_host, nullptr, ns_host, nb_host, k_host, npoints, nll_dev, nullptr, ws_dev,
                        ws_bytes, cuda_stream);
 }
 
 int ipa_expected_hist(int nbins, ipa_range r, const ipa_params* shape_host, double ns, double nb, double k,
                       double* nu_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
   if (nbins < 1 || !range_ok(r) || !shape_host || !nu_dev) return IPA_ERR_INVALID_ARG;
-  return binned_common(nullptr, nbins, r, shape_host, &ns, &nb, &k, 1, nullptr, nu_dev, ws_dev, ws_bytes, cuda_stream);
+  return binned_common(nullptr, nbins, r, shape_host, nullptr, &ns, &nb, &k, 1, nullptr, nu_dev, ws_dev, ws_bytes, cuda_stream);
+}
+
+int ipa_signal_shape(int nbins, ipa_range r, const ipa_params* shape_host, double* sig_dev, void* ws_dev, size_t ws_bytes,
+                     void* cuda_stream) {
+  if (nbins < 1 || !range_ok(r) || !shape_host || !sig_dev) return IPA_ERR_INVALID_ARG;
+  const Layout L = make_layout(1, nbins);
+  if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* ws = static_cast<char*>(ws_dev);
+  ipa_params shape = *shape_host;
+  shape.f = 0.5;
+  shape.k = 0.0;
+  int rc = run_prologue(&shape, 1, r, ws, L, nullptr, nullptr, nullptr, st);
+  if (rc) return rc;
+  ipa_binned_shape_kernel<<<1, 256, 0, st>>>(reinterpret_cast<const IpaSetConsts*>(ws + L.consts), r.lo, r.hi, nbins, sig_dev,
+                                             reinterpret_cast<int32_t*>(ws + L.flag), 0);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
+int ipa_gauss_smear(const double* in_dev, int nbins, ipa_range r, double sigma0, double* out_dev, void* cuda_stream) {
+  if (!in_dev || !out_dev || in_dev == out_dev || nbins < 1 || !range_ok(r) || !ipa_finite(sigma0)) return IPA_ERR_INVALID_ARG;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  if (!(sigma0 > 0.0)) {
+    IPA_CK(cudaMemcpyAsync(out_dev, in_dev, (size_t)nbins * 8, cudaMemcpyDeviceToDevice, st));
+    return IPA_OK;
+  }
+  const double w = (r.hi - r.lo) / (double)nbins;
+  const double Md = ceil(8.0 * sigma0 / w);
+  if (!(Md <= 2800.0)) return IPA_ERR_INVALID_ARG;               // 2M+1 taps must fit 48 KB of shared memory
+  const int M = (int)Md;
+  ipa_gauss_smear_kernel<<<(nbins + 255) / 256, 256, (size_t)(2 * M + 1) * 8, st>>>(in_dev, nbins, w, sigma0, M, out_dev);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
+int ipa_expected_hist_shape(int nbins, ipa_range r, const double* sig_dev, double ns, double nb, double k, double* nu_dev,
+                            void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (nbins < 1 || !range_ok(r) || !sig_dev || !nu_dev) return IPA_ERR_INVALID_ARG;
+  return binned_common(nullptr, nbins, r, nullptr, sig_dev, &ns, &nb, &k, 1, nullptr, nu_dev, ws_dev, ws_bytes, cuda_stream);
+}
+
+int ipa_binned_nll_scan_shape(const uint64_t* counts_dev, int nbins, ipa_range r, const double* sig_dev,
+                              const double* ns_host, const double* nb_host, const double* k_host, int64_t npoints,
+                              double* nll_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (!counts_dev || nbins < 1 || !range_ok(r) || !sig_dev || !ns_host || !nb_host || !k_host || npoints < 1 ||
+      npoints > 0x7fffffffLL || !nll_dev)
+    return IPA_ERR_INVALID_ARG;
+  return binned_common(counts_dev, nbins, r, nullptr, sig_dev, ns_host, nb_host, k_host, npoints, nll_dev, nullptr, ws_dev,
+                       ws_bytes, cuda_stream);
 }
 
 int ipa_poisson_hist_toys(const double* mean_dev, int nbins, const uint64_t* seeds_host, int64_t T,

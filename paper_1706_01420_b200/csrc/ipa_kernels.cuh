@@ -1050,7 +1050,7 @@ __device__ __forceinline__ double ipa_block_sum_256(double v, double* red) {
 // one block of 256 threads: sraw[b] = exp(logI(c_b - mu) - ref), then s[b] = sraw[b] / sum
 __global__ void __launch_bounds__(256)
 ipa_binned_shape_kernel(const IpaSetConsts* __restrict__ consts, double lo, double hi, int nbins,
-                        double* __restrict__ s_out, int32_t* __restrict__ shape_status) {
+                        double* __restrict__ s_out, int32_t* __restrict__ shape_status, int normalise) {
   __shared__ IpaSetConsts c;
   __shared__ double red[8];
   {
@@ -1074,7 +1074,45 @@ ipa_binned_shape_kernel(const IpaSetConsts* __restrict__ consts, double lo, doub
     part += v;
   }
   const double tot = ipa_block_sum_256(part, red);
-  for (int b = threadIdx.x; b < nbins; b += 256) s_out[b] = s_out[b] / tot;
+  if (normalise)
+    for (int b = threadIdx.x; b < nbins; b += 256) s_out[b] = s_out[b] / tot;
+}
+
+// a GIVEN signal shape (row f3: e.g. the smeared one) normalised to unit sum, as PAPER.md:311-312 does
+__global__ void __launch_bounds__(256)
+ipa_shape_normalise_kernel(const double* __restrict__ sig, int nbins, double* __restrict__ s_out,
+                           int32_t* __restrict__ shape_status) {
+  __shared__ double red[8];
+  double part = 0.0;
+  for (int b = threadIdx.x; b < nbins; b += 256) part += sig[b];
+  const double tot = ipa_block_sum_256(part, red);
+  if (threadIdx.x == 0) *shape_status = (tot > 0.0 && ipa_finite(tot)) ? 0 : 3;
+  for (int b = threadIdx.x; b < nbins; b += 256) s_out[b] = sig[b] / tot;
+}
+
+// Gaussian smearing on the bin grid (row f3, reading F3): out_b = sum_j in_j g_{b-j}, |b - j| <= M, the
+// kernel g (2M+1 taps, unit sum) is built in shared memory by every block; direct convolution (a few
+// hundred taps on ~1000 bins: an FFT, as in the paper, would not pay)
+__global__ void __launch_bounds__(256)
+ipa_gauss_smear_kernel(const double* __restrict__ in, int nbins, double w, double sigma0, int M, double* __restrict__ out) {
+  extern __shared__ double g_smem[];   // [2M+1]
+  __shared__ double red[8];
+  double part = 0.0;
+  const double inv = 1.0 / (2.0 * sigma0 * sigma0);
+  for (int i = threadIdx.x; i <= 2 * M; i += 256) {
+    const double xm = (double)(i - M) * w;
+    const double v = exp(-xm * xm * inv);
+    g_smem[i] = v;
+    part += v;
+  }
+  const double norm = ipa_block_sum_256(part, red);
+  __syncthreads();
+  const int b = blockIdx.x * 256 + threadIdx.x;
+  if (b >= nbins) return;
+  const int j0 = b - M > 0 ? b - M : 0, j1 = b + M < nbins - 1 ? b + M : nbins - 1;
+  double acc = 0.0;
+  for (int j = j0; j <= j1; ++j) acc = fma(in[j], g_smem[b - j + M], acc);
+  out[b] = acc / norm;
 }
 
 // one block per scan point q: nu_b = ns s_b + nb e^{k (c_b-lo)} / sum_b' e^{k (c_b'-lo)};

@@ -598,3 +598,33 @@ def test_maximum_batch_of_32_sets(ipa, torch_, orc, x1):
             assert got[i] == ipa.ipa_nll_eval(xd, sets[i], LO, HI)[0].item()
     with pytest.raises(ipa.IpaError):
         ipa.ipa_nll_eval(xd, distinct + [inp.GEN], LO, HI)          # 33 sets: invalid argument
+
+
+# ---------------------------------------------------------------------------------------------
+# Gaussian-smeared signal shape feeding the binned path (reading F3)
+# ---------------------------------------------------------------------------------------------
+def test_gauss_smear_and_given_shape_binned_path(ipa, torch_, orc):
+    for nbins, s0, theta in ((1000, 10.0, inp.GEN), (333, 3.3, inp.P2), (1000, 0.0, inp.GEN), (64, 40.0, inp.GEN)):
+        sig = ipa.ipa_signal_shape(nbins, LO, HI, theta)
+        sm = ipa.ipa_gauss_smear(sig, LO, HI, s0)
+        torch_.cuda.synchronize()
+        sig_ref = orc.signal_shape(nbins, LO, HI, theta)
+        sm_ref = orc.gauss_smear(sig_ref, LO, HI, s0)
+        assert np.abs(sig.cpu().numpy() - sig_ref).max() <= 1e-13 * sig_ref.max()
+        assert np.abs(sm.cpu().numpy() - sm_ref).max() <= 1e-13 * sm_ref.max()
+        # the oracle on the GPU's own input: the convolution alone
+        assert np.abs(sm.cpu().numpy() - orc.gauss_smear(sig.cpu().numpy(), LO, HI, s0)).max() <= 1e-14 * sm_ref.max()
+        n_obs = 1.0e6
+        nu = ipa.ipa_expected_hist_shape(sm, LO, HI, 2500.0, n_obs - 2500.0, -0.002)
+        nu_ref = orc.expected_hist_shape(LO, HI, sm_ref, 2500.0, n_obs - 2500.0, -0.002)
+        assert np.all(np.abs(nu.cpu().numpy() - nu_ref) <= 1e-12 * nu_ref)
+        counts = np.random.Generator(np.random.Philox(nbins)).poisson(nu_ref).astype(np.uint64)
+        ns, nb, kk = inp.scan_grid(7, 5, n_obs=n_obs)
+        got = ipa.ipa_binned_nll_scan_shape(dev(torch_, counts.astype(np.int64)), LO, HI, sm, ns, nb, kk)
+        torch_.cuda.synchronize()
+        ref = orc.binned_nll_scan_shape(counts, LO, HI, sm_ref, ns, nb, kk)
+        assert np.all(np.abs(got.cpu().numpy() - ref) <= 1e-10 * np.abs(ref))
+    # a shape with no content: flagged, not a crash
+    zero = torch_.zeros(100, dtype=torch_.float64, device="cuda")
+    bad = ipa.ipa_binned_nll_scan_shape(dev(torch_, np.ones(100, dtype=np.int64)), LO, HI, zero, [1.0], [10.0], [-0.002])
+    assert np.isposinf(bad.cpu().numpy()).all()
