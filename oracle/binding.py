@@ -51,6 +51,7 @@ def lib():
         L.orc_binned_nll_scan_shape.restype = i32
         L.orc_binned_nll_scan_shape.argtypes = [vp, i32, d, d, vp, vp, vp, vp, i64, vp]
         L.orc_signal_shape.restype = i32; L.orc_signal_shape.argtypes = [i32, d, d, vp, vp]
+        L.orc_nll_extended.restype = i32; L.orc_nll_extended.argtypes = [vp, i64, vp, d, d, d, d, vp]
         L.orc_cls_teststat.restype = None; L.orc_cls_teststat.argtypes = [vp, i32, i64, i32, vp, vp, vp]
         L.orc_cls_count_ge.restype = i64; L.orc_cls_count_ge.argtypes = [vp, i64, d]
         L.orc_cls_from_counts.restype = None; L.orc_cls_from_counts.argtypes = [i64, i64, i64, i64, vp]
@@ -309,3 +310,13 @@ def binned_nll_scan_shape(counts, lo, hi, sig, ns, nb, k):
                                          ns.size, _p(out))
     assert st == 0, st
     return out
+
+
+def nll_extended(x, p, ns, nb, lo, hi):
+    """Extended -log L = (ns + nb) - sum log(ns S + nb B) of one shape (its f is ignored); reading D4."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    P = pack_params(p)
+    out = np.empty(1)
+    st = lib().orc_nll_extended(_p(x), x.size, _p(P), float(ns), float(nb), float(lo), float(hi), _p(out))
+    assert st == 0, st
+    return float(out[0])

@@ -874,4 +874,29 @@ int orc_signal_shape(int nbins, double lo, double hi, const orc_params* shape, d
   for (int b = 0; b < nbins; ++b) out[b] = (double)expl(log_I(s, lo + (b + 0.5L) * w - s.mu) - ref);
   return 0;
 }
+
+/* ------------------------------------------------------------------------------------------
+ * Extended likelihood (reading D4: the paper's FCN works with yields, "fs", "fb" and
+ * "the sum, including normalization terms"):
+ *     -log L_ext(ns, nb, shape) = (ns + nb) - sum_i log( ns S(x_i) + nb B(x_i) )
+ * written out as such (not through the fraction form); the f field of the parameter set is ignored.
+ * ---------------------------------------------------------------------------------------- */
+int orc_nll_extended(const double* x, int64_t n, const orc_params* pp, double ns, double nb, double lo_, double hi_,
+                     double* out) {
+  orc_params p = *pp;
+  p.f = 0.5;                                  /* only the shape and k are used */
+  const Shape s = make_shape(p);
+  if (s.status) return s.status;
+  if (!(ns >= 0) || !(nb >= 0) || !(ns + nb > 0)) return 1;
+  const ld lo = lo_, hi = hi_;
+  const Norm N = make_norm(s, p.k, lo, hi);
+  std::vector<double> l((size_t)n);
+  for (int64_t i = 0; i < n; ++i) {
+    const ld S = expl(log_I(s, (ld)x[i] - s.mu) - N.logref) / N.NS;
+    const ld B = expl((ld)p.k * ((ld)x[i] - lo)) / N.NB;
+    l[i] = (double)logl((ld)ns * S + (ld)nb * B);
+  }
+  *out = (double)(((ld)ns + (ld)nb) - pairwise(l.data(), 0, n));
+  return 0;
+}
 } /* extern "C" */
