@@ -118,6 +118,15 @@ int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K
                  double* nll_dev, double* logpdf_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
                  void* cuda_stream);
 
+/* Extended likelihood (reading D4: the paper's FCN works with yields):
+ *   nll_dev[k] = (ns_k + nb_k) - sum_i log( ns_k S(x_i) + nb_k B(x_i) )
+ * for K sets; the f field of p_host is ignored (the library evaluates the fraction form with
+ * f = ns/(ns+nb), computed in fp64 on the host, and adds (ns+nb) - n log(ns+nb) on the device).
+ * ns_k, nb_k >= 0, ns_k + nb_k > 0, else status 1.  Everything else as ipa_nll_eval. */
+int ipa_nll_eval_extended(const double* x_dev, int64_t n, const ipa_params* p_host, const double* ns_host,
+                          const double* nb_host, int K, ipa_range r, double* nll_dev, int32_t* status_dev,
+                          void* ws_dev, size_t ws_bytes, void* cuda_stream);
+
 /* NLL and its ANALYTIC gradient with respect to (mu, sigma, f, k) in one pass (the
  * paper mentions analytic gradients through iminuit and generated derivative code, PAPER.md:36, 383,
  * without formulae; the derivatives are those of the definition above):

@@ -12,7 +12,8 @@ from . import build as _build
 
 __all__ = [
     "PARAM_FIELDS", "NPAR", "IPA_MAX_K", "IpaError", "lib", "library_path", "pack_params", "workspace",
-    "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes", "ipa_norm", "ipa_core_degree", "ipa_nll_grad_eval", "ipa_nll_eval",
+    "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes", "ipa_norm", "ipa_core_degree", "ipa_nll_grad_eval",
+    "ipa_nll_eval_extended", "ipa_nll_eval",
     "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill", "ipa_binned_nll_scan", "ipa_expected_hist",
     "ipa_poisson_hist_toys", "ipa_signal_shape", "ipa_gauss_smear", "ipa_expected_hist_shape", "ipa_binned_nll_scan_shape",
     "ipa_cls_teststat", "ipa_cls_count_ge", "ipa_cls_from_counts", "ipa_events_sort",
@@ -26,7 +27,7 @@ IPA_MAX_K = 32
 # every symbol include/ipanll.h declares
 EXPORTS = (
     "ipa_strerror", "ipa_last_cuda_error", "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes",
-    "ipa_norm", "ipa_core_degree", "ipa_nll_eval", "ipa_nll_grad_eval", "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill",
+    "ipa_norm", "ipa_core_degree", "ipa_nll_eval", "ipa_nll_eval_extended", "ipa_nll_grad_eval", "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill",
     "ipa_binned_nll_scan", "ipa_expected_hist", "ipa_poisson_hist_toys", "ipa_signal_shape", "ipa_gauss_smear",
     "ipa_expected_hist_shape", "ipa_binned_nll_scan_shape", "ipa_cls_teststat", "ipa_cls_count_ge",
     "ipa_cls_from_counts", "ipa_sort_workspace_bytes", "ipa_events_sort",
@@ -65,6 +66,8 @@ def lib():
     L.ipa_norm.restype = i32; L.ipa_norm.argtypes = [vp, i32, _Range, vp, vp, vp, vp, sz, vp]
     L.ipa_core_degree.restype = i32; L.ipa_core_degree.argtypes = [vp, i32, _Range, vp, vp, sz, vp]
     L.ipa_nll_eval.restype = i32; L.ipa_nll_eval.argtypes = [vp, i64, vp, i32, _Range, vp, vp, vp, vp, sz, vp]
+    L.ipa_nll_eval_extended.restype = i32
+    L.ipa_nll_eval_extended.argtypes = [vp, i64, vp, vp, vp, i32, _Range, vp, vp, vp, sz, vp]
     L.ipa_nll_grad_eval.restype = i32; L.ipa_nll_grad_eval.argtypes = [vp, i64, vp, i32, _Range, vp, vp, vp, vp, sz, vp]
     L.ipa_nll_eval_segmented.restype = i32
     L.ipa_nll_eval_segmented.argtypes = [vp, vp, i64, vp, _Range, vp, vp, vp, sz, vp]
@@ -205,6 +208,22 @@ def ipa_nll_eval(x, params, lo, hi, want_logpdf=False, ws=None, stream=None, out
     _check(lib().ipa_nll_eval(_dptr(x, torch.float64) if n else None, n, _hptr(P), K, _Range(lo, hi), _dptr(nll),
                               _dptr(lp), _dptr(st), _dptr(ws), ws.numel(), _stream(stream)))
     return nll, lp, st
+
+
+def ipa_nll_eval_extended(x, params, ns, nb, lo, hi, ws=None, stream=None):
+    """Extended -log L = (ns+nb) - sum log(ns S + nb B) for K (shape, ns, nb) triples -> (nll[K], status[K])."""
+    _need_cuda()
+    P = pack_params(params)
+    K = P.shape[0]
+    ns = np.ascontiguousarray(np.broadcast_to(np.asarray(ns, dtype=np.float64), (K,)))
+    nb = np.ascontiguousarray(np.broadcast_to(np.asarray(nb, dtype=np.float64), (K,)))
+    n = x.numel()
+    ws = _ws(ws, n, K)
+    nll = torch.empty(K, dtype=torch.float64, device="cuda")
+    st = torch.empty(K, dtype=torch.int32, device="cuda")
+    _check(lib().ipa_nll_eval_extended(_dptr(x, torch.float64) if n else None, n, _hptr(P), _hptr(ns), _hptr(nb), K,
+                                       _Range(lo, hi), _dptr(nll), _dptr(st), _dptr(ws), ws.numel(), _stream(stream)))
+    return nll, st
 
 
 def ipa_nll_grad_eval(x, params, lo, hi, ws=None, stream=None):

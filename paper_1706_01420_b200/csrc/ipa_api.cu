@@ -197,6 +197,28 @@ int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K
   return IPA_OK;
 }
 
+int ipa_nll_eval_extended(const double* x_dev, int64_t n, const ipa_params* p_host, const double* ns_host,
+                          const double* nb_host, int K, ipa_range r, double* nll_dev, int32_t* status_dev,
+                          void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (!p_host || !ns_host || !nb_host || K < 1 || K > IPA_MAX_K) return IPA_ERR_INVALID_ARG;
+  ipa_params q[IPA_MAX_K];
+  double nu[IPA_MAX_K];
+  for (int k = 0; k < K; ++k) {
+    q[k] = p_host[k];
+    nu[k] = ns_host[k] + nb_host[k];
+    const bool ok = ns_host[k] >= 0.0 && nb_host[k] >= 0.0 && nu[k] > 0.0 && ipa_finite(nu[k]);
+    q[k].f = ok ? ns_host[k] / nu[k] : -1.0;          // an invalid yield pair becomes a domain error of the set
+    if (!ok) nu[k] = 1.0;
+  }
+  int rc = ipa_nll_eval(x_dev, n, q, K, r, nll_dev, nullptr, status_dev, ws_dev, ws_bytes, cuda_stream);
+  if (rc) return rc;
+  IpaYields y;
+  for (int k = 0; k < IPA_MAX_K; ++k) y.nu[k] = k < K ? nu[k] : 1.0;
+  ipa_extended_term_kernel<<<1, IPA_MAX_K, 0, static_cast<cudaStream_t>(cuda_stream)>>>(nll_dev, K, (long long)n, y);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
 int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r,
                       double* nll_dev, double* grad_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
                       void* cuda_stream) {

@@ -1234,6 +1234,14 @@ __global__ void ipa_degree_kernel(const IpaSetConsts* __restrict__ consts, int K
   if (k < K) out[k] = consts[k].status ? -2 : (consts[k].mode ? -1 : consts[k].degree);
 }
 
+// extended likelihood (row f4): nll[k] += nu_k - n log nu_k on top of the fraction-form NLL with f = ns/(ns+nb);
+// the total yields travel in the kernel-parameter space
+struct IpaYields { double nu[IPA_MAX_K]; };
+__global__ void ipa_extended_term_kernel(double* __restrict__ nll, int K, long long n, const __grid_constant__ IpaYields y) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k < K) nll[k] += y.nu[k] - (double)n * log(y.nu[k]);
+}
+
 // ------------------------------------------------------------------------------------------------
 // FP64 peak probe: 8 independent DFMA chains per thread
 // ------------------------------------------------------------------------------------------------

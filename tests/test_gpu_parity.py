@@ -628,3 +628,20 @@ def test_gauss_smear_and_given_shape_binned_path(ipa, torch_, orc):
     zero = torch_.zeros(100, dtype=torch_.float64, device="cuda")
     bad = ipa.ipa_binned_nll_scan_shape(dev(torch_, np.ones(100, dtype=np.int64)), LO, HI, zero, [1.0], [10.0], [-0.002])
     assert np.isposinf(bad.cpu().numpy()).all()
+
+
+# ---------------------------------------------------------------------------------------------
+# extended likelihood (reading D4)
+# ---------------------------------------------------------------------------------------------
+def test_extended_likelihood(ipa, torch_, orc, x1):
+    xd = dev(torch_, x1)
+    sets = [inp.GEN, inp.P2, inp.GEN, inp.P2, inp.GEN]
+    ns = np.array([3000.0, 120.5, 0.0, 9000.0, -1.0])
+    nb = np.array([7000.0, 9900.0, 10000.0, 0.0, 5.0])
+    nll, st = ipa.ipa_nll_eval_extended(xd, sets, ns, nb, LO, HI)
+    torch_.cuda.synchronize()
+    nll, st = nll.cpu().numpy(), st.cpu().numpy()
+    assert list(st) == [0, 0, 0, 0, 1] and np.isposinf(nll[4])
+    for i in range(4):
+        ref = orc.nll_extended(x1, sets[i], ns[i], nb[i], LO, HI)
+        assert abs(nll[i] - ref) <= 1e-10 * abs(ref), (i, nll[i], ref)
