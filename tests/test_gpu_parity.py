@@ -645,3 +645,20 @@ def test_extended_likelihood(ipa, torch_, orc, x1):
     for i in range(4):
         ref = orc.nll_extended(x1, sets[i], ns[i], nb[i], LO, HI)
         assert abs(nll[i] - ref) <= 1e-10 * abs(ref), (i, nll[i], ref)
+
+
+def test_edge_cases_of_the_next_rows(ipa, torch_, orc, x1):
+    """Empty and one-element inputs of the rows added after the hot path (f1-f4)."""
+    xd = dev(torch_, x1)
+    nll, grad, st = ipa.ipa_nll_grad_eval(xd[:0], inp.GEN, LO, HI)                       # n = 0
+    assert nll.item() == 0.0 and not np.signbit(nll.item()) and np.all(grad.cpu().numpy() == 0.0) and st.item() == 0
+    nll, grad, _ = ipa.ipa_nll_grad_eval(xd[:1], inp.P2, LO, HI)                          # n = 1
+    r_nll, r_g = orc.nll_gradient(x1[:1], inp.P2, LO, HI)
+    assert abs(nll.item() - r_nll) <= 1e-12 * abs(r_nll) and grad_ok(grad[0].cpu().numpy(), r_g)
+    e, st = ipa.ipa_nll_eval_extended(xd[:0], inp.GEN, 3.0, 4.0, LO, HI)                  # no events: -log L = ns + nb
+    assert e.item() == 7.0 and st.item() == 0
+    one = dev(torch_, np.array([2.0]))
+    assert ipa.ipa_gauss_smear(one, LO, HI, 50.0).item() == pytest.approx(orc.gauss_smear(np.array([2.0]), LO, HI, 50.0)[0], rel=1e-14)
+    q = ipa.ipa_cls_teststat(dev(torch_, np.array([5], dtype=np.int64)).to(torch_.int32), dev(torch_, np.array([6.5])),
+                             dev(torch_, np.array([4.0])))
+    assert abs(q.item() - orc.cls_teststat(np.array([[5]], dtype=np.uint32), [6.5], [4.0])[0]) <= 1e-12
