@@ -356,22 +356,22 @@ __device__ __forceinline__ void ipa_tile_sets(const IpaSetConsts* sc, int K, con
       ipa_eval_set<IPA_NE>(c, xv, l, s_tab);
       ipa_tile_store_acc<LOGPDF, FULL>(k, l, acc, base, n, tid, logpdf);
     }
-    return;
-  }
-  for (int g = 0; g < K; ++g) {
-    if (grp.leader[g] != g) continue;
-    int v = g;                                   // first member with a usable record
-    while (v < K && (grp.leader[v] != g || sc[v].status)) ++v;
-    if (v >= K) continue;
-    double d[IPA_NE], V[IPA_NE];
-    const int region = ipa_shape_stage<IPA_NE>(sc[v], xv, d, V, s_tab);
-    for (int k = v; k < K; ++k) {
-      if (grp.leader[k] != g) continue;
-      const IpaSetConsts& c = sc[k];
-      if (c.status) continue;
-      double l[IPA_NE];
-      ipa_member_stage<IPA_NE>(c, region, d, V, l, s_tab);
-      ipa_tile_store_acc<LOGPDF, FULL>(k, l, acc, base, n, tid, logpdf);
+  } else {
+    for (int g = 0; g < K; ++g) {
+      if (grp.leader[g] != g) continue;
+      int v = g;                                   // first member with a usable record
+      while (v < K && (grp.leader[v] != g || sc[v].status)) ++v;
+      if (v >= K) continue;
+      double d[IPA_NE], V[IPA_NE];
+      const int region = ipa_shape_stage<IPA_NE>(sc[v], xv, d, V, s_tab);
+      for (int k = v; k < K; ++k) {
+        if (grp.leader[k] != g) continue;
+        const IpaSetConsts& c = sc[k];
+        if (c.status) continue;
+        double l[IPA_NE];
+        ipa_member_stage<IPA_NE>(c, region, d, V, l, s_tab);
+        ipa_tile_store_acc<LOGPDF, FULL>(k, l, acc, base, n, tid, logpdf);
+      }
     }
   }
 }
