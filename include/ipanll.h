@@ -15,10 +15,11 @@
  *   - `*_dev` pointers are CUDA device pointers, `*_host` pointers are host pointers.  The caller owns
  *     every buffer.  The library never allocates or frees device memory and never synchronises: all
  *     work is enqueued on `cuda_stream` (a cudaStream_t passed as void*; NULL = the legacy default
- *     stream) and results are valid once the caller has synchronised that stream.  `*_host` inputs are
- *     read completely before the call returns (they are copied into the kernel-parameter space or
- *     into the workspace with kernel arguments, never with an asynchronous host read), so they may be
- *     reused immediately.  ipa_norm, ipa_core_degree and ipa_nll_eval (K <= IPA_MAX_K: the parameter sets
+ *     stream) and results are valid once the caller has synchronised that stream.  `*_host` parameter
+ *     sets of up to IPA_MAX_K entries travel in the kernel-parameter space and may be reused as soon as
+ *     the call returns.  Larger host arrays (more than IPA_MAX_K sets, toy seeds, scan points) are
+ *     uploaded with cudaMemcpyAsync: a pageable array is staged before the call returns and may be reused
+ *     immediately, a PINNED array must stay unchanged until the stream has passed the copy.  ipa_norm, ipa_core_degree and ipa_nll_eval (K <= IPA_MAX_K: the parameter sets
  *     travel in the kernel-parameter space) can be captured in a CUDA graph; a replay re-evaluates the
  *     parameter values given at capture time.  Calls that upload a host array with a copy (more than
  *     IPA_MAX_K sets, toy seeds, scan points) capture only if that array is in pinned host memory.
