@@ -19,7 +19,7 @@ struct IpaParamBatch { ipa_params p[IPA_MAX_K]; };
 // ------------------------------------------------------------------------------------------------
 // Prologue: one block per parameter set.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(IPA_PRO_THREADS)
+__global__ void __launch_bounds__(IPA_PRO_THREADS, 3)
 ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_params* __restrict__ p_dev, double lo,
                     double hi, int policy, IpaSetConsts* __restrict__ consts, unsigned int* counter,
                     double* norm_sig, double* norm_bkg, int32_t* status_out) {

@@ -23,8 +23,8 @@
 #define IPA_JMAX 256            // trapezoid table length
 #define IPA_GL 16               // Gauss-Legendre nodes per panel
 #define IPA_MAXPANEL 24         // 12 per side
-#define IPA_PRO_THREADS 512
-#define IPA_SUB 4               // threads sharing one table-based Bessel evaluation
+#define IPA_PRO_THREADS 256
+#define IPA_SUB 2               // threads sharing one table-based Bessel evaluation
 #define IPA_NBTASK (IPA_MCHEB + 4)  // Chebyshev nodes + K_nu(z0), K_nu(z1), K_{nu-1}(z0), K_{nu-1}(z1)
 
 // What the streaming kernels read, per parameter set (all fp64 except the flags).
