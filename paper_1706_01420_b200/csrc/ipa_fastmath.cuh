@@ -165,6 +165,23 @@ IPA_HD double ipa_flog_1to2(double s, const Tab* tab) {
   return fma(p, r, lj);
 }
 
+// e^{-|D|}: -|D| enters through operand modifiers, the exponent shift is clamped instead of the argument.
+// |D| < 2^50.
+IPA_HD double ipa_fexp_negabs(double D) {
+  const double SHIFT = 6755399441055744.0;
+  const double a = -fabs(D);
+  const double t = fma(a, IPA_LOG2E, SHIFT);
+  int n = ipa_lo(t);
+  const double nf = t - SHIFT;
+  double r = fma(nf, -IPA_LN2_HI, a);
+  r = fma(nf, -IPA_LN2_LO, r);
+  double p = IPA_CEXP(IPA_EXP_DEG);
+#pragma unroll
+  for (int j = IPA_EXP_DEG - 1; j >= 0; --j) p = fma(p, r, IPA_CEXP(j));
+  n = n > -1000 ? n : -1000;
+  return ipa_mk(ipa_hi(p) + (n << 20), ipa_lo(p));
+}
+
 // eb + log(1 + e^D) = eb + log(1 + e^{-|D|}) [+ D if D >= 0].  -|D| enters the exponential through operand
 // modifiers, the exponent shift is clamped instead of the argument, and max(D,0) is a predicated add on
 // the sign word: 2 integer instructions where the clamp / relu pair above needs 7.  |D| < 2^50.

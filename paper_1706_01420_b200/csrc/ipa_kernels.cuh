@@ -526,12 +526,13 @@ IPA_HD void ipa_grad_tail(const IpaSetConsts& c, bool right, double d, double& D
 template <class Tab>
 IPA_HD void ipa_grad_mix(const IpaSetConsts& c, double d, double D, double dd, double ds, double& l, double& gm, double& gs,
                          double& gf, double& gk, const Tab* tab) {
-  const double w = ipa_fexp_neg(ipa_neg_abs_clamped(D));
+  const double w = ipa_fexp_negabs(D);
   const double s1 = 1.0 + w;
   const double rs = ipa_frcp(s1);
   const bool pos = ipa_hi(D) >= 0;
   const double wS = pos ? rs : w * rs, wB = pos ? w * rs : rs;
-  l = fma(c.kd, d, c.eB0) + ipa_relu_bits(D) + ipa_flog_1to2(s1, tab);
+  l = fma(c.kd, d, c.eB0) + ipa_flog_1to2(s1, tab);
+  if (pos) l += D;
   gm = wS * (-dd - c.dlnNS_dmu);
   gs = wS * (ds - c.dlnNS_dsig);
   gf = fma(wS, c.invf, -wB * c.inv1mf);
