@@ -149,6 +149,15 @@ int ipa_nll_eval_segmented(const double* x_dev, const int64_t* offsets_dev, int6
                            ipa_range r, double* nll_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
                            void* cuda_stream);
 
+/* Simultaneous categories with SHARED parameter sets (one model, several categories,
+ * parameters in common): as ipa_nll_eval_segmented, but segment t is evaluated with parameter set
+ * set_of_segment_host[t] in [0, K) of p_host [K]; the prologue runs once per set, not once per segment.
+ * The fit's NLL is the sum of nll_dev [T] (added by the caller or by one more reduction).  Workspace:
+ * ipa_workspace_bytes(n, max(K, T), 0). */
+int ipa_nll_eval_categories(const double* x_dev, const int64_t* offsets_dev, int64_t T, const ipa_params* p_host, int64_t K,
+                            const int32_t* set_of_segment_host, ipa_range r, double* nll_dev, int32_t* status_dev,
+                            void* ws_dev, size_t ws_bytes, void* cuda_stream);
+
 /* Toy-MC generation on the device (readings D13, D14).
  * Toy t draws Ns ~ Poisson(mean_sig), Nb ~ Poisson(mean_bkg) from seeds_host[t] (Philox-4x32-10
  * counter-based streams), then Ns signal events by accept-reject under a flat envelope followed by

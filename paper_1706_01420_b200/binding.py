@@ -13,7 +13,7 @@ from . import build as _build
 __all__ = [
     "PARAM_FIELDS", "NPAR", "IPA_MAX_K", "IpaError", "lib", "library_path", "pack_params", "workspace",
     "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes", "ipa_norm", "ipa_core_degree", "ipa_nll_grad_eval",
-    "ipa_nll_eval_extended", "ipa_nll_eval",
+    "ipa_nll_eval_extended", "ipa_nll_eval_categories", "ipa_nll_eval",
     "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill", "ipa_binned_nll_scan", "ipa_expected_hist",
     "ipa_poisson_hist_toys", "ipa_signal_shape", "ipa_gauss_smear", "ipa_expected_hist_shape", "ipa_binned_nll_scan_shape",
     "ipa_cls_teststat", "ipa_cls_count_ge", "ipa_cls_from_counts", "ipa_events_sort",
@@ -27,7 +27,7 @@ IPA_MAX_K = 32
 # every symbol include/ipanll.h declares
 EXPORTS = (
     "ipa_strerror", "ipa_last_cuda_error", "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes",
-    "ipa_norm", "ipa_core_degree", "ipa_nll_eval", "ipa_nll_eval_extended", "ipa_nll_grad_eval", "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill",
+    "ipa_norm", "ipa_core_degree", "ipa_nll_eval", "ipa_nll_eval_extended", "ipa_nll_grad_eval", "ipa_nll_eval_segmented", "ipa_nll_eval_categories", "ipa_toy_generate", "ipa_hist_fill",
     "ipa_binned_nll_scan", "ipa_expected_hist", "ipa_poisson_hist_toys", "ipa_signal_shape", "ipa_gauss_smear",
     "ipa_expected_hist_shape", "ipa_binned_nll_scan_shape", "ipa_cls_teststat", "ipa_cls_count_ge",
     "ipa_cls_from_counts", "ipa_sort_workspace_bytes", "ipa_events_sort",
@@ -71,6 +71,8 @@ def lib():
     L.ipa_nll_grad_eval.restype = i32; L.ipa_nll_grad_eval.argtypes = [vp, i64, vp, i32, _Range, vp, vp, vp, vp, sz, vp]
     L.ipa_nll_eval_segmented.restype = i32
     L.ipa_nll_eval_segmented.argtypes = [vp, vp, i64, vp, _Range, vp, vp, vp, sz, vp]
+    L.ipa_nll_eval_categories.restype = i32
+    L.ipa_nll_eval_categories.argtypes = [vp, vp, i64, vp, i64, vp, _Range, vp, vp, vp, sz, vp]
     L.ipa_toy_generate.restype = i32
     L.ipa_toy_generate.argtypes = [vp, i64, vp, i64, d, d, _Range, i64, vp, vp, vp, vp, sz, vp]
     L.ipa_hist_fill.restype = i32; L.ipa_hist_fill.argtypes = [vp, i64, _Range, i32, vp, vp]
@@ -252,6 +254,22 @@ def ipa_nll_eval_segmented(x, offsets, params, lo, hi, ws=None, stream=None):
     st = torch.empty(T, dtype=torch.int32, device="cuda")
     _check(lib().ipa_nll_eval_segmented(_dptr(x, torch.float64), _dptr(offsets, torch.int64), T, _hptr(P),
                                         _Range(lo, hi), _dptr(nll), _dptr(st), _dptr(ws), ws.numel(), _stream(stream)))
+    return nll, st
+
+
+def ipa_nll_eval_categories(x, offsets, params, set_of_segment, lo, hi, ws=None, stream=None):
+    """Segments (categories) sharing parameter sets: segment t uses params[set_of_segment[t]] -> (nll[T], status[T])."""
+    _need_cuda()
+    P = pack_params(params)
+    T = offsets.numel() - 1
+    m = np.ascontiguousarray(set_of_segment, dtype=np.int32).ravel()
+    assert m.size == T
+    ws = _ws(ws, x.numel(), max(T, P.shape[0]))
+    nll = torch.empty(T, dtype=torch.float64, device="cuda")
+    st = torch.empty(T, dtype=torch.int32, device="cuda")
+    _check(lib().ipa_nll_eval_categories(_dptr(x, torch.float64), _dptr(offsets, torch.int64), T, _hptr(P), P.shape[0],
+                                         _hptr(m), _Range(lo, hi), _dptr(nll), _dptr(st), _dptr(ws), ws.numel(),
+                                         _stream(stream)))
     return nll, st
 
 

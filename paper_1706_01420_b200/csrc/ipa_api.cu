@@ -248,25 +248,48 @@ int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, 
   return IPA_OK;
 }
 
-int ipa_nll_eval_segmented(const double* x_dev, const int64_t* offsets_dev, int64_t T, const ipa_params* p_host,
-                           ipa_range r, double* nll_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
-                           void* cuda_stream) {
-  if (!x_dev || !offsets_dev || T < 1 || T > 0x7fffffffLL || !p_host || !range_ok(r) || !nll_dev)
+static int segmented_common(const double* x_dev, const int64_t* offsets_dev, int64_t T, const ipa_params* p_host,
+                            int64_t K, const int32_t* set_of_segment_host, ipa_range r, double* nll_dev,
+                            int32_t* status_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (!x_dev || !offsets_dev || T < 1 || T > 0x7fffffffLL || K < 1 || K > 0x7fffffffLL || !p_host || !range_ok(r) ||
+      !nll_dev)
     return IPA_ERR_INVALID_ARG;
-  const Layout L = make_layout(T, 0);
+  if (set_of_segment_host)
+    for (int64_t t = 0; t < T; ++t)
+      if (set_of_segment_host[t] < 0 || set_of_segment_host[t] >= K) return IPA_ERR_INVALID_ARG;
+  const Layout L = make_layout(T > K ? T : K, 0);
   if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   char* ws = static_cast<char*>(ws_dev);
-  int rc = run_prologue(p_host, T, r, ws, L, nullptr, nullptr, nullptr, st);
+  int rc = run_prologue(p_host, K, r, ws, L, nullptr, nullptr, nullptr, st);
   if (rc) return rc;
   const IpaSetConsts* consts = reinterpret_cast<const IpaSetConsts*>(ws + L.consts);
   double* partials = reinterpret_cast<double*>(ws + L.partials);
+  const int* map = nullptr;
+  if (set_of_segment_host) {   // the map travels through the (otherwise unused) yields area of the workspace
+    IPA_CK(cudaMemcpyAsync(ws + L.nsig, set_of_segment_host, (size_t)T * 4, cudaMemcpyHostToDevice, st));
+    map = reinterpret_cast<const int*>(ws + L.nsig);
+  }
   ipa_nll_seg_kernel<<<dim3((unsigned)T, IPA_SEGC), IPA_BLOCK, 0, st>>>(
-      x_dev, reinterpret_cast<const long long*>(offsets_dev), consts, partials);
+      x_dev, reinterpret_cast<const long long*>(offsets_dev), consts, map, partials);
   IPA_CK(cudaGetLastError());
-  ipa_seg_finalize_kernel<<<(unsigned)((T + 127) / 128), 128, 0, st>>>(partials, consts, T, nll_dev, status_dev);
+  ipa_seg_finalize_kernel<<<(unsigned)((T + 127) / 128), 128, 0, st>>>(partials, consts, map, T, nll_dev, status_dev);
   IPA_CK(cudaGetLastError());
   return IPA_OK;
+}
+
+int ipa_nll_eval_segmented(const double* x_dev, const int64_t* offsets_dev, int64_t T, const ipa_params* p_host,
+                           ipa_range r, double* nll_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
+                           void* cuda_stream) {
+  return segmented_common(x_dev, offsets_dev, T, p_host, T, nullptr, r, nll_dev, status_dev, ws_dev, ws_bytes, cuda_stream);
+}
+
+int ipa_nll_eval_categories(const double* x_dev, const int64_t* offsets_dev, int64_t T, const ipa_params* p_host, int64_t K,
+                            const int32_t* set_of_segment_host, ipa_range r, double* nll_dev, int32_t* status_dev,
+                            void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (!set_of_segment_host) return IPA_ERR_INVALID_ARG;
+  return segmented_common(x_dev, offsets_dev, T, p_host, K, set_of_segment_host, r, nll_dev, status_dev, ws_dev, ws_bytes,
+                          cuda_stream);
 }
 
 int ipa_toy_generate(const uint64_t* seeds_host, int64_t T, const ipa_params* gen_host, int64_t gen_count,

@@ -716,7 +716,8 @@ __device__ __forceinline__ void ipa_cp_async8(void* smem_dst, const void* gmem_s
 // of the next tile flies while the current one is evaluated; each thread reads only its own slots.
 __global__ void __launch_bounds__(IPA_BLOCK, IPA_BLOCKS_PER_SM)
 ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ offsets,
-                   const IpaSetConsts* __restrict__ consts, double* __restrict__ partials) {
+                   const IpaSetConsts* __restrict__ consts, const int* __restrict__ set_of_segment,
+                   double* __restrict__ partials) {
   __shared__ IpaSetConsts c;
   __shared__ double red[IPA_BLOCK / 32];
   __shared__ double2 s_tab[33];
@@ -735,7 +736,8 @@ ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ o
   };
   if (cb < ce) issue(cb, 0);
   {
-    const double* src = reinterpret_cast<const double*>(consts + t);
+    // categories may share a parameter set (set_of_segment != NULL): segment t uses record set_of_segment[t]
+    const double* src = reinterpret_cast<const double*>(consts + (set_of_segment ? set_of_segment[t] : t));
     double* dst = reinterpret_cast<double*>(&c);
     for (int i = tid; i < (int)(sizeof(IpaSetConsts) / 8); i += IPA_BLOCK) dst[i] = src[i];
     ipa_load_logtab(s_tab);
@@ -767,12 +769,13 @@ ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ o
 }
 
 __global__ void ipa_seg_finalize_kernel(const double* __restrict__ partials, const IpaSetConsts* __restrict__ consts,
-                                        long long T, double* __restrict__ nll, int32_t* __restrict__ status_out) {
+                                        const int* __restrict__ set_of_segment, long long T, double* __restrict__ nll,
+                                        int32_t* __restrict__ status_out) {
   const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   if (t >= T) return;
   double v = 0.0;
   for (int c = 0; c < IPA_SEGC; ++c) v += partials[t * IPA_SEGC + c];
-  const int st = consts[t].status;
+  const int st = consts[set_of_segment ? set_of_segment[t] : t].status;
   nll[t] = st ? INFINITY : 0.0 - v;
   if (status_out) status_out[t] = st;
 }

@@ -662,3 +662,18 @@ def test_edge_cases_of_the_next_rows(ipa, torch_, orc, x1):
     q = ipa.ipa_cls_teststat(dev(torch_, np.array([5], dtype=np.int64)).to(torch_.int32), dev(torch_, np.array([6.5])),
                              dev(torch_, np.array([4.0])))
     assert abs(q.item() - orc.cls_teststat(np.array([[5]], dtype=np.uint32), [6.5], [4.0])[0]) <= 1e-12
+
+
+def test_categories_with_shared_parameter_sets(ipa, torch_, orc, x1):
+    """Row f4: segments (categories) mapped onto a smaller list of parameter sets."""
+    off = np.array([0, 1500, 1500, 4000, 7777, 10000], dtype=np.int64)
+    sets = [dict(inp.GEN), dict(inp.P2), dict(inp.GEN, f=1.5)]            # the last one is invalid
+    m = np.array([1, 0, 0, 1, 2], dtype=np.int32)
+    nll, st = ipa.ipa_nll_eval_categories(dev(torch_, x1), dev(torch_, off), sets, m, LO, HI)
+    torch_.cuda.synchronize()
+    nll, st = nll.cpu().numpy(), st.cpu().numpy()
+    assert list(st) == [0, 0, 0, 0, 1] and np.isposinf(nll[4])
+    ref = orc.nll_segmented(x1, off[:5], [sets[i] for i in m[:4]], LO, HI)
+    assert np.all(np.abs(nll[:4] - ref) <= 1e-10 * np.abs(ref) + 0.0) and nll[1] == 0.0
+    with pytest.raises(ipa.IpaError):
+        ipa.ipa_nll_eval_categories(dev(torch_, x1), dev(torch_, off), sets, [0, 1, 2, 3, 0], LO, HI)   # index out of range
