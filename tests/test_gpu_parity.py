@@ -677,3 +677,30 @@ def test_categories_with_shared_parameter_sets(ipa, torch_, orc, x1):
     assert np.all(np.abs(nll[:4] - ref) <= 1e-10 * np.abs(ref) + 0.0) and nll[1] == 0.0
     with pytest.raises(ipa.IpaError):
         ipa.ipa_nll_eval_categories(dev(torch_, x1), dev(torch_, off), sets, [0, 1, 2, 3, 0], LO, HI)   # index out of range
+
+
+def test_null_stream_and_error_codes(ipa, torch_, x1):
+    """cuda_stream = NULL (legacy default stream) through the raw C ABI; argument errors on a live device."""
+    import ctypes as C
+    L = ipa.lib()
+    xd = dev(torch_, x1)
+    P = ipa.pack_params(inp.GEN)
+    ws = ipa.workspace(x1.size, 1)
+    out = torch_.empty(1, dtype=torch_.float64, device="cuda")
+    rng = ipa.binding._Range(LO, HI)
+    rc = L.ipa_nll_eval(C.c_void_p(xd.data_ptr()), x1.size, P.ctypes.data_as(C.c_void_p), 1, rng, C.c_void_p(out.data_ptr()),
+                        None, None, C.c_void_p(ws.data_ptr()), ws.numel(), None)
+    assert rc == 0
+    torch_.cuda.synchronize()
+    ref, _, _ = ipa.ipa_nll_eval(xd, inp.GEN, LO, HI)
+    assert out.item() == ref.item()
+    # workspace too small / misaligned, inverted range, K = 0
+    assert L.ipa_nll_eval(C.c_void_p(xd.data_ptr()), x1.size, P.ctypes.data_as(C.c_void_p), 1, rng, C.c_void_p(out.data_ptr()),
+                          None, None, C.c_void_p(ws.data_ptr()), 16, None) == -2
+    assert L.ipa_nll_eval(C.c_void_p(xd.data_ptr()), x1.size, P.ctypes.data_as(C.c_void_p), 1, rng, C.c_void_p(out.data_ptr()),
+                          None, None, C.c_void_p(ws.data_ptr() + 8), ws.numel() - 8, None) == -2
+    assert L.ipa_nll_eval(C.c_void_p(xd.data_ptr()), x1.size, P.ctypes.data_as(C.c_void_p), 1, ipa.binding._Range(HI, LO),
+                          C.c_void_p(out.data_ptr()), None, None, C.c_void_p(ws.data_ptr()), ws.numel(), None) == -1
+    assert L.ipa_nll_eval(C.c_void_p(xd.data_ptr()), x1.size, P.ctypes.data_as(C.c_void_p), 0, rng, C.c_void_p(out.data_ptr()),
+                          None, None, C.c_void_p(ws.data_ptr()), ws.numel(), None) == -1
+    assert L.ipa_strerror(-2).decode().startswith("workspace")
