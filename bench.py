@@ -151,7 +151,7 @@ def other_rows(torch, ipa, x, ws, stream, n):
     # config 2: host minimiser loop, 1e6 events (seed 2), floating (mu, sigma, f, k)
     n2 = min(1_000_000, n)
     x2, _, _ = ipa.ipa_toy_generate([2], inp.GEN, -1.0, -1.0, LO, HI, n2)
-    x2 = ipa.ipa_events_sort(x2)
+    x2 = ipa.ipa_events_prepare(x2, LO, HI)
     ws2 = ipa.workspace(n2, 32)
     th0 = inp.as_array(inp.GEN)
     for name, d in inp.FIT_START_SHIFT.items():
@@ -199,7 +199,7 @@ def other_rows(torch, ipa, x, ws, stream, n):
         ntot = int(off[-1].item())
         sets = inp.toy_param_sets(T)
         ds = t(lambda: ipa.ipa_nll_eval_segmented(xt, off, sets, LO, HI, ws=wst, stream=stream), 10)
-        xs = ipa.ipa_events_sort(xt[:ntot], off)
+        xs = ipa.ipa_events_prepare(xt[:ntot], LO, HI, off)
         dss = t(lambda: ipa.ipa_nll_eval_segmented(xs, off, sets, LO, HI, ws=wst, stream=stream), 10)
         out["config4_toys"] = {"toys": T, "events": ntot, "generate_ms": dg * 1e3, "generate_events_per_s": ntot / dg,
                                "segmented_nll_ms": ds * 1e3, "segmented_nll_sorted_per_toy_ms": dss * 1e3,
@@ -286,12 +286,12 @@ def main():
     stream = torch.cuda.current_stream()
     n = args.events
     P1 = inp.GEN
-    batch9, h = inp.fd_batch(P1)
+    batch9, _ = inp.fd_batch(P1)
 
     # workload: config 3, generated on the device by the method's generator (seed 3 + rank: weak scaling,
     # every rank owns its own n events, no data-path collective)
     x_asis, _, _ = ipa.ipa_toy_generate([3 + rank], P1, -1.0, -1.0, LO, HI, n)
-    x_sorted = ipa.ipa_events_sort(x_asis)          # one-off preparation, outside every timed region
+    x_sorted = ipa.ipa_events_prepare(x_asis, LO, HI)          # one-off preparation, outside every timed region
     x = x_sorted if args.layout == "sorted" else x_asis
     p_core = float(((x_asis >= P1["mu"] - P1["a"] * P1["sigma"]) & (x_asis <= P1["mu"] + P1["a2"] * P1["sigma"]))
                    .double().mean().item())
@@ -302,13 +302,13 @@ def main():
     st9 = torch.empty(9, dtype=torch.int32, device="cuda")
     torch.cuda.synchronize()
 
-    ipa.ipa_set_degree_policy(1)  # general-order path: no half-integer shortcut in the headline (reading D2)
+    POL = 1  # general-order path: no half-integer shortcut in the headline (reading D2)
 
     def step_k1(arr=None):
-        ipa.ipa_nll_eval(x if arr is None else arr, P1, LO, HI, ws=ws, stream=stream, out=out1, status=st1)
+        ipa.ipa_nll_eval(x if arr is None else arr, P1, LO, HI, ws=ws, stream=stream, out=out1, status=st1, policy=POL)
 
     def step_k9(arr=None):
-        ipa.ipa_nll_eval(x if arr is None else arr, batch9, LO, HI, ws=ws, stream=stream, out=out9, status=st9)
+        ipa.ipa_nll_eval(x if arr is None else arr, batch9, LO, HI, ws=ws, stream=stream, out=out9, status=st9, policy=POL)
 
     for _ in range(args.warmup):
         step_k1()
@@ -333,13 +333,13 @@ def main():
                 torch.empty(1, dtype=torch.int32, device="cuda"))
 
     def step_pro():
-        ipa.ipa_norm(P1, LO, HI, ws=ws, stream=stream, out=norm_out)
+        ipa.ipa_norm(P1, LO, HI, ws=ws, stream=stream, out=norm_out, policy=POL)
     for _ in range(3):
         step_pro()
     dt_pro = timed(torch, step_pro, args.steps, stream) / args.steps
     t_step = dt / args.steps
     t_kernel = max(t_step - dt_pro, 1e-9)
-    degree = int(ipa.ipa_core_degree(P1, LO, HI))
+    degree = int(ipa.ipa_core_degree(P1, LO, HI, policy=POL))
 
     extras = {"p_core": p_core, "core_degree": degree, "prologue_ms": dt_pro * 1e3, "nll_kernel_ms": t_kernel * 1e3}
     if not args.no_extras:
@@ -359,24 +359,24 @@ def main():
         dto9 = timed(torch, lambda: step_k9(other), k9steps, stream) / k9steps
         extras[f"k1_layout_{oname}"] = {"ms_per_call": dto * 1e3, "events_per_s": n / dto}
         extras[f"k9_layout_{oname}"] = {"ms_per_call": dto9 * 1e3, "event_sets_per_s": 9 * n / dto9}
-        ipa.ipa_set_degree_policy(0)
+        def step_adaptive():
+            ipa.ipa_nll_eval(x, P1, LO, HI, ws=ws, stream=stream, out=out1, status=st1, policy=0)
         for _ in range(2):
-            step_k1()
-        dta = timed(torch, step_k1, args.steps, stream) / args.steps
+            step_adaptive()
+        dta = timed(torch, step_adaptive, args.steps, stream) / args.steps
         extras["k1_adaptive_degree_half_integer_shortcut"] = {"ms_per_call": dta * 1e3, "events_per_s": n / dta}
 
         def step_p2():
-            ipa.ipa_nll_eval(x, inp.P2, LO, HI, ws=ws, stream=stream, out=out1, status=st1)
+            ipa.ipa_nll_eval(x, inp.P2, LO, HI, ws=ws, stream=stream, out=out1, status=st1, policy=0)
         for _ in range(2):
             step_p2()
         dtp = timed(torch, step_p2, args.steps, stream) / args.steps
         extras["k1_general_shape_P2"] = {"ms_per_call": dtp * 1e3, "events_per_s": n / dtp}
-        ipa.ipa_set_degree_policy(1)
         step_k1()
         # row f1: analytic gradient in one pass, beside the K = 9 finite-difference batch it replaces
         for _ in range(2):
-            ipa.ipa_nll_grad_eval(x, P1, LO, HI, ws=ws, stream=stream)
-        dtg = timed(torch, lambda: ipa.ipa_nll_grad_eval(x, P1, LO, HI, ws=ws, stream=stream), k9steps, stream) / k9steps
+            ipa.ipa_nll_grad_eval(x, P1, LO, HI, ws=ws, stream=stream, policy=POL)
+        dtg = timed(torch, lambda: ipa.ipa_nll_grad_eval(x, P1, LO, HI, ws=ws, stream=stream, policy=POL), k9steps, stream) / k9steps
         extras["f1_analytic_gradient"] = {"ms_per_call": dtg * 1e3, "events_per_s": n / dtg,
                                           "speedup_vs_k9_finite_differences": dt9 / dtg}
         extras.update(other_rows(torch, ipa, x_asis, ws, stream, n))
@@ -396,13 +396,13 @@ def main():
         xh.copy_(x_asis)
         xd = torch.empty(n, dtype=torch.float64, device="cuda")
         torch.cuda.synchronize()
-        ipa.nll_host(xh, P1, LO, HI, x_dev=xd, ws=ws)
+        ipa.nll_host(xh, P1, LO, HI, x_dev=xd, ws=ws, policy=POL)
         e2e_steps = max(2, min(args.steps, 5))
         if dist:
             dist.barrier()
         t0 = time.perf_counter()
         for _ in range(e2e_steps):
-            r = ipa.nll_host(xh, P1, LO, HI, x_dev=xd, ws=ws)
+            r = ipa.nll_host(xh, P1, LO, HI, x_dev=xd, ws=ws, policy=POL)
         torch.cuda.synchronize()
         de = time.perf_counter() - t0
         if dist:

@@ -82,12 +82,17 @@ const char* ipa_last_cuda_error(void);
 /* Library build tag, e.g. "ipanll 0.1 sm_100a". */
 const char* ipa_version(void);
 
-/* Core-approximant degree policy (prologue): 0 = adaptive (the Chebyshev series of
- * log(z^nu K_nu(z)) is cut where its coefficients fall under the fp64 noise floor, so a half-integer
- * order collapses to a very short polynomial); 1 = geometric (at least the a-priori degree for a
- * general order on the same z-interval: no half-integer shortcut; reading D2).  Default 0.
- * Returns the previous policy.  Process-wide; not thread-safe against concurrent calls. */
-int ipa_set_degree_policy(int policy);
+/* Per-call options.  Every entry point that computes per-parameter-set constants takes `const ipa_options* opt_host`
+ * (NULL = all defaults); the struct is read before the call returns.
+ *   degree_policy  core-approximant degree (prologue): 0 = adaptive (default: the Chebyshev
+ *                  series of log(z^nu K_nu(z)) is cut where its coefficients fall under the fp64 noise floor, so a
+ *                  half-integer order collapses to a very short polynomial); 1 = geometric (at least the a-priori
+ *                  degree for a general order on the same z-interval: no half-integer shortcut; reading D2).
+ * Results are bitwise reproducible for fixed options; they differ between the two policies at the 1e-15 level. */
+typedef struct {
+  int32_t degree_policy;
+  int32_t reserved[3]; /* must be 0 */
+} ipa_options;
 
 /* Bytes of workspace needed by any call below for n events, K parameter sets (or T segments / toys:
  * pass the larger of K and T) and nbins histogram bins (0 if unused). */
@@ -98,26 +103,39 @@ size_t ipa_workspace_bytes(int64_t n, int64_t K, int64_t nbins);
  *   norm_bkg_dev[k] = N_B = int_lo^hi exp(k (x - lo)) dx = expm1(k (hi-lo)) / k   (hi-lo at k=0)
  * status_dev[k] as described above (may be NULL).  Invalid sets give NaN. */
 int ipa_norm(const ipa_params* p_host, int K, ipa_range r, double* norm_sig_dev, double* norm_bkg_dev,
-             int32_t* status_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
+             int32_t* status_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream);
 
 /* Introspection of the prologue (step A1e): degree_dev[k] = degree of the core
  * approximant chosen for set k under the current degree policy, -1 for a set evaluated in direct mode
  * (per-event Bessel function), -2 for a set with a domain error.  Used by bench.py to state the
  * algorithmic work of the timed workload. */
-int ipa_core_degree(const ipa_params* p_host, int K, ipa_range r, int32_t* degree_dev, void* ws_dev, size_t ws_bytes,
+int ipa_core_degree(const ipa_params* p_host, int K, ipa_range r, int32_t* degree_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes,
                     void* cuda_stream);
 
 /* The hot path (fused into one pass): NLL of n events for K parameter sets.
  *   x_dev      [n]    event masses, fp64, 8-byte aligned
  *   p_host     [K]    parameter sets
  *   nll_dev    [K]    out: -sum_i log(f S + (1-f) B); +inf for a set with status != 0
- *   logpdf_dev [K*n]  out, optional (NULL to skip): per-event log(f S + (1-f) B), set-major
+ *   logpdf_dev [K*n]  out, optional (NULL to skip): per-event log(f S + (1-f) B), set-major; the row of a set with
+ *                     status != 0 is filled with NaN
  *   status_dev [K]    out, optional
  * K <= IPA_MAX_K per call. */
 #define IPA_MAX_K 32
 int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r,
-                 double* nll_dev, double* logpdf_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
+                 double* nll_dev, double* logpdf_dev, int32_t* status_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes,
                  void* cuda_stream);
+
+/* Finite-difference gradient of the NLL (reading C6; the paper leaves the differences to
+ * Minuit): ONE pass over the events for the K = 2P+1 sets
+ *   set 0 = theta,  sets 2j+1 / 2j+2 = theta with field idx_host[j] replaced by theta[idx] +/- h_host[j]
+ * (each sum computed once, in fp64, on the host), then on the device
+ *   grad_dev[j] = (nll[2j+1] - nll[2j+2]) / (2 h_j).
+ *   theta_host [1]; idx_host [P] field indices 0..10 in the order of ipa_params; h_host [P] > 0; 1 <= P <= 11
+ *   nll_dev [2P+1] out: the NLLs of the batch in that order;  grad_dev [P] out;  status_dev [2P+1] out, optional
+ * A displaced set outside the domain gives +inf / NaN in its entries, as in ipa_nll_eval. */
+int ipa_nll_fd_gradient(const double* x_dev, int64_t n, const ipa_params* theta_host, int P, const int32_t* idx_host,
+                        const double* h_host, ipa_range r, double* nll_dev, double* grad_dev, int32_t* status_dev,
+                        const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream);
 
 /* Extended likelihood (reading D4: the paper's FCN works with yields):
  *   nll_dev[k] = (ns_k + nb_k) - sum_i log( ns_k S(x_i) + nb_k B(x_i) )
@@ -126,7 +144,7 @@ int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K
  * ns_k, nb_k >= 0, ns_k + nb_k > 0, else status 1.  Everything else as ipa_nll_eval. */
 int ipa_nll_eval_extended(const double* x_dev, int64_t n, const ipa_params* p_host, const double* ns_host,
                           const double* nb_host, int K, ipa_range r, double* nll_dev, int32_t* status_dev,
-                          void* ws_dev, size_t ws_bytes, void* cuda_stream);
+                          const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream);
 
 /* NLL and its ANALYTIC gradient with respect to (mu, sigma, f, k) in one pass (the
  * paper mentions analytic gradients through iminuit and generated derivative code, PAPER.md:36, 383,
@@ -137,7 +155,7 @@ int ipa_nll_eval_extended(const double* x_dev, int64_t n, const ipa_params* p_ho
  * Needs 0 < f < 1: a set with f == 0 or f == 1 gets status 4, NLL = +inf and NaN derivatives.  Every
  * set streams the events on its own (the call is meant for one or a few sets).  K <= IPA_MAX_K. */
 int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r,
-                      double* nll_dev, double* grad_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
+                      double* nll_dev, double* grad_dev, int32_t* status_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes,
                       void* cuda_stream);
 
 /* Same likelihood over T segments (toys, categories) of one event array, one parameter set per
@@ -146,7 +164,7 @@ int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, 
  *   p_host      [T]    parameter sets (copied through the workspace by a kernel argument path)
  *   nll_dev     [T]    out */
 int ipa_nll_eval_segmented(const double* x_dev, const int64_t* offsets_dev, int64_t T, const ipa_params* p_host,
-                           ipa_range r, double* nll_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
+                           ipa_range r, double* nll_dev, int32_t* status_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes,
                            void* cuda_stream);
 
 /* Simultaneous categories with SHARED parameter sets (one model, several categories,
@@ -156,7 +174,7 @@ int ipa_nll_eval_segmented(const double* x_dev, const int64_t* offsets_dev, int6
  * ipa_workspace_bytes(n, max(K, T), 0). */
 int ipa_nll_eval_categories(const double* x_dev, const int64_t* offsets_dev, int64_t T, const ipa_params* p_host, int64_t K,
                             const int32_t* set_of_segment_host, ipa_range r, double* nll_dev, int32_t* status_dev,
-                            void* ws_dev, size_t ws_bytes, void* cuda_stream);
+                            const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream);
 
 /* Toy-MC generation on the device (readings D13, D14).
  * Toy t draws Ns ~ Poisson(mean_sig), Nb ~ Poisson(mean_bkg) from seeds_host[t] (Philox-4x32-10
@@ -167,10 +185,13 @@ int ipa_nll_eval_categories(const double* x_dev, const int64_t* offsets_dev, int
  *     events are generated and the component of each event is chosen by u < f.
  *   capacity   size of x_dev in events; if the drawn total exceeds it, offsets are still written,
  *              no event beyond capacity is written and overflow_dev[0] is set to 1.
- *   x_dev      [capacity] out;  offsets_dev [T+1] out;  overflow_dev [1] out (int32) */
+ *   x_dev      [capacity] out;  offsets_dev [T+1] out;  overflow_dev [1] out (int32; bit 0: capacity exceeded,
+ *              bit 1: an accept-reject attempt cap was hit -- cannot happen for a valid shape)
+ *   status_dev [gen_count] out, optional: domain status of every generating set; the events of a toy whose
+ *              generating set is invalid are NaN (offsets are still written) */
 int ipa_toy_generate(const uint64_t* seeds_host, int64_t T, const ipa_params* gen_host, int64_t gen_count,
                      double mean_sig, double mean_bkg, ipa_range r, int64_t capacity, double* x_dev,
-                     int64_t* offsets_dev, int32_t* overflow_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
+                     int64_t* offsets_dev, int32_t* overflow_dev, int32_t* status_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream);
 
 /* Histogram of n events in nbins uniform bins on [lo,hi]:
  * bin = floor((x-lo) nbins/(hi-lo)), x == hi goes to the last bin, events outside are dropped.
@@ -184,11 +205,11 @@ int ipa_hist_fill(const double* x_dev, int64_t n, ipa_range r, int nbins, uint64
  *   ns_host, nb_host, k_host [npoints]; nll_dev [npoints] out. */
 int ipa_binned_nll_scan(const uint64_t* counts_dev, int nbins, ipa_range r, const ipa_params* shape_host,
                         const double* ns_host, const double* nb_host, const double* k_host, int64_t npoints,
-                        double* nll_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
+                        double* nll_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream);
 
 /* Expected histogram nu_b = ns s_b + nb b_b for one point (input of ipa_poisson_hist_toys). */
 int ipa_expected_hist(int nbins, ipa_range r, const ipa_params* shape_host, double ns, double nb, double k,
-                      double* nu_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
+                      double* nu_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream);
 
 /* Gaussian-smeared signal shape on the bin grid ("SM = GaussSmear1(bins_cx, sigma0);
  * sigf_gpu = SM.Smear(sigf_i_gpu)"; kernel, normalisation and edges are not stated -- DESIGN.md reading F3):
@@ -201,7 +222,7 @@ int ipa_expected_hist(int nbins, ipa_range r, const ipa_params* shape_host, doub
  *                      ipa_expected_hist / ipa_binned_nll_scan with a GIVEN signal shape sig_dev [nbins] >= 0
  *                      (normalised to unit sum inside, as PAPER.md:311-312 does) instead of a parameter set;
  *                      a shape whose sum is not positive gives NaN / +inf results */
-int ipa_signal_shape(int nbins, ipa_range r, const ipa_params* shape_host, double* sig_dev, void* ws_dev, size_t ws_bytes,
+int ipa_signal_shape(int nbins, ipa_range r, const ipa_params* shape_host, double* sig_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes,
                      void* cuda_stream);
 int ipa_gauss_smear(const double* in_dev, int nbins, ipa_range r, double sigma0, double* out_dev, void* cuda_stream);
 int ipa_expected_hist_shape(int nbins, ipa_range r, const double* sig_dev, double ns, double nb, double k, double* nu_dev,
@@ -228,18 +249,22 @@ int ipa_cls_count_ge(const double* q_dev, int64_t T, const double* q_obs_dev, in
 int ipa_cls_from_counts(const int64_t* count_sb_dev, int64_t T_sb, const int64_t* count_b_dev, int64_t T_b,
                         double* cl_dev, void* cuda_stream);
 
-/* Optional one-off preparation: ascending sort of the events (whole array, or inside each of T segments
- * when offsets_dev != NULL).  The likelihood does not depend on the order of the events, the data of a
- * fit are constant over the minimiser's calls, and the streaming kernels skip the
- * core polynomial / the tail logarithm for a warp whose 32 x E events all lie in one region: on sorted
- * events nearly every warp is region-uniform.  Unsorted input is always correct.
- * The sum over the sorted array differs from the sum over the original order by rounding only (reading
- * E4).  Radix sort by the toolkit's CUB primitive (a data-layout step, not part of the method); NaN
- * events sort last.  x_out_dev [n] must not alias x_in_dev; ws_dev of ipa_sort_workspace_bytes(n, T)
- * bytes (T = 0 for an unsegmented sort); segmented sorts need n < 2^31. */
-size_t ipa_sort_workspace_bytes(int64_t n, int64_t T);
-int ipa_events_sort(const double* x_in_dev, int64_t n, const int64_t* offsets_dev, int64_t T, double* x_out_dev,
-                    void* ws_dev, size_t ws_bytes, void* cuda_stream);
+/* Optional one-off preparation of the data layout: a STABLE counting sort of the events on a coarse bin index,
+ *   bin(x) = clamp(floor((x - lo) IPA_PREPARE_BINS / (hi - lo)), 0, IPA_PREPARE_BINS - 1),  NaN -> last bin
+ * (whole array, or inside each of T segments when offsets_dev != NULL).  The likelihood does not depend on the
+ * order of the events, the data of a fit are constant over the minimiser's calls, and the
+ * streaming kernels skip the core polynomial / the tail logarithm for a warp whose 32 x E events all lie in one
+ * region: on events grouped by bin nearly every warp is region-uniform, for every parameter set of the fit (the
+ * bins do not depend on the joins).  Unprepared input is always correct.  The output is a permutation of the
+ * input and a pure function of it (original order inside a bin), so results computed from it are bitwise
+ * reproducible; the sum over the prepared array differs from the sum over the original order by rounding only
+ * (reading E4).  Own kernels (histogram, two scans, scatter): csrc/ipa_prepare.cuh.
+ *   x_out_dev [n] must not alias x_in_dev;  n < 2^32;  ws_dev of ipa_prepare_workspace_bytes(n, T) bytes (T = 0
+ *   for an unsegmented array);  r = the fit range the bins span. */
+#define IPA_PREPARE_BINS 2048
+size_t ipa_prepare_workspace_bytes(int64_t n, int64_t T);
+int ipa_events_prepare(const double* x_in_dev, int64_t n, const int64_t* offsets_dev, int64_t T, ipa_range r,
+                       double* x_out_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
 
 /* Measurement aid (not on the hot path): runs `iters` dependent DFMA per thread in 8 independent
  * chains on a full grid, for the FP64 roofline denominator.  out_dev [1]. */

@@ -56,10 +56,12 @@ def fd_batch(theta, floated=FLOATED, steps=FD_STEPS):
     return batch, h
 
 
-def fd_gradient(nll_batch, h):
-    """g_j = (NLL(theta + h_j e_j) - NLL(theta - h_j e_j)) / (2 h_j) from a 2P+1 batch (row G)."""
-    nll_batch = np.asarray(nll_batch, dtype=np.float64)
-    return (nll_batch[1::2] - nll_batch[2::2]) / (2.0 * h)
+def fd_spec(floated=FLOATED, steps=FD_STEPS):
+    """(idx[P] int32 field indices, h[P] steps) of the central-difference gradient (reading C6): the arguments of
+    oracle.fd_gradient and ipa_nll_fd_gradient, which both build the batch of fd_batch() and take the differences
+    themselves (row G is method code: it lives on each side, not here)."""
+    return (np.array([IDX[name] for name in floated], dtype=np.int32),
+            np.array([steps[name] for name in floated], dtype=np.float64))
 
 
 def standin_masses(seed, n, f=0.3, mu=5280.0, sigma=15.0, k=-0.002, lo=LO, hi=HI):

@@ -32,10 +32,12 @@ def lib():
         L.orc_logpdf.restype = i32; L.orc_logpdf.argtypes = [vp, i64, vp, d, d, vp]
         L.orc_signal_pdf.restype = d; L.orc_signal_pdf.argtypes = [vp, d, d, d]
         L.orc_nll.restype = i32; L.orc_nll.argtypes = [vp, i64, vp, i32, d, d, vp, i32]
+        L.orc_fd_gradient.restype = i32; L.orc_fd_gradient.argtypes = [vp, i64, vp, i32, vp, vp, d, d, i32, vp, vp]
         L.orc_nll_segmented.restype = i32; L.orc_nll_segmented.argtypes = [vp, vp, i64, vp, d, d, vp]
         L.orc_philox4x32_10.restype = None; L.orc_philox4x32_10.argtypes = [vp, vp, vp]
         L.orc_uniforms2.restype = None; L.orc_uniforms2.argtypes = [u64, u64, u32, u32, vp]
         L.orc_poisson.restype = i64; L.orc_poisson.argtypes = [u64, u64, u32, d]
+        L.orc_poisson_array.restype = None; L.orc_poisson_array.argtypes = [u64, u64, i64, u32, d, vp, vp]
         L.orc_generate_mixture.restype = i32; L.orc_generate_mixture.argtypes = [u64, i64, vp, d, d, vp]
         L.orc_toy_generate.restype = i32
         L.orc_toy_generate.argtypes = [vp, i64, vp, i32, d, d, d, d, i64, vp, vp]
@@ -142,6 +144,22 @@ def nll(x, p, lo, hi, nthreads=1):
     return out
 
 
+def fd_gradient(x, theta, idx, h, lo, hi, nthreads=1):
+    """Central-difference gradient (row G, reading C6) over the parameter fields idx[P] with steps h[P].
+    -> (nll[2P+1] of the batch theta, theta +/- h_j e_j, grad[P])."""
+    x = np.ascontiguousarray(x, dtype=np.float64)
+    P = pack_params(theta)
+    assert P.shape[0] == 1
+    idx = np.ascontiguousarray(idx, dtype=np.int32)
+    h = np.ascontiguousarray(h, dtype=np.float64)
+    nll = np.empty(2 * idx.size + 1)
+    g = np.empty(idx.size)
+    st = lib().orc_fd_gradient(_p(x), x.size, _p(P), idx.size, _p(idx), _p(h), float(lo), float(hi), int(nthreads),
+                               _p(nll), _p(g))
+    assert st == 0, st
+    return nll, g
+
+
 def nll_segmented(x, offsets, p, lo, hi):
     x = np.ascontiguousarray(x, dtype=np.float64)
     offsets = np.ascontiguousarray(offsets, dtype=np.int64)
@@ -169,6 +187,14 @@ def uniforms2(seed, slot, attempt, stream):
 
 def poisson(seed, slot, stream, mean):
     return lib().orc_poisson(int(seed), int(slot), int(stream), float(mean))
+
+
+def poisson_array(seed, slot0, n, stream, mean, diagnostics=False):
+    """n draws at consecutive slots (same values as n calls of poisson); with diagnostics also (attempts[n], exit[n])."""
+    out = np.empty(int(n), dtype=np.int64)
+    diag = np.empty((int(n), 2), dtype=np.int32) if diagnostics else None
+    lib().orc_poisson_array(int(seed), int(slot0), int(n), int(stream), float(mean), _p(out), _p(diag) if diagnostics else None)
+    return (out, diag[:, 0], diag[:, 1]) if diagnostics else out
 
 
 def generate_mixture(seed, n, p, lo, hi):

@@ -532,7 +532,10 @@ static void uniforms2(uint64_t seed, uint64_t slot, uint32_t attempt, uint32_t s
 
 /* Poisson(mean) on Philox uniforms (reading D14): sequential-search inversion for mean<10,
  * Hoermann's transformed rejection PTRS (Insurance: Math. & Econ. 12 (1993) 39) otherwise. */
-static int64_t poisson_draw(uint64_t seed, uint64_t slot, uint32_t stream, double mean) {
+/* diag (optional, tests only): diag[0] = attempts used, diag[1] = exit taken (0 inversion, 1 the quick
+ * acceptance of the squeeze, 2 the full comparison with the probability function); no effect on the draw. */
+static int64_t poisson_draw(uint64_t seed, uint64_t slot, uint32_t stream, double mean, int32_t* diag = nullptr) {
+  if (diag) { diag[0] = 0; diag[1] = 0; }
   if (!(mean > 0)) return 0;
   if (mean < 10) {
     double u, v;
@@ -554,8 +557,10 @@ static int64_t poisson_draw(uint64_t seed, uint64_t slot, uint32_t stream, doubl
     U -= 0.5;
     const double us = 0.5 - std::fabs(U);
     const double kf = std::floor((2.0 * a / us + b) * U + mean + 0.43);
+    if (diag) { diag[0] = (int32_t)attempt + 1; diag[1] = 1; }
     if (us >= 0.07 && V <= vr) return (int64_t)kf;
     if (kf < 0 || (us < 0.013 && V > us)) continue;
+    if (diag) diag[1] = 2;
     if (std::log(V) + std::log(inv_alpha) - std::log(a / (us * us) + b) <= -mean + kf * lmean - std::lgamma(kf + 1.0))
       return (int64_t)kf;
   }
@@ -660,6 +665,25 @@ int orc_nll(const double* x, int64_t n, const orc_params* p, int K, double lo, d
   return 0;
 }
 
+/* Finite-difference gradient (reading C6): central differences over P floated parameters.
+ * Set 0 = theta, sets 2j+1 / 2j+2 = theta with field idx[j] replaced by theta[idx[j]] +/- h[j] (each sum computed
+ * once, in fp64), g_j = (NLL(theta + h_j e_j) - NLL(theta - h_j e_j)) / (2 h_j).  nll [2P+1] receives the NLLs of
+ * the batch in that order, grad [P] the differences.  nthreads as in orc_nll. */
+int orc_fd_gradient(const double* x, int64_t n, const orc_params* theta, int P, const int32_t* idx, const double* h,
+                    double lo, double hi, int nthreads, double* nll, double* grad) {
+  if (P < 1 || P > 11) return -1;
+  std::vector<orc_params> batch((size_t)(2 * P + 1), *theta);
+  for (int j = 0; j < P; ++j) {
+    if (idx[j] < 0 || idx[j] > 10) return -1;
+    const double base = (&theta->mu)[idx[j]];
+    (&batch[(size_t)(2 * j + 1)].mu)[idx[j]] = base + h[j];
+    (&batch[(size_t)(2 * j + 2)].mu)[idx[j]] = base - h[j];
+  }
+  orc_nll(x, n, batch.data(), 2 * P + 1, lo, hi, nll, nthreads);
+  for (int j = 0; j < P; ++j) grad[j] = (nll[2 * j + 1] - nll[2 * j + 2]) / (2.0 * h[j]);
+  return 0;
+}
+
 /* NLL per segment (toy), one parameter set per segment: offsets[T+1] */
 int orc_nll_segmented(const double* x, const int64_t* offsets, int64_t T, const orc_params* p, double lo, double hi,
                       double* nll) {
@@ -670,6 +694,10 @@ int orc_nll_segmented(const double* x, const int64_t* offsets, int64_t T, const 
 void orc_philox4x32_10(const uint32_t* key, const uint32_t* ctr, uint32_t* out) { philox4x32_10(key, ctr, out); }
 void orc_uniforms2(uint64_t seed, uint64_t slot, uint32_t attempt, uint32_t stream, double* u) { uniforms2(seed, slot, attempt, stream, u, u + 1); }
 int64_t orc_poisson(uint64_t seed, uint64_t slot, uint32_t stream, double mean) { return poisson_draw(seed, slot, stream, mean); }
+/* n draws at slots slot0 .. slot0+n-1 (the same draws as n calls of orc_poisson); diag [2 n] optional: attempts and exit per draw */
+void orc_poisson_array(uint64_t seed, uint64_t slot0, int64_t n, uint32_t stream, double mean, int64_t* out, int32_t* diag) {
+  for (int64_t i = 0; i < n; ++i) out[i] = poisson_draw(seed, slot0 + (uint64_t)i, stream, mean, diag ? diag + 2 * i : nullptr);
+}
 
 /* configs 1-3: n events, component chosen per event by u<f (reading D13) */
 int orc_generate_mixture(uint64_t seed, int64_t n, const orc_params* p, double lo, double hi, double* x) {

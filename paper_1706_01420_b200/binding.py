@@ -3,6 +3,7 @@ and streams (plumbing only).  Each wrapper marshals arguments, sizes the workspa
 return code; no arithmetic of the method happens here.
 """
 import ctypes as C
+import functools
 import os
 
 import numpy as np
@@ -12,12 +13,12 @@ from . import build as _build
 
 __all__ = [
     "PARAM_FIELDS", "NPAR", "IPA_MAX_K", "IpaError", "lib", "library_path", "pack_params", "workspace",
-    "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes", "ipa_norm", "ipa_core_degree", "ipa_nll_grad_eval",
+    "ipa_version", "ipa_workspace_bytes", "ipa_norm", "ipa_core_degree", "ipa_nll_grad_eval", "ipa_nll_fd_gradient",
     "ipa_nll_eval_extended", "ipa_nll_eval_categories", "ipa_nll_eval",
     "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill", "ipa_binned_nll_scan", "ipa_expected_hist",
     "ipa_poisson_hist_toys", "ipa_signal_shape", "ipa_gauss_smear", "ipa_expected_hist_shape", "ipa_binned_nll_scan_shape",
-    "ipa_cls_teststat", "ipa_cls_count_ge", "ipa_cls_from_counts", "ipa_events_sort",
-    "ipa_sort_workspace_bytes", "ipa_fp64_peak_probe", "nll_host", "EXPORTS",
+    "ipa_cls_teststat", "ipa_cls_count_ge", "ipa_cls_from_counts", "ipa_events_prepare",
+    "ipa_prepare_workspace_bytes", "ipa_fp64_peak_probe", "nll_host", "EXPORTS",
 ]
 
 PARAM_FIELDS = ("mu", "sigma", "lambda", "zeta", "beta", "a", "n", "a2", "n2", "f", "k")
@@ -26,11 +27,11 @@ IPA_MAX_K = 32
 
 # every symbol include/ipanll.h declares
 EXPORTS = (
-    "ipa_strerror", "ipa_last_cuda_error", "ipa_version", "ipa_set_degree_policy", "ipa_workspace_bytes",
-    "ipa_norm", "ipa_core_degree", "ipa_nll_eval", "ipa_nll_eval_extended", "ipa_nll_grad_eval", "ipa_nll_eval_segmented", "ipa_nll_eval_categories", "ipa_toy_generate", "ipa_hist_fill",
+    "ipa_strerror", "ipa_last_cuda_error", "ipa_version", "ipa_workspace_bytes",
+    "ipa_norm", "ipa_core_degree", "ipa_nll_eval", "ipa_nll_fd_gradient", "ipa_nll_eval_extended", "ipa_nll_grad_eval", "ipa_nll_eval_segmented", "ipa_nll_eval_categories", "ipa_toy_generate", "ipa_hist_fill",
     "ipa_binned_nll_scan", "ipa_expected_hist", "ipa_poisson_hist_toys", "ipa_signal_shape", "ipa_gauss_smear",
     "ipa_expected_hist_shape", "ipa_binned_nll_scan_shape", "ipa_cls_teststat", "ipa_cls_count_ge",
-    "ipa_cls_from_counts", "ipa_sort_workspace_bytes", "ipa_events_sort",
+    "ipa_cls_from_counts", "ipa_prepare_workspace_bytes", "ipa_events_prepare",
     "ipa_fp64_peak_probe",
 )
 
@@ -41,6 +42,19 @@ class IpaError(RuntimeError):
 
 class _Range(C.Structure):
     _fields_ = [("lo", C.c_double), ("hi", C.c_double)]
+
+
+class _Options(C.Structure):
+    _fields_ = [("degree_policy", C.c_int32), ("reserved", C.c_int32 * 3)]
+
+
+def _opt(policy):
+    """policy None -> NULL options (library defaults), else an ipa_options with that degree policy."""
+    if policy is None:
+        return None
+    o = _Options()
+    o.degree_policy = int(policy)
+    return C.byref(o)
 
 
 _lib = None
@@ -61,26 +75,28 @@ def lib():
     L.ipa_strerror.restype = C.c_char_p; L.ipa_strerror.argtypes = [i32]
     L.ipa_last_cuda_error.restype = C.c_char_p; L.ipa_last_cuda_error.argtypes = []
     L.ipa_version.restype = C.c_char_p; L.ipa_version.argtypes = []
-    L.ipa_set_degree_policy.restype = i32; L.ipa_set_degree_policy.argtypes = [i32]
     L.ipa_workspace_bytes.restype = sz; L.ipa_workspace_bytes.argtypes = [i64, i64, i64]
-    L.ipa_norm.restype = i32; L.ipa_norm.argtypes = [vp, i32, _Range, vp, vp, vp, vp, sz, vp]
-    L.ipa_core_degree.restype = i32; L.ipa_core_degree.argtypes = [vp, i32, _Range, vp, vp, sz, vp]
-    L.ipa_nll_eval.restype = i32; L.ipa_nll_eval.argtypes = [vp, i64, vp, i32, _Range, vp, vp, vp, vp, sz, vp]
+    op = vp  # const ipa_options* (NULL or byref(_Options))
+    L.ipa_norm.restype = i32; L.ipa_norm.argtypes = [vp, i32, _Range, vp, vp, vp, op, vp, sz, vp]
+    L.ipa_core_degree.restype = i32; L.ipa_core_degree.argtypes = [vp, i32, _Range, vp, op, vp, sz, vp]
+    L.ipa_nll_eval.restype = i32; L.ipa_nll_eval.argtypes = [vp, i64, vp, i32, _Range, vp, vp, vp, op, vp, sz, vp]
+    L.ipa_nll_fd_gradient.restype = i32
+    L.ipa_nll_fd_gradient.argtypes = [vp, i64, vp, i32, vp, vp, _Range, vp, vp, vp, op, vp, sz, vp]
     L.ipa_nll_eval_extended.restype = i32
-    L.ipa_nll_eval_extended.argtypes = [vp, i64, vp, vp, vp, i32, _Range, vp, vp, vp, sz, vp]
-    L.ipa_nll_grad_eval.restype = i32; L.ipa_nll_grad_eval.argtypes = [vp, i64, vp, i32, _Range, vp, vp, vp, vp, sz, vp]
+    L.ipa_nll_eval_extended.argtypes = [vp, i64, vp, vp, vp, i32, _Range, vp, vp, op, vp, sz, vp]
+    L.ipa_nll_grad_eval.restype = i32; L.ipa_nll_grad_eval.argtypes = [vp, i64, vp, i32, _Range, vp, vp, vp, op, vp, sz, vp]
     L.ipa_nll_eval_segmented.restype = i32
-    L.ipa_nll_eval_segmented.argtypes = [vp, vp, i64, vp, _Range, vp, vp, vp, sz, vp]
+    L.ipa_nll_eval_segmented.argtypes = [vp, vp, i64, vp, _Range, vp, vp, op, vp, sz, vp]
     L.ipa_nll_eval_categories.restype = i32
-    L.ipa_nll_eval_categories.argtypes = [vp, vp, i64, vp, i64, vp, _Range, vp, vp, vp, sz, vp]
+    L.ipa_nll_eval_categories.argtypes = [vp, vp, i64, vp, i64, vp, _Range, vp, vp, op, vp, sz, vp]
     L.ipa_toy_generate.restype = i32
-    L.ipa_toy_generate.argtypes = [vp, i64, vp, i64, d, d, _Range, i64, vp, vp, vp, vp, sz, vp]
+    L.ipa_toy_generate.argtypes = [vp, i64, vp, i64, d, d, _Range, i64, vp, vp, vp, vp, op, vp, sz, vp]
     L.ipa_hist_fill.restype = i32; L.ipa_hist_fill.argtypes = [vp, i64, _Range, i32, vp, vp]
     L.ipa_binned_nll_scan.restype = i32
-    L.ipa_binned_nll_scan.argtypes = [vp, i32, _Range, vp, vp, vp, vp, i64, vp, vp, sz, vp]
-    L.ipa_expected_hist.restype = i32; L.ipa_expected_hist.argtypes = [i32, _Range, vp, d, d, d, vp, vp, sz, vp]
+    L.ipa_binned_nll_scan.argtypes = [vp, i32, _Range, vp, vp, vp, vp, i64, vp, op, vp, sz, vp]
+    L.ipa_expected_hist.restype = i32; L.ipa_expected_hist.argtypes = [i32, _Range, vp, d, d, d, vp, op, vp, sz, vp]
     L.ipa_poisson_hist_toys.restype = i32; L.ipa_poisson_hist_toys.argtypes = [vp, i32, vp, i64, vp, vp, sz, vp]
-    L.ipa_signal_shape.restype = i32; L.ipa_signal_shape.argtypes = [i32, _Range, vp, vp, vp, sz, vp]
+    L.ipa_signal_shape.restype = i32; L.ipa_signal_shape.argtypes = [i32, _Range, vp, vp, op, vp, sz, vp]
     L.ipa_gauss_smear.restype = i32; L.ipa_gauss_smear.argtypes = [vp, i32, _Range, d, vp, vp]
     L.ipa_expected_hist_shape.restype = i32; L.ipa_expected_hist_shape.argtypes = [i32, _Range, vp, d, d, d, vp, vp, sz, vp]
     L.ipa_binned_nll_scan_shape.restype = i32
@@ -88,8 +104,8 @@ def lib():
     L.ipa_cls_teststat.restype = i32; L.ipa_cls_teststat.argtypes = [vp, i32, i64, i32, vp, vp, vp, vp, sz, vp]
     L.ipa_cls_count_ge.restype = i32; L.ipa_cls_count_ge.argtypes = [vp, i64, vp, vp, vp]
     L.ipa_cls_from_counts.restype = i32; L.ipa_cls_from_counts.argtypes = [vp, i64, vp, i64, vp, vp]
-    L.ipa_sort_workspace_bytes.restype = sz; L.ipa_sort_workspace_bytes.argtypes = [i64, i64]
-    L.ipa_events_sort.restype = i32; L.ipa_events_sort.argtypes = [vp, i64, vp, i64, vp, vp, sz, vp]
+    L.ipa_prepare_workspace_bytes.restype = sz; L.ipa_prepare_workspace_bytes.argtypes = [i64, i64]
+    L.ipa_events_prepare.restype = i32; L.ipa_events_prepare.argtypes = [vp, i64, vp, i64, _Range, vp, vp, sz, vp]
     L.ipa_fp64_peak_probe.restype = i32; L.ipa_fp64_peak_probe.argtypes = [i64, vp, vp]
     _lib = L
     return L
@@ -106,6 +122,20 @@ def _check(rc):
 def _need_cuda():
     if not torch.cuda.is_available():
         raise IpaError("libipanll needs a CUDA device (sm_100a); there is no CPU fallback")
+
+
+def _alloc_on_stream(fn):
+    """Run a wrapper under `with torch.cuda.stream(stream)` when a stream is given, so that the tensors it allocates
+    (workspace, outputs) belong to the stream the kernels are enqueued on: the caching allocator then cannot hand
+    their memory to another stream while that work is pending."""
+    @functools.wraps(fn)
+    def wrapped(*args, **kwargs):
+        st = kwargs.get("stream")
+        if st is None or not torch.cuda.is_available():
+            return fn(*args, **kwargs)
+        with torch.cuda.stream(st):
+            return fn(*args, **kwargs)
+    return wrapped
 
 
 def _stream(stream):
@@ -145,10 +175,6 @@ def ipa_version():
     return lib().ipa_version().decode()
 
 
-def ipa_set_degree_policy(policy):
-    return lib().ipa_set_degree_policy(int(policy))
-
-
 def ipa_workspace_bytes(n, K, nbins=0):
     return int(lib().ipa_workspace_bytes(int(n), int(K), int(nbins)))
 
@@ -165,7 +191,8 @@ def _ws(ws, n, K, nbins=0):
     return ws
 
 
-def ipa_norm(params, lo, hi, ws=None, stream=None, out=None):
+@_alloc_on_stream
+def ipa_norm(params, lo, hi, ws=None, stream=None, out=None, policy=None):
     """-> (norm_sig[K], norm_bkg[K], status[K]) device tensors (out = the same triple, preallocated)."""
     _need_cuda()
     P = pack_params(params)
@@ -177,24 +204,26 @@ def ipa_norm(params, lo, hi, ws=None, stream=None, out=None):
         ns = torch.empty(K, dtype=torch.float64, device="cuda")
         nb = torch.empty(K, dtype=torch.float64, device="cuda")
         st = torch.empty(K, dtype=torch.int32, device="cuda")
-    _check(lib().ipa_norm(_hptr(P), K, _Range(lo, hi), _dptr(ns), _dptr(nb), _dptr(st), _dptr(ws), ws.numel(),
+    _check(lib().ipa_norm(_hptr(P), K, _Range(lo, hi), _dptr(ns), _dptr(nb), _dptr(st), _opt(policy), _dptr(ws), ws.numel(),
                           _stream(stream)))
     return ns, nb, st
 
 
-def ipa_core_degree(params, lo, hi, ws=None, stream=None):
+@_alloc_on_stream
+def ipa_core_degree(params, lo, hi, ws=None, stream=None, policy=None):
     """Degree of the core approximant per set (-1 direct mode, -2 domain error); int for a single set."""
     _need_cuda()
     P = pack_params(params)
     K = P.shape[0]
     ws = _ws(ws, 0, K)
     out = torch.empty(K, dtype=torch.int32, device="cuda")
-    _check(lib().ipa_core_degree(_hptr(P), K, _Range(lo, hi), _dptr(out), _dptr(ws), ws.numel(), _stream(stream)))
+    _check(lib().ipa_core_degree(_hptr(P), K, _Range(lo, hi), _dptr(out), _opt(policy), _dptr(ws), ws.numel(), _stream(stream)))
     r = out.cpu().numpy()
     return int(r[0]) if K == 1 else r
 
 
-def ipa_nll_eval(x, params, lo, hi, want_logpdf=False, ws=None, stream=None, out=None, status=None):
+@_alloc_on_stream
+def ipa_nll_eval(x, params, lo, hi, want_logpdf=False, ws=None, stream=None, out=None, status=None, policy=None):
     """NLL of the events in device tensor x (fp64) for K parameter sets.
 
     -> (nll[K], logpdf[K,n] or None, status[K]) device tensors; nothing is synchronised.
@@ -208,11 +237,34 @@ def ipa_nll_eval(x, params, lo, hi, want_logpdf=False, ws=None, stream=None, out
     st = status if status is not None else torch.empty(K, dtype=torch.int32, device="cuda")
     lp = torch.empty((K, n), dtype=torch.float64, device="cuda") if want_logpdf else None
     _check(lib().ipa_nll_eval(_dptr(x, torch.float64) if n else None, n, _hptr(P), K, _Range(lo, hi), _dptr(nll),
-                              _dptr(lp), _dptr(st), _dptr(ws), ws.numel(), _stream(stream)))
+                              _dptr(lp), _dptr(st), _opt(policy), _dptr(ws), ws.numel(), _stream(stream)))
     return nll, lp, st
 
 
-def ipa_nll_eval_extended(x, params, ns, nb, lo, hi, ws=None, stream=None):
+@_alloc_on_stream
+def ipa_nll_fd_gradient(x, theta, idx, h, lo, hi, ws=None, stream=None, policy=None):
+    """Central-difference gradient from ONE K = 2P+1 pass (row G, reading C6): idx[P] parameter-field indices, h[P] steps.
+    -> (nll[2P+1], grad[P], status[2P+1]) device tensors."""
+    _need_cuda()
+    P = pack_params(theta)
+    assert P.shape[0] == 1
+    idx = np.ascontiguousarray(idx, dtype=np.int32).ravel()
+    h = np.ascontiguousarray(h, dtype=np.float64).ravel()
+    assert idx.size == h.size
+    n = x.numel()
+    K = 2 * idx.size + 1
+    ws = _ws(ws, n, K)
+    nll = torch.empty(K, dtype=torch.float64, device="cuda")
+    grad = torch.empty(idx.size, dtype=torch.float64, device="cuda")
+    st = torch.empty(K, dtype=torch.int32, device="cuda")
+    _check(lib().ipa_nll_fd_gradient(_dptr(x, torch.float64) if n else None, n, _hptr(P), idx.size, _hptr(idx), _hptr(h),
+                                     _Range(lo, hi), _dptr(nll), _dptr(grad), _dptr(st), _opt(policy), _dptr(ws), ws.numel(),
+                                     _stream(stream)))
+    return nll, grad, st
+
+
+@_alloc_on_stream
+def ipa_nll_eval_extended(x, params, ns, nb, lo, hi, ws=None, stream=None, policy=None):
     """Extended -log L = (ns+nb) - sum log(ns S + nb B) for K (shape, ns, nb) triples -> (nll[K], status[K])."""
     _need_cuda()
     P = pack_params(params)
@@ -224,11 +276,12 @@ def ipa_nll_eval_extended(x, params, ns, nb, lo, hi, ws=None, stream=None):
     nll = torch.empty(K, dtype=torch.float64, device="cuda")
     st = torch.empty(K, dtype=torch.int32, device="cuda")
     _check(lib().ipa_nll_eval_extended(_dptr(x, torch.float64) if n else None, n, _hptr(P), _hptr(ns), _hptr(nb), K,
-                                       _Range(lo, hi), _dptr(nll), _dptr(st), _dptr(ws), ws.numel(), _stream(stream)))
+                                       _Range(lo, hi), _dptr(nll), _dptr(st), _opt(policy), _dptr(ws), ws.numel(), _stream(stream)))
     return nll, st
 
 
-def ipa_nll_grad_eval(x, params, lo, hi, ws=None, stream=None):
+@_alloc_on_stream
+def ipa_nll_grad_eval(x, params, lo, hi, ws=None, stream=None, policy=None):
     """NLL and analytic gradient w.r.t. (mu, sigma, f, k): -> (nll[K], grad[K, 4], status[K]) device tensors."""
     _need_cuda()
     P = pack_params(params)
@@ -239,11 +292,12 @@ def ipa_nll_grad_eval(x, params, lo, hi, ws=None, stream=None):
     grad = torch.empty((K, 4), dtype=torch.float64, device="cuda")
     st = torch.empty(K, dtype=torch.int32, device="cuda")
     _check(lib().ipa_nll_grad_eval(_dptr(x, torch.float64) if n else None, n, _hptr(P), K, _Range(lo, hi), _dptr(nll),
-                                   _dptr(grad), _dptr(st), _dptr(ws), ws.numel(), _stream(stream)))
+                                   _dptr(grad), _dptr(st), _opt(policy), _dptr(ws), ws.numel(), _stream(stream)))
     return nll, grad, st
 
 
-def ipa_nll_eval_segmented(x, offsets, params, lo, hi, ws=None, stream=None):
+@_alloc_on_stream
+def ipa_nll_eval_segmented(x, offsets, params, lo, hi, ws=None, stream=None, policy=None):
     """-> (nll[T], status[T]); offsets is an int64 device tensor [T+1]."""
     _need_cuda()
     P = pack_params(params)
@@ -253,11 +307,12 @@ def ipa_nll_eval_segmented(x, offsets, params, lo, hi, ws=None, stream=None):
     nll = torch.empty(T, dtype=torch.float64, device="cuda")
     st = torch.empty(T, dtype=torch.int32, device="cuda")
     _check(lib().ipa_nll_eval_segmented(_dptr(x, torch.float64), _dptr(offsets, torch.int64), T, _hptr(P),
-                                        _Range(lo, hi), _dptr(nll), _dptr(st), _dptr(ws), ws.numel(), _stream(stream)))
+                                        _Range(lo, hi), _dptr(nll), _dptr(st), _opt(policy), _dptr(ws), ws.numel(), _stream(stream)))
     return nll, st
 
 
-def ipa_nll_eval_categories(x, offsets, params, set_of_segment, lo, hi, ws=None, stream=None):
+@_alloc_on_stream
+def ipa_nll_eval_categories(x, offsets, params, set_of_segment, lo, hi, ws=None, stream=None, policy=None):
     """Segments (categories) sharing parameter sets: segment t uses params[set_of_segment[t]] -> (nll[T], status[T])."""
     _need_cuda()
     P = pack_params(params)
@@ -268,15 +323,18 @@ def ipa_nll_eval_categories(x, offsets, params, set_of_segment, lo, hi, ws=None,
     nll = torch.empty(T, dtype=torch.float64, device="cuda")
     st = torch.empty(T, dtype=torch.int32, device="cuda")
     _check(lib().ipa_nll_eval_categories(_dptr(x, torch.float64), _dptr(offsets, torch.int64), T, _hptr(P), P.shape[0],
-                                         _hptr(m), _Range(lo, hi), _dptr(nll), _dptr(st), _dptr(ws), ws.numel(),
+                                         _hptr(m), _Range(lo, hi), _dptr(nll), _dptr(st), _opt(policy), _dptr(ws), ws.numel(),
                                          _stream(stream)))
     return nll, st
 
 
-def ipa_toy_generate(seeds, gen, mean_sig, mean_bkg, lo, hi, capacity, ws=None, stream=None, x=None):
+@_alloc_on_stream
+def ipa_toy_generate(seeds, gen, mean_sig, mean_bkg, lo, hi, capacity, ws=None, stream=None, x=None, policy=None,
+                     status=None):
     """Toy generation.  mean_sig < 0 selects mixture mode (one toy of exactly `capacity` events).
 
-    -> (x[capacity], offsets[T+1] int64, overflow[1] int32) device tensors."""
+    -> (x[capacity], offsets[T+1] int64, overflow[1] int32) device tensors; `status` (int32 [gen_count], optional)
+    receives the domain status of the generating sets."""
     _need_cuda()
     seeds = np.ascontiguousarray(seeds, dtype=np.uint64).ravel()
     T = seeds.size
@@ -288,10 +346,11 @@ def ipa_toy_generate(seeds, gen, mean_sig, mean_bkg, lo, hi, capacity, ws=None, 
     ovf = torch.zeros(1, dtype=torch.int32, device="cuda")
     _check(lib().ipa_toy_generate(_hptr(seeds), T, _hptr(P), P.shape[0], float(mean_sig), float(mean_bkg),
                                   _Range(lo, hi), int(capacity), _dptr(x) if capacity else None, _dptr(off), _dptr(ovf),
-                                  _dptr(ws), ws.numel(), _stream(stream)))
+                                  _dptr(status, torch.int32), _opt(policy), _dptr(ws), ws.numel(), _stream(stream)))
     return x, off, ovf
 
 
+@_alloc_on_stream
 def ipa_hist_fill(x, lo, hi, nbins, stream=None):
     _need_cuda()
     counts = torch.empty(int(nbins), dtype=torch.int64, device="cuda")  # uint64 payload
@@ -301,7 +360,8 @@ def ipa_hist_fill(x, lo, hi, nbins, stream=None):
     return counts
 
 
-def ipa_binned_nll_scan(counts, lo, hi, shape, ns, nb, k, ws=None, stream=None):
+@_alloc_on_stream
+def ipa_binned_nll_scan(counts, lo, hi, shape, ns, nb, k, ws=None, stream=None, policy=None):
     _need_cuda()
     P = pack_params(shape)
     ns = np.ascontiguousarray(ns, dtype=np.float64); nb = np.ascontiguousarray(nb, dtype=np.float64)
@@ -310,20 +370,22 @@ def ipa_binned_nll_scan(counts, lo, hi, shape, ns, nb, k, ws=None, stream=None):
     ws = _ws(ws, 0, npts, nbins)
     out = torch.empty(npts, dtype=torch.float64, device="cuda")
     _check(lib().ipa_binned_nll_scan(_dptr(counts, torch.int64), nbins, _Range(lo, hi), _hptr(P), _hptr(ns), _hptr(nb),
-                                     _hptr(k), npts, _dptr(out), _dptr(ws), ws.numel(), _stream(stream)))
+                                     _hptr(k), npts, _dptr(out), _opt(policy), _dptr(ws), ws.numel(), _stream(stream)))
     return out
 
 
-def ipa_expected_hist(nbins, lo, hi, shape, ns, nb, k, ws=None, stream=None):
+@_alloc_on_stream
+def ipa_expected_hist(nbins, lo, hi, shape, ns, nb, k, ws=None, stream=None, policy=None):
     _need_cuda()
     P = pack_params(shape)
     ws = _ws(ws, 0, 1, nbins)
     out = torch.empty(int(nbins), dtype=torch.float64, device="cuda")
     _check(lib().ipa_expected_hist(int(nbins), _Range(lo, hi), _hptr(P), float(ns), float(nb), float(k), _dptr(out),
-                                   _dptr(ws), ws.numel(), _stream(stream)))
+                                   _opt(policy), _dptr(ws), ws.numel(), _stream(stream)))
     return out
 
 
+@_alloc_on_stream
 def ipa_poisson_hist_toys(mean, seeds, ws=None, stream=None):
     _need_cuda()
     seeds = np.ascontiguousarray(seeds, dtype=np.uint64).ravel()
@@ -335,16 +397,19 @@ def ipa_poisson_hist_toys(mean, seeds, ws=None, stream=None):
     return out
 
 
-def ipa_signal_shape(nbins, lo, hi, shape, ws=None, stream=None):
+@_alloc_on_stream
+def ipa_signal_shape(nbins, lo, hi, shape, ws=None, stream=None, policy=None):
     """Un-normalised signal shape at the bin centres (device tensor [nbins])."""
     _need_cuda()
     P = pack_params(shape)
     ws = _ws(ws, 0, 1, nbins)
     out = torch.empty(int(nbins), dtype=torch.float64, device="cuda")
-    _check(lib().ipa_signal_shape(int(nbins), _Range(lo, hi), _hptr(P), _dptr(out), _dptr(ws), ws.numel(), _stream(stream)))
+    _check(lib().ipa_signal_shape(int(nbins), _Range(lo, hi), _hptr(P), _dptr(out), _opt(policy), _dptr(ws), ws.numel(),
+                                  _stream(stream)))
     return out
 
 
+@_alloc_on_stream
 def ipa_gauss_smear(sig, lo, hi, sigma0, stream=None):
     """Gaussian smearing of a shape on the bin grid (reading F3) -> new device tensor."""
     _need_cuda()
@@ -354,6 +419,7 @@ def ipa_gauss_smear(sig, lo, hi, sigma0, stream=None):
     return out
 
 
+@_alloc_on_stream
 def ipa_expected_hist_shape(sig, lo, hi, ns, nb, k, ws=None, stream=None):
     _need_cuda()
     nbins = sig.numel()
@@ -364,6 +430,7 @@ def ipa_expected_hist_shape(sig, lo, hi, ns, nb, k, ws=None, stream=None):
     return out
 
 
+@_alloc_on_stream
 def ipa_binned_nll_scan_shape(counts, lo, hi, sig, ns, nb, k, ws=None, stream=None):
     _need_cuda()
     ns = np.ascontiguousarray(ns, dtype=np.float64); nb = np.ascontiguousarray(nb, dtype=np.float64)
@@ -377,6 +444,7 @@ def ipa_binned_nll_scan_shape(counts, lo, hi, sig, ns, nb, k, ws=None, stream=No
     return out
 
 
+@_alloc_on_stream
 def ipa_cls_teststat(counts, nu_sb, nu_b, ws=None, stream=None):
     """q[T] of T histograms counts[T, nbins] (int32 payload = uint32 toys, int64 payload = uint64 data)."""
     _need_cuda()
@@ -390,6 +458,7 @@ def ipa_cls_teststat(counts, nu_sb, nu_b, ws=None, stream=None):
     return q
 
 
+@_alloc_on_stream
 def ipa_cls_count_ge(q, q_obs, stream=None):
     """-> int64 device tensor [1]: number of q >= q_obs[0] (q_obs a device tensor)."""
     _need_cuda()
@@ -398,6 +467,7 @@ def ipa_cls_count_ge(q, q_obs, stream=None):
     return out
 
 
+@_alloc_on_stream
 def ipa_cls_from_counts(count_sb, T_sb, count_b, T_b, stream=None):
     """-> device tensor [CL_sb, CL_b, CL_s]."""
     _need_cuda()
@@ -407,23 +477,27 @@ def ipa_cls_from_counts(count_sb, T_sb, count_b, T_b, stream=None):
     return out
 
 
-def ipa_sort_workspace_bytes(n, T=0):
-    return int(lib().ipa_sort_workspace_bytes(int(n), int(T)))
+def ipa_prepare_workspace_bytes(n, T=0):
+    return int(lib().ipa_prepare_workspace_bytes(int(n), int(T)))
 
 
-def ipa_events_sort(x, offsets=None, stream=None):
-    """One-off preparation: ascending sort of the events (inside each segment if offsets is given).
-    -> new device tensor; x is left untouched."""
+@_alloc_on_stream
+def ipa_events_prepare(x, lo, hi, offsets=None, stream=None, out=None, ws=None):
+    """One-off preparation: stable counting sort of the events on the coarse bin index (inside each segment if
+    offsets is given).  -> new device tensor (or `out`); x is left untouched."""
     _need_cuda()
     n = x.numel()
     T = offsets.numel() - 1 if offsets is not None else 0
-    out = torch.empty_like(x)
-    ws = torch.empty(max(256, ipa_sort_workspace_bytes(n, T)), dtype=torch.uint8, device="cuda")
-    _check(lib().ipa_events_sort(_dptr(x, torch.float64) if n else None, n, _dptr(offsets, torch.int64), T,
-                                 _dptr(out) if n else None, _dptr(ws), ws.numel(), _stream(stream)))
+    if out is None:
+        out = torch.empty_like(x)
+    if ws is None:
+        ws = torch.empty(max(256, ipa_prepare_workspace_bytes(n, T)), dtype=torch.uint8, device="cuda")
+    _check(lib().ipa_events_prepare(_dptr(x, torch.float64) if n else None, n, _dptr(offsets, torch.int64), T, _Range(lo, hi),
+                                    _dptr(out) if n else None, _dptr(ws), ws.numel(), _stream(stream)))
     return out
 
 
+@_alloc_on_stream
 def ipa_fp64_peak_probe(iters, stream=None):
     _need_cuda()
     out = torch.zeros(1, dtype=torch.float64, device="cuda")
@@ -431,12 +505,12 @@ def ipa_fp64_peak_probe(iters, stream=None):
     return out
 
 
-def nll_host(x_host, params, lo, hi, x_dev=None, ws=None):
+def nll_host(x_host, params, lo, hi, x_dev=None, ws=None, policy=None):
     """End-to-end convenience used by bench.py's e2e leg: host (pinned) events in, host NLL out.
     Copies x to the device, runs ipa_nll_eval, copies the K results back and synchronises."""
     _need_cuda()
     if x_dev is None:
         x_dev = torch.empty(x_host.numel(), dtype=torch.float64, device="cuda")
     x_dev.copy_(x_host, non_blocking=True)
-    nll, _, _ = ipa_nll_eval(x_dev, params, lo, hi, ws=ws)
+    nll, _, _ = ipa_nll_eval(x_dev, params, lo, hi, ws=ws, policy=policy)
     return nll.cpu()

@@ -4,14 +4,12 @@
 #include <cstdio>
 #include <cstring>
 #include <string>
-#include <cub/device/device_radix_sort.cuh>
-#include <cub/device/device_segmented_radix_sort.cuh>
 #include "ipa_kernels.cuh"
+#include "ipa_prepare.cuh"
 
 namespace {
 
 thread_local std::string g_last_cuda_error;
-int g_degree_policy = 0;
 
 #define IPA_CK(call)                                                                       \
   do {                                                                                     \
@@ -21,6 +19,13 @@ int g_degree_policy = 0;
       return IPA_ERR_CUDA;                                                                 \
     }                                                                                      \
   } while (0)
+
+// degree policy of the call (NULL options = defaults); -1 = invalid options
+int policy_of(const ipa_options* o) {
+  if (!o) return 0;
+  if ((o->degree_policy != 0 && o->degree_policy != 1) || o->reserved[0] || o->reserved[1] || o->reserved[2]) return -1;
+  return o->degree_policy;
+}
 
 constexpr int64_t kGridMax = 2048;  // upper bound of the streaming grid (partials sizing)
 
@@ -66,6 +71,8 @@ int device_info(int* sms) {
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    IPA_CK(cudaFuncSetAttribute(ipa_prep_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, IPA_PREP_SMEM));
+    IPA_CK(cudaFuncSetAttribute(ipa_prep_segment_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, IPA_PREP_SMEM));
     g_dev.dev = dev;
     g_dev.sms = n;
     g_dev.attr_set = true;
@@ -83,7 +90,7 @@ bool ws_ok(const void* ws, size_t bytes, size_t need) {
 
 // Runs the prologue for K sets.  K <= IPA_MAX_K: the sets travel in the kernel-parameter space;
 // larger batches go through the workspace with one host-to-device copy.
-int run_prologue(const ipa_params* p_host, int64_t K, ipa_range r, char* ws, const Layout& L, double* norm_sig,
+int run_prologue(const ipa_params* p_host, int64_t K, ipa_range r, int policy, char* ws, const Layout& L, double* norm_sig,
                  double* norm_bkg, int32_t* status_out, cudaStream_t st, bool want_grad = false) {
   IpaSetConsts* consts = reinterpret_cast<IpaSetConsts*>(ws + L.consts);
   unsigned int* counter = reinterpret_cast<unsigned int*>(ws + L.counter);
@@ -96,7 +103,7 @@ int run_prologue(const ipa_params* p_host, int64_t K, ipa_range r, char* ws, con
     p_dev = reinterpret_cast<const ipa_params*>(ws + L.params);
   }
   ipa_prologue_kernel<<<(unsigned)K, IPA_PRO_THREADS, 0, st>>>(batch, p_dev, r.lo, r.hi,
-                                                               g_degree_policy | (want_grad ? 2 : 0), consts,
+                                                               policy | (want_grad ? 2 : 0), consts,
                                                                counter, norm_sig, norm_bkg, status_out);
   IPA_CK(cudaGetLastError());
   return IPA_OK;
@@ -120,34 +127,30 @@ const char* ipa_strerror(int code) {
 const char* ipa_last_cuda_error(void) { return g_last_cuda_error.c_str(); }
 const char* ipa_version(void) { return "ipanll 0.1 sm_100a"; }
 
-int ipa_set_degree_policy(int policy) {
-  const int old = g_degree_policy;
-  g_degree_policy = policy ? 1 : 0;
-  return old;
-}
-
 size_t ipa_workspace_bytes(int64_t n, int64_t K, int64_t nbins) {
   (void)n;
   return make_layout(K, nbins).total;
 }
 
 int ipa_norm(const ipa_params* p_host, int K, ipa_range r, double* norm_sig_dev, double* norm_bkg_dev,
-             int32_t* status_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
-  if (!p_host || K < 1 || !range_ok(r) || !norm_sig_dev || !norm_bkg_dev) return IPA_ERR_INVALID_ARG;
+             int32_t* status_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  const int policy = policy_of(opt_host);
+  if (!p_host || K < 1 || !range_ok(r) || !norm_sig_dev || !norm_bkg_dev || policy < 0) return IPA_ERR_INVALID_ARG;
   const Layout L = make_layout(K, 0);
   if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
-  return run_prologue(p_host, K, r, static_cast<char*>(ws_dev), L, norm_sig_dev, norm_bkg_dev, status_dev,
+  return run_prologue(p_host, K, r, policy, static_cast<char*>(ws_dev), L, norm_sig_dev, norm_bkg_dev, status_dev,
                       static_cast<cudaStream_t>(cuda_stream));
 }
 
-int ipa_core_degree(const ipa_params* p_host, int K, ipa_range r, int32_t* degree_dev, void* ws_dev, size_t ws_bytes,
-                    void* cuda_stream) {
-  if (!p_host || K < 1 || !range_ok(r) || !degree_dev) return IPA_ERR_INVALID_ARG;
+int ipa_core_degree(const ipa_params* p_host, int K, ipa_range r, int32_t* degree_dev, const ipa_options* opt_host,
+                    void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  const int policy = policy_of(opt_host);
+  if (!p_host || K < 1 || !range_ok(r) || !degree_dev || policy < 0) return IPA_ERR_INVALID_ARG;
   const Layout L = make_layout(K, 0);
   if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   char* ws = static_cast<char*>(ws_dev);
-  int rc = run_prologue(p_host, K, r, ws, L, nullptr, nullptr, nullptr, st);
+  int rc = run_prologue(p_host, K, r, policy, ws, L, nullptr, nullptr, nullptr, st);
   if (rc) return rc;
   ipa_degree_kernel<<<(K + 127) / 128, 128, 0, st>>>(reinterpret_cast<const IpaSetConsts*>(ws + L.consts), K, degree_dev);
   IPA_CK(cudaGetLastError());
@@ -155,8 +158,10 @@ int ipa_core_degree(const ipa_params* p_host, int K, ipa_range r, int32_t* degre
 }
 
 int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r, double* nll_dev,
-                 double* logpdf_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
-  if (n < 0 || (n > 0 && !x_dev) || !p_host || K < 1 || K > IPA_MAX_K || !range_ok(r) || !nll_dev)
+                 double* logpdf_dev, int32_t* status_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes,
+                 void* cuda_stream) {
+  const int policy = policy_of(opt_host);
+  if (n < 0 || (n > 0 && !x_dev) || !p_host || K < 1 || K > IPA_MAX_K || !range_ok(r) || !nll_dev || policy < 0)
     return IPA_ERR_INVALID_ARG;
   if (((uintptr_t)x_dev % 8) != 0) return IPA_ERR_INVALID_ARG;
   const Layout L = make_layout(K, 0);
@@ -166,7 +171,7 @@ int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K
   if (rc) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   char* ws = static_cast<char*>(ws_dev);
-  rc = run_prologue(p_host, K, r, ws, L, nullptr, nullptr, nullptr, st);
+  rc = run_prologue(p_host, K, r, policy, ws, L, nullptr, nullptr, nullptr, st);
   if (rc) return rc;
   const int64_t ntiles = (n + IPA_NTILE - 1) / IPA_NTILE;
   int64_t G = (int64_t)sms * IPA_NB_PER_SM;
@@ -197,9 +202,31 @@ int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K
   return IPA_OK;
 }
 
+int ipa_nll_fd_gradient(const double* x_dev, int64_t n, const ipa_params* theta_host, int P, const int32_t* idx_host,
+                        const double* h_host, ipa_range r, double* nll_dev, double* grad_dev, int32_t* status_dev,
+                        const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (!theta_host || P < 1 || P > 11 || !idx_host || !h_host || !grad_dev) return IPA_ERR_INVALID_ARG;
+  ipa_params batch[2 * 11 + 1];
+  IpaFdSteps hs;
+  for (int j = 0; j < 2 * P + 1; ++j) batch[j] = *theta_host;
+  for (int j = 0; j < 11; ++j) hs.h[j] = 1.0;
+  for (int j = 0; j < P; ++j) {
+    if (idx_host[j] < 0 || idx_host[j] > 10 || !(h_host[j] > 0.0) || !ipa_finite(h_host[j])) return IPA_ERR_INVALID_ARG;
+    const double base = (&theta_host->mu)[idx_host[j]];
+    (&batch[2 * j + 1].mu)[idx_host[j]] = base + h_host[j];
+    (&batch[2 * j + 2].mu)[idx_host[j]] = base - h_host[j];
+    hs.h[j] = h_host[j];
+  }
+  int rc = ipa_nll_eval(x_dev, n, batch, 2 * P + 1, r, nll_dev, nullptr, status_dev, opt_host, ws_dev, ws_bytes, cuda_stream);
+  if (rc) return rc;
+  ipa_fd_difference_kernel<<<1, 32, 0, static_cast<cudaStream_t>(cuda_stream)>>>(nll_dev, P, hs, grad_dev);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
 int ipa_nll_eval_extended(const double* x_dev, int64_t n, const ipa_params* p_host, const double* ns_host,
                           const double* nb_host, int K, ipa_range r, double* nll_dev, int32_t* status_dev,
-                          void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+                          const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
   if (!p_host || !ns_host || !nb_host || K < 1 || K > IPA_MAX_K) return IPA_ERR_INVALID_ARG;
   ipa_params q[IPA_MAX_K];
   double nu[IPA_MAX_K];
@@ -210,7 +237,7 @@ int ipa_nll_eval_extended(const double* x_dev, int64_t n, const ipa_params* p_ho
     q[k].f = ok ? ns_host[k] / nu[k] : -1.0;          // an invalid yield pair becomes a domain error of the set
     if (!ok) nu[k] = 1.0;
   }
-  int rc = ipa_nll_eval(x_dev, n, q, K, r, nll_dev, nullptr, status_dev, ws_dev, ws_bytes, cuda_stream);
+  int rc = ipa_nll_eval(x_dev, n, q, K, r, nll_dev, nullptr, status_dev, opt_host, ws_dev, ws_bytes, cuda_stream);
   if (rc) return rc;
   IpaYields y;
   for (int k = 0; k < IPA_MAX_K; ++k) y.nu[k] = k < K ? nu[k] : 1.0;
@@ -220,9 +247,10 @@ int ipa_nll_eval_extended(const double* x_dev, int64_t n, const ipa_params* p_ho
 }
 
 int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r,
-                      double* nll_dev, double* grad_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
-                      void* cuda_stream) {
-  if (n < 0 || (n > 0 && !x_dev) || !p_host || K < 1 || K > IPA_MAX_K || !range_ok(r) || !nll_dev || !grad_dev)
+                      double* nll_dev, double* grad_dev, int32_t* status_dev, const ipa_options* opt_host, void* ws_dev,
+                      size_t ws_bytes, void* cuda_stream) {
+  const int policy = policy_of(opt_host);
+  if (n < 0 || (n > 0 && !x_dev) || !p_host || K < 1 || K > IPA_MAX_K || !range_ok(r) || !nll_dev || !grad_dev || policy < 0)
     return IPA_ERR_INVALID_ARG;
   if (((uintptr_t)x_dev % 8) != 0) return IPA_ERR_INVALID_ARG;
   const Layout L = make_layout(K, 0);
@@ -232,7 +260,7 @@ int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, 
   if (rc) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   char* ws = static_cast<char*>(ws_dev);
-  rc = run_prologue(p_host, K, r, ws, L, nullptr, nullptr, nullptr, st, true);
+  rc = run_prologue(p_host, K, r, policy, ws, L, nullptr, nullptr, nullptr, st, true);
   if (rc) return rc;
   IPA_CK(cudaMemsetAsync(ws + L.counter, 0, 256, st));          // one ticket counter per set
   const int64_t tile_n = (int64_t)IPA_GB * IPA_GE, ntiles = (n + tile_n - 1) / tile_n;
@@ -250,7 +278,9 @@ int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, 
 
 static int segmented_common(const double* x_dev, const int64_t* offsets_dev, int64_t T, const ipa_params* p_host,
                             int64_t K, const int32_t* set_of_segment_host, ipa_range r, double* nll_dev,
-                            int32_t* status_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+                            int32_t* status_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  const int policy = policy_of(opt_host);
+  if (policy < 0) return IPA_ERR_INVALID_ARG;
   if (!x_dev || !offsets_dev || T < 1 || T > 0x7fffffffLL || K < 1 || K > 0x7fffffffLL || !p_host || !range_ok(r) ||
       !nll_dev)
     return IPA_ERR_INVALID_ARG;
@@ -261,7 +291,7 @@ static int segmented_common(const double* x_dev, const int64_t* offsets_dev, int
   if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   char* ws = static_cast<char*>(ws_dev);
-  int rc = run_prologue(p_host, K, r, ws, L, nullptr, nullptr, nullptr, st);
+  int rc = run_prologue(p_host, K, r, policy, ws, L, nullptr, nullptr, nullptr, st);
   if (rc) return rc;
   const IpaSetConsts* consts = reinterpret_cast<const IpaSetConsts*>(ws + L.consts);
   double* partials = reinterpret_cast<double*>(ws + L.partials);
@@ -279,22 +309,26 @@ static int segmented_common(const double* x_dev, const int64_t* offsets_dev, int
 }
 
 int ipa_nll_eval_segmented(const double* x_dev, const int64_t* offsets_dev, int64_t T, const ipa_params* p_host,
-                           ipa_range r, double* nll_dev, int32_t* status_dev, void* ws_dev, size_t ws_bytes,
-                           void* cuda_stream) {
-  return segmented_common(x_dev, offsets_dev, T, p_host, T, nullptr, r, nll_dev, status_dev, ws_dev, ws_bytes, cuda_stream);
+                           ipa_range r, double* nll_dev, int32_t* status_dev, const ipa_options* opt_host, void* ws_dev,
+                           size_t ws_bytes, void* cuda_stream) {
+  return segmented_common(x_dev, offsets_dev, T, p_host, T, nullptr, r, nll_dev, status_dev, opt_host, ws_dev, ws_bytes,
+                          cuda_stream);
 }
 
 int ipa_nll_eval_categories(const double* x_dev, const int64_t* offsets_dev, int64_t T, const ipa_params* p_host, int64_t K,
                             const int32_t* set_of_segment_host, ipa_range r, double* nll_dev, int32_t* status_dev,
-                            void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+                            const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
   if (!set_of_segment_host) return IPA_ERR_INVALID_ARG;
-  return segmented_common(x_dev, offsets_dev, T, p_host, K, set_of_segment_host, r, nll_dev, status_dev, ws_dev, ws_bytes,
-                          cuda_stream);
+  return segmented_common(x_dev, offsets_dev, T, p_host, K, set_of_segment_host, r, nll_dev, status_dev, opt_host, ws_dev,
+                          ws_bytes, cuda_stream);
 }
 
 int ipa_toy_generate(const uint64_t* seeds_host, int64_t T, const ipa_params* gen_host, int64_t gen_count,
                      double mean_sig, double mean_bkg, ipa_range r, int64_t capacity, double* x_dev,
-                     int64_t* offsets_dev, int32_t* overflow_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+                     int64_t* offsets_dev, int32_t* overflow_dev, int32_t* status_dev, const ipa_options* opt_host,
+                     void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  const int policy = policy_of(opt_host);
+  if (policy < 0) return IPA_ERR_INVALID_ARG;
   const bool mixture = (mean_sig < 0.0) || (mean_bkg < 0.0);
   if (!seeds_host || T < 1 || T > 0x7fffffffLL || !gen_host || (gen_count != 1 && gen_count != T) || !range_ok(r) ||
       capacity < 0 || (capacity > 0 && !x_dev) || !offsets_dev)
@@ -307,7 +341,7 @@ int ipa_toy_generate(const uint64_t* seeds_host, int64_t T, const ipa_params* ge
   if (rc) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   char* ws = static_cast<char*>(ws_dev);
-  rc = run_prologue(gen_host, gen_count, r, ws, L, nullptr, nullptr, nullptr, st);
+  rc = run_prologue(gen_host, gen_count, r, policy, ws, L, nullptr, nullptr, status_dev, st);
   if (rc) return rc;
   IPA_CK(cudaMemcpyAsync(ws + L.seeds, seeds_host, (size_t)T * 8, cudaMemcpyHostToDevice, st));
   const unsigned long long* seeds = reinterpret_cast<const unsigned long long*>(ws + L.seeds);
@@ -334,7 +368,7 @@ int ipa_toy_generate(const uint64_t* seeds_host, int64_t T, const ipa_params* ge
   if (chunks < 1) chunks = 1;
   if (capacity > 0) {
     ipa_toy_events_kernel<<<dim3((unsigned)T, (unsigned)chunks), IPA_BLOCK, 0, st>>>(
-        seeds, consts, gen_count == T && T > 1 ? 1 : 0, nsig, offsets, r.lo, r.hi, capacity, mixture ? 1 : 0, x_dev);
+        seeds, consts, gen_count == T && T > 1 ? 1 : 0, nsig, offsets, r.lo, r.hi, capacity, mixture ? 1 : 0, x_dev, overflow_dev);
     IPA_CK(cudaGetLastError());
   }
   return IPA_OK;
@@ -359,7 +393,10 @@ int ipa_hist_fill(const double* x_dev, int64_t n, ipa_range r, int nbins, uint64
 
 static int binned_common(const uint64_t* counts_dev, int nbins, ipa_range r, const ipa_params* shape_host,
                          const double* sig_dev, const double* ns_host, const double* nb_host, const double* k_host, int64_t npoints,
-                         double* nll_dev, double* nu_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+                         double* nll_dev, double* nu_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes,
+                         void* cuda_stream) {
+  const int policy = policy_of(opt_host);
+  if (policy < 0) return IPA_ERR_INVALID_ARG;
   const Layout L = make_layout(npoints, nbins);
   if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -373,7 +410,7 @@ static int binned_common(const uint64_t* counts_dev, int nbins, ipa_range r, con
     ipa_params shape = *shape_host;
     shape.f = 0.5;  // f and k of the shape set are not used by the binned path
     shape.k = 0.0;
-    int rc = run_prologue(&shape, 1, r, ws, L, nullptr, nullptr, nullptr, st);
+    int rc = run_prologue(&shape, 1, r, policy, ws, L, nullptr, nullptr, nullptr, st);
     if (rc) return rc;
     ipa_binned_shape_kernel<<<1, 256, 0, st>>>(reinterpret_cast<const IpaSetConsts*>(ws + L.consts), r.lo, r.hi, nbins, sbin,
                                                flag, 1);
@@ -391,23 +428,25 @@ static int binned_common(const uint64_t* counts_dev, int nbins, ipa_range r, con
 
 int ipa_binned_nll_scan(const uint64_t* counts_dev, int nbins, ipa_range r, const ipa_params* shape_host,
                         const double* ns_host, const double* nb_host, const double* k_host, int64_t npoints,
-                        double* nll_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+                        double* nll_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
   if (!counts_dev || nbins < 1 || !range_ok(r) || !shape_host || !ns_host || !nb_host || !k_host || npoints < 1 ||
       npoints > 0x7fffffffLL || !nll_dev)
     return IPA_ERR_INVALID_ARG;
-  return binned_common(counts_dev, nbins, r, shape_host, nullptr, ns_host, nb_host, k_host, npoints, nll_dev, nullptr, ws_dev,
-                       ws_bytes, cuda_stream);
+  return binned_common(counts_dev, nbins, r, shape_host, nullptr, ns_host, nb_host, k_host, npoints, nll_dev, nullptr, opt_host,
+                       ws_dev, ws_bytes, cuda_stream);
 }
 
 int ipa_expected_hist(int nbins, ipa_range r, const ipa_params* shape_host, double ns, double nb, double k,
-                      double* nu_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+                      double* nu_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
   if (nbins < 1 || !range_ok(r) || !shape_host || !nu_dev) return IPA_ERR_INVALID_ARG;
-  return binned_common(nullptr, nbins, r, shape_host, nullptr, &ns, &nb, &k, 1, nullptr, nu_dev, ws_dev, ws_bytes, cuda_stream);
+  return binned_common(nullptr, nbins, r, shape_host, nullptr, &ns, &nb, &k, 1, nullptr, nu_dev, opt_host, ws_dev, ws_bytes,
+                       cuda_stream);
 }
 
-int ipa_signal_shape(int nbins, ipa_range r, const ipa_params* shape_host, double* sig_dev, void* ws_dev, size_t ws_bytes,
-                     void* cuda_stream) {
-  if (nbins < 1 || !range_ok(r) || !shape_host || !sig_dev) return IPA_ERR_INVALID_ARG;
+int ipa_signal_shape(int nbins, ipa_range r, const ipa_params* shape_host, double* sig_dev, const ipa_options* opt_host,
+                     void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  const int policy = policy_of(opt_host);
+  if (nbins < 1 || !range_ok(r) || !shape_host || !sig_dev || policy < 0) return IPA_ERR_INVALID_ARG;
   const Layout L = make_layout(1, nbins);
   if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
@@ -415,7 +454,7 @@ int ipa_signal_shape(int nbins, ipa_range r, const ipa_params* shape_host, doubl
   ipa_params shape = *shape_host;
   shape.f = 0.5;
   shape.k = 0.0;
-  int rc = run_prologue(&shape, 1, r, ws, L, nullptr, nullptr, nullptr, st);
+  int rc = run_prologue(&shape, 1, r, policy, ws, L, nullptr, nullptr, nullptr, st);
   if (rc) return rc;
   ipa_binned_shape_kernel<<<1, 256, 0, st>>>(reinterpret_cast<const IpaSetConsts*>(ws + L.consts), r.lo, r.hi, nbins, sig_dev,
                                              reinterpret_cast<int32_t*>(ws + L.flag), 0);
@@ -442,7 +481,7 @@ int ipa_gauss_smear(const double* in_dev, int nbins, ipa_range r, double sigma0,
 int ipa_expected_hist_shape(int nbins, ipa_range r, const double* sig_dev, double ns, double nb, double k, double* nu_dev,
                             void* ws_dev, size_t ws_bytes, void* cuda_stream) {
   if (nbins < 1 || !range_ok(r) || !sig_dev || !nu_dev) return IPA_ERR_INVALID_ARG;
-  return binned_common(nullptr, nbins, r, nullptr, sig_dev, &ns, &nb, &k, 1, nullptr, nu_dev, ws_dev, ws_bytes, cuda_stream);
+  return binned_common(nullptr, nbins, r, nullptr, sig_dev, &ns, &nb, &k, 1, nullptr, nu_dev, nullptr, ws_dev, ws_bytes, cuda_stream);
 }
 
 int ipa_binned_nll_scan_shape(const uint64_t* counts_dev, int nbins, ipa_range r, const double* sig_dev,
@@ -451,8 +490,8 @@ int ipa_binned_nll_scan_shape(const uint64_t* counts_dev, int nbins, ipa_range r
   if (!counts_dev || nbins < 1 || !range_ok(r) || !sig_dev || !ns_host || !nb_host || !k_host || npoints < 1 ||
       npoints > 0x7fffffffLL || !nll_dev)
     return IPA_ERR_INVALID_ARG;
-  return binned_common(counts_dev, nbins, r, nullptr, sig_dev, ns_host, nb_host, k_host, npoints, nll_dev, nullptr, ws_dev,
-                       ws_bytes, cuda_stream);
+  return binned_common(counts_dev, nbins, r, nullptr, sig_dev, ns_host, nb_host, k_host, npoints, nll_dev, nullptr, nullptr,
+                       ws_dev, ws_bytes, cuda_stream);
 }
 
 int ipa_poisson_hist_toys(const double* mean_dev, int nbins, const uint64_t* seeds_host, int64_t T,
@@ -522,38 +561,54 @@ int ipa_cls_from_counts(const int64_t* count_sb_dev, int64_t T_sb, const int64_t
   return IPA_OK;
 }
 
-size_t ipa_sort_workspace_bytes(int64_t n, int64_t T) {
-  if (n < 0 || T < 0) return 0;
-  size_t bytes = 0;
-  const double* in = nullptr;
-  double* out = nullptr;
-  if (T > 0) {
-    if (n > 0x7fffffffLL || T > 0x7fffffffLL) return 0;
-    const long long* off = nullptr;
-    cub::DeviceSegmentedRadixSort::SortKeys(nullptr, bytes, in, out, (int)n, (int)T, off, off + 1, 0, 64, 0);
-  } else {
-    cub::DeviceRadixSort::SortKeys(nullptr, bytes, in, out, (long long)n, 0, 64, 0);
-  }
-  return align_up(bytes + 256, 256);
+// grid of the unsegmented preparation: two resident blocks per SM, never more blocks than tiles
+static int64_t prep_grid(int64_t n, int sms) {
+  const int64_t tiles = (n + IPA_PREP_TILE - 1) / IPA_PREP_TILE;
+  int64_t G = 2 * (int64_t)(sms > 0 ? sms : 148);
+  if (G > tiles) G = tiles;
+  return G < 1 ? 1 : G;
 }
 
-int ipa_events_sort(const double* x_in_dev, int64_t n, const int64_t* offsets_dev, int64_t T, double* x_out_dev,
-                    void* ws_dev, size_t ws_bytes, void* cuda_stream) {
-  if (n < 0 || T < 0 || (n > 0 && (!x_in_dev || !x_out_dev || x_in_dev == x_out_dev))) return IPA_ERR_INVALID_ARG;
-  if (offsets_dev && (T < 1 || n > 0x7fffffffLL || T > 0x7fffffffLL)) return IPA_ERR_INVALID_ARG;
+size_t ipa_prepare_workspace_bytes(int64_t n, int64_t T) {
+  if (n < 0 || T < 0) return 0;
+  if (T > 0) return 256;                                       // segmented: everything lives in shared memory
+  const int64_t Gmax = prep_grid(n, 1024);                     // upper bound over any device (<= 2048 blocks)
+  return align_up((size_t)IPA_PREP_BINS * (size_t)Gmax * 4, 256) + 2 * align_up((size_t)IPA_PREP_BINS * 8, 256);
+}
+
+int ipa_events_prepare(const double* x_in_dev, int64_t n, const int64_t* offsets_dev, int64_t T, ipa_range r,
+                       double* x_out_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  if (n < 0 || T < 0 || n > 0xffffffffLL || (n > 0 && (!x_in_dev || !x_out_dev || x_in_dev == x_out_dev)) || !range_ok(r))
+    return IPA_ERR_INVALID_ARG;
+  if (offsets_dev && (T < 1 || T > 0x7fffffffLL)) return IPA_ERR_INVALID_ARG;
   if (!offsets_dev) T = 0;
   if (n == 0) return IPA_OK;
-  size_t need = ipa_sort_workspace_bytes(n, T);
-  if (!ws_ok(ws_dev, ws_bytes, need)) return IPA_ERR_WORKSPACE;
+  if (!ws_ok(ws_dev, ws_bytes, ipa_prepare_workspace_bytes(n, T))) return IPA_ERR_WORKSPACE;
+  int sms = 0;
+  int rc = device_info(&sms);
+  if (rc) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-  size_t bytes = ws_bytes;
+  const double scale = (double)IPA_PREP_BINS / (r.hi - r.lo);
   if (T > 0) {
-    const long long* off = reinterpret_cast<const long long*>(offsets_dev);
-    IPA_CK(cub::DeviceSegmentedRadixSort::SortKeys(ws_dev, bytes, x_in_dev, x_out_dev, (int)n, (int)T, off, off + 1, 0, 64,
-                                                   st));
-  } else {
-    IPA_CK(cub::DeviceRadixSort::SortKeys(ws_dev, bytes, x_in_dev, x_out_dev, (long long)n, 0, 64, st));
+    ipa_prep_segment_kernel<<<(unsigned)T, IPA_PREP_THREADS, IPA_PREP_SMEM, st>>>(
+        x_in_dev, reinterpret_cast<const long long*>(offsets_dev), r.lo, scale, x_out_dev);
+    IPA_CK(cudaGetLastError());
+    return IPA_OK;
   }
+  const int64_t G = prep_grid(n, sms);
+  char* ws = static_cast<char*>(ws_dev);
+  unsigned int* hist = reinterpret_cast<unsigned int*>(ws);
+  size_t o = align_up((size_t)IPA_PREP_BINS * (size_t)G * 4, 256);
+  unsigned long long* bintot = reinterpret_cast<unsigned long long*>(ws + o);
+  unsigned long long* binbase = reinterpret_cast<unsigned long long*>(ws + o + align_up((size_t)IPA_PREP_BINS * 8, 256));
+  ipa_prep_hist_kernel<<<(unsigned)G, IPA_PREP_THREADS, 0, st>>>(x_in_dev, n, r.lo, scale, hist);
+  IPA_CK(cudaGetLastError());
+  ipa_prep_scan_kernel<<<IPA_PREP_BINS / 8, 256, 0, st>>>(hist, (int)G, bintot);
+  IPA_CK(cudaGetLastError());
+  ipa_prep_binscan_kernel<<<1, IPA_PREP_THREADS, 0, st>>>(bintot, binbase);
+  IPA_CK(cudaGetLastError());
+  ipa_prep_scatter_kernel<<<(unsigned)G, IPA_PREP_THREADS, IPA_PREP_SMEM, st>>>(x_in_dev, n, r.lo, scale, hist, binbase, x_out_dev);
+  IPA_CK(cudaGetLastError());
   return IPA_OK;
 }
 

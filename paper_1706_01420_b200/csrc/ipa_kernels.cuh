@@ -348,6 +348,17 @@ template <bool LOGPDF, bool FULL, bool GROUPED>
 __device__ __forceinline__ void ipa_tile_sets(const IpaSetConsts* sc, int K, const IpaGroups& grp, double* acc,
                                               const double (&xv)[IPA_NE], long long base, long long n, int tid,
                                               double* __restrict__ logpdf, const double2* s_tab) {
+  if (LOGPDF) {
+    // per-event output of a set with a domain error: NaN (its NLL is +inf)
+    for (int k = 0; k < K; ++k) {
+      if (!sc[k].status) continue;
+#pragma unroll
+      for (int e = 0; e < IPA_NE; ++e) {
+        const long long i = base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1);
+        if (FULL || i < n) logpdf[(long long)k * n + i] = NAN;
+      }
+    }
+  }
   if (!GROUPED) {
     for (int k = 0; k < K; ++k) {
       const IpaSetConsts& c = sc[k];
@@ -875,7 +886,7 @@ __global__ void __launch_bounds__(IPA_BLOCK)
 ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSetConsts* __restrict__ consts,
                       int gen_stride,
                       const long long* __restrict__ nsig, const long long* __restrict__ offsets, double lo, double hi,
-                      long long capacity, int mixture, double* __restrict__ x) {
+                      long long capacity, int mixture, double* __restrict__ x, int32_t* __restrict__ overflow) {
   __shared__ IpaSetConsts c;
   __shared__ double red[IPA_BLOCK / 32];
   __shared__ double s_logImax;
@@ -890,7 +901,14 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
     for (int i = tid; i < (int)(sizeof(IpaSetConsts) / 8); i += IPA_BLOCK) dst[i] = src[i];
   }
   __syncthreads();
-  if (c.status) return;
+  if (c.status) {
+    // invalid generating set: the toy's events are NaN (its offsets are still those of the drawn yields)
+    const long long b0 = mixture ? 0 : offsets[t];
+    long long e0 = mixture ? capacity : offsets[t + 1];
+    if (e0 > capacity) e0 = capacity;
+    for (long long i = b0 + (long long)blockIdx.y * IPA_BLOCK + tid; i < e0; i += (long long)gridDim.y * IPA_BLOCK) x[i] = NAN;
+    return;
+  }
   // envelope: log of the maximum of I over the range (reading D13)
   if (c.beta == 0.0 && lo <= c.mu && c.mu <= hi) {
     if (tid == 0) s_logImax = ipa_logI_rec(c, 0.0);
@@ -968,6 +986,7 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
         const double xx = lo + (hi - lo) * u1;
         const double ratio = ipa_fexp_neg(fmax(ipa_logI_fast(c, cshift, xx - c.mu, s_tab) - logImax, -700.0));
         if (u2 * 1.02 < ratio || attempt == 100001u) {
+          if (attempt == 100001u && overflow) atomicOr(overflow, 2);     // attempt cap: not a draw from the density
           x[beg + (long long)j] = xx;
           item = -1;
         } else {
@@ -1244,6 +1263,15 @@ struct IpaYields { double nu[IPA_MAX_K]; };
 __global__ void ipa_extended_term_kernel(double* __restrict__ nll, int K, long long n, const __grid_constant__ IpaYields y) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k < K) nll[k] += y.nu[k] - (double)n * log(y.nu[k]);
+}
+
+// finite-difference gradient (row G, reading C6): g_j = (NLL(theta + h_j e_j) - NLL(theta - h_j e_j)) / (2 h_j) from
+// the 2P+1 results of one batched call; the steps travel in the kernel-parameter space
+struct IpaFdSteps { double h[11]; };
+__global__ void ipa_fd_difference_kernel(const double* __restrict__ nll, int P, const __grid_constant__ IpaFdSteps hs,
+                                         double* __restrict__ grad) {
+  const int j = threadIdx.x;
+  if (j < P) grad[j] = (nll[2 * j + 1] - nll[2 * j + 2]) / (2.0 * hs.h[j]);
 }
 
 // ------------------------------------------------------------------------------------------------

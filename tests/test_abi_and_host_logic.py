@@ -50,20 +50,35 @@ def test_argument_validation_without_gpu(ipa):
     bad = ipa.binding._Range(HI, LO)
     one = C.c_void_p(256)  # non-null dummy; never dereferenced because validation fails first
     p = P.ctypes.data_as(C.c_void_p)
-    assert L.ipa_nll_eval(one, -1, p, 1, rng, one, None, None, one, 1 << 30, None) == -1
-    assert L.ipa_nll_eval(one, 10, p, 0, rng, one, None, None, one, 1 << 30, None) == -1
-    assert L.ipa_nll_eval(one, 10, p, 33, rng, one, None, None, one, 1 << 30, None) == -1
-    assert L.ipa_nll_eval(one, 10, p, 1, bad, one, None, None, one, 1 << 30, None) == -1
-    assert L.ipa_nll_eval(None, 10, p, 1, rng, one, None, None, one, 1 << 30, None) == -1
-    assert L.ipa_nll_eval(C.c_void_p(260), 10, p, 1, rng, one, None, None, one, 1 << 30, None) == -1
-    assert L.ipa_nll_eval(one, 10, p, 1, rng, one, None, None, one, 16, None) == -2
-    assert L.ipa_nll_eval(one, 10, p, 1, rng, one, None, None, C.c_void_p(264), 1 << 30, None) == -2
-    assert L.ipa_norm(None, 1, rng, one, one, None, one, 1 << 30, None) == -1
+    assert L.ipa_nll_eval(one, -1, p, 1, rng, one, None, None, None, one, 1 << 30, None) == -1
+    assert L.ipa_nll_eval(one, 10, p, 0, rng, one, None, None, None, one, 1 << 30, None) == -1
+    assert L.ipa_nll_eval(one, 10, p, 33, rng, one, None, None, None, one, 1 << 30, None) == -1
+    assert L.ipa_nll_eval(one, 10, p, 1, bad, one, None, None, None, one, 1 << 30, None) == -1
+    assert L.ipa_nll_eval(None, 10, p, 1, rng, one, None, None, None, one, 1 << 30, None) == -1
+    assert L.ipa_nll_eval(C.c_void_p(260), 10, p, 1, rng, one, None, None, None, one, 1 << 30, None) == -1
+    assert L.ipa_nll_eval(one, 10, p, 1, rng, one, None, None, None, one, 16, None) == -2
+    assert L.ipa_nll_eval(one, 10, p, 1, rng, one, None, None, None, C.c_void_p(264), 1 << 30, None) == -2
+    # options: an unknown degree policy or a non-zero reserved field is an argument error
+    for pol, res in ((2, 0), (-1, 0), (0, 7)):
+        o = ipa.binding._Options()
+        o.degree_policy = pol
+        o.reserved[1] = res
+        assert L.ipa_nll_eval(one, 10, p, 1, rng, one, None, None, C.byref(o), one, 1 << 30, None) == -1
+    assert L.ipa_norm(None, 1, rng, one, one, None, None, one, 1 << 30, None) == -1
+    idx = np.array([0, 11], dtype=np.int32)
+    hh = np.array([0.01, 0.01])
+    assert L.ipa_nll_fd_gradient(one, 10, p, 2, idx.ctypes.data_as(C.c_void_p), hh.ctypes.data_as(C.c_void_p), rng, one, one,
+                                 None, None, one, 1 << 30, None) == -1           # field index out of range
+    assert L.ipa_nll_fd_gradient(one, 10, p, 12, idx.ctypes.data_as(C.c_void_p), hh.ctypes.data_as(C.c_void_p), rng, one, one,
+                                 None, None, one, 1 << 30, None) == -1           # P > 11
+    assert L.ipa_events_prepare(one, 10, None, 0, rng, one, one, 1 << 30, None) == -1      # output aliases the input
+    assert L.ipa_events_prepare(one, 2 ** 32, None, 0, rng, C.c_void_p(512), one, 1 << 30, None) == -1
+    assert L.ipa_events_prepare(one, 10, None, 0, rng, C.c_void_p(512), one, 16, None) == -2
+    assert ipa.ipa_prepare_workspace_bytes(10 ** 8) >= 2048 * 296 * 4 and ipa.ipa_prepare_workspace_bytes(10 ** 5, 7) == 256
     assert L.ipa_hist_fill(one, 5, rng, 0, one, None) == -1
     assert L.ipa_strerror(-2).decode().startswith("workspace")
     assert ipa.ipa_workspace_bytes(10 ** 8, 9) >= 9 * 600
     assert ipa.ipa_workspace_bytes(10 ** 8, 1000) > ipa.ipa_workspace_bytes(10 ** 8, 9)
-    assert ipa.ipa_set_degree_policy(1) == 0 and ipa.ipa_set_degree_policy(0) == 1
 
 
 def test_compute_fails_loudly_without_gpu(ipa):

@@ -39,8 +39,8 @@ def test_oracle_fit_recovers_generating_parameters(orc):
     for name in inp.FLOATED:
         assert 0.1 < res.errors[name] / (inp.GRAD_SCALE[name] / np.sqrt(n / 1e4)) < 3.0
     # the FD gradient at the minimum vanishes (in 1/sigma units)
-    batch, h = inp.fd_batch(res.theta)
-    g = inp.fd_gradient(orc.nll(x, batch, LO, HI, nthreads=nthreads), h)
+    idx, h = inp.fd_spec()
+    _, g = orc.fd_gradient(x, res.theta, idx, h, LO, HI, nthreads=nthreads)
     assert np.all(np.abs(g) * np.array([res.errors[k] for k in inp.FLOATED]) < 1e-3)
 
 
@@ -103,8 +103,8 @@ def test_config2_fit_parity_gpu_vs_oracle(orc):
         assert abs(a - b) <= 1e-6 * abs(b), (name, a, b)
         assert abs((b - inp.GEN[name]) / res_o.errors[name]) < 4.5
     assert abs(res_g.nll - res_o.nll) <= 1e-10 * abs(res_o.nll)
-    # sorted layout: same minimum
-    xs = ipa.ipa_events_sort(xd)
+    # prepared layout: same minimum
+    xs = ipa.ipa_events_prepare(xd, LO, HI)
 
     def gpu_nll_sorted(th):
         nll, _, _ = ipa.ipa_nll_eval(xs, th, LO, HI, ws=ws)

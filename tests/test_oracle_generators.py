@@ -177,3 +177,115 @@ def test_poisson_hist_toys(orc):
         assert abs(col.var() / mean[b] - 1) < 0.15
     # element (t, b) depends only on (seed_t, b, mean_b)
     assert orc.poisson(7, 3, 4, 120.0) == t[6, 3]
+
+
+# ---------------------------------------------------------------------------------------------
+# PTRS branch of the Poisson sampler (mean >= 10: the branch configs 4 and 5 use).  Pins:
+#  (i)   exact probability function: chi^2 of 2e6 draws against scipy.stats.poisson.pmf (bins pooled to
+#        an expectation >= 20);
+#  (ii)  a theorem of rejection sampling: with k = floor(G(U)), G'(U) = a/us^2 + b and the acceptance test
+#        V <= p(k) G'(U) / inv_alpha, the acceptance probability per attempt is EXACTLY 1/inv_alpha as long as
+#        the hat dominates p everywhere AND the two squeeze steps never change the decision of the full test.
+#        So the mean number of attempts must equal inv_alpha; a squeeze constant that accepts (or rejects)
+#        what the full comparison would not shows up here long before it distorts the distribution;
+#  (iii) the quick acceptance (us >= 0.07 and V <= v_r) is taken with probability (1 - 2*0.07) v_r per attempt
+#        (U and V independent uniforms).
+# test_ptrs_pins_detect_wrong_constants shows that each single mistyped constant fails (i) or (ii).
+# ---------------------------------------------------------------------------------------------
+def _pooled_chi2(k, mean, n):
+    sp = pytest.importorskip("scipy.stats")
+    lo_k = int(max(0, math.floor(mean - 12 * math.sqrt(mean)) - 5))
+    hi_k = int(math.ceil(mean + 12 * math.sqrt(mean)) + 5)
+    ks = np.arange(lo_k, hi_k + 1)
+    exp = n * sp.poisson.pmf(ks, mean)
+    obs = np.bincount(np.clip(k, lo_k, hi_k) - lo_k, minlength=ks.size).astype(np.float64)
+    assert k.min() >= 0 and (k < lo_k).sum() + (k > hi_k).sum() == 0      # 12 sigma: nothing outside
+    # pool from both ends towards the mode until every bin expects >= 20
+    o, e, acc_o, acc_e = [], [], 0.0, 0.0
+    for oi, ei in zip(obs, exp):
+        acc_o += oi
+        acc_e += ei
+        if acc_e >= 20.0:
+            o.append(acc_o); e.append(acc_e); acc_o = acc_e = 0.0
+    o[-1] += acc_o
+    e[-1] += acc_e
+    o, e = np.array(o), np.array(e)
+    return float(((o - e) ** 2 / e).sum()), o.size - 1
+
+
+def _ptrs_constants(mean):
+    b = 0.931 + 2.53 * math.sqrt(mean)
+    return b, 1.1239 + 1.1328 / (b - 3.4), 0.9277 - 3.6224 / (b - 2.0)
+
+
+@pytest.mark.parametrize("mean", [10.0, 37.5, 1.0e3, 3.0e4, 7.0e4, 1.0e5])
+def test_poisson_ptrs_exact_pmf_and_acceptance(orc, mean):
+    n = 2_000_000
+    k, attempts, exit_ = orc.poisson_array(4242, 0, n, 3, mean, diagnostics=True)
+    assert np.array_equal(k[:200], [orc.poisson(4242, i, 3, mean) for i in range(200)])       # same draws as the scalar call
+    chi2, dof = _pooled_chi2(k, mean, n)
+    assert chi2 < dof + 4.5 * math.sqrt(2 * dof), (mean, chi2, dof)
+    b, inv_alpha, vr = _ptrs_constants(mean)
+    p = 1.0 / inv_alpha
+    se = math.sqrt((1 - p) / p ** 2 / n)                       # geometric number of attempts
+    assert abs(attempts.mean() - inv_alpha) < 4.5 * se, (mean, attempts.mean(), inv_alpha)
+    pf = 0.86 * vr
+    quick_first = ((attempts == 1) & (exit_ == 1)).mean()
+    assert abs(quick_first - pf) < 4.5 * math.sqrt(pf * (1 - pf) / n), (mean, quick_first, pf)
+
+
+def _ptrs_numpy(mean, n, rng, c):
+    """Hoermann's transformed rejection with squeeze, vectorised, with every constant taken from `c` -- only used to
+    show that the pins above have the power to see a single wrong constant (it is not the oracle)."""
+    sp = pytest.importorskip("scipy.special")
+    smu = math.sqrt(mean)
+    b = c["b0"] + c["b1"] * smu
+    a = c["a0"] + c["a1"] * b
+    inv_alpha = c["ia0"] + c["ia1"] / (b - c["ia2"])
+    vr = c["vr0"] - c["vr1"] / (b - c["vr2"])
+    out = np.full(n, -1, dtype=np.int64)
+    attempts = np.zeros(n, dtype=np.int64)
+    todo = np.arange(n)
+    while todo.size:
+        U = rng.random(todo.size) - 0.5
+        V = rng.random(todo.size)
+        attempts[todo] += 1
+        us = 0.5 - np.abs(U)
+        kf = np.floor((2.0 * a / us + b) * U + mean + c["shift"])
+        quick = (us >= c["s0"]) & (V <= vr)
+        rej = ~quick & ((kf < 0) | ((us < c["s1"]) & (V > us)))
+        full = ~quick & ~rej
+        ok = np.zeros(todo.size, dtype=bool)
+        kk = np.where(full, kf, 1.0)
+        ok[full] = (np.log(V[full]) + math.log(inv_alpha) - np.log(a / (us[full] ** 2) + b)
+                    <= -mean + kk[full] * math.log(mean) - sp.gammaln(kk[full] + 1.0))
+        acc = quick | ok
+        out[todo[acc]] = kf[acc].astype(np.int64)
+        todo = todo[~acc]
+    return out, attempts, inv_alpha
+
+
+PTRS_PUBLISHED = dict(b0=0.931, b1=2.53, a0=-0.059, a1=0.02483, ia0=1.1239, ia1=1.1328, ia2=3.4, vr0=0.9277, vr1=3.6224,
+                      vr2=2.0, shift=0.43, s0=0.07, s1=0.013)
+
+
+def test_ptrs_pins_detect_wrong_constants():
+    """Power of pins (i) and (ii): the published constants pass; a single mistyped constant that breaks the sampler
+    (a squeeze step that overrides the full comparison, or a hat that no longer dominates) fails one of them at
+    mean 1e3 or 3e4.  The full comparison V <= p(k) G'(U) / inv_alpha is exact for whatever k is proposed, so
+    constants that only move the hat inside its slack (e.g. the 0.43 shift, the 3.4 and 2.0 offsets) change the
+    efficiency, not the distribution: the pins rightly stay green for those, and they are not listed."""
+    n = 2_000_000
+
+    def verdict(c, mean, seed):
+        k, att, inv_alpha = _ptrs_numpy(mean, n, np.random.Generator(np.random.Philox(seed)), c)
+        chi2, dof = _pooled_chi2(k, mean, n) if (k.min() >= 0 and abs(k.mean() - mean) < 5) else (1e30, 1)
+        p = 1.0 / inv_alpha
+        se = math.sqrt((1 - p) / p ** 2 / n)
+        return chi2 < dof + 4.5 * math.sqrt(2 * dof) and abs(att.mean() - inv_alpha) < 4.5 * se
+    for mean in (1.0e3, 3.0e4):
+        assert verdict(PTRS_PUBLISHED, mean, 1)
+    mutations = dict(vr0=0.9727, s0=0.04, s1=0.031, b1=2.35, a1=0.02843, ia0=1.0239, b0=9.31, vr1=0.36224)
+    for j, (name, wrong) in enumerate(mutations.items()):
+        c = dict(PTRS_PUBLISHED, **{name: wrong})
+        assert not (verdict(c, 1.0e3, 100 + j) and verdict(c, 3.0e4, 200 + j)), (name, wrong)

@@ -36,22 +36,33 @@ def test_gradient_vs_mpmath_derivative_of_the_definition(orc, shape):
         assert abs(g[j] - float(ref)) <= 2e-9 * max(abs(float(ref)), 1.0 / inp.GRAD_SCALE[name] * 1e-3), (name, g[j], ref)
 
 
-def test_central_differences_converge_quadratically_to_the_analytic_gradient(orc):
+def test_fd_gradient_batch_layout_and_quadratic_convergence(orc):
+    """Row G (reading C6), orc.fd_gradient: the batch is theta, theta +/- h_j e_j in the order (mu, sigma, f, k); the
+    differences converge to the analytic gradient (pinned above by mpmath) like h^2 -- a wrong sign, index, step or
+    denominator fails one of the two checks."""
     # few events, none within the largest step of a join (the density is only C^1 there)
     x = np.array([5010.0, 5120.0, 5236.0, 5266.0, 5279.0, 5291.5, 5322.0, 5470.0])
     theta = inp.as_array(inp.P2)
     _, g = orc.nll_gradient(x, theta, LO, HI)
-    for j, name in enumerate(NAMES):
-        errs = []
-        for scale in (1.0, 0.5):
-            h = scale * 20 * inp.FD_STEPS[name]
+    idx, h0 = inp.fd_spec()
+    errs = []
+    for scale in (1.0, 0.5):
+        h = scale * 20 * h0
+        nll, fd = orc.fd_gradient(x, theta, idx, h, LO, HI)
+        for j in range(4):                                       # layout: plain NLLs at the displaced points
             tp, tm = theta.copy(), theta.copy()
-            tp[inp.IDX[name]] += h
-            tm[inp.IDX[name]] -= h
-            fd = (orc.nll(x, tp, LO, HI)[0] - orc.nll(x, tm, LO, HI)[0]) / (2 * h)
-            errs.append(fd - g[j])
-        assert abs(errs[0]) < 1e-3 * max(1.0, abs(g[j]))
-        assert 3.0 < errs[0] / errs[1] < 5.0, (name, errs)        # O(h^2): halving h divides the error by 4
+            tp[idx[j]] += h[j]
+            tm[idx[j]] -= h[j]
+            assert nll[2 * j + 1] == orc.nll(x, tp, LO, HI)[0] and nll[2 * j + 2] == orc.nll(x, tm, LO, HI)[0]
+        assert nll[0] == orc.nll(x, theta, LO, HI)[0]
+        errs.append(fd - g)
+    assert np.all(np.abs(errs[0]) < 1e-3 * np.maximum(1.0, np.abs(g)))
+    ratio = errs[0] / errs[1]
+    assert np.all((3.0 < ratio) & (ratio < 5.0)), ratio          # O(h^2): halving h divides the error by 4
+    # a subset of the parameters in another order
+    nll2, fd2 = orc.fd_gradient(x, theta, idx[[3, 0]], (20 * h0)[[3, 0]], LO, HI)
+    _, fd1 = orc.fd_gradient(x, theta, idx, 20 * h0, LO, HI)
+    assert np.array_equal(fd2, fd1[[3, 0]]) and nll2.size == 5
 
 
 def test_gradient_limits(orc):
