@@ -24,6 +24,10 @@ GEN = dict(mu=5280.0, sigma=15.0, **{"lambda": 1.0}, zeta=1.0, beta=0.0, a=2.0, 
 # second, general shape point (reading D2): non-half-integer order, beta != 0, asymmetric tails
 P2 = dict(mu=5280.0, sigma=15.0, **{"lambda": -1.3}, zeta=2.0, beta=0.01, a=1.5, n=2.5, a2=2.2, n2=4.0,
           f=0.3, k=-0.002)
+# zeta = 0 Student-t core (row f4, reading D3): T1 has the Upsilon example's lambda = -2, T2 the
+# delta = sigma branch (-1 <= lambda < 0) with beta != 0 and asymmetric tails
+T1 = dict(mu=5280.0, sigma=15.0, **{"lambda": -2.0}, zeta=0.0, beta=0.0, a=2.0, n=3.0, a2=2.0, n2=3.0, f=0.3, k=-0.002)
+T2 = dict(mu=5280.0, sigma=15.0, **{"lambda": -0.7}, zeta=0.0, beta=0.004, a=1.2, n=2.5, a2=1.8, n2=4.0, f=0.3, k=-0.002)
 
 FLOATED = ("mu", "sigma", "f", "k")                   # reading C6: order of the floated parameters
 FD_STEPS = dict(mu=0.01, sigma=0.01, f=1e-4, k=1e-6)  # reading C6: central-difference steps

@@ -218,13 +218,24 @@ static ld besselk_scaled_l(ld nu, ld x) {
 struct Shape {
   ld mu, sigma, lambda, zeta, beta, a, n, a2, n2;
   ld nu, delta, alpha;
+  int tcore;           /* 1: the zeta = 0 Student-t core below (no Bessel function) */
+  ld sigpow;           /* G(d; sigma) = sigma^sigpow g(d/sigma) e^{beta d}: nu (Bessel core), 2 nu (Student-t core) */
   ld d0, d1;           /* joins: -a sigma, +a2 sigma */
   ld logG0, logG1;     /* log core value at the joins */
   ld L0, L1;           /* log-derivative of the core at the joins */
   int status;          /* 0 ok, 1 basic domain, 2 join slope sign */
 };
 
+/* zeta -> 0 limit of the core for lambda < 0 (reading D3; ref. [10] of the paper,
+ * PAPER.md:450, and the Upsilon example's `Free('lb', -2.0, ...)` with no zeta).  With alpha -> 0,
+ * K_nu(z) -> Gamma(|nu|) 2^{|nu|-1} z^{-|nu|} (A&S 9.6.9) and nu = lambda - 1/2 < 0, so up to a constant factor
+ *     G(d) = (d^2 + delta^2)^{lambda - 1/2} e^{beta d}            (a Student-t core with -2 lambda degrees of freedom)
+ *     L(d) = G'/G = beta + (2 lambda - 1) d / (d^2 + delta^2)
+ * delta: the limit of sigma sqrt(zeta K_lambda(zeta)/K_{lambda+1}(zeta)) is sigma sqrt(-2 lambda - 2) for lambda < -1
+ * (then sigma^2 is still the variance of the symmetric core); for -1 <= lambda < 0 that limit is 0 (the variance
+ * diverges) and delta = sigma is taken as the scale (reading D3).  Tails, normalisation and likelihood are unchanged. */
 static ld core_logG(const Shape& s, ld d) {
+  if (s.tcore) return s.nu * logl(d * d + s.delta * s.delta) + s.beta * d;
   /* log G(d) = nu log r + beta d + log K_nu(alpha r),  r = sqrt(d^2+delta^2) */
   const ld r = sqrtl(d * d + s.delta * s.delta);
   const ld z = s.alpha * r;
@@ -232,6 +243,7 @@ static ld core_logG(const Shape& s, ld d) {
 }
 
 static ld core_logderiv(const Shape& s, ld d) {
+  if (s.tcore) return s.beta + 2 * s.nu * d / (d * d + s.delta * s.delta);
   /* L(d) = beta - alpha (d/r) K_{nu-1}(z)/K_nu(z) */
   const ld r = sqrtl(d * d + s.delta * s.delta);
   const ld z = s.alpha * r;
@@ -249,16 +261,24 @@ static Shape make_shape(const orc_params& p) {
   s.mu = p.mu; s.sigma = p.sigma; s.lambda = p.lambda; s.zeta = p.zeta; s.beta = p.beta;
   s.a = p.a; s.n = p.n; s.a2 = p.a2; s.n2 = p.n2;
   s.status = 0;
-  if (!finite_all(p) || !(p.sigma > 0) || !(p.zeta > 0) || !(p.a > 0) || !(p.a2 > 0) || !(p.n > 0) ||
-      !(p.n2 > 0) || !(p.f >= 0) || !(p.f <= 1)) {
+  s.tcore = (p.zeta == 0) ? 1 : 0;
+  if (!finite_all(p) || !(p.sigma > 0) || !(p.zeta > 0 || (p.zeta == 0 && p.lambda < 0)) || !(p.a > 0) || !(p.a2 > 0) ||
+      !(p.n > 0) || !(p.n2 > 0) || !(p.f >= 0) || !(p.f <= 1)) {
     s.status = 1;
     return s;
   }
   s.nu = s.lambda - 0.5L;
-  const ld Kl = besselk_scaled_l(s.lambda, s.zeta);
-  const ld Kl1 = besselk_scaled_l(s.lambda + 1, s.zeta);
-  s.delta = s.sigma * sqrtl(s.zeta * Kl / Kl1);
-  s.alpha = sqrtl(s.zeta * Kl1 / Kl) / s.sigma;
+  if (s.tcore) {
+    s.delta = (s.lambda < -1) ? s.sigma * sqrtl(-2 * s.lambda - 2) : s.sigma;
+    s.alpha = 0;
+    s.sigpow = 2 * s.nu;
+  } else {
+    const ld Kl = besselk_scaled_l(s.lambda, s.zeta);
+    const ld Kl1 = besselk_scaled_l(s.lambda + 1, s.zeta);
+    s.delta = s.sigma * sqrtl(s.zeta * Kl / Kl1);
+    s.alpha = sqrtl(s.zeta * Kl1 / Kl) / s.sigma;
+    s.sigpow = s.nu;
+  }
   s.d0 = -s.a * s.sigma;
   s.d1 = s.a2 * s.sigma;
   s.logG0 = core_logG(s, s.d0);
@@ -396,6 +416,8 @@ static ld nll_one(const double* x, int64_t n, const orc_params& p, ld lo, ld hi)
  *   d l / d mu    = w_S ( - dlogI/dd (x - mu) - d ln N_S / d mu )
  *   d l / d sigma = w_S ( dlogI/dsigma (x - mu) - d ln N_S / d sigma )
  * with (delta = sigma c1, alpha = c2 / sigma, d0 = -a sigma, d1 = a2 sigma; L = core log-derivative):
+ * (nu below stands for the power of sigma in G(d; sigma) = sigma^p g(d/sigma) e^{beta d}: p = nu for the Bessel core,
+ *  p = 2 nu for the zeta = 0 Student-t core -- Shape::sigpow)
  *   core   dlogI/dd = L(d)              dlogI/dsigma = nu/sigma + (d/sigma)(beta - L(d))
  *   left   dlogI/dd = L0 / u            dlogI/dsigma = nu/sigma - a beta + [ a L0 - (d-d0)(L0-beta)/sigma ] / u
  *   right  dlogI/dd = L1 / u            dlogI/dsigma = nu/sigma + a2 beta - [ a2 L1 + (d-d1)(L1-beta)/sigma ] / u
@@ -412,13 +434,13 @@ static ld dlogI_dd(const Shape& s, ld d) {
 static ld dlogI_dsigma(const Shape& s, ld d) {
   if (d < s.d0) {
     const ld u = 1 - (d - s.d0) * s.L0 / s.n;
-    return s.nu / s.sigma - s.a * s.beta + (s.a * s.L0 - (d - s.d0) * (s.L0 - s.beta) / s.sigma) / u;
+    return s.sigpow / s.sigma - s.a * s.beta + (s.a * s.L0 - (d - s.d0) * (s.L0 - s.beta) / s.sigma) / u;
   }
   if (d > s.d1) {
     const ld u = 1 - (d - s.d1) * s.L1 / s.n2;
-    return s.nu / s.sigma + s.a2 * s.beta - (s.a2 * s.L1 + (d - s.d1) * (s.L1 - s.beta) / s.sigma) / u;
+    return s.sigpow / s.sigma + s.a2 * s.beta - (s.a2 * s.L1 + (d - s.d1) * (s.L1 - s.beta) / s.sigma) / u;
   }
-  return s.nu / s.sigma + (d / s.sigma) * (s.beta - core_logderiv(s, d));
+  return s.sigpow / s.sigma + (d / s.sigma) * (s.beta - core_logderiv(s, d));
 }
 /* int_A^B I(d) dlogI/dsigma(d) e^{-logref} dd inside ONE region (smooth integrand), composite 20-point
  * Gauss-Legendre, panels doubled until stable */
