@@ -29,7 +29,7 @@
  *     work is enqueued.  CUDA launch errors are returned as IPA_ERR_CUDA (text: ipa_last_cuda_error).
  *   - Per-parameter-set DOMAIN errors do not fail the call: the set gets status != 0 in `status_dev`
  *     and NLL = +inf, so that a minimiser stepping outside the domain can recover.  Status values:
- *     0 ok; 1 basic domain (non-finite field, sigma<=0, zeta<=0, a<=0, a2<=0, n<=0, n2<=0, f outside
+ *     0 ok; 1 basic domain (non-finite field, sigma<=0, zeta<0, zeta==0 with lambda>=0, a<=0, a2<=0, n<=0, n2<=0, f outside
  *     [0,1]); 2 join slope sign (L(d0)<=0 or L(d1)>=0: the power-law tail does not exist);
  *     3 internal numerical failure (normalisation not finite or not positive); 4 (ipa_nll_grad_eval only)
  *     f == 0 or f == 1.
@@ -56,7 +56,9 @@ typedef struct {
   double mu;     /* peak position */
   double sigma;  /* core width: the untruncated symmetric core has variance sigma^2 */
   double lambda; /* generalised-hyperbolic index; Bessel order nu = lambda - 1/2 */
-  double zeta;   /* > 0; shape of the core (zeta -> inf: Gaussian) */
+  double zeta;   /* > 0: shape of the Bessel core (zeta -> inf: Gaussian); == 0 with lambda < 0: the zeta -> 0 limit, a
+                    Student-t core (d^2+delta^2)^(lambda-1/2) e^(beta d), delta = sigma sqrt(-2 lambda-2) for lambda < -1,
+                    else sigma (PAPER.md:226-236 `lb = -2.0` without zeta, ref. [10] at PAPER.md:450; reading D3) */
   double beta;   /* asymmetry, exp(beta d) factor */
   double a;      /* left join at d0 = -a sigma, a > 0 */
   double n;      /* left tail power, > 0 */

@@ -108,8 +108,8 @@ IPA_HD int ipa_warp_max(int v) {
 // Core shape value of E events: t = tA sqrt(d^2 + delta^2) + tB, Horner over groups of 4 coefficients
 // (two 128-bit uniform shared loads per group; a[] is zero above the degree) down to a[1], times t.
 // FP64 per event: q 1 + sqrt 5 + t 1 + 4 ceil((D+1)/4).
-template <int E>
-IPA_HD void ipa_core_shape(const IpaSetConsts& c, const double (&d)[E], double (&V)[E]) {
+template <int E, class Tab>
+IPA_HD void ipa_core_shape(const IpaSetConsts& c, const double (&d)[E], double (&V)[E], const Tab* tab) {
   if (c.mode == 0) {
     const double d2 = c.delta2, tA = c.tA, tB = c.tB;
     double t[E], P[E];
@@ -135,6 +135,11 @@ IPA_HD void ipa_core_shape(const IpaSetConsts& c, const double (&d)[E], double (
       P[e] = fma(P[e], t[e], a1);
       V[e] = P[e] * t[e];
     }
+  } else if (c.mode == 2) {
+    // Student-t core (zeta == 0, row f4): V = nu log(d^2 + delta^2), one logarithm, no polynomial
+    const double d2 = c.delta2, nu = c.nu;
+#pragma unroll
+    for (int e = 0; e < E; ++e) V[e] = nu * ipa_flog(fma(d[e], d[e], d2), tab);
   } else {
     // direct mode (shapes the polynomial cannot cover): per-event Bessel evaluation, out of line
     double dt[E], Pt[E];
@@ -163,7 +168,7 @@ IPA_HD void ipa_tail_shape(const IpaSetConsts& c, bool right, const double (&d)[
 template <int E, class Tab>
 IPA_HD void ipa_mixed_shape(const IpaSetConsts& c, const double (&d)[E], double (&V)[E], const Tab* tab) {
   const double d0 = c.d0, d1 = c.d1;
-  ipa_core_shape<E>(c, d, V);
+  ipa_core_shape<E>(c, d, V, tab);
 #pragma unroll
   for (int e = 0; e < E; ++e) {
     const bool left = d[e] < d0, right = d[e] > d1;
@@ -188,7 +193,7 @@ IPA_HD int ipa_shape_stage(const IpaSetConsts& c, const double (&x)[E], double (
   for (int e = 0; e < E; ++e) d[e] = x[e] - mu;
   const bool sane = hmin > 0 && hmax < 0x7ff00000;      // positive, finite events only
   if (sane && hmin > c.hxl && hmax < c.hxr) {
-    ipa_core_shape<E>(c, d, V);
+    ipa_core_shape<E>(c, d, V, tab);
     return IPA_REG_CORE;
   }
   if (sane && hmax < c.hxl) { ipa_tail_shape<E>(c, false, d, V, tab); return IPA_REG_LEFT; }
@@ -254,7 +259,7 @@ IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l
   for (int e = 0; e < E; ++e) d[e] = x[e] - mu;
   const bool sane = hmin > 0 && hmax < 0x7ff00000;
   if (sane && hmin > c.hxl && hmax < c.hxr) {
-    ipa_core_shape<E>(c, d, V);
+    ipa_core_shape<E>(c, d, V, tab);
     ipa_member_stage_r<E, IPA_REG_CORE>(c, d, V, l, tab);
   } else if (sane && hmax < c.hxl) {
     ipa_tail_shape<E>(c, false, d, V, tab);
@@ -604,7 +609,13 @@ IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&
       if (d[e] < c.d0) ipa_grad_tail<Tab>(c, false, d[e], D[e], dd[e], ds[e], tab);
       else if (d[e] > c.d1) ipa_grad_tail<Tab>(c, true, d[e], D[e], dd[e], ds[e], tab);
       else if (c.mode == 0) ipa_grad_core<Tab>(c, d[e], D[e], dd[e], ds[e]);
-      else {   // direct mode: Bessel functions per event (slow path)
+      else if (c.mode == 2) {   // Student-t core: log G = nu log q + beta d, L - beta = 2 nu d / q
+        const double q = fma(d[e], d[e], c.delta2);
+        const double Lmb = 2.0 * c.nu * d[e] * ipa_frcp(q);
+        D[e] = fma(c.bmk, d[e], fma(c.nu, ipa_flog(q, tab), c.a[0]));
+        dd[e] = c.beta + Lmb;
+        ds[e] = fma(-d[e] * c.invsig, Lmb, c.nuosig);
+      } else {   // direct mode: Bessel functions per event (slow path)
         const double r = sqrt(fma(d[e], d[e], c.delta2)), z = c.alpha * r;
         const double Lmb = -c.alpha * (d[e] / r) * ipa_besselk_scaled(c.nu - 1.0, z) / ipa_besselk_scaled(c.nu, z);
         D[e] = fma(c.bmk, d[e], ipa_direct_H(c.nu, z) + c.a[0]);
@@ -797,6 +808,7 @@ __global__ void ipa_seg_finalize_kernel(const double* __restrict__ partials, con
 IPA_HD double ipa_logI_rec(const IpaSetConsts& c, double d) {
   if (d < c.d0) return c.logG0 - c.n0 * log(fma(c.uA0, d, c.uB0));
   if (d > c.d1) return c.logG1 - c.n1 * log(fma(c.uA1, d, c.uB1));
+  if (c.mode == 2) return fma(c.nu, log(fma(d, d, c.delta2)), c.beta * d);
   const double r = sqrt(fma(d, d, c.delta2));
   double H;
   if (c.mode == 0) {

@@ -99,6 +99,9 @@ IPA_HD double ipa_table_partial(const IpaProWork& w, int ord, double z, int sub)
   return s;
 }
 
+// mode 2 (zeta == 0, lambda < 0: row f4, reading D3) is the Student-t core G = (d^2 + delta^2)^nu e^{beta d}, the zeta -> 0
+// limit of the Bessel core: no Bessel function, no polynomial; G is homogeneous of degree 2 nu in sigma (nu otherwise)
+IPA_HD double ipa_sigpow(const IpaProWork& w) { return w.mode == 2 ? 2.0 * w.nu : w.nu; }
 // H(z) = log(z^nu K_nu(z)) from the raw polynomial, r given
 IPA_HD double ipa_core_H(const IpaProWork& w, double r) {
   const double z = w.alpha * r;
@@ -107,12 +110,14 @@ IPA_HD double ipa_core_H(const IpaProWork& w, double r) {
 }
 // log G(d) = nu log r + beta d + log K_nu(alpha r) = H - nu log alpha + beta d
 IPA_HD double ipa_core_logG(const IpaProWork& w, double d) {
+  if (w.mode == 2) return fma(w.nu, log(fma(d, d, w.delta * w.delta)), w.p.beta * d);
   const double r = sqrt(fma(d, d, w.delta * w.delta));
   return ipa_core_H(w, r) - w.nu * log(w.alpha) + w.p.beta * d;
 }
 // L(d) - beta = -alpha (d/r) K_{nu-1}/K_nu = alpha (d/r) H'(z)  (H' = -K_{nu-1}/K_nu): derivative of the fitted
 // polynomial, dH/dz = (1/zh) sum_j j a_j t^{j-1}; direct mode evaluates the Bessel ratio
 IPA_HD double ipa_core_Lmb(const IpaProWork& w, double d) {
+  if (w.mode == 2) return 2.0 * w.nu * d / fma(d, d, w.delta * w.delta);
   const double r = sqrt(fma(d, d, w.delta * w.delta));
   const double z = w.alpha * r;
   double Hp;
@@ -147,11 +152,11 @@ IPA_HD void ipa_pro_phase0(IpaProWork& w, int tid) {
   const double* v = &p.mu;
   bool ok = true;
   for (int i = 0; i < 11; ++i) ok = ok && ipa_finite(v[i]);
-  ok = ok && (p.sigma > 0.0) && (p.zeta > 0.0) && (p.a > 0.0) && (p.a2 > 0.0) && (p.n > 0.0) && (p.n2 > 0.0) &&
+  ok = ok && (p.sigma > 0.0) && (p.zeta > 0.0 || (p.zeta == 0.0 && p.lambda < 0.0)) && (p.a > 0.0) && (p.a2 > 0.0) && (p.n > 0.0) && (p.n2 > 0.0) &&
        (p.f >= 0.0) && (p.f <= 1.0);
   w.status = ok ? 0 : 1;
   w.nu = p.lambda - 0.5;
-  w.mode = 0;
+  w.mode = (p.zeta == 0.0) ? 2 : 0;
   w.degree = 0;
   w.npanel = 0;
 }
@@ -161,6 +166,7 @@ IPA_HD void ipa_pro_phase0(IpaProWork& w, int tid) {
 IPA_HD void ipa_pro_phase1(IpaProWork& w, int tid) {
   if (w.status) return;
   if (tid < 64) {
+    if (w.mode == 2) return;
     const int which = tid >> 5, lane = tid & 31;
     const double ord = fabs(w.p.lambda + (double)which);
     const double x = w.p.zeta;
@@ -183,6 +189,20 @@ IPA_HD void ipa_pro_phase1(IpaProWork& w, int tid) {
 IPA_HD void ipa_pro_phase2(IpaProWork& w, int tid) {
   if (w.status || tid != 0) return;
   const ipa_params& p = w.p;
+  if (w.mode == 2) {
+    // Student-t core: delta = lim sigma sqrt(zeta K_l/K_{l+1}) = sigma sqrt(-2 lambda - 2) for lambda < -1, else sigma
+    w.delta = (p.lambda < -1.0) ? p.sigma * sqrt(-2.0 * p.lambda - 2.0) : p.sigma;
+    w.alpha = 0.0;
+    w.d0 = -p.a * p.sigma;
+    w.d1 = p.a2 * p.sigma;
+    w.r0 = sqrt(fma(w.d0, w.d0, w.delta * w.delta));
+    w.r1 = sqrt(fma(w.d1, w.d1, w.delta * w.delta));
+    w.z0 = w.z1 = 0.0;
+    w.zc = 0.0; w.zh = 1.0;
+    w.h = 1.0; w.J = 0;
+    if (!ipa_finite(w.delta) || !(w.delta > 0.0)) w.status = 3;
+    return;
+  }
   double s0 = 0.5, s1 = 0.5;
   for (int l = 0; l < 32; ++l) { s0 += w.part[0][l]; s1 += w.part[1][l]; }
   w.Kl = s0 * ipa_trap_step(fabs(p.lambda), p.zeta);
@@ -215,7 +235,7 @@ IPA_HD void ipa_pro_phase2(IpaProWork& w, int tid) {
 
 // phase 3: trapezoid table (all threads)
 IPA_HD void ipa_pro_phase3(IpaProWork& w, int tid, int nthr) {
-  if (w.status) return;
+  if (w.status || w.mode == 2) return;
   for (int m = tid; m < 4 * IPA_MCHEB; m += nthr) w.ctab[m] = cos(3.14159265358979323846 * (double)m / (double)(2 * IPA_MCHEB));
   for (int j = tid; j < w.J; j += nthr) {
     const double t = (double)j * w.h;
@@ -236,7 +256,7 @@ IPA_HD double ipa_pro_task_z(const IpaProWork& w, int q) {
 
 // phase 4: Bessel tasks, IPA_SUB threads each
 IPA_HD void ipa_pro_phase4(IpaProWork& w, int tid) {
-  if (w.status) return;
+  if (w.status || w.mode == 2) return;
   const int q = tid / IPA_SUB, sub = tid % IPA_SUB;
   if (q >= IPA_NBTASK) return;
   const int ord = (q >= IPA_MCHEB + 2) ? 1 : 0;
@@ -245,7 +265,7 @@ IPA_HD void ipa_pro_phase4(IpaProWork& w, int tid) {
 
 // phase 5: combine partial sums; H at the Chebyshev nodes
 IPA_HD void ipa_pro_phase5(IpaProWork& w, int tid) {
-  if (w.status || tid >= IPA_NBTASK) return;
+  if (w.status || w.mode == 2 || tid >= IPA_NBTASK) return;
   double s = 0.5;
   for (int i = 0; i < IPA_SUB; ++i) s += w.bpart[tid][i];
   const double Ks = s * w.h;
@@ -258,7 +278,7 @@ IPA_HD void ipa_pro_phase5(IpaProWork& w, int tid) {
 
 // phase 6: Chebyshev coefficients c_j = (2/M) sum_i H_i cos(pi j (i+1/2)/M), c_0 halved
 IPA_HD void ipa_pro_phase6(IpaProWork& w, int tid) {
-  if (w.status || tid >= IPA_MCHEB) return;
+  if (w.status || w.mode == 2 || tid >= IPA_MCHEB) return;
   const int M = IPA_MCHEB;
   double s = 0.0;
   for (int i = 0; i < M; ++i) {
@@ -272,6 +292,16 @@ IPA_HD void ipa_pro_phase6(IpaProWork& w, int tid) {
 IPA_HD void ipa_pro_phase7(IpaProWork& w, int tid) {
   if (w.status) return;
   const ipa_params& p = w.p;
+  if (w.mode == 2) {
+    if (tid == 32) {
+      w.logG0 = fma(w.nu, log(w.r0 * w.r0), p.beta * w.d0);
+      w.L0 = p.beta + 2.0 * w.nu * w.d0 / (w.r0 * w.r0);
+    } else if (tid == 64) {
+      w.logG1 = fma(w.nu, log(w.r1 * w.r1), p.beta * w.d1);
+      w.L1 = p.beta + 2.0 * w.nu * w.d1 / (w.r1 * w.r1);
+    }
+    return;
+  }
   if (tid == 0) {
     double scale = 1.0;
     for (int i = 0; i < IPA_MCHEB; ++i) scale = fmax(scale, fabs(w.H[i]));
@@ -361,7 +391,7 @@ IPA_HD void ipa_pro_phase10(IpaProWork& w, int tid, int nthr) {
     const double d = c + hl * w.glx[i];
     const double g = w.glw[i] * hl * exp(ipa_core_logG(w, d) - w.logref);
     w.pval[q] = g;
-    w.pval2[q] = w.want_grad ? g * (w.nu / w.p.sigma - (d / w.p.sigma) * ipa_core_Lmb(w, d)) : 0.0;   // G dlogG/dsigma
+    w.pval2[q] = w.want_grad ? g * (ipa_sigpow(w) / w.p.sigma - (d / w.p.sigma) * ipa_core_Lmb(w, d)) : 0.0;   // G dlogG/dsigma
   }
 }
 IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
@@ -382,7 +412,7 @@ IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
       const double pre = exp(w.logG0 - w.logref) * (p.n / w.L0);
       const double F = ipa_powint(ul, p.n) - ipa_powint(ur, p.n);
       const double F1 = w.want_grad ? ipa_powint(ul, p.n + 1.0) - ipa_powint(ur, p.n + 1.0) : 0.0;
-      const double A = w.nu / p.sigma - p.a * p.beta, c = p.n * (w.L0 - p.beta) / (w.L0 * p.sigma);
+      const double A = ipa_sigpow(w) / p.sigma - p.a * p.beta, c = p.n * (w.L0 - p.beta) / (w.L0 * p.sigma);
       left = pre * F;
       left2 = pre * ((A + c) * F + (p.a * w.L0 - c) * F1);
     }
@@ -396,7 +426,7 @@ IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
       const double pre = exp(w.logG1 - w.logref) * (p.n2 / (-w.L1));
       const double F = ipa_powint(uh, p.n2) - ipa_powint(ul, p.n2);
       const double F1 = w.want_grad ? ipa_powint(uh, p.n2 + 1.0) - ipa_powint(ul, p.n2 + 1.0) : 0.0;
-      const double A = w.nu / p.sigma + p.a2 * p.beta, c = p.n2 * (w.L1 - p.beta) / (w.L1 * p.sigma);
+      const double A = ipa_sigpow(w) / p.sigma + p.a2 * p.beta, c = p.n2 * (w.L1 - p.beta) / (w.L1 * p.sigma);
       right = pre * F;
       right2 = pre * ((A + c) * F - (p.a2 * w.L1 + c) * F1);
     }
@@ -415,7 +445,7 @@ IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
     w.logf = (p.f > 0.0) ? log(p.f) : 0.0;
     w.log1mf = (p.f < 1.0) ? log1p(-p.f) : 0.0;
   } else if (tid == 160) {
-    w.nulogalpha = w.nu * log(w.alpha);
+    w.nulogalpha = (w.mode == 2) ? 0.0 : w.nu * log(w.alpha);
   } else if (tid == 192) {
     w.expref = exp(w.logref);
   }
@@ -459,14 +489,14 @@ IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
   o.cDir = cS - eB0 - w.nulogalpha;
   o.fsig = p.f; o.kraw = p.k;
   o.beta = p.beta; o.logG0 = w.logG0; o.logG1 = w.logG1; o.logNS = logNS; o.logref = w.logref;
-  o.araw0 = w.mode ? 0.0 : w.araw[0];
+  o.araw0 = w.mode ? 0.0 : w.araw[0];   // modes 1, 2: no polynomial
   double core2 = 0.0;
   for (int i = 0; i < w.npanel; ++i) core2 += w.psum2[i];
   o.dlnNS_dmu = (w.Iedge_l - w.Iedge_h) / NSr;
   o.dlnNS_dsig = (w.tl_left2 + core2 + w.tl_right2) / NSr;
   o.dlnNB_dk = pure ? 0.0 : w.dlnNB_dk;
-  o.nuosig = w.nu / p.sigma; o.invsig = 1.0 / p.sigma; o.mulo = p.mu - w.lo; o.L0 = w.L0; o.L1 = w.L1;
-  o.A0 = w.nu / p.sigma - p.a * p.beta; o.A1 = w.nu / p.sigma + p.a2 * p.beta;
+  o.nuosig = ipa_sigpow(w) / p.sigma; o.invsig = 1.0 / p.sigma; o.mulo = p.mu - w.lo; o.L0 = w.L0; o.L1 = w.L1;
+  o.A0 = o.nuosig - p.a * p.beta; o.A1 = o.nuosig + p.a2 * p.beta;
   o.aL0 = p.a * w.L0; o.a2L1 = p.a2 * w.L1;
   o.c0s = (w.L0 - p.beta) / p.sigma; o.c1s = (w.L1 - p.beta) / p.sigma;
   o.invf = 1.0 / p.f; o.inv1mf = 1.0 / (1.0 - p.f);

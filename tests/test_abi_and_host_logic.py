@@ -121,20 +121,21 @@ def test_device_bessel_vs_mpmath(emu):
 
 
 @pytest.mark.parametrize("policy", [0, 1])
-@pytest.mark.parametrize("shape", ["P1", "P2", "direct"])
+@pytest.mark.parametrize("shape", ["P1", "P2", "direct", "T1", "T2"])
 def test_device_math_vs_oracle(emu, orc, shape, policy):
-    P = {"P1": inp.GEN, "P2": inp.P2, "direct": dict(inp.GEN, zeta=0.2)}[shape]
+    P = {"P1": inp.GEN, "P2": inp.P2, "direct": dict(inp.GEN, zeta=0.2), "T1": inp.T1, "T2": inp.T2}[shape]
     p = inp.as_array(P)
     out = np.zeros(14)
     emu.emu_consts(p.ctypes.data, LO, HI, policy, out.ctypes.data)
     st, sc = orc.shape_consts(P)
     _, nm = orc.norm(P, LO, HI)
     assert out[0] == 0 and st == 0
-    assert out[2] == (1 if shape == "direct" else 0)
+    assert out[2] == {"direct": 1, "T1": 2, "T2": 2}.get(shape, 0)      # mode 2: zeta = 0 Student-t core (row f4)
     if shape == "P1":
         assert out[1] == (1 if policy == 0 else 31)   # K_{1/2}: H(z) is linear in z
     assert abs(out[3] / nm["NS"] - 1) <= 5e-14 and abs(out[4] / nm["NB"] - 1) <= 1e-15
-    assert abs(np.sqrt(out[5]) / sc["delta"] - 1) <= 1e-14 and abs(out[6] / sc["alpha"] - 1) <= 1e-14
+    assert abs(np.sqrt(out[5]) / sc["delta"] - 1) <= 1e-14
+    assert abs(out[6] / sc["alpha"] - 1) <= 1e-14 if sc["alpha"] else out[6] == 0.0
     assert abs(out[7] - sc["logG0"]) <= 1e-13 and abs(out[9] / sc["L0"] - 1) <= 1e-13 and abs(out[10] / sc["L1"] - 1) <= 1e-13
     # row f1: derivatives of the normalisations (d ln N_S / d mu, d ln N_S / d sigma, d ln N_B / d k)
     nd = orc.norm_derivs(P, LO, HI)
@@ -188,10 +189,10 @@ def test_chebyshev_integer_table(emu):
     assert emu.emu_cheb_table_mismatches() == 0
 
 
-@pytest.mark.parametrize("shape", ["P1", "P2", "direct"])
+@pytest.mark.parametrize("shape", ["P1", "P2", "direct", "T1", "T2"])
 def test_device_gradient_math_vs_oracle(emu, orc, shape):
     """Row f1: the CUDA path's per-event gradient arithmetic (host build) against the oracle's analytic gradient."""
-    P = {"P1": inp.GEN, "P2": inp.P2, "direct": dict(inp.GEN, zeta=0.2)}[shape]
+    P = {"P1": inp.GEN, "P2": inp.P2, "direct": dict(inp.GEN, zeta=0.2), "T1": inp.T1, "T2": inp.T2}[shape]
     p = inp.as_array(P)
     n = 3000 if shape != "direct" else 300
     for x in (inp.standin_masses(11, n), np.sort(inp.standin_masses(12, n))):      # mixed and region-uniform groups

@@ -53,10 +53,10 @@ def x1(orc):
     return orc.generate_mixture(1, 10000, inp.GEN, LO, HI)
 
 
-@pytest.mark.parametrize("shape", ["P1", "P2"])
+@pytest.mark.parametrize("shape", ["P1", "P2", "T1", "T2"])     # T1, T2: zeta = 0 Student-t core (row f4, reading D3)
 @pytest.mark.parametrize("policy", [0, 1])
 def test_config1_logpdf_nll_gradient(ipa, torch_, orc, x1, shape, policy):
-    theta = inp.GEN if shape == "P1" else inp.P2
+    theta = {"P1": inp.GEN, "P2": inp.P2, "T1": inp.T1, "T2": inp.T2}[shape]
     batch, _ = inp.fd_batch(theta)
     idx, h = inp.fd_spec()
     xd = dev(torch_, x1)
@@ -608,6 +608,43 @@ def test_analytic_gradient_vs_oracle(ipa, torch_, orc, x1):
             assert grad_ok(grad[i], ref_g), (i, grad[i], ref_g)
 
 
+def test_student_t_core_all_entry_points(ipa, torch_, orc, x1):
+    """Row f4, reading D3: the zeta = 0 Student-t core through every unbinned entry point -- sorted (region-uniform
+    warps) and as-generated layouts, a batch mixing Bessel and Student-t sets, the analytic gradient, the segmented
+    call, ipa_norm, the domain rule (zeta = 0 needs lambda < 0) and the generator."""
+    sets = [inp.T1, inp.GEN, inp.T2, dict(inp.T1, **{"lambda": 0.5}), dict(inp.T2, f=0.2, k=-0.001)]
+    for x in (x1, np.sort(x1)):
+        xd = dev(torch_, x)
+        nll, lp, st = ipa.ipa_nll_eval(xd, sets, LO, HI, want_logpdf=True)
+        gn, grad, gst = ipa.ipa_nll_grad_eval(xd, [inp.T1, inp.T2], LO, HI)
+        torch_.cuda.synchronize()
+        nll, lp, st = nll.cpu().numpy(), lp.cpu().numpy(), st.cpu().numpy()
+        assert list(st) == [0, 0, 0, 1, 0] and np.isposinf(nll[3]) and np.isnan(lp[3]).all()
+        for i in (0, 1, 2, 4):
+            assert np.abs(lp[i] - orc.logpdf(x, sets[i], LO, HI)).max() <= 1e-10
+            ref = orc.nll(x, sets[i], LO, HI)[0]
+            assert abs(nll[i] - ref) <= 1e-10 * abs(ref)
+        for i, th in enumerate((inp.T1, inp.T2)):
+            ref_nll, ref_g = orc.nll_gradient(x, th, LO, HI)
+            assert gst[i].item() == 0 and abs(gn[i].item() - ref_nll) <= 1e-10 * abs(ref_nll)
+            assert grad_ok(grad[i].cpu().numpy(), ref_g), (i, grad[i], ref_g)
+    ns, nb, st = ipa.ipa_norm([inp.T1, inp.T2, dict(inp.T1, mu=5700.0, n=1.0)], LO, HI)
+    torch_.cuda.synchronize()
+    for i, th in enumerate((inp.T1, inp.T2, dict(inp.T1, mu=5700.0, n=1.0))):
+        _, nrm = orc.norm(th, LO, HI)
+        assert st[i].item() == 0 and abs(ns[i].item() / nrm["NS"] - 1) <= 2e-13 and abs(nb[i].item() / nrm["NB"] - 1) <= 1e-14
+    off = np.array([0, 3000, 3000, 10000], dtype=np.int64)
+    seg, sst = ipa.ipa_nll_eval_segmented(dev(torch_, x1), dev(torch_, off), [inp.T1, inp.GEN, inp.T2], LO, HI)
+    torch_.cuda.synchronize()
+    ref = orc.nll_segmented(x1, off, [inp.T1, inp.GEN, inp.T2], LO, HI)
+    assert np.all(np.abs(seg.cpu().numpy() - ref) <= 1e-10 * np.abs(ref))
+    for th, seed in ((inp.T1, 41), (inp.T2, 42)):
+        xg, _, ovf = ipa.ipa_toy_generate([seed], th, -1.0, -1.0, LO, HI, 20000)
+        torch_.cuda.synchronize()
+        assert ovf.item() == 0
+        mismatches(xg.cpu().numpy(), orc.generate_mixture(seed, 20000, th, LO, HI), f"Student-t mixture seed {seed}")
+
+
 def test_analytic_gradient_1e6_and_fit_minimum(ipa, torch_, orc):
     n = 1_000_000
     x = orc.generate_mixture(2, n, inp.GEN, LO, HI)
@@ -781,3 +818,67 @@ def test_repeatability_stress(ipa, torch_, x1):
     for _ in range(30):
         for a, b in zip(first, run()):
             assert torch_.equal(a, b)
+
+
+def test_no_write_outside_the_outputs(ipa, torch_, x1):
+    """Bounds evidence without memcheck (profiles/r02_sanitizer.md): every output of the main calls is carved out of
+    ONE arena pre-filled with a canary byte, with guard zones in between; after the calls (through the raw C ABI, exact
+    sizes, ragged n) every byte outside the outputs still holds the canary and every output byte was written where the
+    call promises a value."""
+    import ctypes as C
+    L = ipa.lib()
+    CAN = 0xA5
+    arena = torch_.full((1 << 22,), CAN, dtype=torch_.uint8, device="cuda")
+    cursor, taken = [4096], []
+
+    def carve(nbytes, align=256):
+        start = (cursor[0] + align - 1) // align * align
+        cursor[0] = start + nbytes + 512                       # 512-byte guard zone after every output
+        taken.append((start, start + nbytes))
+        return arena[start:start + nbytes]
+
+    def ptr(t):
+        return C.c_void_p(t.data_ptr())
+
+    n, K, T = 4099, 2, 5
+    xd = dev(torch_, x1[:n])
+    P = ipa.pack_params([inp.GEN, inp.P2])
+    rng = ipa.binding._Range(LO, HI)
+    ws = ipa.workspace(n, 8)
+    nll, lp, st = carve(8 * K), carve(8 * K * n), carve(4 * K)
+    assert L.ipa_nll_eval(ptr(xd), n, P.ctypes.data_as(C.c_void_p), K, rng, ptr(nll), ptr(lp), ptr(st), None, ptr(ws),
+                          ws.numel(), None) == 0
+    gn, gg, gs = carve(8 * K), carve(8 * 4 * K), carve(4 * K)
+    assert L.ipa_nll_grad_eval(ptr(xd), n, P.ctypes.data_as(C.c_void_p), K, rng, ptr(gn), ptr(gg), ptr(gs), None, ptr(ws),
+                               ws.numel(), None) == 0
+    off = dev(torch_, np.array([0, 7, 7, 1030, 4000, n], dtype=np.int64))
+    PT = ipa.pack_params(inp.toy_param_sets(T, seed=3))
+    sn, ss = carve(8 * T), carve(4 * T)
+    assert L.ipa_nll_eval_segmented(ptr(xd), ptr(off), T, PT.ctypes.data_as(C.c_void_p), rng, ptr(sn), ptr(ss), None, ptr(ws),
+                                    ws.numel(), None) == 0
+    xp = carve(8 * n)
+    wsp = torch_.empty(ipa.ipa_prepare_workspace_bytes(n, 0), dtype=torch_.uint8, device="cuda")
+    assert L.ipa_events_prepare(ptr(xd), n, None, 0, rng, ptr(xp), ptr(wsp), wsp.numel(), None) == 0
+    xq = carve(8 * n)
+    assert L.ipa_events_prepare(ptr(xd), n, ptr(off), T, rng, ptr(xq), ptr(wsp), wsp.numel(), None) == 0
+    hist = carve(8 * 1000)
+    assert L.ipa_hist_fill(ptr(xd), n, rng, 1000, ptr(hist), None) == 0
+    cap = 3001
+    xg, og, ov, sg = carve(8 * cap), carve(8 * 2), carve(4), carve(4)
+    seeds = np.array([9], dtype=np.uint64)
+    PG = ipa.pack_params(inp.GEN)
+    assert L.ipa_toy_generate(seeds.ctypes.data_as(C.c_void_p), 1, PG.ctypes.data_as(C.c_void_p), 1, C.c_double(-1.0),
+                              C.c_double(-1.0), rng, cap, ptr(xg), ptr(og), ptr(ov), ptr(sg), None, ptr(ws), ws.numel(), None) == 0
+    torch_.cuda.synchronize()
+    host = arena.cpu().numpy()
+    mask = np.ones(host.size, dtype=bool)
+    for a, b in taken:
+        mask[a:b] = False
+    assert (host[mask] == CAN).all(), "a kernel wrote outside its output"
+    # the promised outputs were all written (a double made of canary bytes is a fixed finite pattern)
+    can8 = np.frombuffer(bytes([CAN] * 8), dtype=np.float64)[0]
+    for t in (nll, lp, gn, gg, sn, xp, xq, xg):
+        v = t.cpu().numpy().view(np.float64)
+        assert not (v == can8).any()
+    assert np.array_equal(np.sort(xp.cpu().numpy().view(np.float64)), np.sort(x1[:n]))
+    assert int(hist.cpu().numpy().view(np.uint64).sum()) == n
