@@ -39,6 +39,7 @@ def lib():
         L.orc_poisson.restype = i64; L.orc_poisson.argtypes = [u64, u64, u32, d]
         L.orc_poisson_array.restype = None; L.orc_poisson_array.argtypes = [u64, u64, i64, u32, d, vp, vp]
         L.orc_generate_mixture.restype = i32; L.orc_generate_mixture.argtypes = [u64, i64, vp, d, d, vp]
+        L.orc_generate_signal_diag.restype = i32; L.orc_generate_signal_diag.argtypes = [u64, i64, vp, d, d, vp, vp, vp]
         L.orc_toy_generate.restype = i32
         L.orc_toy_generate.argtypes = [vp, i64, vp, i32, d, d, d, d, i64, vp, vp]
         L.orc_hist_fill.restype = None; L.orc_hist_fill.argtypes = [vp, i64, d, d, i32, vp]
@@ -203,6 +204,18 @@ def generate_mixture(seed, n, p, lo, hi):
     st = lib().orc_generate_mixture(int(seed), int(n), _p(P), float(lo), float(hi), _p(x))
     assert st == 0, st
     return x
+
+
+def generate_signal_diag(seed, n, p, lo, hi):
+    """n signal draws (f ignored) -> (x[n], attempts per event, envelope violated?, envelope weight / N_S,
+    max over a dense grid of log G - log(box height))."""
+    P = pack_params(p)
+    x = np.empty(int(n))
+    diag = np.zeros(2, dtype=np.int64)
+    env = np.zeros(2)
+    st = lib().orc_generate_signal_diag(int(seed), int(n), _p(P), float(lo), float(hi), _p(x), _p(diag), _p(env))
+    assert st == 0, st
+    return x, diag[0] / max(int(n), 1), bool(diag[1]), float(env[0]), float(env[1])
 
 
 def toy_generate(seeds, gen, mean_sig, mean_bkg, lo, hi, offsets_only=False):

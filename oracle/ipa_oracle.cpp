@@ -588,25 +588,107 @@ static int64_t poisson_draw(uint64_t seed, uint64_t slot, uint32_t stream, doubl
   }
 }
 
-/* envelope of the signal accept-reject: log of max I over the range (reading D13) */
-static ld log_I_max(const Shape& s, ld lo, ld hi) {
-  if (s.beta == 0 && lo <= s.mu && s.mu <= hi) return log_I(s, 0);
-  ld best = -INFINITY;
-  for (int j = 0; j < 4096; ++j) {
-    const ld x = lo + (j + 0.5L) * (hi - lo) / 4096;
-    best = std::max(best, log_I(s, x - s.mu));
+/* ------------------------------------------------------------------------------------------
+ * Signal draws (reading D13, revised in round 2; PAPER.md:343-351 says only "accept-reject"): accept-reject under a
+ * PIECEWISE envelope that is a true upper bound of I on the range [lo, hi] (d = x - mu in [dl, dh]):
+ *   left tail  [dl, min(d0, dh)]   (if dl < d0):  envelope = I itself; weight = its exact integral (reading C5)
+ *   core       [A, B] = [max(dl, d0), min(dh, d1)] cut into ENV_BOXES equal boxes; the core is unimodal (one sign
+ *              change of L between the joins), so the maximum of G over a box is G at the point of the box closest
+ *              to the mode d_m; box height h_j = that maximum times (1 + 2^-20); weight = h_j * width
+ *   right tail [max(d1, dl), dh]   (if dh > d1):  envelope = I itself; weight = its exact integral
+ * Mode d_m: 0 for beta = 0, else the root of L(d) = 0 between the joins by bisection.
+ * Attempt t = 0, 1, ... of (seed, slot): (u1, u2) = uniforms2(seed, slot, t, STREAM_SIG); v = u1 * (total weight)
+ * selects the region r (cumulative weights in the order left tail, boxes, right tail);
+ *   tail:  the power law is sampled exactly by its inverse CDF with u2 (always accepted): with u = 1 - (d-d_j) L_j/n_j
+ *          the mass from the region's left end is linear in t = u^{1-n} (in log u for n = 1), so
+ *          t = t_a + u2 (t_b - t_a),  u = t^{1/(1-n)},  d = d_j - (u - 1) n_j / L_j
+ *   box:   d = box_lo + width * (v - cum[r]) / weight_r  (the remainder of u1 is uniform);  accept iff u2 h_j < G(d).
+ * All weights are in units of exp(logref) (the level make_norm uses).
+ * ---------------------------------------------------------------------------------------- */
+enum { ENV_BOXES = 16, ENV_MAXREG = ENV_BOXES + 2 };
+struct Envelope {
+  int nreg;
+  int kind[ENV_MAXREG];          /* 0 left tail, 1 box, 2 right tail */
+  ld cum[ENV_MAXREG + 1];        /* cumulative weights, cum[0] = 0 */
+  ld blo[ENV_MAXREG], bw;        /* boxes: left edge, common width */
+  ld logh[ENV_MAXREG];           /* boxes: log of the height (absolute, like log_I) */
+  ld ta[ENV_MAXREG], tb[ENV_MAXREG]; /* tails: t (or log u for n = 1) at the left and right end of the region */
+  ld logref;
+};
+
+static ld core_mode(const Shape& s) {
+  if (s.beta == 0) return 0;
+  ld a = s.d0, b = s.d1;                       /* L(d0) > 0 > L(d1) (status 0) */
+  for (int it = 0; it < 200 && b - a > 1e-18L * (fabsl(a) + fabsl(b)); ++it) {
+    const ld m = 0.5L * (a + b);
+    if (core_logderiv(s, m) > 0) a = m; else b = m;
   }
-  return best;
+  return 0.5L * (a + b);
 }
 
-static double draw_signal(const Shape& s, ld logImax, uint64_t seed, uint64_t slot, double lo, double hi) {
+static ld tail_t(ld u, ld n) { return (n == 1) ? logl(u) : powl(u, 1 - n); }
+
+static Envelope make_envelope(const Shape& s, ld lo, ld hi) {
+  Envelope E;
+  const Norm N = make_norm(s, 0, lo, hi);
+  const ld dl = lo - s.mu, dh = hi - s.mu;
+  E.logref = N.logref;
+  E.nreg = 0;
+  E.cum[0] = 0;
+  E.bw = 0;
+  if (dl < s.d0) {
+    const ld dr = std::min(s.d0, dh);
+    const int r = E.nreg++;
+    E.kind[r] = 0;
+    E.ta[r] = tail_t(1 - (dl - s.d0) * s.L0 / s.n, s.n);
+    E.tb[r] = tail_t(1 - (dr - s.d0) * s.L0 / s.n, s.n);
+    E.cum[r + 1] = E.cum[r] + N.left;
+  }
+  const ld A = std::max(dl, s.d0), B = std::min(dh, s.d1);
+  if (B > A) {
+    const ld dm = core_mode(s);
+    E.bw = (B - A) / ENV_BOXES;
+    for (int j = 0; j < ENV_BOXES; ++j) {
+      const int r = E.nreg++;
+      E.kind[r] = 1;
+      E.blo[r] = A + j * E.bw;
+      const ld bhi = (j == ENV_BOXES - 1) ? B : A + (j + 1) * E.bw;
+      const ld closest = std::min(std::max(dm, E.blo[r]), bhi);
+      E.logh[r] = core_logG(s, closest) + log1pl(ldexpl(1, -20));
+      E.cum[r + 1] = E.cum[r] + expl(E.logh[r] - N.logref) * E.bw;
+    }
+  }
+  if (dh > s.d1) {
+    const ld dL = std::max(s.d1, dl);
+    const int r = E.nreg++;
+    E.kind[r] = 2;
+    E.ta[r] = tail_t(1 - (dL - s.d1) * s.L1 / s.n2, s.n2);
+    E.tb[r] = tail_t(1 - (dh - s.d1) * s.L1 / s.n2, s.n2);
+    E.cum[r + 1] = E.cum[r] + N.right;
+  }
+  return E;
+}
+
+/* diag (tests only): diag[0] += attempts used, diag[1] = 1 if an attempt saw G(d) above its box height */
+static double draw_signal(const Shape& s, const Envelope& E, uint64_t seed, uint64_t slot, int64_t* diag = nullptr) {
   for (uint32_t attempt = 0;; ++attempt) {
     double u1, u2;
     uniforms2(seed, slot, attempt, STREAM_SIG, &u1, &u2);
-    const double x = lo + (hi - lo) * u1;
-    const ld ratio = expl(log_I(s, (ld)x - s.mu) - logImax);
-    if ((ld)u2 * 1.02L < ratio) return x;
-    if (attempt > 100000u) return x; /* unreachable for valid shapes */
+    if (diag) diag[0] += 1;
+    const ld v = (ld)u1 * E.cum[E.nreg];
+    int r = 0;
+    while (r + 1 < E.nreg && v >= E.cum[r + 1]) ++r;
+    if (E.kind[r] != 1) {
+      const ld n = (E.kind[r] == 0) ? s.n : s.n2, L = (E.kind[r] == 0) ? s.L0 : s.L1, dj = (E.kind[r] == 0) ? s.d0 : s.d1;
+      const ld t = E.ta[r] + (ld)u2 * (E.tb[r] - E.ta[r]);
+      const ld u = (n == 1) ? expl(t) : powl(t, 1 / (1 - n));
+      return (double)(s.mu + (dj - (u - 1) * n / L));
+    }
+    const ld d = E.blo[r] + E.bw * ((v - E.cum[r]) / (E.cum[r + 1] - E.cum[r]));
+    const ld lg = core_logG(s, d);
+    if (diag && lg > E.logh[r]) diag[1] = 1;
+    if ((ld)u2 < expl(lg - E.logh[r])) return (double)(s.mu + d);
+    if (attempt > 100000u) return (double)(s.mu + d); /* unreachable: the acceptance is >= 1/2 for any unimodal core */
   }
 }
 
@@ -725,12 +807,33 @@ void orc_poisson_array(uint64_t seed, uint64_t slot0, int64_t n, uint32_t stream
 int orc_generate_mixture(uint64_t seed, int64_t n, const orc_params* p, double lo, double hi, double* x) {
   const Shape s = make_shape(*p);
   if (s.status) return s.status;
-  const ld lim = log_I_max(s, lo, hi);
+  const Envelope env = make_envelope(s, lo, hi);
   for (int64_t i = 0; i < n; ++i) {
     double uc, v;
     uniforms2(seed, (uint64_t)i, 0, STREAM_COMP, &uc, &v);
-    x[i] = (uc < p->f) ? draw_signal(s, lim, seed, (uint64_t)i, lo, hi) : draw_background(p->k, seed, (uint64_t)i, lo, hi);
+    x[i] = (uc < p->f) ? draw_signal(s, env, seed, (uint64_t)i) : draw_background(p->k, seed, (uint64_t)i, lo, hi);
   }
+  return 0;
+}
+
+/* tests only: n signal draws (slots 0..n-1) with the envelope diagnostics: diag[0] = total attempts, diag[1] = 1 if any
+ * attempt found the core above its box height; env_out[0] = total envelope weight / N_S (1 / acceptance), env_out[1] below */
+int orc_generate_signal_diag(uint64_t seed, int64_t n, const orc_params* p, double lo, double hi, double* x, int64_t* diag,
+                             double* env_out) {
+  const Shape s = make_shape(*p);
+  if (s.status) return s.status;
+  const Envelope env = make_envelope(s, lo, hi);
+  const Norm N = make_norm(s, 0, lo, hi);
+  diag[0] = diag[1] = 0;
+  for (int64_t i = 0; i < n; ++i) x[i] = draw_signal(s, env, seed, (uint64_t)i, diag);
+  env_out[0] = (double)(env.cum[env.nreg] / N.NS);
+  /* env_out[1] = max over a dense grid of log G(d) - log h(box of d): the envelope is a bound iff this is <= 0 */
+  ld worst = -INFINITY;
+  for (int r = 0; r < env.nreg; ++r) {
+    if (env.kind[r] != 1) continue;
+    for (int i = 0; i <= 4000; ++i) worst = std::max(worst, core_logG(s, env.blo[r] + env.bw * i / 4000) - env.logh[r]);
+  }
+  env_out[1] = (double)worst;
   return 0;
 }
 
@@ -752,10 +855,10 @@ int orc_toy_generate(const uint64_t* seeds, int64_t T, const orc_params* gen, in
     const orc_params& p = gen[gen_stride ? t : 0];
     const Shape s = make_shape(p);
     if (s.status) return s.status;
-    const ld lim = log_I_max(s, lo, hi);
+    const Envelope env = make_envelope(s, lo, hi);
     const int64_t nt = offsets[t + 1] - offsets[t];
     for (int64_t j = 0; j < nt; ++j)
-      x[offsets[t] + j] = (j < ns[(size_t)t]) ? draw_signal(s, lim, seeds[t], (uint64_t)j, lo, hi)
+      x[offsets[t] + j] = (j < ns[(size_t)t]) ? draw_signal(s, env, seeds[t], (uint64_t)j)
                                                : draw_background(p.k, seeds[t], (uint64_t)j, lo, hi);
   }
   return 0;

@@ -289,3 +289,62 @@ def test_ptrs_pins_detect_wrong_constants():
     for j, (name, wrong) in enumerate(mutations.items()):
         c = dict(PTRS_PUBLISHED, **{name: wrong})
         assert not (verdict(c, 1.0e3, 100 + j) and verdict(c, 3.0e4, 200 + j)), (name, wrong)
+
+
+# ---- signal draws under the piecewise envelope (reading D13 as revised in round 2) ---------------------------------
+ENV_CASES = {
+    "config": P1,
+    "beta_nonzero": P2,
+    "beta_large": dict(P2, beta=0.05),
+    "mode_left_of_range": dict(P1, mu=4998.0, sigma=3.0),          # the advisor's case: maximum at the range end
+    "mode_left_of_range_b": dict(P1, mu=4995.0, sigma=5.0, beta=-0.02),
+    "range_inside_left_tail": dict(P1, mu=5700.0, n=1.0),
+    "range_inside_right_tail": dict(P2, mu=4900.0),
+    "student_t": inp.T1,
+    "student_t_beta": inp.T2,
+    "n_equal_one": dict(P1, n=1.0, n2=1.0),
+}
+
+
+def _signal_cdf(orc, p, grid):
+    """CDF of S on `grid` by composite Simpson (16 sub-intervals per cell) of the oracle's normalised signal density
+    (exp of logpdf at f = 1); the joins and the mode are grid points, so every cell is smooth."""
+    a, b = grid[:-1], grid[1:]
+    t = a[:, None] + (b - a)[:, None] * np.linspace(0.0, 1.0, 17)[None, :]
+    f = np.exp(orc.logpdf(t.ravel(), dict(p, f=1.0), LO, HI)).reshape(t.shape)
+    cell = (b - a) / 48 * (f[:, 0] + f[:, -1] + 4 * f[:, 1:-1:2].sum(axis=1) + 2 * f[:, 2:-1:2].sum(axis=1))
+    return np.concatenate([[0.0], np.cumsum(cell)])
+
+
+@pytest.mark.parametrize("case", sorted(ENV_CASES))
+def test_signal_draws_follow_the_density(orc, case):
+    """chi^2 (100 equal-probability bins) and KS of the signal draws against the integral of the oracle's S, which is
+    pinned on its own (test_oracle_ipatia / test_oracle_studentt): independent of how the draws are made.  Covers
+    beta != 0, the mode outside the range, ranges inside one tail, n = 1 and the Student-t core."""
+    sp = pytest.importorskip("scipy.stats")
+    p = ENV_CASES[case]
+    n = 40000
+    x, attempts, violated, inv_acc, worst = orc.generate_signal_diag(123, n, p, LO, HI)
+    assert x.min() >= LO and x.max() <= HI and not violated
+    assert worst <= 0.0                                   # the envelope bounds the core everywhere on a dense grid
+    special = [p["mu"] + d for d in (-p["a"] * p["sigma"], 0.0, p["a2"] * p["sigma"]) if LO < p["mu"] + d < HI]
+    grid = np.unique(np.concatenate([np.linspace(LO, HI, 24001), special]))   # 0.025 steps: the CDF is interpolated linearly
+    cdf = _signal_cdf(orc, p, grid)
+    assert abs(cdf[-1] - 1.0) <= 1e-9
+    u = np.interp(x, grid, cdf)                           # probability integral transform: uniform if x ~ S
+    assert sp.kstest(u, "uniform").pvalue > 1e-3
+    obs, _ = np.histogram(u, bins=100, range=(0.0, 1.0))
+    chi2 = float(((obs - n / 100) ** 2 / (n / 100)).sum())
+    assert chi2 < 99 + 5 * math.sqrt(2 * 99), chi2
+    # acceptance theorem: attempts per event = envelope weight / N_S (mean of a geometric law), here 1 .. 1.4
+    assert 1.0 <= inv_acc <= 1.4
+    assert abs(attempts - inv_acc) <= 5 * math.sqrt(inv_acc * (inv_acc - 1) / n) + 1e-3, (attempts, inv_acc)
+
+
+def test_signal_draws_are_slot_addressed(orc):
+    """A draw depends on (seed, slot) only: prefix-stable and equal inside the mixture and the toy generators."""
+    a = orc.generate_signal_diag(9, 500, P1, LO, HI)[0]
+    b = orc.generate_signal_diag(9, 2000, P1, LO, HI)[0]
+    assert (a == b[:500]).all()
+    m = orc.generate_mixture(9, 2000, dict(P1, f=1.0), LO, HI)
+    assert (m == b).all()
