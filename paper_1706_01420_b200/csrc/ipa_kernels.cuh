@@ -875,13 +875,24 @@ __device__ __forceinline__ double ipa_draw_background(double k, unsigned long lo
   return lo + log1p(u * expm1(t)) / k;
 }
 
-// log I(d) with the streaming kernels' own sqrt / log and the Horner groups (accept-reject attempt loop).
-// Direct-mode shapes fall back to ipa_logI_rec.
-template <class Tab>
-__device__ __forceinline__ double ipa_logI_fast(const IpaSetConsts& c, double cshift, double d, const Tab* tab) {
-  if (c.mode != 0) return ipa_logI_rec(c, d);
-  if (d < c.d0) return c.logG0 - c.n0 * ipa_flog(fma(c.uA0, d, c.uB0), tab);
-  if (d > c.d1) return c.logG1 - c.n1 * ipa_flog(fma(c.uA1, d, c.uB1), tab);
+// Core-only log G(d) with the streaming kernels' own sqrt and the Horner groups (accept-reject attempt loop; the
+// boxes of the envelope lie inside the core).  Direct-mode and Student-t shapes use the plain functions.
+__host__ __device__ __noinline__ double ipa_logG_rec(const IpaSetConsts& c, double d) {
+  if (c.mode == 2) return fma(c.nu, log(fma(d, d, c.delta2)), c.beta * d);
+  const double r = sqrt(fma(d, d, c.delta2));
+  double H;
+  if (c.mode == 0) {
+    const double t = fma(c.tA, r, c.tB);
+    double acc = c.a[c.degree];
+    for (int j = c.degree - 1; j >= 1; --j) acc = fma(acc, t, c.a[j]);
+    H = c.degree >= 1 ? fma(acc, t, c.araw0) : c.araw0;
+  } else {
+    H = ipa_direct_H(c.nu, c.alpha * r);
+  }
+  return H - c.nu * log(c.alpha) + c.beta * d;
+}
+__device__ __forceinline__ double ipa_logG_fast(const IpaSetConsts& c, double cshift, double d) {
+  if (c.mode != 0) return ipa_logG_rec(c, d);
   const double t = fma(c.tA, ipa_fsqrt(fma(d, d, c.delta2)), c.tB);
   double P = 0.0;
   for (int g = c.degree >> 2; g >= 1; --g) {
@@ -892,6 +903,105 @@ __device__ __forceinline__ double ipa_logI_fast(const IpaSetConsts& c, double cs
   P = fma(P, t, c.a[3]); P = fma(P, t, c.a[2]); P = fma(P, t, c.a[1]);
   return fma(c.beta, d, fma(P, t, cshift));      // cshift = araw0 - nu log alpha
 }
+// core log-derivative L(d) = G'/G from a record (mode of the core for the envelope)
+__host__ __device__ __noinline__ double ipa_L_rec(const IpaSetConsts& c, double d) {
+  const double q = fma(d, d, c.delta2);
+  if (c.mode == 2) return c.beta + 2.0 * c.nu * d / q;
+  const double r = sqrt(q);
+  if (c.mode == 0) {
+    const double t = fma(c.tA, r, c.tB);
+    double acc = 0.0;
+    for (int j = c.degree; j >= 1; --j) acc = fma(acc, t, (double)j * c.a[j]);
+    return c.beta + c.tA * (d / r) * acc;
+  }
+  const double z = c.alpha * r;
+  return c.beta - c.alpha * (d / r) * ipa_besselk_scaled(c.nu - 1.0, z) / ipa_besselk_scaled(c.nu, z);
+}
+
+// Envelope of the signal accept-reject (reading D13 as revised in round 2; PAPER.md:343-351 says only
+// "accept-reject"): exact power-law tails + IPA_ENV_BOXES boxes on the unimodal core, heights at the point of the
+// box closest to the mode times (1 + 2^-20): a true bound of I on the range.  Regions in the order left tail,
+// boxes, right tail; weights in units of exp(logref).
+#define IPA_ENV_BOXES 16
+#define IPA_ENV_MAXREG (IPA_ENV_BOXES + 2)
+struct IpaEnvelope {
+  double cum[IPA_ENV_MAXREG + 1];   // cumulative weights, cum[0] = 0
+  double invw[IPA_ENV_MAXREG];      // 1 / weight
+  double blo[IPA_ENV_MAXREG];       // boxes: left edge
+  double logh[IPA_ENV_MAXREG];      // boxes: log height (absolute, like log I)
+  double ta[IPA_ENV_MAXREG], dt[IPA_ENV_MAXREG];   // tails: t = u^(1-n) (log u at n = 1) at the region's left end, t_b - t_a
+  double w[IPA_ENV_MAXREG];
+  double bw, dm;
+  int kind[IPA_ENV_MAXREG];         // 0 left tail, 1 box, 2 right tail
+  int nreg, box0;
+};
+__device__ __forceinline__ double ipa_tail_t(double u, double n) { return n == 1.0 ? log(u) : pow(u, 1.0 - n); }
+
+// Built by one block (>= 32 threads), result in shared memory; ends with a barrier.
+__device__ void ipa_build_envelope(const IpaSetConsts& c, double lo, double hi, IpaEnvelope& E) {
+  const int tid = threadIdx.x;
+  const double dl = lo - c.mu, dh = hi - c.mu;
+  const double A = fmax(dl, c.d0), B = fmin(dh, c.d1);
+  if (tid == 0) {
+    int nr = 0;
+    if (dl < c.d0) {
+      const double dr = fmin(c.d0, dh);
+      const double ul = fma(c.uA0, dl, c.uB0), ur = fma(c.uA0, dr, c.uB0);
+      double ls;
+      const double Fm = ipa_powint_diff(ul, ur, c.n0, &ls);
+      E.kind[nr] = 0;
+      E.ta[nr] = ipa_tail_t(ul, c.n0);
+      E.dt[nr] = ipa_tail_t(ur, c.n0) - E.ta[nr];
+      E.w[nr] = (c.n0 / c.L0) * exp(c.logG0 - c.logref + ls) * Fm;
+      ++nr;
+    }
+    E.box0 = nr;
+    E.bw = 0.0;
+    if (B > A) {
+      E.bw = (B - A) / (double)IPA_ENV_BOXES;
+      for (int j = 0; j < IPA_ENV_BOXES; ++j) { E.kind[nr + j] = 1; E.blo[nr + j] = A + (double)j * E.bw; }
+      nr += IPA_ENV_BOXES;
+      // mode of the core: 0 for beta = 0, else the root of L between the joins (L(d0) > 0 > L(d1)) by bisection
+      double dm = 0.0;
+      if (c.beta != 0.0) {
+        double a = c.d0, b = c.d1;
+        for (int it = 0; it < 100 && b - a > 4e-16 * (fabs(a) + fabs(b)); ++it) {
+          const double m = 0.5 * (a + b);
+          if (ipa_L_rec(c, m) > 0.0) a = m; else b = m;
+        }
+        dm = 0.5 * (a + b);
+      }
+      E.dm = dm;
+    }
+    if (dh > c.d1) {
+      const double dL = fmax(c.d1, dl);
+      const double uh = fma(c.uA1, dh, c.uB1), ul = fma(c.uA1, dL, c.uB1);
+      double ls;
+      const double Fm = ipa_powint_diff(uh, ul, c.n1, &ls);
+      E.kind[nr] = 2;
+      E.ta[nr] = ipa_tail_t(ul, c.n1);
+      E.dt[nr] = ipa_tail_t(uh, c.n1) - E.ta[nr];
+      E.w[nr] = (c.n1 / (-c.L1)) * exp(c.logG1 - c.logref + ls) * Fm;
+      ++nr;
+    }
+    E.nreg = nr;
+  }
+  __syncthreads();
+  if (B > A && tid < IPA_ENV_BOXES) {
+    const int r = E.box0 + tid;
+    const double bhi = (tid == IPA_ENV_BOXES - 1) ? B : A + (double)(tid + 1) * E.bw;
+    const double closest = fmin(fmax(E.dm, E.blo[r]), bhi);
+    E.logh[r] = ipa_logG_rec(c, closest) + 9.5367386116398572e-07;      // log(1 + 2^-20)
+    E.w[r] = exp(E.logh[r] - c.logref) * E.bw;
+  }
+  __syncthreads();
+  if (tid == 0) {
+    double run = 0.0;
+    E.cum[0] = 0.0;
+    for (int r = 0; r < E.nreg; ++r) { run += E.w[r]; E.cum[r + 1] = run; E.invw[r] = 1.0 / E.w[r]; }
+  }
+  __syncthreads();
+}
 
 // grid (T, chunks).  mixture != 0: T == 1, `capacity` events, component by u < f (configs 1-3).
 __global__ void __launch_bounds__(IPA_BLOCK)
@@ -900,13 +1010,10 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
                       const long long* __restrict__ nsig, const long long* __restrict__ offsets, double lo, double hi,
                       long long capacity, int mixture, double* __restrict__ x, int32_t* __restrict__ overflow) {
   __shared__ IpaSetConsts c;
-  __shared__ double red[IPA_BLOCK / 32];
-  __shared__ double s_logImax;
-  __shared__ double2 s_tab[33];
+  __shared__ IpaEnvelope E;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const long long t = blockIdx.x;
   const long long g = gen_stride ? t : 0;
-  ipa_load_logtab(s_tab);
   {
     const double* src = reinterpret_cast<const double*>(consts + g);
     double* dst = reinterpret_cast<double*>(&c);
@@ -921,23 +1028,9 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
     for (long long i = b0 + (long long)blockIdx.y * IPA_BLOCK + tid; i < e0; i += (long long)gridDim.y * IPA_BLOCK) x[i] = NAN;
     return;
   }
-  // envelope: log of the maximum of I over the range (reading D13)
-  if (c.beta == 0.0 && lo <= c.mu && c.mu <= hi) {
-    if (tid == 0) s_logImax = ipa_logI_rec(c, 0.0);
-  } else {
-    double best = -INFINITY;
-    for (int j = tid; j < 4096; j += IPA_BLOCK) {
-      const double xx = lo + ((double)j + 0.5) * (hi - lo) / 4096.0;
-      best = fmax(best, ipa_logI_rec(c, xx - c.mu));
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) best = fmax(best, __shfl_xor_sync(IPA_FULL, best, o));
-    if (lane == 0) red[warp] = best;
-    __syncthreads();
-    if (tid == 0) s_logImax = fmax(fmax(red[0], red[1]), fmax(red[2], red[3]));
-  }
-  __syncthreads();
-  const double logImax = s_logImax;
+  ipa_build_envelope(c, lo, hi, E);
+  const double W = E.cum[E.nreg];
+  const int nreg = E.nreg;
   const double cshift = c.araw0 - c.nu * log(c.alpha);
   const unsigned long long seed = seeds[t];
   const double f = c.fsig, k = c.kraw;
@@ -948,8 +1041,7 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
   // handed to the lanes in any order.  A warp owns a contiguous range of slots and works in rounds of
   // IPA_GEN_ROUND slots: (A) classify, draw the background events, list the signal slots in shared memory;
   // (B) accept-reject on the listed slots with REFILL: a lane whose attempt is accepted takes the next slot
-  // of the list, so the warp does not wait for its unluckiest lane (the attempt count is geometric with
-  // mean ~20 under the flat envelope).
+  // of the list, so the warp does not wait for its unluckiest lane.
   __shared__ int s_list[IPA_BLOCK / 32][IPA_GEN_ROUND];
   const long long nwarp = (long long)gridDim.y * (IPA_BLOCK / 32), wid = (long long)blockIdx.y * (IPA_BLOCK / 32) + warp;
   long long lim = len;
@@ -995,11 +1087,31 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
         const unsigned long long j = (unsigned long long)(r0 + item);
         double u1, u2;
         ipa_uniforms2(seed, j, attempt, IPA_STREAM_SIG, &u1, &u2);
-        const double xx = lo + (hi - lo) * u1;
-        const double ratio = ipa_fexp_neg(fmax(ipa_logI_fast(c, cshift, xx - c.mu, s_tab) - logImax, -700.0));
-        if (u2 * 1.02 < ratio || attempt == 100001u) {
-          if (attempt == 100001u && overflow) atomicOr(overflow, 2);     // attempt cap: not a draw from the density
-          x[beg + (long long)j] = xx;
+        const double v = u1 * W;
+        int r = 0;
+        for (int q = 1; q < nreg; ++q) r += (v >= E.cum[q]) ? 1 : 0;
+        const int kind = E.kind[r];
+        bool accept;
+        double dd;
+        if (kind != 1) {
+          // power-law tail by its inverse CDF (always accepted): t = u^(1-n) is linear in the mass
+          const double n = kind == 0 ? c.n0 : c.n1, L = kind == 0 ? c.L0 : c.L1, dj = kind == 0 ? c.d0 : c.d1;
+          const double tt = fma(u2, E.dt[r], E.ta[r]);
+          const double u = (n == 1.0) ? exp(tt) : pow(tt, 1.0 / (1.0 - n));
+          dd = dj - (u - 1.0) * n / L;
+          accept = true;
+        } else {
+          dd = fma(E.bw, (v - E.cum[r]) * E.invw[r], E.blo[r]);
+          const double lg = ipa_logG_fast(c, cshift, dd) - E.logh[r];
+          if (lg > 1e-12 && overflow) atomicOr(overflow, 2);      // the envelope must bound the core: a defect if it does not
+          accept = u2 < ipa_fexp_neg(fmin(fmax(lg, -700.0), 0.0));
+        }
+        if (attempt == 100001u) {                                   // attempt cap: not a draw from the density
+          if (overflow) atomicOr(overflow, 2);
+          accept = true;
+        }
+        if (accept) {
+          x[beg + (long long)j] = c.mu + dd;
           item = -1;
         } else {
           ++attempt;

@@ -85,6 +85,19 @@ IPA_HD double ipa_powint(double u, double n) {
   return expm1(y) / e;
 }
 
+// F(ul) - F(ur), F(u) = (u^(1-n) - 1)/(1-n) (log u at n = 1), formed WITHOUT the cancellation of two nearly equal
+// terms (range inside one tail, large n):  = ur^(1-n) expm1((1-n) log(ul/ur)) / (1-n).  Returned as the pair
+// (value without the factor ur^(1-n), *logscale = (1-n) log ur) so that the caller can fold the scale into its
+// log-reference before exponentiating.
+IPA_HD double ipa_powint_diff(double ul, double ur, double n, double* logscale) {
+  const double e = 1.0 - n;
+  const double lq = log(ul / ur);
+  const double y = e * lq;
+  *logscale = e * log(ur);
+  if (fabs(y) < 1e-9) return lq * (1.0 + 0.5 * y);
+  return expm1(y) / e;
+}
+
 // error-free transformations for the double-double accumulation in the basis conversion
 IPA_HD void ipa_two_sum(double a, double b, double* s, double* e) {
   const double t = a + b;

@@ -409,9 +409,12 @@ IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
     if (w.dl < w.d0) {
       const double dr = fmin(w.d0, w.dh);
       const double ul = 1.0 - (w.dl - w.d0) * w.L0 / p.n, ur = 1.0 - (dr - w.d0) * w.L0 / p.n;
-      const double pre = exp(w.logG0 - w.logref) * (p.n / w.L0);
-      const double F = ipa_powint(ul, p.n) - ipa_powint(ur, p.n);
-      const double F1 = w.want_grad ? ipa_powint(ul, p.n + 1.0) - ipa_powint(ur, p.n + 1.0) : 0.0;
+      // F(ul) - F(ur) without cancellation (ipa_powint_diff); its scale ur^(1-n) joins the log-reference
+      double ls, ls1 = 0.0;
+      const double Fm = ipa_powint_diff(ul, ur, p.n, &ls);
+      const double F1m = w.want_grad ? ipa_powint_diff(ul, ur, p.n + 1.0, &ls1) : 0.0;
+      const double pre = p.n / w.L0, lg = w.logG0 - w.logref;
+      const double F = exp(lg + ls) * Fm, F1 = w.want_grad ? exp(lg + ls1) * F1m : 0.0;
       const double A = ipa_sigpow(w) / p.sigma - p.a * p.beta, c = p.n * (w.L0 - p.beta) / (w.L0 * p.sigma);
       left = pre * F;
       left2 = pre * ((A + c) * F + (p.a * w.L0 - c) * F1);
@@ -423,9 +426,11 @@ IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
     if (w.dh > w.d1) {
       const double dL = fmax(w.d1, w.dl);
       const double uh = 1.0 - (w.dh - w.d1) * w.L1 / p.n2, ul = 1.0 - (dL - w.d1) * w.L1 / p.n2;
-      const double pre = exp(w.logG1 - w.logref) * (p.n2 / (-w.L1));
-      const double F = ipa_powint(uh, p.n2) - ipa_powint(ul, p.n2);
-      const double F1 = w.want_grad ? ipa_powint(uh, p.n2 + 1.0) - ipa_powint(ul, p.n2 + 1.0) : 0.0;
+      double ls, ls1 = 0.0;
+      const double Fm = ipa_powint_diff(uh, ul, p.n2, &ls);
+      const double F1m = w.want_grad ? ipa_powint_diff(uh, ul, p.n2 + 1.0, &ls1) : 0.0;
+      const double pre = p.n2 / (-w.L1), lg = w.logG1 - w.logref;
+      const double F = exp(lg + ls) * Fm, F1 = w.want_grad ? exp(lg + ls1) * F1m : 0.0;
       const double A = ipa_sigpow(w) / p.sigma + p.a2 * p.beta, c = p.n2 * (w.L1 - p.beta) / (w.L1 * p.sigma);
       right = pre * F;
       right2 = pre * ((A + c) * F - (p.a2 * w.L1 + c) * F1);

@@ -240,6 +240,41 @@ def test_mixture_generator_matches_oracle(ipa, torch_, orc):
         assert ((got >= LO) & (got <= HI)).all()
 
 
+@pytest.mark.parametrize("case", ["beta_large", "mode_left_of_range", "mode_left_of_range_b", "range_inside_left_tail",
+                                  "range_inside_right_tail", "n_equal_one", "student_t_beta"])
+def test_signal_envelope_cases(ipa, torch_, orc, case):
+    """Reading D13 (revised): exact tails + boxes on the core.  Signal-only draws (f = 1) in the cases the old flat
+    envelope got wrong or slow (advisor finding, round 1): beta != 0, the maximum at a range end, the range inside
+    one tail, n = 1, the Student-t core.  No event differs from the oracle generator's, and the flag that records
+    a core value above its box (code 2) stays clear."""
+    theta = dict({"beta_large": dict(inp.P2, beta=0.05), "mode_left_of_range": dict(inp.GEN, mu=4998.0, sigma=3.0),
+                  "mode_left_of_range_b": dict(inp.GEN, mu=4995.0, sigma=5.0, beta=-0.02),
+                  "range_inside_left_tail": dict(inp.GEN, mu=5700.0, n=1.0), "range_inside_right_tail": dict(inp.P2, mu=4900.0),
+                  "n_equal_one": dict(inp.GEN, n=1.0, n2=1.0), "student_t_beta": inp.T2}[case], f=1.0)
+    n = 30000
+    x, _, ovf = ipa.ipa_toy_generate([77], theta, -1.0, -1.0, LO, HI, n)
+    torch_.cuda.synchronize()
+    assert ovf.item() == 0
+    got = x.cpu().numpy()
+    assert ((got >= LO) & (got <= HI)).all()
+    mismatches(got, orc.generate_mixture(77, n, theta, LO, HI), f"signal envelope, {case}")
+
+
+def test_range_inside_one_tail_with_a_large_exponent(ipa, torch_, orc):
+    """Advisor finding (round 1): F(ul) - F(ur) of the tail normalisation cancels when the whole range lies inside one
+    tail and n is large; the difference is now formed directly (ipa_powint_diff)."""
+    x = np.linspace(LO, HI, 2001)
+    for mu in (5610.0, 5627.0, 5700.0):
+        th = dict(inp.GEN, mu=mu, sigma=0.89, a=2.34, n=66.0)
+        nll, lp, st = ipa.ipa_nll_eval(dev(torch_, x), th, LO, HI, want_logpdf=True)
+        ns, _, _ = ipa.ipa_norm(th, LO, HI)
+        torch_.cuda.synchronize()
+        ost, o = orc.norm(th, LO, HI)
+        assert st.item() == ost == 0
+        assert abs(ns.item() / o["NS"] - 1) <= 1e-12
+        assert np.abs(lp[0].cpu().numpy() - orc.logpdf(x, th, LO, HI)).max() <= 1e-10
+
+
 def test_toy_generator_and_segmented_nll(ipa, torch_, orc):
     T = 24
     seeds = inp.toy_seeds(T)

@@ -278,6 +278,27 @@ def test_range_inside_one_tail_and_n_equal_one(orc):
     assert abs(mp.mpf(nrm["NS"]) - m.NS) <= 1e-14 * m.NS
 
 
+def test_range_deep_inside_one_tail_with_a_large_exponent(orc):
+    """C5 between two points of the same tail: with n = 66 and the range far from the peak, F(ul) and F(ur) agree to
+    all digits and must not be subtracted; N_S and the per-event values against the closed form in mpmath at 50 digits
+    (mpmath's own quadrature needs that many digits here: the integrand spans 50 decades)."""
+    for mu in (5610.0, 5627.0, 5700.0):
+        p = dict(P1, mu=mu, sigma=0.89, a=2.34, n=66.0)
+        with mp.workdps(50):
+            m = MPModel(p)
+            ul = 1 - (m.lo - m.mu - m.d0) * m.L0 / m.n
+            ur = 1 - (m.hi - m.mu - m.d0) * m.L0 / m.n
+            F = lambda u: (u ** (1 - m.n) - 1) / (1 - m.n)
+            closed = m.G0 * (m.n / m.L0) * (F(ul) - F(ur))
+            assert abs(closed - m.NS) <= mp.mpf("1e-13") * closed          # closed form = mpmath quadrature (its own accuracy)
+            st, nrm = orc.norm(p, LO, HI)
+            assert st == 0 and abs(mp.mpf(nrm["NS"]) - closed) <= 2e-14 * closed, (mu, nrm["NS"], closed)
+            xs = np.array([LO, 5123.4, 5400.0, 5599.0, HI])
+            got = orc.logpdf(xs, p, LO, HI)
+            for x, g in zip(xs, got):
+                assert abs(mp.mpf(float(g)) - m.l(float(x))) <= 1e-13, (mu, x)
+
+
 def test_population_facts(orc):
     """E[-l] = 6.0901249 per event and P(core) = 0.34443 for the config model (C8.9)."""
     l = lambda x: orc.logpdf(np.array([float(x)]), P1, LO, HI)[0]
