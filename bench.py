@@ -44,6 +44,80 @@ def algorithmic_flops(degree, p_core):
     return 55.0 + p_core * core + (1.0 - p_core) * 27.0
 
 
+def shape_stage_flops(degree, p_core):
+    """Shape stage of a group of sets sharing (mu, sigma, lambda, zeta, beta, a, n, a2, n2) -- DESIGN.md section 5:
+    d (1), 2 region compares (2), core: q, sqrt, t, Horner = (5 + degree) FMA + 2 mul; tail: u (1 FMA) + log
+    (10 FMA + 1 add) + the product with -n (1 mul)."""
+    return 3.0 + p_core * (2.0 * (5 + degree) + 2.0) + (1.0 - p_core) * (2.0 * 11 + 2.0)
+
+
+MEMBER_STAGE_FLOPS = 55.0
+"""Member stage per set: Delta = s d + (V + c): 1 add + 1 FMA (3); E_B (1 FMA: 2); exp 14 FMA + 1 add (29); 1 + w (1);
+log on [1,2] 9 FMA (18); 2 adds (2)."""
+
+
+def gradient_flops(degree, p_core):
+    """Analytic-gradient pass per event x set (ipa_eval_grad): common = d, 2 compares, exp (29), 1+w, 1/(1+w)
+    (4 FMA), w/(1+w), E_B (2), log (18), 2 adds, the four derivative terms (2 + 2 + 3 + 3) and 5 accumulations = 80;
+    core = q (2), sqrt (8), 1/r (8), t (2), value and derivative Horner 2 FMA per coefficient of the 4 ceil((D+1)/4)
+    slots, L - beta (3), Delta (2), dd (1), ds (3); tail = u (2), 1/u (8), log (21), Delta (4), dd (1), ds (5)."""
+    slots = 4 * (degree // 4) + 4
+    core = 2.0 + 8 + 8 + 2 + 4.0 * slots + 3 + 2 + 1 + 3
+    return 80.0 + p_core * core + (1.0 - p_core) * 41.0
+
+
+def alu_roofline(flops_per_event, events, seconds, extra=None):
+    """'alu' roofline entry: achieved = declared algorithmic FP64 flops / measured time, against the FP64 FMA peak."""
+    ach = flops_per_event * events / seconds / 1e12
+    d = {"bound": "alu", "achieved": ach, "peak": FP64_PEAK_NOMINAL / 1e12, "unit": "TFLOP/s",
+         "frac": ach / (FP64_PEAK_NOMINAL / 1e12), "flops_per_event": flops_per_event, "ms": seconds * 1e3}
+    if extra:
+        d.update(extra)
+    return d
+
+
+def build_hash():
+    """sha256 over the CUDA sources and the header the library was built from (profiles/*.md record the hash of the
+    build an ncu capture was taken on; a capture of another build is not quoted)."""
+    import hashlib
+    h = hashlib.sha256()
+    csrc = os.path.join(ROOT, "paper_1706_01420_b200", "csrc")
+    for name in sorted(os.listdir(csrc)):
+        if name.endswith((".cu", ".cuh", ".inc")):
+            h.update(open(os.path.join(csrc, name), "rb").read())
+    h.update(open(os.path.join(ROOT, "include", "ipanll.h"), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def measured_traffic(n):
+    """dram__bytes_read.sum + dram__bytes_write.sum per launch of the streaming kernel from the committed ncu raw
+    page profiles/r02_nll_kernel_raw.csv (command in the .md beside it), quoted only if that capture was taken on
+    THIS build (hash line in the .md) and scaled by the event count.  -> (bytes or None, note)."""
+    import csv
+    md, raw = os.path.join(ROOT, "profiles", "r02_nll_kernel_raw.md"), os.path.join(ROOT, "profiles", "r02_nll_kernel_raw.csv")
+    if not (os.path.exists(md) and os.path.exists(raw)):
+        return None, "no ncu --set full capture committed for this build"
+    txt = open(md).read()
+    h = build_hash()
+    if ("build_hash: " + h) not in txt:
+        return None, "profiles/r02_nll_kernel_raw.csv was captured on another build (this build: %s)" % h
+    rows = list(csv.reader(open(raw)))
+    hdr = next(r for r in rows if "Kernel Name" in r)
+    ik, ir, iw = hdr.index("Kernel Name"), hdr.index("dram__bytes_read.sum"), hdr.index("dram__bytes_write.sum")
+    units = rows[rows.index(hdr) + 1]
+    scale = {"byte": 1.0, "Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9}
+    vals = [float(r[ir].replace(",", "")) * scale[units[ir]] + float(r[iw].replace(",", "")) * scale[units[iw]]
+            for r in rows[rows.index(hdr) + 2:] if len(r) > iw and "ipa_nll_kernel" in r[ik]]
+    if not vals:
+        return None, "no ipa_nll_kernel row in profiles/r02_nll_kernel_raw.csv"
+    ev = 1e8
+    for line in txt.splitlines():
+        if line.startswith("events: "):
+            ev = float(line.split()[1])
+    return float(np.mean(vals)) * n / ev, ("ncu --set full, mean of %d launches of ipa_nll_kernel at %g events, "
+                                           "profiles/r02_nll_kernel_raw.csv (same build %s), scaled by events" % (len(vals), ev, h))
+
+
 class ClockSampler:
     """SM clock / throttle reasons during the timed region (B200_PROFILING.md recipe), sampled through
     NVML every 5 ms; falls back to nvidia-smi -lms when pynvml is not importable."""
@@ -91,15 +165,24 @@ class ClockSampler:
                 "power_w_max": max(r[2] for r in self.rows) if sm else None, "samples": len(sm), "reasons": reasons}
 
 
-def cpu_baseline(x_host, params, cores, budget_events):
+def cpu_baseline(x_host, params, cores):
+    """The oracle as it stands on the host cores: all-cores figure on the WHOLE workload (its NLL is the parity number of
+    the line) and the single-thread figure on the first 1e6 events (SURVEY.md 8(d) 'Timing the oracle beside it')."""
     import oracle
-    n = int(min(x_host.size, budget_events))
+    n = int(x_host.size)
     t0 = time.perf_counter()
-    v = oracle.nll(x_host[:n], params, LO, HI, nthreads=cores)
+    v = oracle.nll(x_host, params, LO, HI, nthreads=cores)
     dt = time.perf_counter() - t0
-    return {"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
-            "sample": f"first {n} events of the workload, K=1, {cores} threads each on a contiguous chunk, {dt:.2f} s",
-            "nll": float(v[0])}
+    n1 = min(n, 1_000_000)
+    t0 = time.perf_counter()
+    v1 = oracle.nll(x_host[:n1], params, LO, HI, nthreads=1)
+    dt1 = time.perf_counter() - t0
+    return ({"value": n / dt, "unit": UNIT, "cores": cores, "kind": "oracle",
+             "sample": f"all {n} events of the workload, K=1, {cores} threads each on a contiguous chunk, {dt:.2f} s",
+             "nll": float(v[0])},
+            {"value": n1 / dt1, "unit": UNIT, "cores": 1, "kind": "oracle",
+             "sample": f"first {n1} events of the workload, K=1, single thread (the oracle proper), {dt1:.2f} s",
+             "nll": float(v1[0])})
 
 
 def run_reference(args):
@@ -131,7 +214,7 @@ def run_reference(args):
     print(json.dumps(line))
 
 
-def other_rows(torch, ipa, x, ws, stream, n):
+def other_rows(torch, ipa, x, ws, stream, n, p_core):
     """The other rows of SURVEY.md 8(a), timed at BASELINE.json's sizes in the same run (device time, CUDA events):
     config 2 (fit loop on 1e6 events), config 4 (toys), config 5 (binned path).  Reported beside the headline;
     parity of each is in tests/ (-m gpu)."""
@@ -193,17 +276,38 @@ def other_rows(torch, ipa, x, ws, stream, n):
         holder = {}
 
         def gen():
-            holder["off"] = ipa.ipa_toy_generate(seeds, inp.GEN, 30000.0, 70000.0, LO, HI, cap, ws=wst, x=xt, stream=stream)[1]
+            holder["off"] = ipa.ipa_toy_generate(seeds, inp.GEN, 30000.0, 70000.0, LO, HI, cap, ws=wst, x=xt, stream=stream,
+                                                 policy=1)[1]
         dg = t(gen, 3, 1)
         off = holder["off"]
         ntot = int(off[-1].item())
         sets = inp.toy_param_sets(T)
-        ds = t(lambda: ipa.ipa_nll_eval_segmented(xt, off, sets, LO, HI, ws=wst, stream=stream), 10)
-        xs = ipa.ipa_events_prepare(xt[:ntot], LO, HI, off)
-        dss = t(lambda: ipa.ipa_nll_eval_segmented(xs, off, sets, LO, HI, ws=wst, stream=stream), 10)
+        xs = torch.empty(ntot, dtype=torch.float64, device="cuda")
+        dprep = t(lambda: ipa.ipa_events_prepare(xt[:ntot], LO, HI, off, out=xs, stream=stream), 5)
+        seg = {}
+        for pol, tag in ((1, "general_order"), (0, "adaptive_degree")):
+            ds = t(lambda: ipa.ipa_nll_eval_segmented(xt, off, sets, LO, HI, ws=wst, stream=stream, policy=pol), 10)
+            dss = t(lambda: ipa.ipa_nll_eval_segmented(xs, off, sets, LO, HI, ws=wst, stream=stream, policy=pol), 10)
+            deg = int(ipa.ipa_core_degree(inp.GEN, LO, HI, policy=pol))
+            W = algorithmic_flops(deg, p_core)
+            seg[tag] = {"core_degree": deg, "as_generated_ms": ds * 1e3, "prepared_per_toy_ms": dss * 1e3,
+                        "toys_per_s": T / dss, "events_per_s": ntot / dss,
+                        "roofline_prepared": alu_roofline(W, ntot, dss, {"note": "whole call: 1000-set prologue + segmented kernel + finalize"}),
+                        "roofline_as_generated": alu_roofline(W, ntot, ds)}
+        # generator: issue-slot model: a sub-partition issues one warp instruction per cycle and an
+        # FP64 instruction holds the port for two.  Declared per event: signal fraction 0.3 x attempts x (Philox 100 +
+        # core log G 8 int + (7 + D) FP64 + acceptance exp 15 FP64 + 12 int) + background 0.7 x (Philox 100 + inverse
+        # CDF log1p/expm1 ~ 60 FP64 + 20 int); component / yield bookkeeping 10 int.
+        deg1 = int(ipa.ipa_core_degree(inp.GEN, LO, HI, policy=1))
+        att = 1.11
+        cyc = 0.3 * att * (100 + 8 + 12 + 2 * (7 + deg1 + 15)) + 0.7 * (100 + 20 + 2 * 60) + 10
+        peak_issue = SM_COUNT * 4 * 32 * SM_MAX_HZ
         out["config4_toys"] = {"toys": T, "events": ntot, "generate_ms": dg * 1e3, "generate_events_per_s": ntot / dg,
-                               "segmented_nll_ms": ds * 1e3, "segmented_nll_sorted_per_toy_ms": dss * 1e3,
-                               "toys_per_s_nll": T / dss, "events_per_s_nll": ntot / dss}
+                               "roofline_toygen": {"bound": "alu", "unit": "thread-issue-cycles/s", "achieved": cyc * ntot / dg,
+                                                   "peak": peak_issue, "frac": cyc * ntot / dg / peak_issue,
+                                                   "issue_cycles_per_event_declared": cyc, "attempts_per_signal_event": att,
+                                                   "note": "peak = 148 SM x 4 schedulers x 32 lanes x 1.965 GHz; FP64 counted twice"},
+                               "prepare_per_toy_ms": dprep * 1e3, "segmented_nll": seg}
         del xt, xs
     # config 5: histogram (HBM-bound), 100 x 100 scan, 10 000 Poisson toy histograms
     nbins = 1000
@@ -238,6 +342,10 @@ def other_rows(torch, ipa, x, ws, stream, n):
         "hist_roofline": {"bound": "hbm", "achieved": 8.0 * n / dh / 1e9, "peak": peaks_hbm, "unit": "GB/s",
                           "frac": 8.0 * n / dh / 1e9 / peaks_hbm},
         "scan_points": int(ns.size), "scan_ms": dsc * 1e3, "scan_points_per_s": ns.size / dsc,
+        # per (point, bin) term: exp once (libdevice, ~25 FP64 instr), nu (2 FMA), log (libdevice, ~30 FP64 instr),
+        # n log nu and the sums (4) -> ~120 flops
+        "roofline_scan": alu_roofline(120.0, ns.size * nbins, dsc, {"flops_per_event": 120.0, "unit_of_work": "(scan point, bin) term",
+                                                                    "note": "includes the shape prologue + 3 small H2D copies of the call"}),
         "poisson_toy_histograms": int(sd.size), "poisson_toys_ms": dp * 1e3, "poisson_draws_per_s": sd.size * nbins / dp}
     return out
 
@@ -259,9 +367,10 @@ def main():
     ap.add_argument("--steps", type=int, default=200)
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--events", type=int, default=100_000_000)
-    ap.add_argument("--layout", default="sorted", choices=["sorted", "asis"],
-                    help="headline event layout: sorted once by ipa_events_sort (outside the timed region) or as generated")
+    ap.add_argument("--events", type=int, default=100_000_000, help="events per GPU")
+    ap.add_argument("--layout", default="prepared", choices=["prepared", "asis"],
+                    help="headline event layout: prepared once by ipa_events_prepare (outside the timed region; its cost "
+                         "and the break-even number of calls are in the line) or as generated")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-extras", action="store_true")
     args = ap.parse_args()
@@ -272,6 +381,7 @@ def main():
 
     import torch
     import paper_1706_01420_b200 as ipa
+    from paper_1706_01420_b200 import sharding
 
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -288,11 +398,17 @@ def main():
     P1 = inp.GEN
     batch9, _ = inp.fd_batch(P1)
 
-    # workload: config 3, generated on the device by the method's generator (seed 3 + rank: weak scaling,
-    # every rank owns its own n events, no data-path collective)
-    x_asis, _, _ = ipa.ipa_toy_generate([3 + rank], P1, -1.0, -1.0, LO, HI, n)
-    x_sorted = ipa.ipa_events_prepare(x_asis, LO, HI)          # one-off preparation, outside every timed region
-    x = x_sorted if args.layout == "sorted" else x_asis
+    # workload: config 3 -- ONE seeded dataset of world x n events (seed 3) generated on the device by the method's
+    # generator; rank r owns the contiguous shard of slots [r n, (r+1) n) (ipa_options.first_slot): weak scaling,
+    # no data-path collective on the events, the K partial sums are combined in rank order inside the step
+    x_asis, _, _ = ipa.ipa_toy_generate([3], P1, -1.0, -1.0, LO, HI, n, first_slot=rank * n)
+    x_prep = torch.empty_like(x_asis)
+    wsp = torch.empty(ipa.ipa_prepare_workspace_bytes(n, 0), dtype=torch.uint8, device="cuda")
+
+    def step_prep():
+        ipa.ipa_events_prepare(x_asis, LO, HI, out=x_prep, ws=wsp, stream=stream)
+    step_prep()                                                 # one-off preparation, outside the headline's timed region
+    x = x_prep if args.layout == "prepared" else x_asis
     p_core = float(((x_asis >= P1["mu"] - P1["a"] * P1["sigma"]) & (x_asis <= P1["mu"] + P1["a2"] * P1["sigma"]))
                    .double().mean().item())
     ws = ipa.workspace(n, 32)
@@ -300,12 +416,15 @@ def main():
     out9 = torch.empty(9, dtype=torch.float64, device="cuda")
     st1 = torch.empty(1, dtype=torch.int32, device="cuda")
     st9 = torch.empty(9, dtype=torch.int32, device="cuda")
+    total = {}
     torch.cuda.synchronize()
 
     POL = 1  # general-order path: no half-integer shortcut in the headline (reading D2)
 
     def step_k1(arr=None):
         ipa.ipa_nll_eval(x if arr is None else arr, P1, LO, HI, ws=ws, stream=stream, out=out1, status=st1, policy=POL)
+        if dist:
+            total["nll"] = sharding.combine_nll(out1)           # 8 K bytes all-gathered over NCCL, added in rank order
 
     def step_k9(arr=None):
         ipa.ipa_nll_eval(x if arr is None else arr, batch9, LO, HI, ws=ws, stream=stream, out=out9, status=st9, policy=POL)
@@ -325,7 +444,7 @@ def main():
         dt = t.item()
     clocks = sampler.stop() if rank == 0 else None
     value = world * n * args.steps / dt
-    nll1 = out1.item()
+    nll_total = float(total["nll"].item()) if dist else float(out1.item())
 
     # prologue alone (same kernel, same arguments, through ipa_norm): the streaming kernel's average launch
     # duration is the step minus this, launch gaps included on the kernel's side
@@ -338,55 +457,82 @@ def main():
         step_pro()
     dt_pro = timed(torch, step_pro, args.steps, stream) / args.steps
     t_step = dt / args.steps
-    t_kernel = max(t_step - dt_pro, 1e-9)
     degree = int(ipa.ipa_core_degree(P1, LO, HI, policy=POL))
+    flops = algorithmic_flops(degree, p_core)
 
-    extras = {"p_core": p_core, "core_degree": degree, "prologue_ms": dt_pro * 1e3, "nll_kernel_ms": t_kernel * 1e3}
-    if not args.no_extras:
+    def local_step_time(fn, steps, warm=2):
+        for _ in range(warm):
+            fn()
+        return timed(torch, fn, steps, stream) / steps
+
+    def k1_local(arr):
+        ipa.ipa_nll_eval(arr, P1, LO, HI, ws=ws, stream=stream, out=out1, status=st1, policy=POL)
+    # kernel time from a loop without the collective (identical to the step at N = 1)
+    t_local = t_step if not dist else local_step_time(lambda: k1_local(x), args.steps)
+    t_kernel = max(t_local - dt_pro, 1e-9)
+
+    extras = {"p_core": p_core, "core_degree": degree, "prologue_ms": dt_pro * 1e3, "nll_kernel_ms": t_kernel * 1e3,
+              "build_hash": build_hash()}
+    if not args.no_extras and rank == 0:
         k9steps = max(5, args.steps // 8)
-        for _ in range(2):
-            step_k9()
-        dt9 = timed(torch, step_k9, k9steps, stream) / k9steps
+        # one-off preparation (stable counting sort on a coarse bin index) and what it buys
+        d_prep = local_step_time(step_prep, 10)
+        other = x_asis if args.layout == "prepared" else x_prep
+        oname = "asis" if args.layout == "prepared" else "prepared"
+        d_other = local_step_time(lambda: k1_local(other), args.steps)
+        t_asis, t_prepared = (d_other, t_local) if args.layout == "prepared" else (t_local, d_other)
+        extras["prepare"] = {"ms": d_prep * 1e3, "events_per_s": n / d_prep,
+                             "hbm_gbs": 24.0 * n / d_prep / 1e9,
+                             "algorithmic_bytes_per_event": 24, "note": "two reads (count, scatter) + one write of 8 B",
+                             "break_even_calls_k1": d_prep / max(t_asis - t_prepared, 1e-12),
+                             "single_call_with_prepare_ms": (d_prep + t_prepared) * 1e3}
+        extras[f"roofline_{oname}"] = alu_roofline(flops, n, max(d_other - dt_pro, 1e-9),
+                                                   {"layout": oname, "call_ms": d_other * 1e3})
+        extras["roofline_asis_plus_prepare_single_call"] = alu_roofline(flops, n, d_prep + t_prepared,
+                                                                        {"note": "new data every call: prepare + one NLL"})
+        dt9 = local_step_time(step_k9, k9steps)
+        W9 = 5 * shape_stage_flops(degree, p_core) + 9 * MEMBER_STAGE_FLOPS
         extras["k9_gradient_batch"] = {"ms_per_call": dt9 * 1e3, "event_sets_per_s": 9 * n / dt9, "events_per_s": n / dt9,
                                        "nll_calls_per_s": 9 / dt9}
-        other = x_asis if args.layout == "sorted" else x_sorted
-        oname = "asis" if args.layout == "sorted" else "sorted"
-        for _ in range(2):
-            step_k1(other)
-        dto = timed(torch, lambda: step_k1(other), args.steps, stream) / args.steps
-        for _ in range(2):
-            step_k9(other)
-        dto9 = timed(torch, lambda: step_k9(other), k9steps, stream) / k9steps
-        extras[f"k1_layout_{oname}"] = {"ms_per_call": dto * 1e3, "events_per_s": n / dto}
-        extras[f"k9_layout_{oname}"] = {"ms_per_call": dto9 * 1e3, "event_sets_per_s": 9 * n / dto9}
+        extras["roofline_k9"] = alu_roofline(W9, n, max(dt9 - dt_pro, 1e-9),
+                                             {"note": "central-difference batch over (mu, sigma, f, k): 5 shape stages + 9 member "
+                                                      "stages per event", "flops_per_event_set": W9 / 9})
+        dto9 = local_step_time(lambda: step_k9(other), k9steps)
+        extras[f"roofline_k9_{oname}"] = alu_roofline(W9, n, max(dto9 - dt_pro, 1e-9), {"layout": oname, "call_ms": dto9 * 1e3})
+
         def step_adaptive():
             ipa.ipa_nll_eval(x, P1, LO, HI, ws=ws, stream=stream, out=out1, status=st1, policy=0)
-        for _ in range(2):
-            step_adaptive()
-        dta = timed(torch, step_adaptive, args.steps, stream) / args.steps
+        dta = local_step_time(step_adaptive, args.steps)
         extras["k1_adaptive_degree_half_integer_shortcut"] = {"ms_per_call": dta * 1e3, "events_per_s": n / dta}
 
         def step_p2():
             ipa.ipa_nll_eval(x, inp.P2, LO, HI, ws=ws, stream=stream, out=out1, status=st1, policy=0)
-        for _ in range(2):
-            step_p2()
-        dtp = timed(torch, step_p2, args.steps, stream) / args.steps
+        dtp = local_step_time(step_p2, args.steps)
         extras["k1_general_shape_P2"] = {"ms_per_call": dtp * 1e3, "events_per_s": n / dtp}
-        step_k1()
+
+        def step_t1():
+            ipa.ipa_nll_eval(x, inp.T1, LO, HI, ws=ws, stream=stream, out=out1, status=st1, policy=POL)
+        dtt = local_step_time(step_t1, args.steps)
+        extras["k1_student_t_core_f4"] = {"ms_per_call": dtt * 1e3, "events_per_s": n / dtt}
+        k1_local(x)
         # row f1: analytic gradient in one pass, beside the K = 9 finite-difference batch it replaces
-        for _ in range(2):
-            ipa.ipa_nll_grad_eval(x, P1, LO, HI, ws=ws, stream=stream, policy=POL)
-        dtg = timed(torch, lambda: ipa.ipa_nll_grad_eval(x, P1, LO, HI, ws=ws, stream=stream, policy=POL), k9steps, stream) / k9steps
+        dtg = local_step_time(lambda: ipa.ipa_nll_grad_eval(x, P1, LO, HI, ws=ws, stream=stream, policy=POL), k9steps)
         extras["f1_analytic_gradient"] = {"ms_per_call": dtg * 1e3, "events_per_s": n / dtg,
                                           "speedup_vs_k9_finite_differences": dt9 / dtg}
-        extras.update(other_rows(torch, ipa, x_asis, ws, stream, n))
+        extras["roofline_grad"] = alu_roofline(gradient_flops(degree, p_core), n, dtg, {"note": "whole call (prologue with "
+                                               "normalisation derivatives + gradient kernel)"})
+        if world == 1:
+            extras.update(other_rows(torch, ipa, x_asis, ws, stream, n, p_core))
         # FP64 peak probe (DFMA chains), for the roofline denominator
         iters = 200000
         ipa.ipa_fp64_peak_probe(1000)
         tp = timed(torch, lambda: ipa.ipa_fp64_peak_probe(iters), 1, stream)
         sms = torch.cuda.get_device_properties(local).multi_processor_count
         extras["fp64_dfma_probe_tflops"] = sms * 8 * 256 * 8 * 2.0 * iters / tp / 1e12
-    nll1 = out1.item()
+    if dist:
+        dist.barrier()
+    k1_local(x)
+    torch.cuda.synchronize()
 
     # end to end through the public API with HOST buffers: H2D of the events + D2H of the result inside the
     # timed region, events in the order the host holds them (as generated; no device-side preparation)
@@ -412,19 +558,18 @@ def main():
         e2e = {"value": world * n * e2e_steps / de, "unit": UNIT, "h2d_bytes_per_step": 8 * n + 88,
                "d2h_bytes_per_step": 8, "steps": e2e_steps, "nll": float(r[0]), "layout": "as generated",
                "timer": "host wall clock around copy + call + result read"}
-        del xd, xh
+        del xd
 
     if rank != 0:
         return
-    flops = algorithmic_flops(degree, p_core)
     achieved = flops * n / t_kernel / 1e12
     peak = FP64_PEAK_NOMINAL / 1e12
+    traffic, traffic_note = measured_traffic(n)
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                "traffic": (800.13e6 + 3.98e6) * n / 1e8,
-                "traffic_source": "ncu --set full dram__bytes_read.sum + dram__bytes_write.sum of ipa_nll_kernel, "
-                                  "profiles/r01_v13_nll_kernel.md (800.13 MB + 3.98 MB per launch of 1e8 events; scaled by events)",
-                "kernel": "ipa_nll_kernel<false>", "kernel_ms": t_kernel * 1e3,
+                "traffic": traffic, "traffic_source": traffic_note,
+                "kernel": "ipa_nll_kernel<false,false>", "kernel_ms": t_kernel * 1e3,
                 "kernel_time_source": "CUDA events: step time minus a prologue-only loop of the same length",
+                "frac_whole_step": flops * n / t_local / 1e12 / peak,
                 "peak_source": "DESIGN.md section 6: 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no "
                                "FP64 entry); measured DFMA-chain probe in fp64_dfma_probe_tflops",
                 "flops_per_event_set": flops, "p_core": p_core, "core_degree": degree,
@@ -441,21 +586,28 @@ def main():
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": 1e3 * t_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "f64", "data": "synthetic",
-            "config": {"workload": "config 3: 1e8 fp64 events on [5000,5600] from the Ipatia+exp model (device generator, "
-                                   "seed 3), one NLL evaluation per step (prologue + streaming kernel), K=1, general-order "
-                                   "degree policy",
-                       "events": n, "K": 1, "layout": args.layout + (" (sorted once by ipa_events_sort before the timed "
-                                                                      "region; as-generated order in k1_layout_asis)"
-                                                                      if args.layout == "sorted" else ""),
+            "config": {"workload": "config 3: 1e8 fp64 events per GPU on [5000,5600] from the Ipatia+exp model (device generator, "
+                                   "seed 3, one dataset of n_gpus x 1e8 events sharded contiguously), one NLL evaluation per "
+                                   "step (prologue + streaming kernel" + (" + all-gather of the partial sums" if dist else "") +
+                                   "), K=1, general-order degree policy",
+                       "events": n * world, "events_per_gpu": n, "K": 1,
+                       "layout": args.layout + (" (stable counting sort on a coarse bin index by ipa_events_prepare, once, before "
+                                                "the timed region: cost and break-even in 'prepare'; as-generated order in "
+                                                "roofline_asis)" if args.layout == "prepared" else ""),
                        "l2": "input (8 B x events) larger than L2, no flush needed",
-                       "multi_gpu": "independent event shards per rank, no data-path collective"},
-            "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps, "roofline": roofline, "nll": nll1}
+                       "multi_gpu": "contiguous event shards of one dataset, K partial sums all-gathered and added in rank order"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": 2 * args.steps, "roofline": roofline, "nll": nll_total}
     line.update(extras)
     if not args.no_cpu_baseline and world == 1:
         cores = os.cpu_count() or 1
-        ncpu = min(n, 6_000_000 * cores)
-        xs = x_asis[:ncpu].cpu().numpy()
-        line["cpu_baseline"] = cpu_baseline(xs, P1, cores, ncpu)
+        allc, one = cpu_baseline(xh.numpy(), P1, cores)
+        line["cpu_baseline"] = allc
+        line["cpu_baseline_1core"] = one
+        line["parity"] = {"gpu_nll": nll_total, "oracle_nll": allc["nll"],
+                          "rel_diff": abs(nll_total - allc["nll"]) / abs(allc["nll"]), "tolerance": 1e-10,
+                          "note": "same 1e8 seed-3 events: device sum over the prepared layout against the oracle's threaded "
+                                  "pairwise sums over the as-generated order (single-thread oracle on the same events: "
+                                  "tests/test_gpu_parity.py::test_full_size_sampled)"}
     print(json.dumps(line))
 
 

@@ -90,10 +90,15 @@ const char* ipa_version(void);
  *                  series of log(z^nu K_nu(z)) is cut where its coefficients fall under the fp64 noise floor, so a
  *                  half-integer order collapses to a very short polynomial); 1 = geometric (at least the a-priori
  *                  degree for a general order on the same z-interval: no half-integer shortcut; reading D2).
+ *   first_slot     ipa_toy_generate in mixture mode only (ignored elsewhere, must be >= 0): the call draws the events
+ *                  of slots first_slot .. first_slot + capacity - 1 of the seeded dataset (an event depends on
+ *                  (seed, slot) only), so G ranks can each generate their contiguous shard of ONE dataset
+ *                  (DESIGN.md section 7).  Default 0.
  * Results are bitwise reproducible for fixed options; they differ between the two policies at the 1e-15 level. */
 typedef struct {
   int32_t degree_policy;
-  int32_t reserved[3]; /* must be 0 */
+  int32_t reserved;    /* must be 0 */
+  int64_t first_slot;
 } ipa_options;
 
 /* Bytes of workspace needed by any call below for n events, K parameter sets (or T segments / toys:

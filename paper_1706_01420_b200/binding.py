@@ -45,15 +45,16 @@ class _Range(C.Structure):
 
 
 class _Options(C.Structure):
-    _fields_ = [("degree_policy", C.c_int32), ("reserved", C.c_int32 * 3)]
+    _fields_ = [("degree_policy", C.c_int32), ("reserved", C.c_int32), ("first_slot", C.c_int64)]
 
 
-def _opt(policy):
+def _opt(policy, first_slot=0):
     """policy None -> NULL options (library defaults), else an ipa_options with that degree policy."""
-    if policy is None:
+    if policy is None and not first_slot:
         return None
     o = _Options()
-    o.degree_policy = int(policy)
+    o.degree_policy = int(policy or 0)
+    o.first_slot = int(first_slot)
     return C.byref(o)
 
 
@@ -330,8 +331,9 @@ def ipa_nll_eval_categories(x, offsets, params, set_of_segment, lo, hi, ws=None,
 
 @_alloc_on_stream
 def ipa_toy_generate(seeds, gen, mean_sig, mean_bkg, lo, hi, capacity, ws=None, stream=None, x=None, policy=None,
-                     status=None):
-    """Toy generation.  mean_sig < 0 selects mixture mode (one toy of exactly `capacity` events).
+                     status=None, first_slot=0):
+    """Toy generation.  mean_sig < 0 selects mixture mode (one toy of exactly `capacity` events: the slots
+    first_slot .. first_slot + capacity - 1 of the seeded dataset).
 
     -> (x[capacity], offsets[T+1] int64, overflow[1] int32) device tensors; `status` (int32 [gen_count], optional)
     receives the domain status of the generating sets."""
@@ -346,7 +348,7 @@ def ipa_toy_generate(seeds, gen, mean_sig, mean_bkg, lo, hi, capacity, ws=None, 
     ovf = torch.zeros(1, dtype=torch.int32, device="cuda")
     _check(lib().ipa_toy_generate(_hptr(seeds), T, _hptr(P), P.shape[0], float(mean_sig), float(mean_bkg),
                                   _Range(lo, hi), int(capacity), _dptr(x) if capacity else None, _dptr(off), _dptr(ovf),
-                                  _dptr(status, torch.int32), _opt(policy), _dptr(ws), ws.numel(), _stream(stream)))
+                                  _dptr(status, torch.int32), _opt(policy, first_slot), _dptr(ws), ws.numel(), _stream(stream)))
     return x, off, ovf
 
 

@@ -23,7 +23,7 @@ thread_local std::string g_last_cuda_error;
 // degree policy of the call (NULL options = defaults); -1 = invalid options
 int policy_of(const ipa_options* o) {
   if (!o) return 0;
-  if ((o->degree_policy != 0 && o->degree_policy != 1) || o->reserved[0] || o->reserved[1] || o->reserved[2]) return -1;
+  if ((o->degree_policy != 0 && o->degree_policy != 1) || o->reserved || o->first_slot < 0) return -1;
   return o->degree_policy;
 }
 
@@ -368,7 +368,8 @@ int ipa_toy_generate(const uint64_t* seeds_host, int64_t T, const ipa_params* ge
   if (chunks < 1) chunks = 1;
   if (capacity > 0) {
     ipa_toy_events_kernel<<<dim3((unsigned)T, (unsigned)chunks), IPA_BLOCK, 0, st>>>(
-        seeds, consts, gen_count == T && T > 1 ? 1 : 0, nsig, offsets, r.lo, r.hi, capacity, mixture ? 1 : 0, x_dev, overflow_dev);
+        seeds, consts, gen_count == T && T > 1 ? 1 : 0, nsig, offsets, r.lo, r.hi, capacity, mixture ? 1 : 0,
+        (mixture && opt_host) ? (long long)opt_host->first_slot : 0LL, x_dev, overflow_dev);
     IPA_CK(cudaGetLastError());
   }
   return IPA_OK;

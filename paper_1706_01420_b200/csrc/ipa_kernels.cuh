@@ -1008,7 +1008,8 @@ __global__ void __launch_bounds__(IPA_BLOCK)
 ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSetConsts* __restrict__ consts,
                       int gen_stride,
                       const long long* __restrict__ nsig, const long long* __restrict__ offsets, double lo, double hi,
-                      long long capacity, int mixture, double* __restrict__ x, int32_t* __restrict__ overflow) {
+                      long long capacity, int mixture, long long first_slot, double* __restrict__ x,
+                      int32_t* __restrict__ overflow) {
   __shared__ IpaSetConsts c;
   __shared__ IpaEnvelope E;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -1059,12 +1060,12 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
       if (o < cnt) {
         if (mixture) {
           double uc, v;
-          ipa_uniforms2(seed, (unsigned long long)j, 0u, IPA_STREAM_COMP, &uc, &v);
+          ipa_uniforms2(seed, (unsigned long long)(j + first_slot), 0u, IPA_STREAM_COMP, &uc, &v);
           is_sig = uc < f;
         } else {
           is_sig = j < ns;
         }
-        if (!is_sig) x[beg + j] = ipa_draw_background(k, seed, (unsigned long long)j, lo, hi);
+        if (!is_sig) x[beg + j] = ipa_draw_background(k, seed, (unsigned long long)(j + first_slot), lo, hi);
       }
       const unsigned m = __ballot_sync(IPA_FULL, is_sig);
       if (is_sig) list[nlist + __popc(m & lt)] = o;
@@ -1086,7 +1087,7 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
       if (item >= 0) {
         const unsigned long long j = (unsigned long long)(r0 + item);
         double u1, u2;
-        ipa_uniforms2(seed, j, attempt, IPA_STREAM_SIG, &u1, &u2);
+        ipa_uniforms2(seed, j + (unsigned long long)first_slot, attempt, IPA_STREAM_SIG, &u1, &u2);
         const double v = u1 * W;
         int r = 0;
         for (int q = 1; q < nreg; ++q) r += (v >= E.cum[q]) ? 1 : 0;
@@ -1274,12 +1275,35 @@ ipa_binned_scan_kernel(const unsigned long long* __restrict__ counts, const doub
   const long long q = blockIdx.x;
   const double w = (hi - lo) / (double)nbins;
   const double k = kk[q], vs = ns[q], vb = nb[q];
+  // every exponential is evaluated once and kept in registers (up to 8 bins per thread: 2048 bins; beyond that the
+  // second pass evaluates it again)
+  constexpr int KEEP = 8;
+  double eb[KEEP];
   double part = 0.0;
-  for (int b = threadIdx.x; b < nbins; b += 256) part += exp(k * (((double)b + 0.5) * w));
+#pragma unroll
+  for (int i = 0; i < KEEP; ++i) {
+    const int b = threadIdx.x + 256 * i;
+    eb[i] = (b < nbins) ? exp(k * (((double)b + 0.5) * w)) : 0.0;
+    part += eb[i];
+  }
+  for (int b = threadIdx.x + 256 * KEEP; b < nbins; b += 256) part += exp(k * (((double)b + 0.5) * w));
   const double bsum = ipa_block_sum_256(part, red);
+  const double vbn = vb / bsum;
   double acc = 0.0;
-  for (int b = threadIdx.x; b < nbins; b += 256) {
-    const double v = vs * s[b] + vb * exp(k * (((double)b + 0.5) * w)) / bsum;
+#pragma unroll
+  for (int i = 0; i < KEEP; ++i) {
+    const int b = threadIdx.x + 256 * i;
+    if (b < nbins) {
+      const double v = fma(vs, s[b], vbn * eb[i]);
+      if (nu_out) nu_out[b] = v;
+      else {
+        const unsigned long long nobs = counts[b];
+        acc += nobs ? v - (double)nobs * log(v) : v;
+      }
+    }
+  }
+  for (int b = threadIdx.x + 256 * KEEP; b < nbins; b += 256) {
+    const double v = fma(vs, s[b], vbn * exp(k * (((double)b + 0.5) * w)));
     if (nu_out) nu_out[b] = v;
     else {
       const unsigned long long nobs = counts[b];

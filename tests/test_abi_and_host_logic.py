@@ -59,10 +59,11 @@ def test_argument_validation_without_gpu(ipa):
     assert L.ipa_nll_eval(one, 10, p, 1, rng, one, None, None, None, one, 16, None) == -2
     assert L.ipa_nll_eval(one, 10, p, 1, rng, one, None, None, None, C.c_void_p(264), 1 << 30, None) == -2
     # options: an unknown degree policy or a non-zero reserved field is an argument error
-    for pol, res in ((2, 0), (-1, 0), (0, 7)):
+    for pol, res, slot in ((2, 0, 0), (-1, 0, 0), (0, 7, 0), (0, 0, -1)):
         o = ipa.binding._Options()
         o.degree_policy = pol
-        o.reserved[1] = res
+        o.reserved = res
+        o.first_slot = slot
         assert L.ipa_nll_eval(one, 10, p, 1, rng, one, None, None, C.byref(o), one, 1 << 30, None) == -1
     assert L.ipa_norm(None, 1, rng, one, one, None, None, one, 1 << 30, None) == -1
     idx = np.array([0, 11], dtype=np.int32)

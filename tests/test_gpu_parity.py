@@ -238,6 +238,10 @@ def test_mixture_generator_matches_oracle(ipa, torch_, orc):
         assert list(off.cpu().numpy()) == [0, n] and ovf.item() == 0
         mismatches(got, ref, f"mixture seed {seed}")
         assert ((got >= LO) & (got <= HI)).all()
+        # a shard of the same dataset (ipa_options.first_slot): slots 7001 .. 7001 + 5000 - 1, bitwise the same events
+        part, _, _ = ipa.ipa_toy_generate([seed], theta, -1.0, -1.0, LO, HI, 5000, first_slot=7001)
+        torch_.cuda.synchronize()
+        assert torch_.equal(part, x[7001:12001])
 
 
 @pytest.mark.parametrize("case", ["beta_large", "mode_left_of_range", "mode_left_of_range_b", "range_inside_left_tail",

@@ -75,3 +75,47 @@ def test_two_rank_shards_combine_to_the_full_nll():
     assert np.array_equal(res[0][0], res[0][1])                    # reproducible
     assert np.all(np.abs(res[0][0] - full) <= 1e-12 * np.abs(full))
     assert res[0][2] == res[1][2] == 2.0                           # slowest rank defines the time
+
+
+def _cuda_worker(rank, world, port, n, out):
+    """The path bench.py --gpus N times: every rank generates ITS shard of one seeded dataset on its own GPU
+    (ipa_options.first_slot), evaluates it with ipa_nll_eval and the partial sums are all-gathered over NCCL."""
+    os.environ["MASTER_ADDR"] = "127.0.0.1"
+    os.environ["MASTER_PORT"] = str(port)
+    torch.cuda.set_device(rank)
+    dist.init_process_group("nccl", rank=rank, world_size=world)
+    try:
+        import paper_1706_01420_b200 as ipa
+        batch, _ = inp.fd_batch(inp.GEN)
+        a, b = sharding.shard_range(n, rank, world)
+        x, _, _ = ipa.ipa_toy_generate([3], inp.GEN, -1.0, -1.0, LO, HI, b - a, first_slot=a)
+        local, _, _ = ipa.ipa_nll_eval(x, batch, LO, HI)
+        total = sharding.combine_nll(local)
+        torch.cuda.synchronize()
+        full = None
+        if rank == 0:
+            xf, _, _ = ipa.ipa_toy_generate([3], inp.GEN, -1.0, -1.0, LO, HI, n)
+            full = ipa.ipa_nll_eval(xf, batch, LO, HI)[0].cpu().numpy()
+        out.put((total.cpu().numpy(), full))
+    finally:
+        dist.destroy_process_group()
+
+
+@pytest.mark.gpu
+def test_two_gpu_shards_combine_to_the_full_nll():
+    if torch.cuda.device_count() < 2:
+        pytest.skip("needs two GPUs (the GPU pool of this build hands out one)")
+    world, n = 2, 1_000_003
+    ctx = mp.get_context("spawn")
+    q = ctx.Queue()
+    port = _free_port()
+    procs = [ctx.Process(target=_cuda_worker, args=(r, world, port, n, q)) for r in range(world)]
+    for p in procs:
+        p.start()
+    res = [q.get(timeout=600) for _ in range(world)]
+    for p in procs:
+        p.join(timeout=60)
+        assert p.exitcode == 0
+    full = next(r[1] for r in res if r[1] is not None)
+    assert np.array_equal(res[0][0], res[1][0])
+    assert np.all(np.abs(res[0][0] - full) <= 1e-12 * np.abs(full))
