@@ -44,7 +44,7 @@ Layout make_layout(int64_t K, int64_t nbins) {
   L.counter = o;  o += 256;
   const int64_t kk = K < IPA_MAX_K ? K : IPA_MAX_K;
   size_t pb = (size_t)kk * kGridMax * 8;
-  if ((size_t)K * IPA_SEGC * 8 > pb) pb = (size_t)K * IPA_SEGC * 8;
+  if ((size_t)K * IPA_SEGC * 8 > pb) pb = (size_t)K * IPA_SEGC * 8;   // segmented call: T * C partials, T * C <= max(8 T, 592 + T)
   L.partials = o; o += align_up(pb, 256);
   L.params = o;   o += align_up((size_t)K * sizeof(ipa_params), 256);
   L.seeds = o;    o += align_up((size_t)K * 8, 256);
@@ -300,10 +300,18 @@ static int segmented_common(const double* x_dev, const int64_t* offsets_dev, int
     IPA_CK(cudaMemcpyAsync(ws + L.nsig, set_of_segment_host, (size_t)T * 4, cudaMemcpyHostToDevice, st));
     map = reinterpret_cast<const int*>(ws + L.nsig);
   }
-  ipa_nll_seg_kernel<<<dim3((unsigned)T, IPA_SEGC), IPA_BLOCK, 0, st>>>(
+  // chunks per segment: IPA_SEGC, more when few segments would leave SMs idle (T * C >= resident blocks of the device)
+  int sms = 0;
+  rc = device_info(&sms);
+  if (rc) return rc;
+  int64_t C = IPA_SEGC;
+  const int64_t resident = (int64_t)sms * IPA_BLOCKS_PER_SM;
+  if (T * C < resident) C = (resident + T - 1) / T;
+  if (C > 64) C = 64;
+  ipa_nll_seg_kernel<<<dim3((unsigned)T, (unsigned)C), IPA_BLOCK, 0, st>>>(
       x_dev, reinterpret_cast<const long long*>(offsets_dev), consts, map, partials);
   IPA_CK(cudaGetLastError());
-  ipa_seg_finalize_kernel<<<(unsigned)((T + 127) / 128), 128, 0, st>>>(partials, consts, map, T, nll_dev, status_dev);
+  ipa_seg_finalize_kernel<<<(unsigned)((T + 127) / 128), 128, 0, st>>>(partials, consts, map, T, (int)C, nll_dev, status_dev);
   IPA_CK(cudaGetLastError());
   return IPA_OK;
 }

@@ -19,7 +19,7 @@ struct IpaParamBatch { ipa_params p[IPA_MAX_K]; };
 // ------------------------------------------------------------------------------------------------
 // Prologue: one block per parameter set.
 // ------------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(IPA_PRO_THREADS, 3)
+__global__ void __launch_bounds__(IPA_PRO_THREADS, 4)
 ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_params* __restrict__ p_dev, double lo,
                     double hi, int policy, IpaSetConsts* __restrict__ consts, unsigned int* counter,
                     double* norm_sig, double* norm_bkg, int32_t* status_out) {
@@ -295,6 +295,13 @@ __device__ __forceinline__ double ipa_warp_sum(double v) {
 #define IPA_NB_PER_SM 1
 #endif
 
+// Tile layout (streaming and segmented kernels, E = 8 events per thread): the 32 x E events of a WARP are contiguous
+// (2 KB), a thread holds E/2 pairs 512 B apart.  Every cp.async / shared load of a warp covers 512 contiguous bytes,
+// and a warp of a prepared (sorted) array spans 256 consecutive events: the fewest possible region-mixed warps.
+__device__ __forceinline__ int ipa_ev_off(int tid, int e) {
+  return (tid >> 5) * (32 * IPA_NE) + 2 * ((e >> 1) * 32 + (tid & 31)) + (e & 1);
+}
+
 __device__ __forceinline__ void ipa_load_logtab(double2* tab) {
   if (threadIdx.x < 33) tab[threadIdx.x] = ipa_c_logtab[threadIdx.x];
 }
@@ -323,21 +330,21 @@ struct IpaGroups { signed char leader[IPA_MAX_K]; };
 // All K parameter sets on the IPA_NE events a thread holds in registers (A2-A4): one shape stage per
 // group, one member stage per set; optional per-event output; accumulation into the thread's
 // shared-memory accumulators (first level of A5).
-// Event e of thread tid in the tile at `base` is x[base + 2 ((e >> 1) IPA_NB + tid) + (e & 1)].
+// Event e of thread tid in the tile at `base` is x[base + ipa_ev_off(tid, e)].
 template <bool LOGPDF, bool FULL>
 __device__ __forceinline__ void ipa_tile_store_acc(int k, double (&l)[IPA_NE], double* acc, long long base, long long n,
                                                    int tid, double* __restrict__ logpdf) {
   if (!FULL) {
 #pragma unroll
     for (int e = 0; e < IPA_NE; ++e) {
-      const long long i = base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1);
+      const long long i = base + ipa_ev_off(tid, e);
       if (LOGPDF && i < n) logpdf[(long long)k * n + i] = l[e];
       if (i >= n) l[e] = 0.0;
     }
   } else if (LOGPDF) {
 #pragma unroll
     for (int e = 0; e < IPA_NE; ++e)
-      logpdf[(long long)k * n + base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1)] = l[e];
+      logpdf[(long long)k * n + base + ipa_ev_off(tid, e)] = l[e];
   }
   double sl = 0.0;
 #pragma unroll
@@ -359,7 +366,7 @@ __device__ __forceinline__ void ipa_tile_sets(const IpaSetConsts* sc, int K, con
       if (!sc[k].status) continue;
 #pragma unroll
       for (int e = 0; e < IPA_NE; ++e) {
-        const long long i = base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1);
+        const long long i = base + ipa_ev_off(tid, e);
         if (FULL || i < n) logpdf[(long long)k * n + i] = NAN;
       }
     }
@@ -412,13 +419,13 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int G = gridDim.x;
   const int nfull = vec_ok ? (int)(n / IPA_NTILE) : 0;            // tiles of the staged loop (n < 2^43)
-  const unsigned slot = (unsigned)__cvta_generic_to_shared(stage) + 16u * tid;
-  const double* src = x + (long long)blockIdx.x * IPA_NTILE + 2 * tid;
+  const unsigned slot = (unsigned)__cvta_generic_to_shared(stage) + (unsigned)(warp * (32 * IPA_NE * 8) + 16 * lane);
+  const double* src = x + (long long)blockIdx.x * IPA_NTILE + warp * (32 * IPA_NE) + 2 * lane;
   const long long src_step = (long long)G * IPA_NTILE;
   int tile = blockIdx.x;
   if (tile < nfull) {
 #pragma unroll
-    for (int p = 0; p < IPA_NE / 2; ++p) ipa_cp_async16_s(slot + p * (IPA_NB * 16), src + p * (IPA_NB * 2));
+    for (int p = 0; p < IPA_NE / 2; ++p) ipa_cp_async16_s(slot + p * 512, src + p * 64);
   }
   ipa_cp_async_commit();
   {
@@ -436,7 +443,7 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
     ipa_cp_async_wait_all();
 #pragma unroll
     for (int p = 0; p < IPA_NE / 2; ++p) {
-      const double2 v = ipa_lds128(slot + bufoff + p * (IPA_NB * 16));
+      const double2 v = ipa_lds128(slot + bufoff + p * 512);
       xv[2 * p] = v.x;
       xv[2 * p + 1] = v.y;
     }
@@ -445,7 +452,7 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
     if (tile + G < nfull) {
 #pragma unroll
       for (int p = 0; p < IPA_NE / 2; ++p)
-        ipa_cp_async16_s(slot + bufoff + p * (IPA_NB * 16), src + p * (IPA_NB * 2));
+        ipa_cp_async16_s(slot + bufoff + p * 512, src + p * 64);
     }
     ipa_cp_async_commit();
     ipa_tile_sets<LOGPDF, true, GROUPED>(sc, K, grp, acc, xv, (long long)tile * IPA_NTILE, n, tid, logpdf, s_tab);
@@ -465,7 +472,7 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
       double xv[IPA_NE];
 #pragma unroll
       for (int e = 0; e < IPA_NE; ++e) {
-        const long long i = base + 2LL * ((e >> 1) * IPA_NB + tid) + (e & 1);
+        const long long i = base + ipa_ev_off(tid, e);
         xv[e] = (i < n) ? x[i] : xpad;
       }
       ipa_tile_sets<LOGPDF, false, GROUPED>(sc, K, grp, acc, xv, base, n, tid, logpdf, s_tab);
@@ -637,6 +644,7 @@ IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&
 #ifndef IPA_GPSM
 #define IPA_GPSM 1                        // blocks per SM
 #endif
+static_assert(IPA_E == IPA_NE, "ipa_ev_off serves both tile shapes");
 static_assert(IPA_GB >= 160 && IPA_GB % 32 == 0, "the final reduction of the gradient kernel uses one warp per sum");
 // grid (G, K): every set streams the events on its own (the gradient call is made for one or a few sets);
 // per-thread register accumulators, fixed block tree, partials[(k 5 + c) G + b], the last block of each
@@ -726,16 +734,14 @@ ipa_nll_grad_kernel(const double* __restrict__ x, long long n, int vec_ok, const
 }
 
 // ------------------------------------------------------------------------------------------------
-// Segmented NLL (T2): grid (T, IPA_SEGC); block (t, c) takes the c-th eighth of segment t with the
-// parameter set of that segment.
+// Segmented NLL (T2): grid (T, C); block (t, c) takes the c-th of C chunks of segment t with the parameter set of
+// that segment.  Same design as the streaming kernel: the 16-byte aligned body of the chunk travels global ->
+// shared in full tiles with 16-byte cp.async.cg copies two tiles deep (every thread copies and later reads its
+// OWN slots: no barrier in the loop, no per-event bounds test); the at most one unaligned head event and the
+// ragged tail (< one tile) are evaluated afterwards from plain loads in one masked tile whose empty slots repeat
+// the chunk's last event, so that a warp of a prepared (sorted) segment stays region-uniform.
+// partials[t * C + c]; ipa_seg_finalize_kernel adds the C partials of a segment in fixed order.
 // ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ void ipa_cp_async8(void* smem_dst, const void* gmem_src) {
-  const unsigned d = (unsigned)__cvta_generic_to_shared(smem_dst);
-  asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"(d), "l"(gmem_src) : "memory");
-}
-
-// Same staging as the streaming kernel, with 8-byte copies (a segment starts at any event index): the copy
-// of the next tile flies while the current one is evaluated; each thread reads only its own slots.
 __global__ void __launch_bounds__(IPA_BLOCK, IPA_BLOCKS_PER_SM)
 ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ offsets,
                    const IpaSetConsts* __restrict__ consts, const int* __restrict__ set_of_segment,
@@ -745,41 +751,76 @@ ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ o
   __shared__ double2 s_tab[33];
   __shared__ __align__(16) double stage[2][IPA_TILE];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  const int C = gridDim.y;
   const long long t = blockIdx.x;
   const long long beg = offsets[t], len = offsets[t + 1] - beg;
-  const long long cb = beg + len * blockIdx.y / IPA_SEGC, ce = beg + len * (blockIdx.y + 1) / IPA_SEGC;
-  auto issue = [&](long long base, int buf) {
+  const long long end = beg + len;
+  // The 16-byte aligned body of the segment, [a0, a0 + ntl IPA_TILE), is dealt out in whole tiles: chunk c takes tiles
+  // [c per, (c+1) per).  The at most one unaligned head event [beg, a0) and the ragged tail (< one tile) go to the LAST
+  // chunk, so a segment pays ONE masked tile instead of one per chunk.
+  long long a0 = beg + (long long)((reinterpret_cast<unsigned long long>(x + beg) >> 3) & 1ull);
+  if (a0 > end) a0 = end;
+  const long long ntl = (end - a0) / IPA_TILE;
+  const long long per = (ntl + C - 1) / C;
+  long long m0 = per * blockIdx.y, m1 = m0 + per;
+  if (m0 > ntl) m0 = ntl;
+  if (m1 > ntl) m1 = ntl;
+  const bool last_chunk = blockIdx.y == C - 1;
+  const long long v0 = a0 + m0 * IPA_TILE;
+  const int nfull = (int)(m1 - m0);
+  const long long vend = a0 + ntl * IPA_TILE;        // end of the body of the whole segment
+  const unsigned slot = (unsigned)__cvta_generic_to_shared(&stage[0][0]) + (unsigned)(warp * (32 * IPA_E * 8) + 16 * lane);
+  const double* src = x + v0 + warp * (32 * IPA_E) + 2 * lane;
+  if (nfull > 0) {
 #pragma unroll
-    for (int e = 0; e < IPA_E; ++e) {
-      const long long i = base + e * IPA_BLOCK + tid;
-      if (i < ce) ipa_cp_async8(&stage[buf][e * IPA_BLOCK + tid], x + i);
-    }
-    ipa_cp_async_commit();
-  };
-  if (cb < ce) issue(cb, 0);
+    for (int p = 0; p < IPA_E / 2; ++p) ipa_cp_async16_s(slot + p * 512, src + p * 64);
+  }
+  ipa_cp_async_commit();
   {
     // categories may share a parameter set (set_of_segment != NULL): segment t uses record set_of_segment[t]
-    const double* src = reinterpret_cast<const double*>(consts + (set_of_segment ? set_of_segment[t] : t));
+    const double* csrc = reinterpret_cast<const double*>(consts + (set_of_segment ? set_of_segment[t] : t));
     double* dst = reinterpret_cast<double*>(&c);
-    for (int i = tid; i < (int)(sizeof(IpaSetConsts) / 8); i += IPA_BLOCK) dst[i] = src[i];
+    for (int i = tid; i < (int)(sizeof(IpaSetConsts) / 8); i += IPA_BLOCK) dst[i] = csrc[i];
     ipa_load_logtab(s_tab);
   }
   __syncthreads();
   double acc = 0.0;
   if (!c.status) {
-    const double filler = c.mu;   // masked slots of a ragged tile: any finite value, the result is dropped
-    int buf = 0;
-    for (long long base = cb; base < ce; base += IPA_TILE, buf ^= 1) {
+    unsigned bufoff = 0;
+    for (int tile = 0; tile < nfull; ++tile) {
       double xv[IPA_E], l[IPA_E];
       ipa_cp_async_wait_all();
 #pragma unroll
-      for (int e = 0; e < IPA_E; ++e)
-        xv[e] = (base + e * IPA_BLOCK + tid < ce) ? stage[buf][e * IPA_BLOCK + tid] : filler;
-      if (base + IPA_TILE < ce) issue(base + IPA_TILE, buf ^ 1);
+      for (int p = 0; p < IPA_E / 2; ++p) {
+        const double2 v = ipa_lds128(slot + bufoff + p * 512);
+        xv[2 * p] = v.x;
+        xv[2 * p + 1] = v.y;
+      }
+      bufoff ^= IPA_TILE * 8;
+      src += IPA_TILE;
+      if (tile + 1 < nfull) {
+#pragma unroll
+        for (int p = 0; p < IPA_E / 2; ++p) ipa_cp_async16_s(slot + bufoff + p * 512, src + p * 64);
+      }
+      ipa_cp_async_commit();
+      ipa_eval_set<IPA_E>(c, xv, l, s_tab);
+      acc += ((l[0] + l[1]) + (l[2] + l[3])) + ((l[4] + l[5]) + (l[6] + l[7]));
+    }
+    // remainder of the segment (last chunk only): the head event [beg, a0) and the tail [vend, end): at most
+    // IPA_TILE events, plain loads
+    const long long nhead = a0 - beg, nrem = last_chunk ? nhead + (end - vend) : 0;
+    const double xpad = (end > beg) ? x[end - 1] : 0.0;
+    for (long long base = 0; base < nrem; base += IPA_TILE) {
+      double xv[IPA_E], l[IPA_E];
+#pragma unroll
+      for (int e = 0; e < IPA_E; ++e) {
+        const long long r = base + ipa_ev_off(tid, e);
+        xv[e] = (r < nrem) ? x[r < nhead ? beg + r : vend + (r - nhead)] : xpad;
+      }
       ipa_eval_set<IPA_E>(c, xv, l, s_tab);
       double s = 0.0;
 #pragma unroll
-      for (int e = 0; e < IPA_E; ++e) s += (base + e * IPA_BLOCK + tid < ce) ? l[e] : 0.0;
+      for (int e = 0; e < IPA_E; ++e) s += (base + ipa_ev_off(tid, e) < nrem) ? l[e] : 0.0;
       acc += s;
     }
   }
@@ -787,16 +828,16 @@ ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ o
   acc = ipa_warp_sum(acc);
   if (lane == 0) red[warp] = acc;
   __syncthreads();
-  if (tid == 0) partials[t * IPA_SEGC + blockIdx.y] = (red[0] + red[1]) + (red[2] + red[3]);
+  if (tid == 0) partials[t * C + blockIdx.y] = (red[0] + red[1]) + (red[2] + red[3]);
 }
 
 __global__ void ipa_seg_finalize_kernel(const double* __restrict__ partials, const IpaSetConsts* __restrict__ consts,
-                                        const int* __restrict__ set_of_segment, long long T, double* __restrict__ nll,
+                                        const int* __restrict__ set_of_segment, long long T, int C, double* __restrict__ nll,
                                         int32_t* __restrict__ status_out) {
   const long long t = blockIdx.x * (long long)blockDim.x + threadIdx.x;
   if (t >= T) return;
   double v = 0.0;
-  for (int c = 0; c < IPA_SEGC; ++c) v += partials[t * IPA_SEGC + c];
+  for (int c = 0; c < C; ++c) v += partials[t * C + c];
   const int st = consts[set_of_segment ? set_of_segment[t] : t].status;
   nll[t] = st ? INFINITY : 0.0 - v;
   if (status_out) status_out[t] = st;
