@@ -268,7 +268,7 @@ int ipa_cls_from_counts(const int64_t* count_sb_dev, int64_t T_sb, const int64_t
  * (reading E4).  Own kernels (histogram, two scans, scatter): csrc/ipa_prepare.cuh.
  *   x_out_dev [n] must not alias x_in_dev;  n < 2^32;  ws_dev of ipa_prepare_workspace_bytes(n, T) bytes (T = 0
  *   for an unsegmented array);  r = the fit range the bins span. */
-#define IPA_PREPARE_BINS 2048
+#define IPA_PREPARE_BINS 256
 size_t ipa_prepare_workspace_bytes(int64_t n, int64_t T);
 int ipa_events_prepare(const double* x_in_dev, int64_t n, const int64_t* offsets_dev, int64_t T, ipa_range r,
                        double* x_out_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);

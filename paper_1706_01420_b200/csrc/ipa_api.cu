@@ -7,6 +7,8 @@
 #include "ipa_kernels.cuh"
 #include "ipa_prepare.cuh"
 
+static_assert(IPA_PREP_BINS == IPA_PREPARE_BINS, "bin count of ipa_events_prepare");
+
 namespace {
 
 thread_local std::string g_last_cuda_error;
@@ -73,6 +75,9 @@ int device_info(int* sms) {
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     IPA_CK(cudaFuncSetAttribute(ipa_prep_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, IPA_PREP_SMEM));
     IPA_CK(cudaFuncSetAttribute(ipa_prep_segment_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, IPA_PREP_SMEM));
+    // four resident blocks per SM need 4 x 43 KB of shared memory: ask for the largest carve-out
+    IPA_CK(cudaFuncSetAttribute(ipa_prep_scatter_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
+    IPA_CK(cudaFuncSetAttribute(ipa_prep_segment_kernel, cudaFuncAttributePreferredSharedMemoryCarveout, cudaSharedmemCarveoutMaxShared));
     g_dev.dev = dev;
     g_dev.sms = n;
     g_dev.attr_set = true;
@@ -573,7 +578,7 @@ int ipa_cls_from_counts(const int64_t* count_sb_dev, int64_t T_sb, const int64_t
 // grid of the unsegmented preparation: two resident blocks per SM, never more blocks than tiles
 static int64_t prep_grid(int64_t n, int sms) {
   const int64_t tiles = (n + IPA_PREP_TILE - 1) / IPA_PREP_TILE;
-  int64_t G = 2 * (int64_t)(sms > 0 ? sms : 148);
+  int64_t G = IPA_PREP_BLOCKS_PER_SM * (int64_t)(sms > 0 ? sms : 148);
   if (G > tiles) G = tiles;
   return G < 1 ? 1 : G;
 }
@@ -614,7 +619,7 @@ int ipa_events_prepare(const double* x_in_dev, int64_t n, const int64_t* offsets
   IPA_CK(cudaGetLastError());
   ipa_prep_scan_kernel<<<IPA_PREP_BINS / 8, 256, 0, st>>>(hist, (int)G, bintot);
   IPA_CK(cudaGetLastError());
-  ipa_prep_binscan_kernel<<<1, IPA_PREP_THREADS, 0, st>>>(bintot, binbase);
+  ipa_prep_binscan_kernel<<<1, IPA_PREP_BINS, 0, st>>>(bintot, binbase);
   IPA_CK(cudaGetLastError());
   ipa_prep_scatter_kernel<<<(unsigned)G, IPA_PREP_THREADS, IPA_PREP_SMEM, st>>>(x_in_dev, n, r.lo, scale, hist, binbase, x_out_dev);
   IPA_CK(cudaGetLastError());

@@ -6,7 +6,8 @@
 // logarithm for a warp whose events all lie in one region, so events grouped by a fine enough bin index make
 // nearly every warp region-uniform for EVERY theta of the fit (the bins do not depend on the joins).  The kernels
 // only look at which side of a join an event lies on, so a full sort (8 radix passes over 64-bit keys) orders
-// bits nobody reads; one counting pass on 11 bits does the same job.
+// bits nobody reads; ONE counting pass on 8 bits does the same job: only the warps inside the two bins that hold a
+// join stay mixed (2 / 256 of the range: about 1 % of the events of the config model).
 //
 // The result is a pure function of the input: the order inside a bin is the original order (stable), whatever the
 // grid -- so the prepared array, and every NLL computed from it, is bitwise reproducible.  No floating-point
@@ -15,20 +16,26 @@
 //   ipa_prep_hist_kernel     block b counts the bins of its contiguous chunk            -> hist[bin][b]
 //   ipa_prep_scan_kernel     per bin: exclusive prefix over the blocks, total per bin   -> hist (in place), bintot
 //   ipa_prep_binscan_kernel  exclusive prefix over the bins                             -> binbase
-//   ipa_prep_scatter_kernel  block b re-reads its chunk tile by tile, ranks every event inside its bin in original
-//                            order (warp: match_any; block: per-warp counters + a scan over the warps) and writes
-//                            it to  binbase[bin] + hist[bin][b] + rank
+//   ipa_prep_scatter_kernel  block b re-reads its chunk tile by tile (2048 events): ranks every event inside its bin
+//                            in original order (warp: ballots on the bits of the bin; block: per-warp counters + a scan over the warps),
+//                            moves the tile into bin order in SHARED memory and writes it out in runs of consecutive
+//                            addresses (one run per bin), starting at  binbase[bin] + hist[bin][b]
 //   ipa_prep_segment_kernel  one block per segment (toy / category): the same three steps inside the segment
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
 
-#define IPA_PREP_BINS 2048
-#define IPA_PREP_THREADS 512
+#define IPA_PREP_BINS 256                               // == IPA_PREPARE_BINS of the header (asserted in ipa_api.cu)
+#define IPA_PREP_THREADS 256
+#define IPA_PREP_BLOCKS_PER_SM 6                       // 40 registers, 25 KB of shared memory per block
 #define IPA_PREP_WARPS (IPA_PREP_THREADS / 32)
-#define IPA_PREP_E 16                                   // events per thread and tile
-#define IPA_PREP_TILE (IPA_PREP_THREADS * IPA_PREP_E)   // 8192 events: ranks inside a tile fit 16 bits
-#define IPA_PREP_SMEM (IPA_PREP_WARPS * IPA_PREP_BINS * 2 + IPA_PREP_BINS * 8)
+#define IPA_PREP_E 8                                    // events per thread and tile
+#define IPA_PREP_TILE (IPA_PREP_THREADS * IPA_PREP_E)   // 2048 events: ranks and positions inside a tile fit 16 bits
+// dynamic shared memory of the scatter: stage [TILE] double | off [BINS] u64 | delta [BINS] u64 | tilebase [BINS] u32 |
+// wtot [8] u32 | wmap [WARPS][BINS] u32 | wcnt [WARPS][BINS] u16 | sbin [TILE] u8
+#define IPA_PREP_SMEM (IPA_PREP_TILE * 8 + IPA_PREP_BINS * 16 + (IPA_PREP_BINS + 8) * 4 + IPA_PREP_WARPS * IPA_PREP_BINS * 6 + \
+                       IPA_PREP_TILE + 64)
+static_assert(IPA_PREP_BINS == 256 && IPA_PREP_THREADS >= IPA_PREP_BINS, "one thread per bin in the block scans");
 
 __device__ __forceinline__ int ipa_prep_bin(double x, double lo, double scale) {
   const double t = (x - lo) * scale;
@@ -47,8 +54,10 @@ __device__ __forceinline__ void ipa_prep_chunk(long long n, int b, int G, long l
 
 __global__ void __launch_bounds__(IPA_PREP_THREADS)
 ipa_prep_hist_kernel(const double* __restrict__ x, long long n, double lo, double scale, unsigned int* __restrict__ hist) {
-  __shared__ unsigned int cnt[IPA_PREP_BINS];
-  for (int j = threadIdx.x; j < IPA_PREP_BINS; j += IPA_PREP_THREADS) cnt[j] = 0u;
+  // per-WARP private counters (a block-wide array of 256 counters serialises on the few bins under the peak)
+  __shared__ unsigned int cnt[IPA_PREP_WARPS][IPA_PREP_BINS];
+  unsigned int* mine = cnt[threadIdx.x >> 5];
+  for (int j = threadIdx.x; j < IPA_PREP_WARPS * IPA_PREP_BINS; j += IPA_PREP_THREADS) (&cnt[0][0])[j] = 0u;
   __syncthreads();
   long long beg, end;
   ipa_prep_chunk(n, blockIdx.x, gridDim.x, &beg, &end);
@@ -58,11 +67,16 @@ ipa_prep_hist_kernel(const double* __restrict__ x, long long n, double lo, doubl
 #pragma unroll
     for (int u = 0; u < 8; ++u) v[u] = __ldcs(x + i + (long long)u * IPA_PREP_THREADS);
 #pragma unroll
-    for (int u = 0; u < 8; ++u) atomicAdd(&cnt[ipa_prep_bin(v[u], lo, scale)], 1u);
+    for (int u = 0; u < 8; ++u) atomicAdd(&mine[ipa_prep_bin(v[u], lo, scale)], 1u);
   }
-  for (; i < end; i += IPA_PREP_THREADS) atomicAdd(&cnt[ipa_prep_bin(__ldcs(x + i), lo, scale)], 1u);
+  for (; i < end; i += IPA_PREP_THREADS) atomicAdd(&mine[ipa_prep_bin(__ldcs(x + i), lo, scale)], 1u);
   __syncthreads();
-  for (int j = threadIdx.x; j < IPA_PREP_BINS; j += IPA_PREP_THREADS) hist[(long long)j * gridDim.x + blockIdx.x] = cnt[j];
+  for (int j = threadIdx.x; j < IPA_PREP_BINS; j += IPA_PREP_THREADS) {
+    unsigned int s = 0;
+#pragma unroll
+    for (int w = 0; w < IPA_PREP_WARPS; ++w) s += cnt[w][j];
+    hist[(long long)j * gridDim.x + blockIdx.x] = s;
+  }
 }
 
 // one warp per bin: exclusive prefix of hist[bin][0..G) in place, bintot[bin] = total
@@ -82,153 +96,193 @@ ipa_prep_scan_kernel(unsigned int* __restrict__ hist, int G, unsigned long long*
       const unsigned int t = __shfl_up_sync(0xffffffffu, inc, o);
       if (lane >= o) inc += t;
     }
-    if (b < G) row[b] = (unsigned int)run + inc - c;        // a block's chunk holds < 2^32 events of one bin
+    if (b < G) row[b] = (unsigned int)run + inc - c;        // a bin holds < 2^32 events (n <= 2^32 - 1)
     run += __shfl_sync(0xffffffffu, inc, 31);
   }
   if (lane == 0) bintot[bin] = run;
 }
 
-// one block: binbase[bin] = sum of bintot[0..bin)
-__global__ void __launch_bounds__(IPA_PREP_THREADS)
+// one block of IPA_PREP_BINS threads: binbase[bin] = sum of bintot[0..bin)
+__global__ void __launch_bounds__(IPA_PREP_BINS)
 ipa_prep_binscan_kernel(const unsigned long long* __restrict__ bintot, unsigned long long* __restrict__ binbase) {
-  __shared__ unsigned long long part[IPA_PREP_THREADS];
-  constexpr int PER = IPA_PREP_BINS / IPA_PREP_THREADS;
-  unsigned long long v[PER], s = 0;
-#pragma unroll
-  for (int q = 0; q < PER; ++q) { v[q] = bintot[threadIdx.x * PER + q]; s += v[q]; }
-  part[threadIdx.x] = s;
+  __shared__ unsigned long long part[IPA_PREP_BINS];
+  const unsigned long long v = bintot[threadIdx.x];
+  part[threadIdx.x] = v;
   __syncthreads();
-  for (int o = 1; o < IPA_PREP_THREADS; o <<= 1) {
+  for (int o = 1; o < IPA_PREP_BINS; o <<= 1) {
     const unsigned long long add = threadIdx.x >= o ? part[threadIdx.x - o] : 0ull;
     __syncthreads();
     part[threadIdx.x] += add;
     __syncthreads();
   }
-  unsigned long long run = part[threadIdx.x] - s;
-#pragma unroll
-  for (int q = 0; q < PER; ++q) { binbase[threadIdx.x * PER + q] = run; run += v[q]; }
+  binbase[threadIdx.x] = part[threadIdx.x] - v;
+}
+
+struct IpaPrepSmem {
+  double* stage;                 // [TILE]  the tile in bin order
+  unsigned long long* off;       // [BINS]  running output position of this block for every bin
+  unsigned long long* delta;     // [BINS]  off - tilebase: output address of a staged position = delta[bin] + position
+  unsigned int* wmap;            // [WARPS][BINS] lanes of the warp that hold the bin in the current step (bit mask)
+  unsigned int* tilebase;        // [BINS]  first staged position of a bin in the current tile
+  unsigned short* wcnt;          // [WARPS][BINS] events of a bin per warp, then their exclusive prefix over the warps
+  unsigned char* sbin;           // [TILE]  bin of the staged event
+  unsigned int* wtot;            // [8]     warp totals of the scan over the bins
+};
+__device__ __forceinline__ IpaPrepSmem ipa_prep_carve(unsigned char* base) {
+  IpaPrepSmem m;
+  m.stage = reinterpret_cast<double*>(base);
+  unsigned char* p = base + IPA_PREP_TILE * 8;
+  m.off = reinterpret_cast<unsigned long long*>(p);      p += IPA_PREP_BINS * 8;
+  m.delta = reinterpret_cast<unsigned long long*>(p);    p += IPA_PREP_BINS * 8;
+  m.tilebase = reinterpret_cast<unsigned int*>(p);       p += IPA_PREP_BINS * 4;
+  m.wtot = reinterpret_cast<unsigned int*>(p);           p += 32;
+  m.wmap = reinterpret_cast<unsigned int*>(p);           p += IPA_PREP_WARPS * IPA_PREP_BINS * 4;
+  m.wcnt = reinterpret_cast<unsigned short*>(p);         p += IPA_PREP_WARPS * IPA_PREP_BINS * 2;
+  m.sbin = p;
+  return m;
 }
 
 // Stable scatter of x[beg, end) given the running output position off[bin] (shared memory) of this block for every
 // bin.  Tile by tile: (1) warp w ranks its 32 x E events -- event index inside the tile = (w E + e) 32 + lane, so
-// (warp, e, lane) order IS the original order -- with match_any: rank inside the warp = events of the same bin seen
-// before; the first lane of every match group bumps the warp's own 16-bit counter; (2) exclusive scan of the
-// counters over the warps, two bins at a time (packed 16-bit pairs: a tile holds < 2^16 events); (3) every event
-// goes to off[bin] + (events of the bin in earlier warps) + (rank in its warp); (4) off[bin] += tile count.
-// wcnt [WARPS][BINS] uint16, off [BINS] uint64.
+// (warp, e, lane) order IS the original order -- by ballots: rank inside the warp = events of the same bin seen
+// before; the first lane of every match group bumps the warp's own 16-bit counter; (2) thread b: exclusive prefix of
+// bin b's counters over the warps, then an exclusive scan of the tile's bin counts over the bins; (3) every event
+// goes to stage[tilebase[bin] + (events of the bin in earlier warps) + (rank in its warp)]: the tile in bin order,
+// original order inside a bin; (4) the staged tile is written out position by position: consecutive positions of a
+// bin are consecutive addresses, off[bin] + (position - tilebase[bin]); (5) off[bin] += tile count.
 __device__ __forceinline__ void ipa_prep_scatter_range(const double* __restrict__ x, long long beg, long long end, double lo,
-                                                       double scale, unsigned short* wcnt, unsigned long long* off,
-                                                       double* __restrict__ out) {
+                                                       double scale, const IpaPrepSmem& m, double* __restrict__ out) {
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const unsigned lt = (1u << lane) - 1u;
-  unsigned short* mine = wcnt + warp * IPA_PREP_BINS;
-  unsigned int* wcnt32 = reinterpret_cast<unsigned int*>(wcnt);
+  unsigned short* mine = m.wcnt + warp * IPA_PREP_BINS;
+  unsigned int* map = m.wmap + warp * IPA_PREP_BINS;
+  for (int i = tid; i < IPA_PREP_WARPS * IPA_PREP_BINS; i += IPA_PREP_THREADS) m.wmap[i] = 0u;   // kept zero by the leaders
   for (long long base = beg; base < end; base += IPA_PREP_TILE) {
+    const int cnt = (int)((end - base < IPA_PREP_TILE) ? (end - base) : IPA_PREP_TILE);
     {  // zero the per-warp counters (128-bit stores)
-      uint4* z = reinterpret_cast<uint4*>(wcnt);
+      uint4* z = reinterpret_cast<uint4*>(m.wcnt);
       for (int i = tid; i < IPA_PREP_WARPS * IPA_PREP_BINS * 2 / 16; i += IPA_PREP_THREADS) z[i] = make_uint4(0u, 0u, 0u, 0u);
     }
     double v[IPA_PREP_E];
-    const long long first = base + (long long)warp * (32 * IPA_PREP_E) + lane;
+    const int first = warp * (32 * IPA_PREP_E) + lane;
 #pragma unroll
-    for (int e = 0; e < IPA_PREP_E; ++e) {
-      const long long i = first + 32 * e;
-      v[e] = i < end ? __ldcs(x + i) : 0.0;
-    }
+    for (int e = 0; e < IPA_PREP_E; ++e) v[e] = (first + 32 * e < cnt) ? __ldcs(x + base + first + 32 * e) : 0.0;
     __syncthreads();
-    unsigned short rank[IPA_PREP_E];
-    short bin[IPA_PREP_E];
+    unsigned int key[IPA_PREP_E];               // bin << 16 | rank inside the warp
+    const bool full = cnt == IPA_PREP_TILE;
 #pragma unroll
     for (int e = 0; e < IPA_PREP_E; ++e) {
-      const bool live = first + 32 * e < end;
-      const int b = live ? ipa_prep_bin(v[e], lo, scale) : -1;          // empty slots of the ragged tile match each other only
-      const unsigned peers = __match_any_sync(0xffffffffu, b);
+      const bool live = full || first + 32 * e < cnt;
+      const unsigned b = live ? (unsigned)ipa_prep_bin(v[e], lo, scale) : 0u;
+      // lanes of the warp holding the same bin, through the warp's own bit map in shared memory: every live lane ORs
+      // its bit into map[bin] (an OR does not depend on the order the hardware takes the lanes in: deterministic),
+      // reads the mask back, and the first lane of the mask bumps the warp's counter of the bin and clears the map
+      // entry.  3 shared-memory instructions where eight ballots and their logic took 50, and the match.any
+      // instruction serialised on the ~25 distinct bins of a warp of unsorted events.
+      if (live) atomicOr(&map[b], 1u << lane);
+      __syncwarp();
+      const unsigned peers = live ? map[b] : 0u;
+      __syncwarp();
       const int leader = __ffs(peers) - 1;
       unsigned old = 0;
-      if (lane == leader && live) {
+      if (live && lane == leader) {
         old = mine[b];
         mine[b] = (unsigned short)(old + __popc(peers));
+        map[b] = 0u;
       }
-      old = __shfl_sync(0xffffffffu, old, leader);
-      rank[e] = (unsigned short)(old + __popc(peers & lt));
-      bin[e] = (short)b;
+      old = __shfl_sync(0xffffffffu, old, leader & 31);
+      key[e] = (b << 16) | (old + __popc(peers & lt));
       __syncwarp();
     }
     __syncthreads();
-    // exclusive scan over the warps, bins (2 q, 2 q + 1) packed in one 32-bit word; thread owns words q = tid + i 512
-    unsigned int tot[IPA_PREP_BINS / 2 / IPA_PREP_THREADS];
-#pragma unroll
-    for (int i = 0; i < IPA_PREP_BINS / 2 / IPA_PREP_THREADS; ++i) {
-      const int q = tid + i * IPA_PREP_THREADS;
-      unsigned int run = 0;
+    // thread b: exclusive prefix of bin b over the warps; then exclusive scan of the tile counts over the bins
+    unsigned int tot = 0;
+    if (tid < IPA_PREP_BINS) {
 #pragma unroll
       for (int w = 0; w < IPA_PREP_WARPS; ++w) {
-        const unsigned int c = wcnt32[w * (IPA_PREP_BINS / 2) + q];
-        wcnt32[w * (IPA_PREP_BINS / 2) + q] = run;
-        run += c;                                                         // no carry between the halves: sums < 2^16
+        const unsigned int c = m.wcnt[w * IPA_PREP_BINS + tid];
+        m.wcnt[w * IPA_PREP_BINS + tid] = (unsigned short)tot;
+        tot += c;
       }
-      tot[i] = run;
+      unsigned int inc = tot;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) {
+        const unsigned int t = __shfl_up_sync(0xffffffffu, inc, o);
+        if (lane >= o) inc += t;
+      }
+      if (lane == 31) m.wtot[warp] = inc;
+      m.tilebase[tid] = inc - tot;                       // exclusive inside the warp; the warp offset is added below
+    }
+    __syncthreads();
+    if (tid < IPA_PREP_BINS) {
+      unsigned int add = 0;
+      for (int w = 0; w < warp; ++w) add += m.wtot[w];
+      const unsigned int tb = m.tilebase[tid] + add;
+      m.tilebase[tid] = tb;
+      m.delta[tid] = m.off[tid] - tb;
     }
     __syncthreads();
 #pragma unroll
     for (int e = 0; e < IPA_PREP_E; ++e) {
-      if (bin[e] >= 0) out[off[bin[e]] + mine[bin[e]] + rank[e]] = v[e];
+      if (full || first + 32 * e < cnt) {
+        const unsigned int b = key[e] >> 16;
+        const unsigned int pos = m.tilebase[b] + mine[b] + (key[e] & 0xffffu);
+        m.stage[pos] = v[e];
+        m.sbin[pos] = (unsigned char)b;
+      }
     }
     __syncthreads();
-#pragma unroll
-    for (int i = 0; i < IPA_PREP_BINS / 2 / IPA_PREP_THREADS; ++i) {
-      const int q = tid + i * IPA_PREP_THREADS;
-      off[2 * q] += tot[i] & 0xffffu;
-      off[2 * q + 1] += tot[i] >> 16;
+    for (int i = tid; i < cnt; i += IPA_PREP_THREADS) {
+      out[m.delta[m.sbin[i]] + (unsigned int)i] = m.stage[i];
     }
-    // no barrier here: the next tile zeroes wcnt (free since the barrier above) and reads off[] two barriers later
+    __syncthreads();
+    if (tid < IPA_PREP_BINS) m.off[tid] += tot;
+    // no barrier here: the next tile touches wcnt (free since the staging barrier) and reads off[] three barriers later
   }
 }
 
-__global__ void __launch_bounds__(IPA_PREP_THREADS)
+__global__ void __launch_bounds__(IPA_PREP_THREADS, IPA_PREP_BLOCKS_PER_SM)
 ipa_prep_scatter_kernel(const double* __restrict__ x, long long n, double lo, double scale,
                         const unsigned int* __restrict__ hist, const unsigned long long* __restrict__ binbase,
                         double* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char ipa_prep_smem[];
-  unsigned short* wcnt = reinterpret_cast<unsigned short*>(ipa_prep_smem);
-  unsigned long long* off = reinterpret_cast<unsigned long long*>(ipa_prep_smem + IPA_PREP_WARPS * IPA_PREP_BINS * 2);
-  for (int j = threadIdx.x; j < IPA_PREP_BINS; j += IPA_PREP_THREADS)
-    off[j] = binbase[j] + hist[(long long)j * gridDim.x + blockIdx.x];
+  const IpaPrepSmem m = ipa_prep_carve(ipa_prep_smem);
+  if (threadIdx.x < IPA_PREP_BINS) m.off[threadIdx.x] = binbase[threadIdx.x] + hist[(long long)threadIdx.x * gridDim.x + blockIdx.x];
   __syncthreads();
   long long beg, end;
   ipa_prep_chunk(n, blockIdx.x, gridDim.x, &beg, &end);
-  ipa_prep_scatter_range(x, beg, end, lo, scale, wcnt, off, out);
+  ipa_prep_scatter_range(x, beg, end, lo, scale, m, out);
 }
 
 // One block per segment: histogram of the segment, exclusive prefix over the bins, stable scatter inside the segment.
-__global__ void __launch_bounds__(IPA_PREP_THREADS)
+__global__ void __launch_bounds__(IPA_PREP_THREADS, IPA_PREP_BLOCKS_PER_SM)
 ipa_prep_segment_kernel(const double* __restrict__ x, const long long* __restrict__ offsets, double lo, double scale,
                         double* __restrict__ out) {
   extern __shared__ __align__(16) unsigned char ipa_prep_smem[];
-  unsigned short* wcnt = reinterpret_cast<unsigned short*>(ipa_prep_smem);
-  unsigned long long* off = reinterpret_cast<unsigned long long*>(ipa_prep_smem + IPA_PREP_WARPS * IPA_PREP_BINS * 2);
-  unsigned int* cnt = reinterpret_cast<unsigned int*>(ipa_prep_smem);          // the counters' area, before it is needed
-  __shared__ unsigned long long part[IPA_PREP_THREADS];
+  const IpaPrepSmem m = ipa_prep_carve(ipa_prep_smem);
+  unsigned int* cnt = reinterpret_cast<unsigned int*>(m.stage);              // [WARPS][BINS] in the staging area, before it is needed
+  __shared__ unsigned long long part[IPA_PREP_BINS];
+  const int tid = threadIdx.x;
   const long long beg = offsets[blockIdx.x], end = offsets[blockIdx.x + 1];
-  for (int j = threadIdx.x; j < IPA_PREP_BINS; j += IPA_PREP_THREADS) cnt[j] = 0u;
+  for (int j = tid; j < IPA_PREP_WARPS * IPA_PREP_BINS; j += IPA_PREP_THREADS) cnt[j] = 0u;
   __syncthreads();
-  for (long long i = beg + threadIdx.x; i < end; i += IPA_PREP_THREADS) atomicAdd(&cnt[ipa_prep_bin(x[i], lo, scale)], 1u);
+  unsigned int* mine = cnt + (tid >> 5) * IPA_PREP_BINS;
+  for (long long i = beg + tid; i < end; i += IPA_PREP_THREADS) atomicAdd(&mine[ipa_prep_bin(x[i], lo, scale)], 1u);
   __syncthreads();
-  constexpr int PER = IPA_PREP_BINS / IPA_PREP_THREADS;
-  unsigned long long v[PER], s = 0;
-#pragma unroll
-  for (int q = 0; q < PER; ++q) { v[q] = cnt[threadIdx.x * PER + q]; s += v[q]; }
-  part[threadIdx.x] = s;
+  unsigned long long v = 0;
+  if (tid < IPA_PREP_BINS) {
+    for (int w = 0; w < IPA_PREP_WARPS; ++w) v += cnt[w * IPA_PREP_BINS + tid];
+    part[tid] = v;
+  }
   __syncthreads();
-  for (int o = 1; o < IPA_PREP_THREADS; o <<= 1) {
-    const unsigned long long add = threadIdx.x >= o ? part[threadIdx.x - o] : 0ull;
+  for (int o = 1; o < IPA_PREP_BINS; o <<= 1) {
+    unsigned long long add = 0ull;
+    if (tid < IPA_PREP_BINS && tid >= o) add = part[tid - o];
     __syncthreads();
-    part[threadIdx.x] += add;
+    if (tid < IPA_PREP_BINS) part[tid] += add;
     __syncthreads();
   }
-  unsigned long long run = (unsigned long long)beg + part[threadIdx.x] - s;
-#pragma unroll
-  for (int q = 0; q < PER; ++q) { off[threadIdx.x * PER + q] = run; run += v[q]; }
+  if (tid < IPA_PREP_BINS) m.off[tid] = (unsigned long long)beg + part[tid] - v;
   __syncthreads();
-  ipa_prep_scatter_range(x, beg, end, lo, scale, wcnt, off, out);
+  ipa_prep_scatter_range(x, beg, end, lo, scale, m, out);
 }

@@ -75,7 +75,7 @@ def test_argument_validation_without_gpu(ipa):
     assert L.ipa_events_prepare(one, 10, None, 0, rng, one, one, 1 << 30, None) == -1      # output aliases the input
     assert L.ipa_events_prepare(one, 2 ** 32, None, 0, rng, C.c_void_p(512), one, 1 << 30, None) == -1
     assert L.ipa_events_prepare(one, 10, None, 0, rng, C.c_void_p(512), one, 16, None) == -2
-    assert ipa.ipa_prepare_workspace_bytes(10 ** 8) >= 2048 * 296 * 4 and ipa.ipa_prepare_workspace_bytes(10 ** 5, 7) == 256
+    assert ipa.ipa_prepare_workspace_bytes(10 ** 8) >= 256 * 296 * 4 and ipa.ipa_prepare_workspace_bytes(10 ** 5, 7) == 256
     assert L.ipa_hist_fill(one, 5, rng, 0, one, None) == -1
     assert L.ipa_strerror(-2).decode().startswith("workspace")
     assert ipa.ipa_workspace_bytes(10 ** 8, 9) >= 9 * 600

@@ -358,7 +358,7 @@ def test_binned_scan_expected_hist_and_poisson_toys(ipa, torch_, orc):
 # ---------------------------------------------------------------------------------------------
 # optional preparation: events grouped by a coarse bin index (stable counting sort); reading E4
 # ---------------------------------------------------------------------------------------------
-def coarse_bins(x, nb=2048):
+def coarse_bins(x, nb=256):
     """bin index of the header: clamp(floor((x - lo) nb / (hi - lo)), 0, nb - 1), NaN -> last bin (host restatement)."""
     t = (x - LO) * (nb / (HI - LO))
     b = np.where(t < nb, np.floor(np.where(np.isnan(t), 0.0, t)), nb - 1)
@@ -468,7 +468,7 @@ def test_full_size_sampled(ipa, torch_, orc):
     assert abs(nlls.item() - ref1) <= 1e-10 * abs(ref1) and nlls9[0].item() == nlls.item()
     assert np.all(np.abs(nlls9.cpu().numpy() - nll9.cpu().numpy()) <= 1e-12 * np.abs(nll9.cpu().numpy()))
     # the prepared array is the stable counting sort of the input: grouped by non-decreasing bin, a permutation
-    bins = ((xs - LO) * (2048.0 / (HI - LO))).floor().clamp_(0, 2047)
+    bins = ((xs - LO) * (256.0 / (HI - LO))).floor().clamp_(0, 255)
     assert bool((bins[1:] >= bins[:-1]).all().item())
     assert np.array_equal(xs[:1_000_000].cpu().numpy(), stable_by_bin(x)[:1_000_000])
     del bins
