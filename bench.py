@@ -36,34 +36,36 @@ FP64_PEAK_NOMINAL = SM_COUNT * FP64_LANES * 2 * SM_MAX_HZ  # 37.2 TFLOP/s
 def algorithmic_flops(degree, p_core):
     """FP64 flops one event x set needs in this method (table 'work per event'),
     FMA = 2, add / mul / compare = 1; an event pays the core OR the tail arithmetic, never both:
-      common  d, 2 compares, E_B, exp (14 FMA + 1 add), 1+w, log on [1,2] (9 FMA), 2 adds : 24 FMA + 7 other = 55
-      core    q, sqrt (3 FMA + 2 mul), t, Horner (degree FMA), (beta-k) d              : (6 + degree) FMA + 2 mul
-      tail    u, log (10 FMA + 1 add), -n log u + c, -k d                               : 13 FMA + 1 add = 27
-    p_core = fraction of the events inside [mu - a sigma, mu + a2 sigma] (0.344 for the config model)."""
+      common  d (1), 2 compares (2), E_B (1 FMA), exp = 7 FMA + 1 add + 1 mul (16), 1+w (1), log on [1,2] = 6 FMA (12),
+              2 adds                                                                          : 14 FMA + 8 other = 36
+      core    q, sqrt (3 FMA + 2 mul), t, Horner (degree FMA), (beta-k) d                     : (6 + degree) FMA + 2 mul
+      tail    u (1 FMA), log = 7 FMA + 1 add, -n log u + c (1 FMA), -k d (1 FMA)              : 10 FMA + 1 add = 21
+    (table-driven exp / log of round 2: csrc/ipa_fastmath.cuh; the degree-11 / degree-8 polynomials of round 1 made
+    this 55 / 27).  p_core = fraction of the events inside [mu - a sigma, mu + a2 sigma] (0.344 for the config model)."""
     core = 2.0 * (6 + degree) + 2.0
-    return 55.0 + p_core * core + (1.0 - p_core) * 27.0
+    return 36.0 + p_core * core + (1.0 - p_core) * 21.0
 
 
 def shape_stage_flops(degree, p_core):
     """Shape stage of a group of sets sharing (mu, sigma, lambda, zeta, beta, a, n, a2, n2) -- DESIGN.md section 5:
     d (1), 2 region compares (2), core: q, sqrt, t, Horner = (5 + degree) FMA + 2 mul; tail: u (1 FMA) + log
-    (10 FMA + 1 add) + the product with -n (1 mul)."""
-    return 3.0 + p_core * (2.0 * (5 + degree) + 2.0) + (1.0 - p_core) * (2.0 * 11 + 2.0)
+    (7 FMA + 1 add) + the product with -n (1 mul)."""
+    return 3.0 + p_core * (2.0 * (5 + degree) + 2.0) + (1.0 - p_core) * (2.0 * 8 + 2.0)
 
 
-MEMBER_STAGE_FLOPS = 55.0
-"""Member stage per set: Delta = s d + (V + c): 1 add + 1 FMA (3); E_B (1 FMA: 2); exp 14 FMA + 1 add (29); 1 + w (1);
-log on [1,2] 9 FMA (18); 2 adds (2)."""
+MEMBER_STAGE_FLOPS = 36.0
+"""Member stage per set: Delta = s d + (V + c): 1 add + 1 FMA (3); E_B (1 FMA: 2); exp (16); 1 + w (1);
+log on [1,2] (12); 2 adds (2)."""
 
 
 def gradient_flops(degree, p_core):
-    """Analytic-gradient pass per event x set (ipa_eval_grad): common = d, 2 compares, exp (29), 1+w, 1/(1+w)
-    (4 FMA), w/(1+w), E_B (2), log (18), 2 adds, the four derivative terms (2 + 2 + 3 + 3) and 5 accumulations = 80;
+    """Analytic-gradient pass per event x set (ipa_eval_grad): common = d, 2 compares (3), exp (16), 1+w (1), 1/(1+w)
+    (4 FMA: 8), w/(1+w) (1), E_B (2), log (12), 2 adds, the four derivative terms (2 + 2 + 3 + 3) and 5 accumulations = 60;
     core = q (2), sqrt (8), 1/r (8), t (2), value and derivative Horner 2 FMA per coefficient of the 4 ceil((D+1)/4)
-    slots, L - beta (3), Delta (2), dd (1), ds (3); tail = u (2), 1/u (8), log (21), Delta (4), dd (1), ds (5)."""
+    slots, L - beta (3), Delta (2), dd (1), ds (3); tail = u (2), 1/u (8), log (15), Delta (4), dd (1), ds (5) = 35."""
     slots = 4 * (degree // 4) + 4
     core = 2.0 + 8 + 8 + 2 + 4.0 * slots + 3 + 2 + 1 + 3
-    return 80.0 + p_core * core + (1.0 - p_core) * 41.0
+    return 60.0 + p_core * core + (1.0 - p_core) * 35.0
 
 
 def alu_roofline(flops_per_event, events, seconds, extra=None):
@@ -295,12 +297,12 @@ def other_rows(torch, ipa, x, ws, stream, n, p_core):
                         "roofline_prepared": alu_roofline(W, ntot, dss, {"note": "whole call: 1000-set prologue + segmented kernel + finalize"}),
                         "roofline_as_generated": alu_roofline(W, ntot, ds)}
         # generator: issue-slot model: a sub-partition issues one warp instruction per cycle and an
-        # FP64 instruction holds the port for two.  Declared per event: signal fraction 0.3 x attempts x (Philox 100 +
-        # core log G 8 int + (7 + D) FP64 + acceptance exp 15 FP64 + 12 int) + background 0.7 x (Philox 100 + inverse
-        # CDF log1p/expm1 ~ 60 FP64 + 20 int); component / yield bookkeeping 10 int.
+        # FP64 instruction holds the port for two.  Declared per event: signal fraction 0.3 x (bookkeeping Philox 100 +
+        # attempts x (Philox 100 + core log G 8 int + (7 + D) FP64 + acceptance exp 15 FP64 + 12 int)) + background 0.7 x
+        # (2 Philox 200 + inverse CDF log1p/expm1 ~ 60 FP64 + 20 int); list / refill bookkeeping 10 int.
         deg1 = int(ipa.ipa_core_degree(inp.GEN, LO, HI, policy=1))
         att = 1.11
-        cyc = 0.3 * att * (100 + 8 + 12 + 2 * (7 + deg1 + 15)) + 0.7 * (100 + 20 + 2 * 60) + 10
+        cyc = 0.3 * (100 + att * (100 + 8 + 12 + 2 * (7 + deg1 + 15))) + 0.7 * (2 * 100 + 20 + 2 * 60) + 10
         peak_issue = SM_COUNT * 4 * 32 * SM_MAX_HZ
         out["config4_toys"] = {"toys": T, "events": ntot, "generate_ms": dg * 1e3, "generate_events_per_s": ntot / dg,
                                "roofline_toygen": {"bound": "alu", "unit": "thread-issue-cycles/s", "achieved": cyc * ntot / dg,

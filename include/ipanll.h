@@ -33,7 +33,11 @@
  *     [0,1]); 2 join slope sign (L(d0)<=0 or L(d1)>=0: the power-law tail does not exist);
  *     3 internal numerical failure (normalisation not finite or not positive); 4 (ipa_nll_grad_eval only)
  *     f == 0 or f == 1.
- *   - Events outside [lo,hi] are evaluated by the same formulae (no clipping); NaN events give NaN.
+ *   - Events outside [lo,hi] are evaluated by the same formulae (no clipping); NaN events give NaN.  The per-event
+ *     arithmetic is valid while |log(f S) - log((1-f) B)| < 5e6 (the range of the kernels' exponential); parameter
+ *     sets or events beyond that (e.g. |k (x - lo)| > 5e6) give undefined values, not an error.
+ *   - ipa_norm returns the ABSOLUTE N_S, which underflows to 0 (status 0) when log N_S < -745 (e.g. zeta >~ 1000 with
+ *     the unscaled Bessel core); the likelihood calls work with log N_S and are not affected.
  *     Any n >= 0 is accepted (n == 0 gives NLL = +0.0).
  *   - Determinism: for fixed device, build, n and launch geometry the results are bitwise
  *     reproducible, and the result of set k does not depend on which other sets share the batch.

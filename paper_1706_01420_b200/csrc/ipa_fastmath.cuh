@@ -6,7 +6,7 @@
 // same source on the GPU-less box (the rsqrt seed is emulated there with 20 good bits).
 //
 // Accuracy targets (checked in tests/test_abi_and_host_logic.py against mpmath):
-//   ipa_fsqrt    relative error <= 1.2e-16 for normal positive arguments
+//   ipa_fsqrt    relative error <= 2e-16 for normal positive arguments (seed truncated to 20 bits on the host)
 //   ipa_fexp_neg relative error <= 3e-16 for a in [-90, 0]
 //   ipa_flog     absolute error <= 2.5e-16 + 1.5e-16 |log u| for normal positive u
 #pragma once
@@ -22,6 +22,12 @@
 __constant__ double ipa_c_exp[IPA_EXP_DEG + 1] = IPA_EXP_COEFS;
 __constant__ double ipa_c_log1p[IPA_LOG_DEG] = IPA_LOG1P_COEFS;
 __constant__ double2 ipa_c_logtab[33] = IPA_LOG_TABLE;
+// 8 KB table of the streaming kernels (layout: gen_fastmath_tables.py); the kernels copy it to shared memory
+#define IPA_MATHTAB_DOUBLES 1024
+__device__ const double ipa_d_mathtab[IPA_MATHTAB_DOUBLES] = IPA_MATHTAB_RAW;
+static const double ipa_h_mathtab[IPA_MATHTAB_DOUBLES] = IPA_MATHTAB_RAW;
+__constant__ double ipa_c_expq[4] = IPA_EXPQ_COEFS;
+static const double ipa_h_expq[4] = IPA_EXPQ_COEFS;
 __device__ const long long ipa_d_chebT[IPA_CHEB_NC * IPA_CHEB_NC] = IPA_CHEB_TABLE;   // global memory: per-lane index
 static const long long ipa_h_chebT[IPA_CHEB_NC * IPA_CHEB_NC] = IPA_CHEB_TABLE;
 __constant__ double ipa_c_gl16x[16] = IPA_GL16_X;
@@ -35,6 +41,7 @@ static const double ipa_h_log1p[IPA_LOG_DEG] = IPA_LOG1P_COEFS;
 static const ipa_host_double2 ipa_h_logtab[33] = IPA_LOG_TABLE;
 #ifdef __CUDA_ARCH__
 #define IPA_CEXP(j) ipa_c_exp[j]
+#define IPA_CEXPQ(j) ipa_c_expq[j]
 #define IPA_CLOG(j) ipa_c_log1p[j]
 #define IPA_GL16X(i) ipa_c_gl16x[i]
 #define IPA_GL16W(i) ipa_c_gl16w[i]
@@ -44,6 +51,7 @@ static const ipa_host_double2 ipa_h_logtab[33] = IPA_LOG_TABLE;
 #define IPA_GL16X(i) ipa_h_gl16x[i]
 #define IPA_GL16W(i) ipa_h_gl16w[i]
 #define IPA_CEXP(j) ipa_h_exp[j]
+#define IPA_CEXPQ(j) ipa_h_expq[j]
 #define IPA_CLOG(j) ipa_h_log1p[j]
 #endif
 
@@ -166,7 +174,7 @@ IPA_HD double ipa_flog_1to2(double s, const Tab* tab) {
 }
 
 // e^{-|D|}: -|D| enters through operand modifiers, the exponent shift is clamped instead of the argument.
-// |D| < 2^50.
+// |D| < 1.4e9 (beyond that round(-|D| log2 e) leaves 32 bits).
 IPA_HD double ipa_fexp_negabs(double D) {
   const double SHIFT = 6755399441055744.0;
   const double a = -fabs(D);
@@ -184,7 +192,7 @@ IPA_HD double ipa_fexp_negabs(double D) {
 
 // eb + log(1 + e^D) = eb + log(1 + e^{-|D|}) [+ D if D >= 0].  -|D| enters the exponential through operand
 // modifiers, the exponent shift is clamped instead of the argument, and max(D,0) is a predicated add on
-// the sign word: 2 integer instructions where the clamp / relu pair above needs 7.  |D| < 2^50.
+// the sign word: 2 integer instructions where the clamp / relu pair above needs 7.  |D| < 1.4e9.
 template <class Tab>
 IPA_HD double ipa_fsoftplus_add(double eb, double D, const Tab* tab) {
   const double SHIFT = 6755399441055744.0;
@@ -214,4 +222,83 @@ template <class Tab>
 IPA_HD double ipa_fsoftplus(double D, const Tab* tab) {
   const double w = ipa_fexp_neg(ipa_neg_abs_clamped(D));
   return ipa_relu_bits(D) + ipa_flog_1to2(1.0 + w, tab);
+}
+
+// ================================================================================================
+// Table-driven versions for the streaming kernels (round 2).  `mt` points to the 8 KB table
+// (ipa_d_mathtab copied to shared memory; ipa_h_mathtab in the host build):
+//   byte 0     {1/2, ln 2}                 log entry of s == 2
+//   byte 16    2^(j/256), j = 0..255       e^a = 2^n 2^(j/256) e^r, |r| <= ln2/512, e^r = 1 + r q(r), q of degree 3
+//   byte 4096  {c_j, -log c_j}, j = 0..255  log m = -log c_j + log1p(m c_j - 1), |m c_j - 1| < 2^-9,
+//                                           log1p(r) = r (1 + r p(r)), p = -1/2 + r/3 - r^2/4 + r^3/5
+// 9 FP64 instructions for the exponential (15 with the degree-11 polynomial), 6 for the logarithm on [1,2] (10),
+// 8 for the general logarithm (12); each <= 3e-16 relative (exp) / 2.5e-16 + 1.5e-16 |log u| absolute (log),
+// checked against mpmath on the host build.
+// ================================================================================================
+IPA_HD const double2* ipa_mt_at(const double* mt, unsigned byte_off) {
+  return reinterpret_cast<const double2*>(reinterpret_cast<const char*>(mt) + byte_off);
+}
+IPA_HD double ipa_mt_d(const double* mt, unsigned byte_off) {
+  return *reinterpret_cast<const double*>(reinterpret_cast<const char*>(mt) + byte_off);
+}
+
+// r (1 + r p(r)) + l  with p = -1/2 + r/3 - r^2/4 + r^3/5: log1p(r) + l for |r| < 2^-9.  5 FP64.
+IPA_HD double ipa_log1p_small_add(double r, double l) {
+  double p = fma(0.2, r, -0.25);
+  p = fma(p, r, 0.33333333333333331);
+  p = fma(p, r, -0.5);
+  const double q = fma(p, r, 1.0);
+  return fma(r, q, l);
+}
+
+// log(s) for s in [1, 2] (s = 1 + w, w in [0,1]).  Index = lowest exponent bit (1 on [1,2), 0 at s == 2) and the top
+// 8 mantissa bits: byte offset 0 serves s == 2, 4096 + 16 j the rest; a NaN stays in bounds.  6 FP64, 3 integer.
+IPA_HD double ipa_flog12_t(double s, const double* mt) {
+  const unsigned off = ((unsigned)ipa_hi(s) >> 8) & 0x1ff0u;
+  const double2 e = *ipa_mt_at(mt, off);
+  return ipa_log1p_small_add(fma(s, e.x, -1.0), e.y);
+}
+
+// log(u), u > 0 normal: u = 2^e m, table entry of the top 8 mantissa bits.  8 FP64.
+IPA_HD double ipa_flog_t(double u, const double* mt) {
+  const int hu = ipa_hi(u);
+  const int e = (hu >> 20) - 1023;
+  const unsigned off = 4096u + (((unsigned)hu >> 8) & 0xff0u);
+  const double m = ipa_mk((hu & 0x000fffff) | 0x3ff00000, ipa_lo(u));
+  const double ef = ipa_mk(0x43300000, e ^ (int)0x80000000) - 4503601774854144.0;  // 2^52 + 2^31
+  const double2 t = *ipa_mt_at(mt, off);
+  return fma(ef, IPA_LN2, ipa_log1p_small_add(fma(m, t.x, -1.0), t.y));
+}
+
+// e^{-|D|}, any D with |D| < 5e6 (beyond that the integer part of -|D| 256/ln2 leaves 32 bits; the largest |Delta|
+// the kernels produce on purpose is the f == 0 sentinel, 1e4).  9 FP64.
+IPA_HD double ipa_fexp_negabs_t(double D, const double* mt) {
+  const double SHIFT = 6755399441055744.0;
+  const double a = -fabs(D);
+  const double t = fma(a, IPA_LOG2E_256, SHIFT);
+  int m = ipa_lo(t);                                    // round(a 256 / ln 2) = 256 n + j
+  const double nf = t - SHIFT;
+  double r = fma(nf, -IPA_LN2_256_HI, a);
+  r = fma(nf, -IPA_LN2_256_LO, r);
+  const double T = ipa_mt_d(mt, 16u + (((unsigned)m & 255u) << 3));
+  double q = fma(IPA_CEXPQ(3), r, IPA_CEXPQ(2));
+  q = fma(q, r, IPA_CEXPQ(1));
+  q = fma(q, r, IPA_CEXPQ(0));
+  const double w = fma(T * r, q, T);
+  m = m > -256000 ? m : -256000;                        // 2^n stays a normal number (w < 1e-300 is not distinguished)
+  return ipa_mk(ipa_hi(w) + ((m >> 8) << 20), ipa_lo(w));
+}
+
+// eb + log(1 + e^D) = eb + log(1 + e^{-|D|}) [+ D if D >= 0]: max(D, 0) is a predicated add on the sign word.
+// (max(D, 0) = D/2 + |D|/2 folded into two FMAs saves the compare and the selects but cancels for D << 0:
+// 3.5e-15 at D = -52, measured in the host test -- rejected.)
+IPA_HD double ipa_fsoftplus_add_t(double eb, double D, const double* mt) {
+  const double w = ipa_fexp_negabs_t(D, mt);
+  double l = eb + ipa_flog12_t(1.0 + w, mt);
+#ifdef __CUDA_ARCH__
+  asm("{\n\t.reg .pred p;\n\tsetp.ge.s32 p, %2, 0;\n\t@p add.f64 %0, %0, %1;\n\t}" : "+d"(l) : "d"(D), "r"(ipa_hi(D)));
+#else
+  if (ipa_hi(D) >= 0) l += D;
+#endif
+  return l;
 }

@@ -139,7 +139,7 @@ IPA_HD void ipa_core_shape(const IpaSetConsts& c, const double (&d)[E], double (
     // Student-t core (zeta == 0, row f4): V = nu log(d^2 + delta^2), one logarithm, no polynomial
     const double d2 = c.delta2, nu = c.nu;
 #pragma unroll
-    for (int e = 0; e < E; ++e) V[e] = nu * ipa_flog(fma(d[e], d[e], d2), tab);
+    for (int e = 0; e < E; ++e) V[e] = nu * ipa_flog_t(fma(d[e], d[e], d2), tab);
   } else {
     // direct mode (shapes the polynomial cannot cover): per-event Bessel evaluation, out of line
     double dt[E], Pt[E];
@@ -163,7 +163,7 @@ IPA_HD void ipa_tail_shape(const IpaSetConsts& c, bool right, const double (&d)[
   const double* q = right ? &c.uA1 : &c.uA0;
   const double uA = q[0], uB = q[1], nT = q[2];
 #pragma unroll
-  for (int e = 0; e < E; ++e) V[e] = -nT * ipa_flog(fma(uA, d[e], uB), tab);
+  for (int e = 0; e < E; ++e) V[e] = -nT * ipa_flog_t(fma(uA, d[e], uB), tab);
 }
 template <int E, class Tab>
 IPA_HD void ipa_mixed_shape(const IpaSetConsts& c, const double (&d)[E], double (&V)[E], const Tab* tab) {
@@ -173,7 +173,7 @@ IPA_HD void ipa_mixed_shape(const IpaSetConsts& c, const double (&d)[E], double 
   for (int e = 0; e < E; ++e) {
     const bool left = d[e] < d0, right = d[e] > d1;
     const double uA = left ? c.uA0 : c.uA1, uB = left ? c.uB0 : c.uB1, nT = left ? c.n0 : c.n1;
-    const double tl = -nT * ipa_flog(fma(uA, d[e], uB), tab);
+    const double tl = -nT * ipa_flog_t(fma(uA, d[e], uB), tab);
     if (left || right) V[e] = tl;
   }
 }
@@ -229,7 +229,7 @@ IPA_HD void ipa_member_stage_r(const IpaSetConsts& c, const double (&d)[E], cons
     for (int e = 0; e < E; ++e) l[e] = fma(kd, d[e], eB0) + D[e];
   } else {
 #pragma unroll
-    for (int e = 0; e < E; ++e) l[e] = ipa_fsoftplus_add(fma(kd, d[e], eB0), D[e], tab);
+    for (int e = 0; e < E; ++e) l[e] = ipa_fsoftplus_add_t(fma(kd, d[e], eB0), D[e], tab);
   }
 }
 template <int E, class Tab>
@@ -302,8 +302,10 @@ __device__ __forceinline__ int ipa_ev_off(int tid, int e) {
   return (tid >> 5) * (32 * IPA_NE) + 2 * ((e >> 1) * 32 + (tid & 31)) + (e & 1);
 }
 
-__device__ __forceinline__ void ipa_load_logtab(double2* tab) {
-  if (threadIdx.x < 33) tab[threadIdx.x] = ipa_c_logtab[threadIdx.x];
+// the 8 KB math table (ipa_fastmath.cuh) from global to shared memory, 16 bytes per thread and step
+__device__ __forceinline__ void ipa_load_mathtab(double* tab) {
+  const double2* src = reinterpret_cast<const double2*>(ipa_d_mathtab);
+  for (int i = threadIdx.x; i < IPA_MATHTAB_DOUBLES / 2; i += blockDim.x) reinterpret_cast<double2*>(tab)[i] = src[i];
 }
 
 // 16-byte asynchronous global -> shared copy (LDGSTS, L2 only) and its group fences
@@ -359,7 +361,7 @@ __device__ __forceinline__ void ipa_tile_store_acc(int k, double (&l)[IPA_NE], d
 template <bool LOGPDF, bool FULL, bool GROUPED>
 __device__ __forceinline__ void ipa_tile_sets(const IpaSetConsts* sc, int K, const IpaGroups& grp, double* acc,
                                               const double (&xv)[IPA_NE], long long base, long long n, int tid,
-                                              double* __restrict__ logpdf, const double2* s_tab) {
+                                              double* __restrict__ logpdf, const double* s_tab) {
   if (LOGPDF) {
     // per-event output of a set with a domain error: NaN (its NLL is +inf)
     for (int k = 0; k < K; ++k) {
@@ -414,7 +416,7 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
   double* stage = reinterpret_cast<double*>(ipa_smem);                       // [2][IPA_NTILE]
   IpaSetConsts* sc = reinterpret_cast<IpaSetConsts*>(stage + 2 * IPA_NTILE);  // [K]
   double* acc = reinterpret_cast<double*>(sc + K);                            // [K][IPA_NB]
-  __shared__ double2 s_tab[33];
+  __shared__ __align__(16) double s_tab[IPA_MATHTAB_DOUBLES];
   __shared__ int s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int G = gridDim.x;
@@ -434,7 +436,7 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
     double* dst = reinterpret_cast<double*>(sc);
     for (int i = tid; i < nd; i += IPA_NB) dst[i] = csrc[i];
     for (int k = 0; k < K; ++k) acc[k * IPA_NB + tid] = 0.0;
-    ipa_load_logtab(s_tab);
+    ipa_load_mathtab(s_tab);
   }
   __syncthreads();
   unsigned bufoff = 0;
@@ -535,12 +537,12 @@ template <class Tab>
 IPA_HD void ipa_grad_tail(const IpaSetConsts& c, bool right, double d, double& D, double& dd, double& ds, const Tab* tab) {
   if (!right) {
     const double u = fma(c.uA0, d, c.uB0), ru = ipa_frcp(u);
-    D = fma(-c.kd, d, fma(-c.n0, ipa_flog(u, tab), c.cT0));
+    D = fma(-c.kd, d, fma(-c.n0, ipa_flog_t(u, tab), c.cT0));
     dd = c.L0 * ru;
     ds = fma(fma(-(d - c.d0), c.c0s, c.aL0), ru, c.A0);
   } else {
     const double u = fma(c.uA1, d, c.uB1), ru = ipa_frcp(u);
-    D = fma(-c.kd, d, fma(-c.n1, ipa_flog(u, tab), c.cT1));
+    D = fma(-c.kd, d, fma(-c.n1, ipa_flog_t(u, tab), c.cT1));
     dd = c.L1 * ru;
     ds = fma(-fma(d - c.d1, c.c1s, c.a2L1), ru, c.A1);
   }
@@ -549,12 +551,12 @@ IPA_HD void ipa_grad_tail(const IpaSetConsts& c, bool right, double d, double& D
 template <class Tab>
 IPA_HD void ipa_grad_mix(const IpaSetConsts& c, double d, double D, double dd, double ds, double& l, double& gm, double& gs,
                          double& gf, double& gk, const Tab* tab) {
-  const double w = ipa_fexp_negabs(D);
+  const double w = ipa_fexp_negabs_t(D, tab);
   const double s1 = 1.0 + w;
   const double rs = ipa_frcp(s1);
   const bool pos = ipa_hi(D) >= 0;
   const double wS = pos ? rs : w * rs, wB = pos ? w * rs : rs;
-  l = fma(c.kd, d, c.eB0) + ipa_flog_1to2(s1, tab);
+  l = fma(c.kd, d, c.eB0) + ipa_flog12_t(s1, tab);
   if (pos) l += D;
   gm = wS * (-dd - c.dlnNS_dmu);
   gs = wS * (ds - c.dlnNS_dsig);
@@ -619,7 +621,7 @@ IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&
       else if (c.mode == 2) {   // Student-t core: log G = nu log q + beta d, L - beta = 2 nu d / q
         const double q = fma(d[e], d[e], c.delta2);
         const double Lmb = 2.0 * c.nu * d[e] * ipa_frcp(q);
-        D[e] = fma(c.bmk, d[e], fma(c.nu, ipa_flog(q, tab), c.a[0]));
+        D[e] = fma(c.bmk, d[e], fma(c.nu, ipa_flog_t(q, tab), c.a[0]));
         dd[e] = c.beta + Lmb;
         ds[e] = fma(-d[e] * c.invsig, Lmb, c.nuosig);
       } else {   // direct mode: Bessel functions per event (slow path)
@@ -654,7 +656,7 @@ ipa_nll_grad_kernel(const double* __restrict__ x, long long n, int vec_ok, const
                     double* __restrict__ partials, unsigned int* counters, double* __restrict__ nll_out,
                     double* __restrict__ grad_out, int32_t* __restrict__ status_out) {
   __shared__ IpaSetConsts c;
-  __shared__ double2 s_tab[33];
+  __shared__ __align__(16) double s_tab[IPA_MATHTAB_DOUBLES];
   __shared__ double red[5][IPA_GB / 32];
   __shared__ int s_last;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, k = blockIdx.y, G = gridDim.x;
@@ -662,7 +664,7 @@ ipa_nll_grad_kernel(const double* __restrict__ x, long long n, int vec_ok, const
     const double* src = reinterpret_cast<const double*>(consts + k);
     double* dst = reinterpret_cast<double*>(&c);
     for (int i = tid; i < (int)(sizeof(IpaSetConsts) / 8); i += IPA_GB) dst[i] = src[i];
-    ipa_load_logtab(s_tab);
+    ipa_load_mathtab(s_tab);
   }
   __syncthreads();
   const int st = c.status ? c.status : ((c.pure || !(c.fsig > 0.0)) ? 4 : 0);   // 4: the gradient needs 0 < f < 1
@@ -748,7 +750,7 @@ ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ o
                    double* __restrict__ partials) {
   __shared__ IpaSetConsts c;
   __shared__ double red[IPA_BLOCK / 32];
-  __shared__ double2 s_tab[33];
+  __shared__ __align__(16) double s_tab[IPA_MATHTAB_DOUBLES];
   __shared__ __align__(16) double stage[2][IPA_TILE];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   const int C = gridDim.y;
@@ -781,7 +783,7 @@ ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ o
     const double* csrc = reinterpret_cast<const double*>(consts + (set_of_segment ? set_of_segment[t] : t));
     double* dst = reinterpret_cast<double*>(&c);
     for (int i = tid; i < (int)(sizeof(IpaSetConsts) / 8); i += IPA_BLOCK) dst[i] = csrc[i];
-    ipa_load_logtab(s_tab);
+    ipa_load_mathtab(s_tab);
   }
   __syncthreads();
   double acc = 0.0;

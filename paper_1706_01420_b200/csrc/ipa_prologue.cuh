@@ -480,8 +480,9 @@ IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
   o.normB = NB;
   const double logNS = log(NSr) + w.logref;
   const bool pure = !(p.f < 1.0);
-  // f = 0: a finite, hugely negative signal term (softplus(-1e9) == 0 exactly) instead of -inf
-  const double cS = (p.f > 0.0) ? w.logf - logNS : -1.0e9;
+  // f = 0: a finite, very negative signal term (softplus(-1e4) == 0 exactly) instead of -inf; it stays far inside the
+  // range |Delta| < 5e6 of the kernels' exponential (ipa_fexp_negabs_t)
+  const double cS = (p.f > 0.0) ? w.logf - logNS : -1.0e4;
   const double kd = pure ? 0.0 : p.k;
   const double eB0 = pure ? 0.0 : (p.k * (p.mu - w.lo) + w.log1mf - w.logNB);
   o.pure = pure ? 1 : 0;

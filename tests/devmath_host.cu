@@ -51,7 +51,7 @@ void emu_logpdf(const ipa_params* p, double lo, double hi, int policy, const dou
     double xv[8], l[8];
     for (int e = 0; e < 8; ++e) xv[e] = (i + e < n) ? x[i + e] : x[n - 1];
     if (c.status) { for (int e = 0; e < 8; ++e) l[e] = -INFINITY; }
-    else ipa_eval_set<8>(c, xv, l, ipa_h_logtab);
+    else ipa_eval_set<8>(c, xv, l, ipa_h_mathtab);
     for (int e = 0; e < 8 && i + e < n; ++e) out[i + e] = l[e];
   }
 }
@@ -63,7 +63,7 @@ void emu_grad(const ipa_params* p, double lo, double hi, int policy, const doubl
   for (long long i = 0; i < n; i += 4) {
     double xv[4], l[4], gm[4], gs[4], gf[4], gk[4];
     for (int e = 0; e < 4; ++e) xv[e] = (i + e < n) ? x[i + e] : x[n - 1];
-    ipa_eval_grad<4>(c, xv, l, gm, gs, gf, gk, ipa_h_logtab);
+    ipa_eval_grad<4>(c, xv, l, gm, gs, gf, gk, ipa_h_mathtab);
     for (int e = 0; e < 4 && i + e < n; ++e) { out[0] -= l[e]; out[1] -= gm[e]; out[2] -= gs[e]; out[3] -= gf[e]; out[4] -= gk[e]; }
   }
 }
@@ -111,5 +111,12 @@ void emu_fexp_neg(const double* a, long long n, double* out) {
 void emu_flog(const double* u, long long n, double* out) { for (long long i = 0; i < n; ++i) out[i] = ipa_flog(u[i], ipa_h_logtab); }
 void emu_fsoftplus(const double* D, long long n, double* out) {
   for (long long i = 0; i < n; ++i) out[i] = ipa_fsoftplus(D[i], ipa_h_logtab);
+}
+// table-driven versions of the streaming kernels (round 2)
+void emu_fexp_negabs_t(const double* a, long long n, double* out) { for (long long i = 0; i < n; ++i) out[i] = ipa_fexp_negabs_t(a[i], ipa_h_mathtab); }
+void emu_flog_t(const double* u, long long n, double* out) { for (long long i = 0; i < n; ++i) out[i] = ipa_flog_t(u[i], ipa_h_mathtab); }
+void emu_flog12_t(const double* u, long long n, double* out) { for (long long i = 0; i < n; ++i) out[i] = ipa_flog12_t(u[i], ipa_h_mathtab); }
+void emu_fsoftplus_add_t(const double* eb, const double* D, long long n, double* out) {
+  for (long long i = 0; i < n; ++i) out[i] = ipa_fsoftplus_add_t(eb[i], D[i], ipa_h_mathtab);
 }
 }

@@ -203,3 +203,50 @@ def test_device_gradient_math_vs_oracle(emu, orc, shape):
         assert abs(out[0] - nll) <= 1e-12 * abs(nll)
         s = np.array([inp.GRAD_SCALE[k] for k in inp.FLOATED])
         assert np.all(np.abs(out[1:] - g) <= 1e-9 * np.maximum(np.abs(g), 1.0 / s)), (out[1:], g)
+
+
+def test_device_fastmath_vs_mpmath(emu):
+    """The streaming kernels' own sqrt / exp / log (csrc/ipa_fastmath.cuh, host build of the same source) against
+    mpmath at 30 digits: sqrt <= 2e-16 relative, e^{-|D|} <= 3e-16 relative, log <= 2.5e-16 + 1.5e-16 |log u| absolute,
+    log on [1,2] <= 2.5e-16 absolute, the fused softplus eb + log(1 + e^D) <= 2.5e-16 (1 + |eb| + |D|)."""
+    import mpmath as mp
+    mp.mp.dps = 30
+    rng = np.random.Generator(np.random.Philox(17))
+    vp = C.c_void_p
+
+    def run(fn, *arrs):
+        out = np.empty_like(arrs[0])
+        getattr(emu, fn)(*[a.ctypes.data_as(vp) for a in arrs], C.c_longlong(arrs[0].size), out.ctypes.data_as(vp))
+        return out
+    for name in ("emu_fsqrt", "emu_fexp_negabs_t", "emu_flog_t", "emu_flog12_t", "emu_fsoftplus_add_t", "emu_flog", "emu_fexp_neg"):
+        getattr(emu, name).restype = None
+    q = np.concatenate([10.0 ** rng.uniform(-3, 8, 4000), [1.0, 2.0, 4.0, 83.349, 983.0, 1e-300, 1e300]])
+    got = run("emu_fsqrt", q)
+    assert max(abs(mp.mpf(float(g)) / mp.sqrt(mp.mpf(float(v))) - 1) for g, v in zip(got, q)) <= 2e-16
+    D = np.concatenate([rng.uniform(-60, 60, 6000), rng.uniform(-1, 1, 2000) * 1e-3, [0.0, -0.0, 1e-300, 700.0, -745.0, 1.0e4, -1.0e4,
+                                                                                     4.9e6, np.log(2) / 512, -np.log(2) / 512]])
+    got = run("emu_fexp_negabs_t", D)
+    for g, v in zip(got, D):
+        ref = mp.exp(-abs(mp.mpf(float(v))))
+        assert abs(mp.mpf(float(g)) - ref) <= 3e-16 * ref + 1e-300, (v, g)
+    u = np.concatenate([10.0 ** rng.uniform(-8, 8, 6000), 1.0 + rng.uniform(0, 1, 2000) * 2.0 ** -rng.integers(1, 40, 2000),
+                        [1.0, 2.0, 0.5, 9.75, 1.0 + 2.0 ** -52, 2.0 - 2.0 ** -52, 1e-300, 1e300]])
+    for fn in ("emu_flog_t", "emu_flog"):
+        got = run(fn, u)
+        for g, v in zip(got, u):
+            ref = mp.log(mp.mpf(float(v)))
+            assert abs(mp.mpf(float(g)) - ref) <= 2.5e-16 + 1.5e-16 * abs(ref), (fn, v, g)
+    s = np.concatenate([1.0 + rng.uniform(0, 1, 6000), 1.0 + 10.0 ** rng.uniform(-20, 0, 2000), [1.0, 2.0, 1.5, 1.0 + 2.0 ** -52,
+                                                                                             2.0 - 2.0 ** -52, 1.0 + 2.0 ** -9]])
+    s = np.minimum(s, 2.0)
+    got = run("emu_flog12_t", s)
+    assert max(abs(mp.mpf(float(g)) - mp.log(mp.mpf(float(v)))) for g, v in zip(got, s)) <= 2.5e-16
+    eb = rng.uniform(-12, -4, D.size)
+    got = run("emu_fsoftplus_add_t", eb, D)
+    for g, b, v in zip(got, eb, D):
+        ref = mp.mpf(float(b)) + mp.log(1 + mp.exp(mp.mpf(float(v))))
+        assert abs(mp.mpf(float(g)) - ref) <= 2.5e-16 * (1 + abs(b) + abs(v)), (b, v, g)      # three roundings of O(|eb| + |D|) terms
+    # NaN in, NaN out; the table index of a NaN stays inside the 8 KB table
+    nan = np.array([np.nan])
+    assert np.isnan(run("emu_flog12_t", nan)[0])           # (the general log rebuilds the mantissa: a NaN event is
+    assert np.isnan(run("emu_fsoftplus_add_t", nan, nan)[0])   #  carried by E_B = k d + const, tested on the GPU)
