@@ -31,7 +31,9 @@ T2 = dict(mu=5280.0, sigma=15.0, **{"lambda": -0.7}, zeta=0.0, beta=0.004, a=1.2
 
 FLOATED = ("mu", "sigma", "f", "k")                   # reading C6: order of the floated parameters
 FD_STEPS = dict(mu=0.01, sigma=0.01, f=1e-4, k=1e-6)  # reading C6: central-difference steps
-GRAD_SCALE = dict(mu=0.3, sigma=0.3, f=0.007, k=7e-5)  # reading D18: ~1 sigma fit errors at N=1e4
+GRAD_SCALE = dict(mu=0.3, sigma=0.3, f=0.007, k=7e-5,  # reading D18: ~1 sigma fit errors at N=1e4
+                  beta=1.2e-3)                         # analytic gradient only (fifth component): 1 / (sqrt(N_sig) sigma)
+GRAD_NAMES = ("mu", "sigma", "f", "k", "beta")         # components of the analytic gradient (row f1)
 FIT_START_SHIFT = dict(mu=1.0, sigma=1.0, f=0.02, k=1e-4)
 
 

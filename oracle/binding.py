@@ -295,21 +295,21 @@ def cls_from_counts(count_sb, T_sb, count_b, T_b):
 
 
 def nll_gradient(x, p, lo, hi):
-    """Analytic (nll, d nll / d (mu, sigma, f, k)) of one parameter set; SURVEY.md 8(f) row f1."""
+    """Analytic (nll, d nll / d (mu, sigma, f, k, beta)) of one parameter set; SURVEY.md 8(f) row f1."""
     x = np.ascontiguousarray(x, dtype=np.float64)
     P = pack_params(p)
     assert P.shape[0] == 1
     nll = np.empty(1)
-    g = np.empty(4)
+    g = np.empty(5)
     st = lib().orc_nll_gradient(_p(x), x.size, _p(P), float(lo), float(hi), _p(nll), _p(g))
     assert st == 0, st
     return float(nll[0]), g
 
 
 def norm_derivs(p, lo, hi):
-    """(d ln N_S / d mu, d ln N_S / d sigma, d ln N_B / d k) of one parameter set."""
+    """(d ln N_S / d mu, d ln N_S / d sigma, d ln N_B / d k, d ln N_S / d beta) of one parameter set."""
     P = pack_params(p)
-    out = np.empty(3)
+    out = np.empty(4)
     st = lib().orc_norm_derivs(_p(P), float(lo), float(hi), _p(out))
     assert st == 0, st
     return out

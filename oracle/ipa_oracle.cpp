@@ -437,6 +437,11 @@ static ld nll_one(const double* x, int64_t n, const orc_params& p, ld lo, ld hi)
  *   d N_S / d mu    = I(lo - mu) - I(hi - mu)                      (Leibniz: the limits move with mu)
  *   d N_S / d sigma = int_lo^hi I dlogI/dsigma dx                  (composite Gauss-Legendre per region)
  *   d ln N_B / d k  = w e^{k w} / expm1(k w) - 1/k,  w = hi - lo   (-> w/2 as k -> 0)
+ * beta (fifth component, round 2; SURVEY.md 8(f) f1 "(mu,sigma,f,k[,beta,...])"): delta and alpha do not depend on
+ * beta, the core carries e^{beta d}, and the tails inherit beta through log G(d_join) and L_join (dL_join/dbeta = 1):
+ *   d l / d beta = w_S ( dlogI/dbeta (x - mu) - d ln N_S / d beta )
+ *   core   dlogI/dbeta = d        left   dlogI/dbeta = d0 + (d - d0)/u        right  dlogI/dbeta = d1 + (d - d1)/u
+ *   d N_S / d beta = int_lo^hi I dlogI/dbeta dx                        (composite Gauss-Legendre per region)
  * ---------------------------------------------------------------------------------------- */
 static ld dlogI_dd(const Shape& s, ld d) {
   if (d < s.d0) return s.L0 / (1 - (d - s.d0) * s.L0 / s.n);
@@ -454,9 +459,14 @@ static ld dlogI_dsigma(const Shape& s, ld d) {
   }
   return s.sigpow / s.sigma + (d / s.sigma) * (s.beta - core_logderiv(s, d));
 }
-/* int_A^B I(d) dlogI/dsigma(d) e^{-logref} dd inside ONE region (smooth integrand), composite 20-point
- * Gauss-Legendre, panels doubled until stable */
-static ld dsigma_integral_scaled(const Shape& s, ld A, ld B, ld logref) {
+static ld dlogI_dbeta(const Shape& s, ld d) {
+  if (d < s.d0) return s.d0 + (d - s.d0) / (1 - (d - s.d0) * s.L0 / s.n);
+  if (d > s.d1) return s.d1 + (d - s.d1) / (1 - (d - s.d1) * s.L1 / s.n2);
+  return d;
+}
+/* int_A^B I(d) dlogI/dtheta(d) e^{-logref} dd inside ONE region (smooth integrand), theta = sigma (which = 0) or
+ * beta (which = 1); composite 20-point Gauss-Legendre, panels doubled until stable */
+static ld dsigma_integral_scaled(const Shape& s, ld A, ld B, ld logref, int which = 0) {
   if (!(B > A)) return 0;
   std::vector<ld> gx, gw;
   gauss_legendre(20, gx, gw);
@@ -469,7 +479,7 @@ static ld dsigma_integral_scaled(const Shape& s, ld A, ld B, ld logref) {
       ld acc = 0;
       for (int i = 0; i < 20; ++i) {
         const ld d = c + 0.5L * h * gx[i];
-        acc += gw[i] * expl(log_I(s, d) - logref) * dlogI_dsigma(s, d);
+        acc += gw[i] * expl(log_I(s, d) - logref) * (which ? dlogI_dbeta(s, d) : dlogI_dsigma(s, d));
       }
       tot += acc * 0.5L * h;
     }
@@ -479,7 +489,8 @@ static ld dsigma_integral_scaled(const Shape& s, ld A, ld B, ld logref) {
   return prev;
 }
 /* d ln N_S / d mu, d ln N_S / d sigma, d ln N_B / d k  (N.NS is in units of exp(logref)) */
-static void norm_derivs(const Shape& s, const Norm& N, ld k, ld lo, ld hi, ld* dlnNS_dmu, ld* dlnNS_dsig, ld* dlnNB_dk) {
+static void norm_derivs(const Shape& s, const Norm& N, ld k, ld lo, ld hi, ld* dlnNS_dmu, ld* dlnNS_dsig, ld* dlnNB_dk,
+                        ld* dlnNS_dbeta = nullptr) {
   const ld dl = lo - s.mu, dh = hi - s.mu;
   const ld dNS_dmu = expl(log_I(s, dl) - N.logref) - expl(log_I(s, dh) - N.logref);
   ld dNS_dsig = 0;
@@ -489,32 +500,37 @@ static void norm_derivs(const Shape& s, const Norm& N, ld k, ld lo, ld hi, ld* d
   for (int i = 0; i < 3; ++i) if (inner[i] > dl && inner[i] < dh) cuts[nc++] = inner[i];
   cuts[nc++] = dh;
   for (int i = 0; i + 1 < nc; ++i) dNS_dsig += dsigma_integral_scaled(s, cuts[i], cuts[i + 1], N.logref);
+  if (dlnNS_dbeta) {
+    ld dNS_dbeta = 0;
+    for (int i = 0; i + 1 < nc; ++i) dNS_dbeta += dsigma_integral_scaled(s, cuts[i], cuts[i + 1], N.logref, 1);
+    *dlnNS_dbeta = dNS_dbeta / N.NS;
+  }
   *dlnNS_dmu = dNS_dmu / N.NS;
   *dlnNS_dsig = dNS_dsig / N.NS;
   const ld w = hi - lo, t = k * w;
   *dlnNB_dk = (fabsl(t) < 1e-6L) ? w * (0.5L + t / 12) : w * expl(t) / expm1l(t) - 1 / k;
 }
-extern "C" int orc_norm_derivs(const orc_params* pp, double lo, double hi, double* out /* [3] */) {
+extern "C" int orc_norm_derivs(const orc_params* pp, double lo, double hi, double* out /* [4]: mu, sigma, k, beta */) {
   const Shape s = make_shape(*pp);
   if (s.status) return s.status;
   const Norm N = make_norm(s, pp->k, lo, hi);
-  ld a, b, c;
-  norm_derivs(s, N, pp->k, lo, hi, &a, &b, &c);
-  out[0] = (double)a; out[1] = (double)b; out[2] = (double)c;
+  ld a, b, c, e;
+  norm_derivs(s, N, pp->k, lo, hi, &a, &b, &c, &e);
+  out[0] = (double)a; out[1] = (double)b; out[2] = (double)c; out[3] = (double)e;
   return 0;
 }
 extern "C" int orc_nll_gradient(const double* x, int64_t n, const orc_params* pp, double lo_, double hi_, double* nll,
-                                double* grad /* d NLL / d (mu, sigma, f, k) */) {
+                                double* grad /* d NLL / d (mu, sigma, f, k, beta) */) {
   const orc_params& p = *pp;
   const Shape s = make_shape(p);
   if (s.status) return s.status;
   const ld lo = lo_, hi = hi_, f = p.f, k = p.k;
   const Norm N = make_norm(s, k, lo, hi);
   const ld dl = lo - s.mu, dh = hi - s.mu;
-  ld dlnNS_dmu, dlnNS_dsig, dlnNB_dk;
-  norm_derivs(s, N, k, lo, hi, &dlnNS_dmu, &dlnNS_dsig, &dlnNB_dk);
+  ld dlnNS_dmu, dlnNS_dsig, dlnNB_dk, dlnNS_dbeta;
+  norm_derivs(s, N, k, lo, hi, &dlnNS_dmu, &dlnNS_dsig, &dlnNB_dk, &dlnNS_dbeta);
   (void)dl; (void)dh;
-  std::vector<double> g0((size_t)n), g1((size_t)n), g2((size_t)n), g3((size_t)n), l((size_t)n);
+  std::vector<double> g0((size_t)n), g1((size_t)n), g2((size_t)n), g3((size_t)n), g4((size_t)n), l((size_t)n);
   for (int64_t i = 0; i < n; ++i) {
     const ld d = (ld)x[i] - s.mu;
     const ld ES = (f > 0) ? logl(f) + log_I(s, d) - N.logref - logl(N.NS) : -INFINITY;
@@ -529,12 +545,14 @@ extern "C" int orc_nll_gradient(const double* x, int64_t n, const orc_params* pp
     const ld BoverMix = (f < 1) ? wB / (1 - f) : expl(k * ((ld)x[i] - lo) - logl(N.NB) - li);
     g2[i] = (double)(SoverMix - BoverMix);
     g3[i] = (double)(wB * (((ld)x[i] - lo) - dlnNB_dk));
+    g4[i] = (double)(wS * (dlogI_dbeta(s, d) - dlnNS_dbeta));
   }
   *nll = (double)(-pairwise(l.data(), 0, n));
   grad[0] = (double)(-pairwise(g0.data(), 0, n));
   grad[1] = (double)(-pairwise(g1.data(), 0, n));
   grad[2] = (double)(-pairwise(g2.data(), 0, n));
   grad[3] = (double)(-pairwise(g3.data(), 0, n));
+  grad[4] = (double)(-pairwise(g4.data(), 0, n));
   return 0;
 }
 /* ------------------------------------------------------------------------------------------

@@ -11,7 +11,7 @@ import ipa_inputs as inp
 from test_oracle_ipatia import MPModel
 
 LO, HI = inp.LO, inp.HI
-NAMES = ("mu", "sigma", "f", "k")
+NAMES = inp.GRAD_NAMES          # (mu, sigma, f, k, beta)
 
 
 def mp_nll(p, xs):
@@ -44,6 +44,7 @@ def test_fd_gradient_batch_layout_and_quadratic_convergence(orc):
     x = np.array([5010.0, 5120.0, 5236.0, 5266.0, 5279.0, 5291.5, 5322.0, 5470.0])
     theta = inp.as_array(inp.P2)
     _, g = orc.nll_gradient(x, theta, LO, HI)
+    g = g[:4]
     idx, h0 = inp.fd_spec()
     errs = []
     for scale in (1.0, 0.5):
@@ -69,12 +70,20 @@ def test_gradient_limits(orc):
     x = orc.generate_mixture(7, 500, inp.GEN, LO, HI)
     # f = 0: no dependence on the signal shape; f = 1: none on k; k = 0 uses the series of d ln N_B / d k
     _, g0 = orc.nll_gradient(x, dict(inp.GEN, f=0.0), LO, HI)
-    assert g0[0] == 0.0 and g0[1] == 0.0
+    assert g0[0] == 0.0 and g0[1] == 0.0 and g0[4] == 0.0
     _, g1 = orc.nll_gradient(x, dict(inp.GEN, f=1.0), LO, HI)
     assert g1[3] == 0.0
     _, gk = orc.nll_gradient(x, dict(inp.GEN, k=0.0), LO, HI)
     _, gk2 = orc.nll_gradient(x, dict(inp.GEN, k=1e-9), LO, HI)
     assert np.all(np.abs(gk - gk2) <= 1e-6 * np.maximum(1.0, np.abs(gk)))
+    # beta by central differences of the oracle's own NLL (O(h^2)), at a shape with beta != 0 and asymmetric tails
+    xb = inp.standin_masses(31, 3000)
+    _, gb = orc.nll_gradient(xb, inp.P2, LO, HI)
+    errs = []
+    for h in (2e-4, 1e-4):
+        fd = (orc.nll(xb, dict(inp.P2, beta=inp.P2["beta"] + h), LO, HI)[0] - orc.nll(xb, dict(inp.P2, beta=inp.P2["beta"] - h), LO, HI)[0]) / (2 * h)
+        errs.append(fd - gb[4])
+    assert abs(errs[1]) <= 1e-5 * max(abs(gb[4]), 1.0 / inp.GRAD_SCALE["beta"]) and 3.0 < errs[0] / errs[1] < 5.0
     # at the generating parameters of a large sample every component is small in units of its error
     xl = orc.generate_mixture(2, 100000, inp.GEN, LO, HI)
     _, g = orc.nll_gradient(xl, inp.GEN, LO, HI)

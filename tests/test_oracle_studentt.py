@@ -165,8 +165,12 @@ def test_analytic_gradient_and_domain(orc):
     O(h^2) convergence (the sigma-homogeneity power of G is 2 nu here, not nu); domain rules of zeta = 0."""
     x = inp.standin_masses(21, 4000)
     for p in (T1, T2):
-        nll, g = orc.nll_gradient(x, p, LO, HI)
+        nll, g5 = orc.nll_gradient(x, p, LO, HI)
+        g = g5[:4]
         assert abs(nll - orc.nll(x, p, LO, HI)[0]) <= 1e-12 * abs(nll)
+        hb = 1e-4                                             # beta (fifth component) by central differences
+        fdb = (orc.nll(x, dict(p, beta=p["beta"] + hb), LO, HI)[0] - orc.nll(x, dict(p, beta=p["beta"] - hb), LO, HI)[0]) / (2 * hb)
+        assert abs(fdb - g5[4]) <= 1e-5 * max(abs(g5[4]), 1.0 / inp.GRAD_SCALE["beta"])
         idx, h = inp.fd_spec()
         _, g1 = orc.fd_gradient(x, p, idx, h, LO, HI)
         _, g2 = orc.fd_gradient(x, p, idx, h / 2, LO, HI)
