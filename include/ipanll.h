@@ -157,14 +157,15 @@ int ipa_nll_eval_extended(const double* x_dev, int64_t n, const ipa_params* p_ho
                           const double* nb_host, int K, ipa_range r, double* nll_dev, int32_t* status_dev,
                           const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream);
 
-/* NLL and its ANALYTIC gradient with respect to (mu, sigma, f, k) in one pass (the
+/* NLL and its ANALYTIC gradient with respect to (mu, sigma, f, k, beta) in one pass (the
  * paper mentions analytic gradients through iminuit and generated derivative code, PAPER.md:36, 383,
  * without formulae; the derivatives are those of the definition above):
- *   nll_dev  [K]    as ipa_nll_eval (same value up to rounding: the core term is evaluated with one Horner
- *                   pass for the polynomial and its derivative)
- *   grad_dev [4*K]  d NLL / d (mu, sigma, f, k) of set k at grad_dev[4 k .. 4 k + 3]
- * Needs 0 < f < 1: a set with f == 0 or f == 1 gets status 4, NLL = +inf and NaN derivatives.  Every
- * set streams the events on its own (the call is meant for one or a few sets).  K <= IPA_MAX_K. */
+ *   nll_dev  [K]              as ipa_nll_eval (same value up to rounding: the core term is evaluated with one
+ *                             Horner pass for the polynomial and its derivative)
+ *   grad_dev [IPA_NGRAD * K]  d NLL / d (mu, sigma, f, k, beta) of set k at grad_dev[IPA_NGRAD k .. IPA_NGRAD k + 4]
+ * Needs 0 < f < 1: a set with f == 0 or f == 1 gets status 4, NLL = +inf and NaN derivatives.  The events are
+ * read once for up to 4 sets (more sets: one pass per group of 4).  K <= IPA_MAX_K. */
+#define IPA_NGRAD 5
 int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r,
                       double* nll_dev, double* grad_dev, int32_t* status_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes,
                       void* cuda_stream);

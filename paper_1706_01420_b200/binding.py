@@ -283,14 +283,14 @@ def ipa_nll_eval_extended(x, params, ns, nb, lo, hi, ws=None, stream=None, polic
 
 @_alloc_on_stream
 def ipa_nll_grad_eval(x, params, lo, hi, ws=None, stream=None, policy=None):
-    """NLL and analytic gradient w.r.t. (mu, sigma, f, k): -> (nll[K], grad[K, 4], status[K]) device tensors."""
+    """NLL and analytic gradient w.r.t. (mu, sigma, f, k, beta): -> (nll[K], grad[K, 5], status[K]) device tensors."""
     _need_cuda()
     P = pack_params(params)
     K = P.shape[0]
     n = x.numel()
     ws = _ws(ws, n, K)
     nll = torch.empty(K, dtype=torch.float64, device="cuda")
-    grad = torch.empty((K, 4), dtype=torch.float64, device="cuda")
+    grad = torch.empty((K, 5), dtype=torch.float64, device="cuda")
     st = torch.empty(K, dtype=torch.int32, device="cuda")
     _check(lib().ipa_nll_grad_eval(_dptr(x, torch.float64) if n else None, n, _hptr(P), K, _Range(lo, hi), _dptr(nll),
                                    _dptr(grad), _dptr(st), _opt(policy), _dptr(ws), ws.numel(), _stream(stream)))

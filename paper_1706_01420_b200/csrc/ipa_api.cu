@@ -30,6 +30,7 @@ int policy_of(const ipa_options* o) {
 }
 
 constexpr int64_t kGridMax = 2048;  // upper bound of the streaming grid (partials sizing)
+constexpr size_t kGradSmem = 2 * IPA_GTILE * 8 + IPA_GKB * (sizeof(IpaSetConsts) + IPA_GQ * IPA_GB * 8);
 
 size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
@@ -73,6 +74,8 @@ int device_info(int* sms) {
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    IPA_CK(cudaFuncSetAttribute(ipa_nll_grad_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGradSmem));
+    IPA_CK(cudaFuncSetAttribute(ipa_nll_grad_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)kGradSmem));
     IPA_CK(cudaFuncSetAttribute(ipa_prep_scatter_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, IPA_PREP_SMEM));
     IPA_CK(cudaFuncSetAttribute(ipa_prep_segment_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, IPA_PREP_SMEM));
     // four resident blocks per SM need 4 x 43 KB of shared memory: ask for the largest carve-out
@@ -267,15 +270,17 @@ int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, 
   char* ws = static_cast<char*>(ws_dev);
   rc = run_prologue(p_host, K, r, policy, ws, L, nullptr, nullptr, nullptr, st, true);
   if (rc) return rc;
-  IPA_CK(cudaMemsetAsync(ws + L.counter, 0, 256, st));          // one ticket counter per set
-  const int64_t tile_n = (int64_t)IPA_GB * IPA_GE, ntiles = (n + tile_n - 1) / tile_n;
-  int64_t G = (int64_t)sms * IPA_GPSM;
+  IPA_CK(cudaMemsetAsync(ws + L.counter, 0, 256, st));          // one ticket counter per group of IPA_GKB sets
+  const int64_t ntiles = (n + IPA_GTILE - 1) / IPA_GTILE;
+  int64_t G = (int64_t)sms;
   if (G > ntiles) G = ntiles;
   if (G < 1) G = 1;
-  if (G * 5 > kGridMax) G = kGridMax / 5;                        // partials: K x 5 x G doubles fit the K x kGridMax area
+  if (G * IPA_GQ > kGridMax) G = kGridMax / IPA_GQ;              // partials: K x IPA_GQ x G doubles fit the K x kGridMax area
   const int vec_ok = ((uintptr_t)x_dev % 16) == 0;
-  ipa_nll_grad_kernel<<<dim3((unsigned)G, (unsigned)K), IPA_GB, 0, st>>>(
-      x_dev, n, vec_ok, reinterpret_cast<const IpaSetConsts*>(ws + L.consts), reinterpret_cast<double*>(ws + L.partials),
+  const int groups = (K + IPA_GKB - 1) / IPA_GKB;
+  auto kern = (K == 1) ? ipa_nll_grad_kernel<true> : ipa_nll_grad_kernel<false>;
+  kern<<<dim3((unsigned)G, (unsigned)groups), IPA_GB, kGradSmem, st>>>(
+      x_dev, n, vec_ok, reinterpret_cast<const IpaSetConsts*>(ws + L.consts), K, reinterpret_cast<double*>(ws + L.partials),
       reinterpret_cast<unsigned int*>(ws + L.counter), nll_dev, grad_dev, status_dev);
   IPA_CK(cudaGetLastError());
   return IPA_OK;

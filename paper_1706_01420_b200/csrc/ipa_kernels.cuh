@@ -517,6 +517,7 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
 //   w_S = sigmoid(Delta), w_B = 1 - w_S from the same e^{-|Delta|} as the softplus
 // The region of the whole warp is decided as in the NLL kernel; a mixed warp branches per event.
 // ------------------------------------------------------------------------------------------------
+// (dlogI/dbeta is d in the core and d_j + (d - d_j)/u in a tail: computed by the callers)
 template <class Tab>
 IPA_HD void ipa_grad_core(const IpaSetConsts& c, double d, double& D, double& dd, double& ds) {
   const double q = fma(d, d, c.delta2);
@@ -534,23 +535,26 @@ IPA_HD void ipa_grad_core(const IpaSetConsts& c, double d, double& D, double& dd
   ds = fma(-d * c.invsig, Lmb, c.nuosig);
 }
 template <class Tab>
-IPA_HD void ipa_grad_tail(const IpaSetConsts& c, bool right, double d, double& D, double& dd, double& ds, const Tab* tab) {
+IPA_HD void ipa_grad_tail(const IpaSetConsts& c, bool right, double d, double& D, double& dd, double& ds, double& db,
+                          const Tab* tab) {
   if (!right) {
     const double u = fma(c.uA0, d, c.uB0), ru = ipa_frcp(u);
     D = fma(-c.kd, d, fma(-c.n0, ipa_flog_t(u, tab), c.cT0));
     dd = c.L0 * ru;
     ds = fma(fma(-(d - c.d0), c.c0s, c.aL0), ru, c.A0);
+    db = fma(d - c.d0, ru, c.d0);
   } else {
     const double u = fma(c.uA1, d, c.uB1), ru = ipa_frcp(u);
     D = fma(-c.kd, d, fma(-c.n1, ipa_flog_t(u, tab), c.cT1));
     dd = c.L1 * ru;
     ds = fma(-fma(d - c.d1, c.c1s, c.a2L1), ru, c.A1);
+    db = fma(d - c.d1, ru, c.d1);
   }
 }
 // mixture: l = E_B + log(1 + e^Delta) and the four derivative contributions
 template <class Tab>
-IPA_HD void ipa_grad_mix(const IpaSetConsts& c, double d, double D, double dd, double ds, double& l, double& gm, double& gs,
-                         double& gf, double& gk, const Tab* tab) {
+IPA_HD void ipa_grad_mix(const IpaSetConsts& c, double d, double D, double dd, double ds, double db, double& l, double& gm,
+                         double& gs, double& gf, double& gk, double& gb, const Tab* tab) {
   const double w = ipa_fexp_negabs_t(D, tab);
   const double s1 = 1.0 + w;
   const double rs = ipa_frcp(s1);
@@ -562,10 +566,11 @@ IPA_HD void ipa_grad_mix(const IpaSetConsts& c, double d, double D, double dd, d
   gs = wS * (ds - c.dlnNS_dsig);
   gf = fma(wS, c.invf, -wB * c.inv1mf);
   gk = wB * ((d + c.mulo) - c.dlnNB_dk);
+  gb = wS * (db - c.dlnNS_dbeta);
 }
 template <int E, class Tab>
 IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&l)[E], double (&gm)[E], double (&gs)[E],
-                          double (&gf)[E], double (&gk)[E], const Tab* tab) {
+                          double (&gf)[E], double (&gk)[E], double (&gb)[E], const Tab* tab) {
   int hmin = ipa_hi(x[0]), hmax = hmin;
 #pragma unroll
   for (int e = 1; e < E; ++e) {
@@ -576,9 +581,9 @@ IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&
   hmin = ipa_warp_min(hmin);
   hmax = ipa_warp_max(hmax);
   const bool sane = hmin > 0 && hmax < 0x7ff00000;
-  double d[E], D[E], dd[E], ds[E];
+  double d[E], D[E], dd[E], ds[E], db[E];
 #pragma unroll
-  for (int e = 0; e < E; ++e) d[e] = x[e] - c.mu;
+  for (int e = 0; e < E; ++e) { d[e] = x[e] - c.mu; db[e] = d[e]; }      // dlogI/dbeta = d in the core
   if (sane && c.mode == 0 && hmin > c.hxl && hmax < c.hxr) {
     // all E events in the core: one pass over the coefficients (128-bit uniform loads) for H and dH/dt of all of them
     double t[E], rinv[E], P[E], Pd[E];
@@ -611,12 +616,12 @@ IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&
   } else if (sane && (hmax < c.hxl || hmin > c.hxr)) {
     const bool right = hmin > c.hxr;
 #pragma unroll
-    for (int e = 0; e < E; ++e) ipa_grad_tail<Tab>(c, right, d[e], D[e], dd[e], ds[e], tab);
+    for (int e = 0; e < E; ++e) ipa_grad_tail<Tab>(c, right, d[e], D[e], dd[e], ds[e], db[e], tab);
   } else {
 #pragma unroll
     for (int e = 0; e < E; ++e) {
-      if (d[e] < c.d0) ipa_grad_tail<Tab>(c, false, d[e], D[e], dd[e], ds[e], tab);
-      else if (d[e] > c.d1) ipa_grad_tail<Tab>(c, true, d[e], D[e], dd[e], ds[e], tab);
+      if (d[e] < c.d0) ipa_grad_tail<Tab>(c, false, d[e], D[e], dd[e], ds[e], db[e], tab);
+      else if (d[e] > c.d1) ipa_grad_tail<Tab>(c, true, d[e], D[e], dd[e], ds[e], db[e], tab);
       else if (c.mode == 0) ipa_grad_core<Tab>(c, d[e], D[e], dd[e], ds[e]);
       else if (c.mode == 2) {   // Student-t core: log G = nu log q + beta d, L - beta = 2 nu d / q
         const double q = fma(d[e], d[e], c.delta2);
@@ -634,103 +639,162 @@ IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&
     }
   }
 #pragma unroll
-  for (int e = 0; e < E; ++e) ipa_grad_mix<Tab>(c, d[e], D[e], dd[e], ds[e], l[e], gm[e], gs[e], gf[e], gk[e], tab);
+  for (int e = 0; e < E; ++e)
+    ipa_grad_mix<Tab>(c, d[e], D[e], dd[e], ds[e], db[e], l[e], gm[e], gs[e], gf[e], gk[e], gb[e], tab);
 }
 
 #ifndef IPA_GB
 #define IPA_GB 512                        // threads per block of the gradient kernel
 #endif
-#ifndef IPA_GE
-#define IPA_GE 4                          // events per thread and tile
-#endif
-#ifndef IPA_GPSM
-#define IPA_GPSM 1                        // blocks per SM
-#endif
-static_assert(IPA_E == IPA_NE, "ipa_ev_off serves both tile shapes");
-static_assert(IPA_GB >= 160 && IPA_GB % 32 == 0, "the final reduction of the gradient kernel uses one warp per sum");
-// grid (G, K): every set streams the events on its own (the gradient call is made for one or a few sets);
-// per-thread register accumulators, fixed block tree, partials[(k 5 + c) G + b], the last block of each
-// set (ticket counter[k]) adds them in a fixed order.  out: nll[k], grad[4 k + (mu, sigma, f, k)].
-__global__ void __launch_bounds__(IPA_GB, IPA_GPSM)
-ipa_nll_grad_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaSetConsts* __restrict__ consts,
+#define IPA_GE 4                          // events per thread and tile (two Horner chains per event: value, derivative)
+#define IPA_GTILE (IPA_GB * IPA_GE)
+#define IPA_GKB 4                         // parameter sets per pass over the events
+#define IPA_GQ (IPA_NGRAD + 1)            // sums per set: l and the five derivative contributions
+static_assert(IPA_GB >= 32 * IPA_GQ && IPA_GB % 32 == 0, "the final reduction of the gradient kernel uses one warp per sum");
+// tile layout: the 32 x IPA_GE events of a warp are contiguous, a thread holds IPA_GE / 2 pairs 512 B apart
+__device__ __forceinline__ int ipa_gev_off(int tid, int e) {
+  return (tid >> 5) * (32 * IPA_GE) + 2 * ((e >> 1) * 32 + (tid & 31)) + (e & 1);
+}
+// Gradient kernel v2 (round 2): the streaming kernel's structure -- persistent grid (G, ceil(K / IPA_GKB)), events
+// staged global -> shared with 16-byte cp.async.cg two tiles deep, every thread copies and reads its own slots (no
+// barrier in the loop), up to IPA_GKB parameter sets evaluated per event read, per-thread accumulators
+// acc[set][sum][thread] in shared memory, fixed block tree, partials[((k IPA_GQ) + q) G + b], the last block of a set
+// group (ticket counter[blockIdx.y]) adds them in a fixed order.  out: nll[k], grad[IPA_NGRAD k + (mu, sigma, f, k, beta)].
+// ONE = true: a single parameter set (the usual gradient call): its six sums live in registers.
+template <bool ONE>
+__global__ void __launch_bounds__(IPA_GB, 1)
+ipa_nll_grad_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaSetConsts* __restrict__ consts, int K,
                     double* __restrict__ partials, unsigned int* counters, double* __restrict__ nll_out,
                     double* __restrict__ grad_out, int32_t* __restrict__ status_out) {
-  __shared__ IpaSetConsts c;
+  extern __shared__ __align__(16) unsigned char ipa_smem[];
+  double* stage = reinterpret_cast<double*>(ipa_smem);                         // [2][IPA_GTILE]
+  IpaSetConsts* sc = reinterpret_cast<IpaSetConsts*>(stage + 2 * IPA_GTILE);    // [IPA_GKB]
+  double* acc = reinterpret_cast<double*>(sc + IPA_GKB);                        // [IPA_GKB][IPA_GQ][IPA_GB]
   __shared__ __align__(16) double s_tab[IPA_MATHTAB_DOUBLES];
-  __shared__ double red[5][IPA_GB / 32];
+  __shared__ int s_st[IPA_GKB];
   __shared__ int s_last;
-  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, k = blockIdx.y, G = gridDim.x;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5, G = gridDim.x;
+  const int k0 = blockIdx.y * IPA_GKB, nk = (K - k0 < IPA_GKB) ? K - k0 : IPA_GKB;
+  const int nfull = vec_ok ? (int)(n / IPA_GTILE) : 0;
+  const unsigned slot = (unsigned)__cvta_generic_to_shared(stage) + (unsigned)(warp * (32 * IPA_GE * 8) + 16 * lane);
+  const double* src = x + (long long)blockIdx.x * IPA_GTILE + warp * (32 * IPA_GE) + 2 * lane;
+  const long long src_step = (long long)G * IPA_GTILE;
+  int tile = blockIdx.x;
+  if (tile < nfull) {
+#pragma unroll
+    for (int p = 0; p < IPA_GE / 2; ++p) ipa_cp_async16_s(slot + p * 512, src + p * 64);
+  }
+  ipa_cp_async_commit();
   {
-    const double* src = reinterpret_cast<const double*>(consts + k);
-    double* dst = reinterpret_cast<double*>(&c);
-    for (int i = tid; i < (int)(sizeof(IpaSetConsts) / 8); i += IPA_GB) dst[i] = src[i];
+    const int nd = nk * (int)(sizeof(IpaSetConsts) / 8);
+    const double* csrc = reinterpret_cast<const double*>(consts + k0);
+    double* dst = reinterpret_cast<double*>(sc);
+    for (int i = tid; i < nd; i += IPA_GB) dst[i] = csrc[i];
+    for (int i = 0; i < nk * IPA_GQ; ++i) acc[i * IPA_GB + tid] = 0.0;
     ipa_load_mathtab(s_tab);
   }
   __syncthreads();
-  const int st = c.status ? c.status : ((c.pure || !(c.fsig > 0.0)) ? 4 : 0);   // 4: the gradient needs 0 < f < 1
-  double acc[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-  if (!st) {
-    const long long tile_n = (long long)IPA_GB * IPA_GE, ntiles = (n + tile_n - 1) / tile_n;
-    const double xpad = (n > 0) ? x[n - 1] : 0.0;
-    auto load_tile = [&](long long tile, double (&xv)[IPA_GE]) {
-      const long long base = tile * tile_n;
-      if (vec_ok && base + tile_n <= n) {
-#pragma unroll
-        for (int p = 0; p < IPA_GE / 2; ++p) {
-          const double2 v = __ldcs(reinterpret_cast<const double2*>(x + base) + p * IPA_GB + tid);
-          xv[2 * p] = v.x;
-          xv[2 * p + 1] = v.y;
-        }
-      } else {
-#pragma unroll
-        for (int e = 0; e < IPA_GE; ++e) {
-          const long long i = base + 2LL * ((e >> 1) * IPA_GB + tid) + (e & 1);
-          xv[e] = (i < n) ? x[i] : xpad;
-        }
-      }
-    };
-    double xn[IPA_GE];
-    if ((long long)blockIdx.x < ntiles) load_tile(blockIdx.x, xn);
-    for (long long tile = blockIdx.x; tile < ntiles; tile += G) {
-      const long long base = tile * tile_n;
-      double xv[IPA_GE];
-#pragma unroll
-      for (int e = 0; e < IPA_GE; ++e) xv[e] = xn[e];
-      if (tile + G < ntiles) load_tile(tile + G, xn);        // next tile in flight while this one is evaluated
-      double l[IPA_GE], gm[IPA_GE], gs[IPA_GE], gf[IPA_GE], gk[IPA_GE];
-      ipa_eval_grad<IPA_GE>(c, xv, l, gm, gs, gf, gk, s_tab);
-#pragma unroll
-      for (int e = 0; e < IPA_GE; ++e) {
-        const long long i = base + 2LL * ((e >> 1) * IPA_GB + tid) + (e & 1);
-        if (i < n) { acc[0] += l[e]; acc[1] += gm[e]; acc[2] += gs[e]; acc[3] += gf[e]; acc[4] += gk[e]; }
-      }
-    }
-  }
-#pragma unroll
-  for (int q = 0; q < 5; ++q) {
-    const double v = ipa_warp_sum(acc[q]);
-    if (lane == 0) red[q][warp] = v;
+  if (tid < nk) {
+    const IpaSetConsts& c = sc[tid];
+    s_st[tid] = c.status ? c.status : ((c.pure || !(c.fsig > 0.0)) ? 4 : 0);   // 4: the gradient needs 0 < f < 1
   }
   __syncthreads();
-  if (tid < 5) {
+  double racc[IPA_GQ] = {0.0, 0.0, 0.0, 0.0, 0.0, 0.0};
+  auto tile_sets = [&](const double (&xv)[IPA_GE], long long base, bool full) {
+    for (int k = 0; k < (ONE ? 1 : nk); ++k) {
+      if (s_st[k]) continue;
+      double l[IPA_GE], gm[IPA_GE], gs[IPA_GE], gf[IPA_GE], gk[IPA_GE], gb[IPA_GE];
+      ipa_eval_grad<IPA_GE>(sc[k], xv, l, gm, gs, gf, gk, gb, s_tab);
+      if (!full) {
+#pragma unroll
+        for (int e = 0; e < IPA_GE; ++e)
+          if (base + ipa_gev_off(tid, e) >= n) { l[e] = 0.0; gm[e] = 0.0; gs[e] = 0.0; gf[e] = 0.0; gk[e] = 0.0; gb[e] = 0.0; }
+      }
+      if (ONE) {
+        racc[0] += (l[0] + l[1]) + (l[2] + l[3]);
+        racc[1] += (gm[0] + gm[1]) + (gm[2] + gm[3]);
+        racc[2] += (gs[0] + gs[1]) + (gs[2] + gs[3]);
+        racc[3] += (gf[0] + gf[1]) + (gf[2] + gf[3]);
+        racc[4] += (gk[0] + gk[1]) + (gk[2] + gk[3]);
+        racc[5] += (gb[0] + gb[1]) + (gb[2] + gb[3]);
+      } else {
+        double* a = acc + (k * IPA_GQ) * IPA_GB + tid;
+        a[0 * IPA_GB] += (l[0] + l[1]) + (l[2] + l[3]);
+        a[1 * IPA_GB] += (gm[0] + gm[1]) + (gm[2] + gm[3]);
+        a[2 * IPA_GB] += (gs[0] + gs[1]) + (gs[2] + gs[3]);
+        a[3 * IPA_GB] += (gf[0] + gf[1]) + (gf[2] + gf[3]);
+        a[4 * IPA_GB] += (gk[0] + gk[1]) + (gk[2] + gk[3]);
+        a[5 * IPA_GB] += (gb[0] + gb[1]) + (gb[2] + gb[3]);
+      }
+    }
+  };
+  unsigned bufoff = 0;
+  for (; tile < nfull; tile += G) {
+    double xv[IPA_GE];
+    ipa_cp_async_wait_all();
+#pragma unroll
+    for (int p = 0; p < IPA_GE / 2; ++p) {
+      const double2 v = ipa_lds128(slot + bufoff + p * 512);
+      xv[2 * p] = v.x;
+      xv[2 * p + 1] = v.y;
+    }
+    bufoff ^= IPA_GTILE * 8;
+    src += src_step;
+    if (tile + G < nfull) {
+#pragma unroll
+      for (int p = 0; p < IPA_GE / 2; ++p) ipa_cp_async16_s(slot + bufoff + p * 512, src + p * 64);
+    }
+    ipa_cp_async_commit();
+    tile_sets(xv, (long long)tile * IPA_GTILE, true);
+  }
+  ipa_cp_async_wait_all();
+  {
+    // remainder: ragged tiles with plain loads, continuing the round-robin over the blocks; empty slots repeat the last event
+    const long long rem0 = (long long)nfull * IPA_GTILE;
+    const long long nrem = (n - rem0 + IPA_GTILE - 1) / IPA_GTILE;
+    const int first = (int)((blockIdx.x + G - nfull % G) % G);
+    const double xpad = (n > 0) ? x[n - 1] : 0.0;
+    for (long long r = first; r < nrem; r += G) {
+      const long long base = rem0 + r * IPA_GTILE;
+      double xv[IPA_GE];
+#pragma unroll
+      for (int e = 0; e < IPA_GE; ++e) {
+        const long long i = base + ipa_gev_off(tid, e);
+        xv[e] = (i < n) ? x[i] : xpad;
+      }
+      tile_sets(xv, base, false);
+    }
+  }
+  if (ONE) {
+#pragma unroll
+    for (int q = 0; q < IPA_GQ; ++q) acc[q * IPA_GB + tid] = racc[q];      // same tree as the multi-set path from here on
+  }
+  __syncthreads();
+  // block tree: one warp per (set, sum)
+  for (int q = warp; q < nk * IPA_GQ; q += IPA_GB / 32) {
+    const double* a = acc + q * IPA_GB;
     double v = 0.0;
-    for (int w = 0; w < IPA_GB / 32; ++w) v += red[tid][w];
-    partials[((long long)k * 5 + tid) * G + blockIdx.x] = v;
+#pragma unroll
+    for (int w = 0; w < IPA_GB / 32; w += 4)
+      v += (a[lane + 32 * w] + a[lane + 32 * w + 32]) + (a[lane + 32 * w + 64] + a[lane + 32 * w + 96]);
+    v = ipa_warp_sum(v);
+    if (lane == 0) partials[((long long)k0 * IPA_GQ + q) * G + blockIdx.x] = v;
   }
   __threadfence();
   __syncthreads();
-  if (tid == 0) s_last = (atomicAdd(counters + k, 1u) == (unsigned)(G - 1));
+  if (tid == 0) s_last = (atomicAdd(counters + blockIdx.y, 1u) == (unsigned)(G - 1));
   __syncthreads();
   if (!s_last) return;
   __threadfence();
-  if (warp < 5) {
+  for (int q = warp; q < nk * IPA_GQ; q += IPA_GB / 32) {
     double v = 0.0;
-    for (int i = lane; i < G; i += 32) v += __ldcg(partials + ((long long)k * 5 + warp) * G + i);
+    for (int i = lane; i < G; i += 32) v += __ldcg(partials + ((long long)k0 * IPA_GQ + q) * G + i);
     v = ipa_warp_sum(v);
     if (lane == 0) {
-      const double r = st ? (warp == 0 ? INFINITY : NAN) : 0.0 - v;
-      if (warp == 0) { nll_out[k] = r; if (status_out) status_out[k] = st; }
-      else grad_out[4 * k + warp - 1] = r;
+      const int k = q / IPA_GQ, comp = q % IPA_GQ, st = s_st[k];
+      const double r = st ? (comp == 0 ? INFINITY : NAN) : 0.0 - v;
+      if (comp == 0) { nll_out[k0 + k] = r; if (status_out) status_out[k0 + k] = st; }
+      else grad_out[IPA_NGRAD * (k0 + k) + comp - 1] = r;
     }
   }
 }

@@ -48,6 +48,7 @@ struct alignas(16) IpaSetConsts {
   double invsig, mulo, L0, L1;                      // 1 / sigma, mu - lo, join slopes
   double A0, A1, aL0, a2L1;                         // nu/sigma - a beta, nu/sigma + a2 beta, a L0, a2 L1
   double c0s, c1s, invf, inv1mf;                    // (L0 - beta)/sigma, (L1 - beta)/sigma, 1/f, 1/(1-f)
+  double dlnNS_dbeta, pad2;                         // d ln N_S / d beta (fifth gradient component)
   int32_t status, degree, mode, pure;
   int32_t hxl, hxr, pad0, pad1; // high words of the joins in x, mu+d0 and mu+d1 (0 / -1 if not positive): region
                                 // classification of a whole warp by integer min/max of the events' high words
@@ -73,6 +74,8 @@ struct IpaProWork {
   double ctab[4 * IPA_MCHEB];   // cos(pi m / (2 M)), m = 0 .. 4M-1 (Chebyshev nodes and the cosine transform)
   double tl_left, tl_right, NB, logNB, logf, log1mf, nulogalpha, expref;
   double tl_left2, tl_right2, dlnNB_dk, Iedge_l, Iedge_h;   // sigma-derivative tail integrals, d ln N_B / d k, I at the range ends
+  double tl_left3, tl_right3;                               // beta-derivative tail integrals
+  double pval3[IPA_MAXPANEL * IPA_GL], psum3[IPA_MAXPANEL]; // core part of d N_S / d beta: G d
   double pval2[IPA_MAXPANEL * IPA_GL], psum2[IPA_MAXPANEL];   // pieces of phase 12 computed by other warps in phase 11
   int degree, mode;
   long long T[IPA_NCOEF * IPA_NCOEF];  // copy of the integer Chebyshev table (loaded at kernel start, used in phase 8)
@@ -392,20 +395,23 @@ IPA_HD void ipa_pro_phase10(IpaProWork& w, int tid, int nthr) {
     const double g = w.glw[i] * hl * exp(ipa_core_logG(w, d) - w.logref);
     w.pval[q] = g;
     w.pval2[q] = w.want_grad ? g * (ipa_sigpow(w) / w.p.sigma - (d / w.p.sigma) * ipa_core_Lmb(w, d)) : 0.0;   // G dlogG/dsigma
+    w.pval3[q] = w.want_grad ? g * d : 0.0;                                                                    // G dlogG/dbeta
   }
 }
 IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
   if (w.status) return;
   const ipa_params& p = w.p;
   if (tid < w.npanel) {
-    double s = 0.0, s2 = 0.0;
-    for (int i = 0; i < IPA_GL; ++i) { s += w.pval[tid * IPA_GL + i]; s2 += w.pval2[tid * IPA_GL + i]; }
+    double s = 0.0, s2 = 0.0, s3 = 0.0;
+    for (int i = 0; i < IPA_GL; ++i) { s += w.pval[tid * IPA_GL + i]; s2 += w.pval2[tid * IPA_GL + i]; s3 += w.pval3[tid * IPA_GL + i]; }
     w.psum[tid] = s;
     w.psum2[tid] = s2;
+    w.psum3[tid] = s3;
   } else if (tid == 32) {          // left tail: int I and int I dlogI/dsigma, in units of exp(logref)  (reading C5)
     // with u = 1 - (d-d0) L0/n:  dlogI/dsigma = A + [a L0 - c] / u + c,  A = nu/sigma - a beta,
     // c = n (L0 - beta) / (L0 sigma);  int u^-n du and int u^-(n+1) du are ipa_powint(u, n), ipa_powint(u, n+1)
-    double left = 0.0, left2 = 0.0;
+    // dlogI/dbeta = d0 + (d - d0)/u = (d0 - n/L0) + (n/L0)/u
+    double left = 0.0, left2 = 0.0, left3 = 0.0;
     if (w.dl < w.d0) {
       const double dr = fmin(w.d0, w.dh);
       const double ul = 1.0 - (w.dl - w.d0) * w.L0 / p.n, ur = 1.0 - (dr - w.d0) * w.L0 / p.n;
@@ -418,11 +424,13 @@ IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
       const double A = ipa_sigpow(w) / p.sigma - p.a * p.beta, c = p.n * (w.L0 - p.beta) / (w.L0 * p.sigma);
       left = pre * F;
       left2 = pre * ((A + c) * F + (p.a * w.L0 - c) * F1);
+      left3 = pre * ((w.d0 - p.n / w.L0) * F + (p.n / w.L0) * F1);
     }
     w.tl_left = left;
     w.tl_left2 = left2;
+    w.tl_left3 = left3;
   } else if (tid == 64) {          // right tail: dlogI/dsigma = A' + c' - (a2 L1 + c') / u,  c' = n2 (L1 - beta) / (L1 sigma)
-    double right = 0.0, right2 = 0.0;
+    double right = 0.0, right2 = 0.0, right3 = 0.0;   // dlogI/dbeta = (d1 - n2/L1) + (n2/L1)/u
     if (w.dh > w.d1) {
       const double dL = fmax(w.d1, w.dl);
       const double uh = 1.0 - (w.dh - w.d1) * w.L1 / p.n2, ul = 1.0 - (dL - w.d1) * w.L1 / p.n2;
@@ -434,9 +442,11 @@ IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
       const double A = ipa_sigpow(w) / p.sigma + p.a2 * p.beta, c = p.n2 * (w.L1 - p.beta) / (w.L1 * p.sigma);
       right = pre * F;
       right2 = pre * ((A + c) * F - (p.a2 * w.L1 + c) * F1);
+      right3 = pre * ((w.d1 - p.n2 / w.L1) * F + (p.n2 / w.L1) * F1);
     }
     w.tl_right = right;
     w.tl_right2 = right2;
+    w.tl_right3 = right3;
   } else if (tid == 96) {          // background normalisation (shifted by lo) and d ln N_B / d k
     const double wd = w.hi - w.lo, tk = p.k * wd;
     const double NB = (fabs(tk) < 1e-8) ? wd * (1.0 + 0.5 * tk + tk * tk / 6.0) : expm1(tk) / p.k;
@@ -500,6 +510,10 @@ IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
   for (int i = 0; i < w.npanel; ++i) core2 += w.psum2[i];
   o.dlnNS_dmu = (w.Iedge_l - w.Iedge_h) / NSr;
   o.dlnNS_dsig = (w.tl_left2 + core2 + w.tl_right2) / NSr;
+  double core3 = 0.0;
+  for (int i = 0; i < w.npanel; ++i) core3 += w.psum3[i];
+  o.dlnNS_dbeta = (w.tl_left3 + core3 + w.tl_right3) / NSr;
+  o.pad2 = 0.0;
   o.dlnNB_dk = pure ? 0.0 : w.dlnNB_dk;
   o.nuosig = ipa_sigpow(w) / p.sigma; o.invsig = 1.0 / p.sigma; o.mulo = p.mu - w.lo; o.L0 = w.L0; o.L1 = w.L1;
   o.A0 = o.nuosig - p.a * p.beta; o.A1 = o.nuosig + p.a2 * p.beta;

@@ -36,13 +36,13 @@ extern "C" {
 int emu_sizeof_consts() { return (int)sizeof(IpaSetConsts); }
 double emu_besselk_scaled(double nu, double x) { return ipa_besselk_scaled(nu, x); }
 // out: status, degree, mode, normS, normB, delta2, alpha, logG0, logG1, L0 (= -uA0 n0), L1, d ln N_S/d mu,
-// d ln N_S/d sigma, d ln N_B/d k
+// d ln N_S/d sigma, d ln N_B/d k, d ln N_S/d beta
 void emu_consts(const ipa_params* p, double lo, double hi, int policy, double* out) {
   IpaSetConsts c;
   run_prologue_host(*p, lo, hi, policy, &c);
   out[0] = c.status; out[1] = c.degree; out[2] = c.mode; out[3] = c.normS; out[4] = c.normB;
   out[5] = c.delta2; out[6] = c.alpha; out[7] = c.logG0; out[8] = c.logG1; out[9] = -c.uA0 * c.n0; out[10] = -c.uA1 * c.n1;
-  out[11] = c.dlnNS_dmu; out[12] = c.dlnNS_dsig; out[13] = c.dlnNB_dk;
+  out[11] = c.dlnNS_dmu; out[12] = c.dlnNS_dsig; out[13] = c.dlnNB_dk; out[14] = c.dlnNS_dbeta;
 }
 void emu_logpdf(const ipa_params* p, double lo, double hi, int policy, const double* x, long long n, double* out) {
   IpaSetConsts c;
@@ -55,16 +55,18 @@ void emu_logpdf(const ipa_params* p, double lo, double hi, int policy, const dou
     for (int e = 0; e < 8 && i + e < n; ++e) out[i + e] = l[e];
   }
 }
-// row f1: sums of l and of the four derivative contributions over n events (plain left-to-right sums)
+// row f1: sums of l and of the five derivative contributions over n events (plain left-to-right sums)
 void emu_grad(const ipa_params* p, double lo, double hi, int policy, const double* x, long long n, double* out) {
   IpaSetConsts c;
   run_prologue_host(*p, lo, hi, policy, &c);
-  for (int q = 0; q < 5; ++q) out[q] = 0.0;
+  for (int q = 0; q < 6; ++q) out[q] = 0.0;
   for (long long i = 0; i < n; i += 4) {
-    double xv[4], l[4], gm[4], gs[4], gf[4], gk[4];
+    double xv[4], l[4], gm[4], gs[4], gf[4], gk[4], gb[4];
     for (int e = 0; e < 4; ++e) xv[e] = (i + e < n) ? x[i + e] : x[n - 1];
-    ipa_eval_grad<4>(c, xv, l, gm, gs, gf, gk, ipa_h_mathtab);
-    for (int e = 0; e < 4 && i + e < n; ++e) { out[0] -= l[e]; out[1] -= gm[e]; out[2] -= gs[e]; out[3] -= gf[e]; out[4] -= gk[e]; }
+    ipa_eval_grad<4>(c, xv, l, gm, gs, gf, gk, gb, ipa_h_mathtab);
+    for (int e = 0; e < 4 && i + e < n; ++e) {
+      out[0] -= l[e]; out[1] -= gm[e]; out[2] -= gs[e]; out[3] -= gf[e]; out[4] -= gk[e]; out[5] -= gb[e];
+    }
   }
 }
 void emu_logI(const ipa_params* p, double lo, double hi, const double* d, long long n, double* out) {

@@ -126,7 +126,7 @@ def test_device_bessel_vs_mpmath(emu):
 def test_device_math_vs_oracle(emu, orc, shape, policy):
     P = {"P1": inp.GEN, "P2": inp.P2, "direct": dict(inp.GEN, zeta=0.2), "T1": inp.T1, "T2": inp.T2}[shape]
     p = inp.as_array(P)
-    out = np.zeros(14)
+    out = np.zeros(15)
     emu.emu_consts(p.ctypes.data, LO, HI, policy, out.ctypes.data)
     st, sc = orc.shape_consts(P)
     _, nm = orc.norm(P, LO, HI)
@@ -142,6 +142,7 @@ def test_device_math_vs_oracle(emu, orc, shape, policy):
     nd = orc.norm_derivs(P, LO, HI)
     assert abs(out[11] - nd[0]) <= 1e-12 * max(abs(nd[0]), 1e-3)
     assert abs(out[12] - nd[1]) <= 1e-11 * abs(nd[1]) and abs(out[13] - nd[2]) <= 1e-13 * abs(nd[2])
+    assert abs(out[14] - nd[3]) <= 1e-11 * max(abs(nd[3]), 1e-2)          # d ln N_S / d beta (fifth gradient component)
     n = 4000 if shape != "direct" else 400
     x = inp.standin_masses(1, n)
     x[:5] = [LO, HI, 5280.0, 5250.0, 5310.0]
@@ -197,11 +198,11 @@ def test_device_gradient_math_vs_oracle(emu, orc, shape):
     p = inp.as_array(P)
     n = 3000 if shape != "direct" else 300
     for x in (inp.standin_masses(11, n), np.sort(inp.standin_masses(12, n))):      # mixed and region-uniform groups
-        out = np.zeros(5)
+        out = np.zeros(6)
         emu.emu_grad(p.ctypes.data, LO, HI, 1, x.ctypes.data, x.size, out.ctypes.data)
         nll, g = orc.nll_gradient(x, P, LO, HI)
         assert abs(out[0] - nll) <= 1e-12 * abs(nll)
-        s = np.array([inp.GRAD_SCALE[k] for k in inp.FLOATED])
+        s = np.array([inp.GRAD_SCALE[k] for k in inp.GRAD_NAMES])
         assert np.all(np.abs(out[1:] - g) <= 1e-9 * np.maximum(np.abs(g), 1.0 / s)), (out[1:], g)
 
 
