@@ -345,10 +345,10 @@ def other_rows(torch, ipa, x, ws, stream, n, p_core):
         "hist_roofline": {"bound": "hbm", "achieved": 8.0 * n / dh / 1e9, "peak": peaks_hbm, "unit": "GB/s",
                           "frac": 8.0 * n / dh / 1e9 / peaks_hbm},
         "scan_points": int(ns.size), "scan_ms": dsc * 1e3, "scan_points_per_s": ns.size / dsc,
-        # per (point, bin) term: exp once (libdevice, ~25 FP64 instr), nu (2 FMA), log (libdevice, ~30 FP64 instr),
-        # n log nu and the sums (4) -> ~120 flops
-        "roofline_scan": alu_roofline(120.0, ns.size * nbins, dsc, {"flops_per_event": 120.0, "unit_of_work": "(scan point, bin) term",
-                                                                    "note": "includes the shape prologue + 3 small H2D copies of the call"}),
+        # per (point, bin) term: table-driven exp (16) and log (15) of csrc/ipa_fastmath.cuh, nu (2 FMA: 4), n log nu and the
+        # two sums (5) -> 40 flops; the call is four launches and three small uploads around a ~60 us kernel: latency-bound
+        "roofline_scan": alu_roofline(40.0, ns.size * nbins, dsc, {"unit_of_work": "(scan point, bin) term",
+                                                                   "note": "whole call: shape prologue + shape kernel + 3 small H2D copies + scan kernel"}),
         "poisson_toy_histograms": int(sd.size), "poisson_toys_ms": dp * 1e3, "poisson_draws_per_s": sd.size * nbins / dp}
     return out
 

@@ -1382,6 +1382,17 @@ ipa_binned_scan_kernel(const unsigned long long* __restrict__ counts, const doub
   const long long q = blockIdx.x;
   const double w = (hi - lo) / (double)nbins;
   const double k = kk[q], vs = ns[q], vb = nb[q];
+  // b_b = e^{k c_b} / sum: only ratios matter, so the exponent is shifted to be <= 0 (by hi - lo for k > 0) and goes through
+  // the table-driven e^{-|a|} of the streaming kernels (the 8 KB table is read through L1 here: 10 000 blocks of 4 terms per
+  // thread would spend more on copying it to shared memory than on using it); |k| (hi - lo) beyond its range: libdevice.
+  const double* mt = ipa_d_mathtab;
+  const double shift = (k > 0.0) ? (hi - lo) : 0.0;
+  const bool fast = fabs(k) * (hi - lo) < 4.0e6;
+  auto bexp = [&](int b) {
+    const double a = k * ((((double)b + 0.5) * w) - shift);
+    return fast ? ipa_fexp_negabs_t(a, mt) : exp(a);
+  };
+  auto flog = [&](double v) { return (v > 2.3e-308 && v < 1.7e308) ? ipa_flog_t(v, mt) : log(v); };
   // every exponential is evaluated once and kept in registers (up to 8 bins per thread: 2048 bins; beyond that the
   // second pass evaluates it again)
   constexpr int KEEP = 8;
@@ -1390,10 +1401,10 @@ ipa_binned_scan_kernel(const unsigned long long* __restrict__ counts, const doub
 #pragma unroll
   for (int i = 0; i < KEEP; ++i) {
     const int b = threadIdx.x + 256 * i;
-    eb[i] = (b < nbins) ? exp(k * (((double)b + 0.5) * w)) : 0.0;
+    eb[i] = (b < nbins) ? bexp(b) : 0.0;
     part += eb[i];
   }
-  for (int b = threadIdx.x + 256 * KEEP; b < nbins; b += 256) part += exp(k * (((double)b + 0.5) * w));
+  for (int b = threadIdx.x + 256 * KEEP; b < nbins; b += 256) part += bexp(b);
   const double bsum = ipa_block_sum_256(part, red);
   const double vbn = vb / bsum;
   double acc = 0.0;
@@ -1405,16 +1416,16 @@ ipa_binned_scan_kernel(const unsigned long long* __restrict__ counts, const doub
       if (nu_out) nu_out[b] = v;
       else {
         const unsigned long long nobs = counts[b];
-        acc += nobs ? v - (double)nobs * log(v) : v;
+        acc += nobs ? v - (double)nobs * flog(v) : v;
       }
     }
   }
   for (int b = threadIdx.x + 256 * KEEP; b < nbins; b += 256) {
-    const double v = fma(vs, s[b], vbn * exp(k * (((double)b + 0.5) * w)));
+    const double v = fma(vs, s[b], vbn * bexp(b));
     if (nu_out) nu_out[b] = v;
     else {
       const unsigned long long nobs = counts[b];
-      acc += nobs ? v - (double)nobs * log(v) : v;
+      acc += nobs ? v - (double)nobs * flog(v) : v;
     }
   }
   if (nu_out) return;
