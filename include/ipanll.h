@@ -93,7 +93,8 @@ const char* ipa_version(void);
  *   degree_policy  core-approximant degree (prologue): 0 = adaptive (default: the Chebyshev
  *                  series of log(z^nu K_nu(z)) is cut where its coefficients fall under the fp64 noise floor, so a
  *                  half-integer order collapses to a very short polynomial); 1 = geometric (at least the a-priori
- *                  degree for a general order on the same z-interval: no half-integer shortcut; reading D2).
+ *                  degree a general order needs on the same z-interval -- the degree at which the Chebyshev coefficients
+ *                  2 rho^-k / k of its log z term reach the noise threshold: no half-integer shortcut; reading D2).
  *   first_slot     ipa_toy_generate in mixture mode only (ignored elsewhere, must be >= 0): the call draws the events
  *                  of slots first_slot .. first_slot + capacity - 1 of the seeded dataset (an event depends on
  *                  (seed, slot) only), so G ranks can each generate their contiguous shard of ONE dataset

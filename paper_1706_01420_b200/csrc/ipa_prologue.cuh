@@ -311,10 +311,18 @@ IPA_HD void ipa_pro_phase7(IpaProWork& w, int tid) {
     const double thr = 2.5e-16 * scale;
     int D = IPA_MCHEB - 1;
     while (D > 1 && fabs(w.c[D]) <= thr) --D;
-    // a-priori degree for a general order on this interval: the nearest singularity of H is z = 0
+    // a-priori degree for a general order on this interval: the nearest singularity of H is z = 0, where a general
+    // order carries the term (nu - 1/2) log z.  The Chebyshev coefficients of log z on the interval are exactly
+    // -2 rho^-k / k (rho = t0 + sqrt(t0^2 - 1), t0 = centre / half-width): Dg = the first k where that falls under the
+    // noise threshold at unit weight.  (Round 1 used ceil(37 / ln rho), i.e. rho^-k <= 1e-16 without the 1/k and
+    // without the scale of H: 31 instead of 27 for the config interval; orders next to 1/2 need 23 by the noise floor.)
     const double t0 = w.zc / w.zh;
     const double rho = t0 + sqrt(t0 * t0 - 1.0);
-    int Dg = (int)ceil(37.0 / log(rho));
+    int Dg = 2;
+    {
+      const double lr = log(rho);
+      while (Dg < IPA_MCHEB && 2.0 * exp(-lr * (double)Dg) / (double)Dg > thr) ++Dg;
+    }
     if (w.policy == 1 && D < Dg) D = Dg;
     // conditioning of the power basis: needs rho comfortably above 1+sqrt(2)
     if (D > IPA_NCOEF - 1 || rho < 2.6) { w.mode = 1; D = 0; }

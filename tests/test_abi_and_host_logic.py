@@ -133,7 +133,7 @@ def test_device_math_vs_oracle(emu, orc, shape, policy):
     assert out[0] == 0 and st == 0
     assert out[2] == {"direct": 1, "T1": 2, "T2": 2}.get(shape, 0)      # mode 2: zeta = 0 Student-t core (row f4)
     if shape == "P1":
-        assert out[1] == (1 if policy == 0 else 31)   # K_{1/2}: H(z) is linear in z
+        assert out[1] == (1 if policy == 0 else 27)   # K_{1/2}: H(z) is linear in z; 27 = a-priori degree of a general order
     assert abs(out[3] / nm["NS"] - 1) <= 5e-14 and abs(out[4] / nm["NB"] - 1) <= 1e-15
     assert abs(np.sqrt(out[5]) / sc["delta"] - 1) <= 1e-14
     assert abs(out[6] / sc["alpha"] - 1) <= 1e-14 if sc["alpha"] else out[6] == 0.0
