@@ -625,6 +625,19 @@ def test_more_than_2_pow_31_events(ipa, torch_, orc):
         assert abs(got[i] - ref) <= 1e-10 * abs(ref)
     c = counts.cpu().numpy()
     assert int(c.sum()) == n and int(c[416]) == half and int(c[666]) == n - half   # bins of 5250 and 5400
+    # the layout preparation at the same size (64-bit output positions, 32-bit per-block counts): interleave the two
+    # values, prepare, and the result is the two runs again
+    del counts
+    x[0::2] = 5400.0
+    x[1::2] = 5250.0
+    n5400 = (n + 1) // 2
+    y = ipa.ipa_events_prepare(x, LO, HI)
+    torch_.cuda.synchronize()
+    assert bool((y[:n - n5400] == 5250.0).all().item()) and bool((y[n - n5400:] == 5400.0).all().item())
+    nll2, _, _ = ipa.ipa_nll_eval(y, sets, LO, HI)
+    l = orc.logpdf(np.array([5250.0, 5400.0]), sets[0], LO, HI)
+    ref = -((n - n5400) * l[0] + n5400 * l[1])
+    assert abs(nll2[0].item() - ref) <= 1e-10 * abs(ref)
 
 
 # ---------------------------------------------------------------------------------------------
