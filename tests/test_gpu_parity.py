@@ -955,3 +955,18 @@ def test_no_write_outside_the_outputs(ipa, torch_, x1):
         assert not (v == can8).any()
     assert np.array_equal(np.sort(xp.cpu().numpy().view(np.float64)), np.sort(x1[:n]))
     assert int(hist.cpu().numpy().view(np.uint64).sum()) == n
+
+
+def test_host_buffer_path_in_pieces(ipa, torch_, orc):
+    """nll_host (the e2e leg of bench.py): the events travel in pieces on a copy stream while the pieces already on the device
+    are evaluated; the sum of the pieces equals the single call up to rounding and the oracle within tolerance."""
+    n = 5_000_001
+    x = inp.standin_masses(23, n)
+    xh = torch_.from_numpy(x).pin_memory()
+    batch = [inp.GEN, inp.P2]
+    got = ipa.nll_host(xh, batch, LO, HI).numpy()
+    one = ipa.nll_host(xh, batch, LO, HI, chunks=1).numpy()
+    assert np.all(np.abs(got - one) <= 1e-12 * np.abs(one))
+    ref = orc.nll(x, batch, LO, HI, nthreads=8)
+    assert np.all(np.abs(got - ref) <= 1e-10 * np.abs(ref))
+    assert np.array_equal(got, ipa.nll_host(xh, batch, LO, HI).numpy())          # run to run
