@@ -28,7 +28,7 @@ __device__ const double ipa_d_mathtab[IPA_MATHTAB_DOUBLES] = IPA_MATHTAB_RAW;
 static const double ipa_h_mathtab[IPA_MATHTAB_DOUBLES] = IPA_MATHTAB_RAW;
 __constant__ double ipa_c_expq[4] = IPA_EXPQ_COEFS;
 static const double ipa_h_expq[4] = IPA_EXPQ_COEFS;
-__device__ const long long ipa_d_chebT[IPA_CHEB_NC * IPA_CHEB_NC] = IPA_CHEB_TABLE;   // global memory: per-lane index
+__device__ __align__(16) const long long ipa_d_chebT[IPA_CHEB_NC * IPA_CHEB_NC] = IPA_CHEB_TABLE;   // global memory (cp.async source)
 static const long long ipa_h_chebT[IPA_CHEB_NC * IPA_CHEB_NC] = IPA_CHEB_TABLE;
 __constant__ double ipa_c_gl16x[16] = IPA_GL16_X;
 __constant__ double ipa_c_gl16w[16] = IPA_GL16_W;

@@ -40,7 +40,7 @@ ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_param
   ipa_pro_phase5(w, tid); __syncthreads();
   ipa_pro_phase6(w, tid); __syncthreads();
   ipa_pro_phase7(w, tid); __syncthreads();
-  ipa_pro_phase7b(w, tid); __syncthreads();
+  ipa_pro_phase7b(w, tid); ipa_pro_table_ready(); __syncthreads();
   ipa_pro_phase8_finish(w, tid); __syncthreads();
   ipa_pro_phase9(w, tid); __syncthreads();
   ipa_pro_phase10(w, tid, IPA_PRO_THREADS); __syncthreads();
@@ -49,9 +49,9 @@ ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_param
   ipa_pro_phase12(w, o, tid); __syncthreads();
   ipa_pro_phase13(w, o, tid);
   if (tid == 0) {
-    if (norm_sig) norm_sig[set] = o.normS;
-    if (norm_bkg) norm_bkg[set] = o.normB;
-    if (status_out) status_out[set] = o.status;
+    if (norm_sig) norm_sig[set] = w.status ? NAN : w.normS_abs;
+    if (norm_bkg) norm_bkg[set] = w.status ? NAN : w.NB;
+    if (status_out) status_out[set] = w.status;
   }
 }
 

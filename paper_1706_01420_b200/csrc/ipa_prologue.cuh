@@ -78,7 +78,12 @@ struct IpaProWork {
   double pval3[IPA_MAXPANEL * IPA_GL], psum3[IPA_MAXPANEL]; // core part of d N_S / d beta: G d
   double pval2[IPA_MAXPANEL * IPA_GL], psum2[IPA_MAXPANEL];   // pieces of phase 12 computed by other warps in phase 11
   int degree, mode;
-  long long T[IPA_NCOEF * IPA_NCOEF];  // copy of the integer Chebyshev table (loaded at kernel start, used in phase 8)
+  alignas(16) long long T[IPA_NCOEF * IPA_NCOEF];  // copy of the integer Chebyshev table (cp.async at kernel start, used in phase 8)
+  double cDir;                          // per-set constant of the core term (phase 12 -> 13)
+  double normS_abs;                     // N_S (absolute) for the norm outputs (NaN for an invalid set)
+  double hK[2];                         // trapezoid steps of K_lambda(zeta), K_{lambda+1}(zeta) (phase 1 -> phase 2)
+  double hmax4[4];                      // max |H| over the four quarters of the Chebyshev nodes (phase 6 -> 7)
+  int dq4[4];                           // highest coefficient index above the noise threshold, per quarter (phase 7 -> 7b)
   double araw[IPA_NCOEF];
   double logG0, logG1, L0, L1;
   int npanel;
@@ -145,7 +150,22 @@ IPA_HD double ipa_logI(const IpaProWork& w, double d) {
 // loads are in flight during the first phases; per-lane reads from global memory in phase 8 cost as
 // much as building the table)
 IPA_HD void ipa_pro_load_table(IpaProWork& w, int tid, int nthr) {
+#ifdef __CUDA_ARCH__
+  // 16-byte asynchronous copies: nobody waits for the table before phase 8 (ipa_pro_table_ready)
+  for (int i = tid; i < IPA_NCOEF * IPA_NCOEF / 2; i += nthr) {
+    const unsigned dst = (unsigned)__cvta_generic_to_shared(&w.T[2 * i]);
+    asm volatile("cp.async.cg.shared.global [%0], [%1], 16;" ::"r"(dst), "l"(&ipa_d_chebT[2 * i]) : "memory");
+  }
+  asm volatile("cp.async.commit_group;" ::: "memory");
+#else
   for (int i = tid; i < IPA_NCOEF * IPA_NCOEF; i += nthr) w.T[i] = IPA_CHEBT(0, i);
+#endif
+}
+// before the barrier that precedes phase 8
+IPA_HD void ipa_pro_table_ready() {
+#ifdef __CUDA_ARCH__
+  asm volatile("cp.async.wait_group 0;" ::: "memory");
+#endif
 }
 
 // phase 0: validation (one thread)
@@ -182,6 +202,7 @@ IPA_HD void ipa_pro_phase1(IpaProWork& w, int tid) {
       prev = term;
     }
     w.part[which][lane] = s;
+    if (lane == 0) w.hK[which] = h;
   } else if (tid < 64 + IPA_GL) {
     w.glx[tid - 64] = IPA_GL16X(tid - 64);   // generated table (gen_fastmath_tables.py); IPA_GL == 16
     w.glw[tid - 64] = IPA_GL16W(tid - 64);
@@ -208,8 +229,8 @@ IPA_HD void ipa_pro_phase2(IpaProWork& w, int tid) {
   }
   double s0 = 0.5, s1 = 0.5;
   for (int l = 0; l < 32; ++l) { s0 += w.part[0][l]; s1 += w.part[1][l]; }
-  w.Kl = s0 * ipa_trap_step(fabs(p.lambda), p.zeta);
-  w.Kl1 = s1 * ipa_trap_step(fabs(p.lambda + 1.0), p.zeta);
+  w.Kl = s0 * w.hK[0];
+  w.Kl1 = s1 * w.hK[1];
   const double q = p.zeta * w.Kl / w.Kl1;       // (delta/sigma)^2
   w.delta = p.sigma * sqrt(q);
   w.alpha = p.zeta / w.delta;                   // = sqrt(zeta K_{l+1}/K_l)/sigma, alpha delta = zeta
@@ -281,7 +302,17 @@ IPA_HD void ipa_pro_phase5(IpaProWork& w, int tid) {
 
 // phase 6: Chebyshev coefficients c_j = (2/M) sum_i H_i cos(pi j (i+1/2)/M), c_0 halved
 IPA_HD void ipa_pro_phase6(IpaProWork& w, int tid) {
-  if (w.status || w.mode == 2 || tid >= IPA_MCHEB) return;
+  if (w.status || w.mode == 2) return;
+  if (tid >= IPA_MCHEB) {
+    // threads 64..67: max |H| over a quarter of the nodes each (the noise threshold of the degree selection)
+    if (tid < IPA_MCHEB + 4) {
+      const int q = tid - IPA_MCHEB;
+      double m = 0.0;
+      for (int i = 0; i < IPA_MCHEB / 4; ++i) m = fmax(m, fabs(w.H[q * (IPA_MCHEB / 4) + i]));
+      w.hmax4[q] = m;
+    }
+    return;
+  }
   const int M = IPA_MCHEB;
   double s = 0.0;
   for (int i = 0; i < M; ++i) {
@@ -291,7 +322,7 @@ IPA_HD void ipa_pro_phase6(IpaProWork& w, int tid) {
   w.c[tid] = s * (tid == 0 ? 1.0 : 2.0) / (double)M;
 }
 
-// phase 7: degree selection (thread 0) and the two joins (threads 32 and 64, other warps)
+// phase 7: degree selection (four threads, finished in phase 7b) and the two joins (threads 32 and 64, other warps)
 IPA_HD void ipa_pro_phase7(IpaProWork& w, int tid) {
   if (w.status) return;
   const ipa_params& p = w.p;
@@ -305,28 +336,14 @@ IPA_HD void ipa_pro_phase7(IpaProWork& w, int tid) {
     }
     return;
   }
-  if (tid == 0) {
-    double scale = 1.0;
-    for (int i = 0; i < IPA_MCHEB; ++i) scale = fmax(scale, fabs(w.H[i]));
-    const double thr = 2.5e-16 * scale;
-    int D = IPA_MCHEB - 1;
-    while (D > 1 && fabs(w.c[D]) <= thr) --D;
-    // a-priori degree for a general order on this interval: the nearest singularity of H is z = 0, where a general
-    // order carries the term (nu - 1/2) log z.  The Chebyshev coefficients of log z on the interval are exactly
-    // -2 rho^-k / k (rho = t0 + sqrt(t0^2 - 1), t0 = centre / half-width): Dg = the first k where that falls under the
-    // noise threshold at unit weight.  (Round 1 used ceil(37 / ln rho), i.e. rho^-k <= 1e-16 without the 1/k and
-    // without the scale of H: 31 instead of 27 for the config interval; orders next to 1/2 need 23 by the noise floor.)
-    const double t0 = w.zc / w.zh;
-    const double rho = t0 + sqrt(t0 * t0 - 1.0);
-    int Dg = 2;
-    {
-      const double lr = log(rho);
-      while (Dg < IPA_MCHEB && 2.0 * exp(-lr * (double)Dg) / (double)Dg > thr) ++Dg;
-    }
-    if (w.policy == 1 && D < Dg) D = Dg;
-    // conditioning of the power basis: needs rho comfortably above 1+sqrt(2)
-    if (D > IPA_NCOEF - 1 || rho < 2.6) { w.mode = 1; D = 0; }
-    w.degree = D;
+  if (tid == 0 || tid == 96 || tid == 128 || tid == 160) {
+    // four threads, a quarter of the coefficients each: highest index above the noise threshold (combined in phase 7b)
+    const int q = tid == 0 ? 0 : (tid - 64) / 32;
+    const double thr = 2.5e-16 * fmax(fmax(1.0, w.hmax4[0]), fmax(fmax(w.hmax4[1], w.hmax4[2]), w.hmax4[3]));
+    int best = -1;
+    for (int j = q * (IPA_MCHEB / 4); j < (q + 1) * (IPA_MCHEB / 4); ++j)
+      if (fabs(w.c[j]) > thr) best = j;
+    w.dq4[q] = best;
   } else if (tid == 32) {
     const double K0 = w.Ks[IPA_MCHEB], Km0 = w.Ks[IPA_MCHEB + 2];
     w.logG0 = w.nu * log(w.r0) + p.beta * w.d0 + log(K0) - w.z0;
@@ -340,6 +357,27 @@ IPA_HD void ipa_pro_phase7(IpaProWork& w, int tid) {
 // phase 7b: tail validity (after a barrier)
 IPA_HD void ipa_pro_phase7b(IpaProWork& w, int tid) {
   if (w.status || tid != 0) return;
+  if (w.mode != 2) {
+    // degree: the highest coefficient above the noise threshold, at least 1
+    int D = 1;
+    for (int q = 0; q < 4; ++q) D = w.dq4[q] > D ? w.dq4[q] : D;
+    const double thr = 2.5e-16 * fmax(fmax(1.0, w.hmax4[0]), fmax(fmax(w.hmax4[1], w.hmax4[2]), w.hmax4[3]));
+    // a-priori degree for a general order on this interval: the nearest singularity of H is z = 0, where a general
+    // order carries the term (nu - 1/2) log z.  The Chebyshev coefficients of log z on the interval are exactly
+    // -2 rho^-k / k (rho = t0 + sqrt(t0^2 - 1), t0 = centre / half-width): Dg = the first k where that falls under the
+    // noise threshold at unit weight.  (Round 1 used ceil(37 / ln rho), i.e. rho^-k <= 1e-16 without the 1/k and
+    // without the scale of H: 31 instead of 27 for the config interval; orders next to 1/2 need 23 by the noise floor.)
+    const double t0 = w.zc / w.zh;
+    const double rho = t0 + sqrt(t0 * t0 - 1.0);
+    const double rinv = 1.0 / rho;
+    int Dg = 2;
+    double pw = 2.0 * rinv * rinv;                            // 2 rho^-Dg
+    while (Dg < IPA_MCHEB && pw > thr * (double)Dg) { ++Dg; pw *= rinv; }
+    if (w.policy == 1 && D < Dg) D = Dg;
+    // conditioning of the power basis: needs rho comfortably above 1+sqrt(2)
+    if (D > IPA_NCOEF - 1 || rho < 2.6) { w.mode = 1; D = 0; }
+    w.degree = D;
+  }
   if (!(w.L0 > 0.0) || !(w.L1 < 0.0)) w.status = 2;
 }
 
@@ -365,12 +403,17 @@ IPA_HD void ipa_pro_phase8_finish(IpaProWork& w, int k) {
 
 // phase 9: range, panels, reference level (one thread)
 IPA_HD void ipa_pro_phase9(IpaProWork& w, int tid) {
-  if (w.status || tid != 0) return;
-  w.dl = w.lo - w.p.mu;
-  w.dh = w.hi - w.p.mu;
-  const double dref = fmin(fmax(0.0, w.dl), w.dh);
-  w.logref = ipa_logI(w, dref);
-  const double A = fmax(w.dl, w.d0), B = fmin(w.dh, w.d1);
+  if (w.status) return;
+  if (tid == 0) {                 // reference level of the normalisation
+    w.dl = w.lo - w.p.mu;
+    w.dh = w.hi - w.p.mu;
+    const double dref = fmin(fmax(0.0, w.dl), w.dh);
+    w.logref = ipa_logI(w, dref);
+    return;
+  }
+  if (tid != 32) return;          // panels of the core quadrature (another warp, at the same time)
+  const double dl = w.lo - w.p.mu, dh = w.hi - w.p.mu;
+  const double A = fmax(dl, w.d0), B = fmin(dh, w.d1);
   int np = 0;
   if (B > A) {
     for (int side = 0; side < 2; ++side) {
@@ -474,64 +517,78 @@ IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
   }
 }
 
-// phase 12: normalisations and folded constants (one thread writes the header of the record)
-IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
-  if (tid != 0) return;
-  o.status = w.status;
-  o.degree = w.degree;
-  o.mode = w.mode;
-  o.pure = 0;
-  o.normS = o.normB = NAN;
-  if (w.status) return;
+// phase 12: normalisations and folded constants.  Three threads of three warps write disjoint parts of the record at
+// the same time (one thread took 10 000 cycles, a fifth of the prologue: a chain of divisions, a logarithm and a read
+// back of a value it had just stored to global memory); each forms N_S from the same sums in the same order.
+struct IpaProNorm { double NSr, logNS, cS, kd, eB0; bool ok, pure; };
+IPA_HD IpaProNorm ipa_pro_norm(const IpaProWork& w) {
+  IpaProNorm r;
   const ipa_params& p = w.p;
   double core = 0.0;
   for (int i = 0; i < w.npanel; ++i) core += w.psum[i];
-  const double left = w.tl_left, right = w.tl_right;
-  const double NSr = left + core + right;  // in units of exp(logref)
-  const double NB = w.NB;
-  if (!(NSr > 0.0) || !ipa_finite(NSr) || !(NB > 0.0) || !ipa_finite(NB)) {
-    w.status = 3;
-    o.status = 3;
-    return;
-  }
-  o.normS = NSr * w.expref;
-  o.normB = NB;
-  const double logNS = log(NSr) + w.logref;
-  const bool pure = !(p.f < 1.0);
+  r.NSr = w.tl_left + core + w.tl_right;  // in units of exp(logref)
+  r.ok = (r.NSr > 0.0) && ipa_finite(r.NSr) && (w.NB > 0.0) && ipa_finite(w.NB);
+  r.logNS = log(r.NSr) + w.logref;
+  r.pure = !(p.f < 1.0);
   // f = 0: a finite, very negative signal term (softplus(-1e4) == 0 exactly) instead of -inf; it stays far inside the
   // range |Delta| < 5e6 of the kernels' exponential (ipa_fexp_negabs_t)
-  const double cS = (p.f > 0.0) ? w.logf - logNS : -1.0e4;
-  const double kd = pure ? 0.0 : p.k;
-  const double eB0 = pure ? 0.0 : (p.k * (p.mu - w.lo) + w.log1mf - w.logNB);
-  o.pure = pure ? 1 : 0;
-  o.mu = p.mu; o.d0 = w.d0; o.d1 = w.d1; o.delta2 = w.delta * w.delta;
-  o.tA = w.alpha / w.zh; o.tB = -w.zc / w.zh;
-  o.bmk = p.beta - kd; o.kd = kd; o.eB0 = eB0;
-  o.uA0 = -w.L0 / p.n;  o.uB0 = 1.0 + w.d0 * w.L0 / p.n;  o.n0 = p.n;  o.cT0 = w.logG0 + cS - eB0;
-  o.uA1 = -w.L1 / p.n2; o.uB1 = 1.0 + w.d1 * w.L1 / p.n2; o.n1 = p.n2; o.cT1 = w.logG1 + cS - eB0;
-  o.alpha = w.alpha; o.nu = w.nu;
-  o.cDir = cS - eB0 - w.nulogalpha;
-  o.fsig = p.f; o.kraw = p.k;
-  o.beta = p.beta; o.logG0 = w.logG0; o.logG1 = w.logG1; o.logNS = logNS; o.logref = w.logref;
-  o.araw0 = w.mode ? 0.0 : w.araw[0];   // modes 1, 2: no polynomial
-  double core2 = 0.0;
-  for (int i = 0; i < w.npanel; ++i) core2 += w.psum2[i];
-  o.dlnNS_dmu = (w.Iedge_l - w.Iedge_h) / NSr;
-  o.dlnNS_dsig = (w.tl_left2 + core2 + w.tl_right2) / NSr;
-  double core3 = 0.0;
-  for (int i = 0; i < w.npanel; ++i) core3 += w.psum3[i];
-  o.dlnNS_dbeta = (w.tl_left3 + core3 + w.tl_right3) / NSr;
-  o.pad2 = 0.0;
-  o.dlnNB_dk = pure ? 0.0 : w.dlnNB_dk;
-  o.nuosig = ipa_sigpow(w) / p.sigma; o.invsig = 1.0 / p.sigma; o.mulo = p.mu - w.lo; o.L0 = w.L0; o.L1 = w.L1;
-  o.A0 = o.nuosig - p.a * p.beta; o.A1 = o.nuosig + p.a2 * p.beta;
-  o.aL0 = p.a * w.L0; o.a2L1 = p.a2 * w.L1;
-  o.c0s = (w.L0 - p.beta) / p.sigma; o.c1s = (w.L1 - p.beta) / p.sigma;
-  o.invf = 1.0 / p.f; o.inv1mf = 1.0 / (1.0 - p.f);
-  const double xl = p.mu + w.d0, xr = p.mu + w.d1;
-  o.hxl = (xl > 0.0) ? ipa_hi(xl) : 0;
-  o.hxr = (xr > 0.0) ? ipa_hi(xr) : -1;
-  o.pad0 = o.pad1 = 0;
+  r.cS = (p.f > 0.0) ? w.logf - r.logNS : -1.0e4;
+  r.kd = r.pure ? 0.0 : p.k;
+  r.eB0 = r.pure ? 0.0 : (p.k * (p.mu - w.lo) + w.log1mf - w.logNB);
+  return r;
+}
+IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
+  if (tid != 0 && tid != 32 && tid != 64) return;
+  const ipa_params& p = w.p;
+  if (w.status) {
+    if (tid == 0) { o.status = w.status; o.degree = w.degree; o.mode = w.mode; o.pure = 0; o.normS = o.normB = NAN; }
+    return;
+  }
+  const IpaProNorm r = ipa_pro_norm(w);
+  if (!r.ok) {
+    // (threads 32 and 64 may see w.status before or after this store: they write nothing either way)
+    if (tid == 0) { w.status = 3; o.status = 3; o.degree = w.degree; o.mode = w.mode; o.pure = 0; o.normS = o.normB = NAN; }
+    return;
+  }
+  if (tid == 0) {
+    o.status = 0; o.degree = w.degree; o.mode = w.mode; o.pure = r.pure ? 1 : 0;
+    w.normS_abs = r.NSr * w.expref;
+    o.normS = w.normS_abs;
+    o.normB = w.NB;
+    o.mu = p.mu; o.d0 = w.d0; o.d1 = w.d1; o.delta2 = w.delta * w.delta;
+    const double izh = 1.0 / w.zh;
+    o.tA = w.alpha * izh; o.tB = -w.zc * izh;
+    o.bmk = p.beta - r.kd; o.kd = r.kd; o.eB0 = r.eB0;
+    o.alpha = w.alpha; o.nu = w.nu;
+    w.cDir = r.cS - r.eB0 - w.nulogalpha;
+    o.cDir = w.cDir;
+    o.fsig = p.f; o.kraw = p.k;
+    o.beta = p.beta; o.logG0 = w.logG0; o.logG1 = w.logG1; o.logNS = r.logNS; o.logref = w.logref;
+    o.araw0 = w.mode ? 0.0 : w.araw[0];   // modes 1, 2: no polynomial
+    const double xl = p.mu + w.d0, xr = p.mu + w.d1;
+    o.hxl = (xl > 0.0) ? ipa_hi(xl) : 0;
+    o.hxr = (xr > 0.0) ? ipa_hi(xr) : -1;
+    o.pad0 = o.pad1 = 0;
+  } else if (tid == 32) {
+    const double in0 = 1.0 / p.n, in1 = 1.0 / p.n2;
+    o.uA0 = -w.L0 * in0; o.uB0 = fma(w.d0 * w.L0, in0, 1.0); o.n0 = p.n;  o.cT0 = w.logG0 + r.cS - r.eB0;
+    o.uA1 = -w.L1 * in1; o.uB1 = fma(w.d1 * w.L1, in1, 1.0); o.n1 = p.n2; o.cT1 = w.logG1 + r.cS - r.eB0;
+  } else {
+    double core2 = 0.0, core3 = 0.0;
+    for (int i = 0; i < w.npanel; ++i) { core2 += w.psum2[i]; core3 += w.psum3[i]; }
+    const double iN = 1.0 / r.NSr, isg = 1.0 / p.sigma;
+    const double nuosig = ipa_sigpow(w) * isg;
+    o.dlnNS_dmu = (w.Iedge_l - w.Iedge_h) * iN;
+    o.dlnNS_dsig = (w.tl_left2 + core2 + w.tl_right2) * iN;
+    o.dlnNS_dbeta = (w.tl_left3 + core3 + w.tl_right3) * iN;
+    o.pad2 = 0.0;
+    o.dlnNB_dk = r.pure ? 0.0 : w.dlnNB_dk;
+    o.nuosig = nuosig; o.invsig = isg; o.mulo = p.mu - w.lo; o.L0 = w.L0; o.L1 = w.L1;
+    o.A0 = nuosig - p.a * p.beta; o.A1 = nuosig + p.a2 * p.beta;
+    o.aL0 = p.a * w.L0; o.a2L1 = p.a2 * w.L1;
+    o.c0s = (w.L0 - p.beta) * isg; o.c1s = (w.L1 - p.beta) * isg;
+    o.invf = 1.0 / p.f; o.inv1mf = 1.0 / (1.0 - p.f);
+  }
 }
 // phase 13: coefficients (threads 0..47), after phase 12
 IPA_HD void ipa_pro_phase13(IpaProWork& w, IpaSetConsts& o, int k) {
@@ -539,7 +596,7 @@ IPA_HD void ipa_pro_phase13(IpaProWork& w, IpaSetConsts& o, int k) {
   double v = 0.0;
   if (!w.status) {
     if (!w.mode) v = w.araw[k];
-    if (k == 0) v += o.cDir;  // cS - eB0 - nu log alpha: the per-set constant of the core term (both modes)
+    if (k == 0) v += w.cDir;  // cS - eB0 - nu log alpha: the per-set constant of the core term (both modes)
   }
   o.a[k] = v;
 }
