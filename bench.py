@@ -454,11 +454,29 @@ def main():
     norm_out = (torch.empty(1, dtype=torch.float64, device="cuda"), torch.empty(1, dtype=torch.float64, device="cuda"),
                 torch.empty(1, dtype=torch.int32, device="cuda"))
 
-    def step_pro():
-        ipa.ipa_norm(P1, LO, HI, ws=ws, stream=stream, out=norm_out, policy=POL)
-    for _ in range(3):
-        step_pro()
-    dt_pro = timed(torch, step_pro, args.steps, stream) / args.steps
+    def prologue_gpu_time(params, out, reps=20, replays=10):
+        """Device time of the prologue alone: `reps` launches captured in a CUDA graph and replayed, so that the Python /
+        ctypes cost of a launch (~20 us, as long as the kernel itself) does not leave the GPU idle between them."""
+        side = torch.cuda.Stream()
+        side.wait_stream(stream)
+        with torch.cuda.stream(side):
+            ipa.ipa_norm(params, LO, HI, ws=ws, stream=side, out=out, policy=POL)
+            side.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=side):
+                for _ in range(reps):
+                    ipa.ipa_norm(params, LO, HI, ws=ws, stream=torch.cuda.current_stream(), out=out, policy=POL)
+            g.replay()
+            side.synchronize()
+            e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            e0.record(side)
+            for _ in range(replays):
+                g.replay()
+            e1.record(side)
+            side.synchronize()
+        stream.wait_stream(side)
+        return e0.elapsed_time(e1) * 1e-3 / (reps * replays)
+    dt_pro = prologue_gpu_time(P1, norm_out)
     t_step = dt / args.steps
     degree = int(ipa.ipa_core_degree(P1, LO, HI, policy=POL))
     flops = algorithmic_flops(degree, p_core)
@@ -571,7 +589,8 @@ def main():
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": traffic, "traffic_source": traffic_note,
                 "kernel": "ipa_nll_kernel<false,false>", "kernel_ms": t_kernel * 1e3,
-                "kernel_time_source": "CUDA events: step time minus a prologue-only loop of the same length",
+                "kernel_time_source": "CUDA events: step time minus the prologue's device time (20 prologue launches captured "
+                                      "in a CUDA graph and replayed: no host gaps)",
                 "frac_whole_step": flops * n / t_local / 1e12 / peak,
                 "peak_source": "DESIGN.md section 6: 148 SM x 64 FP64 FMA lanes x 2 x 1.965 GHz (MEASURED_PEAKS.json has no "
                                "FP64 entry); measured DFMA-chain probe in fp64_dfma_probe_tflops",

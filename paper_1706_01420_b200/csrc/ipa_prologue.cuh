@@ -81,6 +81,7 @@ struct IpaProWork {
   alignas(16) long long T[IPA_NCOEF * IPA_NCOEF];  // copy of the integer Chebyshev table (cp.async at kernel start, used in phase 8)
   double cDir;                          // per-set constant of the core term (phase 12 -> 13)
   double normS_abs;                     // N_S (absolute) for the norm outputs (NaN for an invalid set)
+  double inv_sigma, inv_f, inv_1mf, inv_n0, inv_n1, inv_zh;   // reciprocals for phase 12, formed by idle threads in phase 11
   double hK[2];                         // trapezoid steps of K_lambda(zeta), K_{lambda+1}(zeta) (phase 1 -> phase 2)
   double hmax4[4];                      // max |H| over the four quarters of the Chebyshev nodes (phase 6 -> 7)
   int dq4[4];                           // highest coefficient index above the noise threshold, per quarter (phase 7 -> 7b)
@@ -250,7 +251,8 @@ IPA_HD void ipa_pro_phase2(IpaProWork& w, int tid) {
   // table length: smallest t with zmin (cosh t - 1) - om t > 46, by fixed-point iteration
   // (cosh t - 1 >= e^t / 2 - 1, so the root of  zmin (e^t/2 - 1) - om t = 46  is an upper bound)
   double t = 4.0;
-  for (int it = 0; it < 4; ++it) t = log(2.0 * (1.0 + (46.0 + om * t) / zmin));
+  const double izmin = 1.0 / zmin;
+  for (int it = 0; it < 3; ++it) t = log(2.0 * fma(fma(om, t, 46.0), izmin, 1.0));   // increasing, < 0.01 from the root after 3
   int J = (int)(t / w.h) + 2;
   if (J > IPA_JMAX) J = IPA_JMAX;
   w.J = J;
@@ -507,6 +509,15 @@ IPA_HD void ipa_pro_phase11(IpaProWork& w, int tid) {
   } else if (tid == 224) {         // I at the ends of the range (d N_S / d mu = I(lo - mu) - I(hi - mu))
     w.Iedge_l = w.want_grad ? exp(ipa_logI(w, w.dl) - w.logref) : 0.0;
     w.Iedge_h = w.want_grad ? exp(ipa_logI(w, w.dh) - w.logref) : 0.0;
+  } else if (tid == 200) {
+    w.inv_sigma = 1.0 / p.sigma;
+    w.inv_zh = 1.0 / w.zh;
+  } else if (tid == 208) {
+    w.inv_f = 1.0 / p.f;
+    w.inv_1mf = 1.0 / (1.0 - p.f);
+  } else if (tid == 216) {
+    w.inv_n0 = 1.0 / p.n;
+    w.inv_n1 = 1.0 / p.n2;
   } else if (tid == 128) {
     w.logf = (p.f > 0.0) ? log(p.f) : 0.0;
     w.log1mf = (p.f < 1.0) ? log1p(-p.f) : 0.0;
@@ -556,8 +567,7 @@ IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
     o.normS = w.normS_abs;
     o.normB = w.NB;
     o.mu = p.mu; o.d0 = w.d0; o.d1 = w.d1; o.delta2 = w.delta * w.delta;
-    const double izh = 1.0 / w.zh;
-    o.tA = w.alpha * izh; o.tB = -w.zc * izh;
+    o.tA = w.alpha * w.inv_zh; o.tB = -w.zc * w.inv_zh;
     o.bmk = p.beta - r.kd; o.kd = r.kd; o.eB0 = r.eB0;
     o.alpha = w.alpha; o.nu = w.nu;
     w.cDir = r.cS - r.eB0 - w.nulogalpha;
@@ -570,13 +580,13 @@ IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
     o.hxr = (xr > 0.0) ? ipa_hi(xr) : -1;
     o.pad0 = o.pad1 = 0;
   } else if (tid == 32) {
-    const double in0 = 1.0 / p.n, in1 = 1.0 / p.n2;
+    const double in0 = w.inv_n0, in1 = w.inv_n1;
     o.uA0 = -w.L0 * in0; o.uB0 = fma(w.d0 * w.L0, in0, 1.0); o.n0 = p.n;  o.cT0 = w.logG0 + r.cS - r.eB0;
     o.uA1 = -w.L1 * in1; o.uB1 = fma(w.d1 * w.L1, in1, 1.0); o.n1 = p.n2; o.cT1 = w.logG1 + r.cS - r.eB0;
   } else {
     double core2 = 0.0, core3 = 0.0;
     for (int i = 0; i < w.npanel; ++i) { core2 += w.psum2[i]; core3 += w.psum3[i]; }
-    const double iN = 1.0 / r.NSr, isg = 1.0 / p.sigma;
+    const double iN = 1.0 / r.NSr, isg = w.inv_sigma;
     const double nuosig = ipa_sigpow(w) * isg;
     o.dlnNS_dmu = (w.Iedge_l - w.Iedge_h) * iN;
     o.dlnNS_dsig = (w.tl_left2 + core2 + w.tl_right2) * iN;
@@ -587,7 +597,7 @@ IPA_HD void ipa_pro_phase12(IpaProWork& w, IpaSetConsts& o, int tid) {
     o.A0 = nuosig - p.a * p.beta; o.A1 = nuosig + p.a2 * p.beta;
     o.aL0 = p.a * w.L0; o.a2L1 = p.a2 * w.L1;
     o.c0s = (w.L0 - p.beta) * isg; o.c1s = (w.L1 - p.beta) * isg;
-    o.invf = 1.0 / p.f; o.inv1mf = 1.0 / (1.0 - p.f);
+    o.invf = w.inv_f; o.inv1mf = w.inv_1mf;
   }
 }
 // phase 13: coefficients (threads 0..47), after phase 12
