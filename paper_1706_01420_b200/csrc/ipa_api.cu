@@ -71,6 +71,7 @@ int device_info(int* sms) {
     IPA_CK(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev));
     const int smem = IPA_MAX_K * (int)(sizeof(IpaSetConsts) + IPA_NB * 8) + 2 * IPA_NTILE * 8;
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+    IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<true, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<true, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
@@ -204,6 +205,7 @@ int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K
   for (int k = 0; k < K; ++k) grouped = grouped || grp.leader[k] != k;
   auto kern = logpdf_dev ? (grouped ? ipa_nll_kernel<true, true> : ipa_nll_kernel<true, false>)
                          : (grouped ? ipa_nll_kernel<false, true> : ipa_nll_kernel<false, false>);
+  if (K == 1 && !logpdf_dev) kern = ipa_nll_kernel<false, false, true>;
   kern<<<(unsigned)G, IPA_NB, smem, st>>>(x_dev, n, vec_ok, consts, K, grp, partials, logpdf_dev, counter, nll_dev,
                                           status_dev);
   IPA_CK(cudaGetLastError());

@@ -333,6 +333,14 @@ struct IpaGroups { signed char leader[IPA_MAX_K]; };
 // group, one member stage per set; optional per-event output; accumulation into the thread's
 // shared-memory accumulators (first level of A5).
 // Event e of thread tid in the tile at `base` is x[base + ipa_ev_off(tid, e)].
+// sum of the IPA_NE values of a thread in a fixed order (first level of A5)
+__device__ __forceinline__ double ipa_tile_sum(const double (&l)[IPA_NE]) {
+  double sl = (l[0] + l[1]) + (l[2] + l[3]);
+#pragma unroll
+  for (int e = 4; e < IPA_NE; e += 4) sl += (l[e] + l[e + 1]) + (l[e + 2] + l[e + 3]);
+  return sl;
+}
+
 template <bool LOGPDF, bool FULL>
 __device__ __forceinline__ void ipa_tile_store_acc(int k, double (&l)[IPA_NE], double* acc, long long base, long long n,
                                                    int tid, double* __restrict__ logpdf) {
@@ -348,10 +356,7 @@ __device__ __forceinline__ void ipa_tile_store_acc(int k, double (&l)[IPA_NE], d
     for (int e = 0; e < IPA_NE; ++e)
       logpdf[(long long)k * n + base + ipa_ev_off(tid, e)] = l[e];
   }
-  double sl = 0.0;
-#pragma unroll
-  for (int e = 0; e < IPA_NE; e += 4) sl += (l[e] + l[e + 1]) + (l[e + 2] + l[e + 3]);
-  acc[k * IPA_NB + tid] += sl;
+  acc[k * IPA_NB + tid] += ipa_tile_sum(l);
 }
 
 // GROUPED = false: no two sets of the batch share a shape (K = 1, a scan over shapes): plain loop over the
@@ -407,7 +412,9 @@ __device__ __forceinline__ void ipa_tile_sets(const IpaSetConsts* sc, int K, con
 // thread copies and later reads its OWN 16-byte slots, so no block barrier is needed in the loop.
 // The staged loop covers the full tiles of a 16-byte aligned array with 32-bit tile counters and
 // shared addresses; the ragged last tile (or a misaligned array) takes plain loads afterwards.
-template <bool LOGPDF, bool GROUPED>
+// ONE = true (K == 1, no per-event output): the set's record sits at a fixed shared address and the thread's sum
+// stays in a register over the staged loop; same additions in the same order as the general loop.
+template <bool LOGPDF, bool GROUPED, bool ONE = false>
 __global__ void __launch_bounds__(IPA_NB, IPA_NB_PER_SM)
 ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaSetConsts* __restrict__ consts, int K,
                const __grid_constant__ IpaGroups grp, double* __restrict__ partials, double* __restrict__ logpdf, unsigned int* counter,
@@ -440,6 +447,8 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
   }
   __syncthreads();
   unsigned bufoff = 0;
+  double racc = 0.0;
+  const bool one_ok = ONE && !sc[0].status;
   for (; tile < nfull; tile += G) {
     double xv[IPA_NE];
     ipa_cp_async_wait_all();
@@ -457,7 +466,15 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
         ipa_cp_async16_s(slot + bufoff + p * 512, src + p * 64);
     }
     ipa_cp_async_commit();
-    ipa_tile_sets<LOGPDF, true, GROUPED>(sc, K, grp, acc, xv, (long long)tile * IPA_NTILE, n, tid, logpdf, s_tab);
+    if (ONE) {
+      if (one_ok) {
+        double l[IPA_NE];
+        ipa_eval_set<IPA_NE>(sc[0], xv, l, s_tab);
+        racc += ipa_tile_sum(l);
+      }
+    } else {
+      ipa_tile_sets<LOGPDF, true, GROUPED>(sc, K, grp, acc, xv, (long long)tile * IPA_NTILE, n, tid, logpdf, s_tab);
+    }
   }
   ipa_cp_async_wait_all();
   {
@@ -480,6 +497,7 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
       ipa_tile_sets<LOGPDF, false, GROUPED>(sc, K, grp, acc, xv, base, n, tid, logpdf, s_tab);
     }
   }
+  if (ONE) acc[tid] = racc + acc[tid];               // staged tiles first, then the remainder tile: the general order
   __syncthreads();
   for (int k = warp; k < K; k += IPA_NB / 32) {
     const double* a = acc + k * IPA_NB;
