@@ -60,6 +60,11 @@ Layout make_layout(int64_t K, int64_t nbins) {
   return L;
 }
 
+// Sets per launch of the streaming kernel: each set takes its record and IPA_NB accumulators in shared memory beside the
+// two staged tiles and the 9 KB of static tables.  A larger batch (up to IPA_MAX_K) runs as two launches over the events.
+constexpr int kStreamKMax = 28;
+static_assert(kStreamKMax * (sizeof(IpaSetConsts) + IPA_NB * 8) + 2 * IPA_NTILE * 8 + 9300 <= 227 * 1024,
+              "streaming kernel: shared memory of a full batch");
 struct DevInfo { int dev = -1; int sms = 0; bool attr_set = false; };
 thread_local DevInfo g_dev;
 
@@ -69,7 +74,7 @@ int device_info(int* sms) {
   if (g_dev.dev != dev || !g_dev.attr_set) {
     int n = 0;
     IPA_CK(cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev));
-    const int smem = IPA_MAX_K * (int)(sizeof(IpaSetConsts) + IPA_NB * 8) + 2 * IPA_NTILE * 8;
+    const int smem = kStreamKMax * (int)(sizeof(IpaSetConsts) + IPA_NB * 8) + 2 * IPA_NTILE * 8;
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false, false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
     IPA_CK(cudaFuncSetAttribute(ipa_nll_kernel<false, true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
@@ -187,28 +192,36 @@ int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K
   if (G > kGridMax) G = kGridMax;
   if (G > ntiles) G = ntiles;
   if (G < 1) G = 1;
-  const size_t smem = (size_t)K * (sizeof(IpaSetConsts) + IPA_NB * 8) + 2 * IPA_NTILE * 8;
   const int vec_ok = ((uintptr_t)x_dev % 16) == 0;
   const IpaSetConsts* consts = reinterpret_cast<const IpaSetConsts*>(ws + L.consts);
   double* partials = reinterpret_cast<double*>(ws + L.partials);
   unsigned int* counter = reinterpret_cast<unsigned int*>(ws + L.counter);
-  // sets with bitwise equal signal-shape parameters (the first 9 doubles) share the shape stage
-  IpaGroups grp;
-  for (int k = 0; k < IPA_MAX_K; ++k) grp.leader[k] = (signed char)k;
-  for (int k = 1; k < K; ++k)
-    for (int j = 0; j < k; ++j)
-      if (grp.leader[j] == j && std::memcmp(&p_host[k], &p_host[j], 9 * sizeof(double)) == 0) {
-        grp.leader[k] = (signed char)j;
-        break;
-      }
-  bool grouped = false;
-  for (int k = 0; k < K; ++k) grouped = grouped || grp.leader[k] != k;
-  auto kern = logpdf_dev ? (grouped ? ipa_nll_kernel<true, true> : ipa_nll_kernel<true, false>)
-                         : (grouped ? ipa_nll_kernel<false, true> : ipa_nll_kernel<false, false>);
-  if (K == 1 && !logpdf_dev) kern = ipa_nll_kernel<false, false, true>;
-  kern<<<(unsigned)G, IPA_NB, smem, st>>>(x_dev, n, vec_ok, consts, K, grp, partials, logpdf_dev, counter, nll_dev,
-                                          status_dev);
-  IPA_CK(cudaGetLastError());
+  // K <= kStreamKMax: one launch; above: two launches of half the batch each (own counter, own rows of the outputs)
+  const int nlaunch = (K + kStreamKMax - 1) / kStreamKMax;
+  const int kper = (K + nlaunch - 1) / nlaunch;
+  for (int b = 0; b < nlaunch; ++b) {
+    const int k0 = b * kper, kb = (K - k0 < kper) ? K - k0 : kper;
+    const ipa_params* ph = p_host + k0;
+    // sets with bitwise equal signal-shape parameters (the first 9 doubles) share the shape stage
+    IpaGroups grp;
+    for (int k = 0; k < IPA_MAX_K; ++k) grp.leader[k] = (signed char)k;
+    for (int k = 1; k < kb; ++k)
+      for (int j = 0; j < k; ++j)
+        if (grp.leader[j] == j && std::memcmp(&ph[k], &ph[j], 9 * sizeof(double)) == 0) {
+          grp.leader[k] = (signed char)j;
+          break;
+        }
+    bool grouped = false;
+    for (int k = 0; k < kb; ++k) grouped = grouped || grp.leader[k] != k;
+    auto kern = logpdf_dev ? (grouped ? ipa_nll_kernel<true, true> : ipa_nll_kernel<true, false>)
+                           : (grouped ? ipa_nll_kernel<false, true> : ipa_nll_kernel<false, false>);
+    if (kb == 1 && !logpdf_dev) kern = ipa_nll_kernel<false, false, true>;
+    const size_t smem = (size_t)kb * (sizeof(IpaSetConsts) + IPA_NB * 8) + 2 * IPA_NTILE * 8;
+    kern<<<(unsigned)G, IPA_NB, smem, st>>>(x_dev, n, vec_ok, consts + k0, kb, grp, partials + (size_t)k0 * G,
+                                            logpdf_dev ? logpdf_dev + (size_t)k0 * n : nullptr, counter + b, nll_dev + k0,
+                                            status_dev ? status_dev + k0 : nullptr);
+    IPA_CK(cudaGetLastError());
+  }
   return IPA_OK;
 }
 

@@ -28,7 +28,7 @@ ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_param
   if (tid == 0) {
     w.p = p_dev ? p_dev[set] : batch.p[set];
     w.lo = lo; w.hi = hi; w.policy = policy & 1; w.want_grad = (policy >> 1) & 1;
-    if (set == 0 && counter) *counter = 0u;
+    if (set == 0 && counter) counter[0] = counter[1] = 0u;   // one ticket counter per launch that follows (at most two)
   }
   __syncthreads();
   ipa_pro_load_table(w, tid, IPA_PRO_THREADS);
@@ -41,12 +41,12 @@ ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_param
   ipa_pro_phase6(w, tid); __syncthreads();
   ipa_pro_phase7(w, tid); __syncthreads();
   ipa_pro_phase7b(w, tid); ipa_pro_table_ready(); __syncthreads();
-  ipa_pro_phase8_finish(w, tid); __syncthreads();
-  ipa_pro_phase9(w, tid); __syncthreads();
+  ipa_pro_phase8_finish(w, tid); ipa_pro_cells_nodes(w, tid); __syncthreads();
+  ipa_pro_phase9(w, tid); ipa_pro_cells_dct(w, tid); __syncthreads();
   ipa_pro_phase10(w, tid, IPA_PRO_THREADS); __syncthreads();
-  ipa_pro_phase11(w, tid); __syncthreads();
+  ipa_pro_phase11(w, tid); ipa_pro_cells_monomial(w, ipa_pro_cells_slot(tid)); __syncthreads();
   IpaSetConsts& o = consts[set];
-  ipa_pro_phase12(w, o, tid); __syncthreads();
+  ipa_pro_phase12(w, o, tid); ipa_pro_cells_record(w, o, tid); __syncthreads();
   ipa_pro_phase13(w, o, tid);
   if (tid == 0) {
     if (norm_sig) norm_sig[set] = w.status ? NAN : w.normS_abs;
@@ -105,19 +105,49 @@ IPA_HD int ipa_warp_max(int v) {
 #define IPA_REG_RIGHT 2
 #define IPA_REG_MIXED 3
 
+// Cell of a warp whose events have high words in [hmin, hmax] (both warp-uniform): 0 .. IPA_NCELL-1 if no cell
+// boundary lies in (hmin, hmax], -1 otherwise.  Lanes 0..7 compare one entry of hb[] each (the last two are INT_MAX).
+IPA_HD int ipa_warp_cell(const IpaSetConsts& c, int hmin, int hmax) {
+#ifdef __CUDA_ARCH__
+  const int hb = c.hb[threadIdx.x & 7];
+  const unsigned below = __ballot_sync(IPA_FULL, hb <= hmin) & 0xffu;
+  const unsigned inside = __ballot_sync(IPA_FULL, hb > hmin && hb <= hmax) & 0xffu;
+  if (inside) return -1;
+  const int cell = __popc(below) - (IPA_NCELL - 1);
+#else
+  int cell = -(IPA_NCELL - 1);
+  for (int i = 0; i < 8; ++i) {
+    if (c.hb[i] > hmin && c.hb[i] <= hmax) return -1;
+    cell += (c.hb[i] <= hmin) ? 1 : 0;
+  }
+#endif
+  return cell < 0 ? -cell : cell;
+}
+
 // Core shape value of E events: t = tA sqrt(d^2 + delta^2) + tB, Horner over groups of 4 coefficients
 // (two 128-bit uniform shared loads per group; a[] is zero above the degree) down to a[1], times t.
-// FP64 per event: q 1 + sqrt 5 + t 1 + 4 ceil((D+1)/4).
+// FP64 per event: q 1 + sqrt 5 + t 1 + 4 ceil((D+1)/4).  cell >= 0: the warp lies in one cell of the core and runs
+// that cell's polynomial (same form, its own t, lower degree, constant term sa[cell][0] = H - araw0 at t = 0).
 template <int E, class Tab>
-IPA_HD void ipa_core_shape(const IpaSetConsts& c, const double (&d)[E], double (&V)[E], const Tab* tab) {
+IPA_HD void ipa_core_shape(const IpaSetConsts& c, const double (&d)[E], double (&V)[E], const Tab* tab, int cell = -1) {
   if (c.mode == 0) {
-    const double d2 = c.delta2, tA = c.tA, tB = c.tB;
+    const double d2 = c.delta2;
+    const double* a = c.a;
+    double tA = c.tA, tB = c.tB, v0 = 0.0;
+    int ng = c.degree >> 2;
+    if (cell >= 0) {
+      a = c.sa[cell];
+      tA = c.stA[cell];
+      tB = c.stB[cell];
+      ng = c.sng[cell];
+      v0 = a[0];
+    }
     double t[E], P[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) { t[e] = fma(tA, ipa_fsqrt(fma(d[e], d[e], d2)), tB); P[e] = 0.0; }
-    for (int g = c.degree >> 2; g >= 1; --g) {
-      const double2 hi2 = *reinterpret_cast<const double2*>(c.a + 4 * g + 2);
-      const double2 lo2 = *reinterpret_cast<const double2*>(c.a + 4 * g);
+    for (int g = ng; g >= 1; --g) {
+      const double2 hi2 = *reinterpret_cast<const double2*>(a + 4 * g + 2);
+      const double2 lo2 = *reinterpret_cast<const double2*>(a + 4 * g);
 #pragma unroll
       for (int e = 0; e < E; ++e) {
         P[e] = fma(P[e], t[e], hi2.y);
@@ -126,14 +156,14 @@ IPA_HD void ipa_core_shape(const IpaSetConsts& c, const double (&d)[E], double (
         P[e] = fma(P[e], t[e], lo2.x);
       }
     }
-    const double2 hi2 = *reinterpret_cast<const double2*>(c.a + 2);
-    const double a1 = c.a[1];
+    const double2 hi2 = *reinterpret_cast<const double2*>(a + 2);
+    const double a1 = a[1];
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       P[e] = fma(P[e], t[e], hi2.y);
       P[e] = fma(P[e], t[e], hi2.x);
       P[e] = fma(P[e], t[e], a1);
-      V[e] = P[e] * t[e];
+      V[e] = fma(P[e], t[e], v0);
     }
   } else if (c.mode == 2) {
     // Student-t core (zeta == 0, row f4): V = nu log(d^2 + delta^2), one logarithm, no polynomial
@@ -193,7 +223,7 @@ IPA_HD int ipa_shape_stage(const IpaSetConsts& c, const double (&x)[E], double (
   for (int e = 0; e < E; ++e) d[e] = x[e] - mu;
   const bool sane = hmin > 0 && hmax < 0x7ff00000;      // positive, finite events only
   if (sane && hmin > c.hxl && hmax < c.hxr) {
-    ipa_core_shape<E>(c, d, V, tab);
+    ipa_core_shape<E>(c, d, V, tab, c.ncell ? ipa_warp_cell(c, hmin, hmax) : -1);
     return IPA_REG_CORE;
   }
   if (sane && hmax < c.hxl) { ipa_tail_shape<E>(c, false, d, V, tab); return IPA_REG_LEFT; }
@@ -259,7 +289,7 @@ IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l
   for (int e = 0; e < E; ++e) d[e] = x[e] - mu;
   const bool sane = hmin > 0 && hmax < 0x7ff00000;
   if (sane && hmin > c.hxl && hmax < c.hxr) {
-    ipa_core_shape<E>(c, d, V, tab);
+    ipa_core_shape<E>(c, d, V, tab, c.ncell ? ipa_warp_cell(c, hmin, hmax) : -1);
     ipa_member_stage_r<E, IPA_REG_CORE>(c, d, V, l, tab);
   } else if (sane && hmax < c.hxl) {
     ipa_tail_shape<E>(c, false, d, V, tab);

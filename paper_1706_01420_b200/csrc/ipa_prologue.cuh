@@ -26,6 +26,12 @@
 #define IPA_PRO_THREADS 256
 #define IPA_SUB 2               // threads sharing one table-based Bessel evaluation
 #define IPA_NBTASK (IPA_MCHEB + 4)  // Chebyshev nodes + K_nu(z0), K_nu(z1), K_{nu-1}(z0), K_{nu-1}(z1)
+#define IPA_HD_NOINLINE IPA_HD   // the cell phases (inline: out of line they cost more, measured)
+#define IPA_NCELL 4              // (the geometry takes a fourth root: static_assert below)
+// cells of the core in r = sqrt(d^2 + delta^2), each with its own low-degree polynomial
+#define IPA_CELLN 16             // coefficients per cell polynomial (degree <= 15)
+#define IPA_CELLM 32             // Chebyshev nodes per cell
+#define IPA_CELL_MIN_DEGREE 16   // cells only where the full polynomial is longer than a cell polynomial can be
 
 // What the streaming kernels read, per parameter set (all fp64 except the flags).
 struct alignas(16) IpaSetConsts {
@@ -52,6 +58,20 @@ struct alignas(16) IpaSetConsts {
   int32_t status, degree, mode, pure;
   int32_t hxl, hxr, pad0, pad1; // high words of the joins in x, mu+d0 and mu+d1 (0 / -1 if not positive): region
                                 // classification of a whole warp by integer min/max of the events' high words
+  // Cells of the core (streaming and segmented kernels).  The core interval of r = sqrt(d^2 + delta^2) is cut into
+  // IPA_NCELL cells of equal ratio; cell s has its own polynomial in t_s = stA[s] r + stB[s], refitted from the
+  // full one: H(alpha r) - araw0 = sa[s][0] + sum_{j>=1} sa[s][j] t_s^j, of degree 4 sng[s] + 3 at most (14 where the full
+  // interval needs 27).  A warp whose events all lie in one cell (a warp of a prepared array nearly always does)
+  // runs the cell polynomial; any other warp runs the full one.  The cell of an event is decided on the high word
+  // of x alone: hb[] holds the high words of the 2 (IPA_NCELL - 1) cell boundaries in x, ascending (0 / INT_MAX for a
+  // boundary outside the core), each boundary a double with a zero low word, so that x >= boundary is exactly
+  // hi(x) >= hb; cell = | #{i : hb[i] <= hi(x)} - (IPA_NCELL - 1) |.  ncell = 0: no cells (modes 1 and 2, a cell
+  // degree above 15, a core too narrow for the 2^-20 relative resolution of the high word).
+  double sa[IPA_NCELL][IPA_CELLN];
+  double stA[IPA_NCELL], stB[IPA_NCELL];
+  int32_t hb[8];
+  int32_t sng[IPA_NCELL];
+  int32_t ncell, sdeg[3];       // sdeg: unused padding (the degrees are 4 sng + 3 at most; ipa_core_cells reports them)
 };
 
 struct IpaProWork {
@@ -90,6 +110,13 @@ struct IpaProWork {
   int npanel;
   double pa[IPA_MAXPANEL], pb[IPA_MAXPANEL], pval[IPA_MAXPANEL * IPA_GL], psum[IPA_MAXPANEL];
   double logref, dl, dh;
+  // cells of the core (phase 7 geometry, 8 values at the nodes, 9 Chebyshev coefficients, 11 monomials)
+  int ncell;
+  int chb[8];
+  double crc[IPA_NCELL], crh[IPA_NCELL];
+  double cH[IPA_NCELL][IPA_CELLM], cc[IPA_NCELL][IPA_CELLM];
+  double csa[IPA_NCELL][IPA_CELLN];
+  int cdeg[IPA_NCELL];
 };
 
 IPA_HD bool ipa_finite(double v) { return fabs(v) <= 1.7976931348623157e308; }
@@ -280,8 +307,10 @@ IPA_HD double ipa_pro_task_z(const IpaProWork& w, int q) {
   return ((q - IPA_MCHEB) & 1) ? w.z1 : w.z0;
 }
 
+IPA_HD_NOINLINE void ipa_pro_cells_geometry(IpaProWork& w);
 // phase 4: Bessel tasks, IPA_SUB threads each
 IPA_HD void ipa_pro_phase4(IpaProWork& w, int tid) {
+  if (tid == 192) { ipa_pro_cells_geometry(w); return; }   // needs phase 2 only; this thread has no Bessel task
   if (w.status || w.mode == 2) return;
   const int q = tid / IPA_SUB, sub = tid % IPA_SUB;
   if (q >= IPA_NBTASK) return;
@@ -381,6 +410,165 @@ IPA_HD void ipa_pro_phase7b(IpaProWork& w, int tid) {
     w.degree = D;
   }
   if (!(w.L0 > 0.0) || !(w.L1 < 0.0)) w.status = 2;
+}
+
+// ---- cells of the core: low-degree polynomials refitted from the full one (no further Bessel evaluation) ----------
+static_assert(IPA_NCELL == 4, "ipa_pro_cells_geometry: ratio of the cell radii is a fourth root");
+// phase 7, one thread: cell boundaries.  Equal ratio in r between delta and the larger join radius gives the nominal
+// boundaries in |d|; in x they are moved to the nearest edge of the IPA_PREPARE_BINS coarse bins of [lo, hi] (the layout
+// of ipa_events_prepare: inside a bin the events are not ordered, so a boundary inside a bin would leave every warp of
+// that bin in two cells) and truncated to a zero low word (the kernels compare high words), which moves them by less
+// than one unit `quant` of the high word: every cell is fitted on its own |d| interval widened by 2 quant on both sides.
+IPA_HD_NOINLINE void ipa_pro_cells_geometry(IpaProWork& w) {
+  w.ncell = 0;
+  for (int i = 0; i < 8; ++i) w.chb[i] = 0x7fffffff;
+  if (w.status || w.mode) return;
+  const ipa_params& p = w.p;
+  const double xl = p.mu + w.d0, xr = p.mu + w.d1;
+  if (!(xl > 0.0) || !ipa_finite(xr)) return;
+  const int ex = ipa_hi(xr) & 0x7ff00000;
+  if (ex < (64 << 20)) return;
+  const double quant = ipa_mk(ex - (20 << 20), 0);
+  const double margin = 2.0 * quant;
+  const double rmax = fmax(w.r0, w.r1), dl2 = w.delta * w.delta;
+  const double qr = sqrt(sqrt(rmax / w.delta));                 // ratio of consecutive cell radii (IPA_NCELL == 4)
+  const double bw = (w.hi - w.lo) / (double)IPA_PREPARE_BINS, ibw = (double)IPA_PREPARE_BINS / (w.hi - w.lo);
+  // boundaries in |d| on the left (L) and on the right (R) of mu; the join where a cell boundary falls outside the core
+  double rhoL[IPA_NCELL + 1], rhoR[IPA_NCELL + 1];
+  rhoL[0] = rhoR[0] = 0.0;
+  rhoL[IPA_NCELL] = -w.d0;
+  rhoR[IPA_NCELL] = w.d1;
+  double wmin = 1.7976931348623157e308, prev = 0.0, rs = w.delta;
+  for (int s = 1; s < IPA_NCELL; ++s) {
+    rs *= qr;
+    const double rho = ipa_fsqrt((rs - w.delta) * (rs + w.delta));
+    rhoL[s] = rhoR[s] = rho;
+    wmin = fmin(wmin, rho - prev);
+    prev = rho;
+  }
+  const bool snap = bw < 0.5 * wmin;
+  for (int s = 1; s < IPA_NCELL; ++s) {
+    double XL = p.mu - rhoL[s], XR = p.mu + rhoR[s];
+    if (snap) {
+      XL = fma(rint((XL - w.lo) * ibw), bw, w.lo);
+      XR = fma(rint((XR - w.lo) * ibw), bw, w.lo);
+    }
+    const bool hasL = XL > xl, hasR = XR < xr;
+    w.chb[IPA_NCELL - 1 - s] = hasL ? ipa_hi(XL) : 0;
+    w.chb[IPA_NCELL - 2 + s] = hasR ? ipa_hi(XR) : 0x7fffffff;
+    rhoL[s] = hasL ? p.mu - XL : -w.d0;
+    rhoR[s] = hasR ? XR - p.mu : w.d1;
+  }
+  bool ok = true;
+  for (int s = 0; s < IPA_NCELL; ++s) {
+    // |d| interval of the cell: its part on the left and its part on the right, whichever exist
+    const bool partL = rhoL[s + 1] > rhoL[s], partR = rhoR[s + 1] > rhoR[s];
+    double a = 1.7976931348623157e308, b = 0.0;
+    if (partL) { a = fmin(a, rhoL[s]); b = fmax(b, rhoL[s + 1]); }
+    if (partR) { a = fmin(a, rhoR[s]); b = fmax(b, rhoR[s + 1]); }
+    ok = ok && (partL || partR) && (margin < 0.01 * (b - a));
+    a = fmax(0.0, a - margin);
+    b = b + margin;
+    const double rl = ipa_fsqrt(fma(a, a, dl2)), rh = fmin(ipa_fsqrt(fma(b, b, dl2)), rmax);
+    w.crc[s] = 0.5 * (rl + rh);
+    w.crh[s] = 0.5 * (rh - rl);
+  }
+  if (!ok) {
+    for (int i = 0; i < 8; ++i) w.chb[i] = 0x7fffffff;
+    return;
+  }
+  w.ncell = IPA_NCELL;
+}
+// phase 8, threads 128..255: the full Chebyshev series (Clenshaw, degree from phase 7b) at the Chebyshev nodes of the cells
+IPA_HD_NOINLINE void ipa_pro_cells_nodes(IpaProWork& w, int tid) {
+  if (w.status || w.mode || !w.ncell || w.degree < IPA_CELL_MIN_DEGREE || tid < 128) return;
+  const int s = (tid - 128) >> 5, i = (tid - 128) & 31;
+  const double r = fma(w.crh[s], w.ctab[4 * i + 2], w.crc[s]);
+  const double t = (w.alpha * r - w.zc) / w.zh;
+  double b1 = 0.0, b2 = 0.0;
+  for (int j = w.degree; j >= 1; --j) {
+    const double b0 = fma(2.0 * t, b1, w.c[j] - b2);
+    b2 = b1;
+    b1 = b0;
+  }
+  w.cH[s][i] = fma(t, b1, w.c[0] - b2);
+}
+// phase 9, threads 128..255: Chebyshev coefficients of the cells (ctab[m] = cos(pi m / 128))
+IPA_HD_NOINLINE void ipa_pro_cells_dct(IpaProWork& w, int tid) {
+  if (w.status || w.mode || !w.ncell || w.degree < IPA_CELL_MIN_DEGREE || tid < 128) return;
+  const int s = (tid - 128) >> 5, j = (tid - 128) & 31;
+  // four partial sums (the loads of one step do not wait for the additions of the one before); index 2 j (2 i + 1) stepped by 4 j
+  double a0 = 0.0, a1 = 0.0, a2 = 0.0, a3 = 0.0;
+  const int m4 = 4 * IPA_MCHEB - 1;
+  int m = 2 * j;
+#pragma unroll
+  for (int i = 0; i < IPA_CELLM; i += 4) {
+    a0 = fma(w.cH[s][i], w.ctab[m & m4], a0);
+    a1 = fma(w.cH[s][i + 1], w.ctab[(m + 4 * j) & m4], a1);
+    a2 = fma(w.cH[s][i + 2], w.ctab[(m + 8 * j) & m4], a2);
+    a3 = fma(w.cH[s][i + 3], w.ctab[(m + 12 * j) & m4], a3);
+    m += 16 * j;
+  }
+  w.cc[s][j] = ((a0 + a1) + (a2 + a3)) * (j == 0 ? 1.0 : 2.0) * (1.0 / (double)IPA_CELLM);
+}
+// phase 11: 64 slots (cell, coefficient) on threads that phase 11 leaves idle: lanes 1..31 of warps 4 and 5, lanes 1, 2 of warp 7
+IPA_HD int ipa_pro_cells_slot(int tid) {
+  if (tid > 128 && tid < 160) return tid - 129;
+  if (tid > 160 && tid < 192) return tid - 161 + 31;
+  if (tid == 225 || tid == 226) return tid - 225 + 62;
+  return -1;
+}
+// degree of the cell (the rules of phase 7b on the cell's own interval) and its monomial coefficients (as phase 8)
+IPA_HD_NOINLINE void ipa_pro_cells_monomial(IpaProWork& w, int slot) {
+  if (slot < 0 || w.status || w.mode || !w.ncell || w.degree < IPA_CELL_MIN_DEGREE) return;
+  const int s = slot >> 4, k = slot & 15;
+  const double thr = 2.5e-16 * fmax(fmax(1.0, w.hmax4[0]), fmax(fmax(w.hmax4[1], w.hmax4[2]), w.hmax4[3]));
+  int D = 1;
+  for (int j = 2; j < IPA_CELLM; ++j)
+    if (fabs(w.cc[s][j]) > thr) D = j;
+  if (w.policy == 1) {
+    const double t0 = w.crc[s] / w.crh[s];
+    const double rinv = 1.0 / (t0 + sqrt(t0 * t0 - 1.0));
+    int Dg = 2;
+    double pw = 2.0 * rinv * rinv;
+    while (Dg < IPA_CELLM && pw > thr * (double)Dg) { ++Dg; pw *= rinv; }
+    if (D < Dg) D = Dg;
+  }
+  if (k == 0) w.cdeg[s] = D;
+  double ahi = 0.0, alo = 0.0;
+  if (D < IPA_CELLN) {
+    for (int j = k; j <= D; j += 2) {
+      const long long v = w.T[j * IPA_NCOEF + k];
+      double ph, pl, sh, sl;
+      ipa_two_prod(w.cc[s][j], (double)v, &ph, &pl);
+      ipa_two_sum(ahi, ph, &sh, &sl);
+      sl += alo + pl;
+      const double hi = sh + sl;
+      alo = sl - (hi - sh);
+      ahi = hi;
+    }
+  }
+  w.csa[s][k] = ahi + alo;
+}
+// phase 12: the cells' part of the record (threads 128..191 the coefficients, thread 96 the rest)
+IPA_HD_NOINLINE void ipa_pro_cells_record(IpaProWork& w, IpaSetConsts& o, int tid) {
+  if (tid != 96 && (tid < 128 || tid >= 128 + IPA_NCELL * IPA_CELLN)) return;
+  bool on = !w.status && !w.mode && w.ncell && w.degree >= IPA_CELL_MIN_DEGREE;
+  if (on)
+    for (int s = 0; s < IPA_NCELL; ++s) on = on && (w.cdeg[s] < IPA_CELLN);
+  if (tid != 96) {
+    const int s = (tid - 128) >> 4, k = (tid - 128) & 15;
+    o.sa[s][k] = on ? (k ? w.csa[s][k] : w.csa[s][0] - w.araw[0]) : 0.0;   // sa[s][0]: H - araw0 at t_s = 0
+    return;
+  }
+  o.ncell = on ? IPA_NCELL : 0;
+  o.sdeg[0] = o.sdeg[1] = o.sdeg[2] = 0;
+  for (int s = 0; s < IPA_NCELL; ++s) {
+    o.stA[s] = on ? 1.0 / w.crh[s] : 0.0;
+    o.stB[s] = on ? -w.crc[s] / w.crh[s] : 0.0;
+    o.sng[s] = on ? (w.cdeg[s] >> 2) : 0;
+  }
+  for (int i = 0; i < 8; ++i) o.hb[i] = on ? w.chb[i] : 0x7fffffff;
 }
 
 // phase 8: Chebyshev -> monomial, a_k = sum_j c_j T[j][k] with the integer coefficients T[j][k] of the

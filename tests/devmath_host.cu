@@ -23,11 +23,11 @@ static void run_prologue_host(const ipa_params& p, double lo, double hi, int pol
   ALL(ipa_pro_phase6(w, tid))
   ALL(ipa_pro_phase7(w, tid))
   ALL(ipa_pro_phase7b(w, tid))
-  ALL(ipa_pro_phase8_finish(w, tid))
-  ALL(ipa_pro_phase9(w, tid))
+  ALL(ipa_pro_phase8_finish(w, tid); ipa_pro_cells_nodes(w, tid))
+  ALL(ipa_pro_phase9(w, tid); ipa_pro_cells_dct(w, tid))
   ALL(ipa_pro_phase10(w, tid, NT))
-  ALL(ipa_pro_phase11(w, tid))
-  ALL(ipa_pro_phase12(w, *out, tid))
+  ALL(ipa_pro_phase11(w, tid); ipa_pro_cells_monomial(w, ipa_pro_cells_slot(tid)))
+  ALL(ipa_pro_phase12(w, *out, tid); ipa_pro_cells_record(w, *out, tid))
   ALL(ipa_pro_phase13(w, *out, tid))
 #undef ALL
 }
@@ -43,6 +43,14 @@ void emu_consts(const ipa_params* p, double lo, double hi, int policy, double* o
   out[0] = c.status; out[1] = c.degree; out[2] = c.mode; out[3] = c.normS; out[4] = c.normB;
   out[5] = c.delta2; out[6] = c.alpha; out[7] = c.logG0; out[8] = c.logG1; out[9] = -c.uA0 * c.n0; out[10] = -c.uA1 * c.n1;
   out[11] = c.dlnNS_dmu; out[12] = c.dlnNS_dsig; out[13] = c.dlnNB_dk; out[14] = c.dlnNS_dbeta;
+}
+// cells of the core: out = ncell, 4 sng[], 8 hb[]
+void emu_cells(const ipa_params* p, double lo, double hi, int policy, int* out) {
+  IpaSetConsts c;
+  run_prologue_host(*p, lo, hi, policy, &c);
+  out[0] = c.ncell;
+  for (int s = 0; s < IPA_NCELL; ++s) out[1 + s] = c.sng[s];
+  for (int i = 0; i < 8; ++i) out[1 + IPA_NCELL + i] = c.hb[i];
 }
 void emu_logpdf(const ipa_params* p, double lo, double hi, int policy, const double* x, long long n, double* out) {
   IpaSetConsts c;
