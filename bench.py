@@ -46,6 +46,26 @@ def algorithmic_flops(degree, p_core):
     return 36.0 + p_core * core + (1.0 - p_core) * 21.0
 
 
+def core_cells(torch, ipa, x, P, policy):
+    """Cells of the core of set P (ipa_core_cells) and the share of the core events of x in each: on a prepared (or
+    sorted) array a warp lies in one cell and runs that cell's polynomial, so the Horner work of a core event is the
+    degree of its cell; `degree_eff` is the mean over the core events.  An as-generated array runs the full polynomial."""
+    info = ipa.ipa_core_cells(P, LO, HI, policy=policy)
+    full = int(ipa.ipa_core_degree(P, LO, HI, policy=policy))
+    if int(info[0]) == 0:
+        return {"ncell": 0, "degree_full": full, "degree_eff": float(full)}
+    core = x[(x >= P["mu"] - P["a"] * P["sigma"]) & (x <= P["mu"] + P["a2"] * P["sigma"])]
+    hi = (core.view(torch.int64) >> 32).to(torch.int32)
+    cnt = torch.zeros_like(hi)
+    for b in info[5:11]:
+        cnt += (hi >= int(b)).to(torch.int32)
+    cell = (cnt - 3).abs()
+    share = [float((cell == c).double().mean().item()) for c in range(4)]
+    deg = [int(d) for d in info[1:5]]
+    return {"ncell": 4, "degree_full": full, "cell_degrees": deg, "cell_share_of_core_events": share,
+            "degree_eff": sum(a * b for a, b in zip(share, deg))}
+
+
 def shape_stage_flops(degree, p_core):
     """Shape stage of a group of sets sharing (mu, sigma, lambda, zeta, beta, a, n, a2, n2) -- DESIGN.md section 5:
     d (1), 2 region compares (2), core: q, sqrt, t, Horner = (5 + degree) FMA + 2 mul; tail: u (1 FMA) + log
@@ -291,12 +311,13 @@ def other_rows(torch, ipa, x, ws, stream, n, p_core):
         for pol, tag in ((1, "general_order"), (0, "adaptive_degree")):
             ds = t(lambda: ipa.ipa_nll_eval_segmented(xt, off, sets, LO, HI, ws=wst, stream=stream, policy=pol), 10)
             dss = t(lambda: ipa.ipa_nll_eval_segmented(xs, off, sets, LO, HI, ws=wst, stream=stream, policy=pol), 10)
-            deg = int(ipa.ipa_core_degree(inp.GEN, LO, HI, policy=pol))
-            W = algorithmic_flops(deg, p_core)
-            seg[tag] = {"core_degree": deg, "as_generated_ms": ds * 1e3, "prepared_per_toy_ms": dss * 1e3,
+            cl = core_cells(torch, ipa, xt[:ntot], inp.GEN, pol)      # (the toys' own sets differ from GEN by a fit error)
+            deg = cl["degree_full"]
+            seg[tag] = {"core_degree": deg, "core_cells": cl, "as_generated_ms": ds * 1e3, "prepared_per_toy_ms": dss * 1e3,
                         "toys_per_s": T / dss, "events_per_s": ntot / dss,
-                        "roofline_prepared": alu_roofline(W, ntot, dss, {"note": "whole call: 1000-set prologue + segmented kernel + finalize"}),
-                        "roofline_as_generated": alu_roofline(W, ntot, ds)}
+                        "roofline_prepared": alu_roofline(algorithmic_flops(cl["degree_eff"], p_core), ntot, dss,
+                                                          {"note": "whole call: 1000-set prologue + segmented kernel + finalize"}),
+                        "roofline_as_generated": alu_roofline(algorithmic_flops(deg, p_core), ntot, ds)}
         # generator: issue-slot model: a sub-partition issues one warp instruction per cycle and an
         # FP64 instruction holds the port for two.  Declared per event: signal fraction 0.3 x (bookkeeping Philox 100 +
         # attempts x (Philox 100 + core log G 8 int + (7 + D) FP64 + acceptance exp 15 FP64 + 12 int)) + background 0.7 x
@@ -478,8 +499,13 @@ def main():
         return e0.elapsed_time(e1) * 1e-3 / (reps * replays)
     dt_pro = prologue_gpu_time(P1, norm_out)
     t_step = dt / args.steps
-    degree = int(ipa.ipa_core_degree(P1, LO, HI, policy=POL))
-    flops = algorithmic_flops(degree, p_core)
+    cells = core_cells(torch, ipa, x_asis, P1, POL)
+    degree = cells["degree_full"]
+    # Horner work per core event: the cell polynomials on the prepared layout, the full polynomial as generated
+    deg_prep, deg_asis = cells["degree_eff"], float(degree)
+    deg_x = deg_prep if args.layout == "prepared" else deg_asis
+    deg_other = deg_asis if args.layout == "prepared" else deg_prep
+    flops = algorithmic_flops(deg_x, p_core)
 
     def local_step_time(fn, steps, warm=2):
         for _ in range(warm):
@@ -492,7 +518,7 @@ def main():
     t_local = t_step if not dist else local_step_time(lambda: k1_local(x), args.steps)
     t_kernel = max(t_local - dt_pro, 1e-9)
 
-    extras = {"p_core": p_core, "core_degree": degree, "prologue_ms": dt_pro * 1e3, "nll_kernel_ms": t_kernel * 1e3,
+    extras = {"p_core": p_core, "core_degree": degree, "core_cells": cells, "prologue_ms": dt_pro * 1e3, "nll_kernel_ms": t_kernel * 1e3,
               "build_hash": build_hash()}
     if not args.no_extras and rank == 0:
         k9steps = max(5, args.steps // 8)
@@ -507,19 +533,21 @@ def main():
                              "algorithmic_bytes_per_event": 24, "note": "two reads (count, scatter) + one write of 8 B",
                              "break_even_calls_k1": d_prep / max(t_asis - t_prepared, 1e-12),
                              "single_call_with_prepare_ms": (d_prep + t_prepared) * 1e3}
-        extras[f"roofline_{oname}"] = alu_roofline(flops, n, max(d_other - dt_pro, 1e-9),
+        extras[f"roofline_{oname}"] = alu_roofline(algorithmic_flops(deg_other, p_core), n, max(d_other - dt_pro, 1e-9),
                                                    {"layout": oname, "call_ms": d_other * 1e3})
         extras["roofline_asis_plus_prepare_single_call"] = alu_roofline(flops, n, d_prep + t_prepared,
                                                                         {"note": "new data every call: prepare + one NLL"})
         dt9 = local_step_time(step_k9, k9steps)
-        W9 = 5 * shape_stage_flops(degree, p_core) + 9 * MEMBER_STAGE_FLOPS
+        # (the four displaced shapes of the batch have cells of their own; their degrees equal the base set's here)
+        W9 = 5 * shape_stage_flops(deg_x, p_core) + 9 * MEMBER_STAGE_FLOPS
+        W9o = 5 * shape_stage_flops(deg_other, p_core) + 9 * MEMBER_STAGE_FLOPS
         extras["k9_gradient_batch"] = {"ms_per_call": dt9 * 1e3, "event_sets_per_s": 9 * n / dt9, "events_per_s": n / dt9,
                                        "nll_calls_per_s": 9 / dt9}
         extras["roofline_k9"] = alu_roofline(W9, n, max(dt9 - dt_pro, 1e-9),
                                              {"note": "central-difference batch over (mu, sigma, f, k): 5 shape stages + 9 member "
                                                       "stages per event", "flops_per_event_set": W9 / 9})
         dto9 = local_step_time(lambda: step_k9(other), k9steps)
-        extras[f"roofline_k9_{oname}"] = alu_roofline(W9, n, max(dto9 - dt_pro, 1e-9), {"layout": oname, "call_ms": dto9 * 1e3})
+        extras[f"roofline_k9_{oname}"] = alu_roofline(W9o, n, max(dto9 - dt_pro, 1e-9), {"layout": oname, "call_ms": dto9 * 1e3})
 
         def step_adaptive():
             ipa.ipa_nll_eval(x, P1, LO, HI, ws=ws, stream=stream, out=out1, status=st1, policy=0)

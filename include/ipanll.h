@@ -41,6 +41,8 @@
  *     Any n >= 0 is accepted (n == 0 gives NLL = +0.0).
  *   - Determinism: for fixed device, build, n and launch geometry the results are bitwise
  *     reproducible, and the result of set k does not depend on which other sets share the batch.
+ *     The per-event value may differ in the last bits (< 2e-13) between two ORDERS of the same events: a warp whose
+ *     events lie in one cell of the core evaluates that cell's polynomial, any other warp the full one (ipa_core_cells).
  */
 #ifndef IPANLL_H
 #define IPANLL_H
@@ -124,6 +126,21 @@ int ipa_norm(const ipa_params* p_host, int K, ipa_range r, double* norm_sig_dev,
 int ipa_core_degree(const ipa_params* p_host, int K, ipa_range r, int32_t* degree_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes,
                     void* cuda_stream);
 
+/* Introspection of the prologue, cells of the core (step A1e).  Where the full core polynomial has
+ * degree 16 or more, the core interval of r = sqrt((x-mu)^2 + delta^2) is cut into 4 cells of equal ratio and each cell gets
+ * its own polynomial of lower degree, refitted from the full one; a warp whose events all lie in one cell (a warp of an
+ * array laid out by ipa_events_prepare, or of a sorted array, nearly always does) evaluates the cell polynomial, any other
+ * warp the full one.  Both approximate the same function to the same tolerance: the value of an event can differ in the
+ * last bits between two layouts of the same events, never between two runs on the same array.
+ *   cells_dev [K][IPA_CELL_INFO] int32: { number of cells (4, or 0: no cells for this set),
+ *                                         degree of cell 0..3 (cell 0 holds the peak),
+ *                                         high 32 bits of the 6 cell boundaries in x, ascending (0 / INT32_MAX: a boundary
+ *                                         outside the core on the left / on the right), INT32_MAX, INT32_MAX }
+ * An event x lies in cell |#{i : hb[i] <= high word of x} - 3|.  Used by bench.py to state the algorithmic work. */
+#define IPA_CELL_INFO 13
+int ipa_core_cells(const ipa_params* p_host, int K, ipa_range r, int32_t* cells_dev, const ipa_options* opt_host,
+                   void* ws_dev, size_t ws_bytes, void* cuda_stream);
+
 /* The hot path (fused into one pass): NLL of n events for K parameter sets.
  *   x_dev      [n]    event masses, fp64, 8-byte aligned
  *   p_host     [K]    parameter sets
@@ -131,7 +148,7 @@ int ipa_core_degree(const ipa_params* p_host, int K, ipa_range r, int32_t* degre
  *   logpdf_dev [K*n]  out, optional (NULL to skip): per-event log(f S + (1-f) B), set-major; the row of a set with
  *                     status != 0 is filled with NaN
  *   status_dev [K]    out, optional
- * K <= IPA_MAX_K per call. */
+ * K <= IPA_MAX_K per call; up to 28 sets share one pass over the events, a larger batch takes two (shared memory). */
 #define IPA_MAX_K 32
 int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r,
                  double* nll_dev, double* logpdf_dev, int32_t* status_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes,

@@ -13,7 +13,7 @@ from . import build as _build
 
 __all__ = [
     "PARAM_FIELDS", "NPAR", "IPA_MAX_K", "IpaError", "lib", "library_path", "pack_params", "workspace",
-    "ipa_version", "ipa_workspace_bytes", "ipa_norm", "ipa_core_degree", "ipa_nll_grad_eval", "ipa_nll_fd_gradient",
+    "ipa_version", "ipa_workspace_bytes", "ipa_norm", "ipa_core_degree", "ipa_core_cells", "ipa_nll_grad_eval", "ipa_nll_fd_gradient",
     "ipa_nll_eval_extended", "ipa_nll_eval_categories", "ipa_nll_eval",
     "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill", "ipa_binned_nll_scan", "ipa_expected_hist",
     "ipa_poisson_hist_toys", "ipa_signal_shape", "ipa_gauss_smear", "ipa_expected_hist_shape", "ipa_binned_nll_scan_shape",
@@ -28,7 +28,7 @@ IPA_MAX_K = 32
 # every symbol include/ipanll.h declares
 EXPORTS = (
     "ipa_strerror", "ipa_last_cuda_error", "ipa_version", "ipa_workspace_bytes",
-    "ipa_norm", "ipa_core_degree", "ipa_nll_eval", "ipa_nll_fd_gradient", "ipa_nll_eval_extended", "ipa_nll_grad_eval", "ipa_nll_eval_segmented", "ipa_nll_eval_categories", "ipa_toy_generate", "ipa_hist_fill",
+    "ipa_norm", "ipa_core_degree", "ipa_core_cells", "ipa_nll_eval", "ipa_nll_fd_gradient", "ipa_nll_eval_extended", "ipa_nll_grad_eval", "ipa_nll_eval_segmented", "ipa_nll_eval_categories", "ipa_toy_generate", "ipa_hist_fill",
     "ipa_binned_nll_scan", "ipa_expected_hist", "ipa_poisson_hist_toys", "ipa_signal_shape", "ipa_gauss_smear",
     "ipa_expected_hist_shape", "ipa_binned_nll_scan_shape", "ipa_cls_teststat", "ipa_cls_count_ge",
     "ipa_cls_from_counts", "ipa_prepare_workspace_bytes", "ipa_events_prepare",
@@ -80,6 +80,7 @@ def lib():
     op = vp  # const ipa_options* (NULL or byref(_Options))
     L.ipa_norm.restype = i32; L.ipa_norm.argtypes = [vp, i32, _Range, vp, vp, vp, op, vp, sz, vp]
     L.ipa_core_degree.restype = i32; L.ipa_core_degree.argtypes = [vp, i32, _Range, vp, op, vp, sz, vp]
+    L.ipa_core_cells.restype = i32; L.ipa_core_cells.argtypes = [vp, i32, _Range, vp, op, vp, sz, vp]
     L.ipa_nll_eval.restype = i32; L.ipa_nll_eval.argtypes = [vp, i64, vp, i32, _Range, vp, vp, vp, op, vp, sz, vp]
     L.ipa_nll_fd_gradient.restype = i32
     L.ipa_nll_fd_gradient.argtypes = [vp, i64, vp, i32, vp, vp, _Range, vp, vp, vp, op, vp, sz, vp]
@@ -221,6 +222,18 @@ def ipa_core_degree(params, lo, hi, ws=None, stream=None, policy=None):
     _check(lib().ipa_core_degree(_hptr(P), K, _Range(lo, hi), _dptr(out), _opt(policy), _dptr(ws), ws.numel(), _stream(stream)))
     r = out.cpu().numpy()
     return int(r[0]) if K == 1 else r
+
+
+def ipa_core_cells(params, lo, hi, ws=None, stream=None, policy=None):
+    """Cells of the core per set: int32 array [K, 13] = (ncell, 4 degrees, 6 boundary high words, 2 pads); [13] for one set."""
+    _need_cuda()
+    P = pack_params(params)
+    K = P.shape[0]
+    ws = _ws(ws, 0, K)
+    out = torch.empty((K, 13), dtype=torch.int32, device="cuda")
+    _check(lib().ipa_core_cells(_hptr(P), K, _Range(lo, hi), _dptr(out), _opt(policy), _dptr(ws), ws.numel(), _stream(stream)))
+    r = out.cpu().numpy()
+    return r[0] if K == 1 else r
 
 
 @_alloc_on_stream

@@ -171,6 +171,22 @@ int ipa_core_degree(const ipa_params* p_host, int K, ipa_range r, int32_t* degre
   return IPA_OK;
 }
 
+int ipa_core_cells(const ipa_params* p_host, int K, ipa_range r, int32_t* cells_dev, const ipa_options* opt_host,
+                   void* ws_dev, size_t ws_bytes, void* cuda_stream) {
+  static_assert(IPA_CELL_INFO == 1 + IPA_NCELL + 8, "ipanll.h: IPA_CELL_INFO");
+  const int policy = policy_of(opt_host);
+  if (!p_host || K < 1 || !range_ok(r) || !cells_dev || policy < 0) return IPA_ERR_INVALID_ARG;
+  const Layout L = make_layout(K, 0);
+  if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
+  cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+  char* ws = static_cast<char*>(ws_dev);
+  int rc = run_prologue(p_host, K, r, policy, ws, L, nullptr, nullptr, nullptr, st);
+  if (rc) return rc;
+  ipa_cells_kernel<<<(K + 127) / 128, 128, 0, st>>>(reinterpret_cast<const IpaSetConsts*>(ws + L.consts), K, cells_dev);
+  IPA_CK(cudaGetLastError());
+  return IPA_OK;
+}
+
 int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r, double* nll_dev,
                  double* logpdf_dev, int32_t* status_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes,
                  void* cuda_stream) {

@@ -1566,6 +1566,17 @@ ipa_poisson_hist_kernel(const double* __restrict__ mean, int nbins, const unsign
   }
 }
 
+// ipa_core_cells: out[k] = { ncell, degree of each cell, high words of the cell boundaries in x }
+__global__ void ipa_cells_kernel(const IpaSetConsts* __restrict__ consts, int K, int32_t* __restrict__ out) {
+  const int k = blockIdx.x * blockDim.x + threadIdx.x;
+  if (k >= K) return;
+  const IpaSetConsts& c = consts[k];
+  int32_t* o = out + (long long)k * IPA_CELL_INFO;
+  const bool on = !c.status && c.ncell;
+  o[0] = on ? c.ncell : 0;
+  for (int s = 0; s < IPA_NCELL; ++s) o[1 + s] = on ? c.sdeg[s] : 0;
+  for (int i = 0; i < 8; ++i) o[1 + IPA_NCELL + i] = on ? c.hb[i] : 0x7fffffff;
+}
 __global__ void ipa_degree_kernel(const IpaSetConsts* __restrict__ consts, int K, int32_t* __restrict__ out) {
   const int k = blockIdx.x * blockDim.x + threadIdx.x;
   if (k < K) out[k] = consts[k].status ? -2 : (consts[k].mode ? -1 : consts[k].degree);

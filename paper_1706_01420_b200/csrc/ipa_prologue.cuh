@@ -71,7 +71,8 @@ struct alignas(16) IpaSetConsts {
   double stA[IPA_NCELL], stB[IPA_NCELL];
   int32_t hb[8];
   int32_t sng[IPA_NCELL];
-  int32_t ncell, sdeg[3];       // sdeg: unused padding (the degrees are 4 sng + 3 at most; ipa_core_cells reports them)
+  int32_t ncell, cpad[3];
+  int32_t sdeg[IPA_NCELL];      // degrees of the cell polynomials (ipa_core_cells reports them; the kernels run 4 sng + 3)
 };
 
 struct IpaProWork {
@@ -562,8 +563,9 @@ IPA_HD_NOINLINE void ipa_pro_cells_record(IpaProWork& w, IpaSetConsts& o, int ti
     return;
   }
   o.ncell = on ? IPA_NCELL : 0;
-  o.sdeg[0] = o.sdeg[1] = o.sdeg[2] = 0;
+  o.cpad[0] = o.cpad[1] = o.cpad[2] = 0;
   for (int s = 0; s < IPA_NCELL; ++s) {
+    o.sdeg[s] = on ? w.cdeg[s] : 0;
     o.stA[s] = on ? 1.0 / w.crh[s] : 0.0;
     o.stB[s] = on ? -w.crc[s] / w.crh[s] : 0.0;
     o.sng[s] = on ? (w.cdeg[s] >> 2) : 0;

@@ -104,6 +104,7 @@ def emu(tmp_path_factory):
     L.emu_consts.argtypes = [vp, d, d, C.c_int, vp]
     L.emu_logpdf.argtypes = [vp, d, d, C.c_int, vp, ll, vp]
     L.emu_logI.argtypes = [vp, d, d, vp, ll, vp]
+    L.emu_cells.argtypes = [vp, d, d, C.c_int, vp]
     L.emu_grad.argtypes = [vp, d, d, C.c_int, vp, ll, vp]
     L.emu_uniforms2.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, C.c_uint32, vp]
     L.emu_poisson.restype = ll; L.emu_poisson.argtypes = [C.c_uint64, C.c_uint64, C.c_uint32, d]
@@ -153,6 +154,39 @@ def test_device_math_vs_oracle(emu, orc, shape, policy):
     gi = np.empty_like(d)
     emu.emu_logI(p.ctypes.data, LO, HI, d.ctypes.data, d.size, gi.ctypes.data)
     assert np.abs(gi - np.array([orc.log_I(P, v) for v in d])).max() <= 5e-14
+
+
+@pytest.mark.parametrize("shape", ["GEN", "P2", "asym", "offgrid"])
+def test_device_core_cells_vs_oracle(emu, orc, shape):
+    """Cells of the core (prologue A1e, host build): each cell polynomial against the oracle on a dense sorted grid (the
+    host 'warp' is 8 consecutive events, so nearly every group lies in one cell), the full one on the same events shuffled."""
+    P, pol = {"GEN": (inp.GEN, 1), "P2": (inp.P2, 0), "asym": (dict(inp.GEN, a=0.8, a2=3.0, beta=0.02), 1),
+              "offgrid": (dict(inp.GEN, mu=5281.37, sigma=13.1), 1)}[shape]
+    p = inp.as_array(P)
+    info = np.zeros(13, dtype=np.int32)
+    emu.emu_cells(p.ctypes.data, LO, HI, pol, info.ctypes.data)
+    assert info[0] == 4 and all(0 <= g <= 3 for g in info[1:5])          # Horner groups of 4: degree 4 g + 3 at most
+    hb = [int(v) for v in info[5:11]]
+    assert hb == sorted(hb)
+    real = [v for v in hb if 0 < v < 2 ** 31 - 1]
+    xb = (np.array(real, dtype=np.int64) << 32).view(np.float64)
+    xl, xr = P["mu"] - P["a"] * P["sigma"], P["mu"] + P["a2"] * P["sigma"]
+    assert np.all((xb > xl) & (xb < xr))
+    x = np.sort(np.concatenate([np.linspace(xl - 5.0, xr + 5.0, 60000), xb, np.nextafter(xb, 0.0), np.nextafter(xb, 1e9)]))
+    ref = orc.logpdf(x, P, LO, HI)
+    got = np.empty_like(x)
+    emu.emu_logpdf(p.ctypes.data, LO, HI, pol, x.ctypes.data, x.size, got.ctypes.data)
+    assert np.abs(got - ref).max() <= 2e-14
+    perm = np.random.Generator(np.random.Philox(9)).permutation(x.size)
+    xp = x[perm].copy()
+    got2 = np.empty_like(x)
+    emu.emu_logpdf(p.ctypes.data, LO, HI, pol, xp.ctypes.data, xp.size, got2.ctypes.data)
+    assert np.abs(got2 - ref[perm]).max() <= 2e-14
+    assert (got[perm] != got2).any()                                       # the sorted pass did run the cell polynomials
+    # no cells: degree below 16 (K_{1/2} under the adaptive policy), a core too narrow for the high-word resolution
+    for Q, qpol in ((inp.GEN, 0), (dict(inp.GEN, sigma=0.02), 1), (inp.T1, 1), (dict(inp.GEN, zeta=0.2), 1)):
+        emu.emu_cells(inp.as_array(Q).ctypes.data, LO, HI, qpol, info.ctypes.data)
+        assert info[0] == 0
 
 
 def test_device_generators_vs_oracle(emu, orc):

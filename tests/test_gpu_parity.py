@@ -752,8 +752,51 @@ def test_maximum_batch_of_32_sets(ipa, torch_, orc, x1):
         assert np.all(np.abs(got - ref) <= 1e-10 * np.abs(ref))
         for i in (0, 13, 31):
             assert got[i] == ipa.ipa_nll_eval(xd, sets[i], LO, HI)[0].item()
+    # above 28 sets the batch runs as two launches (shared memory): rows of the per-event output, odd split
+    nll29, lp29, _ = ipa.ipa_nll_eval(xd, distinct[:29], LO, HI, want_logpdf=True)
+    torch_.cuda.synchronize()
+    for i in (0, 14, 15, 28):
+        one, lp1, _ = ipa.ipa_nll_eval(xd, distinct[i], LO, HI, want_logpdf=True)
+        assert nll29[i].item() == one.item() and bool((lp29[i] == lp1[0]).all())
     with pytest.raises(ipa.IpaError):
         ipa.ipa_nll_eval(xd, distinct + [inp.GEN], LO, HI)          # 33 sets: invalid argument
+
+
+def test_core_cells(ipa, torch_, orc):
+    """Cells of the core (A1e): a warp of a sorted or prepared array runs the low-degree polynomial of its cell, a warp of
+    the same events in random order the full polynomial; both against the oracle, per event."""
+    full = ipa.ipa_core_degree(inp.GEN, LO, HI, policy=1)
+    info = ipa.ipa_core_cells(inp.GEN, LO, HI, policy=1)
+    assert info[0] == 4 and all(3 <= d < 16 for d in info[1:5]) and max(info[1:5]) < full
+    hb = [int(v) for v in info[5:11]]
+    assert hb == sorted(hb) and info[11] == info[12] == 2 ** 31 - 1
+    # boundaries sit on the edges of the coarse bins of ipa_events_prepare (bin width (HI - LO) / 256)
+    edges = np.array(hb, dtype=np.int64) << 32
+    xb = edges.view(np.float64)
+    assert np.all(np.abs((xb - LO) * 256 / (HI - LO) - np.rint((xb - LO) * 256 / (HI - LO))) < 1e-3)
+    assert ipa.ipa_core_cells(inp.GEN, LO, HI, policy=0)[0] == 0          # degree 1 (K_{1/2}): nothing to gain
+    assert ipa.ipa_core_cells(dict(inp.GEN, sigma=0.02), LO, HI, policy=1)[0] == 0   # core narrower than the high-word resolution allows
+    xg, _, _ = ipa.ipa_toy_generate([11], inp.GEN, -1.0, -1.0, LO, HI, 300_000)
+    x = xg.cpu().numpy()
+    # the boundary doubles themselves and their neighbours
+    x[:18] = np.concatenate([xb, np.nextafter(xb, 0.0), np.nextafter(xb, 1e9)])
+    xs = np.sort(x)
+    perm = np.random.Generator(np.random.Philox(5)).permutation(x.size)
+    ref = orc.logpdf(xs, inp.GEN, LO, HI)
+    for P, pol in ((inp.GEN, 1), (inp.P2, 0), (dict(inp.GEN, a=0.8, a2=3.0, beta=0.02), 1)):
+        if P is not inp.GEN:
+            ref = orc.logpdf(xs, P, LO, HI)
+            assert ipa.ipa_core_cells(P, LO, HI, policy=pol)[0] == 4
+        n1, lp_s, _ = ipa.ipa_nll_eval(dev(torch_, xs), P, LO, HI, want_logpdf=True, policy=pol)
+        n2, lp_r, _ = ipa.ipa_nll_eval(dev(torch_, xs[perm]), P, LO, HI, want_logpdf=True, policy=pol)
+        n3 = ipa.ipa_nll_eval(ipa.ipa_events_prepare(dev(torch_, xs[perm]), LO, HI), P, LO, HI, policy=pol)[0]
+        torch_.cuda.synchronize()
+        a, b = lp_s[0].cpu().numpy(), lp_r[0].cpu().numpy()
+        assert np.abs(a - ref).max() <= 1e-10 and np.abs(b - ref[perm]).max() <= 1e-10
+        assert np.abs(a[perm] - b).max() <= 2e-13 and (a[perm] != b).any()      # two polynomials for the same function
+        tot = orc.nll(xs, P, LO, HI)
+        for v in (n1, n2, n3):
+            assert abs(v.item() - tot) <= 1e-10 * abs(tot)
 
 
 # ---------------------------------------------------------------------------------------------
