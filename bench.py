@@ -568,7 +568,7 @@ def main():
         dtg = local_step_time(lambda: ipa.ipa_nll_grad_eval(x, P1, LO, HI, ws=ws, stream=stream, policy=POL), k9steps)
         extras["f1_analytic_gradient"] = {"ms_per_call": dtg * 1e3, "events_per_s": n / dtg,
                                           "speedup_vs_k9_finite_differences": dt9 / dtg}
-        extras["roofline_grad"] = alu_roofline(gradient_flops(degree, p_core), n, dtg, {"note": "whole call (prologue with "
+        extras["roofline_grad"] = alu_roofline(gradient_flops(int(deg_x), p_core), n, dtg, {"note": "whole call (prologue with "
                                                "normalisation derivatives + gradient kernel)"})
         if world == 1:
             extras.update(other_rows(torch, ipa, x_asis, ws, stream, n, p_core))

@@ -633,19 +633,33 @@ IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&
 #pragma unroll
   for (int e = 0; e < E; ++e) { d[e] = x[e] - c.mu; db[e] = d[e]; }      // dlogI/dbeta = d in the core
   if (sane && c.mode == 0 && hmin > c.hxl && hmax < c.hxr) {
-    // all E events in the core: one pass over the coefficients (128-bit uniform loads) for H and dH/dt of all of them
+    // all E events in the core: one pass over the coefficients (128-bit uniform loads) for H and dH/dt of all of them;
+    // a warp inside one cell of the core runs the cell's polynomial (its constant term lacks the folded a[0]: k0)
+    const double* a = c.a;
+    double tA = c.tA, tB = c.tB, k0 = 0.0;
+    int ng = c.degree >> 2;
+    if (c.ncell) {
+      const int cell = ipa_warp_cell(c, hmin, hmax);
+      if (cell >= 0) {
+        a = c.sa[cell];
+        tA = c.stA[cell];
+        tB = c.stB[cell];
+        ng = c.sng[cell];
+        k0 = c.a[0];
+      }
+    }
     double t[E], rinv[E], P[E], Pd[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) {
       const double r = ipa_fsqrt(fma(d[e], d[e], c.delta2));
       rinv[e] = ipa_frcp(r);
-      t[e] = fma(c.tA, r, c.tB);
+      t[e] = fma(tA, r, tB);
       P[e] = 0.0;
       Pd[e] = 0.0;
     }
-    for (int g = c.degree >> 2; g >= 0; --g) {
-      const double2 hi2 = *reinterpret_cast<const double2*>(c.a + 4 * g + 2);
-      const double2 lo2 = *reinterpret_cast<const double2*>(c.a + 4 * g);
+    for (int g = ng; g >= 0; --g) {
+      const double2 hi2 = *reinterpret_cast<const double2*>(a + 4 * g + 2);
+      const double2 lo2 = *reinterpret_cast<const double2*>(a + 4 * g);
 #pragma unroll
       for (int e = 0; e < E; ++e) {
         Pd[e] = fma(Pd[e], t[e], P[e]); P[e] = fma(P[e], t[e], hi2.y);
@@ -656,8 +670,8 @@ IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&
     }
 #pragma unroll
     for (int e = 0; e < E; ++e) {
-      const double Lmb = c.tA * d[e] * rinv[e] * Pd[e];
-      D[e] = fma(c.bmk, d[e], P[e]);
+      const double Lmb = tA * d[e] * rinv[e] * Pd[e];
+      D[e] = fma(c.bmk, d[e], P[e] + k0);
       dd[e] = c.beta + Lmb;
       ds[e] = fma(-d[e] * c.invsig, Lmb, c.nuosig);
     }

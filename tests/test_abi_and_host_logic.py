@@ -183,6 +183,15 @@ def test_device_core_cells_vs_oracle(emu, orc, shape):
     emu.emu_logpdf(p.ctypes.data, LO, HI, pol, xp.ctypes.data, xp.size, got2.ctypes.data)
     assert np.abs(got2 - ref[perm]).max() <= 2e-14
     assert (got[perm] != got2).any()                                       # the sorted pass did run the cell polynomials
+    # analytic gradient (row f1) through the cell polynomials: value and derivative chains, four consecutive events per group
+    g1, g2 = np.zeros(6), np.zeros(6)
+    emu.emu_grad(p.ctypes.data, LO, HI, pol, x.ctypes.data, x.size, g1.ctypes.data)
+    emu.emu_grad(p.ctypes.data, LO, HI, pol, xp.ctypes.data, xp.size, g2.ctypes.data)
+    ref_n, ref_g = orc.nll_gradient(x, P, LO, HI)
+    assert abs(g1[0] - ref_n) <= 1e-12 * abs(ref_n) and abs(g2[0] - ref_n) <= 1e-12 * abs(ref_n)
+    tol = 1e-7 * np.maximum(np.abs(ref_g), 1.0 / np.array([inp.GRAD_SCALE[k] for k in inp.GRAD_NAMES]))   # reading D18
+    assert np.all(np.abs(g1[1:] - ref_g) <= tol) and np.all(np.abs(g2[1:] - ref_g) <= tol)
+    assert (g1 != g2).any()
     # no cells: degree below 16 (K_{1/2} under the adaptive policy), a core too narrow for the high-word resolution
     for Q, qpol in ((inp.GEN, 0), (dict(inp.GEN, sigma=0.02), 1), (inp.T1, 1), (dict(inp.GEN, zeta=0.2), 1)):
         emu.emu_cells(inp.as_array(Q).ctypes.data, LO, HI, qpol, info.ctypes.data)

@@ -797,6 +797,11 @@ def test_core_cells(ipa, torch_, orc):
         tot = orc.nll(xs, P, LO, HI)
         for v in (n1, n2, n3):
             assert abs(v.item() - tot) <= 1e-10 * abs(tot)
+        # analytic gradient (f1): value and derivative chains of the cell polynomials (sorted) / of the full one (shuffled)
+        ref_n, ref_g = orc.nll_gradient(xs, P, LO, HI)
+        for arr in (xs, xs[perm]):
+            gn, gg, _ = ipa.ipa_nll_grad_eval(dev(torch_, arr), P, LO, HI, policy=pol)
+            assert abs(gn.item() - ref_n) <= 1e-10 * abs(ref_n) and grad_ok(gg.cpu().numpy().reshape(-1), ref_g)
 
 
 # ---------------------------------------------------------------------------------------------
