@@ -297,16 +297,11 @@ IPA_HD double ipa_fexp_negabs_t(double D, const double* mt) {
 #endif
 }
 
-// eb + log(1 + e^D) = eb + log(1 + e^{-|D|}) [+ D if D >= 0]: max(D, 0) is a predicated add on the sign word.
-// (max(D, 0) = D/2 + |D|/2 folded into two FMAs saves the compare and the selects but cancels for D << 0:
-// 3.5e-15 at D = -52, measured in the host test -- rejected.)
+// eb + log(1 + e^D) = eb + log(1 + e^{-|D|}) + max(D, 0), and max(D, 0) = (D + |D|) / 2 with D + |D| EXACT (0 or 2 D): the
+// final FMA rounds once, like the addition of D it replaces -- same bits, no compare and no select (ptxas turned a
+// predicated add into an unconditional one plus two FSEL: 4 issue slots against 2 FP64 instructions here).
+// (Folding D/2 + |D|/2 into the two FMAs of the sum instead cancels for D << 0: 3.5e-15 at D = -52 -- rejected.)
 IPA_HD double ipa_fsoftplus_add_t(double eb, double D, const double* mt) {
   const double w = ipa_fexp_negabs_t(D, mt);
-  double l = eb + ipa_flog12_t(1.0 + w, mt);
-#ifdef __CUDA_ARCH__
-  asm("{\n\t.reg .pred p;\n\tsetp.ge.s32 p, %2, 0;\n\t@p add.f64 %0, %0, %1;\n\t}" : "+d"(l) : "d"(D), "r"(ipa_hi(D)));
-#else
-  if (ipa_hi(D) >= 0) l += D;
-#endif
-  return l;
+  return fma(0.5, D + fabs(D), eb + ipa_flog12_t(1.0 + w, mt));
 }
