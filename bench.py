@@ -616,7 +616,7 @@ def main():
     traffic, traffic_note = measured_traffic(n)
     roofline = {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                 "traffic": traffic, "traffic_source": traffic_note,
-                "kernel": "ipa_nll_kernel<false,false>", "kernel_ms": t_kernel * 1e3,
+                "kernel": "ipa_nll_kernel<false,false,true>", "kernel_ms": t_kernel * 1e3,
                 "kernel_time_source": "CUDA events: step time minus the prologue's device time (20 prologue launches captured "
                                       "in a CUDA graph and replayed: no host gaps)",
                 "frac_whole_step": flops * n / t_local / 1e12 / peak,
