@@ -198,6 +198,44 @@ def test_device_core_cells_vs_oracle(emu, orc, shape):
         assert info[0] == 0
 
 
+def test_device_core_cells_random_shapes(emu, orc):
+    """Random shapes and ranges, among them cores that straddle a power of two (the unit of the high word of x doubles
+    there): every cell polynomial against the oracle on a sorted grid that holds the boundary doubles and their neighbours."""
+    rng = np.random.Generator(np.random.Philox(77))
+    with_cells = 0
+    for it in range(60):
+        if it % 2:
+            base = 2.0 ** rng.integers(-3, 14)
+            sigma = base * rng.uniform(0.002, 0.02)
+            mu = base + rng.uniform(-2, 2) * sigma
+        else:
+            base = 5280.0 * rng.choice([1.0, 1e-3, 37.0])
+            mu, sigma = base * (1 + rng.uniform(-0.01, 0.01)), base / 5280.0 * rng.uniform(3, 30)
+        sc = base / 5280.0
+        lo, hi = mu - rng.uniform(8, 20) * sigma, mu + rng.uniform(8, 20) * sigma
+        lo = lo if lo > 0 else 0.2 * mu
+        P = dict(mu=mu, sigma=sigma, zeta=10 ** rng.uniform(-0.3, 1.2), beta=rng.uniform(-0.02, 0.02) / sc,
+                 a=rng.uniform(0.7, 3.5), n=rng.uniform(1.1, 6), a2=rng.uniform(0.7, 3.5), n2=rng.uniform(1.1, 6),
+                 f=rng.uniform(0.05, 0.95), k=rng.uniform(-0.004, 0.001) / sc)
+        P["lambda"] = rng.uniform(-3, 2)
+        p = inp.as_array(P)
+        c, info = np.zeros(15), np.zeros(13, dtype=np.int32)
+        emu.emu_consts(p.ctypes.data, lo, hi, 1, c.ctypes.data)
+        emu.emu_cells(p.ctypes.data, lo, hi, 1, info.ctypes.data)
+        if c[0] != 0 or info[0] == 0:
+            continue
+        with_cells += 1
+        xl, xr = mu - P["a"] * sigma, mu + P["a2"] * sigma
+        xb = (np.array([int(v) for v in info[5:11] if 0 < v < 2 ** 31 - 1], dtype=np.int64) << 32).view(np.float64)
+        assert np.all((xb > xl) & (xb < xr))
+        x = np.sort(np.concatenate([np.linspace(max(lo, xl - 3 * sigma), min(hi, xr + 3 * sigma), 8000), xb,
+                                    np.nextafter(xb, 0.0), np.nextafter(xb, 1e300)]))
+        got = np.empty_like(x)
+        emu.emu_logpdf(p.ctypes.data, lo, hi, 1, x.ctypes.data, x.size, got.ctypes.data)
+        assert np.abs(got - orc.logpdf(x, P, lo, hi)).max() <= 5e-14, P
+    assert with_cells >= 15
+
+
 def test_device_generators_vs_oracle(emu, orc):
     rng = np.random.Generator(np.random.Philox(3))
     for _ in range(200):
