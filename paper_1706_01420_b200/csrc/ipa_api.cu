@@ -229,6 +229,17 @@ int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K
         }
     bool grouped = false;
     for (int k = 0; k < kb; ++k) grouped = grouped || grp.leader[k] != k;
+    int ng = 0, nm = 0;
+    for (int g = 0; g < kb; ++g) {
+      if (grp.leader[g] != g) continue;
+      grp.first[ng++] = (unsigned char)nm;
+      for (int k = g; k < kb; ++k)
+        if (grp.leader[k] == g) grp.member[nm++] = (unsigned char)k;
+    }
+    grp.first[ng] = (unsigned char)nm;
+    grp.ngroups = (unsigned char)ng;
+    for (int i = ng + 1; i <= IPA_MAX_K; ++i) grp.first[i] = (unsigned char)nm;
+    for (int i = nm; i < IPA_MAX_K; ++i) grp.member[i] = 0;
     auto kern = logpdf_dev ? (grouped ? ipa_nll_kernel<true, true> : ipa_nll_kernel<true, false>)
                            : (grouped ? ipa_nll_kernel<false, true> : ipa_nll_kernel<false, false>);
     if (kb == 1 && !logpdf_dev) kern = ipa_nll_kernel<false, false, true>;

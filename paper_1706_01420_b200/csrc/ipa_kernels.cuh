@@ -207,10 +207,11 @@ IPA_HD void ipa_mixed_shape(const IpaSetConsts& c, const double (&d)[E], double 
     if (left || right) V[e] = tl;
   }
 }
-template <int E, class Tab>
-IPA_HD int ipa_shape_stage(const IpaSetConsts& c, const double (&x)[E], double (&d)[E], double (&V)[E], const Tab* tab) {
-  const double mu = c.mu;
-  int hmin = ipa_hi(x[0]), hmax = hmin;
+// smallest and largest high word of the warp's events (once per tile, for all sets)
+template <int E>
+IPA_HD void ipa_warp_hi_range(const double (&x)[E], int& hmin, int& hmax) {
+  hmin = ipa_hi(x[0]);
+  hmax = hmin;
 #pragma unroll
   for (int e = 1; e < E; ++e) {
     const int h = ipa_hi(x[e]);
@@ -219,6 +220,11 @@ IPA_HD int ipa_shape_stage(const IpaSetConsts& c, const double (&x)[E], double (
   }
   hmin = ipa_warp_min(hmin);
   hmax = ipa_warp_max(hmax);
+}
+template <int E, class Tab>
+IPA_HD int ipa_shape_stage(const IpaSetConsts& c, const double (&x)[E], int hmin, int hmax, double (&d)[E], double (&V)[E],
+                           const Tab* tab) {
+  const double mu = c.mu;
 #pragma unroll
   for (int e = 0; e < E; ++e) d[e] = x[e] - mu;
   const bool sane = hmin > 0 && hmax < 0x7ff00000;      // positive, finite events only
@@ -273,18 +279,9 @@ IPA_HD void ipa_member_stage(const IpaSetConsts& c, int region, const double (&d
 
 // One set on its own: the same two stages with the same record, the member stage inlined per region.
 template <int E, class Tab>
-IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l)[E], const Tab* tab) {
+IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], int hmin, int hmax, double (&l)[E], const Tab* tab) {
   double d[E], V[E];
   const double mu = c.mu;
-  int hmin = ipa_hi(x[0]), hmax = hmin;
-#pragma unroll
-  for (int e = 1; e < E; ++e) {
-    const int h = ipa_hi(x[e]);
-    hmin = h < hmin ? h : hmin;
-    hmax = h > hmax ? h : hmax;
-  }
-  hmin = ipa_warp_min(hmin);
-  hmax = ipa_warp_max(hmax);
 #pragma unroll
   for (int e = 0; e < E; ++e) d[e] = x[e] - mu;
   const bool sane = hmin > 0 && hmax < 0x7ff00000;
@@ -301,6 +298,13 @@ IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l
     ipa_mixed_shape<E>(c, d, V, tab);
     ipa_member_stage_r<E, IPA_REG_MIXED>(c, d, V, l, tab);
   }
+}
+
+template <int E, class Tab>
+IPA_HD void ipa_eval_set(const IpaSetConsts& c, const double (&x)[E], double (&l)[E], const Tab* tab) {
+  int hmin, hmax;
+  ipa_warp_hi_range<E>(x, hmin, hmax);
+  ipa_eval_set<E>(c, x, hmin, hmax, l, tab);
 }
 
 __device__ __forceinline__ double ipa_warp_sum(double v) {
@@ -357,7 +361,12 @@ __device__ __forceinline__ double2 ipa_lds128(unsigned smem_addr) {
 
 // Sets of a batch grouped by signal shape: leader[k] = smallest index with the same shape parameters
 // (built on the host by ipa_nll_eval; leader[k] == k for a set on its own).
-struct IpaGroups { signed char leader[IPA_MAX_K]; };
+// The kernel gets them as a schedule: member[first[g] .. first[g+1]) are the sets of group g (ascending), so that the
+// loops of a tile run over groups and members only (a scan of leader[] per group cost 50 instructions per event at K = 9).
+struct IpaGroups {
+  signed char leader[IPA_MAX_K];
+  unsigned char ngroups, first[IPA_MAX_K + 1], member[IPA_MAX_K];
+};
 
 // All K parameter sets on the IPA_NE events a thread holds in registers (A2-A4): one shape stage per
 // group, one member stage per set; optional per-event output; accumulation into the thread's
@@ -408,24 +417,27 @@ __device__ __forceinline__ void ipa_tile_sets(const IpaSetConsts* sc, int K, con
       }
     }
   }
+  int hmin, hmax;
+  ipa_warp_hi_range<IPA_NE>(xv, hmin, hmax);
   if (!GROUPED) {
     for (int k = 0; k < K; ++k) {
       const IpaSetConsts& c = sc[k];
       if (c.status) continue;
       double l[IPA_NE];
-      ipa_eval_set<IPA_NE>(c, xv, l, s_tab);
+      ipa_eval_set<IPA_NE>(c, xv, hmin, hmax, l, s_tab);
       ipa_tile_store_acc<LOGPDF, FULL>(k, l, acc, base, n, tid, logpdf);
     }
   } else {
-    for (int g = 0; g < K; ++g) {
-      if (grp.leader[g] != g) continue;
-      int v = g;                                   // first member with a usable record
-      while (v < K && (grp.leader[v] != g || sc[v].status)) ++v;
-      if (v >= K) continue;
+    const int ng = grp.ngroups;
+    for (int g = 0; g < ng; ++g) {
+      const int mend = grp.first[g + 1];
+      int m = grp.first[g];                        // first member with a usable record
+      while (m < mend && sc[grp.member[m]].status) ++m;
+      if (m >= mend) continue;
       double d[IPA_NE], V[IPA_NE];
-      const int region = ipa_shape_stage<IPA_NE>(sc[v], xv, d, V, s_tab);
-      for (int k = v; k < K; ++k) {
-        if (grp.leader[k] != g) continue;
+      const int region = ipa_shape_stage<IPA_NE>(sc[grp.member[m]], xv, hmin, hmax, d, V, s_tab);
+      for (; m < mend; ++m) {
+        const int k = grp.member[m];
         const IpaSetConsts& c = sc[k];
         if (c.status) continue;
         double l[IPA_NE];
