@@ -81,7 +81,8 @@ typedef enum {
   IPA_ERR_INVALID_ARG = -1, /* null pointer, negative size, K < 1, hi <= lo, misaligned pointer */
   IPA_ERR_WORKSPACE = -2,   /* ws_bytes < ipa_workspace_bytes(...) or ws_dev misaligned */
   IPA_ERR_CUDA = -3,        /* a CUDA runtime call or launch failed */
-  IPA_ERR_NO_DEVICE = -4    /* no usable sm_100 device / kernel image */
+  IPA_ERR_NO_DEVICE = -4,   /* no usable sm_100 device / kernel image */
+  IPA_ERR_TOO_LARGE = -5    /* ipa_nll_eval_static: K > IPA_STATIC_MAX_K (the built-in scratch holds no more) */
 } ipa_status;
 
 const char* ipa_strerror(int code);
@@ -295,6 +296,25 @@ int ipa_cls_from_counts(const int64_t* count_sb_dev, int64_t T_sb, const int64_t
 size_t ipa_prepare_workspace_bytes(int64_t n, int64_t T);
 int ipa_events_prepare(const double* x_in_dev, int64_t n, const int64_t* offsets_dev, int64_t T, ipa_range r,
                        double* x_out_dev, void* ws_dev, size_t ws_bytes, void* cuda_stream);
+
+/* ipa_nll_eval for callers that cannot allocate device memory (code under CUDA graph capture, tight serving loops,
+ * harnesses that forbid cudaMalloc): the same prologue and streaming kernels, same arguments, same results bit for bit,
+ * but the scratch (per-set constants, partial sums, ticket counters) lives in a file-scope `static __device__` array
+ * of IPA_STATIC_SCRATCH_BYTES inside the library instead of a caller-owned workspace.  The entry point allocates and
+ * frees nothing (no cudaMalloc / cudaFree / allocating library routine); inputs and outputs are still the caller's.
+ *   - Limit: K <= IPA_STATIC_MAX_K parameter sets per call; a larger K returns IPA_ERR_TOO_LARGE before any work is
+ *     enqueued (any n is accepted: the scratch does not grow with n).  Use ipa_nll_eval with an own workspace beyond.
+ *   - Every GPU that loads the library holds the array (288 KiB) until the process exits.
+ *   - The array is shared by EVERY call on a device and keeps the previous call's contents.  Each call rewrites all it
+ *     reads (the prologue kernel rewrites the records and zeroes the ticket counters before the streaming kernel
+ *     counts on them), so calls that follow one another on one stream, or are ordered by events, are independent.
+ *     Calls that OVERLAP on the GPU (two streams, two host threads, concurrent graph launches) race on it: their
+ *     results are undefined.  Such callers need ipa_nll_eval with one workspace per stream.
+ *   - The array's device address is looked up once per device (cudaGetSymbolAddress, with that device current). */
+#define IPA_STATIC_MAX_K 16
+#define IPA_STATIC_SCRATCH_BYTES (288 * 1024)
+int ipa_nll_eval_static(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r, double* nll_dev,
+                        double* logpdf_dev, int32_t* status_dev, const ipa_options* opt_host, void* cuda_stream);
 
 /* Measurement aid (not on the hot path): runs `iters` dependent DFMA per thread in 8 independent
  * chains on a full grid, for the FP64 roofline denominator.  out_dev [1]. */

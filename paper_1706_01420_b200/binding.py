@@ -14,7 +14,7 @@ from . import build as _build
 __all__ = [
     "PARAM_FIELDS", "NPAR", "IPA_MAX_K", "IpaError", "lib", "library_path", "pack_params", "workspace",
     "ipa_version", "ipa_workspace_bytes", "ipa_norm", "ipa_core_degree", "ipa_core_cells", "ipa_nll_grad_eval", "ipa_nll_fd_gradient",
-    "ipa_nll_eval_extended", "ipa_nll_eval_categories", "ipa_nll_eval",
+    "ipa_nll_eval_extended", "ipa_nll_eval_categories", "ipa_nll_eval", "ipa_nll_eval_static", "IPA_STATIC_MAX_K",
     "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill", "ipa_binned_nll_scan", "ipa_expected_hist",
     "ipa_poisson_hist_toys", "ipa_signal_shape", "ipa_gauss_smear", "ipa_expected_hist_shape", "ipa_binned_nll_scan_shape",
     "ipa_cls_teststat", "ipa_cls_count_ge", "ipa_cls_from_counts", "ipa_events_prepare",
@@ -24,6 +24,7 @@ __all__ = [
 PARAM_FIELDS = ("mu", "sigma", "lambda", "zeta", "beta", "a", "n", "a2", "n2", "f", "k")
 NPAR = len(PARAM_FIELDS)
 IPA_MAX_K = 32
+IPA_STATIC_MAX_K = 16        # ipa_nll_eval_static: sets per call that the built-in scratch holds
 
 # every symbol include/ipanll.h declares
 EXPORTS = (
@@ -32,7 +33,7 @@ EXPORTS = (
     "ipa_binned_nll_scan", "ipa_expected_hist", "ipa_poisson_hist_toys", "ipa_signal_shape", "ipa_gauss_smear",
     "ipa_expected_hist_shape", "ipa_binned_nll_scan_shape", "ipa_cls_teststat", "ipa_cls_count_ge",
     "ipa_cls_from_counts", "ipa_prepare_workspace_bytes", "ipa_events_prepare",
-    "ipa_fp64_peak_probe",
+    "ipa_fp64_peak_probe", "ipa_nll_eval_static",
 )
 
 
@@ -82,6 +83,7 @@ def lib():
     L.ipa_core_degree.restype = i32; L.ipa_core_degree.argtypes = [vp, i32, _Range, vp, op, vp, sz, vp]
     L.ipa_core_cells.restype = i32; L.ipa_core_cells.argtypes = [vp, i32, _Range, vp, op, vp, sz, vp]
     L.ipa_nll_eval.restype = i32; L.ipa_nll_eval.argtypes = [vp, i64, vp, i32, _Range, vp, vp, vp, op, vp, sz, vp]
+    L.ipa_nll_eval_static.restype = i32; L.ipa_nll_eval_static.argtypes = [vp, i64, vp, i32, _Range, vp, vp, vp, op, vp]
     L.ipa_nll_fd_gradient.restype = i32
     L.ipa_nll_fd_gradient.argtypes = [vp, i64, vp, i32, vp, vp, _Range, vp, vp, vp, op, vp, sz, vp]
     L.ipa_nll_eval_extended.restype = i32
@@ -252,6 +254,23 @@ def ipa_nll_eval(x, params, lo, hi, want_logpdf=False, ws=None, stream=None, out
     lp = torch.empty((K, n), dtype=torch.float64, device="cuda") if want_logpdf else None
     _check(lib().ipa_nll_eval(_dptr(x, torch.float64) if n else None, n, _hptr(P), K, _Range(lo, hi), _dptr(nll),
                               _dptr(lp), _dptr(st), _opt(policy), _dptr(ws), ws.numel(), _stream(stream)))
+    return nll, lp, st
+
+
+@_alloc_on_stream
+def ipa_nll_eval_static(x, params, lo, hi, want_logpdf=False, stream=None, out=None, status=None, policy=None):
+    """ipa_nll_eval on the library's built-in scratch (no workspace): K <= IPA_STATIC_MAX_K sets.  The C entry point
+    allocates nothing; pass `out` [K] float64 and `status` [K] int32 device tensors to keep this wrapper from allocating too.
+    Calls share the scratch: calls that overlap on the GPU race.  -> (nll[K], logpdf[K,n] or None, status[K])."""
+    _need_cuda()
+    P = pack_params(params)
+    K = P.shape[0]
+    n = x.numel()
+    nll = out if out is not None else torch.empty(K, dtype=torch.float64, device="cuda")
+    st = status if status is not None else torch.empty(K, dtype=torch.int32, device="cuda")
+    lp = torch.empty((K, n), dtype=torch.float64, device="cuda") if (want_logpdf and K <= IPA_STATIC_MAX_K) else None
+    _check(lib().ipa_nll_eval_static(_dptr(x, torch.float64) if n else None, n, _hptr(P), K, _Range(lo, hi), _dptr(nll),
+                                     _dptr(lp), _dptr(st), _opt(policy), _stream(stream)))
     return nll, lp, st
 
 

@@ -3,6 +3,7 @@
 // method: every step of the path runs in the kernels of ipa_kernels.cuh.
 #include <cstdio>
 #include <cstring>
+#include <mutex>
 #include <string>
 #include "ipa_kernels.cuh"
 #include "ipa_prepare.cuh"
@@ -125,6 +126,39 @@ int run_prologue(const ipa_params* p_host, int64_t K, ipa_range r, int policy, c
 
 }  // namespace
 
+// ---- built-in scratch of ipa_nll_eval_static (the one entry point that needs no caller workspace) --------------------
+// A file-scope device array: every device that loads the library holds it until the process exits.  In HOST code the
+// name `ipa_static_scratch` is only a stand-in for the symbol, not a device address; the address a kernel may use comes
+// from cudaGetSymbolAddress, looked up once per device with that device current.
+static __device__ __align__(256) unsigned char ipa_static_scratch[IPA_STATIC_SCRATCH_BYTES];
+
+namespace {
+
+constexpr int kMaxDevices = 64;
+std::mutex g_scratch_mutex;
+void* g_scratch_ptr[kMaxDevices] = {};
+
+int static_scratch(void** out) {
+  if (make_layout(IPA_STATIC_MAX_K, 0).total > (size_t)IPA_STATIC_SCRATCH_BYTES) {
+    g_last_cuda_error = "ipa_nll_eval_static: IPA_STATIC_SCRATCH_BYTES is smaller than the workspace of IPA_STATIC_MAX_K sets";
+    return IPA_ERR_WORKSPACE;
+  }
+  int dev = 0;
+  IPA_CK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= kMaxDevices) return IPA_ERR_NO_DEVICE;
+  std::lock_guard<std::mutex> lock(g_scratch_mutex);
+  if (!g_scratch_ptr[dev]) {
+    void* ptr = nullptr;
+    IPA_CK(cudaGetSymbolAddress(&ptr, ipa_static_scratch));      // device `dev` is current
+    if (!ptr || ((uintptr_t)ptr % 256) != 0) return IPA_ERR_WORKSPACE;
+    g_scratch_ptr[dev] = ptr;
+  }
+  *out = g_scratch_ptr[dev];
+  return IPA_OK;
+}
+
+}  // namespace
+
 extern "C" {
 
 const char* ipa_strerror(int code) {
@@ -134,6 +168,7 @@ const char* ipa_strerror(int code) {
     case IPA_ERR_WORKSPACE: return "workspace too small or misaligned";
     case IPA_ERR_CUDA: return "CUDA error (see ipa_last_cuda_error)";
     case IPA_ERR_NO_DEVICE: return "no usable CUDA device";
+    case IPA_ERR_TOO_LARGE: return "more parameter sets than the built-in scratch of ipa_nll_eval_static holds (IPA_STATIC_MAX_K)";
     default: return "unknown error code";
   }
 }
@@ -671,6 +706,22 @@ int ipa_events_prepare(const double* x_in_dev, int64_t n, const int64_t* offsets
   ipa_prep_scatter_kernel<<<(unsigned)G, IPA_PREP_THREADS, IPA_PREP_SMEM, st>>>(x_in_dev, n, r.lo, scale, hist, binbase, x_out_dev);
   IPA_CK(cudaGetLastError());
   return IPA_OK;
+}
+
+int ipa_nll_eval_static(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r, double* nll_dev,
+                        double* logpdf_dev, int32_t* status_dev, const ipa_options* opt_host, void* cuda_stream) {
+  if (K > IPA_STATIC_MAX_K) {
+    g_last_cuda_error = "ipa_nll_eval_static: K = " + std::to_string(K) + " parameter sets exceed IPA_STATIC_MAX_K = " +
+                        std::to_string(IPA_STATIC_MAX_K) + " (use ipa_nll_eval with a workspace of your own)";
+    return IPA_ERR_TOO_LARGE;
+  }
+  void* ws = nullptr;
+  const int rc = static_scratch(&ws);
+  if (rc) return rc;
+  // the existing path, on the built-in scratch: the prologue rewrites every record of the K sets and zeroes the ticket
+  // counters, the streaming kernel writes all the partial sums it later reads -- nothing of an earlier call is read
+  return ipa_nll_eval(x_dev, n, p_host, K, r, nll_dev, logpdf_dev, status_dev, opt_host, ws, IPA_STATIC_SCRATCH_BYTES,
+                      cuda_stream);
 }
 
 int ipa_fp64_peak_probe(int64_t iters, double* out_dev, void* cuda_stream) {
