@@ -233,7 +233,8 @@ int ipa_hist_fill(const double* x_dev, int64_t n, ipa_range r, int nbins, uint64
  *   s_b = I(c_b - mu) / sum_b' I(c_b' - mu),  b_b = e^{k c_b} / sum_b' e^{k c_b'}  at bin centres c_b,
  *   nu_b = ns s_b + nb b_b,   NLL = sum_b [ nu_b - n_b log nu_b ]   (n_b = 0: nu_b).
  *   counts_dev [nbins]; shape_host: one parameter set (its f and k are ignored);
- *   ns_host, nb_host, k_host [npoints]; nll_dev [npoints] out. */
+ *   ns_host, nb_host, k_host [npoints] (three uploads; ONE if the arrays lie back to back in host memory, ns then nb then k,
+ *   as the Python binding packs them); nll_dev [npoints] out. */
 int ipa_binned_nll_scan(const uint64_t* counts_dev, int nbins, ipa_range r, const ipa_params* shape_host,
                         const double* ns_host, const double* nb_host, const double* k_host, int64_t npoints,
                         double* nll_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes, void* cuda_stream);

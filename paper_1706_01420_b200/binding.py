@@ -395,11 +395,18 @@ def ipa_hist_fill(x, lo, hi, nbins, stream=None):
 
 
 @_alloc_on_stream
+def _pack_points(ns, nb, k):
+    """The three scan-point arrays back to back in one host buffer: the library then uploads them with one copy."""
+    ns = np.asarray(ns, dtype=np.float64).ravel()
+    buf = np.empty((3, ns.size), dtype=np.float64)
+    buf[0], buf[1], buf[2] = ns, np.asarray(nb, dtype=np.float64).ravel(), np.asarray(k, dtype=np.float64).ravel()
+    return buf[0], buf[1], buf[2]
+
+
 def ipa_binned_nll_scan(counts, lo, hi, shape, ns, nb, k, ws=None, stream=None, policy=None):
     _need_cuda()
     P = pack_params(shape)
-    ns = np.ascontiguousarray(ns, dtype=np.float64); nb = np.ascontiguousarray(nb, dtype=np.float64)
-    k = np.ascontiguousarray(k, dtype=np.float64)
+    ns, nb, k = _pack_points(ns, nb, k)
     npts, nbins = ns.size, counts.numel()
     ws = _ws(ws, 0, npts, nbins)
     out = torch.empty(npts, dtype=torch.float64, device="cuda")
@@ -467,8 +474,7 @@ def ipa_expected_hist_shape(sig, lo, hi, ns, nb, k, ws=None, stream=None):
 @_alloc_on_stream
 def ipa_binned_nll_scan_shape(counts, lo, hi, sig, ns, nb, k, ws=None, stream=None):
     _need_cuda()
-    ns = np.ascontiguousarray(ns, dtype=np.float64); nb = np.ascontiguousarray(nb, dtype=np.float64)
-    k = np.ascontiguousarray(k, dtype=np.float64)
+    ns, nb, k = _pack_points(ns, nb, k)
     npts, nbins = ns.size, counts.numel()
     ws = _ws(ws, 0, npts, nbins)
     out = torch.empty(npts, dtype=torch.float64, device="cuda")

@@ -512,10 +512,15 @@ static int binned_common(const uint64_t* counts_dev, int nbins, ipa_range r, con
                                                flag, 1);
   }
   IPA_CK(cudaGetLastError());
-  IPA_CK(cudaMemcpyAsync(pts, ns_host, (size_t)npoints * 8, cudaMemcpyHostToDevice, st));
-  IPA_CK(cudaMemcpyAsync(pts + npoints, nb_host, (size_t)npoints * 8, cudaMemcpyHostToDevice, st));
-  IPA_CK(cudaMemcpyAsync(pts + 2 * npoints, k_host, (size_t)npoints * 8, cudaMemcpyHostToDevice, st));
-  ipa_binned_scan_kernel<<<(unsigned)npoints, 256, 0, st>>>(reinterpret_cast<const unsigned long long*>(counts_dev), sbin,
+  if (nb_host == ns_host + npoints && k_host == nb_host + npoints) {
+    // the three arrays lie back to back in host memory (the Python binding packs them so): one upload instead of three
+    IPA_CK(cudaMemcpyAsync(pts, ns_host, (size_t)npoints * 24, cudaMemcpyHostToDevice, st));
+  } else {
+    IPA_CK(cudaMemcpyAsync(pts, ns_host, (size_t)npoints * 8, cudaMemcpyHostToDevice, st));
+    IPA_CK(cudaMemcpyAsync(pts + npoints, nb_host, (size_t)npoints * 8, cudaMemcpyHostToDevice, st));
+    IPA_CK(cudaMemcpyAsync(pts + 2 * npoints, k_host, (size_t)npoints * 8, cudaMemcpyHostToDevice, st));
+  }
+  ipa_binned_scan_kernel<<<(unsigned)npoints, IPA_SCAN_THREADS, 0, st>>>(reinterpret_cast<const unsigned long long*>(counts_dev), sbin,
                                                             nbins, r.lo, r.hi, pts, pts + npoints, pts + 2 * npoints, flag,
                                                             nll_dev, nu_dev);
   IPA_CK(cudaGetLastError());
