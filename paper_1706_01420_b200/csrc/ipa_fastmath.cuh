@@ -100,8 +100,20 @@ IPA_HD double ipa_fsqrt(double q) {
   return fma(g, p, g);
 }
 
-// 1/u, u > 0 normal: reciprocal seed (about 20 good bits, MUFU.RCP64H on the device) + two Newton steps.
-IPA_HD double ipa_frcp(double u) {
+// sqrt(q) and 1/sqrt(q) from the same third-order step: 1/sqrt(q) = y (1 + p), one more FMA (the gradient kernel needs
+// d/r beside r; a separate reciprocal of r cost a second seed and four FMAs)
+IPA_HD double ipa_fsqrt_rsqrt(double q, double* rinv) {
+  const double y = ipa_rsqrt_seed(q);
+  const double g = q * y;
+  const double e = fma(-g, y, 1.0);
+  const double p = fma(0.375, e, 0.5) * e;
+  *rinv = fma(y, p, y);
+  return fma(g, p, g);
+}
+
+// 1/u, u > 0 normal: reciprocal seed (about 20 good bits, MUFU.RCP64H on the device) + ONE third-order step,
+// y (1 + e + e^2), e = 1 - u y: the error e^3 is below 2^-58 (two Newton steps took one FMA more).
+IPA_HD double ipa_frcp3(double u) {
 #ifdef __CUDA_ARCH__
   double y;
   asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(u));
@@ -109,10 +121,8 @@ IPA_HD double ipa_frcp(double u) {
   double y = 1.0 / u;
   y = ipa_mk(ipa_hi(y), 0);
 #endif
-  double e = fma(-u, y, 1.0);
-  y = fma(y, e, y);
-  e = fma(-u, y, 1.0);
-  return fma(y, e, y);
+  const double e = fma(-u, y, 1.0);
+  return fma(y, fma(e, e, e), y);
 }
 
 // e^a for a <= 0 (|a| is clamped to about 64 by the caller or here: results below 1e-27 are not

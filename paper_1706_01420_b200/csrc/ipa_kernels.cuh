@@ -581,8 +581,8 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
 template <class Tab>
 IPA_HD void ipa_grad_core(const IpaSetConsts& c, double d, double& D, double& dd, double& ds) {
   const double q = fma(d, d, c.delta2);
-  const double r = ipa_fsqrt(q);
-  const double rinv = ipa_frcp(r);
+  double rinv;
+  const double r = ipa_fsqrt_rsqrt(q, &rinv);
   const double t = fma(c.tA, r, c.tB);
   double P = 0.0, Pd = 0.0;
   for (int j = 4 * (c.degree >> 2) + 3; j >= 0; --j) {
@@ -598,13 +598,13 @@ template <class Tab>
 IPA_HD void ipa_grad_tail(const IpaSetConsts& c, bool right, double d, double& D, double& dd, double& ds, double& db,
                           const Tab* tab) {
   if (!right) {
-    const double u = fma(c.uA0, d, c.uB0), ru = ipa_frcp(u);
+    const double u = fma(c.uA0, d, c.uB0), ru = ipa_frcp3(u);
     D = fma(-c.kd, d, fma(-c.n0, ipa_flog_t(u, tab), c.cT0));
     dd = c.L0 * ru;
     ds = fma(fma(-(d - c.d0), c.c0s, c.aL0), ru, c.A0);
     db = fma(d - c.d0, ru, c.d0);
   } else {
-    const double u = fma(c.uA1, d, c.uB1), ru = ipa_frcp(u);
+    const double u = fma(c.uA1, d, c.uB1), ru = ipa_frcp3(u);
     D = fma(-c.kd, d, fma(-c.n1, ipa_flog_t(u, tab), c.cT1));
     dd = c.L1 * ru;
     ds = fma(-fma(d - c.d1, c.c1s, c.a2L1), ru, c.A1);
@@ -617,11 +617,10 @@ IPA_HD void ipa_grad_mix(const IpaSetConsts& c, double d, double D, double dd, d
                          double& gs, double& gf, double& gk, double& gb, const Tab* tab) {
   const double w = ipa_fexp_negabs_t(D, tab);
   const double s1 = 1.0 + w;
-  const double rs = ipa_frcp(s1);
+  const double rs = ipa_frcp3(s1);
   const bool pos = ipa_hi(D) >= 0;
   const double wS = pos ? rs : w * rs, wB = pos ? w * rs : rs;
-  l = fma(c.kd, d, c.eB0) + ipa_flog12_t(s1, tab);
-  if (pos) l += D;
+  l = fma(0.5, D + fabs(D), fma(c.kd, d, c.eB0) + ipa_flog12_t(s1, tab));   // + max(D, 0), exact (ipa_fsoftplus_add_t)
   gm = wS * (-dd - c.dlnNS_dmu);
   gs = wS * (ds - c.dlnNS_dsig);
   gf = fma(wS, c.invf, -wB * c.inv1mf);
@@ -663,8 +662,7 @@ IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&
     double t[E], rinv[E], P[E], Pd[E];
 #pragma unroll
     for (int e = 0; e < E; ++e) {
-      const double r = ipa_fsqrt(fma(d[e], d[e], c.delta2));
-      rinv[e] = ipa_frcp(r);
+      const double r = ipa_fsqrt_rsqrt(fma(d[e], d[e], c.delta2), &rinv[e]);
       t[e] = fma(tA, r, tB);
       P[e] = 0.0;
       Pd[e] = 0.0;
@@ -699,7 +697,7 @@ IPA_HD void ipa_eval_grad(const IpaSetConsts& c, const double (&x)[E], double (&
       else if (c.mode == 0) ipa_grad_core<Tab>(c, d[e], D[e], dd[e], ds[e]);
       else if (c.mode == 2) {   // Student-t core: log G = nu log q + beta d, L - beta = 2 nu d / q
         const double q = fma(d[e], d[e], c.delta2);
-        const double Lmb = 2.0 * c.nu * d[e] * ipa_frcp(q);
+        const double Lmb = 2.0 * c.nu * d[e] * ipa_frcp3(q);
         D[e] = fma(c.bmk, d[e], fma(c.nu, ipa_flog_t(q, tab), c.a[0]));
         dd[e] = c.beta + Lmb;
         ds[e] = fma(-d[e] * c.invsig, Lmb, c.nuosig);

@@ -114,6 +114,10 @@ long long emu_poisson(unsigned long long seed, unsigned long long slot, unsigned
 
 // ---- the streaming kernels' own sqrt / exp / log (csrc/ipa_fastmath.cuh) ---------------------------
 extern "C" {
+void emu_frcp3(const double* u, long long n, double* out) { for (long long i = 0; i < n; ++i) out[i] = ipa_frcp3(u[i]); }
+void emu_fsqrt_rsqrt(const double* q, long long n, double* r, double* rinv) {
+  for (long long i = 0; i < n; ++i) r[i] = ipa_fsqrt_rsqrt(q[i], &rinv[i]);
+}
 void emu_fsqrt(const double* q, long long n, double* out) { for (long long i = 0; i < n; ++i) out[i] = ipa_fsqrt(q[i]); }
 void emu_fexp_neg(const double* a, long long n, double* out) {
   for (long long i = 0; i < n; ++i) out[i] = ipa_fexp_neg(ipa_neg_abs_clamped(a[i]));

@@ -305,6 +305,15 @@ def test_device_fastmath_vs_mpmath(emu):
     q = np.concatenate([10.0 ** rng.uniform(-3, 8, 4000), [1.0, 2.0, 4.0, 83.349, 983.0, 1e-300, 1e300]])
     got = run("emu_fsqrt", q)
     assert max(abs(mp.mpf(float(g)) / mp.sqrt(mp.mpf(float(v))) - 1) for g, v in zip(got, q)) <= 2e-16
+    # gradient kernel: 1/u by one third-order step, sqrt and 1/sqrt from one step (<= 2.5e-16 relative each)
+    emu.emu_frcp3.restype = None
+    emu.emu_fsqrt_rsqrt.restype = None
+    got = run("emu_frcp3", q)
+    assert max(abs(mp.mpf(float(g)) * mp.mpf(float(v)) - 1) for g, v in zip(got, q)) <= 2.5e-16
+    r, ri = np.empty_like(q), np.empty_like(q)
+    emu.emu_fsqrt_rsqrt(q.ctypes.data_as(vp), C.c_longlong(q.size), r.ctypes.data_as(vp), ri.ctypes.data_as(vp))
+    assert max(abs(mp.mpf(float(g)) / mp.sqrt(mp.mpf(float(v))) - 1) for g, v in zip(r, q)) <= 2e-16
+    assert max(abs(mp.mpf(float(g)) * mp.sqrt(mp.mpf(float(v))) - 1) for g, v in zip(ri, q)) <= 2.5e-16
     D = np.concatenate([rng.uniform(-60, 60, 6000), rng.uniform(-1, 1, 2000) * 1e-3, [0.0, -0.0, 1e-300, 700.0, -745.0, 1.0e4, -1.0e4,
                                                                                      4.9e6, np.log(2) / 512, -np.log(2) / 512]])
     got = run("emu_fexp_negabs_t", D)
