@@ -284,14 +284,23 @@ IPA_HD double ipa_flog_t(double u, const double* mt) {
 
 // e^{-|D|}, any D with |D| < 5e6 (beyond that the integer part of -|D| 256/ln2 leaves 32 bits; the largest |Delta|
 // the kernels produce on purpose is the f == 0 sentinel, 1e4).  9 FP64.
+// COARSE: the reduction r = a - m ln2/256 in ONE step with ln2/256 rounded to fp64 (the product is exact inside the FMA, so
+// the only error is m times the representation error of the constant, < |a| 8e-17 relative in the result).  For the
+// softplus, where the result w enters as log(1 + w), that is an absolute error below |a| e^{-|a|} 8e-17 < 3e-17: 8 FP64.
+template <bool COARSE = false>
 IPA_HD double ipa_fexp_negabs_t(double D, const double* mt) {
   const double SHIFT = 6755399441055744.0;
   const double a = -fabs(D);
   const double t = fma(a, IPA_LOG2E_256, SHIFT);
   int m = ipa_lo(t);                                    // round(a 256 / ln 2) = 256 n + j
   const double nf = t - SHIFT;
-  double r = fma(nf, -IPA_LN2_256_HI, a);
-  r = fma(nf, -IPA_LN2_256_LO, r);
+  double r;
+  if (COARSE) {
+    r = fma(nf, -(IPA_LN2_256_HI + IPA_LN2_256_LO), a);
+  } else {
+    r = fma(nf, -IPA_LN2_256_HI, a);
+    r = fma(nf, -IPA_LN2_256_LO, r);
+  }
   const double T = ipa_mt_d(mt, 16u + (((unsigned)m & 255u) << 3));
   double q = fma(IPA_CEXPQ(3), r, IPA_CEXPQ(2));
   q = fma(q, r, IPA_CEXPQ(1));
@@ -312,6 +321,6 @@ IPA_HD double ipa_fexp_negabs_t(double D, const double* mt) {
 // predicated add into an unconditional one plus two FSEL: 4 issue slots against 2 FP64 instructions here).
 // (Folding D/2 + |D|/2 into the two FMAs of the sum instead cancels for D << 0: 3.5e-15 at D = -52 -- rejected.)
 IPA_HD double ipa_fsoftplus_add_t(double eb, double D, const double* mt) {
-  const double w = ipa_fexp_negabs_t(D, mt);
+  const double w = ipa_fexp_negabs_t<true>(D, mt);
   return fma(0.5, D + fabs(D), eb + ipa_flog12_t(1.0 + w, mt));
 }
