@@ -279,10 +279,21 @@ int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K
                            : (grouped ? ipa_nll_kernel<false, true> : ipa_nll_kernel<false, false>);
     if (kb == 1 && !logpdf_dev) kern = ipa_nll_kernel<false, false, true>;
     const size_t smem = (size_t)kb * (sizeof(IpaSetConsts) + IPA_NB * 8) + 2 * IPA_NTILE * 8;
-    kern<<<(unsigned)G, IPA_NB, smem, st>>>(x_dev, n, vec_ok, consts + k0, kb, grp, partials + (size_t)k0 * G,
-                                            logpdf_dev ? logpdf_dev + (size_t)k0 * n : nullptr, counter + b, nll_dev + k0,
-                                            status_dev ? status_dev + k0 : nullptr);
-    IPA_CK(cudaGetLastError());
+    // the first launch is a programmatic dependent of the prologue kernel enqueued just before it: its blocks load the
+    // math table and their first tile while the prologue runs, and wait for its end before they read the records
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3((unsigned)G);
+    cfg.blockDim = dim3(IPA_NB);
+    cfg.dynamicSmemBytes = smem;
+    cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = (b == 0) ? 1 : 0;
+    IPA_CK(cudaLaunchKernelEx(&cfg, kern, x_dev, (long long)n, vec_ok, consts + k0, kb, grp, partials + (size_t)k0 * G,
+                              logpdf_dev ? logpdf_dev + (size_t)k0 * n : (double*)nullptr, counter + b, nll_dev + k0,
+                              status_dev ? status_dev + k0 : (int32_t*)nullptr));
   }
   return IPA_OK;
 }
@@ -345,9 +356,9 @@ int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, 
   if (rc) return rc;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   char* ws = static_cast<char*>(ws_dev);
-  rc = run_prologue(p_host, K, r, policy, ws, L, nullptr, nullptr, nullptr, st, true);
-  if (rc) return rc;
   IPA_CK(cudaMemsetAsync(ws + L.counter, 0, 256, st));          // one ticket counter per group of IPA_GKB sets
+  rc = run_prologue(p_host, K, r, policy, ws, L, nullptr, nullptr, nullptr, st, true);   // (zeroes the first two again)
+  if (rc) return rc;
   const int64_t ntiles = (n + IPA_GTILE - 1) / IPA_GTILE;
   int64_t G = (int64_t)sms;
   if (G > ntiles) G = ntiles;
@@ -356,10 +367,20 @@ int ipa_nll_grad_eval(const double* x_dev, int64_t n, const ipa_params* p_host, 
   const int vec_ok = ((uintptr_t)x_dev % 16) == 0;
   const int groups = (K + IPA_GKB - 1) / IPA_GKB;
   auto kern = (K == 1) ? ipa_nll_grad_kernel<true> : ipa_nll_grad_kernel<false>;
-  kern<<<dim3((unsigned)G, (unsigned)groups), IPA_GB, kGradSmem, st>>>(
-      x_dev, n, vec_ok, reinterpret_cast<const IpaSetConsts*>(ws + L.consts), K, reinterpret_cast<double*>(ws + L.partials),
-      reinterpret_cast<unsigned int*>(ws + L.counter), nll_dev, grad_dev, status_dev);
-  IPA_CK(cudaGetLastError());
+  // programmatic dependent of the prologue kernel just before it (as the streaming kernel of ipa_nll_eval)
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)G, (unsigned)groups);
+  cfg.blockDim = dim3(IPA_GB);
+  cfg.dynamicSmemBytes = kGradSmem;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  IPA_CK(cudaLaunchKernelEx(&cfg, kern, x_dev, (long long)n, vec_ok, reinterpret_cast<const IpaSetConsts*>(ws + L.consts), K,
+                            reinterpret_cast<double*>(ws + L.partials), reinterpret_cast<unsigned int*>(ws + L.counter),
+                            nll_dev, grad_dev, status_dev));
   return IPA_OK;
 }
 
@@ -378,8 +399,6 @@ static int segmented_common(const double* x_dev, const int64_t* offsets_dev, int
   if (!ws_ok(ws_dev, ws_bytes, L.total)) return IPA_ERR_WORKSPACE;
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   char* ws = static_cast<char*>(ws_dev);
-  int rc = run_prologue(p_host, K, r, policy, ws, L, nullptr, nullptr, nullptr, st);
-  if (rc) return rc;
   const IpaSetConsts* consts = reinterpret_cast<const IpaSetConsts*>(ws + L.consts);
   double* partials = reinterpret_cast<double*>(ws + L.partials);
   const int* map = nullptr;
@@ -387,6 +406,9 @@ static int segmented_common(const double* x_dev, const int64_t* offsets_dev, int
     IPA_CK(cudaMemcpyAsync(ws + L.nsig, set_of_segment_host, (size_t)T * 4, cudaMemcpyHostToDevice, st));
     map = reinterpret_cast<const int*>(ws + L.nsig);
   }
+  // (the copy above comes first so that the segmented kernel directly follows the prologue: programmatic dependent launch)
+  int rc = run_prologue(p_host, K, r, policy, ws, L, nullptr, nullptr, nullptr, st);
+  if (rc) return rc;
   // chunks per segment: IPA_SEGC, more when few segments would leave SMs idle (T * C >= resident blocks of the device)
   int sms = 0;
   rc = device_info(&sms);
@@ -395,9 +417,18 @@ static int segmented_common(const double* x_dev, const int64_t* offsets_dev, int
   const int64_t resident = (int64_t)sms * IPA_BLOCKS_PER_SM;
   if (T * C < resident) C = (resident + T - 1) / T;
   if (C > 64) C = 64;
-  ipa_nll_seg_kernel<<<dim3((unsigned)T, (unsigned)C), IPA_BLOCK, 0, st>>>(
-      x_dev, reinterpret_cast<const long long*>(offsets_dev), consts, map, partials);
-  IPA_CK(cudaGetLastError());
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3((unsigned)T, (unsigned)C);
+  cfg.blockDim = dim3(IPA_BLOCK);
+  cfg.dynamicSmemBytes = 0;
+  cfg.stream = st;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  attr[0].val.programmaticStreamSerializationAllowed = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  IPA_CK(cudaLaunchKernelEx(&cfg, ipa_nll_seg_kernel, x_dev, reinterpret_cast<const long long*>(offsets_dev), consts, map,
+                            partials));
   ipa_seg_finalize_kernel<<<(unsigned)((T + 127) / 128), 128, 0, st>>>(partials, consts, map, T, (int)C, nll_dev, status_dev);
   IPA_CK(cudaGetLastError());
   return IPA_OK;

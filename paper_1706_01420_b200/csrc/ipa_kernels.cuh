@@ -16,6 +16,11 @@
 
 struct IpaParamBatch { ipa_params p[IPA_MAX_K]; };
 
+// programmatic dependent launch (sm_90+): wait for the grid this one depends on / allow the dependent grid to start
+__device__ __forceinline__ void ipa_grid_dependency_wait() { asm volatile("griddepcontrol.wait;" ::: "memory"); }
+__device__ __forceinline__ void ipa_launch_dependents() { asm volatile("griddepcontrol.launch_dependents;" ::: "memory"); }
+
+
 // ------------------------------------------------------------------------------------------------
 // Prologue: one block per parameter set.
 // ------------------------------------------------------------------------------------------------
@@ -25,6 +30,7 @@ ipa_prologue_kernel(const __grid_constant__ IpaParamBatch batch, const ipa_param
                     double* norm_sig, double* norm_bkg, int32_t* status_out) {
   __shared__ IpaProWork w;
   const int tid = threadIdx.x, set = blockIdx.x;
+  ipa_launch_dependents();      // a dependent streaming kernel may start its own preamble now; it waits for this grid's end
   if (tid == 0) {
     w.p = p_dev ? p_dev[set] : batch.p[set];
     w.lo = lo; w.hi = hi; w.policy = policy & 1; w.want_grad = (policy >> 1) & 1;
@@ -480,12 +486,18 @@ ipa_nll_kernel(const double* __restrict__ x, long long n, int vec_ok, const IpaS
   }
   ipa_cp_async_commit();
   {
+    for (int k = 0; k < K; ++k) acc[k * IPA_NB + tid] = 0.0;
+    ipa_load_mathtab(s_tab);
+    // Everything above is independent of the prologue.  The kernel is launched as a programmatic dependent of the
+    // prologue kernel (ipa_api.cu): its blocks may start while the prologue still runs and wait HERE until the prologue
+    // grid has completed and its writes (records, ticket counters) are visible.  Launched without the attribute the wait
+    // is a no-op.  The records are read through L2 (no line of them can be in this SM's L1, but the read-only path is
+    // not a promise).
+    ipa_grid_dependency_wait();
     const int nd = K * (int)(sizeof(IpaSetConsts) / 8);
     const double* csrc = reinterpret_cast<const double*>(consts);
     double* dst = reinterpret_cast<double*>(sc);
-    for (int i = tid; i < nd; i += IPA_NB) dst[i] = csrc[i];
-    for (int k = 0; k < K; ++k) acc[k * IPA_NB + tid] = 0.0;
-    ipa_load_mathtab(s_tab);
+    for (int i = tid; i < nd; i += IPA_NB) dst[i] = __ldcg(csrc + i);
   }
   __syncthreads();
   unsigned bufoff = 0;
@@ -758,12 +770,13 @@ ipa_nll_grad_kernel(const double* __restrict__ x, long long n, int vec_ok, const
   }
   ipa_cp_async_commit();
   {
+    for (int i = 0; i < nk * IPA_GQ; ++i) acc[i * IPA_GB + tid] = 0.0;
+    ipa_load_mathtab(s_tab);
+    ipa_grid_dependency_wait();          // the prologue's records from here on (see ipa_nll_kernel)
     const int nd = nk * (int)(sizeof(IpaSetConsts) / 8);
     const double* csrc = reinterpret_cast<const double*>(consts + k0);
     double* dst = reinterpret_cast<double*>(sc);
-    for (int i = tid; i < nd; i += IPA_GB) dst[i] = csrc[i];
-    for (int i = 0; i < nk * IPA_GQ; ++i) acc[i * IPA_GB + tid] = 0.0;
-    ipa_load_mathtab(s_tab);
+    for (int i = tid; i < nd; i += IPA_GB) dst[i] = __ldcg(csrc + i);
   }
   __syncthreads();
   if (tid < nk) {
@@ -915,11 +928,12 @@ ipa_nll_seg_kernel(const double* __restrict__ x, const long long* __restrict__ o
   }
   ipa_cp_async_commit();
   {
+    ipa_load_mathtab(s_tab);
+    ipa_grid_dependency_wait();          // the prologue's records from here on (see ipa_nll_kernel)
     // categories may share a parameter set (set_of_segment != NULL): segment t uses record set_of_segment[t]
     const double* csrc = reinterpret_cast<const double*>(consts + (set_of_segment ? set_of_segment[t] : t));
     double* dst = reinterpret_cast<double*>(&c);
-    for (int i = tid; i < (int)(sizeof(IpaSetConsts) / 8); i += IPA_BLOCK) dst[i] = csrc[i];
-    ipa_load_mathtab(s_tab);
+    for (int i = tid; i < (int)(sizeof(IpaSetConsts) / 8); i += IPA_BLOCK) dst[i] = __ldcg(csrc + i);
   }
   __syncthreads();
   double acc = 0.0;
