@@ -263,16 +263,26 @@ def other_rows(torch, ipa, x, ws, stream, n, p_core):
     for name, d in inp.FIT_START_SHIFT.items():
         th0[inp.IDX[name]] += d
 
-    def nll_batch(th):
+    def nll_batch_plain(th):                                    # the general-purpose wrapper: tensors allocated per call
         return ipa.ipa_nll_eval(x2, th, LO, HI, ws=ws2, stream=stream)[0].cpu().numpy()
+    minimiser.minimise(nll_batch_plain, th0, inp.FLOATED, inp.FD_STEPS, inp.GRAD_SCALE)
+    torch.cuda.synchronize()
+    t0 = time.perf_counter()
+    minimiser.minimise(nll_batch_plain, th0, inp.FLOATED, inp.FD_STEPS, inp.GRAD_SCALE)
+    wall_plain = time.perf_counter() - t0
+    ev = ipa.NllEvaluator(x2, LO, HI, stream=stream)            # the fit loop's evaluator: buffers allocated once
+
+    def nll_batch(th):
+        return ev(th)
     minimiser.minimise(nll_batch, th0, inp.FLOATED, inp.FD_STEPS, inp.GRAD_SCALE)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
     res = minimiser.minimise(nll_batch, th0, inp.FLOATED, inp.FD_STEPS, inp.GRAD_SCALE)
     wall = time.perf_counter() - t0
+
     def grad_batch(th):
-        nll, g, _ = ipa.ipa_nll_grad_eval(x2, th, LO, HI, ws=ws2, stream=stream)
-        return nll.cpu().numpy(), g.cpu().numpy()[:, :4]
+        nll, g = ev.gradient(th)
+        return nll, g[:, :4]
     minimiser.minimise(nll_batch, th0, inp.FLOATED, inp.FD_STEPS, inp.GRAD_SCALE, grad_batch=grad_batch)
     torch.cuda.synchronize()
     t0 = time.perf_counter()
@@ -282,7 +292,7 @@ def other_rows(torch, ipa, x, ws, stream, n, p_core):
     o9 = torch.empty(9, dtype=torch.float64, device="cuda")
     d9 = t(lambda: ipa.ipa_nll_eval(x2, b9, LO, HI, ws=ws2, stream=stream, out=o9), 200, 10)
     out["config2_fit_1e6_events"] = {
-        "wall_s": wall, "nll_evaluations": res.n_evals, "batched_calls": res.n_calls, "edm": res.edm,
+        "wall_s": wall, "wall_s_general_wrapper": wall_plain, "nll_evaluations": res.n_evals, "batched_calls": res.n_calls, "edm": res.edm,
         "nll_evaluations_per_s_wall": res.n_evals / wall, "k9_call_ms_device": d9 * 1e3,
         "nll_evaluations_per_s_device_k9": 9 / d9,
         "fitted": {k: res.par[k] for k in inp.FLOATED}, "errors": {k: res.errors[k] for k in inp.FLOATED},

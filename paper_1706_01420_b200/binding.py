@@ -14,7 +14,7 @@ from . import build as _build
 __all__ = [
     "PARAM_FIELDS", "NPAR", "IPA_MAX_K", "IpaError", "lib", "library_path", "pack_params", "workspace",
     "ipa_version", "ipa_workspace_bytes", "ipa_norm", "ipa_core_degree", "ipa_core_cells", "ipa_nll_grad_eval", "ipa_nll_fd_gradient",
-    "ipa_nll_eval_extended", "ipa_nll_eval_categories", "ipa_nll_eval", "ipa_nll_eval_static", "IPA_STATIC_MAX_K",
+    "ipa_nll_eval_extended", "ipa_nll_eval_categories", "ipa_nll_eval", "ipa_nll_eval_static", "IPA_STATIC_MAX_K", "NllEvaluator",
     "ipa_nll_eval_segmented", "ipa_toy_generate", "ipa_hist_fill", "ipa_binned_nll_scan", "ipa_expected_hist",
     "ipa_poisson_hist_toys", "ipa_signal_shape", "ipa_gauss_smear", "ipa_expected_hist_shape", "ipa_binned_nll_scan_shape",
     "ipa_cls_teststat", "ipa_cls_count_ge", "ipa_cls_from_counts", "ipa_events_prepare",
@@ -272,6 +272,84 @@ def ipa_nll_eval_static(x, params, lo, hi, want_logpdf=False, stream=None, out=N
     _check(lib().ipa_nll_eval_static(_dptr(x, torch.float64) if n else None, n, _hptr(P), K, _Range(lo, hi), _dptr(nll),
                                      _dptr(lp), _dptr(st), _opt(policy), _stream(stream)))
     return nll, lp, st
+
+
+_cudart = None
+
+
+def _runtime():
+    """The CUDA runtime libipanll.so itself is linked against (already loaded: looked up by its soname)."""
+    global _cudart
+    if _cudart is None:
+        lib()
+        R = C.CDLL("libcudart.so.12")
+        R.cudaMemcpyAsync.restype = C.c_int
+        R.cudaMemcpyAsync.argtypes = [C.c_void_p, C.c_void_p, C.c_size_t, C.c_int, C.c_void_p]
+        R.cudaStreamSynchronize.restype = C.c_int
+        R.cudaStreamSynchronize.argtypes = [C.c_void_p]
+        _cudart = R
+    return _cudart
+
+
+class NllEvaluator:
+    """The inner loop of a fit: many ipa_nll_eval / ipa_nll_grad_eval calls on ONE event array, each followed by a read of
+    the K results on the host.  Workspace, device outputs and a pinned host buffer are allocated once; a call packs the
+    parameter sets, enqueues the library call and one device-to-host copy of the results on the stream, and waits for
+    that stream.  Argument marshalling only: the arithmetic is the library's.
+
+        ev = NllEvaluator(x, lo, hi)            # x: device tensor (fp64), stays alive and unchanged
+        nll = ev(thetas)                        # numpy [K]; +inf for a set with a domain error
+        nll, grad = ev.gradient(thetas)         # numpy [K], [K, 5]  (mu, sigma, f, k, beta)
+    """
+
+    def __init__(self, x, lo, hi, policy=None, stream=None):
+        _need_cuda()
+        assert x.is_cuda and x.dtype == torch.float64 and x.is_contiguous()
+        self.x, self.n = x, x.numel()
+        self.range = _Range(lo, hi)
+        self.opt = _opt(policy)
+        self.stream = stream if stream is not None else torch.cuda.current_stream()
+        self._st = C.c_void_p(self.stream.cuda_stream)
+        with torch.cuda.stream(self.stream):
+            self.ws = workspace(self.n, IPA_MAX_K)
+            self.dev = torch.empty(IPA_MAX_K * 7, dtype=torch.float64, device="cuda")   # nll [K] | grad [K, 5] | status
+        self.host = torch.empty(IPA_MAX_K * 7, dtype=torch.float64).pin_memory()
+        self._hnp = self.host.numpy()
+        self._hst = self._hnp[IPA_MAX_K * 6:].view(np.int32)
+        base = self.dev.data_ptr()
+        self._xp = C.c_void_p(x.data_ptr()) if self.n else None
+        self._nll = C.c_void_p(base)
+        self._grad = C.c_void_p(base + 8 * IPA_MAX_K)
+        self._status = C.c_void_p(base + 48 * IPA_MAX_K)
+        self._wsp, self._wsn = C.c_void_p(self.ws.data_ptr()), self.ws.numel()
+        self._devp, self._hostp = C.c_void_p(base), C.c_void_p(self.host.data_ptr())
+        self._lib, self._rt = lib(), _runtime()
+
+    def _read(self):
+        rc = self._rt.cudaMemcpyAsync(self._hostp, self._devp, IPA_MAX_K * 56, 2, self._st)       # 2 = device to host
+        rc = rc or self._rt.cudaStreamSynchronize(self._st)
+        if rc:
+            raise IpaError(f"CUDA runtime error {rc} while reading the results")
+
+    def __call__(self, params):
+        P = pack_params(params)
+        K = P.shape[0]
+        _check(self._lib.ipa_nll_eval(self._xp, self.n, _hptr(P), K, self.range, self._nll, None, self._status, self.opt,
+                                      self._wsp, self._wsn, self._st))
+        self._read()
+        return self._hnp[:K].copy()
+
+    def gradient(self, params):
+        P = pack_params(params)
+        K = P.shape[0]
+        _check(self._lib.ipa_nll_grad_eval(self._xp, self.n, _hptr(P), K, self.range, self._nll, self._grad, self._status,
+                                           self.opt, self._wsp, self._wsn, self._st))
+        self._read()
+        return self._hnp[:K].copy(), self._hnp[IPA_MAX_K:IPA_MAX_K + 5 * K].reshape(K, 5).copy()
+
+    def status(self, K):
+        """status codes of the K sets of the last call"""
+        return self._hst[:K].copy()
 
 
 @_alloc_on_stream

@@ -762,6 +762,29 @@ def test_maximum_batch_of_32_sets(ipa, torch_, orc, x1):
         ipa.ipa_nll_eval(xd, distinct + [inp.GEN], LO, HI)          # 33 sets: invalid argument
 
 
+def test_nll_evaluator_matches_the_plain_calls(ipa, torch_, orc, x1):
+    """NllEvaluator (the fit loop's evaluator: buffers allocated once, results read back through pinned memory) against
+    ipa_nll_eval / ipa_nll_grad_eval on the same inputs: same library calls, same bits; calls in a row, a side stream."""
+    xd = dev(torch_, x1)
+    side = torch_.cuda.Stream()
+    side.wait_stream(torch_.cuda.current_stream())
+    b9, _ = inp.fd_batch(inp.GEN)
+    bad = np.array(b9[:3]); bad[1, 1] = -1.0                 # a domain error: +inf, status 1
+    for ev in (ipa.NllEvaluator(xd, LO, HI, policy=1), ipa.NllEvaluator(xd, LO, HI, policy=1, stream=side)):
+        for th in (b9, inp.GEN, bad, b9):
+            K = ipa.pack_params(th).shape[0]
+            got = ev(th)
+            ref, _, st = ipa.ipa_nll_eval(xd, th, LO, HI, policy=1)
+            torch_.cuda.synchronize()
+            assert got.shape == (K,) and np.array_equal(got, ref.cpu().numpy())
+            assert np.array_equal(ev.status(K), st.cpu().numpy())
+        n5, g5 = ev.gradient(b9[:5])
+        rn, rg, _ = ipa.ipa_nll_grad_eval(xd, b9[:5], LO, HI, policy=1)
+        torch_.cuda.synchronize()
+        assert np.array_equal(n5, rn.cpu().numpy()) and np.array_equal(g5, rg.cpu().numpy())
+    assert abs(got[0] - orc.nll(x1, inp.GEN, LO, HI)) <= 1e-10 * abs(got[0])
+
+
 def test_core_cells(ipa, torch_, orc):
     """Cells of the core (A1e): a warp of a sorted or prepared array runs the low-degree polynomial of its cell, a warp of
     the same events in random order the full polynomial; both against the oracle, per event."""
