@@ -36,14 +36,14 @@ FP64_PEAK_NOMINAL = SM_COUNT * FP64_LANES * 2 * SM_MAX_HZ  # 37.2 TFLOP/s
 def algorithmic_flops(degree, p_core):
     """FP64 flops one event x set needs in this method (table 'work per event'),
     FMA = 2, add / mul / compare = 1; an event pays the core OR the tail arithmetic, never both:
-      common  d (1), 2 compares (2), E_B (1 FMA), exp = 6 FMA + 1 add + 1 mul (14), 1+w (1), log on [1,2] = 6 FMA (12),
-              2 adds                                                                          : 13 FMA + 8 other = 34
+      common  d (1), 2 compares (2), E_B (1 FMA), exp = 5 FMA + 1 add + 1 mul (12), 1+w (1), log on [1,2] = 6 FMA (12),
+              2 adds                                                                          : 12 FMA + 8 other = 32
       core    q, sqrt (3 FMA + 2 mul), t, Horner (degree FMA), (beta-k) d                     : (6 + degree) FMA + 2 mul
       tail    u (1 FMA), log = 7 FMA + 1 add, -n log u + c (1 FMA), -k d (1 FMA)              : 10 FMA + 1 add = 21
     (table-driven exp / log of round 2: csrc/ipa_fastmath.cuh; the degree-11 / degree-8 polynomials of round 1 made
     this 55 / 27).  p_core = fraction of the events inside [mu - a sigma, mu + a2 sigma] (0.344 for the config model)."""
     core = 2.0 * (6 + degree) + 2.0
-    return 34.0 + p_core * core + (1.0 - p_core) * 21.0
+    return 32.0 + p_core * core + (1.0 - p_core) * 21.0
 
 
 def core_cells(torch, ipa, x, P, policy):
@@ -73,8 +73,8 @@ def shape_stage_flops(degree, p_core):
     return 3.0 + p_core * (2.0 * (5 + degree) + 2.0) + (1.0 - p_core) * (2.0 * 8 + 2.0)
 
 
-MEMBER_STAGE_FLOPS = 34.0
-"""Member stage per set: Delta = s d + (V + c): 1 add + 1 FMA (3); E_B (1 FMA: 2); exp (14); 1 + w (1);
+MEMBER_STAGE_FLOPS = 32.0
+"""Member stage per set: Delta = s d + (V + c): 1 add + 1 FMA (3); E_B (1 FMA: 2); exp (12); 1 + w (1);
 log on [1,2] (12); 2 adds (2)."""
 
 

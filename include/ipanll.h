@@ -34,8 +34,8 @@
  *     3 internal numerical failure (normalisation not finite or not positive); 4 (ipa_nll_grad_eval only)
  *     f == 0 or f == 1.
  *   - Events outside [lo,hi] are evaluated by the same formulae (no clipping); NaN events give NaN.  The per-event
- *     arithmetic is valid while |log(f S) - log((1-f) B)| < 5e6 (the range of the kernels' exponential); parameter
- *     sets or events beyond that (e.g. |k (x - lo)| > 5e6) give undefined values, not an error.
+ *     arithmetic is valid while |log(f S) - log((1-f) B)| < 1e6 (the range of the kernels' exponential); parameter
+ *     sets or events beyond that (e.g. |k (x - lo)| > 1e6) give undefined values, not an error.
  *   - ipa_norm returns the ABSOLUTE N_S, which underflows to 0 (status 0) when log N_S < -745 (e.g. zeta >~ 1000 with
  *     the unscaled Bessel core); the likelihood calls work with log N_S and are not affected.
  *     Any n >= 0 is accepted (n == 0 gives NLL = +0.0).
@@ -149,7 +149,7 @@ int ipa_core_cells(const ipa_params* p_host, int K, ipa_range r, int32_t* cells_
  *   logpdf_dev [K*n]  out, optional (NULL to skip): per-event log(f S + (1-f) B), set-major; the row of a set with
  *                     status != 0 is filled with NaN
  *   status_dev [K]    out, optional
- * K <= IPA_MAX_K per call; up to 28 sets share one pass over the events, a larger batch takes two (shared memory). */
+ * K <= IPA_MAX_K per call; up to 26 sets share one pass over the events, a larger batch takes two (shared memory). */
 #define IPA_MAX_K 32
 int ipa_nll_eval(const double* x_dev, int64_t n, const ipa_params* p_host, int K, ipa_range r,
                  double* nll_dev, double* logpdf_dev, int32_t* status_dev, const ipa_options* opt_host, void* ws_dev, size_t ws_bytes,

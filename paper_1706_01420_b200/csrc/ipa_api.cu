@@ -62,9 +62,9 @@ Layout make_layout(int64_t K, int64_t nbins) {
 }
 
 // Sets per launch of the streaming kernel: each set takes its record and IPA_NB accumulators in shared memory beside the
-// two staged tiles and the 9 KB of static tables.  A larger batch (up to IPA_MAX_K) runs as two launches over the events.
-constexpr int kStreamKMax = 28;
-static_assert(kStreamKMax * (sizeof(IpaSetConsts) + IPA_NB * 8) + 2 * IPA_NTILE * 8 + 9300 <= 227 * 1024,
+// two staged tiles and the 17 KB of static tables.  A larger batch (up to IPA_MAX_K) runs as two launches over the events.
+constexpr int kStreamKMax = 26;
+static_assert(kStreamKMax * (sizeof(IpaSetConsts) + IPA_NB * 8) + 2 * IPA_NTILE * 8 + IPA_MATHTAB_DOUBLES * 8 + 1200 <= 227 * 1024,
               "streaming kernel: shared memory of a full batch");
 struct DevInfo { int dev = -1; int sms = 0; bool attr_set = false; };
 thread_local DevInfo g_dev;

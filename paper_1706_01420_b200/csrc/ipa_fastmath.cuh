@@ -22,12 +22,14 @@
 __constant__ double ipa_c_exp[IPA_EXP_DEG + 1] = IPA_EXP_COEFS;
 __constant__ double ipa_c_log1p[IPA_LOG_DEG] = IPA_LOG1P_COEFS;
 __constant__ double2 ipa_c_logtab[33] = IPA_LOG_TABLE;
-// 8 KB table of the streaming kernels (layout: gen_fastmath_tables.py); the kernels copy it to shared memory
-#define IPA_MATHTAB_DOUBLES 1024
+// 16 KB table of the streaming kernels (layout: gen_fastmath_tables.py); the kernels copy it to shared memory
+#define IPA_MATHTAB_DOUBLES 2048
 __device__ const double ipa_d_mathtab[IPA_MATHTAB_DOUBLES] = IPA_MATHTAB_RAW;
 static const double ipa_h_mathtab[IPA_MATHTAB_DOUBLES] = IPA_MATHTAB_RAW;
 __constant__ double ipa_c_expq[4] = IPA_EXPQ_COEFS;
 static const double ipa_h_expq[4] = IPA_EXPQ_COEFS;
+__constant__ double ipa_c_expq2[3] = IPA_EXPQ2_COEFS;
+static const double ipa_h_expq2[3] = IPA_EXPQ2_COEFS;
 __device__ __align__(16) const long long ipa_d_chebT[IPA_CHEB_NC * IPA_CHEB_NC] = IPA_CHEB_TABLE;   // global memory (cp.async source)
 static const long long ipa_h_chebT[IPA_CHEB_NC * IPA_CHEB_NC] = IPA_CHEB_TABLE;
 __constant__ double ipa_c_gl16x[16] = IPA_GL16_X;
@@ -42,6 +44,7 @@ static const ipa_host_double2 ipa_h_logtab[33] = IPA_LOG_TABLE;
 #ifdef __CUDA_ARCH__
 #define IPA_CEXP(j) ipa_c_exp[j]
 #define IPA_CEXPQ(j) ipa_c_expq[j]
+#define IPA_CEXPQ2(j) ipa_c_expq2[j]
 #define IPA_CLOG(j) ipa_c_log1p[j]
 #define IPA_GL16X(i) ipa_c_gl16x[i]
 #define IPA_GL16W(i) ipa_c_gl16w[i]
@@ -52,6 +55,7 @@ static const ipa_host_double2 ipa_h_logtab[33] = IPA_LOG_TABLE;
 #define IPA_GL16W(i) ipa_h_gl16w[i]
 #define IPA_CEXP(j) ipa_h_exp[j]
 #define IPA_CEXPQ(j) ipa_h_expq[j]
+#define IPA_CEXPQ2(j) ipa_h_expq2[j]
 #define IPA_CLOG(j) ipa_h_log1p[j]
 #endif
 
@@ -316,11 +320,36 @@ IPA_HD double ipa_fexp_negabs_t(double D, const double* mt) {
 #endif
 }
 
+// The softplus' own e^{-|D|}: 2^(j/1024) from the second half of the table (byte 8192), so that |r| <= ln2/2048 and
+// e^r = 1 + r q(r) needs a q of degree 2 only (1.4e-16 relative); one-step reduction as in the COARSE variant above.
+// The result enters the softplus as log(1 + w): its relative error counts times w / (1 + w) <= 1/2.  7 FP64.
+// |D| < 1.4e6 (m = round(-|D| 1024 / ln 2) must fit 32 bits).
+IPA_HD double ipa_fexp_negabs_sp(double D, const double* mt) {
+  const double SHIFT = 6755399441055744.0;
+  const double a = -fabs(D);
+  const double t = fma(a, IPA_LOG2E_1024, SHIFT);
+  int m = ipa_lo(t);                                    // round(a 1024 / ln 2) = 1024 n + j
+  const double nf = t - SHIFT;
+  const double r = fma(nf, -IPA_LN2_1024, a);
+  const double T = ipa_mt_d(mt, 8192u + (((unsigned)m & 1023u) << 3));
+  double q = fma(IPA_CEXPQ2(2), r, IPA_CEXPQ2(1));
+  q = fma(q, r, IPA_CEXPQ2(0));
+  const double w = fma(T * r, q, T);
+  m = m > -1024000 ? m : -1024000;                      // 2^n stays a normal number
+#ifdef __CUDA_ARCH__
+  int hw;                                               // hi(w) + (m >> 10) 2^20 = hi(w) + (m & ~1023) 1024
+  asm("mad.lo.s32 %0, %1, 1024, %2;" : "=r"(hw) : "r"(m & ~1023), "r"(ipa_hi(w)));
+  return ipa_mk(hw, ipa_lo(w));
+#else
+  return ipa_mk(ipa_hi(w) + ((m >> 10) << 20), ipa_lo(w));
+#endif
+}
+
 // eb + log(1 + e^D) = eb + log(1 + e^{-|D|}) + max(D, 0), and max(D, 0) = (D + |D|) / 2 with D + |D| EXACT (0 or 2 D): the
 // final FMA rounds once, like the addition of D it replaces -- same bits, no compare and no select (ptxas turned a
 // predicated add into an unconditional one plus two FSEL: 4 issue slots against 2 FP64 instructions here).
 // (Folding D/2 + |D|/2 into the two FMAs of the sum instead cancels for D << 0: 3.5e-15 at D = -52 -- rejected.)
 IPA_HD double ipa_fsoftplus_add_t(double eb, double D, const double* mt) {
-  const double w = ipa_fexp_negabs_t<true>(D, mt);
+  const double w = ipa_fexp_negabs_sp(D, mt);
   return fma(0.5, D + fabs(D), eb + ipa_flog12_t(1.0 + w, mt));
 }

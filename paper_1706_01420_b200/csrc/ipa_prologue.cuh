@@ -732,7 +732,7 @@ IPA_HD IpaProNorm ipa_pro_norm(const IpaProWork& w) {
   r.logNS = log(r.NSr) + w.logref;
   r.pure = !(p.f < 1.0);
   // f = 0: a finite, very negative signal term (softplus(-1e4) == 0 exactly) instead of -inf; it stays far inside the
-  // range |Delta| < 5e6 of the kernels' exponential (ipa_fexp_negabs_t)
+  // range |Delta| < 1.4e6 of the softplus exponential (ipa_fexp_negabs_sp)
   r.cS = (p.f > 0.0) ? w.logf - r.logNS : -1.0e4;
   r.kd = r.pure ? 0.0 : p.k;
   r.eB0 = r.pure ? 0.0 : (p.k * (p.mu - w.lo) + w.log1mf - w.logNB);
