@@ -288,23 +288,14 @@ IPA_HD double ipa_flog_t(double u, const double* mt) {
 
 // e^{-|D|}, any D with |D| < 5e6 (beyond that the integer part of -|D| 256/ln2 leaves 32 bits; the largest |Delta|
 // the kernels produce on purpose is the f == 0 sentinel, 1e4).  9 FP64.
-// COARSE: the reduction r = a - m ln2/256 in ONE step with ln2/256 rounded to fp64 (the product is exact inside the FMA, so
-// the only error is m times the representation error of the constant, < |a| 8e-17 relative in the result).  For the
-// softplus, where the result w enters as log(1 + w), that is an absolute error below |a| e^{-|a|} 8e-17 < 3e-17: 8 FP64.
-template <bool COARSE = false>
 IPA_HD double ipa_fexp_negabs_t(double D, const double* mt) {
   const double SHIFT = 6755399441055744.0;
   const double a = -fabs(D);
   const double t = fma(a, IPA_LOG2E_256, SHIFT);
   int m = ipa_lo(t);                                    // round(a 256 / ln 2) = 256 n + j
   const double nf = t - SHIFT;
-  double r;
-  if (COARSE) {
-    r = fma(nf, -(IPA_LN2_256_HI + IPA_LN2_256_LO), a);
-  } else {
-    r = fma(nf, -IPA_LN2_256_HI, a);
-    r = fma(nf, -IPA_LN2_256_LO, r);
-  }
+  double r = fma(nf, -IPA_LN2_256_HI, a);
+  r = fma(nf, -IPA_LN2_256_LO, r);
   const double T = ipa_mt_d(mt, 16u + (((unsigned)m & 255u) << 3));
   double q = fma(IPA_CEXPQ(3), r, IPA_CEXPQ(2));
   q = fma(q, r, IPA_CEXPQ(1));
@@ -321,7 +312,9 @@ IPA_HD double ipa_fexp_negabs_t(double D, const double* mt) {
 }
 
 // The softplus' own e^{-|D|}: 2^(j/1024) from the second half of the table (byte 8192), so that |r| <= ln2/2048 and
-// e^r = 1 + r q(r) needs a q of degree 2 only (1.4e-16 relative); one-step reduction as in the COARSE variant above.
+// e^r = 1 + r q(r) needs a q of degree 2 only (1.4e-16 relative).  The reduction r = a - m ln2/1024 takes ONE step with
+// ln2/1024 rounded to fp64: the product is exact inside the FMA, so the only error is m times the representation error of
+// the constant, < |a| 8e-17 relative in the result, i.e. < |a| e^{-|a|} 8e-17 < 3e-17 absolute in the softplus.
 // The result enters the softplus as log(1 + w): its relative error counts times w / (1 + w) <= 1/2.  7 FP64.
 // |D| < 1.4e6 (m = round(-|D| 1024 / ln 2) must fit 32 bits).
 IPA_HD double ipa_fexp_negabs_sp(double D, const double* mt) {

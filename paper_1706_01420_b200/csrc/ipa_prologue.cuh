@@ -26,9 +26,7 @@
 #define IPA_PRO_THREADS 256
 #define IPA_SUB 2               // threads sharing one table-based Bessel evaluation
 #define IPA_NBTASK (IPA_MCHEB + 4)  // Chebyshev nodes + K_nu(z0), K_nu(z1), K_{nu-1}(z0), K_{nu-1}(z1)
-#define IPA_HD_NOINLINE IPA_HD   // the cell phases (inline: out of line they cost more, measured)
-#define IPA_NCELL 4              // (the geometry takes a fourth root: static_assert below)
-// cells of the core in r = sqrt(d^2 + delta^2), each with its own low-degree polynomial
+#define IPA_NCELL 4              // cells of the core in r = sqrt(d^2 + delta^2), each with its own low-degree polynomial
 #define IPA_CELLN 16             // coefficients per cell polynomial (degree <= 15)
 #define IPA_CELLM 32             // Chebyshev nodes per cell
 #define IPA_CELL_MIN_DEGREE 16   // cells only where the full polynomial is longer than a cell polynomial can be
@@ -308,7 +306,7 @@ IPA_HD double ipa_pro_task_z(const IpaProWork& w, int q) {
   return ((q - IPA_MCHEB) & 1) ? w.z1 : w.z0;
 }
 
-IPA_HD_NOINLINE void ipa_pro_cells_geometry(IpaProWork& w);
+IPA_HD void ipa_pro_cells_geometry(IpaProWork& w);
 // phase 4: Bessel tasks, IPA_SUB threads each
 IPA_HD void ipa_pro_phase4(IpaProWork& w, int tid) {
   if (tid == 192) { ipa_pro_cells_geometry(w); return; }   // needs phase 2 only; this thread has no Bessel task
@@ -420,7 +418,7 @@ static_assert(IPA_NCELL == 4, "ipa_pro_cells_geometry: ratio of the cell radii i
 // of ipa_events_prepare: inside a bin the events are not ordered, so a boundary inside a bin would leave every warp of
 // that bin in two cells) and truncated to a zero low word (the kernels compare high words), which moves them by less
 // than one unit `quant` of the high word: every cell is fitted on its own |d| interval widened by 2 quant on both sides.
-IPA_HD_NOINLINE void ipa_pro_cells_geometry(IpaProWork& w) {
+IPA_HD void ipa_pro_cells_geometry(IpaProWork& w) {
   w.ncell = 0;
   for (int i = 0; i < 8; ++i) w.chb[i] = 0x7fffffff;
   if (w.status || w.mode) return;
@@ -481,7 +479,7 @@ IPA_HD_NOINLINE void ipa_pro_cells_geometry(IpaProWork& w) {
   w.ncell = IPA_NCELL;
 }
 // phase 8, threads 128..255: the full Chebyshev series (Clenshaw, degree from phase 7b) at the Chebyshev nodes of the cells
-IPA_HD_NOINLINE void ipa_pro_cells_nodes(IpaProWork& w, int tid) {
+IPA_HD void ipa_pro_cells_nodes(IpaProWork& w, int tid) {
   if (w.status || w.mode || !w.ncell || w.degree < IPA_CELL_MIN_DEGREE || tid < 128) return;
   const int s = (tid - 128) >> 5, i = (tid - 128) & 31;
   const double r = fma(w.crh[s], w.ctab[4 * i + 2], w.crc[s]);
@@ -495,7 +493,7 @@ IPA_HD_NOINLINE void ipa_pro_cells_nodes(IpaProWork& w, int tid) {
   w.cH[s][i] = fma(t, b1, w.c[0] - b2);
 }
 // phase 9, threads 128..255: Chebyshev coefficients of the cells (ctab[m] = cos(pi m / 128))
-IPA_HD_NOINLINE void ipa_pro_cells_dct(IpaProWork& w, int tid) {
+IPA_HD void ipa_pro_cells_dct(IpaProWork& w, int tid) {
   if (w.status || w.mode || !w.ncell || w.degree < IPA_CELL_MIN_DEGREE || tid < 128) return;
   const int s = (tid - 128) >> 5, j = (tid - 128) & 31;
   // four partial sums (the loads of one step do not wait for the additions of the one before); index 2 j (2 i + 1) stepped by 4 j
@@ -520,7 +518,7 @@ IPA_HD int ipa_pro_cells_slot(int tid) {
   return -1;
 }
 // degree of the cell (the rules of phase 7b on the cell's own interval) and its monomial coefficients (as phase 8)
-IPA_HD_NOINLINE void ipa_pro_cells_monomial(IpaProWork& w, int slot) {
+IPA_HD void ipa_pro_cells_monomial(IpaProWork& w, int slot) {
   if (slot < 0 || w.status || w.mode || !w.ncell || w.degree < IPA_CELL_MIN_DEGREE) return;
   const int s = slot >> 4, k = slot & 15;
   const double thr = 2.5e-16 * fmax(fmax(1.0, w.hmax4[0]), fmax(fmax(w.hmax4[1], w.hmax4[2]), w.hmax4[3]));
@@ -552,7 +550,7 @@ IPA_HD_NOINLINE void ipa_pro_cells_monomial(IpaProWork& w, int slot) {
   w.csa[s][k] = ahi + alo;
 }
 // phase 12: the cells' part of the record (threads 128..191 the coefficients, thread 96 the rest)
-IPA_HD_NOINLINE void ipa_pro_cells_record(IpaProWork& w, IpaSetConsts& o, int tid) {
+IPA_HD void ipa_pro_cells_record(IpaProWork& w, IpaSetConsts& o, int tid) {
   if (tid != 96 && (tid < 128 || tid >= 128 + IPA_NCELL * IPA_CELLN)) return;
   bool on = !w.status && !w.mode && w.ncell && w.degree >= IPA_CELL_MIN_DEGREE;
   if (on)
