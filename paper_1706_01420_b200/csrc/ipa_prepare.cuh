@@ -16,7 +16,7 @@
 //   ipa_prep_hist_kernel     block b counts the bins of its contiguous chunk            -> hist[bin][b]
 //   ipa_prep_scan_kernel     per bin: exclusive prefix over the blocks, total per bin   -> hist (in place), bintot
 //   ipa_prep_binscan_kernel  exclusive prefix over the bins                             -> binbase
-//   ipa_prep_scatter_kernel  block b re-reads its chunk tile by tile (2048 events): ranks every event inside its bin
+//   ipa_prep_scatter_kernel  block b re-reads its chunk tile by tile (4096 events): ranks every event inside its bin
 //                            in original order (warp: ballots on the bits of the bin; block: per-warp counters + a scan over the warps),
 //                            moves the tile into bin order in SHARED memory and writes it out in runs of consecutive
 //                            addresses (one run per bin), starting at  binbase[bin] + hist[bin][b]
@@ -26,11 +26,11 @@
 #include <stdint.h>
 
 #define IPA_PREP_BINS 256                               // == IPA_PREPARE_BINS of the header (asserted in ipa_api.cu)
-#define IPA_PREP_THREADS 256
-#define IPA_PREP_BLOCKS_PER_SM 6                       // 40 registers, 25 KB of shared memory per block
+#define IPA_PREP_THREADS 512                           // measured per 1e8 events: 256 x 6 blocks per SM 0.88 ms, 256 x 4 0.83, 512 x 2 0.79, 512 x 3 0.78, 1024 x 1 0.81
+#define IPA_PREP_BLOCKS_PER_SM 3                       // 40 registers, 62 KB of shared memory per block
 #define IPA_PREP_WARPS (IPA_PREP_THREADS / 32)
 #define IPA_PREP_E 8                                    // events per thread and tile
-#define IPA_PREP_TILE (IPA_PREP_THREADS * IPA_PREP_E)   // 2048 events: ranks and positions inside a tile fit 16 bits
+#define IPA_PREP_TILE (IPA_PREP_THREADS * IPA_PREP_E)   // 4096 events: ranks and positions inside a tile fit 16 bits
 // dynamic shared memory of the scatter: stage [TILE] double | off [BINS] u64 | delta [BINS] u64 | tilebase [BINS] u32 |
 // wtot [8] u32 | wmap [WARPS][BINS] u32 | wcnt [WARPS][BINS] u16 | sbin [TILE] u8
 #define IPA_PREP_SMEM (IPA_PREP_TILE * 8 + IPA_PREP_BINS * 16 + (IPA_PREP_BINS + 8) * 4 + IPA_PREP_WARPS * IPA_PREP_BINS * 6 + \
@@ -157,16 +157,20 @@ __device__ __forceinline__ void ipa_prep_scatter_range(const double* __restrict_
   unsigned short* mine = m.wcnt + warp * IPA_PREP_BINS;
   unsigned int* map = m.wmap + warp * IPA_PREP_BINS;
   for (int i = tid; i < IPA_PREP_WARPS * IPA_PREP_BINS; i += IPA_PREP_THREADS) m.wmap[i] = 0u;   // kept zero by the leaders
+  const int first = warp * (32 * IPA_PREP_E) + lane;
+  // the events of a tile are loaded one tile ahead (right after the previous tile has been staged, when v[] is free): the
+  // loads fly during the write-out of the previous tile and the zeroing below
+  double v[IPA_PREP_E], vn[IPA_PREP_E];
+#pragma unroll
+  for (int e = 0; e < IPA_PREP_E; ++e) vn[e] = (beg + first + 32 * e < end) ? __ldcs(x + beg + first + 32 * e) : 0.0;
   for (long long base = beg; base < end; base += IPA_PREP_TILE) {
     const int cnt = (int)((end - base < IPA_PREP_TILE) ? (end - base) : IPA_PREP_TILE);
     {  // zero the per-warp counters (128-bit stores)
       uint4* z = reinterpret_cast<uint4*>(m.wcnt);
       for (int i = tid; i < IPA_PREP_WARPS * IPA_PREP_BINS * 2 / 16; i += IPA_PREP_THREADS) z[i] = make_uint4(0u, 0u, 0u, 0u);
     }
-    double v[IPA_PREP_E];
-    const int first = warp * (32 * IPA_PREP_E) + lane;
 #pragma unroll
-    for (int e = 0; e < IPA_PREP_E; ++e) v[e] = (first + 32 * e < cnt) ? __ldcs(x + base + first + 32 * e) : 0.0;
+    for (int e = 0; e < IPA_PREP_E; ++e) v[e] = vn[e];
     __syncthreads();
     unsigned int key[IPA_PREP_E];               // bin << 16 | rank inside the warp
     const bool full = cnt == IPA_PREP_TILE;
@@ -230,6 +234,11 @@ __device__ __forceinline__ void ipa_prep_scatter_range(const double* __restrict_
         m.stage[pos] = v[e];
         m.sbin[pos] = (unsigned char)b;
       }
+    }
+    {
+      const long long nb = base + IPA_PREP_TILE;
+#pragma unroll
+      for (int e = 0; e < IPA_PREP_E; ++e) vn[e] = (nb + first + 32 * e < end) ? __ldcs(x + nb + first + 32 * e) : 0.0;
     }
     __syncthreads();
     for (int i = tid; i < cnt; i += IPA_PREP_THREADS) {
