@@ -1059,13 +1059,29 @@ ipa_scan_kernel(const long long* __restrict__ ntot, long long T, long long* __re
   }
 }
 
-__device__ __forceinline__ double ipa_draw_background(double k, unsigned long long seed, unsigned long long slot,
-                                                      double lo, double hi) {
+// inverse CDF of the exponential background on [lo, hi]: x = lo + log1p(u expm1(k (hi-lo))) / k.  The two per-set
+// constants (em1 = expm1(k (hi-lo)), invk = 1/k; invk == 0 marks the flat case |k| (hi-lo) < 1e-8) are formed once per
+// thread, not per event: expm1 and the division were a sixth of the generator's instructions.
+// With |k| (hi-lo) > 1e-3 the logarithm is the kernels' own table-driven one on 1 + u em1 (the rounding of that sum moves
+// x by less than 1e-16 / |k| < 1e-10; table through L1); flatter slopes keep libdevice's log1p.
+struct IpaBkgDraw { double em1, invk, w; bool fastlog; };
+__device__ __forceinline__ IpaBkgDraw ipa_bkg_draw_consts(double k, double lo, double hi) {
+  IpaBkgDraw b;
+  b.w = hi - lo;
+  const double t = k * b.w;
+  const bool flat = fabs(t) < 1e-8;
+  b.em1 = flat ? 0.0 : expm1(t);
+  b.invk = flat ? 0.0 : 1.0 / k;
+  b.fastlog = fabs(t) > 1e-3 && fabs(t) < 700.0;
+  return b;
+}
+__device__ __forceinline__ double ipa_draw_background(const IpaBkgDraw& b, unsigned long long seed, unsigned long long slot,
+                                                      double lo) {
   double u, v;
   ipa_uniforms2(seed, slot, 0u, IPA_STREAM_BKG, &u, &v);
-  const double w = hi - lo, t = k * w;
-  if (fabs(t) < 1e-8) return lo + u * w;
-  return lo + log1p(u * expm1(t)) / k;
+  if (b.invk == 0.0) return lo + u * b.w;
+  const double y = u * b.em1;
+  return fma(b.fastlog ? ipa_flog_t(1.0 + y, ipa_d_mathtab) : log1p(y), b.invk, lo);
 }
 
 // Core-only log G(d) with the streaming kernels' own sqrt and the Horner groups (accept-reject attempt loop; the
@@ -1227,7 +1243,8 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
   const int nreg = E.nreg;
   const double cshift = c.araw0 - c.nu * log(c.alpha);
   const unsigned long long seed = seeds[t];
-  const double f = c.fsig, k = c.kraw;
+  const double f = c.fsig;
+  const IpaBkgDraw bkg = ipa_bkg_draw_consts(c.kraw, lo, hi);
   const long long beg = mixture ? 0 : offsets[t];
   const long long len = mixture ? capacity : offsets[t + 1] - beg;
   const long long ns = mixture ? 0 : nsig[t];
@@ -1247,6 +1264,7 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
   for (long long r0 = w0; r0 < w1; r0 += IPA_GEN_ROUND) {
     const int cnt = (int)((w1 - r0 < IPA_GEN_ROUND) ? (w1 - r0) : IPA_GEN_ROUND);
     int nlist = 0;
+#pragma unroll 2
     for (int o = lane; o < ((cnt + 31) & ~31); o += 32) {
       const long long j = r0 + o;
       bool is_sig = false;
@@ -1258,7 +1276,7 @@ ipa_toy_events_kernel(const unsigned long long* __restrict__ seeds, const IpaSet
         } else {
           is_sig = j < ns;
         }
-        if (!is_sig) x[beg + j] = ipa_draw_background(k, seed, (unsigned long long)(j + first_slot), lo, hi);
+        if (!is_sig) x[beg + j] = ipa_draw_background(bkg, seed, (unsigned long long)(j + first_slot), lo);
       }
       const unsigned m = __ballot_sync(IPA_FULL, is_sig);
       if (is_sig) list[nlist + __popc(m & lt)] = o;
