@@ -637,10 +637,15 @@ int ipa_poisson_hist_toys(const double* mean_dev, int nbins, const uint64_t* see
   cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
   char* ws = static_cast<char*>(ws_dev);
   IPA_CK(cudaMemcpyAsync(ws + L.seeds, seeds_host, (size_t)T * 8, cudaMemcpyHostToDevice, st));
-  const int64_t total = T * (int64_t)nbins;
-  int64_t G = (total + 255) / 256;
-  if (G > (int64_t)sms * 16) G = (int64_t)sms * 16;
-  ipa_poisson_hist_kernel<<<(unsigned)G, 256, 0, st>>>(mean_dev, nbins,
+  int bw = 256;                                                      // bins per block: a power of two
+  while (bw > 1 && bw / 2 >= nbins) bw /= 2;
+  const int64_t gx = ((int64_t)nbins + bw - 1) / bw;                 // bins across the threads, toys in chunks over grid y
+  int64_t gy = ((int64_t)sms * 8 + gx - 1) / gx;
+  const int64_t tgroups = (T + 256 / bw - 1) / (256 / bw);
+  if (gy > tgroups) gy = tgroups;
+  if (gy > 65535) gy = 65535;
+  if (gy < 1) gy = 1;
+  ipa_poisson_hist_kernel<<<dim3((unsigned)gx, (unsigned)gy), 256, 0, st>>>(mean_dev, nbins, bw,
                                                        reinterpret_cast<const unsigned long long*>(ws + L.seeds), T,
                                                        counts_dev);
   IPA_CK(cudaGetLastError());

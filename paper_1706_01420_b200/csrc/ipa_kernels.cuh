@@ -1626,16 +1626,22 @@ __global__ void ipa_cls_from_counts_kernel(const long long* count_sb, long long 
 // ------------------------------------------------------------------------------------------------
 // Per-bin Poisson toys (B3)
 // ------------------------------------------------------------------------------------------------
+// Thread = one bin over a chunk of the toys (blockIdx.y): the constants of the bin's mean are formed once per thread, the
+// draws of a toy are written to consecutive addresses by consecutive threads.  A block covers bw bins (a power of two,
+// 256 unless there are fewer bins) by 256 / bw toys at a time.
 __global__ void __launch_bounds__(256)
-ipa_poisson_hist_kernel(const double* __restrict__ mean, int nbins, const unsigned long long* __restrict__ seeds,
+ipa_poisson_hist_kernel(const double* __restrict__ mean, int nbins, int bw, const unsigned long long* __restrict__ seeds,
                         long long T, unsigned int* __restrict__ counts) {
-  const long long total = T * (long long)nbins;
-  const long long stride = (long long)gridDim.x * blockDim.x;
-  for (long long i = blockIdx.x * (long long)blockDim.x + threadIdx.x; i < total; i += stride) {
-    const long long t = i / nbins;
-    const int b = (int)(i - t * nbins);
-    counts[i] = (unsigned int)ipa_poisson(seeds[t], (unsigned long long)b, IPA_STREAM_BIN, mean[b]);
-  }
+  const int b = blockIdx.x * bw + (threadIdx.x & (bw - 1));
+  if (b >= nbins) return;
+  const int tl = threadIdx.x / bw, tstep = 256 / bw;
+  const IpaPoissonConsts pc = ipa_poisson_consts(mean[b]);
+  const long long per = (T + gridDim.y - 1) / gridDim.y;
+  const long long t0 = per * blockIdx.y;
+  long long t1 = t0 + per;
+  if (t1 > T) t1 = T;
+  for (long long t = t0 + tl; t < t1; t += tstep)
+    counts[t * nbins + b] = (unsigned int)ipa_poisson_draw(pc, seeds[t], (unsigned long long)b, IPA_STREAM_BIN);
 }
 
 // ipa_core_cells: out[k] = { ncell, degree of each cell, high words of the cell boundaries in x }

@@ -153,26 +153,40 @@ enum { IPA_STREAM_COMP = 0, IPA_STREAM_SIG = 1, IPA_STREAM_BKG = 2, IPA_STREAM_Y
 
 // Poisson(mean) (reading D14): sequential-search inversion below 10, Hoermann's transformed
 // rejection with squeeze (PTRS, Insurance: Math. & Econ. 12 (1993) 39-45) above.
-IPA_HD int64_t ipa_poisson(uint64_t seed, uint64_t slot, uint32_t stream, double mean) {
-  if (!(mean > 0.0)) return 0;
-  if (mean < 10.0) {
+// The constants of a mean (IpaPoissonConsts) are separate from the draw, so that a caller with many draws of one mean
+// (a bin over many toys) forms them once; ipa_poisson is the two in a row -- same expressions, same values.
+struct IpaPoissonConsts { double mean, p0, b, a, vr, lmean, linva; int kind; };   // kind: 0 zero, 1 inversion, 2 PTRS
+IPA_HD IpaPoissonConsts ipa_poisson_consts(double mean) {
+  IpaPoissonConsts c;
+  c.mean = mean;
+  c.p0 = c.b = c.a = c.vr = c.lmean = c.linva = 0.0;
+  if (!(mean > 0.0)) { c.kind = 0; return c; }
+  if (mean < 10.0) { c.kind = 1; c.p0 = exp(-mean); return c; }
+  c.kind = 2;
+  const double smu = sqrt(mean);
+  c.b = 0.931 + 2.53 * smu;
+  c.a = -0.059 + 0.02483 * c.b;
+  const double inv_alpha = 1.1239 + 1.1328 / (c.b - 3.4);
+  c.vr = 0.9277 - 3.6224 / (c.b - 2.0);
+  c.lmean = log(mean);
+  c.linva = log(inv_alpha);
+  return c;
+}
+IPA_HD int64_t ipa_poisson_draw(const IpaPoissonConsts& c, uint64_t seed, uint64_t slot, uint32_t stream) {
+  if (c.kind == 0) return 0;
+  if (c.kind == 1) {
     double u, v;
     ipa_uniforms2(seed, slot, 0u, stream, &u, &v);
     int64_t k = 0;
-    double p = exp(-mean), F = p;
+    double p = c.p0, F = p;
     while (u > F && k < 1000) {
       ++k;
-      p *= mean / (double)k;
+      p *= c.mean / (double)k;
       F += p;
     }
     return k;
   }
-  const double smu = sqrt(mean);
-  const double b = 0.931 + 2.53 * smu;
-  const double a = -0.059 + 0.02483 * b;
-  const double inv_alpha = 1.1239 + 1.1328 / (b - 3.4);
-  const double vr = 0.9277 - 3.6224 / (b - 2.0);
-  const double lmean = log(mean);
+  const double mean = c.mean, b = c.b, a = c.a, vr = c.vr, lmean = c.lmean;
   for (uint32_t attempt = 0;; ++attempt) {
     double U, V;
     ipa_uniforms2(seed, slot, attempt, stream, &U, &V);
@@ -181,7 +195,10 @@ IPA_HD int64_t ipa_poisson(uint64_t seed, uint64_t slot, uint32_t stream, double
     const double kf = floor((2.0 * a / us + b) * U + mean + 0.43);
     if (us >= 0.07 && V <= vr) return (int64_t)kf;
     if (kf < 0.0 || (us < 0.013 && V > us)) continue;
-    if (log(V) + log(inv_alpha) - log(a / (us * us) + b) <= -mean + kf * lmean - lgamma(kf + 1.0)) return (int64_t)kf;
+    if (log(V) + c.linva - log(a / (us * us) + b) <= -mean + kf * lmean - lgamma(kf + 1.0)) return (int64_t)kf;
     if (attempt > 1000000u) return (int64_t)kf;
   }
+}
+IPA_HD int64_t ipa_poisson(uint64_t seed, uint64_t slot, uint32_t stream, double mean) {
+  return ipa_poisson_draw(ipa_poisson_consts(mean), seed, slot, stream);
 }

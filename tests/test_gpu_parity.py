@@ -354,6 +354,12 @@ def test_binned_scan_expected_hist_and_poisson_toys(ipa, torch_, orc):
     ref_t = orc.poisson_hist_toys(mean, seeds)
     got_t = toys.cpu().numpy().astype(np.uint32)
     mismatches(got_t.astype(np.float64), ref_t.astype(np.float64), "per-bin Poisson toys", tol=0.0)   # integer draws: equal
+    # few bins, many toys (a block then covers several toys at a time), one bin, one toy
+    for m2, T2 in ((np.array([0.0, 4.5, 12.0, 3e4, 7e4]), 301), (np.array([37.5]), 77), (mean[:300], 1), (mean[:257], 3)):
+        sd = np.arange(100, 100 + T2, dtype=np.uint64)
+        g2 = ipa.ipa_poisson_hist_toys(dev(torch_, m2), sd)
+        torch_.cuda.synchronize()
+        assert np.array_equal(g2.cpu().numpy().astype(np.uint32).reshape(T2, m2.size), orc.poisson_hist_toys(m2, sd).reshape(T2, m2.size))
 
 
 # ---------------------------------------------------------------------------------------------
