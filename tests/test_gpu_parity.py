@@ -805,8 +805,7 @@ def test_core_cells(ipa, torch_, orc):
     assert np.all(np.abs((xb - LO) * 256 / (HI - LO) - np.rint((xb - LO) * 256 / (HI - LO))) < 1e-3)
     assert ipa.ipa_core_cells(inp.GEN, LO, HI, policy=0)[0] == 0          # degree 1 (K_{1/2}): nothing to gain
     assert ipa.ipa_core_cells(dict(inp.GEN, sigma=0.02), LO, HI, policy=1)[0] == 0   # core narrower than the high-word resolution allows
-    xg, _, _ = ipa.ipa_toy_generate([11], inp.GEN, -1.0, -1.0, LO, HI, 300_000)
-    x = xg.cpu().numpy()
+    x = orc.generate_mixture(11, 300_000, inp.GEN, LO, HI)           # the oracle's own generator: no input from the CUDA path
     # the boundary doubles themselves and their neighbours
     x[:18] = np.concatenate([xb, np.nextafter(xb, 0.0), np.nextafter(xb, 1e9)])
     xs = np.sort(x)
